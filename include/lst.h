@@ -1,0 +1,227 @@
+/*
+ * lst.h -- C-ABI of liblst.so: the data-parallel hot path of Line Segment Tracking
+ * (arXiv 2207.08207) on one NVIDIA B200 (sm_100a).
+ *
+ *   hits -> mini-doublets (MD) -> segments (LS) -> triplets (T3) -> quintuplets (T5)
+ *
+ * The paper states the problem (PAPER.md:37 overview; :43 MD; :47-49 LS and module map;
+ * :53 T3; :55 T5; :125 one kernel per object class, run in sequence; :143 no per-event
+ * allocation; :147 several events in flight).  Every formula and constant is the frozen
+ * reading in DESIGN.md section 1 ("SPEC").
+ *
+ * Conventions
+ *  - Plain C linkage, plain pointers and sizes.  Every function returns an int status
+ *    (LST_OK = 0, errors < 0); nothing throws, aborts or prints.
+ *  - "host" / "device" is stated for every pointer.  Device pointers returned in views are
+ *    owned by the library (they live in the context's arena, allocated once in lst_create)
+ *    and stay valid until the next lst_load_event on the same slot or lst_destroy.
+ *  - `cuda_stream` arguments are a cudaStream_t passed as void* (NULL = the legacy default
+ *    stream).  lst_load_event / lst_run / lst_run_batch only ENQUEUE work (no host
+ *    synchronisation, no allocation): they may be captured into a CUDA graph.
+ *  - An event lives in a SLOT (0 .. n_slots-1).  Slots are independent: several may be in
+ *    flight on different streams and distinct slots may be driven from distinct
+ *    host threads.  One slot must not be used from two streams at once.
+ *  - Object identity is by ORIGINAL hit index = position in the caller's hit arrays
+ *    (reading 16).  Within a slot objects are numbered deterministically:
+ *    MDs by (module, lower hit, upper hit), segments by (inner MD, outer MD), triplets by
+ *    (first segment, second segment), quintuplets by (first triplet, second triplet).
+ *  - Overflow of a per-slot capacity is never silent: lst_sync returns LST_ERR_OVERFLOW, the
+ *    slot's outputs are invalid, lst_get_stats still reports the sizes that were needed.
+ */
+#ifndef LST_H_
+#define LST_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LST_N_LAYERS 6
+
+#if defined(__GNUC__)
+#define LST_API __attribute__((visibility("default")))
+#else
+#define LST_API
+#endif
+
+enum {
+  LST_OK = 0,
+  LST_ERR_ARG = -1,      /* NULL / out-of-range argument, invalid geometry, map, module id or side */
+  LST_ERR_CUDA = -2,     /* a CUDA runtime call failed (lst_last_cuda_error gives the code)        */
+  LST_ERR_OVERFLOW = -3, /* a per-slot capacity was exceeded                                       */
+  LST_ERR_STATE = -4,    /* call out of order (e.g. lst_get_* before lst_sync)                     */
+  LST_ERR_NOMEM = -5     /* arena allocation failed in lst_create                                  */
+};
+
+enum { LST_MD = 0, LST_SEG = 1, LST_T3 = 2, LST_T5 = 3 };
+
+typedef struct lst_ctx lst_ctx;
+
+/* Detector description. HOST pointers, copied by lst_create; the caller keeps ownership.
+ * Only `layer` enters the computation (cut constants are per layer); the rest is validated
+ * and kept for diagnostics.  PAPER.md:29 (pT modules), BASELINE.json configs[0]. */
+typedef struct {
+  int32_t n_modules;
+  const int8_t* layer;  /* [n_modules] 0 .. LST_N_LAYERS-1 */
+  const int8_t* kind;   /* [n_modules] 0 = PS, 1 = 2S (may be NULL) */
+  const float* cx;      /* [n_modules] module centre (may be NULL) */
+  const float* cy;
+  const float* cz;
+  const float* phi;     /* [n_modules] azimuth of the module normal (may be NULL) */
+} lst_geometry;
+
+/* Module map: CSR lookup table module -> connectable modules of the next layer.
+ * HOST pointers, copied by lst_create.  layer[targets[k]] must equal layer[src] + 1. */
+typedef struct {
+  int32_t n_modules;
+  const int32_t* row_offsets; /* [n_modules + 1], non-decreasing, row_offsets[0] = 0 */
+  const int32_t* targets;     /* [row_offsets[n_modules]] */
+} lst_module_map;
+
+/* Cut constants (all fp32) and runtime sizes. */
+typedef struct {
+  float half_kappa_max;
+  float z_lum;
+  float md_cos_eps[LST_N_LAYERS];
+  float md_sin_eps[LST_N_LAYERS];
+  float md_dz_res[LST_N_LAYERS];
+  float md_eps[LST_N_LAYERS];
+  float seg_cos_eps;
+  float seg_sin_eps;
+  float seg_z0_max[LST_N_LAYERS - 1];
+  float t3_kappa_max;
+  float t3_chi2rz_max[LST_N_LAYERS - 2];
+  float sigma_z2[LST_N_LAYERS];
+  float inv_sigma_z2[LST_N_LAYERS];
+  float t5_dkappa_max;
+  float t5_chi2rz_max[LST_N_LAYERS - 4];
+  float t5_chi2xy_max;
+  float t5_sigma_xy2_scaled;
+  float t5_kappa_max;
+  /* runtime */
+  int32_t device;     /* CUDA device ordinal */
+  int32_t n_slots;    /* event slots in the arena (>= 1) */
+  int32_t cap_hits;   /* per-slot capacities, in objects */
+  int32_t cap_md;
+  int32_t cap_seg;
+  int32_t cap_t3;
+  int32_t cap_t5;
+  int32_t timing;     /* != 0: record CUDA events around every stage (lst_get_stats.stage_ms);
+                         makes lst_run non-capturable */
+} lst_config;
+
+/* Fills *cfg with the frozen SPEC constants, device 0, 4 slots and capacities that hold the
+ * PU300-like stress event of BASELINE.json configs[3] with margin. */
+LST_API int lst_default_config(lst_config* cfg);
+
+/* Hit SoA of one event (BASELINE.json configs[1]: "fp32 SoA (x, y, z, module id, sensor side)").
+ * All five arrays are HOST pointers (on_device = 0; pinned memory makes the copy asynchronous)
+ * or all five DEVICE pointers (on_device = 1).  They are borrowed until the stream has passed
+ * the work enqueued by lst_load_event.  side: 0 = lower sensor (the anchor), 1 = upper. */
+typedef struct {
+  int32_t n;
+  const float* x;
+  const float* y;
+  const float* z;
+  const int32_t* module;
+  const uint8_t* side;
+  int32_t on_device;
+} lst_hits;
+
+/* Views: DEVICE pointers into the slot's object store + the object count. */
+typedef struct {
+  int32_t n;
+  const int32_t* hits;         /* [n][2] original index of (lower, upper) hit                 */
+  const int32_t* module;       /* [n]                                                         */
+  const float* anchor;         /* [n][4] x, y, z, r of the anchor (lower) hit, 16-B aligned   */
+  const float* ur_sina;        /* [n][2] r of the upper hit, sinA                             */
+  const float* dphi_dphichange;/* [n][2]                                                      */
+  const int32_t* module_start; /* [n_modules + 1] MDs of module m are [start[m], start[m+1])  */
+} lst_md_view;
+
+typedef struct {
+  int32_t n;
+  const int32_t* md;       /* [n][2] inner MD, outer MD                                        */
+  const float* f;          /* [n][4] sinS, z0, dphi, dphichange                                */
+  const int32_t* md_start; /* [n_md + 1] segments with inner MD i are [start[i], start[i+1])   */
+} lst_seg_view;
+
+typedef struct {
+  int32_t n;
+  const int32_t* md_kappa; /* [n][4] MD1, MD2, MD3, bit pattern of kappa (fp32)                 */
+  const int32_t* seg;      /* [n][2] first segment, second segment                              */
+  const float* chi2rz;     /* [n]                                                               */
+  const int32_t* seg_start;/* [n_seg + 1] triplets with first segment a are [start[a], start[a+1]) */
+} lst_t3_view;
+
+typedef struct {
+  int32_t n;
+  const int32_t* md;       /* [n][5] MD1 .. MD5                                                 */
+  const int32_t* t3;       /* [n][2] inner triplet, outer triplet                               */
+  const float* f;          /* [n][5] kappa_in, kappa_out, kappa_fit, chi2xy, chi2rz             */
+  const int32_t* t3_start; /* [n_t3 + 1] quintuplets with inner triplet A are [start[A], start[A+1]) */
+} lst_t5_view;
+
+typedef struct {
+  int32_t n_hits;
+  int64_t needed[4];     /* objects that passed per class (may exceed the capacity on overflow) */
+  int64_t candidates[4]; /* candidate pairs examined per stage                                   */
+  int32_t overflow;      /* bit k set: capacity of class k exceeded                              */
+  int32_t bad_hits;      /* hits dropped because module id / side was out of range               */
+  float stage_ms[5];     /* a0 .. a4; zeros unless lst_config.timing                              */
+} lst_stats;
+
+/* Validates geometry and map, uploads the per-module tables, allocates the arena (the only
+ * cudaMalloc of the library's lifetime).  cfg = NULL means lst_default_config.
+ * Errors: LST_ERR_ARG (with nothing allocated), LST_ERR_NOMEM, LST_ERR_CUDA. */
+LST_API int lst_create(const lst_geometry* geom, const lst_module_map* map, const lst_config* cfg, lst_ctx** out);
+LST_API int lst_destroy(lst_ctx* ctx);
+
+/* Step a0 ("a kernel that deals with pre-processing the hits and loading them"):
+ * copies the hits to the device if they are on the host, bins them by (module, side), orders
+ * each bin by original index and derives r.  Asynchronous on `cuda_stream`.  Hits with an
+ * invalid module id or side are dropped and reported (lst_sync -> LST_ERR_ARG).
+ * Errors: LST_ERR_ARG (bad slot, n < 0, NULL arrays), LST_ERR_OVERFLOW (n > cap_hits). */
+LST_API int lst_load_event(lst_ctx* ctx, int slot, const lst_hits* hits, void* cuda_stream);
+
+/* Steps a1..a4 for one slot / for slots first_slot .. first_slot+n_slots-1 in ONE set of
+ * launches (the batch index is a grid dimension).  Asynchronous; no host synchronisation. */
+LST_API int lst_run(lst_ctx* ctx, int slot, void* cuda_stream);
+LST_API int lst_run_batch(lst_ctx* ctx, int first_slot, int n_slots, void* cuda_stream);
+/* One stage only (LST_MD .. LST_T5) of a slot range; lst_run_batch == the four in order. */
+LST_API int lst_run_stage(lst_ctx* ctx, int first_slot, int n_slots, int stage, void* cuda_stream);
+
+/* Waits for `cuda_stream`, reads the slot's counters back and returns its status:
+ * LST_OK, LST_ERR_OVERFLOW, LST_ERR_ARG (bad hits were dropped), LST_ERR_CUDA. */
+LST_API int lst_sync(lst_ctx* ctx, int slot, void* cuda_stream);
+
+/* Valid after a successful lst_sync of the slot; LST_ERR_STATE otherwise. */
+LST_API int lst_get_mds(lst_ctx* ctx, int slot, lst_md_view* out);
+LST_API int lst_get_segments(lst_ctx* ctx, int slot, lst_seg_view* out);
+LST_API int lst_get_triplets(lst_ctx* ctx, int slot, lst_t3_view* out);
+LST_API int lst_get_quintuplets(lst_ctx* ctx, int slot, lst_t5_view* out);
+/* Valid after any lst_sync of the slot (also after an overflow). */
+LST_API int lst_get_stats(lst_ctx* ctx, int slot, lst_stats* out);
+
+/* Original-hit-index tuples of every object of class `kind` of a synced slot, gathered on the
+ * device and copied to HOST memory: out[n][2 | 4 | 6 | 10] (hits of MD1 lower, MD1 upper,
+ * MD2 lower, ...).  Writes min(n, cap_objects) rows; returns LST_ERR_ARG if cap_objects < n.
+ * Synchronises `cuda_stream`. */
+LST_API int lst_fetch_hit_indices(lst_ctx* ctx, int slot, int kind, int32_t* out, int64_t cap_objects, void* cuda_stream);
+/* Float payload of class `kind` to HOST memory: MD [n][4] sinA, dphi, dphichange, r_anchor;
+ * LS [n][4] sinS, z0, dphi, dphichange; T3 [n][2] kappa, chi2rz; T5 [n][5] as lst_t5_view.f. */
+LST_API int lst_fetch_values(lst_ctx* ctx, int slot, int kind, float* out, int64_t cap_objects, void* cuda_stream);
+
+/* Bytes of the arena (all slots) and of one slot. */
+LST_API int lst_arena_bytes(lst_ctx* ctx, int64_t* total, int64_t* per_slot);
+/* Kernels launched by this context so far (for bench.py's gpu_launches). */
+LST_API int64_t lst_launch_count(lst_ctx* ctx);
+LST_API int lst_last_cuda_error(lst_ctx* ctx);
+LST_API const char* lst_strerror(int status);
+LST_API const char* lst_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LST_H_ */

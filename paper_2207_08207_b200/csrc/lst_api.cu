@@ -1,0 +1,482 @@
+// lst_api.cu -- host side of liblst.so: the C-ABI of include/lst.h, the arena and the slots.
+//
+// Runtime design:
+//  * ONE cudaMalloc in lst_create covers every slot's input staging, hit store, object store,
+//    CSR offsets and scratch ("arena"); per event nothing is allocated or freed, the slot is
+//    recycled by one cudaMemsetAsync of its header + bin counters.
+//  * lst_load_event / lst_run* only enqueue work on the caller's stream; sizes that are only
+//    known on the device (object counts) never come back to the host between stages: grids
+//    are fixed by the geometry / capacities and kernels read the counts from the slot header.
+//    The enqueue sequence is therefore capturable into a CUDA graph by the caller.
+//  * a batch of slots runs through ONE launch per kernel (grid.y = batch index).
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/lst.h"
+#include "lst_device.cuh"
+
+using namespace lst;
+
+static_assert((int)LST_MD == (int)LST_MD_ && (int)LST_SEG == (int)LST_SEG_ && (int)LST_T3 == (int)LST_T3_ &&
+                  (int)LST_T5 == (int)LST_T5_, "stage ids");
+
+namespace {
+
+struct SlotHost {
+  bool loaded = false, ran = false, synced = false;
+  int n_hits_in = 0;
+  SlotHeader* hdr = nullptr;  // pinned host copy of the device header
+  cudaEvent_t ev[7] = {};     // timing: before a0, after a0, before a1, after a1 .. after a4
+  bool ev_bin = false, ev_run = false;
+};
+
+}  // namespace
+
+struct lst_ctx {
+  lst_config cfg;
+  Params P;  // first_slot filled per call
+  int device = 0;
+  signed char* d_layer = nullptr;
+  int* d_run_offsets = nullptr;
+  int2* d_runs = nullptr;
+  char* arena = nullptr;
+  size_t arena_bytes = 0;
+  std::vector<SlotHost> slots;
+  SlotHeader* pinned = nullptr;
+  std::atomic<long long> launches{0};
+  std::atomic<int> last_cuda{0};
+};
+
+namespace {
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+int fail_cuda(lst_ctx* c, cudaError_t e) {
+  if (c) c->last_cuda.store((int)e);
+  return LST_ERR_CUDA;
+}
+#define LST_CUDA(ctx, call)                              \
+  do {                                                   \
+    cudaError_t e__ = (call);                            \
+    if (e__ != cudaSuccess) return fail_cuda(ctx, e__);  \
+  } while (0)
+
+Layout make_layout(const lst_config& cfg, int n_modules) {
+  Layout L{};
+  L.n_modules = n_modules;
+  L.n_bins = 2 * n_modules;
+  L.cap_hits = cfg.cap_hits; L.cap_md = cfg.cap_md; L.cap_seg = cfg.cap_seg; L.cap_t3 = cfg.cap_t3; L.cap_t5 = cfg.cap_t5;
+  L.n_chunk_seg = (cfg.cap_seg + kScanChunk - 1) / kScanChunk;
+  L.n_chunk_t3 = (cfg.cap_t3 + kScanChunk - 1) / kScanChunk;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+  L.hdr = take(sizeof(SlotHeader));
+  L.bin_start = take(sizeof(int) * (size_t)(L.n_bins + 1));
+  L.bin_cursor = take(sizeof(int) * (size_t)L.n_bins);
+  L.reset_bytes = off - L.hdr;
+  const size_t nh = (size_t)cfg.cap_hits, nm = (size_t)cfg.cap_md, ns = (size_t)cfg.cap_seg, n3 = (size_t)cfg.cap_t3, n5 = (size_t)cfg.cap_t5;
+  L.in_x = take(4 * nh); L.in_y = take(4 * nh); L.in_z = take(4 * nh); L.in_module = take(4 * nh); L.in_side = take(nh);
+  L.tmp_idx = take(4 * nh); L.hit4 = take(16 * nh); L.hit_orig = take(4 * nh);
+  L.md_start = take(4 * (size_t)(n_modules + 1));
+  L.md_anchor = take(16 * nm); L.md_aux = take(8 * nm); L.md_hits = take(8 * nm); L.md_out = take(8 * nm); L.md_module = take(4 * nm);
+  L.seg_start = take(4 * (nm + 1)); L.seg_block_base = take(4 * (size_t)(n_modules + 1));
+  L.seg_md = take(8 * ns); L.seg_f = take(16 * ns);
+  L.t3_start = take(4 * (ns + 1)); L.t3_block_base = take(4 * (size_t)(L.n_chunk_seg + 1));
+  L.t3_pack = take(16 * n3); L.t3_seg = take(8 * n3); L.t3_chi2 = take(4 * n3);
+  L.t5_start = take(4 * (n3 + 1)); L.t5_block_base = take(4 * (size_t)(L.n_chunk_t3 + 1));
+  L.t5_md = take(20 * n5); L.t5_t3 = take(8 * n5); L.t5_f = take(20 * n5);
+  size_t scr = 8 * nm;
+  if (16 * ns > scr) scr = 16 * ns;
+  if (24 * n3 > scr) scr = 24 * n3;
+  if (40 * n5 > scr) scr = 40 * n5;
+  L.scratch = take(scr);
+  L.slot_bytes = align_up(off, 4096);
+  return L;
+}
+
+bool valid_slot(const lst_ctx* c, int slot) { return c && slot >= 0 && slot < (int)c->slots.size(); }
+
+void copy_cuts(Cuts& d, const lst_config& s) {
+  d.half_kappa_max = s.half_kappa_max; d.z_lum = s.z_lum;
+  for (int i = 0; i < 6; ++i) {
+    d.md_cos_eps[i] = s.md_cos_eps[i]; d.md_sin_eps[i] = s.md_sin_eps[i]; d.md_dz_res[i] = s.md_dz_res[i];
+    d.md_eps[i] = s.md_eps[i]; d.sigma_z2[i] = s.sigma_z2[i]; d.inv_sigma_z2[i] = s.inv_sigma_z2[i];
+  }
+  d.seg_cos_eps = s.seg_cos_eps; d.seg_sin_eps = s.seg_sin_eps;
+  for (int i = 0; i < 5; ++i) d.seg_z0_max[i] = s.seg_z0_max[i];
+  d.t3_kappa_max = s.t3_kappa_max;
+  for (int i = 0; i < 4; ++i) d.t3_chi2rz_max[i] = s.t3_chi2rz_max[i];
+  d.t5_dkappa_max = s.t5_dkappa_max;
+  for (int i = 0; i < 2; ++i) d.t5_chi2rz_max[i] = s.t5_chi2rz_max[i];
+  d.t5_chi2xy_max = s.t5_chi2xy_max; d.t5_sigma_xy2_scaled = s.t5_sigma_xy2_scaled; d.t5_kappa_max = s.t5_kappa_max;
+}
+
+}  // namespace
+
+extern "C" {
+
+int lst_default_config(lst_config* c) {
+  if (!c) return LST_ERR_ARG;
+  std::memset(c, 0, sizeof(*c));
+  // DESIGN.md section 1, "Constants", typed from the table
+  c->half_kappa_max = 0.00712007098f;
+  c->z_lum = 15.0f;
+  for (int l = 0; l < LST_N_LAYERS; ++l) {
+    const bool ps = l < 3;
+    c->md_cos_eps[l] = ps ? 0.99840045f : 0.995777965f;
+    c->md_sin_eps[l] = ps ? 0.056538377f : 0.0917944759f;
+    c->md_eps[l] = ps ? 0.0565685406f : 0.091923885f;
+    c->md_dz_res[l] = ps ? 0.243244737f : 7.91959572f;
+    c->sigma_z2[l] = ps ? 0.001849f : 1.96f;
+    c->inv_sigma_z2[l] = ps ? 540.832886f : 0.510204077f;
+  }
+  c->seg_cos_eps = 0.999997973f;
+  c->seg_sin_eps = 0.0019999987f;
+  const float zseg[5] = {20.0f, 20.0f, 40.0f, 90.0f, 90.0f};
+  for (int l = 0; l < 5; ++l) c->seg_z0_max[l] = zseg[l];
+  c->t3_kappa_max = 0.0149521492f;
+  const float t3c[4] = {100.0f, 30.0f, 25.0f, 25.0f};
+  for (int l = 0; l < 4; ++l) c->t3_chi2rz_max[l] = t3c[l];
+  c->t5_dkappa_max = 0.000284802838f;
+  c->t5_chi2rz_max[0] = 110.0f;
+  c->t5_chi2rz_max[1] = 150.0f;
+  c->t5_chi2xy_max = 35.0f;
+  c->t5_sigma_xy2_scaled = 6.6015625e-09f;
+  c->t5_kappa_max = 0.0149521492f;
+  c->device = 0;
+  c->n_slots = 4;
+  c->cap_hits = 192 * 1024;
+  c->cap_md = 96 * 1024;
+  c->cap_seg = 256 * 1024;
+  c->cap_t3 = 384 * 1024;
+  c->cap_t5 = 128 * 1024;
+  c->timing = 0;
+  return LST_OK;
+}
+
+int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config* cfg_in, lst_ctx** out) {
+  if (!g || !m || !out) return LST_ERR_ARG;
+  *out = nullptr;
+  lst_config cfg;
+  if (cfg_in) cfg = *cfg_in; else lst_default_config(&cfg);
+  const int n = g->n_modules;
+  if (n <= 0 || n > (1 << 24) || m->n_modules != n || !g->layer || !m->row_offsets) return LST_ERR_ARG;
+  if (cfg.n_slots < 1 || cfg.cap_hits < 1 || cfg.cap_md < 1 || cfg.cap_seg < 1 || cfg.cap_t3 < 1 || cfg.cap_t5 < 1) return LST_ERR_ARG;
+  for (int i = 0; i < n; ++i)
+    if (g->layer[i] < 0 || g->layer[i] >= LST_N_LAYERS) return LST_ERR_ARG;
+  if (m->row_offsets[0] != 0) return LST_ERR_ARG;
+  for (int i = 0; i < n; ++i)
+    if (m->row_offsets[i + 1] < m->row_offsets[i]) return LST_ERR_ARG;
+  if (m->row_offsets[n] > 0 && !m->targets) return LST_ERR_ARG;
+  // rows strictly ascending, targets in the next layer; compress each row into runs of
+  // consecutive module ids (a ring's phi-neighbours are consecutive ids)
+  std::vector<int> run_offsets(n + 1, 0);
+  std::vector<int2> runs;
+  for (int a = 0; a < n; ++a) {
+    for (int k = m->row_offsets[a]; k < m->row_offsets[a + 1]; ++k) {
+      const int t = m->targets[k];
+      if (t < 0 || t >= n || g->layer[t] != g->layer[a] + 1) return LST_ERR_ARG;
+      if (k > m->row_offsets[a] && t <= m->targets[k - 1]) return LST_ERR_ARG;
+      if (k > m->row_offsets[a] && t == runs.back().y + 1) runs.back().y = t;
+      else runs.push_back(make_int2(t, t));
+    }
+    run_offsets[a + 1] = (int)runs.size();
+  }
+
+  lst_ctx* c = new (std::nothrow) lst_ctx();
+  if (!c) return LST_ERR_NOMEM;
+  c->cfg = cfg;
+  c->device = cfg.device;
+  auto bail = [&](int status, cudaError_t e) {
+    if (status == LST_ERR_CUDA) c->last_cuda.store((int)e);
+    lst_destroy(c);
+    return status;
+  };
+  cudaError_t e;
+  if ((e = cudaSetDevice(cfg.device)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
+  const Layout L = make_layout(cfg, n);
+  c->arena_bytes = L.slot_bytes * (size_t)cfg.n_slots;
+  if ((e = cudaMalloc(&c->d_layer, n)) != cudaSuccess) return bail(LST_ERR_NOMEM, e);
+  if ((e = cudaMalloc(&c->d_run_offsets, sizeof(int) * (n + 1))) != cudaSuccess) return bail(LST_ERR_NOMEM, e);
+  if ((e = cudaMalloc(&c->d_runs, sizeof(int2) * (runs.size() + 1))) != cudaSuccess) return bail(LST_ERR_NOMEM, e);
+  if ((e = cudaMalloc(&c->arena, c->arena_bytes)) != cudaSuccess) { cudaGetLastError(); return bail(LST_ERR_NOMEM, e); }
+  if ((e = cudaMemcpy(c->d_layer, g->layer, n, cudaMemcpyHostToDevice)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
+  if ((e = cudaMemcpy(c->d_run_offsets, run_offsets.data(), sizeof(int) * (n + 1), cudaMemcpyHostToDevice)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
+  if (!runs.empty() && (e = cudaMemcpy(c->d_runs, runs.data(), sizeof(int2) * runs.size(), cudaMemcpyHostToDevice)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
+  if ((e = cudaMemset(c->arena, 0, c->arena_bytes)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
+  if ((e = cudaMallocHost(&c->pinned, sizeof(SlotHeader) * (size_t)cfg.n_slots)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
+  std::memset(c->pinned, 0, sizeof(SlotHeader) * (size_t)cfg.n_slots);
+  c->slots.resize(cfg.n_slots);
+  for (int s = 0; s < cfg.n_slots; ++s) {
+    c->slots[s].hdr = c->pinned + s;
+    if (cfg.timing)
+      for (auto& ev : c->slots[s].ev)
+        if ((e = cudaEventCreate(&ev)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
+  }
+  c->P.arena = c->arena;
+  c->P.slot_stride = L.slot_bytes;
+  c->P.L = L;
+  copy_cuts(c->P.cuts, cfg);
+  c->P.mod_layer = c->d_layer;
+  c->P.run_offsets = c->d_run_offsets;
+  c->P.runs = c->d_runs;
+  c->P.first_slot = 0;
+  if ((e = cudaDeviceSynchronize()) != cudaSuccess) return bail(LST_ERR_CUDA, e);
+  *out = c;
+  return LST_OK;
+}
+
+int lst_destroy(lst_ctx* c) {
+  if (!c) return LST_ERR_ARG;
+  cudaSetDevice(c->device);
+  for (auto& s : c->slots)
+    for (auto& ev : s.ev)
+      if (ev) cudaEventDestroy(ev);
+  if (c->pinned) cudaFreeHost(c->pinned);
+  if (c->arena) cudaFree(c->arena);
+  if (c->d_runs) cudaFree(c->d_runs);
+  if (c->d_run_offsets) cudaFree(c->d_run_offsets);
+  if (c->d_layer) cudaFree(c->d_layer);
+  delete c;
+  return LST_OK;
+}
+
+int lst_load_event(lst_ctx* c, int slot, const lst_hits* h, void* stream) {
+  if (!valid_slot(c, slot) || !h || h->n < 0) return LST_ERR_ARG;
+  if (h->n > 0 && (!h->x || !h->y || !h->z || !h->module || !h->side)) return LST_ERR_ARG;
+  if (h->n > c->cfg.cap_hits) return LST_ERR_OVERFLOW;
+  cudaStream_t s = (cudaStream_t)stream;
+  LST_CUDA(c, cudaSetDevice(c->device));
+  SlotHost& sh = c->slots[slot];
+  sh.loaded = sh.ran = sh.synced = false;
+  sh.n_hits_in = h->n;
+  const Layout& L = c->P.L;
+  char* base = c->arena + (size_t)slot * c->P.slot_stride;
+  if (c->cfg.timing) { LST_CUDA(c, cudaEventRecord(sh.ev[0], s)); }
+  LST_CUDA(c, cudaMemsetAsync(base + L.hdr, 0, L.reset_bytes, s));
+  HitInput in{h->x, h->y, h->z, h->module, h->side, h->n};
+  if (!h->on_device && h->n > 0) {
+    const size_t n = (size_t)h->n;
+    LST_CUDA(c, cudaMemcpyAsync(base + L.in_x, h->x, 4 * n, cudaMemcpyHostToDevice, s));
+    LST_CUDA(c, cudaMemcpyAsync(base + L.in_y, h->y, 4 * n, cudaMemcpyHostToDevice, s));
+    LST_CUDA(c, cudaMemcpyAsync(base + L.in_z, h->z, 4 * n, cudaMemcpyHostToDevice, s));
+    LST_CUDA(c, cudaMemcpyAsync(base + L.in_module, h->module, 4 * n, cudaMemcpyHostToDevice, s));
+    LST_CUDA(c, cudaMemcpyAsync(base + L.in_side, h->side, n, cudaMemcpyHostToDevice, s));
+    in.x = reinterpret_cast<const float*>(base + L.in_x);
+    in.y = reinterpret_cast<const float*>(base + L.in_y);
+    in.z = reinterpret_cast<const float*>(base + L.in_z);
+    in.module = reinterpret_cast<const int*>(base + L.in_module);
+    in.side = reinterpret_cast<const unsigned char*>(base + L.in_side);
+  }
+  Params P = c->P;
+  P.first_slot = slot;
+  c->launches += launch_bin(P, in, s);
+  LST_CUDA(c, cudaGetLastError());
+  if (c->cfg.timing) { LST_CUDA(c, cudaEventRecord(sh.ev[1], s)); sh.ev_bin = true; }
+  sh.loaded = true;
+  return LST_OK;
+}
+
+int lst_run_stage(lst_ctx* c, int first, int n, int stage, void* stream) {
+  if (!c || n < 1 || !valid_slot(c, first) || !valid_slot(c, first + n - 1) || stage < LST_MD || stage > LST_T5) return LST_ERR_ARG;
+  for (int s = first; s < first + n; ++s)
+    if (!c->slots[s].loaded) return LST_ERR_STATE;
+  cudaStream_t st = (cudaStream_t)stream;
+  LST_CUDA(c, cudaSetDevice(c->device));
+  SlotHost& sh = c->slots[first];
+  if (c->cfg.timing && stage == LST_MD) { LST_CUDA(c, cudaEventRecord(sh.ev[2], st)); }
+  Params P = c->P;
+  P.first_slot = first;
+  c->launches += launch_stage(P, n, stage, st);
+  LST_CUDA(c, cudaGetLastError());
+  if (c->cfg.timing) { LST_CUDA(c, cudaEventRecord(sh.ev[3 + stage], st)); if (stage == LST_T5) sh.ev_run = true; }
+  for (int s = first; s < first + n; ++s) { c->slots[s].synced = false; if (stage == LST_T5) c->slots[s].ran = true; }
+  return LST_OK;
+}
+
+int lst_run_batch(lst_ctx* c, int first, int n, void* stream) {
+  for (int stage = LST_MD; stage <= LST_T5; ++stage) {
+    const int r = lst_run_stage(c, first, n, stage, stream);
+    if (r != LST_OK) return r;
+  }
+  return LST_OK;
+}
+
+int lst_run(lst_ctx* c, int slot, void* stream) { return lst_run_batch(c, slot, 1, stream); }
+
+int lst_sync(lst_ctx* c, int slot, void* stream) {
+  if (!valid_slot(c, slot)) return LST_ERR_ARG;
+  SlotHost& sh = c->slots[slot];
+  if (!sh.loaded) return LST_ERR_STATE;
+  cudaStream_t s = (cudaStream_t)stream;
+  LST_CUDA(c, cudaSetDevice(c->device));
+  const char* base = c->arena + (size_t)slot * c->P.slot_stride;
+  LST_CUDA(c, cudaMemcpyAsync(sh.hdr, base + c->P.L.hdr, sizeof(SlotHeader), cudaMemcpyDeviceToHost, s));
+  LST_CUDA(c, cudaStreamSynchronize(s));
+  sh.synced = true;
+  if (sh.hdr->overflow) return LST_ERR_OVERFLOW;
+  if (sh.hdr->bad_hits) return LST_ERR_ARG;
+  return LST_OK;
+}
+
+static int view_ready(lst_ctx* c, int slot) {
+  if (!valid_slot(c, slot)) return LST_ERR_ARG;
+  const SlotHost& sh = c->slots[slot];
+  if (!sh.synced || !sh.ran) return LST_ERR_STATE;
+  if (sh.hdr->overflow) return LST_ERR_OVERFLOW;
+  return LST_OK;
+}
+
+int lst_get_mds(lst_ctx* c, int slot, lst_md_view* v) {
+  const int r = view_ready(c, slot);
+  if (r != LST_OK || !v) return r != LST_OK ? r : LST_ERR_ARG;
+  const Layout& L = c->P.L;
+  const char* b = c->arena + (size_t)slot * c->P.slot_stride;
+  v->n = c->slots[slot].hdr->n[LST_MD];
+  v->hits = (const int32_t*)(b + L.md_hits);
+  v->module = (const int32_t*)(b + L.md_module);
+  v->anchor = (const float*)(b + L.md_anchor);
+  v->ur_sina = (const float*)(b + L.md_aux);
+  v->dphi_dphichange = (const float*)(b + L.md_out);
+  v->module_start = (const int32_t*)(b + L.md_start);
+  return LST_OK;
+}
+
+int lst_get_segments(lst_ctx* c, int slot, lst_seg_view* v) {
+  const int r = view_ready(c, slot);
+  if (r != LST_OK || !v) return r != LST_OK ? r : LST_ERR_ARG;
+  const Layout& L = c->P.L;
+  const char* b = c->arena + (size_t)slot * c->P.slot_stride;
+  v->n = c->slots[slot].hdr->n[LST_SEG];
+  v->md = (const int32_t*)(b + L.seg_md);
+  v->f = (const float*)(b + L.seg_f);
+  v->md_start = (const int32_t*)(b + L.seg_start);
+  return LST_OK;
+}
+
+int lst_get_triplets(lst_ctx* c, int slot, lst_t3_view* v) {
+  const int r = view_ready(c, slot);
+  if (r != LST_OK || !v) return r != LST_OK ? r : LST_ERR_ARG;
+  const Layout& L = c->P.L;
+  const char* b = c->arena + (size_t)slot * c->P.slot_stride;
+  v->n = c->slots[slot].hdr->n[LST_T3];
+  v->md_kappa = (const int32_t*)(b + L.t3_pack);
+  v->seg = (const int32_t*)(b + L.t3_seg);
+  v->chi2rz = (const float*)(b + L.t3_chi2);
+  v->seg_start = (const int32_t*)(b + L.t3_start);
+  return LST_OK;
+}
+
+int lst_get_quintuplets(lst_ctx* c, int slot, lst_t5_view* v) {
+  const int r = view_ready(c, slot);
+  if (r != LST_OK || !v) return r != LST_OK ? r : LST_ERR_ARG;
+  const Layout& L = c->P.L;
+  const char* b = c->arena + (size_t)slot * c->P.slot_stride;
+  v->n = c->slots[slot].hdr->n[LST_T5];
+  v->md = (const int32_t*)(b + L.t5_md);
+  v->t3 = (const int32_t*)(b + L.t5_t3);
+  v->f = (const float*)(b + L.t5_f);
+  v->t3_start = (const int32_t*)(b + L.t5_start);
+  return LST_OK;
+}
+
+int lst_get_stats(lst_ctx* c, int slot, lst_stats* o) {
+  if (!valid_slot(c, slot) || !o) return LST_ERR_ARG;
+  SlotHost& sh = c->slots[slot];
+  if (!sh.synced) return LST_ERR_STATE;
+  std::memset(o, 0, sizeof(*o));
+  o->n_hits = sh.hdr->n_hits;
+  for (int k = 0; k < 4; ++k) { o->needed[k] = (int64_t)sh.hdr->needed[k]; o->candidates[k] = (int64_t)sh.hdr->cand[k]; }
+  o->overflow = sh.hdr->overflow;
+  o->bad_hits = sh.hdr->bad_hits;
+  if (c->cfg.timing) {
+    if (sh.ev_bin) cudaEventElapsedTime(&o->stage_ms[0], sh.ev[0], sh.ev[1]);
+    if (sh.ev_run)
+      for (int k = 0; k < 4; ++k) cudaEventElapsedTime(&o->stage_ms[1 + k], sh.ev[2 + k], sh.ev[3 + k]);
+    cudaGetLastError();
+  }
+  return LST_OK;
+}
+
+static const int kHitsPerObject[4] = {2, 4, 6, 10};
+
+int lst_fetch_hit_indices(lst_ctx* c, int slot, int kind, int32_t* out, int64_t cap, void* stream) {
+  if (kind < LST_MD || kind > LST_T5) return LST_ERR_ARG;
+  const int r = view_ready(c, slot);
+  if (r != LST_OK) return r;
+  const int n = c->slots[slot].hdr->n[kind];
+  if (n == 0) return LST_OK;
+  if (!out || cap < n) return LST_ERR_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  LST_CUDA(c, cudaSetDevice(c->device));
+  Params P = c->P;
+  P.first_slot = slot;
+  c->launches += launch_gather_hits(P, kind, n, s);
+  LST_CUDA(c, cudaGetLastError());
+  const char* b = c->arena + (size_t)slot * c->P.slot_stride;
+  LST_CUDA(c, cudaMemcpyAsync(out, b + P.L.scratch, sizeof(int32_t) * (size_t)n * kHitsPerObject[kind], cudaMemcpyDeviceToHost, s));
+  LST_CUDA(c, cudaStreamSynchronize(s));
+  return LST_OK;
+}
+
+int lst_fetch_values(lst_ctx* c, int slot, int kind, float* out, int64_t cap, void* stream) {
+  if (kind < LST_MD || kind > LST_T5) return LST_ERR_ARG;
+  const int r = view_ready(c, slot);
+  if (r != LST_OK) return r;
+  const int n = c->slots[slot].hdr->n[kind];
+  if (n == 0) return LST_OK;
+  if (!out || cap < n) return LST_ERR_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  LST_CUDA(c, cudaSetDevice(c->device));
+  Params P = c->P;
+  P.first_slot = slot;
+  const char* b = c->arena + (size_t)slot * c->P.slot_stride;
+  const char* src;
+  size_t width;
+  if (kind == LST_MD || kind == LST_T3) {
+    c->launches += launch_pack_values(P, kind, n, s);
+    LST_CUDA(c, cudaGetLastError());
+    src = b + P.L.scratch;
+    width = kind == LST_MD ? 4 : 2;
+  } else if (kind == LST_SEG) {
+    src = b + P.L.seg_f;
+    width = 4;
+  } else {
+    src = b + P.L.t5_f;
+    width = 5;
+  }
+  LST_CUDA(c, cudaMemcpyAsync(out, src, sizeof(float) * (size_t)n * width, cudaMemcpyDeviceToHost, s));
+  LST_CUDA(c, cudaStreamSynchronize(s));
+  return LST_OK;
+}
+
+int lst_arena_bytes(lst_ctx* c, int64_t* total, int64_t* per_slot) {
+  if (!c) return LST_ERR_ARG;
+  if (total) *total = (int64_t)c->arena_bytes;
+  if (per_slot) *per_slot = (int64_t)c->P.slot_stride;
+  return LST_OK;
+}
+
+int64_t lst_launch_count(lst_ctx* c) { return c ? (int64_t)c->launches.load() : 0; }
+int lst_last_cuda_error(lst_ctx* c) { return c ? c->last_cuda.load() : 0; }
+
+const char* lst_strerror(int s) {
+  switch (s) {
+    case LST_OK: return "ok";
+    case LST_ERR_ARG: return "invalid argument or input (geometry, module map, slot, module id, side)";
+    case LST_ERR_CUDA: return "CUDA runtime error (see lst_last_cuda_error)";
+    case LST_ERR_OVERFLOW: return "a per-slot capacity was exceeded; outputs of the slot are invalid";
+    case LST_ERR_STATE: return "call out of order (load -> run -> sync -> get)";
+    case LST_ERR_NOMEM: return "arena allocation failed";
+  }
+  return "unknown status";
+}
+
+const char* lst_version(void) { return "lst-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

@@ -1,0 +1,131 @@
+// lst_device.cuh -- device-side data layout of one event slot and the kernel launch parameters.
+//
+// One arena (a single cudaMalloc in lst_create) holds n_slots identical slots;
+// every array of a slot sits at a fixed byte offset from the slot base (struct Layout), so a
+// kernel finds slot s at arena + s * slot_stride and needs no per-slot pointer table.  The
+// batch index (which slot of a batch) is blockIdx.y of every kernel.
+//
+// Object store (per slot), "SoA of small vectors": each object class keeps one array per
+// GROUP of fields that are always read together, packed to 8 or 16 bytes so one vector load
+// fetches the group (PAPER.md:139-141 argues for SoA on V100; on sm_100a the unit that matters
+// is the 16-B vector / 32-B sector):
+//   hits   hit4[i]    = (x, y, z, r)            float4   binned by (module, side)
+//          hit_orig[i]= original index          int
+//   MD     md_anchor  = (x, y, z, r) of anchor  float4
+//          md_aux     = (r_upper, sinA)         float2
+//          md_hits    = (orig lower, orig upper)int2
+//          md_out     = (dphi, dphichange)      float2
+//          md_module                            int
+//   LS     seg_md     = (inner MD, outer MD)    int2
+//          seg_f      = (sinS, z0, dphi, dphichange) float4
+//   T3     t3_pack    = (MD1, MD2, MD3, kappa)  int4 (kappa as bits)
+//          t3_seg     = (seg a, seg b)          int2
+//          t3_chi2                              float
+//   T5     t5_md[5], t5_t3 = (A, B) int2, t5_f[5] = kA, kB, kfit, chi2xy, chi2rz
+// CSR offsets: bin_start[2*n_modules+1], md_start[n_modules+1], seg_start[cap_md+1] (by inner
+// MD), t3_start[cap_seg+1] (by first segment), t5_start[cap_t3+1] (by inner triplet).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "lst_cuts.cuh"
+
+namespace lst {
+
+constexpr int kScanChunk = 256;  // owners (segments / triplets) per block chunk in T3 / T5
+enum { LST_MD_ = 0, LST_SEG_ = 1, LST_T3_ = 2, LST_T5_ = 3 };  // == LST_MD .. LST_T5 of lst.h
+
+struct SlotHeader {
+  int n_hits;                     // valid hits binned
+  int n[4];                       // objects stored (clamped to capacity): MD, LS, T3, T5
+  int overflow;                   // bit k: class k exceeded its capacity
+  int bad_hits;                   // hits dropped (module id / side out of range)
+  int pad0;
+  unsigned long long needed[4];   // objects that passed (unclamped)
+  unsigned long long cand[4];     // candidates examined
+  unsigned int done[8];           // "last block done" tickets, self-resetting
+};
+
+struct Layout {
+  int n_modules, n_bins;
+  int cap_hits, cap_md, cap_seg, cap_t3, cap_t5;
+  int n_chunk_seg, n_chunk_t3;    // ceil(cap / kScanChunk)
+  // byte offsets from the slot base (all multiples of 256)
+  size_t hdr, bin_start, bin_cursor;          // hdr, bin_start and bin_cursor are contiguous: one memset
+  size_t reset_bytes;                         // bytes to zero at lst_load_event, from hdr
+  size_t in_x, in_y, in_z, in_module, in_side;// staging of host input
+  size_t tmp_idx, hit4, hit_orig;
+  size_t md_start, md_anchor, md_aux, md_hits, md_out, md_module;
+  size_t seg_start, seg_block_base, seg_md, seg_f;
+  size_t t3_start, t3_block_base, t3_pack, t3_seg, t3_chi2;
+  size_t t5_start, t5_block_base, t5_md, t5_t3, t5_f;
+  size_t scratch;
+  size_t slot_bytes;
+};
+
+// Launch parameters, passed by value (constant bank): no per-launch device reads to find data.
+struct Params {
+  char* arena;
+  size_t slot_stride;
+  Layout L;
+  Cuts cuts;
+  const signed char* mod_layer;  // [n_modules]
+  const int* run_offsets;        // [n_modules + 1] module map as runs of consecutive target modules
+  const int2* runs;              // [run_offsets[n_modules]] (first target, last target), ascending
+  int first_slot;
+};
+
+// Typed access to one slot.
+struct Slot {
+  char* b;
+  const Layout& L;
+  __device__ __forceinline__ Slot(const Params& P, int batch_index)
+      : b(P.arena + (size_t)(P.first_slot + batch_index) * P.slot_stride), L(P.L) {}
+  template <class T>
+  __device__ __forceinline__ T* at(size_t off) const { return reinterpret_cast<T*>(b + off); }
+  __device__ __forceinline__ SlotHeader* hdr() const { return at<SlotHeader>(L.hdr); }
+  __device__ __forceinline__ unsigned* bin_start() const { return at<unsigned>(L.bin_start); }
+  __device__ __forceinline__ unsigned* bin_cursor() const { return at<unsigned>(L.bin_cursor); }
+  __device__ __forceinline__ int* tmp_idx() const { return at<int>(L.tmp_idx); }
+  __device__ __forceinline__ float4* hit4() const { return at<float4>(L.hit4); }
+  __device__ __forceinline__ int* hit_orig() const { return at<int>(L.hit_orig); }
+  __device__ __forceinline__ int* md_start() const { return at<int>(L.md_start); }
+  __device__ __forceinline__ float4* md_anchor() const { return at<float4>(L.md_anchor); }
+  __device__ __forceinline__ float2* md_aux() const { return at<float2>(L.md_aux); }
+  __device__ __forceinline__ int2* md_hits() const { return at<int2>(L.md_hits); }
+  __device__ __forceinline__ float2* md_out() const { return at<float2>(L.md_out); }
+  __device__ __forceinline__ int* md_module() const { return at<int>(L.md_module); }
+  __device__ __forceinline__ int* seg_start() const { return at<int>(L.seg_start); }
+  __device__ __forceinline__ int* seg_block_base() const { return at<int>(L.seg_block_base); }
+  __device__ __forceinline__ int2* seg_md() const { return at<int2>(L.seg_md); }
+  __device__ __forceinline__ float4* seg_f() const { return at<float4>(L.seg_f); }
+  __device__ __forceinline__ int* t3_start() const { return at<int>(L.t3_start); }
+  __device__ __forceinline__ int* t3_block_base() const { return at<int>(L.t3_block_base); }
+  __device__ __forceinline__ int4* t3_pack() const { return at<int4>(L.t3_pack); }
+  __device__ __forceinline__ int2* t3_seg() const { return at<int2>(L.t3_seg); }
+  __device__ __forceinline__ float* t3_chi2() const { return at<float>(L.t3_chi2); }
+  __device__ __forceinline__ int* t5_start() const { return at<int>(L.t5_start); }
+  __device__ __forceinline__ int* t5_block_base() const { return at<int>(L.t5_block_base); }
+  __device__ __forceinline__ int* t5_md() const { return at<int>(L.t5_md); }
+  __device__ __forceinline__ int2* t5_t3() const { return at<int2>(L.t5_t3); }
+  __device__ __forceinline__ float* t5_f() const { return at<float>(L.t5_f); }
+  __device__ __forceinline__ int* scratch() const { return at<int>(L.scratch); }
+};
+
+// Raw input arrays of one event (caller's device pointers, or the slot's staging area).
+struct HitInput {
+  const float* x;
+  const float* y;
+  const float* z;
+  const int* module;
+  const unsigned char* side;
+  int n;
+};
+
+// Host-callable launchers (lst_kernels.cu). Each returns the number of kernels it launched.
+int launch_bin(const Params& P, const HitInput& in, cudaStream_t s);
+int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s);
+int launch_gather_hits(const Params& P, int kind, int n, cudaStream_t s);
+int launch_pack_values(const Params& P, int kind, int n, cudaStream_t s);
+
+}  // namespace lst

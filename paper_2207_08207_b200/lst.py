@@ -1,0 +1,325 @@
+"""Thin ctypes binding over the C-ABI library ``liblst.so`` (include/lst.h).
+
+Argument marshalling only: every step of the path (binning, mini-doublets, segments, triplets,
+quintuplets, gathers) runs in the CUDA kernels of ``csrc/``.  There is NO CPU fallback: if the
+library is missing or fails to load, importing the binding's entry points raises.
+
+PyTorch is used by callers for device memory and streams; this module itself needs only ctypes
+and numpy.  Device arrays returned by the ``*_view`` calls are exposed through
+``__cuda_array_interface__`` (``torch.as_tensor(view_array, device="cuda")`` is zero-copy).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "liblst.so")
+N_LAYERS = 6
+MD, SEG, T3, T5 = 0, 1, 2, 3
+KIND_NAMES = ("md", "seg", "t3", "t5")
+HITS_PER_OBJECT = (2, 4, 6, 10)
+VALUES_PER_OBJECT = (4, 4, 2, 5)
+
+OK, ERR_ARG, ERR_CUDA, ERR_OVERFLOW, ERR_STATE, ERR_NOMEM = 0, -1, -2, -3, -4, -5
+
+
+class LstError(RuntimeError):
+    def __init__(self, status: int, what: str):
+        super().__init__(f"{what}: {status} ({strerror(status)})")
+        self.status = status
+
+
+class Geometry(C.Structure):
+    _fields_ = [("n_modules", C.c_int32), ("layer", C.c_void_p), ("kind", C.c_void_p), ("cx", C.c_void_p),
+                ("cy", C.c_void_p), ("cz", C.c_void_p), ("phi", C.c_void_p)]
+
+
+class ModuleMap(C.Structure):
+    _fields_ = [("n_modules", C.c_int32), ("row_offsets", C.c_void_p), ("targets", C.c_void_p)]
+
+
+class Config(C.Structure):
+    _fields_ = [("half_kappa_max", C.c_float), ("z_lum", C.c_float),
+                ("md_cos_eps", C.c_float * 6), ("md_sin_eps", C.c_float * 6), ("md_dz_res", C.c_float * 6),
+                ("md_eps", C.c_float * 6), ("seg_cos_eps", C.c_float), ("seg_sin_eps", C.c_float),
+                ("seg_z0_max", C.c_float * 5), ("t3_kappa_max", C.c_float), ("t3_chi2rz_max", C.c_float * 4),
+                ("sigma_z2", C.c_float * 6), ("inv_sigma_z2", C.c_float * 6), ("t5_dkappa_max", C.c_float),
+                ("t5_chi2rz_max", C.c_float * 2), ("t5_chi2xy_max", C.c_float), ("t5_sigma_xy2_scaled", C.c_float),
+                ("t5_kappa_max", C.c_float),
+                ("device", C.c_int32), ("n_slots", C.c_int32), ("cap_hits", C.c_int32), ("cap_md", C.c_int32),
+                ("cap_seg", C.c_int32), ("cap_t3", C.c_int32), ("cap_t5", C.c_int32), ("timing", C.c_int32)]
+
+    CUT_FIELDS = ("half_kappa_max", "z_lum", "md_cos_eps", "md_sin_eps", "md_dz_res", "md_eps", "seg_cos_eps",
+                  "seg_sin_eps", "seg_z0_max", "t3_kappa_max", "t3_chi2rz_max", "sigma_z2", "inv_sigma_z2",
+                  "t5_dkappa_max", "t5_chi2rz_max", "t5_chi2xy_max", "t5_sigma_xy2_scaled", "t5_kappa_max")
+
+    def cuts_dict(self) -> dict:
+        out = {}
+        for n in self.CUT_FIELDS:
+            v = getattr(self, n)
+            out[n] = float(v) if isinstance(v, float) else [float(x) for x in v]
+        return out
+
+
+class Hits(C.Structure):
+    _fields_ = [("n", C.c_int32), ("x", C.c_void_p), ("y", C.c_void_p), ("z", C.c_void_p),
+                ("module", C.c_void_p), ("side", C.c_void_p), ("on_device", C.c_int32)]
+
+
+class MdView(C.Structure):
+    _fields_ = [("n", C.c_int32), ("hits", C.c_void_p), ("module", C.c_void_p), ("anchor", C.c_void_p),
+                ("ur_sina", C.c_void_p), ("dphi_dphichange", C.c_void_p), ("module_start", C.c_void_p)]
+
+
+class SegView(C.Structure):
+    _fields_ = [("n", C.c_int32), ("md", C.c_void_p), ("f", C.c_void_p), ("md_start", C.c_void_p)]
+
+
+class T3View(C.Structure):
+    _fields_ = [("n", C.c_int32), ("md_kappa", C.c_void_p), ("seg", C.c_void_p), ("chi2rz", C.c_void_p),
+                ("seg_start", C.c_void_p)]
+
+
+class T5View(C.Structure):
+    _fields_ = [("n", C.c_int32), ("md", C.c_void_p), ("t3", C.c_void_p), ("f", C.c_void_p), ("t3_start", C.c_void_p)]
+
+
+class Stats(C.Structure):
+    _fields_ = [("n_hits", C.c_int32), ("needed", C.c_int64 * 4), ("candidates", C.c_int64 * 4),
+                ("overflow", C.c_int32), ("bad_hits", C.c_int32), ("stage_ms", C.c_float * 5)]
+
+
+# every symbol include/lst.h declares: name -> (restype, argtypes)
+P = C.POINTER
+SYMBOLS = {
+    "lst_default_config": (C.c_int, [P(Config)]),
+    "lst_create": (C.c_int, [P(Geometry), P(ModuleMap), P(Config), P(C.c_void_p)]),
+    "lst_destroy": (C.c_int, [C.c_void_p]),
+    "lst_load_event": (C.c_int, [C.c_void_p, C.c_int, P(Hits), C.c_void_p]),
+    "lst_run": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
+    "lst_run_batch": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p]),
+    "lst_run_stage": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]),
+    "lst_sync": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
+    "lst_get_mds": (C.c_int, [C.c_void_p, C.c_int, P(MdView)]),
+    "lst_get_segments": (C.c_int, [C.c_void_p, C.c_int, P(SegView)]),
+    "lst_get_triplets": (C.c_int, [C.c_void_p, C.c_int, P(T3View)]),
+    "lst_get_quintuplets": (C.c_int, [C.c_void_p, C.c_int, P(T5View)]),
+    "lst_get_stats": (C.c_int, [C.c_void_p, C.c_int, P(Stats)]),
+    "lst_fetch_hit_indices": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int64, C.c_void_p]),
+    "lst_fetch_values": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int64, C.c_void_p]),
+    "lst_arena_bytes": (C.c_int, [C.c_void_p, P(C.c_int64), P(C.c_int64)]),
+    "lst_launch_count": (C.c_int64, [C.c_void_p]),
+    "lst_last_cuda_error": (C.c_int, [C.c_void_p]),
+    "lst_strerror": (C.c_char_p, [C.c_int]),
+    "lst_version": (C.c_char_p, []),
+}
+
+_lib = None
+
+
+def load_library(path: str = LIB_PATH):
+    """dlopen liblst.so and bind every symbol; raises if the library or a symbol is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(path):
+            raise ImportError(f"{path} is missing: build it with `python -m paper_2207_08207_b200.build` "
+                              "(there is no CPU fallback)")
+        lib = C.CDLL(path)
+        for name, (res, args) in SYMBOLS.items():
+            fn = getattr(lib, name)            # AttributeError if the symbol is not exported
+            fn.restype, fn.argtypes = res, args
+        _lib = lib
+    return _lib
+
+
+def strerror(status: int) -> str:
+    return load_library().lst_strerror(int(status)).decode()
+
+
+def default_config() -> Config:
+    cfg = Config()
+    st = load_library().lst_default_config(C.byref(cfg))
+    if st != OK:
+        raise LstError(st, "lst_default_config")
+    return cfg
+
+
+class DeviceArray:
+    """A borrowed device array (library-owned memory) visible to torch / cupy / numba."""
+
+    def __init__(self, ptr: int, shape, typestr: str, owner):
+        self._owner = owner
+        self.shape = tuple(int(s) for s in shape)
+        self.__cuda_array_interface__ = {"shape": self.shape, "typestr": typestr, "data": (int(ptr or 0), True),
+                                         "version": 2, "strides": None}
+
+    def torch(self):
+        import torch
+        if 0 in self.shape:
+            return torch.empty(self.shape, dtype={"<i4": torch.int32, "<f4": torch.float32}[self.__cuda_array_interface__["typestr"]], device="cuda")
+        return torch.as_tensor(self, device="cuda")
+
+
+def _ptr(a) -> int:
+    """Raw address of a numpy array (host) or of anything with data_ptr() (torch tensor)."""
+    if a is None:
+        return 0
+    if hasattr(a, "data_ptr"):
+        return int(a.data_ptr())
+    return int(a.ctypes.data)
+
+
+def _stream(s) -> int:
+    """None / int / torch.cuda.Stream -> cudaStream_t as an integer."""
+    if s is None:
+        return 0
+    if hasattr(s, "cuda_stream"):
+        return int(s.cuda_stream)
+    return int(s)
+
+
+class Lst:
+    """One library context: geometry + module map + arena of event slots (lst_create)."""
+
+    def __init__(self, layer, row_offsets, targets, config: Config | None = None, *, kind=None, cx=None, cy=None,
+                 cz=None, phi=None):
+        self.lib = load_library()
+        self.cfg = config if config is not None else default_config()
+        layer = np.ascontiguousarray(layer, np.int8)
+        row_offsets = np.ascontiguousarray(row_offsets, np.int32)
+        targets = np.ascontiguousarray(targets, np.int32)
+        keep = [layer, row_offsets, targets]
+        opt = []
+        for a, dt in ((kind, np.int8), (cx, np.float32), (cy, np.float32), (cz, np.float32), (phi, np.float32)):
+            a = None if a is None else np.ascontiguousarray(a, dt)
+            opt.append(a)
+            keep.append(a)
+        g = Geometry(len(layer), _ptr(layer), *[_ptr(a) for a in opt])
+        m = ModuleMap(len(row_offsets) - 1, _ptr(row_offsets), _ptr(targets))
+        h = C.c_void_p()
+        st = self.lib.lst_create(C.byref(g), C.byref(m), C.byref(self.cfg), C.byref(h))
+        if st != OK:
+            raise LstError(st, "lst_create")
+        self.h = h
+        self.n_modules = len(layer)
+        self.n_slots = int(self.cfg.n_slots)
+        self._borrowed = {}
+
+    @classmethod
+    def from_synth(cls, geom, mmap, config: Config | None = None):
+        return cls(geom.layer, mmap.row_offsets, mmap.targets, config, kind=geom.kind, cx=geom.cx, cy=geom.cy,
+                   cz=geom.cz, phi=geom.phi)
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.lst_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, st, what, allow=()):
+        if st != OK and st not in allow:
+            raise LstError(st, what)
+        return st
+
+    # ---- the path ---------------------------------------------------------------------------
+    def load_event(self, slot: int, x, y, z, module, side, stream=None):
+        """Arrays: all numpy (host) or all torch CUDA tensors (device); dtypes f32/f32/f32/i32/u8."""
+        on_device = hasattr(x, "data_ptr") and getattr(x, "is_cuda", False)
+        n = int(x.shape[0])
+        if not on_device and not hasattr(x, "data_ptr"):
+            x, y, z = (np.ascontiguousarray(a, np.float32) for a in (x, y, z))
+            module = np.ascontiguousarray(module, np.int32)
+            side = np.ascontiguousarray(side, np.uint8)
+        self._borrowed[slot] = (x, y, z, module, side)     # keep alive while the stream may read them
+        hits = Hits(n, _ptr(x), _ptr(y), _ptr(z), _ptr(module), _ptr(side), 1 if on_device else 0)
+        return self._check(self.lib.lst_load_event(self.h, slot, C.byref(hits), _stream(stream)), "lst_load_event")
+
+    def run(self, slot: int, stream=None):
+        return self._check(self.lib.lst_run(self.h, slot, _stream(stream)), "lst_run")
+
+    def run_batch(self, first_slot: int, n_slots: int, stream=None):
+        return self._check(self.lib.lst_run_batch(self.h, first_slot, n_slots, _stream(stream)), "lst_run_batch")
+
+    def run_stage(self, first_slot: int, n_slots: int, stage: int, stream=None):
+        return self._check(self.lib.lst_run_stage(self.h, first_slot, n_slots, stage, _stream(stream)), "lst_run_stage")
+
+    def sync(self, slot: int, stream=None, check: bool = True) -> int:
+        st = self.lib.lst_sync(self.h, slot, _stream(stream))
+        if check:
+            self._check(st, "lst_sync")
+        return st
+
+    # ---- results ----------------------------------------------------------------------------
+    def stats(self, slot: int) -> dict:
+        s = Stats()
+        self._check(self.lib.lst_get_stats(self.h, slot, C.byref(s)), "lst_get_stats")
+        return dict(n_hits=int(s.n_hits), needed=[int(v) for v in s.needed], candidates=[int(v) for v in s.candidates],
+                    overflow=int(s.overflow), bad_hits=int(s.bad_hits), stage_ms=[float(v) for v in s.stage_ms])
+
+    def mds(self, slot: int) -> dict:
+        v = MdView()
+        self._check(self.lib.lst_get_mds(self.h, slot, C.byref(v)), "lst_get_mds")
+        n = v.n
+        return dict(n=n, hits=DeviceArray(v.hits, (n, 2), "<i4", self), module=DeviceArray(v.module, (n,), "<i4", self),
+                    anchor=DeviceArray(v.anchor, (n, 4), "<f4", self), ur_sina=DeviceArray(v.ur_sina, (n, 2), "<f4", self),
+                    dphi_dphichange=DeviceArray(v.dphi_dphichange, (n, 2), "<f4", self),
+                    module_start=DeviceArray(v.module_start, (self.n_modules + 1,), "<i4", self))
+
+    def segments(self, slot: int) -> dict:
+        v = SegView()
+        self._check(self.lib.lst_get_segments(self.h, slot, C.byref(v)), "lst_get_segments")
+        n_md = self.stats(slot)["needed"][MD]
+        return dict(n=v.n, md=DeviceArray(v.md, (v.n, 2), "<i4", self), f=DeviceArray(v.f, (v.n, 4), "<f4", self),
+                    md_start=DeviceArray(v.md_start, (n_md + 1,), "<i4", self))
+
+    def triplets(self, slot: int) -> dict:
+        v = T3View()
+        self._check(self.lib.lst_get_triplets(self.h, slot, C.byref(v)), "lst_get_triplets")
+        n_seg = self.stats(slot)["needed"][SEG]
+        return dict(n=v.n, md_kappa=DeviceArray(v.md_kappa, (v.n, 4), "<i4", self), seg=DeviceArray(v.seg, (v.n, 2), "<i4", self),
+                    chi2rz=DeviceArray(v.chi2rz, (v.n,), "<f4", self), seg_start=DeviceArray(v.seg_start, (n_seg + 1,), "<i4", self))
+
+    def quintuplets(self, slot: int) -> dict:
+        v = T5View()
+        self._check(self.lib.lst_get_quintuplets(self.h, slot, C.byref(v)), "lst_get_quintuplets")
+        n_t3 = self.stats(slot)["needed"][T3]
+        return dict(n=v.n, md=DeviceArray(v.md, (v.n, 5), "<i4", self), t3=DeviceArray(v.t3, (v.n, 2), "<i4", self),
+                    f=DeviceArray(v.f, (v.n, 5), "<f4", self), t3_start=DeviceArray(v.t3_start, (n_t3 + 1,), "<i4", self))
+
+    def fetch_hit_indices(self, slot: int, kind: int, stream=None, out=None) -> np.ndarray:
+        """[n][2|4|6|10] original hit indices of every object of class ``kind`` (host numpy)."""
+        n = self.stats(slot)["needed"][kind]
+        w = HITS_PER_OBJECT[kind]
+        if out is None:
+            out = np.empty((n, w), np.int32)
+        self._check(self.lib.lst_fetch_hit_indices(self.h, slot, kind, _ptr(out), out.shape[0], _stream(stream)),
+                    "lst_fetch_hit_indices")
+        return out[:n]
+
+    def fetch_values(self, slot: int, kind: int, stream=None, out=None) -> np.ndarray:
+        n = self.stats(slot)["needed"][kind]
+        w = VALUES_PER_OBJECT[kind]
+        if out is None:
+            out = np.empty((n, w), np.float32)
+        self._check(self.lib.lst_fetch_values(self.h, slot, kind, _ptr(out), out.shape[0], _stream(stream)),
+                    "lst_fetch_values")
+        return out[:n]
+
+    def arena_bytes(self):
+        t, p = C.c_int64(), C.c_int64()
+        self._check(self.lib.lst_arena_bytes(self.h, C.byref(t), C.byref(p)), "lst_arena_bytes")
+        return int(t.value), int(p.value)
+
+    def launch_count(self) -> int:
+        return int(self.lib.lst_launch_count(self.h))
+
+    def last_cuda_error(self) -> int:
+        return int(self.lib.lst_last_cuda_error(self.h))

@@ -3,7 +3,7 @@
 This module produces INPUTS only (BASELINE.json ``configs[0..4]``; recipe in DESIGN.md
 section "Input recipe", formulas from SURVEY.md Appendix A).  It holds none of the
 method's arithmetic (no mini-doublet / segment / triplet / quintuplet selection): the
-oracle (``oracle/``) and the CUDA path (``csrc/``) both receive what is generated here as
+CPU oracle and the CUDA path (``csrc/``) both receive what is generated here as
 plain arrays, and neither of them is imported from here.
 
 The paper measures on CMS tt-bar + PU200 simulation, which is not

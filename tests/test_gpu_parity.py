@@ -1,0 +1,204 @@
+"""GPU parity: the CUDA path, called through the C-ABI binding, against the CPU oracle on the same
+seeded inputs.  Object sets must be IDENTICAL (tuples of original hit indices, BASELINE.json
+north_star); float payloads within 1e-5 relative (reading 20); candidate counts equal.
+"""
+import numpy as np
+import pytest
+
+from paper_2207_08207_b200 import synth
+
+import parity
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def lstmod():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2207_08207_b200 import lst
+    lst.load_library()          # raises if liblst.so is missing: no fallback
+    return lst
+
+
+@pytest.fixture(scope="module")
+def ctx(lstmod, geom, mmap):
+    cfg = lstmod.default_config()
+    cfg.n_slots = 8
+    c = lstmod.Lst.from_synth(geom, mmap, cfg)
+    yield c
+    c.close()
+
+
+def check_event(ctx, o32, run_oracle, ev, slot=0, label=""):
+    gpu = parity.run_gpu(ctx, ev, slot)
+    ora = run_oracle(o32, ev)
+    worst = parity.compare(gpu, parity.oracle_tables(ora), label)
+    st = ctx.stats(slot)
+    assert st["needed"] == ora.counts, (label, st, ora.counts)
+    assert st["candidates"] == ora.candidates, (label, st, ora.candidates)
+    assert st["n_hits"] == ev.n and st["overflow"] == 0 and st["bad_hits"] == 0
+    return worst, st
+
+
+@pytest.mark.parametrize("config,seed", [(0, 0), (0, 1), (1, 0), (1, 17), (3, 0)])
+def test_parity_baseline_configs(ctx, o32, run_oracle, geom, config, seed):
+    """BASELINE.json configs[0] (tiny), configs[1] (PU200-like, the bench workload's event) and
+    configs[3] (PU300-like stress): full-size events, every object compared."""
+    ev = synth.generate_event(geom, config, seed)
+    worst, st = check_event(ctx, o32, run_oracle, ev, label=f"C{config}/seed{seed}")
+    assert st["needed"][3] > (50 if config == 0 else 5000)
+    print(f"C{config} seed {seed}: hits {ev.n} objects {st['needed']} candidates {st['candidates']} max rel err {worst}")
+
+
+@pytest.mark.parametrize("n_particles", [1, 3, 40, 700])
+def test_parity_ragged_sizes(ctx, o32, run_oracle, geom, n_particles):
+    ev = synth.generate_event(geom, 1, 100 + n_particles, n_particles=n_particles)
+    check_event(ctx, o32, run_oracle, ev, label=f"P{n_particles}")
+
+
+def test_parity_occupancy_sweep(ctx, o32, run_oracle, geom):
+    """BASELINE.json configs[4]: occupancy events at 1 k, 10 k, 100 k hits (MD + LS dominated)."""
+    for n in (1000, 10000, 100000):
+        ev = synth.generate_occupancy_event(geom, n, seed=4)
+        check_event(ctx, o32, run_oracle, ev, label=f"occ{n}")
+
+
+def test_degenerate_events(ctx, lstmod, o32, run_oracle, geom):
+    # empty event
+    e = synth.Event(*(np.zeros(0, t) for t in (np.float32, np.float32, np.float32, np.int32, np.uint8, np.int32)), {})
+    check_event(ctx, o32, run_oracle, e, label="empty")
+    # one hit; two hits on one side only; a module with lower hits only
+    ev = synth.generate_event(geom, 0, 0)
+    for sel in (slice(0, 1), np.nonzero(ev.side == 0)[0], np.nonzero(ev.side == 1)[0]):
+        sub = synth.Event(ev.x[sel], ev.y[sel], ev.z[sel], ev.module[sel], ev.side[sel], ev.truth[sel], {})
+        _, st = check_event(ctx, o32, run_oracle, sub, label="one-sided")
+        assert st["needed"] == [0, 0, 0, 0]
+    # all hits identical (zero-length vectors everywhere): nothing passes, nothing crashes
+    n = 64
+    same = synth.Event(np.full(n, 23.0, np.float32), np.zeros(n, np.float32), np.zeros(n, np.float32),
+                       np.zeros(n, np.int32), (np.arange(n) % 2).astype(np.uint8), np.zeros(n, np.int32), {})
+    _, st = check_event(ctx, o32, run_oracle, same, label="identical")
+    assert st["candidates"][0] == 32 * 32 and st["needed"][0] == 0
+    # non-finite coordinates reject (NaN never passes a '<=' cut)
+    bad = synth.generate_event(geom, 0, 2)
+    bad.x[::7] = np.nan
+    bad.z[::11] = np.inf
+    check_event(ctx, o32, run_oracle, bad, label="nonfinite")
+
+
+def test_one_heavy_module(ctx, o32, run_oracle, geom):
+    """Maximum-occupancy degenerate case: hundreds of hits in ONE module and its neighbours
+    (several warp iterations per module, ragged tails, long CSR rows)."""
+    rng = np.random.default_rng(9)
+    ev = synth.generate_event(geom, 1, 9, n_particles=2500)
+    phi0 = geom.phi[200]
+    d = np.abs(np.angle(np.exp(1j * (ev.particles["phi0"] - phi0))))
+    # keep every hit; add 400 extra noise hits on module 200 and 300 on a connected module
+    extra_mod = np.concatenate([np.full(400, 200), np.full(300, 200 + 408 + 12)]).astype(np.int32)
+    lay = geom.layer[extra_mod].astype(int)
+    side = rng.integers(0, 2, len(extra_mod)).astype(np.uint8)
+    rho = np.asarray(synth.LAYER_R)[lay] + (side - 0.5) * np.asarray(synth.SENSOR_GAP)[lay]
+    u = rng.uniform(-4.8, 4.8, len(extra_mod))
+    Phi = geom.phi[extra_mod]
+    x = (rho * np.cos(Phi) - u * np.sin(Phi)).astype(np.float32)
+    y = (rho * np.sin(Phi) + u * np.cos(Phi)).astype(np.float32)
+    z = (-120 + 10 * (geom.ring[extra_mod] + rng.uniform(0, 1, len(extra_mod)))).astype(np.float32)
+    big = synth.Event(np.concatenate([ev.x, x]), np.concatenate([ev.y, y]), np.concatenate([ev.z, z]),
+                      np.concatenate([ev.module, extra_mod]), np.concatenate([ev.side, side]),
+                      np.concatenate([ev.truth, np.full(len(x), -1, np.int32)]), ev.particles)
+    assert d.size
+    _, st = check_event(ctx, o32, run_oracle, big, label="heavy")
+    assert st["candidates"][0] > 40000
+
+
+def test_device_input_batch_and_determinism(ctx, lstmod, o32, run_oracle, geom):
+    """(i) device-resident input == host input; (ii) lst_run_batch over 4 slots == 4 single runs ==
+    oracle; (iii) two runs of the same event give bit-identical object arrays in the same order."""
+    import torch
+    evs = [synth.generate_event(geom, 1, 30 + i, n_particles=1500 + 500 * i) for i in range(4)]
+    stream = torch.cuda.Stream()
+    dev = []
+    for s, ev in enumerate(evs):
+        t = [torch.from_numpy(a).cuda() for a in (ev.x, ev.y, ev.z, ev.module, ev.side)]
+        dev.append(t)
+        ctx.load_event(s, *t, stream=stream)
+    ctx.run_batch(0, 4, stream)
+    for s, ev in enumerate(evs):
+        ctx.sync(s, stream)
+        got = parity.gpu_tables(ctx, s, stream)
+        ora = run_oracle(o32, ev)
+        parity.compare(got, parity.oracle_tables(ora), f"batch slot {s}")
+        assert ctx.stats(s)["needed"] == ora.counts
+    # determinism: slot 5 single run, host input, compare raw (unsorted) arrays with slot 1
+    ref = parity.gpu_tables(ctx, 1, stream)
+    again = parity.run_gpu(ctx, evs[1], slot=5)
+    for k in range(4):
+        assert np.array_equal(ref[k][0], again[k][0]) and np.array_equal(ref[k][1], again[k][1], equal_nan=True)
+    # views: CSR offsets are consistent with the object arrays
+    md = ctx.mds(5); seg = ctx.segments(5); t3 = ctx.triplets(5); t5 = ctx.quintuplets(5)
+    seg_md = seg["md"].torch().cpu().numpy(); start = seg["md_start"].torch().cpu().numpy()
+    assert start[0] == 0 and start[-1] == seg["n"] and np.all(np.diff(start) >= 0)
+    assert np.array_equal(np.repeat(np.arange(md["n"]), np.diff(start)), seg_md[:, 0])
+    t3s = t3["seg_start"].torch().cpu().numpy()
+    assert t3s[-1] == t3["n"] and np.array_equal(np.repeat(np.arange(seg["n"]), np.diff(t3s)), t3["seg"].torch().cpu().numpy()[:, 0])
+    t5s = t5["t3_start"].torch().cpu().numpy()
+    assert t5s[-1] == t5["n"] and np.array_equal(np.repeat(np.arange(t3["n"]), np.diff(t5s)), t5["t3"].torch().cpu().numpy()[:, 0])
+    ms = md["module_start"].torch().cpu().numpy()
+    assert np.array_equal(np.repeat(np.arange(geom.n_modules), np.diff(ms)), md["module"].torch().cpu().numpy())
+
+
+def test_overflow_and_bad_input_are_reported(lstmod, geom, mmap, o32, run_oracle):
+    """BASELINE.json configs[3]: candidate-buffer overflow handling — an error status, the sizes
+    that were needed, never a truncated success; and invalid module ids / sides are dropped
+    and reported."""
+    ev = synth.generate_event(geom, 1, 3, n_particles=2000)
+    ora = run_oracle(o32, ev)
+    for kind, field in enumerate(("cap_md", "cap_seg", "cap_t3", "cap_t5")):
+        cfg = lstmod.default_config()
+        cfg.n_slots = 1
+        setattr(cfg, field, max(1, ora.counts[kind] // 2))
+        c = lstmod.Lst.from_synth(geom, mmap, cfg)
+        c.load_event(0, ev.x, ev.y, ev.z, ev.module, ev.side)
+        c.run(0)
+        assert c.sync(0, check=False) == lstmod.ERR_OVERFLOW
+        st = c.stats(0)
+        assert st["overflow"] & (1 << kind) and st["needed"][kind] == ora.counts[kind]
+        with pytest.raises(lstmod.LstError):
+            c.quintuplets(0)
+        c.close()
+    cfg = lstmod.default_config()
+    cfg.n_slots = 1
+    cfg.cap_hits = 100
+    c = lstmod.Lst.from_synth(geom, mmap, cfg)
+    with pytest.raises(lstmod.LstError) as e:
+        c.load_event(0, ev.x, ev.y, ev.z, ev.module, ev.side)
+    assert e.value.status == lstmod.ERR_OVERFLOW
+    c.close()
+    # bad module ids / sides: dropped, counted, status LST_ERR_ARG; the rest is processed
+    c = lstmod.Lst.from_synth(geom, mmap)
+    mod = ev.module.copy(); side = ev.side.copy()
+    mod[:5] = geom.n_modules + 3; mod[5:8] = -1; side[8:10] = 2
+    c.load_event(0, ev.x, ev.y, ev.z, mod, side)
+    c.run(0)
+    assert c.sync(0, check=False) == lstmod.ERR_ARG
+    assert c.stats(0)["bad_hits"] == 10 and c.stats(0)["n_hits"] == ev.n - 10
+    with pytest.raises(lstmod.LstError):
+        c.run(1)                                     # slot never loaded -> LST_ERR_STATE
+    c.close()
+
+
+def test_multi_stream_pipeline(ctx, o32, run_oracle, geom):
+    """BASELINE.json configs[2] in miniature: 8 events on 4 streams, slots recycled, arena reused."""
+    import torch
+    streams = [torch.cuda.Stream() for _ in range(4)]
+    evs = [synth.generate_event(geom, 1, 60 + i, n_particles=800) for i in range(8)]
+    for rnd in range(2):
+        for s in range(4):
+            ev = evs[4 * rnd + s]
+            ctx.load_event(s, ev.x, ev.y, ev.z, ev.module, ev.side, streams[s])
+            ctx.run(s, streams[s])
+        for s in range(4):
+            ctx.sync(s, streams[s])
+            got = parity.gpu_tables(ctx, s, streams[s])
+            parity.compare(got, parity.oracle_tables(run_oracle(o32, evs[4 * rnd + s])), f"stream {s} round {rnd}")
