@@ -1,0 +1,375 @@
+#!/usr/bin/env python
+"""bench.py -- events/s of the LST hot path on B200 (BASELINE.json metric), with roofline and
+CPU-oracle baseline.  One JSON line on stdout (rank 0).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+Workload (config.workload): BASELINE.json configs[2] = 64 independent PU200-like events
+(configs[1] recipe, seeds 0..63), pipelined on 4 CUDA streams, 16-event batched launches, the
+arena allocated once.  A "step" is one pass of the WHOLE hot path (a0 bin/sort, a1 MD, a2 LS,
+a3 T3, a4 T5) over these 64 events.  `value` = events/s with the hit SoA already resident in
+HBM; `e2e` = the same through the C-ABI with HOST (pinned) buffers: H2D of the hits and D2H of
+the quintuplets inside the timed region.  N > 1: independent replicas (events are independent,
+PAPER.md:147), one process per GPU, no data-path collective.
+
+--impl reference times the CPU oracle (the tier's reference arm) on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "events/sec at PU200-like density (1 B200)"
+UNIT = "events/s"
+N_EVENTS = 64
+N_STREAMS = 4
+# SURVEY.md 8(d) algorithmic bytes per unit (each input read once, each output written once)
+MAP_BYTES = 4 * (69630 + 6121)
+# SPEC operations per candidate (every sqrt and div counted as one)
+FLOPS_PER_CAND = (34, 51, 45, 255)
+
+
+def algorithmic_bytes(stage: int, n_hits, needed):
+    md, ls, t3, t5 = needed
+    return (37 * n_hits,
+            16 * n_hits + 40 * md,
+            24 * md + MAP_BYTES + 24 * ls,
+            8 * ls + 16 * md + 16 * t3,
+            12 * t3 + 16 * md + 28 * t5)[stage]
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+            self.t = threading.Thread(target=lambda: self.lines.extend(self.proc.stdout), daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def stop(self) -> dict:
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for ln in self.lines:
+            f = [v.strip() for v in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for name, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def make_events(seed0: int, n: int):
+    from paper_2207_08207_b200 import synth
+    geom = synth.make_geometry()
+    mmap = synth.make_module_map(geom)
+    return geom, mmap, [synth.generate_event(geom, 1, seed0 + i) for i in range(n)]
+
+
+# ------------------------------------------------------------------------------------------
+# reference arm: the CPU oracle, as it stands, on a bounded sample
+# ------------------------------------------------------------------------------------------
+def oracle_events_per_s(geom, mmap, events):
+    from oracle import oracle
+    o = oracle.load("f32")
+    t0 = time.perf_counter()
+    for ev in events:
+        o.run(geom.layer, mmap.row_offsets, mmap.targets, ev.x, ev.y, ev.z, ev.module, ev.side)
+    dt = time.perf_counter() - t0
+    return len(events) / dt, dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    per_step = 4                                     # bounded sample: 4 of the 64 events per step
+    geom, mmap, events = make_events(0, per_step)
+    for _ in range(args.warmup):
+        oracle_events_per_s(geom, mmap, events[:1])
+    tot = 0.0
+    for _ in range(args.steps):
+        tot += oracle_events_per_s(geom, mmap, events)[1]
+    value = per_step * args.steps / tot
+    cpu = {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
+           "sample": f"{per_step} events (seeds 0..{per_step - 1}) of the 64-event workload per step, single thread"}
+    print(json.dumps({"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+                      "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps,
+                      "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+                      "data": "synthetic", "config": workload_config(), "cpu_baseline": cpu,
+                      "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                      "gpu_launches": 0}))
+
+
+def workload_config():
+    return {"workload": "BASELINE.json configs[2]: 64 PU200-like events (configs[1] recipe, seeds 0..63), "
+                        "4 CUDA streams x 16-event batched launches, arena reused",
+            "events_per_step": N_EVENTS, "streams": N_STREAMS, "geometry": "6-layer barrel, 6120 pT modules",
+            "l2": "explicit L2 flush (256 MiB memset) between timed steps, outside the timed intervals"}
+
+
+# ------------------------------------------------------------------------------------------
+# our arm
+# ------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    from paper_2207_08207_b200 import lst
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+
+    geom, mmap, events = make_events(rank * N_EVENTS, N_EVENTS)
+    per_stream = N_EVENTS // N_STREAMS
+    cfg = lst.default_config()
+    cfg.device, cfg.n_slots = local, N_EVENTS
+    ctx = lst.Lst.from_synth(geom, mmap, cfg)
+    streams = [torch.cuda.Stream(dev) for _ in range(N_STREAMS)]
+    main = torch.cuda.current_stream(dev)
+    d_in = [[torch.from_numpy(a).to(dev) for a in (e.x, e.y, e.z, e.module, e.side)] for e in events]
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    torch.cuda.synchronize(dev)
+
+    def step_device():
+        for s, st in enumerate(streams):
+            for k in range(s * per_stream, (s + 1) * per_stream):
+                ctx.load_event(k, *d_in[k], stream=st)
+            ctx.run_batch(s * per_stream, per_stream, st)
+
+    def timed(step_fn, n_steps):
+        """n_steps steps, each bracketed by CUDA events on the launching streams, L2 flushed between."""
+        e0 = [torch.cuda.Event(enable_timing=True) for _ in range(n_steps)]
+        e1 = [torch.cuda.Event(enable_timing=True) for _ in range(n_steps)]
+        done = [torch.cuda.Event() for _ in streams]
+        for i in range(n_steps):
+            flush.zero_()
+            e0[i].record(main)
+            for st in streams:
+                st.wait_event(e0[i])
+            step_fn()
+            for st, d in zip(streams, done):
+                d.record(st)
+                main.wait_event(d)
+            e1[i].record(main)
+        torch.cuda.synchronize(dev)
+        return [a.elapsed_time(b) for a, b in zip(e0, e1)]
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if dist:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # warm-up, then check every slot finished without overflow / bad input
+    timed(step_device, max(3, args.warmup))
+    stats = []
+    for k in range(N_EVENTS):
+        ctx.sync(k, streams[k // per_stream])
+        stats.append(ctx.stats(k))
+    n_hits = sum(s["n_hits"] for s in stats)
+    needed = [sum(s["needed"][j] for s in stats) for j in range(4)]
+    cands = [sum(s["candidates"][j] for s in stats) for j in range(4)]
+
+    # ---- the timed region ---------------------------------------------------------------
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    l0 = ctx.launch_count()
+    w0 = time.perf_counter()
+    ms = timed(step_device, args.steps)
+    barrier()
+    wall = time.perf_counter() - w0
+    launches = ctx.launch_count() - l0
+    clocks = sampler.stop()
+    total_ms = sum(ms)
+    if dist:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    value = world * N_EVENTS * args.steps / (total_ms * 1e-3)
+
+    # ---- end to end: pinned host hits in, quintuplets out, through the C-ABI -------------
+    h_in = [[torch.from_numpy(a).pin_memory() for a in (e.x, e.y, e.z, e.module, e.side)] for e in events]
+    cap5 = max(s["needed"][3] for s in stats) * 2 + 1024
+    h_out = [(torch.empty((cap5, 10), dtype=torch.int32).pin_memory(), torch.empty((cap5, 5), dtype=torch.float32).pin_memory())
+             for _ in range(N_EVENTS)]
+    np_in = [[t.numpy() for t in ev] for ev in h_in]
+    np_out = [(a.numpy(), b.numpy()) for a, b in h_out]
+
+    def step_e2e():
+        for s, st in enumerate(streams):
+            for k in range(s * per_stream, (s + 1) * per_stream):
+                ctx.load_event(k, *np_in[k], stream=st)
+            ctx.run_batch(s * per_stream, per_stream, st)
+        for s, st in enumerate(streams):
+            for k in range(s * per_stream, (s + 1) * per_stream):
+                ctx.sync(k, st)
+                ctx.fetch_hit_indices(k, lst.T5, st, out=np_out[k][0])
+                ctx.fetch_values(k, lst.T5, st, out=np_out[k][1])
+
+    e2e_steps = max(3, min(args.steps, 10))
+    for _ in range(2):
+        step_e2e()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        step_e2e()
+    torch.cuda.synchronize(dev)
+    e2e_s = time.perf_counter() - t0
+    if dist:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    h2d = sum(sum(t.numel() * t.element_size() for t in ev) for ev in h_in)
+    d2h = needed[3] * (40 + 20) + N_EVENTS * 128
+    e2e = {"value": world * N_EVENTS * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+           "d2h_bytes_per_step": int(d2h), "steps": e2e_steps,
+           "how": "lst_load_event(host pinned SoA) + lst_run_batch + lst_sync + lst_fetch_{hit_indices,values}(T5) per event"}
+
+    # ---- per-kernel times (CUDA events inside the library, timing mode), one 64-event batch ----
+    kernel_ms = per_kernel_times(lst, geom, mmap, d_in, local)
+    peaks = measured_peaks()
+    roof, per_stage = roofline(kernel_ms, n_hits, needed, cands, peaks)
+
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
+           "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f32", "data": "synthetic", "config": workload_config(), "clocks": clocks, "e2e": e2e,
+           "gpu_launches": int(launches), "roofline": roof, "per_stage": per_stage,
+           "us_per_event": 1e3 * total_ms / (args.steps * N_EVENTS), "wall_s_timed_region": wall,
+           "objects_per_step": dict(hits=n_hits, md=needed[0], ls=needed[1], t3=needed[2], t5=needed[3]),
+           "candidates_per_step": dict(md=cands[0], ls=cands[1], t3=cands[2], t5=cands[3]),
+           "arena_mib": ctx.arena_bytes()[0] / 2 ** 20, "impl": "ours"}
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        v, dt = oracle_events_per_s(geom, mmap, events)
+        out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
+                               "sample": f"all {N_EVENTS} events of the workload once, single thread, {dt:.1f} s"}
+    ctx.close()
+    if rank == 0:
+        print(json.dumps(out))
+    if dist:
+        dist.destroy_process_group()
+
+
+def per_kernel_times(lst, geom, mmap, d_in, local, reps=5):
+    """Median per-kernel duration (ms) for ONE batch of all 64 events on one stream, from CUDA
+    events recorded by the library around every launch (lst_config.timing)."""
+    import torch
+    cfg = lst.default_config()
+    cfg.device, cfg.n_slots, cfg.timing = local, N_EVENTS, 1
+    ctx = lst.Lst.from_synth(geom, mmap, cfg)
+    st = torch.cuda.Stream()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    rows = []
+    for _ in range(reps + 2):
+        with torch.cuda.stream(st):
+            flush.zero_()
+        for k in range(N_EVENTS):
+            ctx.load_event(k, *d_in[k], stream=st)
+        ctx.run_batch(0, N_EVENTS, st)
+        ctx.sync(0, st)
+        k_ms = np.zeros(12)
+        for k in range(N_EVENTS):
+            ctx.sync(k, st)
+            k_ms[:4] += np.asarray(ctx.stats(k)["kernel_ms"][:4])
+        k_ms[4:] = np.asarray(ctx.stats(0)["kernel_ms"][4:])
+        rows.append(k_ms)
+    ctx.close()
+    return dict(zip(lst.KERNEL_NAMES, np.median(np.asarray(rows[2:]), axis=0).tolist()))
+
+
+def roofline(kernel_ms, n_hits, needed, cands, peaks):
+    """Per-stage table and the `roofline` object for the dominant kernel. Two lower bounds per stage:
+    HBM (algorithmic bytes / measured copy bandwidth) and ALU (SPEC flops of all candidates / fp32
+    non-FMA peak = 148 SMs x 128 lanes x sm_max clock; FMA is excluded by the SPEC's arithmetic)."""
+    alu_peak_tflops = 148 * 128 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    groups = (("a0_bin", ("bin_count", "bin_scan", "bin_scatter", "bin_order")), ("a1_md", ("md_count", "md_fill")),
+              ("a2_ls", ("seg_count", "seg_fill")), ("a3_t3", ("t3_count", "t3_fill")), ("a4_t5", ("t5_count", "t5_fill")))
+    per_stage = {}
+    for i, (name, ks) in enumerate(groups):
+        ms = sum(kernel_ms[k] for k in ks)
+        b = algorithmic_bytes(i, n_hits, needed)
+        fl = cands[i - 1] * FLOPS_PER_CAND[i - 1] if i else 0
+        per_stage[name] = {"ms": ms, "kernels_ms": {k: kernel_ms[k] for k in ks}, "algorithmic_bytes": int(b),
+                           "hbm_gbs": b / (ms * 1e-3) / 1e9 if ms else None,
+                           "hbm_frac": b / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"] if ms else None,
+                           "spec_flops": int(fl), "alu_tflops": fl / (ms * 1e-3) / 1e12 if ms else None,
+                           "alu_frac": fl / (ms * 1e-3) / 1e12 / alu_peak_tflops if ms else None}
+    top = max(kernel_ms, key=kernel_ms.get)
+    si = next(i for i, (_, ks) in enumerate(groups) if top in ks)
+    ms = kernel_ms[top]
+    b = algorithmic_bytes(si, n_hits, needed)
+    fl = cands[si - 1] * FLOPS_PER_CAND[si - 1] if si else 0
+    t_hbm, t_alu = b / (peaks["hbm_gbs"] * 1e9), fl / (alu_peak_tflops * 1e12)
+    if t_alu > t_hbm:
+        roof = {"bound": "alu", "achieved": fl / (ms * 1e-3) / 1e12, "peak": alu_peak_tflops, "unit": "TFLOP/s"}
+    else:
+        roof = {"bound": "hbm", "achieved": b / (ms * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s"}
+    roof.update({"frac": roof["achieved"] / roof["peak"], "traffic": None, "kernel": top, "kernel_ms": ms,
+                 "launch": f"one launch over all {N_EVENTS} events (grid.y = event)", "peak_source": peaks["source"],
+                 "hbm_view": {"achieved_gbs": b / (ms * 1e-3) / 1e9, "peak_gbs": peaks["hbm_gbs"],
+                              "frac": b / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"], "algorithmic_bytes": int(b)}})
+    return roof, per_stage
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -107,8 +107,8 @@ typedef struct {
   int32_t cap_seg;
   int32_t cap_t3;
   int32_t cap_t5;
-  int32_t timing;     /* != 0: record CUDA events around every stage (lst_get_stats.stage_ms);
-                         makes lst_run non-capturable */
+  int32_t timing;     /* != 0: record CUDA events around every kernel (lst_get_stats.stage_ms /
+                         kernel_ms; for a batch they are kept on its first slot) */
 } lst_config;
 
 /* Fills *cfg with the frozen SPEC constants, device 0, 4 slots and capacities that hold the
@@ -170,6 +170,7 @@ typedef struct {
   int32_t overflow;      /* bit k set: capacity of class k exceeded                              */
   int32_t bad_hits;      /* hits dropped because module id / side was out of range               */
   float stage_ms[5];     /* a0 .. a4; zeros unless lst_config.timing                              */
+  float kernel_ms[12];   /* bin count, scan, scatter, order; then count, fill of MD, LS, T3, T5   */
 } lst_stats;
 
 /* Validates geometry and map, uploads the per-module tables, allocates the arena (the only

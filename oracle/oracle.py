@@ -193,7 +193,7 @@ class OracleResult:
         return np.stack([self.md_lower, self.md_upper], 1).reshape(-1, 2)
 
     def _hits(self, mds):
-        return self.md_hits()[mds].reshape(len(mds), -1)
+        return self.md_hits()[mds].reshape(len(mds), 2 * mds.shape[1])
 
     def seg_hits(self):
         return self._hits(self.seg_mds())

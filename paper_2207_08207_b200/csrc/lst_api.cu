@@ -31,8 +31,8 @@ struct SlotHost {
   bool loaded = false, ran = false, synced = false;
   int n_hits_in = 0;
   SlotHeader* hdr = nullptr;  // pinned host copy of the device header
-  cudaEvent_t ev[7] = {};     // timing: before a0, after a0, before a1, after a1 .. after a4
-  bool ev_bin = false, ev_run = false;
+  cudaEvent_t ev[17] = {};    // timing mode: ev[0..4] around the 4 a0 kernels, ev[5 + 3 s .. 7 + 3 s] around stage s
+  bool ev_bin = false, ev_stage[4] = {false, false, false, false};
 };
 
 }  // namespace
@@ -257,7 +257,6 @@ int lst_load_event(lst_ctx* c, int slot, const lst_hits* h, void* stream) {
   sh.n_hits_in = h->n;
   const Layout& L = c->P.L;
   char* base = c->arena + (size_t)slot * c->P.slot_stride;
-  if (c->cfg.timing) { LST_CUDA(c, cudaEventRecord(sh.ev[0], s)); }
   LST_CUDA(c, cudaMemsetAsync(base + L.hdr, 0, L.reset_bytes, s));
   HitInput in{h->x, h->y, h->z, h->module, h->side, h->n};
   if (!h->on_device && h->n > 0) {
@@ -275,9 +274,10 @@ int lst_load_event(lst_ctx* c, int slot, const lst_hits* h, void* stream) {
   }
   Params P = c->P;
   P.first_slot = slot;
-  c->launches += launch_bin(P, in, s);
+  c->launches += launch_bin(P, in, s, c->cfg.timing ? sh.ev : nullptr);
   LST_CUDA(c, cudaGetLastError());
-  if (c->cfg.timing) { LST_CUDA(c, cudaEventRecord(sh.ev[1], s)); sh.ev_bin = true; }
+  sh.ev_bin = c->cfg.timing != 0;
+  for (bool& b : sh.ev_stage) b = false;
   sh.loaded = true;
   return LST_OK;
 }
@@ -289,12 +289,11 @@ int lst_run_stage(lst_ctx* c, int first, int n, int stage, void* stream) {
   cudaStream_t st = (cudaStream_t)stream;
   LST_CUDA(c, cudaSetDevice(c->device));
   SlotHost& sh = c->slots[first];
-  if (c->cfg.timing && stage == LST_MD) { LST_CUDA(c, cudaEventRecord(sh.ev[2], st)); }
   Params P = c->P;
   P.first_slot = first;
-  c->launches += launch_stage(P, n, stage, st);
+  c->launches += launch_stage(P, n, stage, st, c->cfg.timing ? sh.ev + 5 + 3 * stage : nullptr);
   LST_CUDA(c, cudaGetLastError());
-  if (c->cfg.timing) { LST_CUDA(c, cudaEventRecord(sh.ev[3 + stage], st)); if (stage == LST_T5) sh.ev_run = true; }
+  if (c->cfg.timing) sh.ev_stage[stage] = true;
   for (int s = first; s < first + n; ++s) { c->slots[s].synced = false; if (stage == LST_T5) c->slots[s].ran = true; }
   return LST_OK;
 }
@@ -395,9 +394,17 @@ int lst_get_stats(lst_ctx* c, int slot, lst_stats* o) {
   o->overflow = sh.hdr->overflow;
   o->bad_hits = sh.hdr->bad_hits;
   if (c->cfg.timing) {
-    if (sh.ev_bin) cudaEventElapsedTime(&o->stage_ms[0], sh.ev[0], sh.ev[1]);
-    if (sh.ev_run)
-      for (int k = 0; k < 4; ++k) cudaEventElapsedTime(&o->stage_ms[1 + k], sh.ev[2 + k], sh.ev[3 + k]);
+    if (sh.ev_bin) {
+      cudaEventElapsedTime(&o->stage_ms[0], sh.ev[0], sh.ev[4]);
+      for (int k = 0; k < 4; ++k) cudaEventElapsedTime(&o->kernel_ms[k], sh.ev[k], sh.ev[k + 1]);
+    }
+    for (int st = 0; st < 4; ++st)
+      if (sh.ev_stage[st]) {
+        cudaEvent_t* e = sh.ev + 5 + 3 * st;
+        cudaEventElapsedTime(&o->stage_ms[1 + st], e[0], e[2]);
+        cudaEventElapsedTime(&o->kernel_ms[4 + 2 * st], e[0], e[1]);
+        cudaEventElapsedTime(&o->kernel_ms[5 + 2 * st], e[1], e[2]);
+      }
     cudaGetLastError();
   }
   return LST_OK;

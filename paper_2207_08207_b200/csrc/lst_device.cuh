@@ -123,8 +123,8 @@ struct HitInput {
 };
 
 // Host-callable launchers (lst_kernels.cu). Each returns the number of kernels it launched.
-int launch_bin(const Params& P, const HitInput& in, cudaStream_t s);
-int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s);
+int launch_bin(const Params& P, const HitInput& in, cudaStream_t s, cudaEvent_t* ev);
+int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEvent_t* ev);
 int launch_gather_hits(const Params& P, int kind, int n, cudaStream_t s);
 int launch_pack_values(const Params& P, int kind, int n, cudaStream_t s);
 

@@ -485,50 +485,63 @@ __global__ void __launch_bounds__(256) k_pack_values(const __grid_constant__ Par
 // ------------------------------------------------------------------------------------------
 // launchers
 // ------------------------------------------------------------------------------------------
-int launch_bin(const Params& P, const HitInput& in, cudaStream_t s) {
+// `ev` (optional, timing mode): ev[0] is recorded before the first kernel, ev[k + 1] after kernel k.
+#define LST_EV(k) do { if (ev) cudaEventRecord(ev[k], s); } while (0)
+
+int launch_bin(const Params& P, const HitInput& in, cudaStream_t s, cudaEvent_t* ev) {
   const int nb = in.n > 0 ? min((in.n + 255) / 256, 1184) : 0;
   int launches = 0;
+  LST_EV(0);
   if (nb) { k_bin_count<<<nb, 256, 0, s>>>(P, in); ++launches; }
+  LST_EV(1);
   k_bin_scan<<<1, 1024, 0, s>>>(P); ++launches;
-  if (nb) {
-    k_bin_scatter<<<nb, 256, 0, s>>>(P, in);
-    k_bin_order<<<(P.L.n_bins + 7) / 8, 256, 0, s>>>(P, in);
-    launches += 2;
-  }
+  LST_EV(2);
+  if (nb) { k_bin_scatter<<<nb, 256, 0, s>>>(P, in); ++launches; }
+  LST_EV(3);
+  if (nb) { k_bin_order<<<(P.L.n_bins + 7) / 8, 256, 0, s>>>(P, in); ++launches; }
+  LST_EV(4);
   return launches;
 }
 
-int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s) {
+int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEvent_t* ev) {
   const unsigned nb = (unsigned)n_batch;
   // persistent chunk loops of T3 / T5: enough blocks to fill the machine across the batch
   const int per_event = max(8, 1184 / n_batch);
+  LST_EV(0);
   switch (stage) {
     case LST_MD_: {
       dim3 g((P.L.n_modules + kMdWarps - 1) / kMdWarps, nb);
       k_md<false><<<g, kMdWarps * 32, 0, s>>>(P);
+      LST_EV(1);
       k_md<true><<<g, kMdWarps * 32, 0, s>>>(P);
-      return 2;
+      break;
     }
     case LST_SEG_: {
       dim3 g(P.L.n_modules, nb);
       k_seg<false><<<g, kSegThreads, 0, s>>>(P);
+      LST_EV(1);
       k_seg<true><<<g, kSegThreads, 0, s>>>(P);
-      return 2;
+      break;
     }
     case LST_T3_: {
       dim3 g(min(per_event, P.L.n_chunk_seg), nb);
       k_t3<false><<<g, kScanChunk, 0, s>>>(P);
+      LST_EV(1);
       k_t3<true><<<g, kScanChunk, 0, s>>>(P);
-      return 2;
+      break;
     }
     case LST_T5_: {
       dim3 g(min(per_event, P.L.n_chunk_t3), nb);
       k_t5<false><<<g, kScanChunk, 0, s>>>(P);
+      LST_EV(1);
       k_t5<true><<<g, kScanChunk, 0, s>>>(P);
-      return 2;
+      break;
     }
+    default:
+      return 0;
   }
-  return 0;
+  LST_EV(2);
+  return 2;
 }
 
 int launch_gather_hits(const Params& P, int kind, int n, cudaStream_t s) {

@@ -20,6 +20,8 @@ LIB_PATH = os.path.join(HERE, "liblst.so")
 N_LAYERS = 6
 MD, SEG, T3, T5 = 0, 1, 2, 3
 KIND_NAMES = ("md", "seg", "t3", "t5")
+KERNEL_NAMES = ("bin_count", "bin_scan", "bin_scatter", "bin_order", "md_count", "md_fill", "seg_count", "seg_fill",
+                "t3_count", "t3_fill", "t5_count", "t5_fill")
 HITS_PER_OBJECT = (2, 4, 6, 10)
 VALUES_PER_OBJECT = (4, 4, 2, 5)
 
@@ -89,7 +91,7 @@ class T5View(C.Structure):
 
 class Stats(C.Structure):
     _fields_ = [("n_hits", C.c_int32), ("needed", C.c_int64 * 4), ("candidates", C.c_int64 * 4),
-                ("overflow", C.c_int32), ("bad_hits", C.c_int32), ("stage_ms", C.c_float * 5)]
+                ("overflow", C.c_int32), ("bad_hits", C.c_int32), ("stage_ms", C.c_float * 5), ("kernel_ms", C.c_float * 12)]
 
 
 # every symbol include/lst.h declares: name -> (restype, argtypes)
@@ -262,7 +264,8 @@ class Lst:
         s = Stats()
         self._check(self.lib.lst_get_stats(self.h, slot, C.byref(s)), "lst_get_stats")
         return dict(n_hits=int(s.n_hits), needed=[int(v) for v in s.needed], candidates=[int(v) for v in s.candidates],
-                    overflow=int(s.overflow), bad_hits=int(s.bad_hits), stage_ms=[float(v) for v in s.stage_ms])
+                    overflow=int(s.overflow), bad_hits=int(s.bad_hits), stage_ms=[float(v) for v in s.stage_ms],
+                    kernel_ms=[float(v) for v in s.kernel_ms])
 
     def mds(self, slot: int) -> dict:
         v = MdView()
