@@ -5,14 +5,21 @@
 // kernel finds slot s at arena + s * slot_stride and needs no per-slot pointer table.  The
 // batch index (which slot of a batch) is blockIdx.y of every kernel.
 //
-// Object store (per slot), "SoA of small vectors": each object class keeps one array per
-// GROUP of fields that are always read together, packed to 8 or 16 bytes so one vector load
-// fetches the group (PAPER.md:139-141 argues for SoA on V100; on sm_100a the unit that matters
-// is the 16-B vector / 32-B sector):
-//   hits   hit4[i]    = (x, y, z, r)            float4   binned by (module, side)
-//          hit_orig[i]= original index          int
-//   MD     md_anchor  = (x, y, z, r) of anchor  float4
+// Hit store (per slot): hits are binned by (side, module) -- all lower-sensor hits first, in
+// module order, then all upper-sensor hits -- and ordered inside a bin by their azimuth
+// relative to the module normal (`key`), ties by original index.  Lower hit i of the event is
+// simply element i: the MD kernel is "one thread per lower hit".
+//   hit4[i]      = (x, y, z, r)            float4
+//   hit_key[i]   = azimuth - module azimuth float   (FLT_MAX for non-finite x / y)
+//   hit_orig[i]  = original index           int
+//   hit_module[i]                           int
+// Object store, "SoA of small vectors": each class keeps one array per GROUP of fields that
+// are always read together, packed to 8 or 16 bytes so one vector load fetches the group
+// (PAPER.md:139-141 argues for SoA on V100; on sm_100a the unit that matters is the 16-B
+// vector / 32-B sector):
+//   MD     md_anchor  = (x, y, z, r) of anchor  float4   ordered by (module, key of anchor hit)
 //          md_aux     = (r_upper, sinA)         float2
+//          md_key     = key of the anchor hit   float    (the segment search window runs on it)
 //          md_hits    = (orig lower, orig upper)int2
 //          md_out     = (dphi, dphichange)      float2
 //          md_module                            int
@@ -32,30 +39,37 @@
 
 namespace lst {
 
-constexpr int kScanChunk = 256;  // owners (segments / triplets) per block chunk in T3 / T5
+constexpr int kScanChunk = 256;   // owners (lower hits / segments / triplets) per block chunk
+constexpr int kMaxBatch = 16;     // events per launch of the a0 kernels (pointer table in the launch parameters)
+constexpr int kMaxRow = 64;       // longest module-map row the segment kernel stages
 enum { LST_MD_ = 0, LST_SEG_ = 1, LST_T3_ = 2, LST_T5_ = 3 };  // == LST_MD .. LST_T5 of lst.h
 
 struct SlotHeader {
   int n_hits;                     // valid hits binned
+  int n_lower;                    // of which on the lower sensor (= bin_start[n_modules])
   int n[4];                       // objects stored (clamped to capacity): MD, LS, T3, T5
   int overflow;                   // bit k: class k exceeded its capacity
   int bad_hits;                   // hits dropped (module id / side out of range)
-  int pad0;
   unsigned long long needed[4];   // objects that passed (unclamped)
-  unsigned long long cand[4];     // candidates examined
+  unsigned long long cand[4];     // candidates of the search space (map-restricted pairs)
+  unsigned long long eval[4];     // candidates the selection was evaluated on (after windowing)
+  // per side, per layer: range of r over the finite hits, as float bit patterns;
+  // r_min is stored as 0x7f800000 - bits so that the zeroed header means "+inf"
+  int r_min_inv[2][6];
+  int r_max[2][6];
   unsigned int done[8];           // "last block done" tickets, self-resetting
 };
 
 struct Layout {
   int n_modules, n_bins;
   int cap_hits, cap_md, cap_seg, cap_t3, cap_t5;
-  int n_chunk_seg, n_chunk_t3;    // ceil(cap / kScanChunk)
+  int n_chunk_hits, n_chunk_seg, n_chunk_t3;  // ceil(cap / kScanChunk)
   // byte offsets from the slot base (all multiples of 256)
   size_t hdr, bin_start, bin_cursor;          // hdr, bin_start and bin_cursor are contiguous: one memset
   size_t reset_bytes;                         // bytes to zero at lst_load_event, from hdr
   size_t in_x, in_y, in_z, in_module, in_side;// staging of host input
-  size_t tmp_idx, hit4, hit_orig;
-  size_t md_start, md_anchor, md_aux, md_hits, md_out, md_module;
+  size_t tmp_idx, tmp_key, hit4, hit_key, hit_orig, hit_module;
+  size_t md_off, md_block_base, md_start, md_anchor, md_aux, md_key, md_hits, md_out, md_module;
   size_t seg_start, seg_block_base, seg_md, seg_f;
   size_t t3_start, t3_block_base, t3_pack, t3_seg, t3_chi2;
   size_t t5_start, t5_block_base, t5_md, t5_t3, t5_f;
@@ -70,8 +84,10 @@ struct Params {
   Layout L;
   Cuts cuts;
   const signed char* mod_layer;  // [n_modules]
-  const int* run_offsets;        // [n_modules + 1] module map as runs of consecutive target modules
-  const int2* runs;              // [run_offsets[n_modules]] (first target, last target), ascending
+  const float2* mod_cs;          // [n_modules] (cos, sin) of the azimuth of the module normal
+  const int* map_offsets;        // [n_modules + 1] module map, CSR
+  const int* map_targets;        // [map_offsets[n_modules]] ascending per row
+  const float* map_dphi;         // [map_offsets[n_modules]] azimuth(source normal) - azimuth(target normal), in (-pi, pi]
   int first_slot;
 };
 
@@ -87,11 +103,17 @@ struct Slot {
   __device__ __forceinline__ unsigned* bin_start() const { return at<unsigned>(L.bin_start); }
   __device__ __forceinline__ unsigned* bin_cursor() const { return at<unsigned>(L.bin_cursor); }
   __device__ __forceinline__ int* tmp_idx() const { return at<int>(L.tmp_idx); }
+  __device__ __forceinline__ float* tmp_key() const { return at<float>(L.tmp_key); }
   __device__ __forceinline__ float4* hit4() const { return at<float4>(L.hit4); }
+  __device__ __forceinline__ float* hit_key() const { return at<float>(L.hit_key); }
   __device__ __forceinline__ int* hit_orig() const { return at<int>(L.hit_orig); }
+  __device__ __forceinline__ int* hit_module() const { return at<int>(L.hit_module); }
+  __device__ __forceinline__ int* md_off() const { return at<int>(L.md_off); }
+  __device__ __forceinline__ int* md_block_base() const { return at<int>(L.md_block_base); }
   __device__ __forceinline__ int* md_start() const { return at<int>(L.md_start); }
   __device__ __forceinline__ float4* md_anchor() const { return at<float4>(L.md_anchor); }
   __device__ __forceinline__ float2* md_aux() const { return at<float2>(L.md_aux); }
+  __device__ __forceinline__ float* md_key() const { return at<float>(L.md_key); }
   __device__ __forceinline__ int2* md_hits() const { return at<int2>(L.md_hits); }
   __device__ __forceinline__ float2* md_out() const { return at<float2>(L.md_out); }
   __device__ __forceinline__ int* md_module() const { return at<int>(L.md_module); }
@@ -121,9 +143,13 @@ struct HitInput {
   const unsigned char* side;
   int n;
 };
+// Inputs of a batch of events: slot first_slot + b reads ev[b].
+struct HitBatch {
+  HitInput ev[kMaxBatch];
+};
 
 // Host-callable launchers (lst_kernels.cu). Each returns the number of kernels it launched.
-int launch_bin(const Params& P, const HitInput& in, cudaStream_t s, cudaEvent_t* ev);
+int launch_bin(const Params& P, const HitBatch& in, int n_batch, cudaStream_t s, cudaEvent_t* ev);
 int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEvent_t* ev);
 int launch_gather_hits(const Params& P, int kind, int n, cudaStream_t s);
 int launch_pack_values(const Params& P, int kind, int n, cudaStream_t s);

@@ -155,7 +155,7 @@ class DeviceArray:
     def __init__(self, ptr: int, shape, typestr: str, owner):
         self._owner = owner
         self.shape = tuple(int(s) for s in shape)
-        self.__cuda_array_interface__ = {"shape": self.shape, "typestr": typestr, "data": (int(ptr or 0), True),
+        self.__cuda_array_interface__ = {"shape": self.shape, "typestr": typestr, "data": (int(ptr or 0), False),
                                          "version": 2, "strides": None}
 
     def torch(self):
