@@ -23,7 +23,8 @@
  *    host threads.  One slot must not be used from two streams at once.
  *  - Object identity is by ORIGINAL hit index = position in the caller's hit arrays
  *    (reading 16).  Within a slot objects are numbered deterministically:
- *    MDs by (module, lower hit, upper hit), segments by (inner MD, outer MD), triplets by
+ *    MDs by (module, azimuth of the lower hit, azimuth of the upper hit; ties by original hit
+ *    index), segments by (inner MD, outer MD), triplets by
  *    (first segment, second segment), quintuplets by (first triplet, second triplet).
  *  - Overflow of a per-slot capacity is never silent: lst_sync returns LST_ERR_OVERFLOW, the
  *    slot's outputs are invalid, lst_get_stats still reports the sizes that were needed.
@@ -38,6 +39,7 @@ extern "C" {
 #endif
 
 #define LST_N_LAYERS 6
+#define LST_MAX_ROW 64
 
 #if defined(__GNUC__)
 #define LST_API __attribute__((visibility("default")))
@@ -59,8 +61,11 @@ enum { LST_MD = 0, LST_SEG = 1, LST_T3 = 2, LST_T5 = 3 };
 typedef struct lst_ctx lst_ctx;
 
 /* Detector description. HOST pointers, copied by lst_create; the caller keeps ownership.
- * Only `layer` enters the computation (cut constants are per layer); the rest is validated
- * and kept for diagnostics.  PAPER.md:29 (pT modules), BASELINE.json configs[0]. */
+ * `layer` enters the computation (cut constants are per layer).  `phi` does not change any
+ * result: it is the reference direction against which the hits of a module are ordered in
+ * azimuth, so that the search for partners can be restricted to a window (DESIGN.md section
+ * 6); it must be finite.  The rest is optional and unused.
+ * PAPER.md:29 (pT modules), BASELINE.json configs[0]. */
 typedef struct {
   int32_t n_modules;
   const int8_t* layer;  /* [n_modules] 0 .. LST_N_LAYERS-1 */
@@ -68,11 +73,12 @@ typedef struct {
   const float* cx;      /* [n_modules] module centre (may be NULL) */
   const float* cy;
   const float* cz;
-  const float* phi;     /* [n_modules] azimuth of the module normal (may be NULL) */
+  const float* phi;     /* [n_modules] azimuth of the module normal, radians (required) */
 } lst_geometry;
 
 /* Module map: CSR lookup table module -> connectable modules of the next layer.
- * HOST pointers, copied by lst_create.  layer[targets[k]] must equal layer[src] + 1. */
+ * HOST pointers, copied by lst_create.  layer[targets[k]] must equal layer[src] + 1; a row
+ * is strictly ascending and holds at most LST_MAX_ROW targets. */
 typedef struct {
   int32_t n_modules;
   const int32_t* row_offsets; /* [n_modules + 1], non-decreasing, row_offsets[0] = 0 */
@@ -166,11 +172,16 @@ typedef struct {
 typedef struct {
   int32_t n_hits;
   int64_t needed[4];     /* objects that passed per class (may exceed the capacity on overflow) */
-  int64_t candidates[4]; /* candidate pairs examined per stage                                   */
+  int64_t candidates[4]; /* size of the search space per stage: pairs the method defines as
+                            candidates (hit pairs of a module; MD pairs on map-connected modules;
+                            segment pairs sharing an MD; triplet pairs sharing an MD)            */
+  int64_t evaluated[4];  /* pairs the selection was actually evaluated on (<= candidates: the MD
+                            and segment stages only look inside an azimuth window that is a
+                            superset of what the selection can accept)                           */
   int32_t overflow;      /* bit k set: capacity of class k exceeded                              */
   int32_t bad_hits;      /* hits dropped because module id / side was out of range               */
   float stage_ms[5];     /* a0 .. a4; zeros unless lst_config.timing                              */
-  float kernel_ms[12];   /* bin count, scan, scatter, order; then count, fill of MD, LS, T3, T5   */
+  float kernel_ms[12];   /* bin count+scan, (unused), scatter, order; then count, fill of MD, LS, T3, T5 */
 } lst_stats;
 
 /* Validates geometry and map, uploads the per-module tables, allocates the arena (the only
@@ -180,11 +191,14 @@ LST_API int lst_create(const lst_geometry* geom, const lst_module_map* map, cons
 LST_API int lst_destroy(lst_ctx* ctx);
 
 /* Step a0 ("a kernel that deals with pre-processing the hits and loading them"):
- * copies the hits to the device if they are on the host, bins them by (module, side), orders
- * each bin by original index and derives r.  Asynchronous on `cuda_stream`.  Hits with an
- * invalid module id or side are dropped and reported (lst_sync -> LST_ERR_ARG).
+ * copies the hits to the device if they are on the host, bins them by (side, module), orders
+ * each bin by azimuth (ties by original index) and derives r.  Asynchronous on `cuda_stream`.
+ * Hits with an invalid module id or side are dropped and reported (lst_sync -> LST_ERR_ARG).
+ * lst_load_events loads hits[b] into slot first_slot + b for b < n_slots with ONE set of
+ * launches per 16 events.
  * Errors: LST_ERR_ARG (bad slot, n < 0, NULL arrays), LST_ERR_OVERFLOW (n > cap_hits). */
 LST_API int lst_load_event(lst_ctx* ctx, int slot, const lst_hits* hits, void* cuda_stream);
+LST_API int lst_load_events(lst_ctx* ctx, int first_slot, int n_slots, const lst_hits* hits, void* cuda_stream);
 
 /* Steps a1..a4 for one slot / for slots first_slot .. first_slot+n_slots-1 in ONE set of
  * launches (the batch index is a grid dimension).  Asynchronous; no host synchronisation. */

@@ -13,6 +13,7 @@
 
 #include <atomic>
 #include <cstdlib>
+#include <cmath>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -42,8 +43,10 @@ struct lst_ctx {
   Params P;  // first_slot filled per call
   int device = 0;
   signed char* d_layer = nullptr;
-  int* d_run_offsets = nullptr;
-  int2* d_runs = nullptr;
+  float2* d_mod_cs = nullptr;
+  int* d_map_offsets = nullptr;
+  int* d_map_targets = nullptr;
+  float* d_map_dphi = nullptr;
   char* arena = nullptr;
   size_t arena_bytes = 0;
   std::vector<SlotHost> slots;
@@ -71,6 +74,7 @@ Layout make_layout(const lst_config& cfg, int n_modules) {
   L.n_modules = n_modules;
   L.n_bins = 2 * n_modules;
   L.cap_hits = cfg.cap_hits; L.cap_md = cfg.cap_md; L.cap_seg = cfg.cap_seg; L.cap_t3 = cfg.cap_t3; L.cap_t5 = cfg.cap_t5;
+  L.n_chunk_hits = (cfg.cap_hits + kScanChunk - 1) / kScanChunk;
   L.n_chunk_seg = (cfg.cap_seg + kScanChunk - 1) / kScanChunk;
   L.n_chunk_t3 = (cfg.cap_t3 + kScanChunk - 1) / kScanChunk;
   size_t off = 0;
@@ -81,9 +85,12 @@ Layout make_layout(const lst_config& cfg, int n_modules) {
   L.reset_bytes = off - L.hdr;
   const size_t nh = (size_t)cfg.cap_hits, nm = (size_t)cfg.cap_md, ns = (size_t)cfg.cap_seg, n3 = (size_t)cfg.cap_t3, n5 = (size_t)cfg.cap_t5;
   L.in_x = take(4 * nh); L.in_y = take(4 * nh); L.in_z = take(4 * nh); L.in_module = take(4 * nh); L.in_side = take(nh);
-  L.tmp_idx = take(4 * nh); L.hit4 = take(16 * nh); L.hit_orig = take(4 * nh);
+  L.tmp_idx = take(4 * nh); L.tmp_key = take(4 * nh);
+  L.hit4 = take(16 * nh); L.hit_key = take(4 * nh); L.hit_orig = take(4 * nh); L.hit_module = take(4 * nh);
+  L.md_off = take(4 * (nh + 1)); L.md_block_base = take(4 * (size_t)(L.n_chunk_hits + 1));
   L.md_start = take(4 * (size_t)(n_modules + 1));
-  L.md_anchor = take(16 * nm); L.md_aux = take(8 * nm); L.md_hits = take(8 * nm); L.md_out = take(8 * nm); L.md_module = take(4 * nm);
+  L.md_anchor = take(16 * nm); L.md_aux = take(8 * nm); L.md_key = take(4 * nm); L.md_hits = take(8 * nm);
+  L.md_out = take(8 * nm); L.md_module = take(4 * nm);
   L.seg_start = take(4 * (nm + 1)); L.seg_block_base = take(4 * (size_t)(n_modules + 1));
   L.seg_md = take(8 * ns); L.seg_f = take(16 * ns);
   L.t3_start = take(4 * (ns + 1)); L.t3_block_base = take(4 * (size_t)(L.n_chunk_seg + 1));
@@ -165,7 +172,7 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
   lst_config cfg;
   if (cfg_in) cfg = *cfg_in; else lst_default_config(&cfg);
   const int n = g->n_modules;
-  if (n <= 0 || n > (1 << 24) || m->n_modules != n || !g->layer || !m->row_offsets) return LST_ERR_ARG;
+  if (n <= 0 || n > (1 << 24) || m->n_modules != n || !g->layer || !g->phi || !m->row_offsets) return LST_ERR_ARG;
   if (cfg.n_slots < 1 || cfg.cap_hits < 1 || cfg.cap_md < 1 || cfg.cap_seg < 1 || cfg.cap_t3 < 1 || cfg.cap_t5 < 1) return LST_ERR_ARG;
   for (int i = 0; i < n; ++i)
     if (g->layer[i] < 0 || g->layer[i] >= LST_N_LAYERS) return LST_ERR_ARG;
@@ -173,19 +180,25 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
   for (int i = 0; i < n; ++i)
     if (m->row_offsets[i + 1] < m->row_offsets[i]) return LST_ERR_ARG;
   if (m->row_offsets[n] > 0 && !m->targets) return LST_ERR_ARG;
-  // rows strictly ascending, targets in the next layer; compress each row into runs of
-  // consecutive module ids (a ring's phi-neighbours are consecutive ids)
-  std::vector<int> run_offsets(n + 1, 0);
-  std::vector<int2> runs;
+  // rows strictly ascending, targets in the next layer, at most kMaxRow connections per module
+  const double kPi = 3.14159265358979323846;
+  const int n_conn = m->row_offsets[n];
+  std::vector<float> map_dphi((size_t)n_conn + 1, 0.0f);
+  std::vector<float2> mod_cs(n);
   for (int a = 0; a < n; ++a) {
+    if (!std::isfinite(g->phi[a])) return LST_ERR_ARG;
+    mod_cs[a] = make_float2((float)std::cos((double)g->phi[a]), (float)std::sin((double)g->phi[a]));
+    if (m->row_offsets[a + 1] - m->row_offsets[a] > kMaxRow) return LST_ERR_ARG;
     for (int k = m->row_offsets[a]; k < m->row_offsets[a + 1]; ++k) {
       const int t = m->targets[k];
       if (t < 0 || t >= n || g->layer[t] != g->layer[a] + 1) return LST_ERR_ARG;
       if (k > m->row_offsets[a] && t <= m->targets[k - 1]) return LST_ERR_ARG;
-      if (k > m->row_offsets[a] && t == runs.back().y + 1) runs.back().y = t;
-      else runs.push_back(make_int2(t, t));
+      if (!std::isfinite(g->phi[t])) return LST_ERR_ARG;
+      double d = std::fmod((double)g->phi[a] - (double)g->phi[t], 2.0 * kPi);  // into (-pi, pi]
+      if (d > kPi) d -= 2.0 * kPi;
+      if (d <= -kPi) d += 2.0 * kPi;
+      map_dphi[k] = (float)d;
     }
-    run_offsets[a + 1] = (int)runs.size();
   }
 
   lst_ctx* c = new (std::nothrow) lst_ctx();
@@ -202,12 +215,16 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
   const Layout L = make_layout(cfg, n);
   c->arena_bytes = L.slot_bytes * (size_t)cfg.n_slots;
   if ((e = cudaMalloc(&c->d_layer, n)) != cudaSuccess) return bail(LST_ERR_NOMEM, e);
-  if ((e = cudaMalloc(&c->d_run_offsets, sizeof(int) * (n + 1))) != cudaSuccess) return bail(LST_ERR_NOMEM, e);
-  if ((e = cudaMalloc(&c->d_runs, sizeof(int2) * (runs.size() + 1))) != cudaSuccess) return bail(LST_ERR_NOMEM, e);
+  if ((e = cudaMalloc(&c->d_mod_cs, sizeof(float2) * n)) != cudaSuccess) return bail(LST_ERR_NOMEM, e);
+  if ((e = cudaMalloc(&c->d_map_offsets, sizeof(int) * (n + 1))) != cudaSuccess) return bail(LST_ERR_NOMEM, e);
+  if ((e = cudaMalloc(&c->d_map_targets, sizeof(int) * ((size_t)n_conn + 1))) != cudaSuccess) return bail(LST_ERR_NOMEM, e);
+  if ((e = cudaMalloc(&c->d_map_dphi, sizeof(float) * ((size_t)n_conn + 1))) != cudaSuccess) return bail(LST_ERR_NOMEM, e);
   if ((e = cudaMalloc(&c->arena, c->arena_bytes)) != cudaSuccess) { cudaGetLastError(); return bail(LST_ERR_NOMEM, e); }
   if ((e = cudaMemcpy(c->d_layer, g->layer, n, cudaMemcpyHostToDevice)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
-  if ((e = cudaMemcpy(c->d_run_offsets, run_offsets.data(), sizeof(int) * (n + 1), cudaMemcpyHostToDevice)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
-  if (!runs.empty() && (e = cudaMemcpy(c->d_runs, runs.data(), sizeof(int2) * runs.size(), cudaMemcpyHostToDevice)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
+  if ((e = cudaMemcpy(c->d_mod_cs, mod_cs.data(), sizeof(float2) * n, cudaMemcpyHostToDevice)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
+  if ((e = cudaMemcpy(c->d_map_offsets, m->row_offsets, sizeof(int) * (n + 1), cudaMemcpyHostToDevice)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
+  if (n_conn > 0 && (e = cudaMemcpy(c->d_map_targets, m->targets, sizeof(int) * (size_t)n_conn, cudaMemcpyHostToDevice)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
+  if (n_conn > 0 && (e = cudaMemcpy(c->d_map_dphi, map_dphi.data(), sizeof(float) * (size_t)n_conn, cudaMemcpyHostToDevice)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   if ((e = cudaMemset(c->arena, 0, c->arena_bytes)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   if ((e = cudaMallocHost(&c->pinned, sizeof(SlotHeader) * (size_t)cfg.n_slots)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   std::memset(c->pinned, 0, sizeof(SlotHeader) * (size_t)cfg.n_slots);
@@ -223,8 +240,10 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
   c->P.L = L;
   copy_cuts(c->P.cuts, cfg);
   c->P.mod_layer = c->d_layer;
-  c->P.run_offsets = c->d_run_offsets;
-  c->P.runs = c->d_runs;
+  c->P.mod_cs = c->d_mod_cs;
+  c->P.map_offsets = c->d_map_offsets;
+  c->P.map_targets = c->d_map_targets;
+  c->P.map_dphi = c->d_map_dphi;
   c->P.first_slot = 0;
   if ((e = cudaDeviceSynchronize()) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   *out = c;
@@ -239,48 +258,68 @@ int lst_destroy(lst_ctx* c) {
       if (ev) cudaEventDestroy(ev);
   if (c->pinned) cudaFreeHost(c->pinned);
   if (c->arena) cudaFree(c->arena);
-  if (c->d_runs) cudaFree(c->d_runs);
-  if (c->d_run_offsets) cudaFree(c->d_run_offsets);
+  if (c->d_map_dphi) cudaFree(c->d_map_dphi);
+  if (c->d_map_targets) cudaFree(c->d_map_targets);
+  if (c->d_map_offsets) cudaFree(c->d_map_offsets);
+  if (c->d_mod_cs) cudaFree(c->d_mod_cs);
   if (c->d_layer) cudaFree(c->d_layer);
   delete c;
   return LST_OK;
 }
 
-int lst_load_event(lst_ctx* c, int slot, const lst_hits* h, void* stream) {
-  if (!valid_slot(c, slot) || !h || h->n < 0) return LST_ERR_ARG;
-  if (h->n > 0 && (!h->x || !h->y || !h->z || !h->module || !h->side)) return LST_ERR_ARG;
-  if (h->n > c->cfg.cap_hits) return LST_ERR_OVERFLOW;
+int lst_load_events(lst_ctx* c, int first, int n_ev, const lst_hits* hits, void* stream) {
+  if (!c || n_ev < 1 || !valid_slot(c, first) || !valid_slot(c, first + n_ev - 1) || !hits) return LST_ERR_ARG;
+  for (int b = 0; b < n_ev; ++b) {
+    const lst_hits* h = hits + b;
+    if (h->n < 0) return LST_ERR_ARG;
+    if (h->n > 0 && (!h->x || !h->y || !h->z || !h->module || !h->side)) return LST_ERR_ARG;
+    if (h->n > c->cfg.cap_hits) return LST_ERR_OVERFLOW;
+  }
   cudaStream_t s = (cudaStream_t)stream;
   LST_CUDA(c, cudaSetDevice(c->device));
-  SlotHost& sh = c->slots[slot];
-  sh.loaded = sh.ran = sh.synced = false;
-  sh.n_hits_in = h->n;
   const Layout& L = c->P.L;
-  char* base = c->arena + (size_t)slot * c->P.slot_stride;
-  LST_CUDA(c, cudaMemsetAsync(base + L.hdr, 0, L.reset_bytes, s));
-  HitInput in{h->x, h->y, h->z, h->module, h->side, h->n};
-  if (!h->on_device && h->n > 0) {
-    const size_t n = (size_t)h->n;
-    LST_CUDA(c, cudaMemcpyAsync(base + L.in_x, h->x, 4 * n, cudaMemcpyHostToDevice, s));
-    LST_CUDA(c, cudaMemcpyAsync(base + L.in_y, h->y, 4 * n, cudaMemcpyHostToDevice, s));
-    LST_CUDA(c, cudaMemcpyAsync(base + L.in_z, h->z, 4 * n, cudaMemcpyHostToDevice, s));
-    LST_CUDA(c, cudaMemcpyAsync(base + L.in_module, h->module, 4 * n, cudaMemcpyHostToDevice, s));
-    LST_CUDA(c, cudaMemcpyAsync(base + L.in_side, h->side, n, cudaMemcpyHostToDevice, s));
-    in.x = reinterpret_cast<const float*>(base + L.in_x);
-    in.y = reinterpret_cast<const float*>(base + L.in_y);
-    in.z = reinterpret_cast<const float*>(base + L.in_z);
-    in.module = reinterpret_cast<const int*>(base + L.in_module);
-    in.side = reinterpret_cast<const unsigned char*>(base + L.in_side);
+  for (int b0 = 0; b0 < n_ev; b0 += kMaxBatch) {
+    const int nb = n_ev - b0 < kMaxBatch ? n_ev - b0 : kMaxBatch;
+    HitBatch batch;
+    std::memset(&batch, 0, sizeof(batch));
+    for (int b = 0; b < nb; ++b) {
+      const int slot = first + b0 + b;
+      const lst_hits* h = hits + b0 + b;
+      SlotHost& sh = c->slots[slot];
+      sh.loaded = sh.ran = sh.synced = false;
+      sh.n_hits_in = h->n;
+      sh.ev_bin = false;
+      for (bool& f : sh.ev_stage) f = false;
+      char* base = c->arena + (size_t)slot * c->P.slot_stride;
+      LST_CUDA(c, cudaMemsetAsync(base + L.hdr, 0, L.reset_bytes, s));
+      HitInput in{h->x, h->y, h->z, h->module, h->side, h->n};
+      if (!h->on_device && h->n > 0) {
+        const size_t n = (size_t)h->n;
+        LST_CUDA(c, cudaMemcpyAsync(base + L.in_x, h->x, 4 * n, cudaMemcpyHostToDevice, s));
+        LST_CUDA(c, cudaMemcpyAsync(base + L.in_y, h->y, 4 * n, cudaMemcpyHostToDevice, s));
+        LST_CUDA(c, cudaMemcpyAsync(base + L.in_z, h->z, 4 * n, cudaMemcpyHostToDevice, s));
+        LST_CUDA(c, cudaMemcpyAsync(base + L.in_module, h->module, 4 * n, cudaMemcpyHostToDevice, s));
+        LST_CUDA(c, cudaMemcpyAsync(base + L.in_side, h->side, n, cudaMemcpyHostToDevice, s));
+        in.x = reinterpret_cast<const float*>(base + L.in_x);
+        in.y = reinterpret_cast<const float*>(base + L.in_y);
+        in.z = reinterpret_cast<const float*>(base + L.in_z);
+        in.module = reinterpret_cast<const int*>(base + L.in_module);
+        in.side = reinterpret_cast<const unsigned char*>(base + L.in_side);
+      }
+      batch.ev[b] = in;
+    }
+    SlotHost& sh0 = c->slots[first + b0];
+    Params P = c->P;
+    P.first_slot = first + b0;
+    c->launches += launch_bin(P, batch, nb, s, c->cfg.timing ? sh0.ev : nullptr);
+    LST_CUDA(c, cudaGetLastError());
+    sh0.ev_bin = c->cfg.timing != 0;
+    for (int b = 0; b < nb; ++b) c->slots[first + b0 + b].loaded = true;
   }
-  Params P = c->P;
-  P.first_slot = slot;
-  c->launches += launch_bin(P, in, s, c->cfg.timing ? sh.ev : nullptr);
-  LST_CUDA(c, cudaGetLastError());
-  sh.ev_bin = c->cfg.timing != 0;
-  for (bool& b : sh.ev_stage) b = false;
-  sh.loaded = true;
   return LST_OK;
 }
+
+int lst_load_event(lst_ctx* c, int slot, const lst_hits* h, void* stream) { return lst_load_events(c, slot, 1, h, stream); }
 
 int lst_run_stage(lst_ctx* c, int first, int n, int stage, void* stream) {
   if (!c || n < 1 || !valid_slot(c, first) || !valid_slot(c, first + n - 1) || stage < LST_MD || stage > LST_T5) return LST_ERR_ARG;
@@ -390,7 +429,7 @@ int lst_get_stats(lst_ctx* c, int slot, lst_stats* o) {
   if (!sh.synced) return LST_ERR_STATE;
   std::memset(o, 0, sizeof(*o));
   o->n_hits = sh.hdr->n_hits;
-  for (int k = 0; k < 4; ++k) { o->needed[k] = (int64_t)sh.hdr->needed[k]; o->candidates[k] = (int64_t)sh.hdr->cand[k]; }
+  for (int k = 0; k < 4; ++k) { o->needed[k] = (int64_t)sh.hdr->needed[k]; o->candidates[k] = (int64_t)sh.hdr->cand[k]; o->evaluated[k] = (int64_t)sh.hdr->eval[k]; }
   o->overflow = sh.hdr->overflow;
   o->bad_hits = sh.hdr->bad_hits;
   if (c->cfg.timing) {

@@ -1,5 +1,9 @@
 // lst_kernels.cu -- sm_100a kernels of the LST hot path (DESIGN.md sections 5-6).
 //
+// Hits and mini-doublets are kept ordered by azimuth inside their module, so the MD and the
+// segment stage look only at a window of candidates found by binary search (DESIGN.md
+// section 6); every candidate in a window goes through the exact SPEC selection.
+//
 // Every stage is  count -> (last block scans) -> fill : the count kernel evaluates the
 // selection and leaves per-owner counts; the last block to finish turns block totals into block
 // bases (no extra launch, no host round trip); the fill kernel re-walks the same candidates in
@@ -98,207 +102,469 @@ __device__ __forceinline__ void publish_total(SlotHeader* h, int kind, int total
 }
 
 // ------------------------------------------------------------------------------------------
-// a0: load + bin by (module, side) + order by original index + derive r
+// search windows.  A window is a conservative superset of what the SPEC
+// selection can accept, derived from the selection's own inequalities and the per-event range
+// of r per (side, layer); every candidate inside it goes through the exact SPEC selection, so
+// the object set does not depend on the window.  Geometry of a pair seen from the beam line:
+// with alpha the angle between the inner position vector and the inner->outer displacement
+// (sin alpha is the cut variable sinA / sinS) and delta the azimuth difference,
+//     delta = alpha - asin((r_in / r_out) sin alpha)          (law of sines; dot > 0, r_out > r_in)
+// which grows with alpha, and for alpha > 0 with r_out.
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_bin_count(const __grid_constant__ Params P, const HitInput in) {
-  Slot S(P, 0);
+__device__ __forceinline__ float delta_of(float s, float ratio) {
+  return asinf(s) - asinf(ratio * s);
+}
+
+__device__ __forceinline__ int lower_bound_f(const float* a, int lo, int hi, float v) {  // first a[i] >= v
+  while (lo < hi) {
+    const int mid = (lo + hi) >> 1;
+    if (a[mid] < v) lo = mid + 1; else hi = mid;
+  }
+  return lo;
+}
+__device__ __forceinline__ int upper_bound_f(const float* a, int lo, int hi, float v) {  // first a[i] > v
+  while (lo < hi) {
+    const int mid = (lo + hi) >> 1;
+    if (a[mid] <= v) lo = mid + 1; else hi = mid;
+  }
+  return lo;
+}
+
+// M2 bounds |sinA| by thr(r_u) <= thr(r_max_upper); M1 (dot > 0) gives r_u > r_l.
+// Returns the half width of the azimuth window around the lower hit, < 0 if nothing can pass.
+__device__ __forceinline__ float md_window(const Cuts& c, int layer, float r_l, float r_max_upper) {
+  if (!(r_max_upper > 0.0f) || !(r_max_upper * 1.000001f >= r_l)) return -1.0f;
+  const float thr = fminf(1.0f, sin_threshold(c, r_max_upper, c.md_cos_eps[layer], c.md_sin_eps[layer]) * 1.00001f);
+  const float d = delta_of(thr, fminf(1.0f, r_l / r_max_upper));
+  return d * 1.001f + 2e-5f;
+}
+
+// S2 bounds |sinS| by thr(r_o); S4 on the inner MD bounds sinS * (ur_i / r_o) by sinA_i +- eps;
+// S3 needs r_o > r_i.  [r_min_o, r_max_o] is the range of r of the anchors of the outer layer.
+// Returns the window [dlo, dhi] of azimuth(outer) - azimuth(inner); dlo > dhi if nothing can pass.
+__device__ __forceinline__ void seg_window(const Cuts& c, int layer, float r_i, float ur_i, float sinA_i,
+                                           float r_min_o, float r_max_o, float& dlo, float& dhi) {
+  dlo = 1.0f;
+  dhi = -1.0f;
+  if (!(r_max_o > r_i)) return;
+  const float r_lo = fmaxf(r_min_o, r_i);
+  float s_hi = fminf(1.0f, sin_threshold(c, r_max_o, c.seg_cos_eps, c.seg_sin_eps) * 1.00001f);
+  float s_lo = -s_hi;
+  if (ur_i > 0.0f && ur_i < 3.0e38f) {
+    const float e = c.md_eps[layer] + 1e-5f;
+    const float c_lo = (sinA_i - e) / ur_i, c_hi = (sinA_i + e) / ur_i;
+    const float a = (c_lo >= 0.0f) ? c_lo * r_lo : c_lo * r_max_o;   // min over r_o of c_lo * r_o
+    const float b = (c_hi >= 0.0f) ? c_hi * r_max_o : c_hi * r_lo;   // max over r_o of c_hi * r_o
+    s_lo = fmaxf(s_lo, a - (1e-5f + 1e-5f * fabsf(a)));
+    s_hi = fminf(s_hi, b + (1e-5f + 1e-5f * fabsf(b)));
+  }
+  if (!(s_lo <= s_hi)) return;
+  const float q_lo = fminf(1.0f, r_i / r_lo), q_hi = r_i / r_max_o;
+  const float hi = fmaxf(delta_of(s_hi, q_lo), delta_of(s_hi, q_hi));
+  const float lo = fminf(delta_of(s_lo, q_lo), delta_of(s_lo, q_hi));
+  dlo = lo - (3e-5f + 1e-3f * fabsf(lo));
+  dhi = hi + (3e-5f + 1e-3f * fabsf(hi));
+}
+
+__device__ __forceinline__ float r_min_of(const SlotHeader* h, int side, int layer) {
+  return __int_as_float(0x7f800000 - h->r_min_inv[side][layer]);
+}
+__device__ __forceinline__ float r_max_of(const SlotHeader* h, int side, int layer) {
+  return __int_as_float(h->r_max[side][layer]);
+}
+
+// ------------------------------------------------------------------------------------------
+// a0: load + bin by (side, module) + order by azimuth + derive r
+// blockIdx.y = event of the batch; its input arrays come from the pointer table `B`.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_bin_count(const __grid_constant__ Params P, const __grid_constant__ HitBatch B) {
+  Slot S(P, blockIdx.y);
+  const HitInput& in = B.ev[blockIdx.y];
   unsigned* cnt = S.bin_start();
+  const int nmod = P.L.n_modules;
   int bad = 0;
   for (int h = blockIdx.x * blockDim.x + threadIdx.x; h < in.n; h += gridDim.x * blockDim.x) {
     const int m = in.module[h];
     const unsigned sd = in.side[h];
-    if (m < 0 || m >= P.L.n_modules || sd > 1u) { ++bad; continue; }
-    atomicAdd(cnt + (2 * m + (int)sd), 1u);
+    if (m < 0 || m >= nmod || sd > 1u) { ++bad; continue; }
+    atomicAdd(cnt + ((int)sd * nmod + m), 1u);
   }
   if (bad) atomicAdd(&S.hdr()->bad_hits, bad);
-}
-
-__global__ void __launch_bounds__(1024) k_bin_scan(const __grid_constant__ Params P) {
-  Slot S(P, 0);
-  int* start = reinterpret_cast<int*>(S.bin_start());
-  const int total = block_scan_array<1024>(start, P.L.n_bins, -1);
+  // the last block of the event turns the counts into bin offsets
+  if (!last_block_done(&S.hdr()->done[4], gridDim.x)) return;
+  int* start = reinterpret_cast<int*>(cnt);
+  const int total = block_scan_array<256>(start, P.L.n_bins, -1);
   __syncthreads();
-  // candidate count of the MD stage: sum over modules of (#lower hits) x (#upper hits)
+  // search space of the MD stage: sum over modules of (#lower hits) x (#upper hits)
   unsigned long long c = 0;
-  for (int m = threadIdx.x; m < P.L.n_modules; m += 1024) {
-    const unsigned long long l = start[2 * m + 1] - start[2 * m], u = start[2 * m + 2] - start[2 * m + 1];
+  for (int m = threadIdx.x; m < nmod; m += 256) {
+    const unsigned long long l = start[m + 1] - start[m], u = start[nmod + m + 1] - start[nmod + m];
     c += l * u;
   }
 #pragma unroll
   for (int d = 16; d > 0; d >>= 1) c += __shfl_down_sync(0xffffffffu, c, d);
   if (lane_id() == 0 && c) atomicAdd(&S.hdr()->cand[LST_MD_], c);
-  if (threadIdx.x == 0) S.hdr()->n_hits = total;
-}
-
-__global__ void __launch_bounds__(256) k_bin_scatter(const __grid_constant__ Params P, const HitInput in) {
-  Slot S(P, 0);
-  const unsigned* start = S.bin_start();
-  unsigned* cur = S.bin_cursor();
-  int* tmp = S.tmp_idx();
-  for (int h = blockIdx.x * blockDim.x + threadIdx.x; h < in.n; h += gridDim.x * blockDim.x) {
-    const int m = in.module[h];
-    const unsigned sd = in.side[h];
-    if (m < 0 || m >= P.L.n_modules || sd > 1u) continue;
-    const int b = 2 * m + (int)sd;
-    tmp[start[b] + atomicAdd(cur + b, 1u)] = h;
+  if (threadIdx.x == 0) {
+    S.hdr()->n_hits = total;
+    S.hdr()->n_lower = start[nmod];
   }
 }
 
-// One warp per bin: rank the bin's original indices (ascending) and gather the coordinates.
-__global__ void __launch_bounds__(256) k_bin_order(const __grid_constant__ Params P, const HitInput in) {
-  Slot S(P, 0);
+__global__ void __launch_bounds__(256) k_bin_scatter(const __grid_constant__ Params P, const __grid_constant__ HitBatch B) {
+  Slot S(P, blockIdx.y);
+  const HitInput& in = B.ev[blockIdx.y];
+  const unsigned* start = S.bin_start();
+  unsigned* cur = S.bin_cursor();
+  int* tmp = S.tmp_idx();
+  float* tkey = S.tmp_key();
+  const int nmod = P.L.n_modules;
+  for (int h = blockIdx.x * blockDim.x + threadIdx.x; h < in.n; h += gridDim.x * blockDim.x) {
+    const int m = in.module[h];
+    const unsigned sd = in.side[h];
+    if (m < 0 || m >= nmod || sd > 1u) continue;
+    const int b = (int)sd * nmod + m;
+    const float x = in.x[h], y = in.y[h];
+    const float2 cs = P.mod_cs[m];
+    // azimuth relative to the module normal; non-finite hits (they can never pass a cut) go last
+    const float k = atan2f(cs.x * y - cs.y * x, cs.x * x + cs.y * y);
+    const unsigned pos = start[b] + atomicAdd(cur + b, 1u);
+    tmp[pos] = h;
+    tkey[pos] = (fabsf(k) <= 4.0f) ? k : 3.0e38f;
+  }
+}
+
+// One warp per bin: rank the bin's hits by (key, original index) and gather the coordinates.
+__global__ void __launch_bounds__(256) k_bin_order(const __grid_constant__ Params P, const __grid_constant__ HitBatch B) {
+  Slot S(P, blockIdx.y);
+  const HitInput& in = B.ev[blockIdx.y];
   const int b = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (b >= P.L.n_bins) return;
   const unsigned* start = S.bin_start();
   const int s = start[b], n = start[b + 1] - s;
+  if (n == 0) return;
+  const int nmod = P.L.n_modules;
+  const int side = b >= nmod, m = b - side * nmod;
   const int* tmp = S.tmp_idx() + s;
+  const float* tkey = S.tmp_key() + s;
   float4* hit4 = S.hit4() + s;
+  float* hkey = S.hit_key() + s;
   int* orig = S.hit_orig() + s;
-  for (int i = lane_id(); i < n; i += 32) {
-    const int mine = tmp[i];
-    int rank = 0;
-    for (int j = 0; j < n; ++j) rank += (tmp[j] < mine);
-    const float x = in.x[mine], y = in.y[mine], z = in.z[mine];
-    hit4[rank] = make_float4(x, y, z, sqrtf(x * x + y * y));
-    orig[rank] = mine;
+  int* hmod = S.hit_module() + s;
+  float rmin = 3.0e38f, rmax = 0.0f;
+  for (int i0 = 0; i0 < n; i0 += 32) {
+    const int i = i0 + lane_id();
+    int mine = 0, rank = 0;
+    float key = 0.0f;
+    if (i < n) { mine = tmp[i]; key = tkey[i]; }
+    if (n <= 32) {
+      for (int j = 0; j < n; ++j) {
+        const float kj = __shfl_sync(0xffffffffu, key, j);
+        const int ij = __shfl_sync(0xffffffffu, mine, j);
+        rank += (kj < key) || (kj == key && ij < mine);
+      }
+    } else if (i < n) {
+      for (int j = 0; j < n; ++j) {
+        const float kj = tkey[j];
+        const int ij = tmp[j];
+        rank += (kj < key) || (kj == key && ij < mine);
+      }
+    }
+    if (i < n) {
+      const float x = in.x[mine], y = in.y[mine], z = in.z[mine];
+      const float r = sqrtf(x * x + y * y);
+      hit4[rank] = make_float4(x, y, z, r);
+      hkey[rank] = key;
+      orig[rank] = mine;
+      hmod[rank] = m;
+      if (r < 3.0e38f) { rmin = fminf(rmin, r); rmax = fmaxf(rmax, r); }
+    }
+  }
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) {
+    rmin = fminf(rmin, __shfl_down_sync(0xffffffffu, rmin, d));
+    rmax = fmaxf(rmax, __shfl_down_sync(0xffffffffu, rmax, d));
+  }
+  if (lane_id() == 0 && rmin <= rmax) {
+    const int layer = P.mod_layer[m];
+    SlotHeader* h = S.hdr();
+    atomicMax(&h->r_min_inv[side][layer], 0x7f800000 - __float_as_int(rmin));
+    atomicMax(&h->r_max[side][layer], __float_as_int(rmax));
   }
 }
 
 // ------------------------------------------------------------------------------------------
-// a1: mini-doublets. One warp per module; lanes sweep the (lower, upper) pairs of the module
-// in row-major order p = l * U + u.
+// a1: mini-doublets. One thread per lower hit; its candidates are the upper hits of the same
+// module inside the azimuth window (a binary search in the key-ordered upper bin).
 // ------------------------------------------------------------------------------------------
-constexpr int kMdWarps = 8;
-
 template <bool FILL>
-__global__ void __launch_bounds__(kMdWarps * 32) k_md(const __grid_constant__ Params P) {
+__global__ void __launch_bounds__(kScanChunk) k_md(const __grid_constant__ Params P) {
   Slot S(P, blockIdx.y);
-  const int m = blockIdx.x * kMdWarps + (threadIdx.x >> 5);
-  int* md_start = S.md_start();
-  if (m < P.L.n_modules) {
-    const unsigned* bs = S.bin_start();
-    const unsigned s0 = bs[2 * m], s1 = bs[2 * m + 1], s2 = bs[2 * m + 2];
-    const unsigned L = s1 - s0, U = s2 - s1, T = L * U;
-    const int layer = P.mod_layer[m];
-    const float4* hit4 = S.hit4();
-    int running = 0;
-    const int base = FILL ? md_start[m] : 0;
-    for (unsigned p0 = 0; p0 < T; p0 += 32) {
-      const unsigned p = p0 + lane_id();
-      bool pass = false;
-      float4 lo, up;
-      MdOut o;
-      unsigned l = 0, u = 0;
-      if (p < T) {
-        l = p / U;
-        u = p - l * U;
-        lo = hit4[s0 + l];
-        up = hit4[s1 + u];
-        pass = md_select(P.cuts, layer, lo, up, o);
-      }
-      const unsigned bal = __ballot_sync(0xffffffffu, pass);
-      if (FILL && pass) {
-        const int pos = base + running + __popc(bal & lanemask_lt());
-        if (pos < P.L.cap_md) {
-          S.md_anchor()[pos] = lo;
-          S.md_aux()[pos] = make_float2(up.w, o.sinA);
-          S.md_hits()[pos] = make_int2(S.hit_orig()[s0 + l], S.hit_orig()[s1 + u]);
-          S.md_out()[pos] = make_float2(atan2f(lo.x * up.y - lo.y * up.x, lo.x * up.x + lo.y * up.y),
-                                        atan2f(o.cross, o.dot));
-          S.md_module()[pos] = m;
+  SlotHeader* H = S.hdr();
+  const int nmod = P.L.n_modules;
+  const int nLower = H->n_lower;
+  const int nChunks = (nLower + kScanChunk - 1) / kScanChunk;
+  const unsigned* bs = S.bin_start();
+  const float4* hit4 = S.hit4();
+  const float* hkey = S.hit_key();
+  int* md_off = S.md_off();
+  int* block_base = S.md_block_base();
+  unsigned long long evals = 0;
+  for (int c = blockIdx.x; c < nChunks; c += gridDim.x) {
+    const int i = c * kScanChunk + threadIdx.x;
+    int count = 0;
+    if (i < nLower) {
+      const int m = S.hit_module()[i];
+      const int layer = P.mod_layer[m];
+      const int u0 = bs[nmod + m], u1 = bs[nmod + m + 1];
+      if (u1 > u0) {
+        const float4 lo = hit4[i];
+        const float kl = hkey[i];
+        const float w = md_window(P.cuts, layer, lo.w, r_max_of(H, 1, layer));
+        int j0 = u0, j1 = u1;
+        if (w < 0.0f) {
+          j1 = j0;
+        } else if (fabsf(kl) + w < 1.5f) {
+          j0 = lower_bound_f(hkey, u0, u1, kl - w);
+          j1 = upper_bound_f(hkey, j0, u1, kl + w);
+        }
+        evals += (unsigned long long)(j1 - j0);
+        const int base = FILL ? block_base[c] + md_off[i] : 0;
+        for (int j = j0; j < j1; ++j) {
+          const float4 up = hit4[j];
+          MdOut o;
+          if (md_select(P.cuts, layer, lo, up, o)) {
+            if (FILL) {
+              const int pos = base + count;
+              if (pos < P.L.cap_md) {
+                S.md_anchor()[pos] = lo;
+                S.md_aux()[pos] = make_float2(up.w, o.sinA);
+                S.md_key()[pos] = kl;
+                S.md_hits()[pos] = make_int2(S.hit_orig()[i], S.hit_orig()[j]);
+                S.md_out()[pos] = make_float2(atan2f(lo.x * up.y - lo.y * up.x, lo.x * up.x + lo.y * up.y),
+                                              atan2f(o.cross, o.dot));
+                S.md_module()[pos] = m;
+              }
+            }
+            ++count;
+          }
         }
       }
-      running += __popc(bal);
     }
-    if (!FILL && lane_id() == 0) md_start[m] = running;
+    if (!FILL) {
+      int tot;
+      const int ex = block_excl_scan<kScanChunk>(count, tot);
+      if (i < nLower) md_off[i] = ex;
+      if (threadIdx.x == 0) block_base[c] = tot;
+    }
   }
-  if (!FILL) {
-    if (last_block_done(&S.hdr()->done[0], gridDim.x)) {
-      const int total = block_scan_array<kMdWarps * 32>(md_start, P.L.n_modules, P.L.cap_md);
-      if (threadIdx.x == 0) publish_total(S.hdr(), LST_MD_, total, P.L.cap_md);
+  if (FILL) {
+    // md_start[m] = index of the first MD of module m = offset of the module's first lower hit
+    const int total = H->n[LST_MD_];
+    for (int m = blockIdx.x * kScanChunk + threadIdx.x; m <= nmod; m += gridDim.x * kScanChunk) {
+      const int ls = (m < nmod) ? (int)bs[m] : nLower;
+      S.md_start()[m] = (ls < nLower) ? min(block_base[ls / kScanChunk] + md_off[ls], P.L.cap_md) : total;
+    }
+  } else {
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) evals += __shfl_down_sync(0xffffffffu, evals, d);
+    if (lane_id() == 0 && evals) atomicAdd(&H->eval[LST_MD_], evals);
+    if (last_block_done(&H->done[0], gridDim.x)) {
+      const int total = block_scan_array<kScanChunk>(block_base, nChunks, -1);
+      if (threadIdx.x == 0) publish_total(H, LST_MD_, total, P.L.cap_md);
     }
   }
 }
 
 // ------------------------------------------------------------------------------------------
-// a2: segments. One block per inner module A; one warp per inner MD at a time; lanes sweep the
-// outer MDs of the modules connected to A.  The module map is stored as runs of consecutive
-// target modules, and MDs are stored in module order, so every run is ONE contiguous range of
-// MD indices: coalesced 16-B loads, no per-module indirection.
+// a2: segments. One block per inner module A.  The module's mini-doublets are taken in tiles;
+// for a tile, (1) every (inner MD, connected module) pair finds its window of outer MDs by a
+// binary search in the connected module's key-ordered MD list, (2) a block scan of the window
+// sizes numbers the candidates in (inner MD, outer MD) order, (3) one thread per candidate
+// evaluates the SPEC selection.  Segments come out ordered by (inner MD, outer MD).
 // ------------------------------------------------------------------------------------------
 constexpr int kSegThreads = 128;
+constexpr int kSegTile = 128;    // inner MDs per tile
+constexpr int kSegPairs = 2048;  // (inner MD, connected module) pairs per tile
 
 template <bool FILL>
 __global__ void __launch_bounds__(kSegThreads) k_seg(const __grid_constant__ Params P) {
+  __shared__ int tB0[kMaxRow], tB1[kMaxRow];
+  __shared__ float tOff[kMaxRow], tKmin[kMaxRow], tKmax[kMaxRow];
+  __shared__ float4 iAnchor[kSegTile];
+  __shared__ float2 iAux[kSegTile];
+  __shared__ float iKey[kSegTile], iDlo[kSegTile], iDhi[kSegTile];
+  __shared__ int kCnt[kSegTile];
+  __shared__ int pLo[kSegPairs], pOff[kSegPairs + 1];
+  __shared__ int warpTot[kSegThreads / 32];
+
   Slot S(P, blockIdx.y);
+  SlotHeader* H = S.hdr();
   const int A = blockIdx.x;
   const int* md_start = S.md_start();
   int* seg_start = S.seg_start();
   const int mdLo = md_start[A], nA = md_start[A + 1] - mdLo;
-  const int r0 = P.run_offsets[A], r1 = P.run_offsets[A + 1];
-  const int layer = P.mod_layer[A];
+  const int row0 = P.map_offsets[A], nT = P.map_offsets[A + 1] - row0;
   const float4* anchor = S.md_anchor();
   const float2* aux = S.md_aux();
-  const int warp = threadIdx.x >> 5;
-  const int blockBase = FILL ? S.seg_block_base()[A] : 0;
-  unsigned long long nOut = 0;
-  for (int k = warp; k < nA; k += kSegThreads / 32) {
-    const int i = mdLo + k;
-    const float4 ai = anchor[i];
-    const float2 xi = aux[i];
-    int running = 0;
-    const int base = FILL ? blockBase + seg_start[i] : 0;
-    for (int r = r0; r < r1; ++r) {
-      const int2 run = P.runs[r];
-      const int lo = md_start[run.x], hi = md_start[run.y + 1];
-      if (k == warp) nOut += (unsigned long long)(hi - lo);
-      for (int o0 = lo; o0 < hi; o0 += 32) {
-        const int o = o0 + lane_id();
-        bool pass = false;
-        SegOut so;
-        float4 ao;
-        if (o < hi) {
-          ao = anchor[o];
-          const float2 xo = aux[o];
-          pass = seg_select(P.cuts, layer, ai, xi, ao, xo, so);
-        }
-        const unsigned bal = __ballot_sync(0xffffffffu, pass);
-        if (FILL && pass) {
-          const int pos = base + running + __popc(bal & lanemask_lt());
-          if (pos < P.L.cap_seg) {
-            S.seg_md()[pos] = make_int2(i, o);
-            S.seg_f()[pos] = make_float4(so.sinS, so.z0,
-                                         atan2f(ai.x * ao.y - ai.y * ao.x, ai.x * ao.x + ai.y * ao.y),
-                                         atan2f(so.cross, so.dot));
+  const float* mkey = S.md_key();
+  const int tid = threadIdx.x, warp = tid >> 5;
+  int blockTotal = 0;  // segments of this block so far (uniform across the block)
+
+  if (nA > 0 && nT > 0) {
+    const int layer = P.mod_layer[A];
+    const float rMinO = r_min_of(H, 0, layer + 1), rMaxO = r_max_of(H, 0, layer + 1);
+    const int blockBase = FILL ? S.seg_block_base()[A] : 0;
+    // connected modules: MD range, azimuth offset, key range
+    if (tid < nT) {
+      const int Bm = P.map_targets[row0 + tid];
+      const int b0 = md_start[Bm], b1 = md_start[Bm + 1];
+      tB0[tid] = b0;
+      tB1[tid] = b1;
+      tOff[tid] = P.map_dphi[row0 + tid];
+      tKmin[tid] = (b1 > b0) ? mkey[b0] : 3.0e38f;
+      tKmax[tid] = (b1 > b0) ? mkey[b1 - 1] : -3.0e38f;
+    }
+    __syncthreads();
+    if (!FILL && tid == 0) {
+      unsigned long long nOut = 0;
+      for (int t = 0; t < nT; ++t) nOut += (unsigned long long)(tB1[t] - tB0[t]);
+      if (nOut) atomicAdd(&H->cand[LST_SEG_], nOut * (unsigned long long)nA);
+    }
+    const int kTile = min(kSegTile, kSegPairs / nT);
+    unsigned long long evals = 0;
+    for (int k0 = 0; k0 < nA; k0 += kTile) {
+      const int kn = min(kTile, nA - k0);
+      for (int k = tid; k < kn; k += kSegThreads) {
+        const int i = mdLo + k0 + k;
+        const float4 a = anchor[i];
+        const float2 x = aux[i];
+        iAnchor[k] = a;
+        iAux[k] = x;
+        iKey[k] = mkey[i];
+        float dlo, dhi;
+        seg_window(P.cuts, layer, a.w, x.x, x.y, rMinO, rMaxO, dlo, dhi);
+        iDlo[k] = dlo;
+        iDhi[k] = dhi;
+        kCnt[k] = 0;
+      }
+      __syncthreads();
+      // (1) windows
+      const int nPairs = kn * nT;
+      for (int p = tid; p < nPairs; p += kSegThreads) {
+        const int k = p / nT, t = p - k * nT;
+        const int b0 = tB0[t], b1 = tB1[t];
+        int lo = b0, n = 0;
+        const float dlo = iDlo[k], dhi = iDhi[k];
+        if (b1 > b0 && dlo <= dhi) {
+          const float c0 = iKey[k] + tOff[t];
+          if (!(fabsf(c0) + fmaxf(fabsf(dlo), fabsf(dhi)) < 3.0f)) {
+            n = b1 - b0;  // azimuth wrap possible (never with a sane geometry): no window
+          } else if (c0 + dhi >= tKmin[t] && c0 + dlo <= tKmax[t]) {
+            lo = lower_bound_f(mkey, b0, b1, c0 + dlo);
+            n = upper_bound_f(mkey, lo, b1, c0 + dhi) - lo;
           }
         }
-        running += __popc(bal);
+        pLo[p] = lo;
+        pOff[p] = n;
       }
+      __syncthreads();
+      // (2) exclusive scan of the window sizes
+      int nCand;
+      {
+        const int ipt = (nPairs + kSegThreads - 1) / kSegThreads;
+        const int lo = min(nPairs, tid * ipt), hi = min(nPairs, lo + ipt);
+        int s = 0;
+        for (int p = lo; p < hi; ++p) s += pOff[p];
+        int run = block_excl_scan<kSegThreads>(s, nCand);
+        for (int p = lo; p < hi; ++p) {
+          const int v = pOff[p];
+          pOff[p] = run;
+          run += v;
+        }
+        if (tid == 0) pOff[nPairs] = nCand;
+      }
+      __syncthreads();
+      evals += (tid == 0) ? (unsigned long long)nCand : 0ull;
+      // (3) one thread per candidate
+      for (int c0 = 0; c0 < nCand; c0 += kSegThreads) {
+        const int c = c0 + tid;
+        bool pass = false;
+        SegOut so;
+        float4 ai, ao;
+        int k = 0, o = 0;
+        if (c < nCand) {
+          int lo = 0, hi = nPairs;  // last p with pOff[p] <= c
+          while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (pOff[mid] <= c) lo = mid; else hi = mid;
+          }
+          k = lo / nT;
+          o = pLo[lo] + (c - pOff[lo]);
+          ai = iAnchor[k];
+          ao = anchor[o];
+          pass = seg_select(P.cuts, layer, ai, iAux[k], ao, aux[o], so);
+        }
+        if (!FILL) {
+          if (pass) atomicAdd(&kCnt[k], 1);
+        } else {
+          const unsigned bal = __ballot_sync(0xffffffffu, pass);
+          if (lane_id() == 0) warpTot[warp] = __popc(bal);
+          __syncthreads();
+          int before = 0, all = 0;
+#pragma unroll
+          for (int w = 0; w < kSegThreads / 32; ++w) {
+            const int v = warpTot[w];
+            before += (w < warp) ? v : 0;
+            all += v;
+          }
+          if (pass) {
+            const int pos = blockBase + blockTotal + before + __popc(bal & lanemask_lt());
+            if (pos < P.L.cap_seg) {
+              S.seg_md()[pos] = make_int2(mdLo + k0 + k, o);
+              S.seg_f()[pos] = make_float4(so.sinS, so.z0,
+                                           atan2f(ai.x * ao.y - ai.y * ao.x, ai.x * ao.x + ai.y * ao.y),
+                                           atan2f(so.cross, so.dot));
+            }
+          }
+          blockTotal += all;
+          __syncthreads();
+        }
+      }
+      if (!FILL) {
+        __syncthreads();
+        for (int k = tid; k < kn; k += kSegThreads) seg_start[mdLo + k0 + k] = kCnt[k];
+      }
+      __syncthreads();
     }
-    __syncwarp();  // every lane has read seg_start[i] (the local offset) before it is replaced
-    if (lane_id() == 0) seg_start[i] = FILL ? min(base, P.L.cap_seg) : running;
+    if (!FILL && tid == 0 && evals) atomicAdd(&H->eval[LST_SEG_], evals);
+    if (FILL) {
+      // local offsets (left by the count pass) -> global segment index of each inner MD
+      for (int k = tid; k < nA; k += kSegThreads) seg_start[mdLo + k] = min(blockBase + seg_start[mdLo + k], P.L.cap_seg);
+    }
+  } else if (!FILL) {
+    for (int k = tid; k < nA; k += kSegThreads) seg_start[mdLo + k] = 0;
+  } else {
+    const int blockBase = S.seg_block_base()[A];
+    for (int k = tid; k < nA; k += kSegThreads) seg_start[mdLo + k] = min(blockBase, P.L.cap_seg);
   }
   if (FILL) return;
   // block-local exclusive scan of the per-MD counts (in place), block total -> seg_block_base[A]
   __syncthreads();
   int carry = 0;
   for (int k0 = 0; k0 < nA; k0 += kSegThreads) {
-    const int k = k0 + threadIdx.x;
+    const int k = k0 + tid;
     const int v = (k < nA) ? seg_start[mdLo + k] : 0;
     int tot;
     const int ex = block_excl_scan<kSegThreads>(v, tot);
     if (k < nA) seg_start[mdLo + k] = carry + ex;
     carry += tot;
   }
-  if (threadIdx.x == 0) {
-    S.seg_block_base()[A] = carry;
-    if (nA > 0 && nOut) atomicAdd(&S.hdr()->cand[LST_SEG_], nOut * (unsigned long long)nA);
-  }
-  if (last_block_done(&S.hdr()->done[1], gridDim.x)) {
+  if (tid == 0) S.seg_block_base()[A] = carry;
+  if (last_block_done(&H->done[1], gridDim.x)) {
     const int total = block_scan_array<kSegThreads>(S.seg_block_base(), P.L.n_modules, -1);
-    if (threadIdx.x == 0) {
-      publish_total(S.hdr(), LST_SEG_, total, P.L.cap_seg);
-      seg_start[S.hdr()->n[LST_MD_]] = min(total, P.L.cap_seg);
+    if (tid == 0) {
+      publish_total(H, LST_SEG_, total, P.L.cap_seg);
+      seg_start[H->n[LST_MD_]] = min(total, P.L.cap_seg);
     }
   }
 }
@@ -355,7 +621,7 @@ __global__ void __launch_bounds__(kScanChunk) k_t3(const __grid_constant__ Param
   if (!FILL) {
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) cand += __shfl_down_sync(0xffffffffu, cand, d);
-    if (lane_id() == 0 && cand) atomicAdd(&H->cand[LST_T3_], cand);
+    if (lane_id() == 0 && cand) { atomicAdd(&H->cand[LST_T3_], cand); atomicAdd(&H->eval[LST_T3_], cand); }
     if (last_block_done(&H->done[2], gridDim.x)) {
       const int total = block_scan_array<kScanChunk>(S.t3_block_base(), nChunks, -1);
       if (threadIdx.x == 0) {
@@ -431,7 +697,7 @@ __global__ void __launch_bounds__(kScanChunk) k_t5(const __grid_constant__ Param
   if (!FILL) {
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) cand += __shfl_down_sync(0xffffffffu, cand, d);
-    if (lane_id() == 0 && cand) atomicAdd(&H->cand[LST_T5_], cand);
+    if (lane_id() == 0 && cand) { atomicAdd(&H->cand[LST_T5_], cand); atomicAdd(&H->eval[LST_T5_], cand); }
     if (last_block_done(&H->done[3], gridDim.x)) {
       const int total = block_scan_array<kScanChunk>(S.t5_block_base(), nChunks, -1);
       if (threadIdx.x == 0) {
@@ -488,19 +754,20 @@ __global__ void __launch_bounds__(256) k_pack_values(const __grid_constant__ Par
 // `ev` (optional, timing mode): ev[0] is recorded before the first kernel, ev[k + 1] after kernel k.
 #define LST_EV(k) do { if (ev) cudaEventRecord(ev[k], s); } while (0)
 
-int launch_bin(const Params& P, const HitInput& in, cudaStream_t s, cudaEvent_t* ev) {
-  const int nb = in.n > 0 ? min((in.n + 255) / 256, 1184) : 0;
-  int launches = 0;
+int launch_bin(const Params& P, const HitBatch& in, int n_batch, cudaStream_t s, cudaEvent_t* ev) {
+  int n_max = 0;
+  for (int b = 0; b < n_batch; ++b) n_max = max(n_max, in.ev[b].n);
+  const int per_event = max(8, 1184 / n_batch);
+  const dim3 g(max(1, min((n_max + 255) / 256, per_event)), (unsigned)n_batch);
   LST_EV(0);
-  if (nb) { k_bin_count<<<nb, 256, 0, s>>>(P, in); ++launches; }
+  k_bin_count<<<g, 256, 0, s>>>(P, in);   // + scan of the bin counts by the event's last block
   LST_EV(1);
-  k_bin_scan<<<1, 1024, 0, s>>>(P); ++launches;
   LST_EV(2);
-  if (nb) { k_bin_scatter<<<nb, 256, 0, s>>>(P, in); ++launches; }
+  k_bin_scatter<<<g, 256, 0, s>>>(P, in);
   LST_EV(3);
-  if (nb) { k_bin_order<<<(P.L.n_bins + 7) / 8, 256, 0, s>>>(P, in); ++launches; }
+  k_bin_order<<<dim3((P.L.n_bins + 7) / 8, (unsigned)n_batch), 256, 0, s>>>(P, in);
   LST_EV(4);
-  return launches;
+  return 3;
 }
 
 int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEvent_t* ev) {
@@ -510,10 +777,10 @@ int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEv
   LST_EV(0);
   switch (stage) {
     case LST_MD_: {
-      dim3 g((P.L.n_modules + kMdWarps - 1) / kMdWarps, nb);
-      k_md<false><<<g, kMdWarps * 32, 0, s>>>(P);
+      dim3 g(min(per_event, P.L.n_chunk_hits), nb);
+      k_md<false><<<g, kScanChunk, 0, s>>>(P);
       LST_EV(1);
-      k_md<true><<<g, kMdWarps * 32, 0, s>>>(P);
+      k_md<true><<<g, kScanChunk, 0, s>>>(P);
       break;
     }
     case LST_SEG_: {

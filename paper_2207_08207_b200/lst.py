@@ -20,7 +20,7 @@ LIB_PATH = os.path.join(HERE, "liblst.so")
 N_LAYERS = 6
 MD, SEG, T3, T5 = 0, 1, 2, 3
 KIND_NAMES = ("md", "seg", "t3", "t5")
-KERNEL_NAMES = ("bin_count", "bin_scan", "bin_scatter", "bin_order", "md_count", "md_fill", "seg_count", "seg_fill",
+KERNEL_NAMES = ("bin_count", "bin_unused", "bin_scatter", "bin_order", "md_count", "md_fill", "seg_count", "seg_fill",
                 "t3_count", "t3_fill", "t5_count", "t5_fill")
 HITS_PER_OBJECT = (2, 4, 6, 10)
 VALUES_PER_OBJECT = (4, 4, 2, 5)
@@ -91,7 +91,7 @@ class T5View(C.Structure):
 
 class Stats(C.Structure):
     _fields_ = [("n_hits", C.c_int32), ("needed", C.c_int64 * 4), ("candidates", C.c_int64 * 4),
-                ("overflow", C.c_int32), ("bad_hits", C.c_int32), ("stage_ms", C.c_float * 5), ("kernel_ms", C.c_float * 12)]
+                ("evaluated", C.c_int64 * 4), ("overflow", C.c_int32), ("bad_hits", C.c_int32), ("stage_ms", C.c_float * 5), ("kernel_ms", C.c_float * 12)]
 
 
 # every symbol include/lst.h declares: name -> (restype, argtypes)
@@ -101,6 +101,7 @@ SYMBOLS = {
     "lst_create": (C.c_int, [P(Geometry), P(ModuleMap), P(Config), P(C.c_void_p)]),
     "lst_destroy": (C.c_int, [C.c_void_p]),
     "lst_load_event": (C.c_int, [C.c_void_p, C.c_int, P(Hits), C.c_void_p]),
+    "lst_load_events": (C.c_int, [C.c_void_p, C.c_int, C.c_int, P(Hits), C.c_void_p]),
     "lst_run": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
     "lst_run_batch": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p]),
     "lst_run_stage": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]),
@@ -232,17 +233,28 @@ class Lst:
         return st
 
     # ---- the path ---------------------------------------------------------------------------
-    def load_event(self, slot: int, x, y, z, module, side, stream=None):
-        """Arrays: all numpy (host) or all torch CUDA tensors (device); dtypes f32/f32/f32/i32/u8."""
+    def _marshal(self, x, y, z, module, side):
         on_device = hasattr(x, "data_ptr") and getattr(x, "is_cuda", False)
         n = int(x.shape[0])
         if not on_device and not hasattr(x, "data_ptr"):
             x, y, z = (np.ascontiguousarray(a, np.float32) for a in (x, y, z))
             module = np.ascontiguousarray(module, np.int32)
             side = np.ascontiguousarray(side, np.uint8)
-        self._borrowed[slot] = (x, y, z, module, side)     # keep alive while the stream may read them
-        hits = Hits(n, _ptr(x), _ptr(y), _ptr(z), _ptr(module), _ptr(side), 1 if on_device else 0)
+        return (x, y, z, module, side), Hits(n, _ptr(x), _ptr(y), _ptr(z), _ptr(module), _ptr(side), 1 if on_device else 0)
+
+    def load_event(self, slot: int, x, y, z, module, side, stream=None):
+        """Arrays: all numpy (host) or all torch CUDA tensors (device); dtypes f32/f32/f32/i32/u8."""
+        keep, hits = self._marshal(x, y, z, module, side)
+        self._borrowed[slot] = keep                        # keep alive while the stream may read them
         return self._check(self.lib.lst_load_event(self.h, slot, C.byref(hits), _stream(stream)), "lst_load_event")
+
+    def load_events(self, first_slot: int, events, stream=None):
+        """events: sequence of (x, y, z, module, side) tuples; event b goes to slot first_slot + b."""
+        arr = (Hits * len(events))()
+        for b, ev in enumerate(events):
+            keep, arr[b] = self._marshal(*ev)
+            self._borrowed[first_slot + b] = keep
+        return self._check(self.lib.lst_load_events(self.h, first_slot, len(events), arr, _stream(stream)), "lst_load_events")
 
     def run(self, slot: int, stream=None):
         return self._check(self.lib.lst_run(self.h, slot, _stream(stream)), "lst_run")
@@ -264,7 +276,7 @@ class Lst:
         s = Stats()
         self._check(self.lib.lst_get_stats(self.h, slot, C.byref(s)), "lst_get_stats")
         return dict(n_hits=int(s.n_hits), needed=[int(v) for v in s.needed], candidates=[int(v) for v in s.candidates],
-                    overflow=int(s.overflow), bad_hits=int(s.bad_hits), stage_ms=[float(v) for v in s.stage_ms],
+                    evaluated=[int(v) for v in s.evaluated], overflow=int(s.overflow), bad_hits=int(s.bad_hits), stage_ms=[float(v) for v in s.stage_ms],
                     kernel_ms=[float(v) for v in s.kernel_ms])
 
     def mds(self, slot: int) -> dict:

@@ -59,10 +59,10 @@ def test_strerror_and_status_codes(lst_mod):
 def test_create_rejects_bad_arguments_before_any_cuda_call(lst_mod, geom, mmap):
     L = lst_mod.Lst
     def status(**kw):
-        args = dict(layer=geom.layer, row_offsets=mmap.row_offsets, targets=mmap.targets)
+        args = dict(layer=geom.layer, row_offsets=mmap.row_offsets, targets=mmap.targets, phi=geom.phi)
         args.update(kw)
         try:
-            L(args["layer"], args["row_offsets"], args["targets"], args.get("config"))
+            L(args["layer"], args["row_offsets"], args["targets"], args.get("config"), phi=args["phi"])
         except lst_mod.LstError as e:
             return e.status
         return 0
@@ -76,6 +76,16 @@ def test_create_rejects_bad_arguments_before_any_cuda_call(lst_mod, geom, mmap):
     assert status(row_offsets=bad_r) == lst_mod.ERR_ARG
     cfg = lst_mod.default_config(); cfg.n_slots = 0
     assert status(config=cfg) == lst_mod.ERR_ARG
+    assert status(phi=None) == lst_mod.ERR_ARG                     # module azimuths are required
+    bad_phi = geom.phi.copy(); bad_phi[7] = np.nan
+    assert status(phi=bad_phi) == lst_mod.ERR_ARG
+    # a map row longer than LST_MAX_ROW (64) is rejected
+    n1 = int(geom.n_phi[1]) * 24
+    big_t = np.concatenate([np.arange(int(geom.base[1]), int(geom.base[1]) + 65, dtype=np.int32), mmap.targets[mmap.row_offsets[1]:]])
+    big_r = mmap.row_offsets.copy(); big_r[1:] += 65 - (mmap.row_offsets[1] - mmap.row_offsets[0])
+    assert n1 > 65 and status(targets=big_t, row_offsets=big_r) == lst_mod.ERR_ARG
+    if __import__("torch").cuda.is_available():
+        assert status() == 0
 
 
 def test_no_cpu_fallback(lst_mod, geom, mmap):

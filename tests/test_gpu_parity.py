@@ -38,6 +38,8 @@ def check_event(ctx, o32, run_oracle, ev, slot=0, label=""):
     assert st["needed"] == ora.counts, (label, st, ora.counts)
     assert st["candidates"] == ora.candidates, (label, st, ora.candidates)
     assert st["n_hits"] == ev.n and st["overflow"] == 0 and st["bad_hits"] == 0
+    for k in range(4):      # windows only ever shrink the evaluated set, never below what passes
+        assert st["needed"][k] <= st["evaluated"][k] <= st["candidates"][k], (label, st)
     return worst, st
 
 
@@ -120,9 +122,8 @@ def test_device_input_batch_and_determinism(ctx, lstmod, o32, run_oracle, geom):
     stream = torch.cuda.Stream()
     dev = []
     for s, ev in enumerate(evs):
-        t = [torch.from_numpy(a).cuda() for a in (ev.x, ev.y, ev.z, ev.module, ev.side)]
-        dev.append(t)
-        ctx.load_event(s, *t, stream=stream)
+        dev.append([torch.from_numpy(a).cuda() for a in (ev.x, ev.y, ev.z, ev.module, ev.side)])
+    ctx.load_events(0, dev, stream=stream)               # one set of a0 launches for the 4 events
     ctx.run_batch(0, 4, stream)
     for s, ev in enumerate(evs):
         ctx.sync(s, stream)
@@ -202,3 +203,21 @@ def test_multi_stream_pipeline(ctx, o32, run_oracle, geom):
             ctx.sync(s, streams[s])
             got = parity.gpu_tables(ctx, s, streams[s])
             parity.compare(got, parity.oracle_tables(run_oracle(o32, evs[4 * rnd + s])), f"stream {s} round {rnd}")
+
+
+@pytest.mark.parametrize("how", ["shifted", "random", "near_pi"])
+def test_search_windows_never_change_the_result(lstmod, geom, mmap, o32, run_oracle, how):
+    """lst_geometry.phi only orders hits for the windowed search: with a
+    wrong reference azimuth per module -- shifted, random, or sitting on the +-pi cut -- windows
+    degrade to full scans where an azimuth wrap is possible and the object sets stay those of the
+    oracle."""
+    rng = np.random.default_rng(5)
+    phi = {"shifted": geom.phi + 1.0, "random": rng.uniform(-np.pi, np.pi, geom.n_modules),
+           "near_pi": geom.phi + np.pi - 0.05}[how]
+    cfg = lstmod.default_config()
+    cfg.n_slots = 1
+    c = lstmod.Lst(geom.layer, mmap.row_offsets, mmap.targets, cfg, phi=phi)
+    ev = synth.generate_event(geom, 1, 77, n_particles=1200)
+    _, st = check_event(c, o32, run_oracle, ev, label=how)
+    assert st["needed"][3] > 500
+    c.close()
