@@ -76,6 +76,7 @@ Layout make_layout(const lst_config& cfg, int n_modules) {
   L.cap_hits = cfg.cap_hits; L.cap_md = cfg.cap_md; L.cap_seg = cfg.cap_seg; L.cap_t3 = cfg.cap_t3; L.cap_t5 = cfg.cap_t5;
   L.n_chunk_hits = (cfg.cap_hits + kScanChunk - 1) / kScanChunk;
   L.n_chunk_seg = (cfg.cap_seg + kScanChunk - 1) / kScanChunk;
+  L.n_chunk_md = (cfg.cap_md + kSegChunkMd - 1) / kSegChunkMd;
   L.n_chunk_t3 = (cfg.cap_t3 + kScanChunk - 1) / kScanChunk;
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
@@ -88,10 +89,10 @@ Layout make_layout(const lst_config& cfg, int n_modules) {
   L.tmp_idx = take(4 * nh); L.tmp_key = take(4 * nh);
   L.hit4 = take(16 * nh); L.hit_key = take(4 * nh); L.hit_orig = take(4 * nh); L.hit_module = take(4 * nh);
   L.md_off = take(4 * (nh + 1)); L.md_block_base = take(4 * (size_t)(L.n_chunk_hits + 1));
-  L.md_start = take(4 * (size_t)(n_modules + 1));
+  L.md_start = take(4 * (size_t)(n_modules + 1)); L.mod_info = take(16 * (size_t)n_modules);
   L.md_anchor = take(16 * nm); L.md_aux = take(8 * nm); L.md_key = take(4 * nm); L.md_hits = take(8 * nm);
   L.md_out = take(8 * nm); L.md_module = take(4 * nm);
-  L.seg_start = take(4 * (nm + 1)); L.seg_block_base = take(4 * (size_t)(n_modules + 1));
+  L.seg_start = take(4 * (nm + 1)); L.seg_block_base = take(4 * (size_t)(L.n_chunk_md + 1));
   L.seg_md = take(8 * ns); L.seg_f = take(16 * ns);
   L.t3_start = take(4 * (ns + 1)); L.t3_block_base = take(4 * (size_t)(L.n_chunk_seg + 1));
   L.t3_pack = take(16 * n3); L.t3_seg = take(8 * n3); L.t3_chi2 = take(4 * n3);

@@ -40,6 +40,7 @@
 namespace lst {
 
 constexpr int kScanChunk = 256;   // owners (lower hits / segments / triplets) per block chunk
+constexpr int kSegChunkMd = 64;   // inner MDs per block of the segment kernel
 constexpr int kMaxBatch = 16;     // events per launch of the a0 kernels (pointer table in the launch parameters)
 constexpr int kMaxRow = 64;       // longest module-map row the segment kernel stages
 enum { LST_MD_ = 0, LST_SEG_ = 1, LST_T3_ = 2, LST_T5_ = 3 };  // == LST_MD .. LST_T5 of lst.h
@@ -64,12 +65,13 @@ struct Layout {
   int n_modules, n_bins;
   int cap_hits, cap_md, cap_seg, cap_t3, cap_t5;
   int n_chunk_hits, n_chunk_seg, n_chunk_t3;  // ceil(cap / kScanChunk)
+  int n_chunk_md;                             // ceil(cap_md / kSegChunkMd)
   // byte offsets from the slot base (all multiples of 256)
   size_t hdr, bin_start, bin_cursor;          // hdr, bin_start and bin_cursor are contiguous: one memset
   size_t reset_bytes;                         // bytes to zero at lst_load_event, from hdr
   size_t in_x, in_y, in_z, in_module, in_side;// staging of host input
   size_t tmp_idx, tmp_key, hit4, hit_key, hit_orig, hit_module;
-  size_t md_off, md_block_base, md_start, md_anchor, md_aux, md_key, md_hits, md_out, md_module;
+  size_t md_off, md_block_base, md_start, mod_info, md_anchor, md_aux, md_key, md_hits, md_out, md_module;
   size_t seg_start, seg_block_base, seg_md, seg_f;
   size_t t3_start, t3_block_base, t3_pack, t3_seg, t3_chi2;
   size_t t5_start, t5_block_base, t5_md, t5_t3, t5_f;
@@ -111,6 +113,7 @@ struct Slot {
   __device__ __forceinline__ int* md_off() const { return at<int>(L.md_off); }
   __device__ __forceinline__ int* md_block_base() const { return at<int>(L.md_block_base); }
   __device__ __forceinline__ int* md_start() const { return at<int>(L.md_start); }
+  __device__ __forceinline__ int4* mod_info() const { return at<int4>(L.mod_info); }
   __device__ __forceinline__ float4* md_anchor() const { return at<float4>(L.md_anchor); }
   __device__ __forceinline__ float2* md_aux() const { return at<float2>(L.md_aux); }
   __device__ __forceinline__ float* md_key() const { return at<float>(L.md_key); }

@@ -362,7 +362,15 @@ __global__ void __launch_bounds__(kScanChunk) k_md(const __grid_constant__ Param
     const int total = H->n[LST_MD_];
     for (int m = blockIdx.x * kScanChunk + threadIdx.x; m <= nmod; m += gridDim.x * kScanChunk) {
       const int ls = (m < nmod) ? (int)bs[m] : nLower;
-      S.md_start()[m] = (ls < nLower) ? min(block_base[ls / kScanChunk] + md_off[ls], P.L.cap_md) : total;
+      const int b0 = (ls < nLower) ? min(block_base[ls / kScanChunk] + md_off[ls], P.L.cap_md) : total;
+      S.md_start()[m] = b0;
+      if (m < nmod) {
+        // (first MD, end MD, key range of the module's lower hits >= key range of its MDs)
+        const int le = (int)bs[m + 1];
+        const int b1 = (le < nLower) ? min(block_base[le / kScanChunk] + md_off[le], P.L.cap_md) : total;
+        const bool any = le > ls;
+        S.mod_info()[m] = make_int4(b0, b1, __float_as_int(any ? hkey[ls] : 3.0e38f), __float_as_int(any ? hkey[le - 1] : -3.0e38f));
+      }
     }
   } else {
 #pragma unroll
@@ -376,96 +384,111 @@ __global__ void __launch_bounds__(kScanChunk) k_md(const __grid_constant__ Param
 }
 
 // ------------------------------------------------------------------------------------------
-// a2: segments. One block per inner module A.  The module's mini-doublets are taken in tiles;
-// for a tile, (1) every (inner MD, connected module) pair finds its window of outer MDs by a
+// a2: segments. One block per chunk of kSegChunk consecutive inner MDs (they may sit in several
+// modules).  (1) every (inner MD, connected module) pair finds its window of outer MDs by a
 // binary search in the connected module's key-ordered MD list, (2) a block scan of the window
 // sizes numbers the candidates in (inner MD, outer MD) order, (3) one thread per candidate
 // evaluates the SPEC selection.  Segments come out ordered by (inner MD, outer MD).
 // ------------------------------------------------------------------------------------------
 constexpr int kSegThreads = 128;
-constexpr int kSegTile = 128;    // inner MDs per tile
-constexpr int kSegPairs = 2048;  // (inner MD, connected module) pairs per tile
+constexpr int kSegChunk = kSegChunkMd;
+constexpr int kSegPairs = 2048;  // (inner MD, connected module) pairs per tile (>= kMaxRow)
 
 template <bool FILL>
 __global__ void __launch_bounds__(kSegThreads) k_seg(const __grid_constant__ Params P) {
-  __shared__ int tB0[kMaxRow], tB1[kMaxRow];
-  __shared__ float tOff[kMaxRow], tKmin[kMaxRow], tKmax[kMaxRow];
-  __shared__ float4 iAnchor[kSegTile];
-  __shared__ float2 iAux[kSegTile];
-  __shared__ float iKey[kSegTile], iDlo[kSegTile], iDhi[kSegTile];
-  __shared__ int kCnt[kSegTile];
+  __shared__ float4 iAnchor[kSegChunk];
+  __shared__ float2 iAux[kSegChunk];
+  __shared__ float iKey[kSegChunk], iDlo[kSegChunk], iDhi[kSegChunk];
+  __shared__ int iRow0[kSegChunk], iLayer[kSegChunk];
+  __shared__ int pairBase[kSegChunk + 1];
+  __shared__ int kCnt[kSegChunk];
   __shared__ int pLo[kSegPairs], pOff[kSegPairs + 1];
+  __shared__ unsigned char pK[kSegPairs];
   __shared__ int warpTot[kSegThreads / 32];
+  __shared__ float rMinO[6], rMaxO[6];
 
   Slot S(P, blockIdx.y);
   SlotHeader* H = S.hdr();
-  const int A = blockIdx.x;
-  const int* md_start = S.md_start();
+  const int nMD = H->n[LST_MD_];
+  const int nChunks = (nMD + kSegChunk - 1) / kSegChunk;
   int* seg_start = S.seg_start();
-  const int mdLo = md_start[A], nA = md_start[A + 1] - mdLo;
-  const int row0 = P.map_offsets[A], nT = P.map_offsets[A + 1] - row0;
+  int* block_base = S.seg_block_base();
   const float4* anchor = S.md_anchor();
   const float2* aux = S.md_aux();
   const float* mkey = S.md_key();
+  const int4* mod_info = S.mod_info();
   const int tid = threadIdx.x, warp = tid >> 5;
-  int blockTotal = 0;  // segments of this block so far (uniform across the block)
+  if (tid < 6) {
+    rMinO[tid] = r_min_of(H, 0, tid);
+    rMaxO[tid] = r_max_of(H, 0, tid);
+  }
+  unsigned long long space = 0, evals = 0;
 
-  if (nA > 0 && nT > 0) {
-    const int layer = P.mod_layer[A];
-    const float rMinO = r_min_of(H, 0, layer + 1), rMaxO = r_max_of(H, 0, layer + 1);
-    const int blockBase = FILL ? S.seg_block_base()[A] : 0;
-    // connected modules: MD range, azimuth offset, key range
-    if (tid < nT) {
-      const int Bm = P.map_targets[row0 + tid];
-      const int b0 = md_start[Bm], b1 = md_start[Bm + 1];
-      tB0[tid] = b0;
-      tB1[tid] = b1;
-      tOff[tid] = P.map_dphi[row0 + tid];
-      tKmin[tid] = (b1 > b0) ? mkey[b0] : 3.0e38f;
-      tKmax[tid] = (b1 > b0) ? mkey[b1 - 1] : -3.0e38f;
+  for (int c = blockIdx.x; c < nChunks; c += gridDim.x) {
+    const int i0 = c * kSegChunk, kn = min(kSegChunk, nMD - i0);
+    __syncthreads();  // previous chunk fully consumed (and rMinO / rMaxO visible)
+    int nt = 0;
+    if (tid < kn) {
+      const int i = i0 + tid;
+      const float4 a = anchor[i];
+      const float2 x = aux[i];
+      const int A = S.md_module()[i];
+      const int row0 = P.map_offsets[A];
+      nt = P.map_offsets[A + 1] - row0;
+      const int layer = P.mod_layer[A];
+      float dlo = 1.0f, dhi = -1.0f;
+      if (nt > 0) seg_window(P.cuts, layer, a.w, x.x, x.y, rMinO[layer + 1], rMaxO[layer + 1], dlo, dhi);
+      iAnchor[tid] = a;
+      iAux[tid] = x;
+      iKey[tid] = mkey[i];
+      iDlo[tid] = dlo;
+      iDhi[tid] = dhi;
+      iRow0[tid] = row0;
+      iLayer[tid] = layer;
+    }
+    if (tid < kSegChunk) kCnt[tid] = 0;
+    {
+      int tot;
+      const int ex = block_excl_scan<kSegThreads>(nt, tot);
+      if (tid < kSegChunk) pairBase[tid] = ex;
+      if (tid == 0) pairBase[kSegChunk] = tot;
     }
     __syncthreads();
-    if (!FILL && tid == 0) {
-      unsigned long long nOut = 0;
-      for (int t = 0; t < nT; ++t) nOut += (unsigned long long)(tB1[t] - tB0[t]);
-      if (nOut) atomicAdd(&H->cand[LST_SEG_], nOut * (unsigned long long)nA);
-    }
-    const int kTile = min(kSegTile, kSegPairs / nT);
-    unsigned long long evals = 0;
-    for (int k0 = 0; k0 < nA; k0 += kTile) {
-      const int kn = min(kTile, nA - k0);
-      for (int k = tid; k < kn; k += kSegThreads) {
-        const int i = mdLo + k0 + k;
-        const float4 a = anchor[i];
-        const float2 x = aux[i];
-        iAnchor[k] = a;
-        iAux[k] = x;
-        iKey[k] = mkey[i];
-        float dlo, dhi;
-        seg_window(P.cuts, layer, a.w, x.x, x.y, rMinO, rMaxO, dlo, dhi);
-        iDlo[k] = dlo;
-        iDhi[k] = dhi;
-        kCnt[k] = 0;
-      }
-      __syncthreads();
+    const int blockBase = FILL ? block_base[c] : 0;
+    int blockTotal = 0;  // segments of this chunk so far (uniform across the block)
+    int kBeg = 0;
+    while (kBeg < kn) {
+      // tile = inner MDs [kBeg, kEnd) with at most kSegPairs pairs
+      const int p0 = pairBase[kBeg];
+      int kEnd = kBeg + 1;
+      while (kEnd < kn && pairBase[kEnd + 1] - p0 <= kSegPairs) ++kEnd;
+      const int nPairs = pairBase[kEnd] - p0;
       // (1) windows
-      const int nPairs = kn * nT;
-      for (int p = tid; p < nPairs; p += kSegThreads) {
-        const int k = p / nT, t = p - k * nT;
-        const int b0 = tB0[t], b1 = tB1[t];
-        int lo = b0, n = 0;
+      for (int q = tid; q < nPairs; q += kSegThreads) {
+        const int p = p0 + q;
+        int lo = kBeg, hi = kEnd;  // last k in [kBeg, kEnd) with pairBase[k] <= p
+        while (hi - lo > 1) {
+          const int mid = (lo + hi) >> 1;
+          if (pairBase[mid] <= p) lo = mid; else hi = mid;
+        }
+        const int k = lo, e = iRow0[k] + (p - pairBase[k]);
+        const int4 info = mod_info[P.map_targets[e]];
+        const int b0 = info.x, b1 = info.y;
+        space += (unsigned long long)(b1 - b0);
+        int first = b0, n = 0;
         const float dlo = iDlo[k], dhi = iDhi[k];
         if (b1 > b0 && dlo <= dhi) {
-          const float c0 = iKey[k] + tOff[t];
+          const float c0 = iKey[k] + P.map_dphi[e];
           if (!(fabsf(c0) + fmaxf(fabsf(dlo), fabsf(dhi)) < 3.0f)) {
             n = b1 - b0;  // azimuth wrap possible (never with a sane geometry): no window
-          } else if (c0 + dhi >= tKmin[t] && c0 + dlo <= tKmax[t]) {
-            lo = lower_bound_f(mkey, b0, b1, c0 + dlo);
-            n = upper_bound_f(mkey, lo, b1, c0 + dhi) - lo;
+          } else if (c0 + dhi >= __int_as_float(info.z) && c0 + dlo <= __int_as_float(info.w)) {
+            first = lower_bound_f(mkey, b0, b1, c0 + dlo);
+            n = upper_bound_f(mkey, first, b1, c0 + dhi) - first;
           }
         }
-        pLo[p] = lo;
-        pOff[p] = n;
+        pLo[q] = first;
+        pOff[q] = n;
+        pK[q] = (unsigned char)k;
       }
       __syncthreads();
       // (2) exclusive scan of the window sizes
@@ -474,11 +497,11 @@ __global__ void __launch_bounds__(kSegThreads) k_seg(const __grid_constant__ Par
         const int ipt = (nPairs + kSegThreads - 1) / kSegThreads;
         const int lo = min(nPairs, tid * ipt), hi = min(nPairs, lo + ipt);
         int s = 0;
-        for (int p = lo; p < hi; ++p) s += pOff[p];
+        for (int q = lo; q < hi; ++q) s += pOff[q];
         int run = block_excl_scan<kSegThreads>(s, nCand);
-        for (int p = lo; p < hi; ++p) {
-          const int v = pOff[p];
-          pOff[p] = run;
+        for (int q = lo; q < hi; ++q) {
+          const int v = pOff[q];
+          pOff[q] = run;
           run += v;
         }
         if (tid == 0) pOff[nPairs] = nCand;
@@ -487,22 +510,22 @@ __global__ void __launch_bounds__(kSegThreads) k_seg(const __grid_constant__ Par
       evals += (tid == 0) ? (unsigned long long)nCand : 0ull;
       // (3) one thread per candidate
       for (int c0 = 0; c0 < nCand; c0 += kSegThreads) {
-        const int c = c0 + tid;
+        const int cc = c0 + tid;
         bool pass = false;
         SegOut so;
         float4 ai, ao;
         int k = 0, o = 0;
-        if (c < nCand) {
-          int lo = 0, hi = nPairs;  // last p with pOff[p] <= c
+        if (cc < nCand) {
+          int lo = 0, hi = nPairs;  // last q with pOff[q] <= cc
           while (hi - lo > 1) {
             const int mid = (lo + hi) >> 1;
-            if (pOff[mid] <= c) lo = mid; else hi = mid;
+            if (pOff[mid] <= cc) lo = mid; else hi = mid;
           }
-          k = lo / nT;
-          o = pLo[lo] + (c - pOff[lo]);
+          k = pK[lo];
+          o = pLo[lo] + (cc - pOff[lo]);
           ai = iAnchor[k];
           ao = anchor[o];
-          pass = seg_select(P.cuts, layer, ai, iAux[k], ao, aux[o], so);
+          pass = seg_select(P.cuts, iLayer[k], ai, iAux[k], ao, aux[o], so);
         }
         if (!FILL) {
           if (pass) atomicAdd(&kCnt[k], 1);
@@ -520,7 +543,7 @@ __global__ void __launch_bounds__(kSegThreads) k_seg(const __grid_constant__ Par
           if (pass) {
             const int pos = blockBase + blockTotal + before + __popc(bal & lanemask_lt());
             if (pos < P.L.cap_seg) {
-              S.seg_md()[pos] = make_int2(mdLo + k0 + k, o);
+              S.seg_md()[pos] = make_int2(i0 + k, o);
               S.seg_f()[pos] = make_float4(so.sinS, so.z0,
                                            atan2f(ai.x * ao.y - ai.y * ao.x, ai.x * ao.x + ai.y * ao.y),
                                            atan2f(so.cross, so.dot));
@@ -530,41 +553,31 @@ __global__ void __launch_bounds__(kSegThreads) k_seg(const __grid_constant__ Par
           __syncthreads();
         }
       }
-      if (!FILL) {
-        __syncthreads();
-        for (int k = tid; k < kn; k += kSegThreads) seg_start[mdLo + k0 + k] = kCnt[k];
-      }
       __syncthreads();
+      kBeg = kEnd;
     }
-    if (!FILL && tid == 0 && evals) atomicAdd(&H->eval[LST_SEG_], evals);
-    if (FILL) {
-      // local offsets (left by the count pass) -> global segment index of each inner MD
-      for (int k = tid; k < nA; k += kSegThreads) seg_start[mdLo + k] = min(blockBase + seg_start[mdLo + k], P.L.cap_seg);
+    // per inner MD: count -> chunk-local offset (count pass) -> global segment index (fill pass)
+    if (!FILL) {
+      const int v = (tid < kn) ? kCnt[tid] : 0;
+      int tot;
+      const int ex = block_excl_scan<kSegThreads>(v, tot);
+      if (tid < kn) seg_start[i0 + tid] = ex;
+      if (tid == 0) block_base[c] = tot;
+    } else if (tid < kn) {
+      seg_start[i0 + tid] = min(blockBase + seg_start[i0 + tid], P.L.cap_seg);
     }
-  } else if (!FILL) {
-    for (int k = tid; k < nA; k += kSegThreads) seg_start[mdLo + k] = 0;
-  } else {
-    const int blockBase = S.seg_block_base()[A];
-    for (int k = tid; k < nA; k += kSegThreads) seg_start[mdLo + k] = min(blockBase, P.L.cap_seg);
   }
-  if (FILL) return;
-  // block-local exclusive scan of the per-MD counts (in place), block total -> seg_block_base[A]
-  __syncthreads();
-  int carry = 0;
-  for (int k0 = 0; k0 < nA; k0 += kSegThreads) {
-    const int k = k0 + tid;
-    const int v = (k < nA) ? seg_start[mdLo + k] : 0;
-    int tot;
-    const int ex = block_excl_scan<kSegThreads>(v, tot);
-    if (k < nA) seg_start[mdLo + k] = carry + ex;
-    carry += tot;
-  }
-  if (tid == 0) S.seg_block_base()[A] = carry;
-  if (last_block_done(&H->done[1], gridDim.x)) {
-    const int total = block_scan_array<kSegThreads>(S.seg_block_base(), P.L.n_modules, -1);
-    if (tid == 0) {
-      publish_total(H, LST_SEG_, total, P.L.cap_seg);
-      seg_start[H->n[LST_MD_]] = min(total, P.L.cap_seg);
+  if (!FILL) {
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) space += __shfl_down_sync(0xffffffffu, space, d);
+    if (lane_id() == 0 && space) atomicAdd(&H->cand[LST_SEG_], space);
+    if (tid == 0 && evals) atomicAdd(&H->eval[LST_SEG_], evals);
+    if (last_block_done(&H->done[1], gridDim.x)) {
+      const int total = block_scan_array<kSegThreads>(block_base, nChunks, -1);
+      if (tid == 0) {
+        publish_total(H, LST_SEG_, total, P.L.cap_seg);
+        seg_start[nMD] = min(total, P.L.cap_seg);
+      }
     }
   }
 }
@@ -784,7 +797,7 @@ int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEv
       break;
     }
     case LST_SEG_: {
-      dim3 g(P.L.n_modules, nb);
+      dim3 g(min(2 * per_event, P.L.n_chunk_md), nb);   // 128-thread blocks: twice as many per SM
       k_seg<false><<<g, kSegThreads, 0, s>>>(P);
       LST_EV(1);
       k_seg<true><<<g, kSegThreads, 0, s>>>(P);
