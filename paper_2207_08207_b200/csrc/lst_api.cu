@@ -83,6 +83,7 @@ Layout make_layout(const lst_config& cfg, int n_modules) {
   L.hdr = take(sizeof(SlotHeader));
   L.bin_start = take(sizeof(int) * (size_t)(L.n_bins + 1));
   L.bin_cursor = take(sizeof(int) * (size_t)L.n_bins);
+  L.lb_seg = take(8 * (size_t)(L.n_chunk_md + 1));
   L.reset_bytes = off - L.hdr;
   const size_t nh = (size_t)cfg.cap_hits, nm = (size_t)cfg.cap_md, ns = (size_t)cfg.cap_seg, n3 = (size_t)cfg.cap_t3, n5 = (size_t)cfg.cap_t5;
   L.in_x = take(4 * nh); L.in_y = take(4 * nh); L.in_z = take(4 * nh); L.in_module = take(4 * nh); L.in_side = take(nh);
@@ -174,6 +175,7 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
   if (cfg_in) cfg = *cfg_in; else lst_default_config(&cfg);
   const int n = g->n_modules;
   if (n <= 0 || n > (1 << 24) || m->n_modules != n || !g->layer || !g->phi || !m->row_offsets) return LST_ERR_ARG;
+  if (cfg.cap_md > (1 << 24)) return LST_ERR_ARG;  /* MD indices are packed into 24 bits by the segment kernel */
   if (cfg.n_slots < 1 || cfg.cap_hits < 1 || cfg.cap_md < 1 || cfg.cap_seg < 1 || cfg.cap_t3 < 1 || cfg.cap_t5 < 1) return LST_ERR_ARG;
   for (int i = 0; i < n; ++i)
     if (g->layer[i] < 0 || g->layer[i] >= LST_N_LAYERS) return LST_ERR_ARG;

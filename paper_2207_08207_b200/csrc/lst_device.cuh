@@ -59,6 +59,7 @@ struct SlotHeader {
   int r_min_inv[2][6];
   int r_max[2][6];
   unsigned int done[8];           // "last block done" tickets, self-resetting
+  unsigned int ticket[4];         // next chunk of the single-pass kernels (zeroed with the header)
 };
 
 struct Layout {
@@ -67,7 +68,7 @@ struct Layout {
   int n_chunk_hits, n_chunk_seg, n_chunk_t3;  // ceil(cap / kScanChunk)
   int n_chunk_md;                             // ceil(cap_md / kSegChunkMd)
   // byte offsets from the slot base (all multiples of 256)
-  size_t hdr, bin_start, bin_cursor;          // hdr, bin_start and bin_cursor are contiguous: one memset
+  size_t hdr, bin_start, bin_cursor, lb_seg;  // contiguous: zeroed by one memset at lst_load_event
   size_t reset_bytes;                         // bytes to zero at lst_load_event, from hdr
   size_t in_x, in_y, in_z, in_module, in_side;// staging of host input
   size_t tmp_idx, tmp_key, hit4, hit_key, hit_orig, hit_module;
@@ -104,6 +105,7 @@ struct Slot {
   __device__ __forceinline__ SlotHeader* hdr() const { return at<SlotHeader>(L.hdr); }
   __device__ __forceinline__ unsigned* bin_start() const { return at<unsigned>(L.bin_start); }
   __device__ __forceinline__ unsigned* bin_cursor() const { return at<unsigned>(L.bin_cursor); }
+  __device__ __forceinline__ unsigned long long* lb_seg() const { return at<unsigned long long>(L.lb_seg); }
   __device__ __forceinline__ int* tmp_idx() const { return at<int>(L.tmp_idx); }
   __device__ __forceinline__ float* tmp_key() const { return at<float>(L.tmp_key); }
   __device__ __forceinline__ float4* hit4() const { return at<float4>(L.hit4); }

@@ -384,202 +384,322 @@ __global__ void __launch_bounds__(kScanChunk) k_md(const __grid_constant__ Param
 }
 
 // ------------------------------------------------------------------------------------------
-// a2: segments. One block per chunk of kSegChunk consecutive inner MDs (they may sit in several
-// modules).  (1) every (inner MD, connected module) pair finds its window of outer MDs by a
-// binary search in the connected module's key-ordered MD list, (2) a block scan of the window
-// sizes numbers the candidates in (inner MD, outer MD) order, (3) one thread per candidate
-// evaluates the SPEC selection.  Segments come out ordered by (inner MD, outer MD).
+// single-pass ordered output: chunks of owners are handed out in order by a ticket; a block
+// learns where its chunk's objects start by decoupled look-back over the totals of the chunks
+// before it (each chunk publishes its total as soon as it is known, so nothing waits on a
+// block that has not started).  status word: bits 63:62 = 1 total only, 2 = inclusive prefix.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ void st_status(unsigned long long* p, unsigned long long v) {
+  asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ unsigned long long ld_status(const unsigned long long* p) {
+  unsigned long long v;
+  asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+  return v;
+}
+// Called by all lanes of ONE warp. Returns the number of objects of chunks 0 .. c-1.
+__device__ __forceinline__ int lookback_exclusive(unsigned long long* status, int c, int total) {
+  const int lane = (int)lane_id();
+  if (lane == 0) st_status(status + c, ((c == 0 ? 2ull : 1ull) << 62) | (unsigned)total);
+  if (c == 0) return 0;
+  int sum = 0;
+  for (int j = c - 1;; j -= 32) {
+    const int idx = j - lane;
+    unsigned long long v = (idx >= 0) ? ld_status(status + idx) : (2ull << 62);
+    while (__any_sync(0xffffffffu, (v >> 62) == 0)) {
+      if ((v >> 62) == 0) v = ld_status(status + idx);
+    }
+    const unsigned pmask = __ballot_sync(0xffffffffu, (v >> 62) == 2);
+    const int firstP = pmask ? __ffs(pmask) - 1 : 32;
+    int contrib = (lane <= firstP) ? (int)(unsigned)(v & 0xffffffffull) : 0;
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) contrib += __shfl_xor_sync(0xffffffffu, contrib, d);
+    sum += contrib;
+    if (pmask) break;
+  }
+  if (lane == 0) st_status(status + c, (2ull << 62) | (unsigned)(sum + total));
+  return sum;
+}
+
+// Exclusive max-scan of one non-negative int per thread over the block (0 for thread 0).
+// Ends with a barrier.
+template <int NT>
+__device__ __forceinline__ int block_excl_scan_max(int v) {
+  __shared__ int warp_max[NT / 32];
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const int t = __shfl_up_sync(0xffffffffu, v, d);
+    if ((int)lane_id() >= d) v = max(v, t);
+  }
+  const int w = threadIdx.x >> 5;
+  if (lane_id() == 31) warp_max[w] = v;
+  int ex = __shfl_up_sync(0xffffffffu, v, 1);
+  if (lane_id() == 0) ex = 0;
+  __syncthreads();
+#pragma unroll
+  for (int i = 0; i < NT / 32; ++i) ex = (i < w) ? max(ex, warp_max[i]) : ex;
+  __syncthreads();
+  return ex;
+}
+
+// ------------------------------------------------------------------------------------------
+// a2: segments, single pass. One block per chunk of kSegChunk consecutive inner MDs (they may
+// sit in several modules).  (1) every (inner MD, connected module) pair finds its window of
+// outer MDs by a binary search in the connected module's key-ordered MD list, (2) a block scan
+// of the window sizes numbers the candidates in (inner MD, outer MD) order, (3) one thread per
+// candidate evaluates the SPEC selection ONCE; what passes is kept in shared memory, in order,
+// until the look-back has told the block where its segments start.  Segments come out ordered
+// by (inner MD, outer MD).
 // ------------------------------------------------------------------------------------------
 constexpr int kSegThreads = 128;
-constexpr int kSegChunk = kSegChunkMd;
-constexpr int kSegPairs = 2048;  // (inner MD, connected module) pairs per tile (>= kMaxRow)
+constexpr int kSegChunk = kSegChunkMd;  // inner MDs per chunk
+constexpr int kSegPairs = 1024;  // (inner MD, connected module) pairs per tile (>= kMaxRow)
+constexpr int kSegCand = 1024;   // candidates per lookup tile
+constexpr int kSegStash = 512;   // segments of a chunk kept in shared memory
 
-template <bool FILL>
-__global__ void __launch_bounds__(kSegThreads) k_seg(const __grid_constant__ Params P) {
-  __shared__ float4 iAnchor[kSegChunk];
-  __shared__ float2 iAux[kSegChunk];
-  __shared__ float iKey[kSegChunk], iDlo[kSegChunk], iDhi[kSegChunk];
-  __shared__ int iRow0[kSegChunk], iLayer[kSegChunk];
-  __shared__ int pairBase[kSegChunk + 1];
-  __shared__ int kCnt[kSegChunk];
-  __shared__ int pLo[kSegPairs], pOff[kSegPairs + 1];
-  __shared__ unsigned char pK[kSegPairs];
-  __shared__ int warpTot[kSegThreads / 32];
-  __shared__ float rMinO[6], rMaxO[6];
+struct SegShared {
+  float4 iAnchor[kSegChunk];
+  float2 iAux[kSegChunk];
+  float iKey[kSegChunk], iDlo[kSegChunk], iDhi[kSegChunk];
+  int iRow0[kSegChunk], iNt[kSegChunk], iLayer[kSegChunk], kCnt[kSegChunk];
+  int pLo[kSegPairs], pOff[kSegPairs + 1];
+  unsigned short cPair[kSegCand];
+  int stKO[kSegStash];
+  float4 stV[kSegStash];
+  int warpTot[kSegThreads / 32];
+  float rMinO[6], rMaxO[6];
+  int chunk, base, tMax;
+};
 
-  Slot S(P, blockIdx.y);
-  SlotHeader* H = S.hdr();
-  const int nMD = H->n[LST_MD_];
-  const int nChunks = (nMD + kSegChunk - 1) / kSegChunk;
-  int* seg_start = S.seg_start();
-  int* block_base = S.seg_block_base();
+// Walks the chunk's candidates in order. direct = false: passing candidates go to the stash
+// (positions < kSegStash) and are counted per inner MD; direct = true: they are written to
+// global memory at `base` + position.  Returns the number of passing candidates.
+__device__ __forceinline__ int seg_walk(const Params& P, const Slot& S, SegShared& sh, int i0, int kn, int tStar,
+                                        bool direct, int base, unsigned long long& space, unsigned long long& evals) {
   const float4* anchor = S.md_anchor();
   const float2* aux = S.md_aux();
   const float* mkey = S.md_key();
   const int4* mod_info = S.mod_info();
   const int tid = threadIdx.x, warp = tid >> 5;
-  if (tid < 6) {
-    rMinO[tid] = r_min_of(H, 0, tid);
-    rMaxO[tid] = r_max_of(H, 0, tid);
-  }
-  unsigned long long space = 0, evals = 0;
-
-  for (int c = blockIdx.x; c < nChunks; c += gridDim.x) {
-    const int i0 = c * kSegChunk, kn = min(kSegChunk, nMD - i0);
-    __syncthreads();  // previous chunk fully consumed (and rMinO / rMaxO visible)
-    int nt = 0;
-    if (tid < kn) {
-      const int i = i0 + tid;
-      const float4 a = anchor[i];
-      const float2 x = aux[i];
-      const int A = S.md_module()[i];
-      const int row0 = P.map_offsets[A];
-      nt = P.map_offsets[A + 1] - row0;
-      const int layer = P.mod_layer[A];
-      float dlo = 1.0f, dhi = -1.0f;
-      if (nt > 0) seg_window(P.cuts, layer, a.w, x.x, x.y, rMinO[layer + 1], rMaxO[layer + 1], dlo, dhi);
-      iAnchor[tid] = a;
-      iAux[tid] = x;
-      iKey[tid] = mkey[i];
-      iDlo[tid] = dlo;
-      iDhi[tid] = dhi;
-      iRow0[tid] = row0;
-      iLayer[tid] = layer;
-    }
-    if (tid < kSegChunk) kCnt[tid] = 0;
-    {
-      int tot;
-      const int ex = block_excl_scan<kSegThreads>(nt, tot);
-      if (tid < kSegChunk) pairBase[tid] = ex;
-      if (tid == 0) pairBase[kSegChunk] = tot;
-    }
-    __syncthreads();
-    const int blockBase = FILL ? block_base[c] : 0;
-    int blockTotal = 0;  // segments of this chunk so far (uniform across the block)
-    int kBeg = 0;
-    while (kBeg < kn) {
-      // tile = inner MDs [kBeg, kEnd) with at most kSegPairs pairs
-      const int p0 = pairBase[kBeg];
-      int kEnd = kBeg + 1;
-      while (kEnd < kn && pairBase[kEnd + 1] - p0 <= kSegPairs) ++kEnd;
-      const int nPairs = pairBase[kEnd] - p0;
-      // (1) windows
-      for (int q = tid; q < nPairs; q += kSegThreads) {
-        const int p = p0 + q;
-        int lo = kBeg, hi = kEnd;  // last k in [kBeg, kEnd) with pairBase[k] <= p
-        while (hi - lo > 1) {
-          const int mid = (lo + hi) >> 1;
-          if (pairBase[mid] <= p) lo = mid; else hi = mid;
-        }
-        const int k = lo, e = iRow0[k] + (p - pairBase[k]);
+  const unsigned magic = 0xffffffffu / (unsigned)tStar + 1u;  // q / tStar == umulhi(q, magic) for q < 65536
+  const int kTile = min(kn, kSegPairs / tStar);
+  int running = 0;  // passing candidates so far (uniform across the block)
+  for (int kb = 0; kb < kn; kb += kTile) {
+    const int kt = min(kTile, kn - kb), nPairs = kt * tStar;
+    // (1) windows
+    for (int q = tid; q < nPairs; q += kSegThreads) {
+      const int kk = (int)__umulhi((unsigned)q, magic), t = q - kk * tStar, k = kb + kk;
+      int first = 0, n = 0;
+      if (t < sh.iNt[k]) {
+        const int e = sh.iRow0[k] + t;
         const int4 info = mod_info[P.map_targets[e]];
         const int b0 = info.x, b1 = info.y;
-        space += (unsigned long long)(b1 - b0);
-        int first = b0, n = 0;
-        const float dlo = iDlo[k], dhi = iDhi[k];
+        if (!direct) space += (unsigned long long)(b1 - b0);
+        const float dlo = sh.iDlo[k], dhi = sh.iDhi[k];
         if (b1 > b0 && dlo <= dhi) {
-          const float c0 = iKey[k] + P.map_dphi[e];
+          const float c0 = sh.iKey[k] + P.map_dphi[e];
           if (!(fabsf(c0) + fmaxf(fabsf(dlo), fabsf(dhi)) < 3.0f)) {
-            n = b1 - b0;  // azimuth wrap possible (never with a sane geometry): no window
+            first = b0;  // azimuth wrap possible (never with a sane geometry): no window
+            n = b1 - b0;
           } else if (c0 + dhi >= __int_as_float(info.z) && c0 + dlo <= __int_as_float(info.w)) {
             first = lower_bound_f(mkey, b0, b1, c0 + dlo);
             n = upper_bound_f(mkey, first, b1, c0 + dhi) - first;
           }
         }
-        pLo[q] = first;
-        pOff[q] = n;
-        pK[q] = (unsigned char)k;
       }
+      sh.pLo[q] = first;
+      sh.pOff[q] = n;
+    }
+    __syncthreads();
+    // (2) exclusive scan of the window sizes
+    int nCand;
+    {
+      const int ipt = (nPairs + kSegThreads - 1) / kSegThreads;
+      const int lo = min(nPairs, tid * ipt), hi = min(nPairs, lo + ipt);
+      int s = 0;
+      for (int q = lo; q < hi; ++q) s += sh.pOff[q];
+      int run = block_excl_scan<kSegThreads>(s, nCand);
+      for (int q = lo; q < hi; ++q) {
+        const int v = sh.pOff[q];
+        sh.pOff[q] = run;
+        run += v;
+      }
+      if (tid == 0) sh.pOff[nPairs] = nCand;
+    }
+    __syncthreads();
+    if (!direct && tid == 0) evals += (unsigned long long)nCand;
+    for (int cb = 0; cb < nCand; cb += kSegCand) {
+      const int nc = min(kSegCand, nCand - cb);
+      // candidate -> pair table: every non-empty pair marks its first candidate, a max-scan fills the rest
+      for (int j = tid; j < nc; j += kSegThreads) sh.cPair[j] = 0;
       __syncthreads();
-      // (2) exclusive scan of the window sizes
-      int nCand;
-      {
-        const int ipt = (nPairs + kSegThreads - 1) / kSegThreads;
-        const int lo = min(nPairs, tid * ipt), hi = min(nPairs, lo + ipt);
-        int s = 0;
-        for (int q = lo; q < hi; ++q) s += pOff[q];
-        int run = block_excl_scan<kSegThreads>(s, nCand);
-        for (int q = lo; q < hi; ++q) {
-          const int v = pOff[q];
-          pOff[q] = run;
-          run += v;
+      for (int q = tid; q < nPairs; q += kSegThreads) {
+        const int s = sh.pOff[q];
+        if (sh.pOff[q + 1] > s && s >= cb && s < cb + nc) sh.cPair[s - cb] = (unsigned short)q;
+      }
+      if (tid == 0 && cb > 0) {
+        int lo = 0, hi = nPairs;  // last q with pOff[q] <= cb: the pair candidate cb belongs to
+        while (hi - lo > 1) {
+          const int mid = (lo + hi) >> 1;
+          if (sh.pOff[mid] <= cb) lo = mid; else hi = mid;
         }
-        if (tid == 0) pOff[nPairs] = nCand;
+        sh.cPair[0] = (unsigned short)lo;
       }
       __syncthreads();
-      evals += (tid == 0) ? (unsigned long long)nCand : 0ull;
+      {
+        const int ipt = (nc + kSegThreads - 1) / kSegThreads;
+        const int lo = min(nc, tid * ipt), hi = min(nc, lo + ipt);
+        int m = 0;
+        for (int j = lo; j < hi; ++j) m = max(m, (int)sh.cPair[j]);
+        int carry = block_excl_scan_max<kSegThreads>(m);  // max over the entries of the threads before
+        for (int j = lo; j < hi; ++j) {
+          carry = max(carry, (int)sh.cPair[j]);
+          sh.cPair[j] = (unsigned short)carry;
+        }
+      }
+      __syncthreads();
       // (3) one thread per candidate
-      for (int c0 = 0; c0 < nCand; c0 += kSegThreads) {
-        const int cc = c0 + tid;
+      for (int j0 = 0; j0 < nc; j0 += kSegThreads) {
+        const int j = j0 + tid;
         bool pass = false;
         SegOut so;
-        float4 ai, ao;
         int k = 0, o = 0;
-        if (cc < nCand) {
-          int lo = 0, hi = nPairs;  // last q with pOff[q] <= cc
-          while (hi - lo > 1) {
-            const int mid = (lo + hi) >> 1;
-            if (pOff[mid] <= cc) lo = mid; else hi = mid;
-          }
-          k = pK[lo];
-          o = pLo[lo] + (cc - pOff[lo]);
-          ai = iAnchor[k];
-          ao = anchor[o];
-          pass = seg_select(P.cuts, iLayer[k], ai, iAux[k], ao, aux[o], so);
+        if (j < nc) {
+          const int q = sh.cPair[j];
+          k = kb + (int)__umulhi((unsigned)q, magic);
+          o = sh.pLo[q] + (cb + j - sh.pOff[q]);
+          pass = seg_select(P.cuts, sh.iLayer[k], sh.iAnchor[k], sh.iAux[k], anchor[o], aux[o], so);
         }
-        if (!FILL) {
-          if (pass) atomicAdd(&kCnt[k], 1);
-        } else {
-          const unsigned bal = __ballot_sync(0xffffffffu, pass);
-          if (lane_id() == 0) warpTot[warp] = __popc(bal);
-          __syncthreads();
-          int before = 0, all = 0;
+        const unsigned bal = __ballot_sync(0xffffffffu, pass);
+        if (lane_id() == 0) sh.warpTot[warp] = __popc(bal);
+        __syncthreads();
+        int before = 0, all = 0;
 #pragma unroll
-          for (int w = 0; w < kSegThreads / 32; ++w) {
-            const int v = warpTot[w];
-            before += (w < warp) ? v : 0;
-            all += v;
-          }
-          if (pass) {
-            const int pos = blockBase + blockTotal + before + __popc(bal & lanemask_lt());
-            if (pos < P.L.cap_seg) {
-              S.seg_md()[pos] = make_int2(i0 + k, o);
-              S.seg_f()[pos] = make_float4(so.sinS, so.z0,
-                                           atan2f(ai.x * ao.y - ai.y * ao.x, ai.x * ao.x + ai.y * ao.y),
-                                           atan2f(so.cross, so.dot));
+        for (int w = 0; w < kSegThreads / 32; ++w) {
+          const int v = sh.warpTot[w];
+          before += (w < warp) ? v : 0;
+          all += v;
+        }
+        if (pass) {
+          const int pos = running + before + __popc(bal & lanemask_lt());
+          if (!direct) {
+            atomicAdd(&sh.kCnt[k], 1);
+            if (pos < kSegStash) {
+              sh.stKO[pos] = (k << 24) | o;
+              sh.stV[pos] = make_float4(so.sinS, so.z0, so.cross, so.dot);
             }
+          } else if (base + pos < P.L.cap_seg) {
+            const float4 ai = sh.iAnchor[k], ao = anchor[o];
+            S.seg_md()[base + pos] = make_int2(i0 + k, o);
+            S.seg_f()[base + pos] = make_float4(so.sinS, so.z0,
+                                                atan2f(ai.x * ao.y - ai.y * ao.x, ai.x * ao.x + ai.y * ao.y),
+                                                atan2f(so.cross, so.dot));
           }
-          blockTotal += all;
-          __syncthreads();
+        }
+        running += all;
+        __syncthreads();
+      }
+    }
+    __syncthreads();
+  }
+  return running;
+}
+
+__global__ void __launch_bounds__(kSegThreads) k_seg(const __grid_constant__ Params P) {
+  __shared__ SegShared sh;
+  Slot S(P, blockIdx.y);
+  SlotHeader* H = S.hdr();
+  const int nMD = H->n[LST_MD_];
+  const int nChunks = (nMD + kSegChunk - 1) / kSegChunk;
+  int* seg_start = S.seg_start();
+  const float4* anchor = S.md_anchor();
+  const int tid = threadIdx.x;
+  if (tid < 6) {
+    sh.rMinO[tid] = r_min_of(H, 0, tid);
+    sh.rMaxO[tid] = r_max_of(H, 0, tid);
+  }
+  unsigned long long space = 0, evals = 0;
+  for (;;) {
+    __syncthreads();  // previous chunk fully consumed (and rMinO / rMaxO visible)
+    if (tid == 0) {
+      sh.chunk = (int)atomicAdd(&H->ticket[LST_SEG_], 1u);
+      sh.tMax = 0;
+    }
+    __syncthreads();
+    const int c = sh.chunk;
+    if (c >= nChunks) {
+      if (c == 0 && tid == 0) {  // no MDs at all: the first ticket publishes the empty result
+        publish_total(H, LST_SEG_, 0, P.L.cap_seg);
+        seg_start[0] = 0;
+      }
+      break;
+    }
+    const int i0 = c * kSegChunk, kn = min(kSegChunk, nMD - i0);
+    int nt = 0;
+    if (tid < kn) {
+      const int i = i0 + tid;
+      const float4 a = anchor[i];
+      const float2 x = S.md_aux()[i];
+      const int A = S.md_module()[i];
+      const int row0 = P.map_offsets[A];
+      nt = P.map_offsets[A + 1] - row0;
+      const int layer = P.mod_layer[A];
+      float dlo = 1.0f, dhi = -1.0f;
+      if (nt > 0) seg_window(P.cuts, layer, a.w, x.x, x.y, sh.rMinO[layer + 1], sh.rMaxO[layer + 1], dlo, dhi);
+      sh.iAnchor[tid] = a;
+      sh.iAux[tid] = x;
+      sh.iKey[tid] = S.md_key()[i];
+      sh.iDlo[tid] = dlo;
+      sh.iDhi[tid] = dhi;
+      sh.iRow0[tid] = row0;
+      sh.iNt[tid] = nt;
+      sh.iLayer[tid] = layer;
+    }
+    if (tid < kSegChunk) sh.kCnt[tid] = 0;
+    if (tid < kSegChunk) {  // warps 0 and 1
+      const int m = __reduce_max_sync(0xffffffffu, nt);
+      if (lane_id() == 0 && m > 0) atomicMax(&sh.tMax, m);
+    }
+    __syncthreads();
+    const int tStar = sh.tMax;
+    int total = 0;
+    if (tStar > 0) total = seg_walk(P, S, sh, i0, kn, tStar, false, 0, space, evals);
+    // where do this chunk's segments start?
+    if (tid < 32) {
+      const int b = lookback_exclusive(S.lb_seg(), c, total);
+      if (tid == 0) sh.base = b;
+    }
+    __syncthreads();
+    const int base = sh.base;
+    if (total <= kSegStash) {
+      for (int j = tid; j < total; j += kSegThreads) {
+        const int ko = sh.stKO[j], k = (int)((unsigned)ko >> 24), o = ko & 0xffffff;
+        if (base + j < P.L.cap_seg) {
+          const float4 v = sh.stV[j], ai = sh.iAnchor[k], ao = anchor[o];
+          S.seg_md()[base + j] = make_int2(i0 + k, o);
+          S.seg_f()[base + j] = make_float4(v.x, v.y, atan2f(ai.x * ao.y - ai.y * ao.x, ai.x * ao.x + ai.y * ao.y),
+                                            atan2f(v.z, v.w));
         }
       }
-      __syncthreads();
-      kBeg = kEnd;
+    } else {
+      seg_walk(P, S, sh, i0, kn, tStar, true, base, space, evals);  // rare: more segments than the stash holds
     }
-    // per inner MD: count -> chunk-local offset (count pass) -> global segment index (fill pass)
-    if (!FILL) {
-      const int v = (tid < kn) ? kCnt[tid] : 0;
+    // first segment of every inner MD of the chunk
+    {
+      const int v = (tid < kn) ? sh.kCnt[tid] : 0;
       int tot;
       const int ex = block_excl_scan<kSegThreads>(v, tot);
-      if (tid < kn) seg_start[i0 + tid] = ex;
-      if (tid == 0) block_base[c] = tot;
-    } else if (tid < kn) {
-      seg_start[i0 + tid] = min(blockBase + seg_start[i0 + tid], P.L.cap_seg);
+      if (tid < kn) seg_start[i0 + tid] = min(base + ex, P.L.cap_seg);
+    }
+    if (c == nChunks - 1 && tid == 0) {
+      publish_total(H, LST_SEG_, base + total, P.L.cap_seg);
+      seg_start[nMD] = min(base + total, P.L.cap_seg);
     }
   }
-  if (!FILL) {
 #pragma unroll
-    for (int d = 16; d > 0; d >>= 1) space += __shfl_down_sync(0xffffffffu, space, d);
-    if (lane_id() == 0 && space) atomicAdd(&H->cand[LST_SEG_], space);
-    if (tid == 0 && evals) atomicAdd(&H->eval[LST_SEG_], evals);
-    if (last_block_done(&H->done[1], gridDim.x)) {
-      const int total = block_scan_array<kSegThreads>(block_base, nChunks, -1);
-      if (tid == 0) {
-        publish_total(H, LST_SEG_, total, P.L.cap_seg);
-        seg_start[nMD] = min(total, P.L.cap_seg);
-      }
-    }
-  }
+  for (int d = 16; d > 0; d >>= 1) space += __shfl_down_sync(0xffffffffu, space, d);
+  if (lane_id() == 0 && space) atomicAdd(&H->cand[LST_SEG_], space);
+  if (tid == 0 && evals) atomicAdd(&H->eval[LST_SEG_], evals);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -798,10 +918,10 @@ int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEv
     }
     case LST_SEG_: {
       dim3 g(min(2 * per_event, P.L.n_chunk_md), nb);   // 128-thread blocks: twice as many per SM
-      k_seg<false><<<g, kSegThreads, 0, s>>>(P);
+      k_seg<<<g, kSegThreads, 0, s>>>(P);               // single pass (ticket + look-back)
       LST_EV(1);
-      k_seg<true><<<g, kSegThreads, 0, s>>>(P);
-      break;
+      LST_EV(2);
+      return 1;
     }
     case LST_T3_: {
       dim3 g(min(per_event, P.L.n_chunk_seg), nb);
