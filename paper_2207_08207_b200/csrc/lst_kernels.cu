@@ -79,6 +79,48 @@ __device__ int block_scan_array(int* a, int n, int clamp) {
   return total;
 }
 
+// In-place exclusive scan of the ints a[0 .. n] (a[n] must be 0 on entry and receives the total)
+// by the whole block, 16 bytes per lane and coalesced.  The array is padded with zeros to a
+// multiple of 4 ints (the slot layout rounds every array up to 256 bytes).  The values were
+// written by other blocks: ld.cg.  Returns the total.
+template <int NT>
+__device__ int block_scan_array4(int* a, int n) {
+  __shared__ int warp_tot[NT / 32];
+  constexpr int W = NT / 32;
+  int4* a4 = reinterpret_cast<int4*>(a);
+  const int n4 = (n + 1 + 3) / 4, per = (n4 + W - 1) / W;
+  const int w = threadIdx.x >> 5, lane = (int)lane_id();
+  const int lo = min(n4, w * per), hi = min(n4, lo + per);
+  int s = 0;
+  for (int j = lo + lane; j < hi; j += 32) {
+    const int4 v = __ldcg(a4 + j);
+    s += (v.x + v.y) + (v.z + v.w);
+  }
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+  if (lane == 0) warp_tot[w] = s;
+  __syncthreads();
+  int carry = 0, total = 0;
+#pragma unroll
+  for (int i = 0; i < W; ++i) {
+    const int v = warp_tot[i];
+    carry += (i < w) ? v : 0;
+    total += v;
+  }
+  for (int j0 = lo; j0 < hi; j0 += 32) {
+    const int j = j0 + lane;
+    int4 v = make_int4(0, 0, 0, 0);
+    if (j < hi) v = __ldcg(a4 + j);
+    const int t = (v.x + v.y) + (v.z + v.w);
+    const int incl = warp_incl_scan(t);
+    const int ex = carry + incl - t;
+    if (j < hi) a4[j] = make_int4(ex, ex + v.x, ex + v.x + v.y, ex + v.x + v.y + v.z);
+    carry += __shfl_sync(0xffffffffu, incl, 31);
+  }
+  __syncthreads();
+  return total;
+}
+
 // Ticket: true in every thread of the block that finishes last among `n_blocks`.
 __device__ __forceinline__ bool last_block_done(unsigned* counter, unsigned n_blocks) {
   __shared__ bool is_last;
@@ -193,17 +235,16 @@ __global__ void __launch_bounds__(256) k_bin_count(const __grid_constant__ Param
   // the last block of the event turns the counts into bin offsets
   if (!last_block_done(&S.hdr()->done[4], gridDim.x)) return;
   int* start = reinterpret_cast<int*>(cnt);
-  const int total = block_scan_array<256>(start, P.L.n_bins, -1);
-  __syncthreads();
   // search space of the MD stage: sum over modules of (#lower hits) x (#upper hits)
   unsigned long long c = 0;
-  for (int m = threadIdx.x; m < nmod; m += 256) {
-    const unsigned long long l = start[m + 1] - start[m], u = start[nmod + m + 1] - start[nmod + m];
-    c += l * u;
-  }
+#pragma unroll 4
+  for (int m = threadIdx.x; m < nmod; m += 256)
+    c += (unsigned long long)__ldcg(start + m) * (unsigned long long)__ldcg(start + nmod + m);
 #pragma unroll
   for (int d = 16; d > 0; d >>= 1) c += __shfl_down_sync(0xffffffffu, c, d);
   if (lane_id() == 0 && c) atomicAdd(&S.hdr()->cand[LST_MD_], c);
+  __syncthreads();
+  const int total = block_scan_array4<256>(start, P.L.n_bins);
   if (threadIdx.x == 0) {
     S.hdr()->n_hits = total;
     S.hdr()->n_lower = start[nmod];
@@ -233,11 +274,23 @@ __global__ void __launch_bounds__(256) k_bin_scatter(const __grid_constant__ Par
   }
 }
 
-// One warp per bin: rank the bin's hits by (key, original index) and gather the coordinates.
-__global__ void __launch_bounds__(256) k_bin_order(const __grid_constant__ Params P, const __grid_constant__ HitBatch B) {
+// One warp per bin: order the bin's hits by (key, original index) and gather the coordinates.
+// n <= 32: rank by shuffles; n <= kSortMax: bitonic sort of 64-bit (key, index) words in shared
+// memory; beyond: rank by an O(n^2) sweep over global memory.
+constexpr int kSortMax = 256;
+constexpr int kOrderWarps = 8;
+
+__device__ __forceinline__ unsigned ordered_bits(float f) {  // monotone map float -> unsigned
+  const unsigned u = __float_as_uint(f);
+  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+
+__global__ void __launch_bounds__(kOrderWarps * 32) k_bin_order(const __grid_constant__ Params P, const __grid_constant__ HitBatch B) {
+  __shared__ unsigned long long sortbuf[kOrderWarps][kSortMax];
   Slot S(P, blockIdx.y);
   const HitInput& in = B.ev[blockIdx.y];
-  const int b = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  const int wib = threadIdx.x >> 5, lane = (int)lane_id();
+  const int b = blockIdx.x * kOrderWarps + wib;
   if (b >= P.L.n_bins) return;
   const unsigned* start = S.bin_start();
   const int s = start[b], n = start[b + 1] - s;
@@ -251,22 +304,51 @@ __global__ void __launch_bounds__(256) k_bin_order(const __grid_constant__ Param
   int* orig = S.hit_orig() + s;
   int* hmod = S.hit_module() + s;
   float rmin = 3.0e38f, rmax = 0.0f;
-  for (int i0 = 0; i0 < n; i0 += 32) {
-    const int i = i0 + lane_id();
-    int mine = 0, rank = 0;
-    float key = 0.0f;
-    if (i < n) { mine = tmp[i]; key = tkey[i]; }
-    if (n <= 32) {
-      for (int j = 0; j < n; ++j) {
-        const float kj = __shfl_sync(0xffffffffu, key, j);
-        const int ij = __shfl_sync(0xffffffffu, mine, j);
-        rank += (kj < key) || (kj == key && ij < mine);
+  unsigned long long* buf = sortbuf[wib];
+  const bool sorted = n > 32 && n <= kSortMax;
+  if (sorted) {
+    int N = 64;
+    while (N < n) N <<= 1;
+    for (int i = lane; i < N; i += 32)
+      buf[i] = (i < n) ? (((unsigned long long)ordered_bits(tkey[i]) << 32) | (unsigned)tmp[i]) : ~0ull;
+    __syncwarp();
+    for (int k = 2; k <= N; k <<= 1) {
+      for (int j = k >> 1; j > 0; j >>= 1) {
+        for (int p = lane; p < (N >> 1); p += 32) {
+          const int i = ((p & ~(j - 1)) << 1) | (p & (j - 1)), l = i | j;
+          const unsigned long long a = buf[i], c = buf[l];
+          const bool up = (i & k) == 0;
+          if ((a > c) == up) { buf[i] = c; buf[l] = a; }
+        }
+        __syncwarp();
       }
-    } else if (i < n) {
-      for (int j = 0; j < n; ++j) {
-        const float kj = tkey[j];
-        const int ij = tmp[j];
-        rank += (kj < key) || (kj == key && ij < mine);
+    }
+  }
+  for (int i0 = 0; i0 < n; i0 += 32) {
+    const int i = i0 + lane;
+    int mine = 0, rank = i;
+    float key = 0.0f;
+    if (sorted) {
+      if (i < n) {
+        mine = (int)(unsigned)(buf[i] & 0xffffffffull);
+        const unsigned u = (unsigned)(buf[i] >> 32);
+        key = __uint_as_float((u & 0x80000000u) ? (u & 0x7fffffffu) : ~u);
+      }
+    } else {
+      if (i < n) { mine = tmp[i]; key = tkey[i]; }
+      rank = 0;
+      if (n <= 32) {
+        for (int j = 0; j < n; ++j) {
+          const float kj = __shfl_sync(0xffffffffu, key, j);
+          const int ij = __shfl_sync(0xffffffffu, mine, j);
+          rank += (kj < key) || (kj == key && ij < mine);
+        }
+      } else if (i < n) {
+        for (int j = 0; j < n; ++j) {
+          const float kj = tkey[j];
+          const int ij = tmp[j];
+          rank += (kj < key) || (kj == key && ij < mine);
+        }
       }
     }
     if (i < n) {
@@ -284,7 +366,7 @@ __global__ void __launch_bounds__(256) k_bin_order(const __grid_constant__ Param
     rmin = fminf(rmin, __shfl_down_sync(0xffffffffu, rmin, d));
     rmax = fmaxf(rmax, __shfl_down_sync(0xffffffffu, rmax, d));
   }
-  if (lane_id() == 0 && rmin <= rmax) {
+  if (lane == 0 && rmin <= rmax) {
     const int layer = P.mod_layer[m];
     SlotHeader* h = S.hdr();
     atomicMax(&h->r_min_inv[side][layer], 0x7f800000 - __float_as_int(rmin));
@@ -898,7 +980,7 @@ int launch_bin(const Params& P, const HitBatch& in, int n_batch, cudaStream_t s,
   LST_EV(2);
   k_bin_scatter<<<g, 256, 0, s>>>(P, in);
   LST_EV(3);
-  k_bin_order<<<dim3((P.L.n_bins + 7) / 8, (unsigned)n_batch), 256, 0, s>>>(P, in);
+  k_bin_order<<<dim3((P.L.n_bins + kOrderWarps - 1) / kOrderWarps, (unsigned)n_batch), kOrderWarps * 32, 0, s>>>(P, in);
   LST_EV(4);
   return 3;
 }
