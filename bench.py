@@ -319,11 +319,11 @@ def per_kernel_times(lst, geom, mmap, d_in, local, reps=5):
         ctx.load_events(0, d_in, stream=st)
         ctx.run_batch(0, N_EVENTS, st)
         ctx.sync(0, st)
-        k_ms = np.zeros(12)
+        k_ms = np.zeros(8)
         for k in range(0, N_EVENTS, 16):                  # a0 runs in launches of 16 events
             ctx.sync(k, st)
             k_ms[:4] += np.asarray(ctx.stats(k)["kernel_ms"][:4])
-        k_ms[4:] = np.asarray(ctx.stats(0)["kernel_ms"][4:])
+        k_ms[4:] = np.asarray(ctx.stats(0)["kernel_ms"][4:8])
         rows.append(k_ms)
     ctx.close()
     return dict(zip(lst.KERNEL_NAMES, np.median(np.asarray(rows[2:]), axis=0).tolist()))
@@ -334,8 +334,8 @@ def roofline(kernel_ms, n_hits, needed, cands, peaks):
     HBM (algorithmic bytes / measured copy bandwidth) and ALU (SPEC flops of all candidates / fp32
     non-FMA peak = 148 SMs x 128 lanes x sm_max clock; FMA is excluded by the SPEC's arithmetic)."""
     alu_peak_tflops = 148 * 128 * peaks["sm_max_mhz"] * 1e6 / 1e12
-    groups = (("a0_bin", ("bin_count", "bin_scatter", "bin_order")), ("a1_md", ("md_count", "md_fill")),
-              ("a2_ls", ("seg_count", "seg_fill")), ("a3_t3", ("t3_count", "t3_fill")), ("a4_t5", ("t5_count", "t5_fill")))
+    groups = (("a0_bin", ("reset", "bin_count", "bin_scatter", "bin_order")), ("a1_md", ("md",)),
+              ("a2_ls", ("seg",)), ("a3_t3", ("t3",)), ("a4_t5", ("t5",)))
     per_stage = {}
     for i, (name, ks) in enumerate(groups):
         ms = sum(kernel_ms[k] for k in ks)
@@ -346,7 +346,6 @@ def roofline(kernel_ms, n_hits, needed, cands, peaks):
                            "hbm_frac": b / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"] if ms else None,
                            "spec_flops": int(fl), "alu_tflops": fl / (ms * 1e-3) / 1e12 if ms else None,
                            "alu_frac": fl / (ms * 1e-3) / 1e12 / alu_peak_tflops if ms else None}
-    kernel_ms = {k: v for k, v in kernel_ms.items() if k != "bin_unused"}
     top = max(kernel_ms, key=kernel_ms.get)
     si = next(i for i, (_, ks) in enumerate(groups) if top in ks)
     ms = kernel_ms[top]

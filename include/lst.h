@@ -181,7 +181,8 @@ typedef struct {
   int32_t overflow;      /* bit k set: capacity of class k exceeded                              */
   int32_t bad_hits;      /* hits dropped because module id / side was out of range               */
   float stage_ms[5];     /* a0 .. a4; zeros unless lst_config.timing                              */
-  float kernel_ms[12];   /* bin count+scan, (unused), scatter, order; then count, fill of MD, LS, T3, T5 */
+  float kernel_ms[12];   /* a0: reset, bin count + scan, scatter, order; then the MD, LS, T3, T5 kernel; rest 0 */
+  int64_t rewalks[4];    /* chunks of 32 owners whose objects exceeded the on-chip stash and were walked twice */
 } lst_stats;
 
 /* Validates geometry and map, uploads the per-module tables, allocates the arena (the only

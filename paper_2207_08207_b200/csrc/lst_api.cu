@@ -3,7 +3,7 @@
 // Runtime design:
 //  * ONE cudaMalloc in lst_create covers every slot's input staging, hit store, object store,
 //    CSR offsets and scratch ("arena"); per event nothing is allocated or freed, the slot is
-//    recycled by one cudaMemsetAsync of its header + bin counters.
+//    recycled by one small kernel (k_reset) that zeroes its header, bin counters and look-back words.
 //  * lst_load_event / lst_run* only enqueue work on the caller's stream; sizes that are only
 //    known on the device (object counts) never come back to the host between stages: grids
 //    are fixed by the geometry / capacities and kernels read the counts from the slot header.
@@ -32,7 +32,7 @@ struct SlotHost {
   bool loaded = false, ran = false, synced = false;
   int n_hits_in = 0;
   SlotHeader* hdr = nullptr;  // pinned host copy of the device header
-  cudaEvent_t ev[17] = {};    // timing mode: ev[0..4] around the 4 a0 kernels, ev[5 + 3 s .. 7 + 3 s] around stage s
+  cudaEvent_t ev[13] = {};    // timing mode: ev[0..4] around the 4 a0 kernels, ev[5 + 2 s], ev[6 + 2 s] around stage s
   bool ev_bin = false, ev_stage[4] = {false, false, false, false};
 };
 
@@ -74,30 +74,27 @@ Layout make_layout(const lst_config& cfg, int n_modules) {
   L.n_modules = n_modules;
   L.n_bins = 2 * n_modules;
   L.cap_hits = cfg.cap_hits; L.cap_md = cfg.cap_md; L.cap_seg = cfg.cap_seg; L.cap_t3 = cfg.cap_t3; L.cap_t5 = cfg.cap_t5;
-  L.n_chunk_hits = (cfg.cap_hits + kScanChunk - 1) / kScanChunk;
-  L.n_chunk_seg = (cfg.cap_seg + kScanChunk - 1) / kScanChunk;
-  L.n_chunk_md = (cfg.cap_md + kSegChunkMd - 1) / kSegChunkMd;
-  L.n_chunk_t3 = (cfg.cap_t3 + kScanChunk - 1) / kScanChunk;
+  const int owner_cap[4] = {cfg.cap_hits, cfg.cap_md, cfg.cap_seg, cfg.cap_t3};
+  for (int k = 0; k < 4; ++k) L.n_chunk[k] = (owner_cap[k] + kChunk - 1) / kChunk;
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
   L.hdr = take(sizeof(SlotHeader));
   L.bin_start = take(sizeof(int) * (size_t)(L.n_bins + 1));
   L.bin_cursor = take(sizeof(int) * (size_t)L.n_bins);
-  L.lb_seg = take(8 * (size_t)(L.n_chunk_md + 1));
+  for (int k = 0; k < 4; ++k) L.lb[k] = take(8 * (size_t)(L.n_chunk[k] + 1));
   L.reset_bytes = off - L.hdr;
   const size_t nh = (size_t)cfg.cap_hits, nm = (size_t)cfg.cap_md, ns = (size_t)cfg.cap_seg, n3 = (size_t)cfg.cap_t3, n5 = (size_t)cfg.cap_t5;
   L.in_x = take(4 * nh); L.in_y = take(4 * nh); L.in_z = take(4 * nh); L.in_module = take(4 * nh); L.in_side = take(nh);
-  L.tmp_idx = take(4 * nh); L.tmp_key = take(4 * nh);
+  L.tmp_ki = take(8 * nh); L.tmp_bin = take(4 * nh);
   L.hit4 = take(16 * nh); L.hit_key = take(4 * nh); L.hit_orig = take(4 * nh); L.hit_module = take(4 * nh);
-  L.md_off = take(4 * (nh + 1)); L.md_block_base = take(4 * (size_t)(L.n_chunk_hits + 1));
   L.md_start = take(4 * (size_t)(n_modules + 1)); L.mod_info = take(16 * (size_t)n_modules);
   L.md_anchor = take(16 * nm); L.md_aux = take(8 * nm); L.md_key = take(4 * nm); L.md_hits = take(8 * nm);
   L.md_out = take(8 * nm); L.md_module = take(4 * nm);
-  L.seg_start = take(4 * (nm + 1)); L.seg_block_base = take(4 * (size_t)(L.n_chunk_md + 1));
+  L.seg_start = take(4 * (nm + 1));
   L.seg_md = take(8 * ns); L.seg_f = take(16 * ns);
-  L.t3_start = take(4 * (ns + 1)); L.t3_block_base = take(4 * (size_t)(L.n_chunk_seg + 1));
+  L.t3_start = take(4 * (ns + 1));
   L.t3_pack = take(16 * n3); L.t3_seg = take(8 * n3); L.t3_chi2 = take(4 * n3);
-  L.t5_start = take(4 * (n3 + 1)); L.t5_block_base = take(4 * (size_t)(L.n_chunk_t3 + 1));
+  L.t5_start = take(4 * (n3 + 1));
   L.t5_md = take(20 * n5); L.t5_t3 = take(8 * n5); L.t5_f = take(20 * n5);
   size_t scr = 8 * nm;
   if (16 * ns > scr) scr = 16 * ns;
@@ -175,7 +172,8 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
   if (cfg_in) cfg = *cfg_in; else lst_default_config(&cfg);
   const int n = g->n_modules;
   if (n <= 0 || n > (1 << 24) || m->n_modules != n || !g->layer || !g->phi || !m->row_offsets) return LST_ERR_ARG;
-  if (cfg.cap_md > (1 << 24)) return LST_ERR_ARG;  /* MD indices are packed into 24 bits by the segment kernel */
+  /* object indices are packed into 26 bits, module ids into 24 bits by the stage kernels */
+  if (cfg.cap_hits > kMaxCap || cfg.cap_md > kMaxCap || cfg.cap_seg > kMaxCap || cfg.cap_t3 > kMaxCap || cfg.cap_t5 > kMaxCap) return LST_ERR_ARG;
   if (cfg.n_slots < 1 || cfg.cap_hits < 1 || cfg.cap_md < 1 || cfg.cap_seg < 1 || cfg.cap_t3 < 1 || cfg.cap_t5 < 1) return LST_ERR_ARG;
   for (int i = 0; i < n; ++i)
     if (g->layer[i] < 0 || g->layer[i] >= LST_N_LAYERS) return LST_ERR_ARG;
@@ -294,7 +292,6 @@ int lst_load_events(lst_ctx* c, int first, int n_ev, const lst_hits* hits, void*
       sh.ev_bin = false;
       for (bool& f : sh.ev_stage) f = false;
       char* base = c->arena + (size_t)slot * c->P.slot_stride;
-      LST_CUDA(c, cudaMemsetAsync(base + L.hdr, 0, L.reset_bytes, s));
       HitInput in{h->x, h->y, h->z, h->module, h->side, h->n};
       if (!h->on_device && h->n > 0) {
         const size_t n = (size_t)h->n;
@@ -333,7 +330,7 @@ int lst_run_stage(lst_ctx* c, int first, int n, int stage, void* stream) {
   SlotHost& sh = c->slots[first];
   Params P = c->P;
   P.first_slot = first;
-  c->launches += launch_stage(P, n, stage, st, c->cfg.timing ? sh.ev + 5 + 3 * stage : nullptr);
+  c->launches += launch_stage(P, n, stage, st, c->cfg.timing ? sh.ev + 5 + 2 * stage : nullptr);
   LST_CUDA(c, cudaGetLastError());
   if (c->cfg.timing) sh.ev_stage[stage] = true;
   for (int s = first; s < first + n; ++s) { c->slots[s].synced = false; if (stage == LST_T5) c->slots[s].ran = true; }
@@ -432,7 +429,7 @@ int lst_get_stats(lst_ctx* c, int slot, lst_stats* o) {
   if (!sh.synced) return LST_ERR_STATE;
   std::memset(o, 0, sizeof(*o));
   o->n_hits = sh.hdr->n_hits;
-  for (int k = 0; k < 4; ++k) { o->needed[k] = (int64_t)sh.hdr->needed[k]; o->candidates[k] = (int64_t)sh.hdr->cand[k]; o->evaluated[k] = (int64_t)sh.hdr->eval[k]; }
+  for (int k = 0; k < 4; ++k) { o->needed[k] = (int64_t)sh.hdr->needed[k]; o->candidates[k] = (int64_t)sh.hdr->cand[k]; o->evaluated[k] = (int64_t)sh.hdr->eval[k]; o->rewalks[k] = (int64_t)sh.hdr->rewalk[k]; }
   o->overflow = sh.hdr->overflow;
   o->bad_hits = sh.hdr->bad_hits;
   if (c->cfg.timing) {
@@ -442,10 +439,9 @@ int lst_get_stats(lst_ctx* c, int slot, lst_stats* o) {
     }
     for (int st = 0; st < 4; ++st)
       if (sh.ev_stage[st]) {
-        cudaEvent_t* e = sh.ev + 5 + 3 * st;
-        cudaEventElapsedTime(&o->stage_ms[1 + st], e[0], e[2]);
-        cudaEventElapsedTime(&o->kernel_ms[4 + 2 * st], e[0], e[1]);
-        cudaEventElapsedTime(&o->kernel_ms[5 + 2 * st], e[1], e[2]);
+        cudaEvent_t* e = sh.ev + 5 + 2 * st;
+        cudaEventElapsedTime(&o->stage_ms[1 + st], e[0], e[1]);
+        o->kernel_ms[4 + st] = o->stage_ms[1 + st];
       }
     cudaGetLastError();
   }

@@ -8,7 +8,7 @@
 // Hit store (per slot): hits are binned by (side, module) -- all lower-sensor hits first, in
 // module order, then all upper-sensor hits -- and ordered inside a bin by their azimuth
 // relative to the module normal (`key`), ties by original index.  Lower hit i of the event is
-// simply element i: the MD kernel is "one thread per lower hit".
+// simply element i: the MD kernel's owners are the lower hits.
 //   hit4[i]      = (x, y, z, r)            float4
 //   hit_key[i]   = azimuth - module azimuth float   (FLT_MAX for non-finite x / y)
 //   hit_orig[i]  = original index           int
@@ -31,6 +31,7 @@
 //   T5     t5_md[5], t5_t3 = (A, B) int2, t5_f[5] = kA, kB, kfit, chi2xy, chi2rz
 // CSR offsets: bin_start[2*n_modules+1], md_start[n_modules+1], seg_start[cap_md+1] (by inner
 // MD), t3_start[cap_seg+1] (by first segment), t5_start[cap_t3+1] (by inner triplet).
+// mod_info[m] = (first MD, end MD, smallest key, largest key of the module's lower hits).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -39,10 +40,10 @@
 
 namespace lst {
 
-constexpr int kScanChunk = 256;   // owners (lower hits / segments / triplets) per block chunk
-constexpr int kSegChunkMd = 64;   // inner MDs per block of the segment kernel
+constexpr int kChunk = 32;        // owners (lower hits / MDs / segments / triplets) per warp chunk
 constexpr int kMaxBatch = 16;     // events per launch of the a0 kernels (pointer table in the launch parameters)
-constexpr int kMaxRow = 64;       // longest module-map row the segment kernel stages
+constexpr int kMaxRow = 64;       // longest module-map row accepted
+constexpr int kMaxCap = 1 << 26;  // largest per-slot capacity: object indices are packed into 26 bits
 enum { LST_MD_ = 0, LST_SEG_ = 1, LST_T3_ = 2, LST_T5_ = 3 };  // == LST_MD .. LST_T5 of lst.h
 
 struct SlotHeader {
@@ -54,6 +55,7 @@ struct SlotHeader {
   unsigned long long needed[4];   // objects that passed (unclamped)
   unsigned long long cand[4];     // candidates of the search space (map-restricted pairs)
   unsigned long long eval[4];     // candidates the selection was evaluated on (after windowing)
+  unsigned long long rewalk[4];   // chunks whose objects did not fit the shared-memory stash (walked twice)
   // per side, per layer: range of r over the finite hits, as float bit patterns;
   // r_min is stored as 0x7f800000 - bits so that the zeroed header means "+inf"
   int r_min_inv[2][6];
@@ -65,17 +67,16 @@ struct SlotHeader {
 struct Layout {
   int n_modules, n_bins;
   int cap_hits, cap_md, cap_seg, cap_t3, cap_t5;
-  int n_chunk_hits, n_chunk_seg, n_chunk_t3;  // ceil(cap / kScanChunk)
-  int n_chunk_md;                             // ceil(cap_md / kSegChunkMd)
+  int n_chunk[4];                 // ceil(cap of the OWNER class / kChunk): hits, MD, LS, T3
   // byte offsets from the slot base (all multiples of 256)
-  size_t hdr, bin_start, bin_cursor, lb_seg;  // contiguous: zeroed by one memset at lst_load_event
+  size_t hdr, bin_start, bin_cursor, lb[4];   // contiguous: zeroed by k_reset at lst_load_event
   size_t reset_bytes;                         // bytes to zero at lst_load_event, from hdr
   size_t in_x, in_y, in_z, in_module, in_side;// staging of host input
-  size_t tmp_idx, tmp_key, hit4, hit_key, hit_orig, hit_module;
-  size_t md_off, md_block_base, md_start, mod_info, md_anchor, md_aux, md_key, md_hits, md_out, md_module;
-  size_t seg_start, seg_block_base, seg_md, seg_f;
-  size_t t3_start, t3_block_base, t3_pack, t3_seg, t3_chi2;
-  size_t t5_start, t5_block_base, t5_md, t5_t3, t5_f;
+  size_t tmp_ki, tmp_bin, hit4, hit_key, hit_orig, hit_module;
+  size_t md_start, mod_info, md_anchor, md_aux, md_key, md_hits, md_out, md_module;
+  size_t seg_start, seg_md, seg_f;
+  size_t t3_start, t3_pack, t3_seg, t3_chi2;
+  size_t t5_start, t5_md, t5_t3, t5_f;
   size_t scratch;
   size_t slot_bytes;
 };
@@ -105,15 +106,13 @@ struct Slot {
   __device__ __forceinline__ SlotHeader* hdr() const { return at<SlotHeader>(L.hdr); }
   __device__ __forceinline__ unsigned* bin_start() const { return at<unsigned>(L.bin_start); }
   __device__ __forceinline__ unsigned* bin_cursor() const { return at<unsigned>(L.bin_cursor); }
-  __device__ __forceinline__ unsigned long long* lb_seg() const { return at<unsigned long long>(L.lb_seg); }
-  __device__ __forceinline__ int* tmp_idx() const { return at<int>(L.tmp_idx); }
-  __device__ __forceinline__ float* tmp_key() const { return at<float>(L.tmp_key); }
+  __device__ __forceinline__ unsigned long long* lb(int kind) const { return at<unsigned long long>(L.lb[kind]); }
+  __device__ __forceinline__ int2* tmp_ki() const { return at<int2>(L.tmp_ki); }
+  __device__ __forceinline__ int* tmp_bin() const { return at<int>(L.tmp_bin); }
   __device__ __forceinline__ float4* hit4() const { return at<float4>(L.hit4); }
   __device__ __forceinline__ float* hit_key() const { return at<float>(L.hit_key); }
   __device__ __forceinline__ int* hit_orig() const { return at<int>(L.hit_orig); }
   __device__ __forceinline__ int* hit_module() const { return at<int>(L.hit_module); }
-  __device__ __forceinline__ int* md_off() const { return at<int>(L.md_off); }
-  __device__ __forceinline__ int* md_block_base() const { return at<int>(L.md_block_base); }
   __device__ __forceinline__ int* md_start() const { return at<int>(L.md_start); }
   __device__ __forceinline__ int4* mod_info() const { return at<int4>(L.mod_info); }
   __device__ __forceinline__ float4* md_anchor() const { return at<float4>(L.md_anchor); }
@@ -123,16 +122,13 @@ struct Slot {
   __device__ __forceinline__ float2* md_out() const { return at<float2>(L.md_out); }
   __device__ __forceinline__ int* md_module() const { return at<int>(L.md_module); }
   __device__ __forceinline__ int* seg_start() const { return at<int>(L.seg_start); }
-  __device__ __forceinline__ int* seg_block_base() const { return at<int>(L.seg_block_base); }
   __device__ __forceinline__ int2* seg_md() const { return at<int2>(L.seg_md); }
   __device__ __forceinline__ float4* seg_f() const { return at<float4>(L.seg_f); }
   __device__ __forceinline__ int* t3_start() const { return at<int>(L.t3_start); }
-  __device__ __forceinline__ int* t3_block_base() const { return at<int>(L.t3_block_base); }
   __device__ __forceinline__ int4* t3_pack() const { return at<int4>(L.t3_pack); }
   __device__ __forceinline__ int2* t3_seg() const { return at<int2>(L.t3_seg); }
   __device__ __forceinline__ float* t3_chi2() const { return at<float>(L.t3_chi2); }
   __device__ __forceinline__ int* t5_start() const { return at<int>(L.t5_start); }
-  __device__ __forceinline__ int* t5_block_base() const { return at<int>(L.t5_block_base); }
   __device__ __forceinline__ int* t5_md() const { return at<int>(L.t5_md); }
   __device__ __forceinline__ int2* t5_t3() const { return at<int2>(L.t5_t3); }
   __device__ __forceinline__ float* t5_f() const { return at<float>(L.t5_f); }
@@ -154,8 +150,9 @@ struct HitBatch {
 };
 
 // Host-callable launchers (lst_kernels.cu). Each returns the number of kernels it launched.
-int launch_bin(const Params& P, const HitBatch& in, int n_batch, cudaStream_t s, cudaEvent_t* ev);
-int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEvent_t* ev);
+// `ev` (optional, timing mode): ev[0] is recorded before the first kernel, ev[k + 1] after kernel k.
+int launch_bin(const Params& P, const HitBatch& in, int n_batch, cudaStream_t s, cudaEvent_t* ev);   // 4 kernels
+int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEvent_t* ev);          // 1 kernel
 int launch_gather_hits(const Params& P, int kind, int n, cudaStream_t s);
 int launch_pack_values(const Params& P, int kind, int n, cudaStream_t s);
 

@@ -1,21 +1,32 @@
-// lst_kernels.cu -- sm_100a kernels of the LST hot path (DESIGN.md sections 5-6).
+// lst_kernels.cu -- sm_100a kernels of the LST hot path (DESIGN.md sections 5-7).
 //
 // Hits and mini-doublets are kept ordered by azimuth inside their module, so the MD and the
 // segment stage look only at a window of candidates found by binary search (DESIGN.md
 // section 6); every candidate in a window goes through the exact SPEC selection.
 //
-// Every stage is  count -> (last block scans) -> fill : the count kernel evaluates the
-// selection and leaves per-owner counts; the last block to finish turns block totals into block
-// bases (no extra launch, no host round trip); the fill kernel re-walks the same candidates in
-// the same order and writes each object at its final, deterministic position.  No global atomic
-// is issued per candidate or per object: compaction is warp ballot + popc, block scan, and one
-// ticket atomic per block.
+// Every stage is ONE single-pass kernel built from the same warp-level pipeline
+// (DESIGN.md section 7):
+//   * a warp takes a chunk of 32 consecutive OWNERS (lower hits / inner MDs / first segments /
+//     inner triplets) from a ticket counter; each owner has a contiguous range of candidates;
+//   * the ranges are flattened: a warp scan numbers the candidates, and every tile of 32
+//     candidates finds its owners with one redux + popc (no search, no barrier), so all 32 lanes
+//     evaluate one candidate each whatever the occupancy skew between owners;
+//   * where a cheap test removes most candidates (module key ranges and windows for segments, the
+//     curvature match for quintuplets) survivors are compacted into a small shared-memory
+//     queue and the expensive selection runs on full tiles of survivors;
+//   * what passes is kept, in (owner, candidate) order, in a shared-memory stash until a
+//     decoupled look-back over the chunk totals has told the warp where its objects start;
+//     objects are then written once, contiguous per owner (CSR), in a deterministic order.
+// No global atomic is issued per candidate or per object, and no block-wide barrier is used:
+// warps are independent, compaction is ballot + popc.
 //
 // blockIdx.y = index of the event within the batch (lst_run_batch): all events of a batch go
 // through one launch per kernel.
 #include "lst_device.cuh"
 
 namespace lst {
+
+constexpr unsigned kFull = 0xffffffffu;
 
 // ------------------------------------------------------------------------------------------
 // small device utilities
@@ -26,57 +37,29 @@ __device__ __forceinline__ unsigned lanemask_lt() {
   asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
   return m;
 }
+__device__ __forceinline__ unsigned lanemask_le() {
+  unsigned m;
+  asm("mov.u32 %0, %%lanemask_le;" : "=r"(m));
+  return m;
+}
 
 __device__ __forceinline__ int warp_incl_scan(int v) {
 #pragma unroll
   for (int d = 1; d < 32; d <<= 1) {
-    int t = __shfl_up_sync(0xffffffffu, v, d);
+    int t = __shfl_up_sync(kFull, v, d);
     if ((int)lane_id() >= d) v += t;
   }
   return v;
 }
-
-// Exclusive scan of one int per thread over the block; returns the prefix, total in `total`.
-// NT = blockDim.x (multiple of 32, <= 1024). Ends with a barrier: safe to call repeatedly.
-template <int NT>
-__device__ __forceinline__ int block_excl_scan(int v, int& total) {
-  __shared__ int warp_sum[NT / 32];
-  __shared__ int block_total;
+__device__ __forceinline__ int warp_excl_scan(int v, int& total) {
   const int incl = warp_incl_scan(v);
-  const int w = threadIdx.x >> 5;
-  if (lane_id() == 31) warp_sum[w] = incl;
-  __syncthreads();
-  if (w == 0) {
-    int s = (lane_id() < NT / 32) ? warp_sum[lane_id()] : 0;
-    const int si = warp_incl_scan(s);
-    if (lane_id() < NT / 32) warp_sum[lane_id()] = si - s;
-    if (lane_id() == 31) block_total = si;
-  }
-  __syncthreads();
-  const int r = incl - v + warp_sum[w];
-  total = block_total;
-  __syncthreads();
-  return r;
+  total = __shfl_sync(kFull, incl, 31);
+  return incl - v;
 }
-
-// In-place exclusive scan of a[0..n) by the whole block, a[n] = total (unclamped total is
-// returned to every thread). Values are read with ld.cg: they were written by other blocks.
-// If clamp >= 0 the stored prefixes are min(prefix, clamp).
-template <int NT>
-__device__ int block_scan_array(int* a, int n, int clamp) {
-  const int ipt = (n + NT - 1) / NT;
-  const int lo = min(n, (int)threadIdx.x * ipt), hi = min(n, lo + ipt);
-  int s = 0;
-  for (int i = lo; i < hi; ++i) s += __ldcg(a + i);
-  int total;
-  int run = block_excl_scan<NT>(s, total);
-  for (int i = lo; i < hi; ++i) {
-    const int v = __ldcg(a + i);
-    a[i] = (clamp >= 0) ? min(run, clamp) : run;
-    run += v;
-  }
-  if (threadIdx.x == 0) a[n] = (clamp >= 0) ? min(total, clamp) : total;
-  return total;
+__device__ __forceinline__ unsigned long long warp_sum_ull(unsigned long long v) {
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) v += __shfl_down_sync(kFull, v, d);
+  return v;
 }
 
 // In-place exclusive scan of the ints a[0 .. n] (a[n] must be 0 on entry and receives the total)
@@ -97,7 +80,7 @@ __device__ int block_scan_array4(int* a, int n) {
     s += (v.x + v.y) + (v.z + v.w);
   }
 #pragma unroll
-  for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+  for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(kFull, s, d);
   if (lane == 0) warp_tot[w] = s;
   __syncthreads();
   int carry = 0, total = 0;
@@ -115,7 +98,7 @@ __device__ int block_scan_array4(int* a, int n) {
     const int incl = warp_incl_scan(t);
     const int ex = carry + incl - t;
     if (j < hi) a4[j] = make_int4(ex, ex + v.x, ex + v.x + v.y, ex + v.x + v.y + v.z);
-    carry += __shfl_sync(0xffffffffu, incl, 31);
+    carry += __shfl_sync(kFull, incl, 31);
   }
   __syncthreads();
   return total;
@@ -172,7 +155,8 @@ __device__ __forceinline__ int upper_bound_f(const float* a, int lo, int hi, flo
   return lo;
 }
 
-// M2 bounds |sinA| by thr(r_u) <= thr(r_max_upper); M1 (dot > 0) gives r_u > r_l.
+// M2 bounds |sinA| by thr(r_u) <= thr(r_max_upper); M1 (dot > 0) gives r_u > r_l.  The window
+// shrinks as r_l grows, so evaluated at the smallest r of the layer's lower hits it covers them all.
 // Returns the half width of the azimuth window around the lower hit, < 0 if nothing can pass.
 __device__ __forceinline__ float md_window(const Cuts& c, int layer, float r_l, float r_max_upper) {
   if (!(r_max_upper > 0.0f) || !(r_max_upper * 1.000001f >= r_l)) return -1.0f;
@@ -219,6 +203,14 @@ __device__ __forceinline__ float r_max_of(const SlotHeader* h, int side, int lay
 // a0: load + bin by (side, module) + order by azimuth + derive r
 // blockIdx.y = event of the batch; its input arrays come from the pointer table `B`.
 // ------------------------------------------------------------------------------------------
+// Recycles the slot: zeroes header, bin counters, bin cursors and the look-back status words.
+__global__ void __launch_bounds__(256) k_reset(const __grid_constant__ Params P) {
+  Slot S(P, blockIdx.y);
+  int4* p = S.at<int4>(P.L.hdr);
+  const size_t n = P.L.reset_bytes / 16;
+  for (size_t i = (size_t)blockIdx.x * 256 + threadIdx.x; i < n; i += (size_t)gridDim.x * 256) p[i] = make_int4(0, 0, 0, 0);
+}
+
 __global__ void __launch_bounds__(256) k_bin_count(const __grid_constant__ Params P, const __grid_constant__ HitBatch B) {
   Slot S(P, blockIdx.y);
   const HitInput& in = B.ev[blockIdx.y];
@@ -240,8 +232,7 @@ __global__ void __launch_bounds__(256) k_bin_count(const __grid_constant__ Param
 #pragma unroll 4
   for (int m = threadIdx.x; m < nmod; m += 256)
     c += (unsigned long long)__ldcg(start + m) * (unsigned long long)__ldcg(start + nmod + m);
-#pragma unroll
-  for (int d = 16; d > 0; d >>= 1) c += __shfl_down_sync(0xffffffffu, c, d);
+  c = warp_sum_ull(c);
   if (lane_id() == 0 && c) atomicAdd(&S.hdr()->cand[LST_MD_], c);
   __syncthreads();
   const int total = block_scan_array4<256>(start, P.L.n_bins);
@@ -256,8 +247,8 @@ __global__ void __launch_bounds__(256) k_bin_scatter(const __grid_constant__ Par
   const HitInput& in = B.ev[blockIdx.y];
   const unsigned* start = S.bin_start();
   unsigned* cur = S.bin_cursor();
-  int* tmp = S.tmp_idx();
-  float* tkey = S.tmp_key();
+  int2* tki = S.tmp_ki();
+  int* tbin = S.tmp_bin();
   const int nmod = P.L.n_modules;
   for (int h = blockIdx.x * blockDim.x + threadIdx.x; h < in.n; h += gridDim.x * blockDim.x) {
     const int m = in.module[h];
@@ -267,210 +258,93 @@ __global__ void __launch_bounds__(256) k_bin_scatter(const __grid_constant__ Par
     const float x = in.x[h], y = in.y[h];
     const float2 cs = P.mod_cs[m];
     // azimuth relative to the module normal; non-finite hits (they can never pass a cut) go last
-    const float k = atan2f(cs.x * y - cs.y * x, cs.x * x + cs.y * y);
+    float k = atan2f(cs.x * y - cs.y * x, cs.x * x + cs.y * y);
+    if (!(fabsf(k) <= 4.0f)) k = 3.0e38f;
     const unsigned pos = start[b] + atomicAdd(cur + b, 1u);
-    tmp[pos] = h;
-    tkey[pos] = (fabsf(k) <= 4.0f) ? k : 3.0e38f;
+    tki[pos] = make_int2(__float_as_int(k), h);
+    tbin[pos] = b;
   }
 }
 
-// One warp per bin: order the bin's hits by (key, original index) and gather the coordinates.
-// n <= 32: rank by shuffles; n <= kSortMax: bitonic sort of 64-bit (key, index) words in shared
-// memory; beyond: rank by an O(n^2) sweep over global memory.
-constexpr int kSortMax = 256;
-constexpr int kOrderWarps = 8;
-
-__device__ __forceinline__ unsigned ordered_bits(float f) {  // monotone map float -> unsigned
-  const unsigned u = __float_as_uint(f);
-  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
-}
-
-__global__ void __launch_bounds__(kOrderWarps * 32) k_bin_order(const __grid_constant__ Params P, const __grid_constant__ HitBatch B) {
-  __shared__ unsigned long long sortbuf[kOrderWarps][kSortMax];
+// One thread per hit: its rank inside the bin by (key, original index) is the number of hits
+// of the bin that come before it -- a loop over the bin (6 hits on average, all lanes busy
+// whatever the bin sizes; neighbouring threads sit in the same or the next bin).  Then gather the
+// coordinates, derive r, and keep the range of r per (side, layer) and the key range per module.
+__global__ void __launch_bounds__(256) k_bin_order(const __grid_constant__ Params P, const __grid_constant__ HitBatch B) {
+  __shared__ int s_rng[24];
   Slot S(P, blockIdx.y);
   const HitInput& in = B.ev[blockIdx.y];
-  const int wib = threadIdx.x >> 5, lane = (int)lane_id();
-  const int b = blockIdx.x * kOrderWarps + wib;
-  if (b >= P.L.n_bins) return;
-  const unsigned* start = S.bin_start();
-  const int s = start[b], n = start[b + 1] - s;
-  if (n == 0) return;
-  const int nmod = P.L.n_modules;
-  const int side = b >= nmod, m = b - side * nmod;
-  const int* tmp = S.tmp_idx() + s;
-  const float* tkey = S.tmp_key() + s;
-  float4* hit4 = S.hit4() + s;
-  float* hkey = S.hit_key() + s;
-  int* orig = S.hit_orig() + s;
-  int* hmod = S.hit_module() + s;
-  float rmin = 3.0e38f, rmax = 0.0f;
-  unsigned long long* buf = sortbuf[wib];
-  const bool sorted = n > 32 && n <= kSortMax;
-  if (sorted) {
-    int N = 64;
-    while (N < n) N <<= 1;
-    for (int i = lane; i < N; i += 32)
-      buf[i] = (i < n) ? (((unsigned long long)ordered_bits(tkey[i]) << 32) | (unsigned)tmp[i]) : ~0ull;
-    __syncwarp();
-    for (int k = 2; k <= N; k <<= 1) {
-      for (int j = k >> 1; j > 0; j >>= 1) {
-        for (int p = lane; p < (N >> 1); p += 32) {
-          const int i = ((p & ~(j - 1)) << 1) | (p & (j - 1)), l = i | j;
-          const unsigned long long a = buf[i], c = buf[l];
-          const bool up = (i & k) == 0;
-          if ((a > c) == up) { buf[i] = c; buf[l] = a; }
-        }
-        __syncwarp();
-      }
-    }
-  }
-  for (int i0 = 0; i0 < n; i0 += 32) {
-    const int i = i0 + lane;
-    int mine = 0, rank = i;
-    float key = 0.0f;
-    if (sorted) {
-      if (i < n) {
-        mine = (int)(unsigned)(buf[i] & 0xffffffffull);
-        const unsigned u = (unsigned)(buf[i] >> 32);
-        key = __uint_as_float((u & 0x80000000u) ? (u & 0x7fffffffu) : ~u);
-      }
-    } else {
-      if (i < n) { mine = tmp[i]; key = tkey[i]; }
-      rank = 0;
-      if (n <= 32) {
-        for (int j = 0; j < n; ++j) {
-          const float kj = __shfl_sync(0xffffffffu, key, j);
-          const int ij = __shfl_sync(0xffffffffu, mine, j);
-          rank += (kj < key) || (kj == key && ij < mine);
-        }
-      } else if (i < n) {
-        for (int j = 0; j < n; ++j) {
-          const float kj = tkey[j];
-          const int ij = tmp[j];
-          rank += (kj < key) || (kj == key && ij < mine);
-        }
-      }
-    }
-    if (i < n) {
-      const float x = in.x[mine], y = in.y[mine], z = in.z[mine];
-      const float r = sqrtf(x * x + y * y);
-      hit4[rank] = make_float4(x, y, z, r);
-      hkey[rank] = key;
-      orig[rank] = mine;
-      hmod[rank] = m;
-      if (r < 3.0e38f) { rmin = fminf(rmin, r); rmax = fmaxf(rmax, r); }
-    }
-  }
-#pragma unroll
-  for (int d = 16; d > 0; d >>= 1) {
-    rmin = fminf(rmin, __shfl_down_sync(0xffffffffu, rmin, d));
-    rmax = fmaxf(rmax, __shfl_down_sync(0xffffffffu, rmax, d));
-  }
-  if (lane == 0 && rmin <= rmax) {
-    const int layer = P.mod_layer[m];
-    SlotHeader* h = S.hdr();
-    atomicMax(&h->r_min_inv[side][layer], 0x7f800000 - __float_as_int(rmin));
-    atomicMax(&h->r_max[side][layer], __float_as_int(rmax));
-  }
-}
-
-// ------------------------------------------------------------------------------------------
-// a1: mini-doublets. One thread per lower hit; its candidates are the upper hits of the same
-// module inside the azimuth window (a binary search in the key-ordered upper bin).
-// ------------------------------------------------------------------------------------------
-template <bool FILL>
-__global__ void __launch_bounds__(kScanChunk) k_md(const __grid_constant__ Params P) {
-  Slot S(P, blockIdx.y);
   SlotHeader* H = S.hdr();
   const int nmod = P.L.n_modules;
-  const int nLower = H->n_lower;
-  const int nChunks = (nLower + kScanChunk - 1) / kScanChunk;
-  const unsigned* bs = S.bin_start();
-  const float4* hit4 = S.hit4();
-  const float* hkey = S.hit_key();
-  int* md_off = S.md_off();
-  int* block_base = S.md_block_base();
-  unsigned long long evals = 0;
-  for (int c = blockIdx.x; c < nChunks; c += gridDim.x) {
-    const int i = c * kScanChunk + threadIdx.x;
-    int count = 0;
-    if (i < nLower) {
-      const int m = S.hit_module()[i];
+  if (threadIdx.x < 24) s_rng[threadIdx.x] = 0;
+  __syncthreads();
+  const int nh = H->n_hits;
+  const unsigned* start = S.bin_start();
+  const int2* tki = S.tmp_ki();
+  int* info = reinterpret_cast<int*>(S.mod_info());
+  const int p = blockIdx.x * 256 + threadIdx.x;
+  if (p < nh) {
+    const int b = S.tmp_bin()[p];
+    const int s = (int)start[b], e = (int)start[b + 1];
+    const int2 me = tki[p];
+    const float key = __int_as_float(me.x);
+    int rank = 0;
+    for (int j = s; j < e; ++j) {
+      const int2 o = tki[j];
+      const float kj = __int_as_float(o.x);
+      rank += (kj < key) || (kj == key && o.y < me.y);
+    }
+    const int side = b >= nmod, m = b - side * nmod;
+    const float x = in.x[me.y], y = in.y[me.y], z = in.z[me.y];
+    const float r = sqrtf(x * x + y * y);
+    const int dst = s + rank;
+    S.hit4()[dst] = make_float4(x, y, z, r);
+    S.hit_key()[dst] = key;
+    S.hit_orig()[dst] = me.y;
+    S.hit_module()[dst] = m;
+    if (!side) {
+      if (rank == 0) info[4 * m + 2] = me.x;
+      if (rank == e - s - 1) info[4 * m + 3] = me.x;
+    }
+    if (r < 3.0e38f) {
       const int layer = P.mod_layer[m];
-      const int u0 = bs[nmod + m], u1 = bs[nmod + m + 1];
-      if (u1 > u0) {
-        const float4 lo = hit4[i];
-        const float kl = hkey[i];
-        const float w = md_window(P.cuts, layer, lo.w, r_max_of(H, 1, layer));
-        int j0 = u0, j1 = u1;
-        if (w < 0.0f) {
-          j1 = j0;
-        } else if (fabsf(kl) + w < 1.5f) {
-          j0 = lower_bound_f(hkey, u0, u1, kl - w);
-          j1 = upper_bound_f(hkey, j0, u1, kl + w);
-        }
-        evals += (unsigned long long)(j1 - j0);
-        const int base = FILL ? block_base[c] + md_off[i] : 0;
-        for (int j = j0; j < j1; ++j) {
-          const float4 up = hit4[j];
-          MdOut o;
-          if (md_select(P.cuts, layer, lo, up, o)) {
-            if (FILL) {
-              const int pos = base + count;
-              if (pos < P.L.cap_md) {
-                S.md_anchor()[pos] = lo;
-                S.md_aux()[pos] = make_float2(up.w, o.sinA);
-                S.md_key()[pos] = kl;
-                S.md_hits()[pos] = make_int2(S.hit_orig()[i], S.hit_orig()[j]);
-                S.md_out()[pos] = make_float2(atan2f(lo.x * up.y - lo.y * up.x, lo.x * up.x + lo.y * up.y),
-                                              atan2f(o.cross, o.dot));
-                S.md_module()[pos] = m;
-              }
-            }
-            ++count;
-          }
-        }
-      }
-    }
-    if (!FILL) {
-      int tot;
-      const int ex = block_excl_scan<kScanChunk>(count, tot);
-      if (i < nLower) md_off[i] = ex;
-      if (threadIdx.x == 0) block_base[c] = tot;
+      atomicMax(&s_rng[side * 6 + layer], 0x7f800000 - __float_as_int(r));
+      atomicMax(&s_rng[12 + side * 6 + layer], __float_as_int(r));
     }
   }
-  if (FILL) {
-    // md_start[m] = index of the first MD of module m = offset of the module's first lower hit
-    const int total = H->n[LST_MD_];
-    for (int m = blockIdx.x * kScanChunk + threadIdx.x; m <= nmod; m += gridDim.x * kScanChunk) {
-      const int ls = (m < nmod) ? (int)bs[m] : nLower;
-      const int b0 = (ls < nLower) ? min(block_base[ls / kScanChunk] + md_off[ls], P.L.cap_md) : total;
-      S.md_start()[m] = b0;
-      if (m < nmod) {
-        // (first MD, end MD, key range of the module's lower hits >= key range of its MDs)
-        const int le = (int)bs[m + 1];
-        const int b1 = (le < nLower) ? min(block_base[le / kScanChunk] + md_off[le], P.L.cap_md) : total;
-        const bool any = le > ls;
-        S.mod_info()[m] = make_int4(b0, b1, __float_as_int(any ? hkey[ls] : 3.0e38f), __float_as_int(any ? hkey[le - 1] : -3.0e38f));
-      }
-    }
-  } else {
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) evals += __shfl_down_sync(0xffffffffu, evals, d);
-    if (lane_id() == 0 && evals) atomicAdd(&H->eval[LST_MD_], evals);
-    if (last_block_done(&H->done[0], gridDim.x)) {
-      const int total = block_scan_array<kScanChunk>(block_base, nChunks, -1);
-      if (threadIdx.x == 0) publish_total(H, LST_MD_, total, P.L.cap_md);
-    }
+  if (p < nmod && start[p + 1] == start[p]) {  // no lower hits: an empty key range
+    info[4 * p + 2] = __float_as_int(3.0e38f);
+    info[4 * p + 3] = __float_as_int(-3.0e38f);
   }
+  __syncthreads();
+  if (threadIdx.x < 24 && s_rng[threadIdx.x]) atomicMax(&H->r_min_inv[0][0] + threadIdx.x, s_rng[threadIdx.x]);
 }
 
 // ------------------------------------------------------------------------------------------
-// single-pass ordered output: chunks of owners are handed out in order by a ticket; a block
+// the warp pipeline
+// ------------------------------------------------------------------------------------------
+// Flattened ranges: lane l owns `n` consecutive items starting at flat position `off` (exclusive
+// scan of n over the warp).  For the tile of flat positions [tb, tb + 32) returns, for the lane at
+// position tb + lane, the rank of its owner among the NON-EMPTY owners (index into a table of
+// their lanes that the caller keeps).  Every non-empty owner that starts inside the tile sets the
+// bit of its start; the owner of a position is the last start at or before it.
+__device__ __forceinline__ int tile_owner(int n, int off, int tb) {
+  const unsigned startbit = (n > 0 && off >= tb && off < tb + 32) ? (1u << (off - tb)) : 0u;
+  const unsigned mask = __reduce_or_sync(kFull, startbit);
+  const int before = __popc(__ballot_sync(kFull, n > 0 && off < tb));
+  return before + __popc(mask & lanemask_le()) - 1;
+}
+// Table of the lanes of the non-empty owners, in order (tab[rank] = lane).
+__device__ __forceinline__ void build_owner_table(int n, int* tab) {
+  const unsigned ne = __ballot_sync(kFull, n > 0);
+  if (n > 0) tab[__popc(ne & lanemask_lt())] = (int)lane_id();
+  __syncwarp();
+}
+
+// single-pass ordered output: chunks of owners are handed out in order by a ticket; a warp
 // learns where its chunk's objects start by decoupled look-back over the totals of the chunks
 // before it (each chunk publishes its total as soon as it is known, so nothing waits on a
-// block that has not started).  status word: bits 63:62 = 1 total only, 2 = inclusive prefix.
-// ------------------------------------------------------------------------------------------
+// warp that has not started).  status word: bits 63:62 = 1 total only, 2 = inclusive prefix.
 __device__ __forceinline__ void st_status(unsigned long long* p, unsigned long long v) {
   asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
@@ -479,448 +353,719 @@ __device__ __forceinline__ unsigned long long ld_status(const unsigned long long
   asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
   return v;
 }
-// Called by all lanes of ONE warp. Returns the number of objects of chunks 0 .. c-1.
-__device__ __forceinline__ int lookback_exclusive(unsigned long long* status, int c, int total) {
+// Called by all lanes of a warp. Returns the number of objects of chunks 0 .. c-1.  Only the
+// warp with publish = true writes chunk c's status; the other warps of the block read along.
+__device__ __forceinline__ int lookback_exclusive(unsigned long long* status, int c, int total, bool publish) {
   const int lane = (int)lane_id();
-  if (lane == 0) st_status(status + c, ((c == 0 ? 2ull : 1ull) << 62) | (unsigned)total);
+  if (publish && lane == 0) st_status(status + c, ((c == 0 ? 2ull : 1ull) << 62) | (unsigned)total);
   if (c == 0) return 0;
   int sum = 0;
   for (int j = c - 1;; j -= 32) {
     const int idx = j - lane;
     unsigned long long v = (idx >= 0) ? ld_status(status + idx) : (2ull << 62);
-    while (__any_sync(0xffffffffu, (v >> 62) == 0)) {
+    while (__any_sync(kFull, (v >> 62) == 0)) {
       if ((v >> 62) == 0) v = ld_status(status + idx);
     }
-    const unsigned pmask = __ballot_sync(0xffffffffu, (v >> 62) == 2);
+    const unsigned pmask = __ballot_sync(kFull, (v >> 62) == 2);
     const int firstP = pmask ? __ffs(pmask) - 1 : 32;
     int contrib = (lane <= firstP) ? (int)(unsigned)(v & 0xffffffffull) : 0;
 #pragma unroll
-    for (int d = 16; d > 0; d >>= 1) contrib += __shfl_xor_sync(0xffffffffu, contrib, d);
+    for (int d = 16; d > 0; d >>= 1) contrib += __shfl_xor_sync(kFull, contrib, d);
     sum += contrib;
     if (pmask) break;
   }
-  if (lane == 0) st_status(status + c, (2ull << 62) | (unsigned)(sum + total));
+  if (publish && lane == 0) st_status(status + c, (2ull << 62) | (unsigned)(sum + total));
   return sum;
 }
 
-// Exclusive max-scan of one non-negative int per thread over the block (0 for thread 0).
-// Ends with a barrier.
-template <int NT>
-__device__ __forceinline__ int block_excl_scan_max(int v) {
-  __shared__ int warp_max[NT / 32];
-#pragma unroll
-  for (int d = 1; d < 32; d <<= 1) {
-    const int t = __shfl_up_sync(0xffffffffu, v, d);
-    if ((int)lane_id() >= d) v = max(v, t);
-  }
-  const int w = threadIdx.x >> 5;
-  if (lane_id() == 31) warp_max[w] = v;
-  int ex = __shfl_up_sync(0xffffffffu, v, 1);
-  if (lane_id() == 0) ex = 0;
+// The unit of the ticket and of the look-back is the BLOCK: NW warps take NW consecutive chunks
+// of 32 owners (a "super-chunk"), so an event has few units in flight and the look-back is one
+// or two steps deep.  Two block barriers per super-chunk; everything between them is per warp.
+struct BlockShared {
+  int ticket;
+  int tot[8];
+};
+// Next super-chunk of the block (barrier: also separates the shared-memory use of two rounds).
+__device__ __forceinline__ int block_ticket(unsigned* ticket, BlockShared& bs) {
+  if (threadIdx.x == 0) bs.ticket = (int)atomicAdd(ticket, 1u);
   __syncthreads();
-#pragma unroll
-  for (int i = 0; i < NT / 32; ++i) ex = (i < w) ? max(ex, warp_max[i]) : ex;
+  return bs.ticket;
+}
+// Index of the first object of this warp's chunk, given the number of objects `total` it found.
+template <int NW>
+__device__ __forceinline__ int block_base(unsigned long long* status, int C, int total, BlockShared& bs) {
+  const int w = threadIdx.x >> 5, lane = (int)lane_id();
+  if (lane == 0) bs.tot[w] = total;
   __syncthreads();
-  return ex;
+  int block_total;
+  const int ex = warp_excl_scan(lane < NW ? bs.tot[lane] : 0, block_total);
+  return lookback_exclusive(status, C, block_total, w == 0) + __shfl_sync(kFull, ex, w);
 }
 
-// ------------------------------------------------------------------------------------------
-// a2: segments, single pass. One block per chunk of kSegChunk consecutive inner MDs (they may
-// sit in several modules).  (1) every (inner MD, connected module) pair finds its window of
-// outer MDs by a binary search in the connected module's key-ordered MD list, (2) a block scan
-// of the window sizes numbers the candidates in (inner MD, outer MD) order, (3) one thread per
-// candidate evaluates the SPEC selection ONCE; what passes is kept in shared memory, in order,
-// until the look-back has told the block where its segments start.  Segments come out ordered
-// by (inner MD, outer MD).
-// ------------------------------------------------------------------------------------------
-constexpr int kSegThreads = 128;
-constexpr int kSegChunk = kSegChunkMd;  // inner MDs per chunk
-constexpr int kSegPairs = 1024;  // (inner MD, connected module) pairs per tile (>= kMaxRow)
-constexpr int kSegCand = 1024;   // candidates per lookup tile
-constexpr int kSegStash = 512;   // segments of a chunk kept in shared memory
+constexpr int kWarps = 8;        // warps per block of the MD / T3 / T5 kernels
+constexpr int kSegWarps = 4;     // of the segment kernel (more shared memory per warp)
+constexpr int kQueue = 64;       // queue slots per warp (a push adds <= 32, a drain starts at >= 32)
 
-struct SegShared {
-  float4 iAnchor[kSegChunk];
-  float2 iAux[kSegChunk];
-  float iKey[kSegChunk], iDlo[kSegChunk], iDhi[kSegChunk];
-  int iRow0[kSegChunk], iNt[kSegChunk], iLayer[kSegChunk], kCnt[kSegChunk];
-  int pLo[kSegPairs], pOff[kSegPairs + 1];
-  unsigned short cPair[kSegCand];
-  int stKO[kSegStash];
-  float4 stV[kSegStash];
-  int warpTot[kSegThreads / 32];
-  float rMinO[6], rMaxO[6];
-  int chunk, base, tMax;
+// ------------------------------------------------------------------------------------------
+// a1: mini-doublets.  Owner = lower hit; its candidates are the upper hits of the same module
+// inside the azimuth window (two binary searches in the key-ordered upper bin).
+// ------------------------------------------------------------------------------------------
+constexpr int kMdStash = 96;
+struct MdWarp {
+  float4 lo[32];
+  float key[32];
+  int mod[32], layer[32], tab[32], cnt[32];
+  int stI[kMdStash];
+  float stS[kMdStash];
 };
 
-// Walks the chunk's candidates in order. direct = false: passing candidates go to the stash
-// (positions < kSegStash) and are counted per inner MD; direct = true: they are written to
-// global memory at `base` + position.  Returns the number of passing candidates.
-__device__ __forceinline__ int seg_walk(const Params& P, const Slot& S, SegShared& sh, int i0, int kn, int tStar,
-                                        bool direct, int base, unsigned long long& space, unsigned long long& evals) {
-  const float4* anchor = S.md_anchor();
-  const float2* aux = S.md_aux();
-  const float* mkey = S.md_key();
-  const int4* mod_info = S.mod_info();
-  const int tid = threadIdx.x, warp = tid >> 5;
-  const unsigned magic = 0xffffffffu / (unsigned)tStar + 1u;  // q / tStar == umulhi(q, magic) for q < 65536
-  const int kTile = min(kn, kSegPairs / tStar);
-  int running = 0;  // passing candidates so far (uniform across the block)
-  for (int kb = 0; kb < kn; kb += kTile) {
-    const int kt = min(kTile, kn - kb), nPairs = kt * tStar;
-    // (1) windows
-    for (int q = tid; q < nPairs; q += kSegThreads) {
-      const int kk = (int)__umulhi((unsigned)q, magic), t = q - kk * tStar, k = kb + kk;
-      int first = 0, n = 0;
-      if (t < sh.iNt[k]) {
-        const int e = sh.iRow0[k] + t;
-        const int4 info = mod_info[P.map_targets[e]];
-        const int b0 = info.x, b1 = info.y;
-        if (!direct) space += (unsigned long long)(b1 - b0);
-        const float dlo = sh.iDlo[k], dhi = sh.iDhi[k];
-        if (b1 > b0 && dlo <= dhi) {
-          const float c0 = sh.iKey[k] + P.map_dphi[e];
-          if (!(fabsf(c0) + fmaxf(fabsf(dlo), fabsf(dhi)) < 3.0f)) {
-            first = b0;  // azimuth wrap possible (never with a sane geometry): no window
-            n = b1 - b0;
-          } else if (c0 + dhi >= __int_as_float(info.z) && c0 + dlo <= __int_as_float(info.w)) {
-            first = lower_bound_f(mkey, b0, b1, c0 + dlo);
-            n = upper_bound_f(mkey, first, b1, c0 + dhi) - first;
-          }
-        }
-      }
-      sh.pLo[q] = first;
-      sh.pOff[q] = n;
+__device__ __forceinline__ void md_emit(const Params& P, const Slot& S, const MdWarp& sh, int pos, int i, int ol, int u,
+                                        float sinA) {
+  if (pos >= P.L.cap_md) return;
+  const float4 lo = sh.lo[ol], up = S.hit4()[u];
+  const float dx = up.x - lo.x, dy = up.y - lo.y;
+  const float cross = lo.x * dy - lo.y * dx, dot = lo.x * dx + lo.y * dy;   // as in md_select
+  S.md_anchor()[pos] = lo;
+  S.md_aux()[pos] = make_float2(up.w, sinA);
+  S.md_key()[pos] = sh.key[ol];
+  S.md_hits()[pos] = make_int2(S.hit_orig()[i], S.hit_orig()[u]);
+  S.md_out()[pos] = make_float2(atan2f(lo.x * up.y - lo.y * up.x, lo.x * up.x + lo.y * up.y), atan2f(cross, dot));
+  S.md_module()[pos] = sh.mod[ol];
+}
+
+template <bool DIRECT>
+__device__ __forceinline__ int md_walk(const Params& P, const Slot& S, MdWarp& sh, int n, int off, int total, int j0,
+                                       int i0, int base) {
+  const float4* hit4 = S.hit4();
+  const int lane = (int)lane_id();
+  int running = 0;
+  for (int tb = 0; tb < total; tb += 32) {
+    const int rk = tile_owner(n, off, tb);
+    const int j = tb + lane;
+    const int ol = (j < total) ? sh.tab[rk] : 0;
+    const int ooff = __shfl_sync(kFull, off, ol), oj0 = __shfl_sync(kFull, j0, ol);
+    bool pass = false;
+    MdOut o;
+    int u = 0;
+    if (j < total) {
+      u = oj0 + (j - ooff);
+      pass = md_select(P.cuts, sh.layer[ol], sh.lo[ol], hit4[u], o);
     }
-    __syncthreads();
-    // (2) exclusive scan of the window sizes
-    int nCand;
-    {
-      const int ipt = (nPairs + kSegThreads - 1) / kSegThreads;
-      const int lo = min(nPairs, tid * ipt), hi = min(nPairs, lo + ipt);
-      int s = 0;
-      for (int q = lo; q < hi; ++q) s += sh.pOff[q];
-      int run = block_excl_scan<kSegThreads>(s, nCand);
-      for (int q = lo; q < hi; ++q) {
-        const int v = sh.pOff[q];
-        sh.pOff[q] = run;
-        run += v;
-      }
-      if (tid == 0) sh.pOff[nPairs] = nCand;
-    }
-    __syncthreads();
-    if (!direct && tid == 0) evals += (unsigned long long)nCand;
-    for (int cb = 0; cb < nCand; cb += kSegCand) {
-      const int nc = min(kSegCand, nCand - cb);
-      // candidate -> pair table: every non-empty pair marks its first candidate, a max-scan fills the rest
-      for (int j = tid; j < nc; j += kSegThreads) sh.cPair[j] = 0;
-      __syncthreads();
-      for (int q = tid; q < nPairs; q += kSegThreads) {
-        const int s = sh.pOff[q];
-        if (sh.pOff[q + 1] > s && s >= cb && s < cb + nc) sh.cPair[s - cb] = (unsigned short)q;
-      }
-      if (tid == 0 && cb > 0) {
-        int lo = 0, hi = nPairs;  // last q with pOff[q] <= cb: the pair candidate cb belongs to
-        while (hi - lo > 1) {
-          const int mid = (lo + hi) >> 1;
-          if (sh.pOff[mid] <= cb) lo = mid; else hi = mid;
-        }
-        sh.cPair[0] = (unsigned short)lo;
-      }
-      __syncthreads();
-      {
-        const int ipt = (nc + kSegThreads - 1) / kSegThreads;
-        const int lo = min(nc, tid * ipt), hi = min(nc, lo + ipt);
-        int m = 0;
-        for (int j = lo; j < hi; ++j) m = max(m, (int)sh.cPair[j]);
-        int carry = block_excl_scan_max<kSegThreads>(m);  // max over the entries of the threads before
-        for (int j = lo; j < hi; ++j) {
-          carry = max(carry, (int)sh.cPair[j]);
-          sh.cPair[j] = (unsigned short)carry;
-        }
-      }
-      __syncthreads();
-      // (3) one thread per candidate
-      for (int j0 = 0; j0 < nc; j0 += kSegThreads) {
-        const int j = j0 + tid;
-        bool pass = false;
-        SegOut so;
-        int k = 0, o = 0;
-        if (j < nc) {
-          const int q = sh.cPair[j];
-          k = kb + (int)__umulhi((unsigned)q, magic);
-          o = sh.pLo[q] + (cb + j - sh.pOff[q]);
-          pass = seg_select(P.cuts, sh.iLayer[k], sh.iAnchor[k], sh.iAux[k], anchor[o], aux[o], so);
-        }
-        const unsigned bal = __ballot_sync(0xffffffffu, pass);
-        if (lane_id() == 0) sh.warpTot[warp] = __popc(bal);
-        __syncthreads();
-        int before = 0, all = 0;
-#pragma unroll
-        for (int w = 0; w < kSegThreads / 32; ++w) {
-          const int v = sh.warpTot[w];
-          before += (w < warp) ? v : 0;
-          all += v;
-        }
-        if (pass) {
-          const int pos = running + before + __popc(bal & lanemask_lt());
-          if (!direct) {
-            atomicAdd(&sh.kCnt[k], 1);
-            if (pos < kSegStash) {
-              sh.stKO[pos] = (k << 24) | o;
-              sh.stV[pos] = make_float4(so.sinS, so.z0, so.cross, so.dot);
-            }
-          } else if (base + pos < P.L.cap_seg) {
-            const float4 ai = sh.iAnchor[k], ao = anchor[o];
-            S.seg_md()[base + pos] = make_int2(i0 + k, o);
-            S.seg_f()[base + pos] = make_float4(so.sinS, so.z0,
-                                                atan2f(ai.x * ao.y - ai.y * ao.x, ai.x * ao.x + ai.y * ao.y),
-                                                atan2f(so.cross, so.dot));
-          }
-        }
-        running += all;
-        __syncthreads();
+    const unsigned bal = __ballot_sync(kFull, pass);
+    if (pass) {
+      const int pos = running + __popc(bal & lanemask_lt());
+      if (!DIRECT) {
+        atomicAdd(&sh.cnt[ol], 1);
+        if (pos < kMdStash) { sh.stI[pos] = (ol << 26) | u; sh.stS[pos] = o.sinA; }
+      } else {
+        md_emit(P, S, sh, base + pos, i0 + ol, ol, u, o.sinA);
       }
     }
-    __syncthreads();
+    running += __popc(bal);
   }
   return running;
 }
 
-__global__ void __launch_bounds__(kSegThreads) k_seg(const __grid_constant__ Params P) {
-  __shared__ SegShared sh;
+__global__ void __launch_bounds__(kWarps * 32) k_md(const __grid_constant__ Params P) {
+  __shared__ MdWarp shw[kWarps];
+  __shared__ float s_w[6], s_rmaxU[6];
+  __shared__ BlockShared bsh;
   Slot S(P, blockIdx.y);
   SlotHeader* H = S.hdr();
-  const int nMD = H->n[LST_MD_];
-  const int nChunks = (nMD + kSegChunk - 1) / kSegChunk;
-  int* seg_start = S.seg_start();
-  const float4* anchor = S.md_anchor();
-  const int tid = threadIdx.x;
-  if (tid < 6) {
-    sh.rMinO[tid] = r_min_of(H, 0, tid);
-    sh.rMaxO[tid] = r_max_of(H, 0, tid);
+  const int nmod = P.L.n_modules, cap = P.L.cap_md;
+  const int nLower = H->n_lower;
+  const int nSuper = (nLower + kWarps * kChunk - 1) / (kWarps * kChunk);
+  const int lane = (int)lane_id();
+  MdWarp& sh = shw[threadIdx.x >> 5];
+  if (threadIdx.x < 6) {
+    const float ru = r_max_of(H, 1, threadIdx.x);
+    s_rmaxU[threadIdx.x] = ru;
+    s_w[threadIdx.x] = md_window(P.cuts, threadIdx.x, r_min_of(H, 0, threadIdx.x), ru);
   }
+  __syncthreads();
+  const unsigned* bs = S.bin_start();
+  const float* hkey = S.hit_key();
+  const int* hmod = S.hit_module();
+  int* md_start = S.md_start();
+  int* info = reinterpret_cast<int*>(S.mod_info());
+  unsigned long long evals = 0;
+  for (;;) {
+    const int C = block_ticket(&H->ticket[LST_MD_], bsh);
+    if (C >= nSuper) {
+      if (C == 0 && threadIdx.x < 32) {  // no lower hits at all: the first ticket publishes the empty result
+        for (int m = lane; m <= nmod; m += 32) {
+          md_start[m] = 0;
+          if (m < nmod) { info[4 * m] = 0; info[4 * m + 1] = 0; }
+        }
+        if (lane == 0) publish_total(H, LST_MD_, 0, cap);
+      }
+      break;
+    }
+    const int i0 = (C * kWarps + (int)(threadIdx.x >> 5)) * kChunk, i = i0 + lane;
+    int n = 0, j0 = 0, m = 0;
+    if (i < nLower) {
+      m = hmod[i];
+      const int layer = P.mod_layer[m];
+      const int u0 = (int)bs[nmod + m], u1 = (int)bs[nmod + m + 1];
+      const float4 lo = S.hit4()[i];
+      const float kl = hkey[i];
+      sh.lo[lane] = lo;
+      sh.key[lane] = kl;
+      sh.mod[lane] = m;
+      sh.layer[lane] = layer;
+      const float w = s_w[layer];
+      if (u1 > u0 && w >= 0.0f && s_rmaxU[layer] * 1.000001f >= lo.w) {
+        int j1 = u1;
+        j0 = u0;
+        if (fabsf(kl) + w < 1.5f) {
+          j0 = lower_bound_f(hkey, u0, u1, kl - w);
+          j1 = upper_bound_f(hkey, j0, u1, kl + w);
+        }
+        n = j1 - j0;
+      }
+    }
+    sh.cnt[lane] = 0;
+    evals += (unsigned long long)n;
+    int total_c;
+    const int off = warp_excl_scan(n, total_c);
+    build_owner_table(n, sh.tab);
+    const int total = md_walk<false>(P, S, sh, n, off, total_c, j0, i0, 0);
+    const int base = block_base<kWarps>(S.lb(LST_MD_), C, total, bsh);
+    __syncwarp();
+    if (total <= kMdStash) {
+      for (int t = lane; t < total; t += 32) {
+        const int v = sh.stI[t], ol = (int)((unsigned)v >> 26), u = v & (kMaxCap - 1);
+        md_emit(P, S, sh, base + t, i0 + ol, ol, u, sh.stS[t]);
+      }
+    } else {
+      if (lane == 0) atomicAdd(&H->rewalk[LST_MD_], 1ull);
+      md_walk<true>(P, S, sh, n, off, total_c, j0, i0, base);
+    }
+    // module table: the first lower hit of a module (and the modules without lower hits before it)
+    {
+      int tot;
+      const int first = min(base + warp_excl_scan(sh.cnt[lane], tot), cap);
+      if (i < nLower) {
+        const int m_prev = (i > 0) ? hmod[i - 1] : -1;
+        for (int mm = m_prev + 1; mm <= m; ++mm) {
+          md_start[mm] = first;
+          info[4 * mm] = first;
+          if (mm > 0) info[4 * (mm - 1) + 1] = first;
+        }
+        if (i == nLower - 1) {
+          const int end = min(base + total, cap);
+          for (int mm = m + 1; mm <= nmod; ++mm) {
+            md_start[mm] = end;
+            if (mm < nmod) info[4 * mm] = end;
+            info[4 * (mm - 1) + 1] = end;
+          }
+          publish_total(H, LST_MD_, base + total, cap);
+        }
+      }
+    }
+    __syncwarp();
+  }
+  evals = warp_sum_ull(evals);
+  if (lane == 0 && evals) atomicAdd(&H->eval[LST_MD_], evals);
+}
+
+// ------------------------------------------------------------------------------------------
+// a2: segments.  Owner = inner MD.  Three levels, each compacted before the next:
+//   A  every (inner MD, connected module) pair: module has MDs and its key range meets the
+//      MD's azimuth window?                                             -> pair queue
+//   B  surviving pairs: window of outer MDs by two binary searches in the module's key-ordered
+//      MD list; the windows are flattened into candidates               -> candidate queue
+//   C  candidates, 32 at a time: the SPEC selection                     -> stash
+// Segments come out ordered by (inner MD, outer MD).
+// ------------------------------------------------------------------------------------------
+constexpr int kSegStash = 160;
+struct SegWarp {
+  float4 a4[32];
+  float2 aux[32];
+  float key[32], dlo[32], dhi[32];
+  int layer[32], tab[32], ptab[32], cnt[32];
+  int2 pq[kQueue], cq[kQueue];
+  int stI[kSegStash];
+  float2 stV[kSegStash];
+};
+
+__device__ __forceinline__ void seg_emit(const Params& P, const Slot& S, const SegWarp& sh, int pos, int i, int ol, int o,
+                                         float sinS, float z0) {
+  if (pos >= P.L.cap_seg) return;
+  const float4 ai = sh.a4[ol], ao = S.md_anchor()[o];
+  const float dx = ao.x - ai.x, dy = ao.y - ai.y;
+  const float cross = ai.x * dy - ai.y * dx, dot = ai.x * dx + ai.y * dy;   // as in seg_select
+  S.seg_md()[pos] = make_int2(i, o);
+  S.seg_f()[pos] = make_float4(sinS, z0, atan2f(ai.x * ao.y - ai.y * ao.x, ai.x * ao.x + ai.y * ao.y), atan2f(cross, dot));
+}
+
+template <bool DIRECT>
+__device__ __forceinline__ int seg_walk(const Params& P, const Slot& S, SegWarp& sh, int nt, int off, int nPairs, int row0,
+                                        int i0, int base, unsigned long long& space, unsigned long long& evals) {
+  const float4* anchor = S.md_anchor();
+  const float2* aux = S.md_aux();
+  const float* mkey = S.md_key();
+  const int4* mod_info = S.mod_info();
+  const int lane = (int)lane_id();
+  int running = 0;
+  int ph = 0, pt = 0, ch = 0, ct = 0;   // heads / tails of the pair and candidate queues
+
+  // C: the selection on up to 32 candidates (inner lane, outer MD)
+  auto levelC = [&](bool valid, int2 it) {
+    bool pass = false;
+    SegOut so;
+    const int ol = it.x, o = it.y;
+    if (valid) pass = seg_select(P.cuts, sh.layer[ol], sh.a4[ol], sh.aux[ol], anchor[o], aux[o], so);
+    const unsigned bal = __ballot_sync(kFull, pass);
+    if (pass) {
+      const int pos = running + __popc(bal & lanemask_lt());
+      if (!DIRECT) {
+        atomicAdd(&sh.cnt[ol], 1);
+        if (pos < kSegStash) { sh.stI[pos] = (ol << 26) | o; sh.stV[pos] = make_float2(so.sinS, so.z0); }
+      } else {
+        seg_emit(P, S, sh, base + pos, i0 + ol, ol, o, so.sinS, so.z0);
+      }
+    }
+    running += __popc(bal);
+  };
+  auto drainC = [&](bool all) {
+    while (ct - ch >= 32 || (all && ct > ch)) {
+      __syncwarp();
+      const bool valid = lane < ct - ch;
+      int2 it = make_int2(0, 0);
+      if (valid) it = sh.cq[(ch + lane) & (kQueue - 1)];
+      levelC(valid, it);
+      ch += min(32, ct - ch);
+      __syncwarp();
+    }
+  };
+  // B: windows of up to 32 surviving pairs (inner lane << 26 | target module, c0)
+  auto levelB = [&](bool valid, int2 it) {
+    int first = 0, cnt = 0;
+    const int ol = (int)((unsigned)it.x >> 26);
+    if (valid) {
+      const int4 info = mod_info[it.x & (kMaxCap - 1)];
+      const float c0 = __int_as_float(it.y), dlo = sh.dlo[ol], dhi = sh.dhi[ol];
+      if (!(fabsf(c0) + fmaxf(fabsf(dlo), fabsf(dhi)) < 3.0f)) {
+        first = info.x;  // azimuth wrap possible (never with a sane geometry): no window
+        cnt = info.y - info.x;
+      } else {
+        first = lower_bound_f(mkey, info.x, info.y, c0 + dlo);
+        cnt = upper_bound_f(mkey, first, info.y, c0 + dhi) - first;
+      }
+    }
+    if (!DIRECT) evals += (unsigned long long)cnt;
+    int nc;
+    const int coff = warp_excl_scan(cnt, nc);
+    build_owner_table(cnt, sh.ptab);
+    for (int tb = 0; tb < nc; tb += 32) {
+      const int rk = tile_owner(cnt, coff, tb);
+      const int j = tb + lane;
+      const int pl = (j < nc) ? sh.ptab[rk] : 0;
+      const int o = __shfl_sync(kFull, first, pl) + (j - __shfl_sync(kFull, coff, pl));
+      const int iol = __shfl_sync(kFull, ol, pl);
+      if (j < nc) sh.cq[(ct + lane) & (kQueue - 1)] = make_int2(iol, o);
+      ct += min(32, nc - tb);
+      drainC(false);
+    }
+    __syncwarp();
+  };
+  auto drainB = [&](bool all) {
+    while (pt - ph >= 32 || (all && pt > ph)) {
+      __syncwarp();
+      const bool valid = lane < pt - ph;
+      int2 it = make_int2(0, 0);
+      if (valid) it = sh.pq[(ph + lane) & (kQueue - 1)];
+      levelB(valid, it);
+      ph += min(32, pt - ph);
+      __syncwarp();
+    }
+  };
+  // A: all (inner MD, connected module) pairs of the chunk
+  for (int tb = 0; tb < nPairs; tb += 32) {
+    const int rk = tile_owner(nt, off, tb);
+    const int q = tb + lane;
+    const int ol = (q < nPairs) ? sh.tab[rk] : 0;
+    const int e = __shfl_sync(kFull, row0, ol) + (q - __shfl_sync(kFull, off, ol));
+    bool keep = false;
+    int tgt = 0;
+    float c0 = 0.0f;
+    if (q < nPairs) {
+      tgt = P.map_targets[e];
+      const int4 info = mod_info[tgt];
+      if (!DIRECT) space += (unsigned long long)(info.y - info.x);
+      const float dlo = sh.dlo[ol], dhi = sh.dhi[ol];
+      if (info.y > info.x && dlo <= dhi) {
+        c0 = sh.key[ol] + P.map_dphi[e];
+        keep = !(fabsf(c0) + fmaxf(fabsf(dlo), fabsf(dhi)) < 3.0f) ||
+               (c0 + dhi >= __int_as_float(info.z) && c0 + dlo <= __int_as_float(info.w));
+      }
+    }
+    const unsigned bal = __ballot_sync(kFull, keep);
+    if (keep) sh.pq[(pt + __popc(bal & lanemask_lt())) & (kQueue - 1)] = make_int2((ol << 26) | tgt, __float_as_int(c0));
+    pt += __popc(bal);
+    drainB(false);
+  }
+  drainB(true);
+  drainC(true);
+  return running;
+}
+
+__global__ void __launch_bounds__(kSegWarps * 32) k_seg(const __grid_constant__ Params P) {
+  __shared__ SegWarp shw[kSegWarps];
+  __shared__ float s_rMinO[6], s_rMaxO[6];
+  __shared__ BlockShared bsh;
+  Slot S(P, blockIdx.y);
+  SlotHeader* H = S.hdr();
+  const int cap = P.L.cap_seg;
+  const int nMD = H->n[LST_MD_];
+  const int nSuper = (nMD + kSegWarps * kChunk - 1) / (kSegWarps * kChunk);
+  const int lane = (int)lane_id();
+  SegWarp& sh = shw[threadIdx.x >> 5];
+  if (threadIdx.x < 6) {
+    s_rMinO[threadIdx.x] = r_min_of(H, 0, threadIdx.x);
+    s_rMaxO[threadIdx.x] = r_max_of(H, 0, threadIdx.x);
+  }
+  __syncthreads();
+  int* seg_start = S.seg_start();
   unsigned long long space = 0, evals = 0;
   for (;;) {
-    __syncthreads();  // previous chunk fully consumed (and rMinO / rMaxO visible)
-    if (tid == 0) {
-      sh.chunk = (int)atomicAdd(&H->ticket[LST_SEG_], 1u);
-      sh.tMax = 0;
-    }
-    __syncthreads();
-    const int c = sh.chunk;
-    if (c >= nChunks) {
-      if (c == 0 && tid == 0) {  // no MDs at all: the first ticket publishes the empty result
-        publish_total(H, LST_SEG_, 0, P.L.cap_seg);
+    const int C = block_ticket(&H->ticket[LST_SEG_], bsh);
+    if (C >= nSuper) {
+      if (C == 0 && threadIdx.x == 0) {  // no MDs at all: the first ticket publishes the empty result
+        publish_total(H, LST_SEG_, 0, cap);
         seg_start[0] = 0;
       }
       break;
     }
-    const int i0 = c * kSegChunk, kn = min(kSegChunk, nMD - i0);
-    int nt = 0;
-    if (tid < kn) {
-      const int i = i0 + tid;
-      const float4 a = anchor[i];
+    const int i0 = (C * kSegWarps + (int)(threadIdx.x >> 5)) * kChunk, i = i0 + lane;
+    int nt = 0, row0 = 0;
+    if (i < nMD) {
+      const float4 a = S.md_anchor()[i];
       const float2 x = S.md_aux()[i];
       const int A = S.md_module()[i];
-      const int row0 = P.map_offsets[A];
+      row0 = P.map_offsets[A];
       nt = P.map_offsets[A + 1] - row0;
       const int layer = P.mod_layer[A];
       float dlo = 1.0f, dhi = -1.0f;
-      if (nt > 0) seg_window(P.cuts, layer, a.w, x.x, x.y, sh.rMinO[layer + 1], sh.rMaxO[layer + 1], dlo, dhi);
-      sh.iAnchor[tid] = a;
-      sh.iAux[tid] = x;
-      sh.iKey[tid] = S.md_key()[i];
-      sh.iDlo[tid] = dlo;
-      sh.iDhi[tid] = dhi;
-      sh.iRow0[tid] = row0;
-      sh.iNt[tid] = nt;
-      sh.iLayer[tid] = layer;
+      if (nt > 0) seg_window(P.cuts, layer, a.w, x.x, x.y, s_rMinO[layer + 1], s_rMaxO[layer + 1], dlo, dhi);
+      sh.a4[lane] = a;
+      sh.aux[lane] = x;
+      sh.key[lane] = S.md_key()[i];
+      sh.dlo[lane] = dlo;
+      sh.dhi[lane] = dhi;
+      sh.layer[lane] = layer;
     }
-    if (tid < kSegChunk) sh.kCnt[tid] = 0;
-    if (tid < kSegChunk) {  // warps 0 and 1
-      const int m = __reduce_max_sync(0xffffffffu, nt);
-      if (lane_id() == 0 && m > 0) atomicMax(&sh.tMax, m);
-    }
-    __syncthreads();
-    const int tStar = sh.tMax;
-    int total = 0;
-    if (tStar > 0) total = seg_walk(P, S, sh, i0, kn, tStar, false, 0, space, evals);
-    // where do this chunk's segments start?
-    if (tid < 32) {
-      const int b = lookback_exclusive(S.lb_seg(), c, total);
-      if (tid == 0) sh.base = b;
-    }
-    __syncthreads();
-    const int base = sh.base;
+    sh.cnt[lane] = 0;
+    int nPairs;
+    const int off = warp_excl_scan(nt, nPairs);
+    build_owner_table(nt, sh.tab);
+    const int total = seg_walk<false>(P, S, sh, nt, off, nPairs, row0, i0, 0, space, evals);
+    const int base = block_base<kSegWarps>(S.lb(LST_SEG_), C, total, bsh);
+    __syncwarp();
     if (total <= kSegStash) {
-      for (int j = tid; j < total; j += kSegThreads) {
-        const int ko = sh.stKO[j], k = (int)((unsigned)ko >> 24), o = ko & 0xffffff;
-        if (base + j < P.L.cap_seg) {
-          const float4 v = sh.stV[j], ai = sh.iAnchor[k], ao = anchor[o];
-          S.seg_md()[base + j] = make_int2(i0 + k, o);
-          S.seg_f()[base + j] = make_float4(v.x, v.y, atan2f(ai.x * ao.y - ai.y * ao.x, ai.x * ao.x + ai.y * ao.y),
-                                            atan2f(v.z, v.w));
-        }
+      for (int t = lane; t < total; t += 32) {
+        const int v = sh.stI[t], ol = (int)((unsigned)v >> 26), o = v & (kMaxCap - 1);
+        const float2 f = sh.stV[t];
+        seg_emit(P, S, sh, base + t, i0 + ol, ol, o, f.x, f.y);
       }
     } else {
-      seg_walk(P, S, sh, i0, kn, tStar, true, base, space, evals);  // rare: more segments than the stash holds
+      if (lane == 0) atomicAdd(&H->rewalk[LST_SEG_], 1ull);
+      seg_walk<true>(P, S, sh, nt, off, nPairs, row0, i0, base, space, evals);
     }
-    // first segment of every inner MD of the chunk
     {
-      const int v = (tid < kn) ? sh.kCnt[tid] : 0;
       int tot;
-      const int ex = block_excl_scan<kSegThreads>(v, tot);
-      if (tid < kn) seg_start[i0 + tid] = min(base + ex, P.L.cap_seg);
+      const int ex = warp_excl_scan(sh.cnt[lane], tot);
+      if (i < nMD) seg_start[i] = min(base + ex, cap);
+      if (i == nMD - 1) {
+        seg_start[nMD] = min(base + total, cap);
+        publish_total(H, LST_SEG_, base + total, cap);
+      }
     }
-    if (c == nChunks - 1 && tid == 0) {
-      publish_total(H, LST_SEG_, base + total, P.L.cap_seg);
-      seg_start[nMD] = min(base + total, P.L.cap_seg);
-    }
+    __syncwarp();
   }
-#pragma unroll
-  for (int d = 16; d > 0; d >>= 1) space += __shfl_down_sync(0xffffffffu, space, d);
-  if (lane_id() == 0 && space) atomicAdd(&H->cand[LST_SEG_], space);
-  if (tid == 0 && evals) atomicAdd(&H->eval[LST_SEG_], evals);
+  space = warp_sum_ull(space);
+  evals = warp_sum_ull(evals);
+  if (lane == 0 && space) atomicAdd(&H->cand[LST_SEG_], space);
+  if (lane == 0 && evals) atomicAdd(&H->eval[LST_SEG_], evals);
 }
 
 // ------------------------------------------------------------------------------------------
-// a3: triplets. One thread per first segment a = (m1, m2); candidates are the segments leaving
-// m2, a contiguous range because segments are stored by inner MD.
+// a3: triplets.  Owner = first segment a = (m1, m2); candidates are the segments leaving m2, a
+// contiguous range because segments are stored by inner MD.
 // ------------------------------------------------------------------------------------------
-template <bool FILL>
-__global__ void __launch_bounds__(kScanChunk) k_t3(const __grid_constant__ Params P) {
-  Slot S(P, blockIdx.y);
-  SlotHeader* H = S.hdr();
-  const int nSeg = H->n[LST_SEG_];
-  const int nChunks = (nSeg + kScanChunk - 1) / kScanChunk;
-  const int* seg_start = S.seg_start();
+constexpr int kT3Stash = 128;
+struct T3Warp {
+  float4 p1[32], p2[32];
+  int2 md[32];
+  int layer[32], tab[32], cnt[32];
+  int stI[kT3Stash];
+  float2 stV[kT3Stash];
+};
+
+__device__ __forceinline__ void t3_emit(const Params& P, const Slot& S, const T3Warp& sh, int pos, int a, int ol, int b,
+                                        float kappa, float chi2) {
+  if (pos >= P.L.cap_t3) return;
+  const int2 ma = sh.md[ol];
+  S.t3_pack()[pos] = make_int4(ma.x, ma.y, S.seg_md()[b].y, __float_as_int(kappa));
+  S.t3_seg()[pos] = make_int2(a, b);
+  S.t3_chi2()[pos] = chi2;
+}
+
+template <bool DIRECT>
+__device__ __forceinline__ int t3_walk(const Params& P, const Slot& S, T3Warp& sh, int n, int off, int total, int b0,
+                                       int a0, int base) {
   const int2* seg_md = S.seg_md();
   const float4* anchor = S.md_anchor();
+  const int lane = (int)lane_id();
+  int running = 0;
+  for (int tb = 0; tb < total; tb += 32) {
+    const int rk = tile_owner(n, off, tb);
+    const int j = tb + lane;
+    const int ol = (j < total) ? sh.tab[rk] : 0;
+    const int b = __shfl_sync(kFull, b0, ol) + (j - __shfl_sync(kFull, off, ol));
+    bool pass = false;
+    float kappa = 0.0f, chi2 = 0.0f;
+    if (j < total) pass = t3_select(P.cuts, sh.layer[ol], sh.p1[ol], sh.p2[ol], anchor[seg_md[b].y], kappa, chi2);
+    const unsigned bal = __ballot_sync(kFull, pass);
+    if (pass) {
+      const int pos = running + __popc(bal & lanemask_lt());
+      if (!DIRECT) {
+        atomicAdd(&sh.cnt[ol], 1);
+        if (pos < kT3Stash) { sh.stI[pos] = (ol << 26) | b; sh.stV[pos] = make_float2(kappa, chi2); }
+      } else {
+        t3_emit(P, S, sh, base + pos, a0 + ol, ol, b, kappa, chi2);
+      }
+    }
+    running += __popc(bal);
+  }
+  return running;
+}
+
+__global__ void __launch_bounds__(kWarps * 32) k_t3(const __grid_constant__ Params P) {
+  __shared__ T3Warp shw[kWarps];
+  __shared__ BlockShared bsh;
+  Slot S(P, blockIdx.y);
+  SlotHeader* H = S.hdr();
+  const int cap = P.L.cap_t3;
+  const int nSeg = H->n[LST_SEG_];
+  const int nSuper = (nSeg + kWarps * kChunk - 1) / (kWarps * kChunk);
+  const int lane = (int)lane_id();
+  T3Warp& sh = shw[threadIdx.x >> 5];
+  const int* seg_start = S.seg_start();
   int* t3_start = S.t3_start();
   unsigned long long cand = 0;
-  for (int c = blockIdx.x; c < nChunks; c += gridDim.x) {
-    const int a = c * kScanChunk + threadIdx.x;
-    int count = 0;
+  for (;;) {
+    const int C = block_ticket(&H->ticket[LST_T3_], bsh);
+    if (C >= nSuper) {
+      if (C == 0 && threadIdx.x == 0) {
+        publish_total(H, LST_T3_, 0, cap);
+        t3_start[0] = 0;
+      }
+      break;
+    }
+    const int a0 = (C * kWarps + (int)(threadIdx.x >> 5)) * kChunk, a = a0 + lane;
+    int n = 0, b0 = 0;
     if (a < nSeg) {
-      const int2 ma = seg_md[a];
-      const int b0 = seg_start[ma.y], b1 = seg_start[ma.y + 1];
-      const float4 p1 = anchor[ma.x], p2 = anchor[ma.y];
-      const int layer = P.mod_layer[S.md_module()[ma.x]];
-      const int base = FILL ? S.t3_block_base()[c] + t3_start[a] : 0;
-      cand += (unsigned long long)(b1 - b0);
-      for (int b = b0; b < b1; ++b) {
-        const int m3 = seg_md[b].y;
-        float kappa, chi2;
-        if (t3_select(P.cuts, layer, p1, p2, anchor[m3], kappa, chi2)) {
-          if (FILL) {
-            const int pos = base + count;
-            if (pos < P.L.cap_t3) {
-              S.t3_pack()[pos] = make_int4(ma.x, ma.y, m3, __float_as_int(kappa));
-              S.t3_seg()[pos] = make_int2(a, b);
-              S.t3_chi2()[pos] = chi2;
-            }
-          }
-          ++count;
-        }
+      const int2 ma = S.seg_md()[a];
+      b0 = seg_start[ma.y];
+      n = seg_start[ma.y + 1] - b0;
+      sh.md[lane] = ma;
+      if (n > 0) {
+        sh.p1[lane] = S.md_anchor()[ma.x];
+        sh.p2[lane] = S.md_anchor()[ma.y];
+        sh.layer[lane] = P.mod_layer[S.md_module()[ma.x]];
       }
-      if (FILL) t3_start[a] = min(base, P.L.cap_t3);
     }
-    if (!FILL) {
+    sh.cnt[lane] = 0;
+    cand += (unsigned long long)n;
+    int total_c;
+    const int off = warp_excl_scan(n, total_c);
+    build_owner_table(n, sh.tab);
+    const int total = t3_walk<false>(P, S, sh, n, off, total_c, b0, a0, 0);
+    const int base = block_base<kWarps>(S.lb(LST_T3_), C, total, bsh);
+    __syncwarp();
+    if (total <= kT3Stash) {
+      for (int t = lane; t < total; t += 32) {
+        const int v = sh.stI[t], ol = (int)((unsigned)v >> 26), b = v & (kMaxCap - 1);
+        const float2 f = sh.stV[t];
+        t3_emit(P, S, sh, base + t, a0 + ol, ol, b, f.x, f.y);
+      }
+    } else {
+      if (lane == 0) atomicAdd(&H->rewalk[LST_T3_], 1ull);
+      t3_walk<true>(P, S, sh, n, off, total_c, b0, a0, base);
+    }
+    {
       int tot;
-      const int ex = block_excl_scan<kScanChunk>(count, tot);
-      if (a < nSeg) t3_start[a] = ex;
-      if (threadIdx.x == 0) S.t3_block_base()[c] = tot;
-    }
-  }
-  if (!FILL) {
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) cand += __shfl_down_sync(0xffffffffu, cand, d);
-    if (lane_id() == 0 && cand) { atomicAdd(&H->cand[LST_T3_], cand); atomicAdd(&H->eval[LST_T3_], cand); }
-    if (last_block_done(&H->done[2], gridDim.x)) {
-      const int total = block_scan_array<kScanChunk>(S.t3_block_base(), nChunks, -1);
-      if (threadIdx.x == 0) {
-        publish_total(H, LST_T3_, total, P.L.cap_t3);
-        t3_start[nSeg] = min(total, P.L.cap_t3);
+      const int ex = warp_excl_scan(sh.cnt[lane], tot);
+      if (a < nSeg) t3_start[a] = min(base + ex, cap);
+      if (a == nSeg - 1) {
+        t3_start[nSeg] = min(base + total, cap);
+        publish_total(H, LST_T3_, base + total, cap);
       }
     }
+    __syncwarp();
   }
+  cand = warp_sum_ull(cand);
+  if (lane == 0 && cand) { atomicAdd(&H->cand[LST_T3_], cand); atomicAdd(&H->eval[LST_T3_], cand); }
 }
 
 // ------------------------------------------------------------------------------------------
-// a4: quintuplets. One thread per inner triplet A = (m1, m2, m3); candidates are the triplets
-// whose first MD is m3: [t3_start[seg_start[m3]], t3_start[seg_start[m3 + 1]]), contiguous
-// because triplets are stored by first segment and segments by inner MD.
+// a4: quintuplets.  Owner = inner triplet A = (m1, m2, m3); candidates are the triplets whose
+// first MD is m3: [t3_start[seg_start[m3]], t3_start[seg_start[m3 + 1]]), contiguous because
+// triplets are stored by first segment and segments by inner MD.  Two levels: the curvature match
+// Q2 (one 4-byte load and a compare) on every candidate, survivors compacted into a queue; the
+// two fits on full tiles of survivors.
 // ------------------------------------------------------------------------------------------
-template <bool FILL>
-__global__ void __launch_bounds__(kScanChunk) k_t5(const __grid_constant__ Params P) {
-  Slot S(P, blockIdx.y);
-  SlotHeader* H = S.hdr();
-  const int nT3 = H->n[LST_T3_];
-  const int nChunks = (nT3 + kScanChunk - 1) / kScanChunk;
-  const int* seg_start = S.seg_start();
-  const int* t3_start = S.t3_start();
+constexpr int kT5Stash = 64;
+struct T5Warp {
+  float4 p[3][32];
+  float kA[32];
+  int layer[32], tab[32], cnt[32];
+  int2 q[kQueue];
+  int stI[kT5Stash];
+  float stV[3][kT5Stash];
+};
+
+__device__ __forceinline__ void t5_emit(const Params& P, const Slot& S, int pos, int A, int B, float kfit, float chi2xy,
+                                        float chi2rz) {
+  if (pos >= P.L.cap_t5) return;
+  const int4 ta = S.t3_pack()[A], tb = S.t3_pack()[B];
+  int* md = S.t5_md() + 5 * (size_t)pos;
+  md[0] = ta.x; md[1] = ta.y; md[2] = ta.z; md[3] = tb.y; md[4] = tb.z;
+  S.t5_t3()[pos] = make_int2(A, B);
+  float* f = S.t5_f() + 5 * (size_t)pos;
+  f[0] = __int_as_float(ta.w); f[1] = __int_as_float(tb.w); f[2] = kfit; f[3] = chi2xy; f[4] = chi2rz;
+}
+
+template <bool DIRECT>
+__device__ __forceinline__ int t5_walk(const Params& P, const Slot& S, T5Warp& sh, int n, int off, int total, int B0,
+                                       int A0, int base) {
   const int4* t3_pack = S.t3_pack();
   const float4* anchor = S.md_anchor();
+  const int lane = (int)lane_id();
+  const float dk = P.cuts.t5_dkappa_max;
+  int running = 0, qh = 0, qt = 0;
+  auto fits = [&](bool valid, int2 it) {
+    bool pass = false;
+    T5Out o;
+    const int ol = it.x, Bi = it.y;
+    if (valid) {
+      const int4 tb = t3_pack[Bi];
+      const float4 p[5] = {sh.p[0][ol], sh.p[1][ol], sh.p[2][ol], anchor[tb.y], anchor[tb.z]};
+      pass = t5_select(P.cuts, sh.layer[ol], sh.kA[ol], __int_as_float(tb.w), p, o);
+    }
+    const unsigned bal = __ballot_sync(kFull, pass);
+    if (pass) {
+      const int pos = running + __popc(bal & lanemask_lt());
+      if (!DIRECT) {
+        atomicAdd(&sh.cnt[ol], 1);
+        if (pos < kT5Stash) {
+          sh.stI[pos] = (ol << 26) | Bi;
+          sh.stV[0][pos] = o.kfit; sh.stV[1][pos] = o.chi2xy; sh.stV[2][pos] = o.chi2rz;
+        }
+      } else {
+        t5_emit(P, S, base + pos, A0 + ol, Bi, o.kfit, o.chi2xy, o.chi2rz);
+      }
+    }
+    running += __popc(bal);
+  };
+  auto drain = [&](bool all) {
+    while (qt - qh >= 32 || (all && qt > qh)) {
+      __syncwarp();
+      const bool valid = lane < qt - qh;
+      int2 it = make_int2(0, 0);
+      if (valid) it = sh.q[(qh + lane) & (kQueue - 1)];
+      fits(valid, it);
+      qh += min(32, qt - qh);
+      __syncwarp();
+    }
+  };
+  for (int tb = 0; tb < total; tb += 32) {
+    const int rk = tile_owner(n, off, tb);
+    const int j = tb + lane;
+    const int ol = (j < total) ? sh.tab[rk] : 0;
+    const int Bi = __shfl_sync(kFull, B0, ol) + (j - __shfl_sync(kFull, off, ol));
+    bool keep = false;
+    if (j < total) keep = fabsf(sh.kA[ol] - __int_as_float(t3_pack[Bi].w)) <= dk;   // Q2, exactly as t5_select
+    const unsigned bal = __ballot_sync(kFull, keep);
+    if (keep) sh.q[(qt + __popc(bal & lanemask_lt())) & (kQueue - 1)] = make_int2(ol, Bi);
+    qt += __popc(bal);
+    drain(false);
+  }
+  drain(true);
+  return running;
+}
+
+__global__ void __launch_bounds__(kWarps * 32) k_t5(const __grid_constant__ Params P) {
+  __shared__ T5Warp shw[kWarps];
+  __shared__ BlockShared bsh;
+  Slot S(P, blockIdx.y);
+  SlotHeader* H = S.hdr();
+  const int cap = P.L.cap_t5;
+  const int nT3 = H->n[LST_T3_];
+  const int nSuper = (nT3 + kWarps * kChunk - 1) / (kWarps * kChunk);
+  const int lane = (int)lane_id();
+  T5Warp& sh = shw[threadIdx.x >> 5];
+  const int* seg_start = S.seg_start();
+  const int* t3_start = S.t3_start();
   int* t5_start = S.t5_start();
   unsigned long long cand = 0;
-  for (int c = blockIdx.x; c < nChunks; c += gridDim.x) {
-    const int A = c * kScanChunk + threadIdx.x;
-    int count = 0;
+  for (;;) {
+    const int C = block_ticket(&H->ticket[LST_T5_], bsh);
+    if (C >= nSuper) {
+      if (C == 0 && threadIdx.x == 0) {
+        publish_total(H, LST_T5_, 0, cap);
+        t5_start[0] = 0;
+      }
+      break;
+    }
+    const int A0 = (C * kWarps + (int)(threadIdx.x >> 5)) * kChunk, A = A0 + lane;
+    int n = 0, B0 = 0;
     if (A < nT3) {
-      const int4 ta = t3_pack[A];
-      const int B0 = t3_start[seg_start[ta.z]], B1 = t3_start[seg_start[ta.z + 1]];
-      const int base = FILL ? S.t5_block_base()[c] + t5_start[A] : 0;
-      cand += (unsigned long long)(B1 - B0);
-      if (B1 > B0) {
-        float4 p[5];
-        p[0] = anchor[ta.x];
-        p[1] = anchor[ta.y];
-        p[2] = anchor[ta.z];
+      const int4 ta = S.t3_pack()[A];
+      B0 = t3_start[seg_start[ta.z]];
+      n = t3_start[seg_start[ta.z + 1]] - B0;
+      if (n > 0) {
+        sh.p[0][lane] = S.md_anchor()[ta.x];
+        sh.p[1][lane] = S.md_anchor()[ta.y];
+        sh.p[2][lane] = S.md_anchor()[ta.z];
+        sh.kA[lane] = __int_as_float(ta.w);
         const int layer = P.mod_layer[S.md_module()[ta.x]];
-        const float kA = __int_as_float(ta.w);
-        for (int B = B0; B < B1; ++B) {
-          const int4 tb = t3_pack[B];
-          const float kB = __int_as_float(tb.w);
-          p[3] = anchor[tb.y];
-          p[4] = anchor[tb.z];
-          T5Out o;
-          if (layer <= 1 && t5_select(P.cuts, layer, kA, kB, p, o)) {
-            if (FILL) {
-              const int pos = base + count;
-              if (pos < P.L.cap_t5) {
-                int* md = S.t5_md() + 5 * (size_t)pos;
-                md[0] = ta.x; md[1] = ta.y; md[2] = ta.z; md[3] = tb.y; md[4] = tb.z;
-                S.t5_t3()[pos] = make_int2(A, B);
-                float* f = S.t5_f() + 5 * (size_t)pos;
-                f[0] = kA; f[1] = kB; f[2] = o.kfit; f[3] = o.chi2xy; f[4] = o.chi2rz;
-              }
-            }
-            ++count;
-          }
-        }
+        sh.layer[lane] = layer;
+        if (layer > 1) n = 0;   // cannot happen with a valid module map (targets one layer out); t5_select indexes [layer + 4]
       }
-      if (FILL) t5_start[A] = min(base, P.L.cap_t5);
     }
-    if (!FILL) {
+    sh.cnt[lane] = 0;
+    cand += (unsigned long long)n;
+    int total_c;
+    const int off = warp_excl_scan(n, total_c);
+    build_owner_table(n, sh.tab);
+    const int total = t5_walk<false>(P, S, sh, n, off, total_c, B0, A0, 0);
+    const int base = block_base<kWarps>(S.lb(LST_T5_), C, total, bsh);
+    __syncwarp();
+    if (total <= kT5Stash) {
+      for (int t = lane; t < total; t += 32) {
+        const int v = sh.stI[t], ol = (int)((unsigned)v >> 26), Bi = v & (kMaxCap - 1);
+        t5_emit(P, S, base + t, A0 + ol, Bi, sh.stV[0][t], sh.stV[1][t], sh.stV[2][t]);
+      }
+    } else {
+      if (lane == 0) atomicAdd(&H->rewalk[LST_T5_], 1ull);
+      t5_walk<true>(P, S, sh, n, off, total_c, B0, A0, base);
+    }
+    {
       int tot;
-      const int ex = block_excl_scan<kScanChunk>(count, tot);
-      if (A < nT3) t5_start[A] = ex;
-      if (threadIdx.x == 0) S.t5_block_base()[c] = tot;
-    }
-  }
-  if (!FILL) {
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) cand += __shfl_down_sync(0xffffffffu, cand, d);
-    if (lane_id() == 0 && cand) { atomicAdd(&H->cand[LST_T5_], cand); atomicAdd(&H->eval[LST_T5_], cand); }
-    if (last_block_done(&H->done[3], gridDim.x)) {
-      const int total = block_scan_array<kScanChunk>(S.t5_block_base(), nChunks, -1);
-      if (threadIdx.x == 0) {
-        publish_total(H, LST_T5_, total, P.L.cap_t5);
-        t5_start[nT3] = min(total, P.L.cap_t5);
+      const int ex = warp_excl_scan(sh.cnt[lane], tot);
+      if (A < nT3) t5_start[A] = min(base + ex, cap);
+      if (A == nT3 - 1) {
+        t5_start[nT3] = min(base + total, cap);
+        publish_total(H, LST_T5_, base + total, cap);
       }
     }
+    __syncwarp();
   }
+  cand = warp_sum_ull(cand);
+  if (lane == 0 && cand) { atomicAdd(&H->cand[LST_T5_], cand); atomicAdd(&H->eval[LST_T5_], cand); }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -966,64 +1111,52 @@ __global__ void __launch_bounds__(256) k_pack_values(const __grid_constant__ Par
 // ------------------------------------------------------------------------------------------
 // launchers
 // ------------------------------------------------------------------------------------------
-// `ev` (optional, timing mode): ev[0] is recorded before the first kernel, ev[k + 1] after kernel k.
 #define LST_EV(k) do { if (ev) cudaEventRecord(ev[k], s); } while (0)
+
+// blocks per event of a grid-stride / persistent kernel: enough to fill the machine across the batch
+static int blocks_per_event(int wanted, int n_batch, int resident_per_sm) {
+  const int per_event = max(8, 148 * resident_per_sm / n_batch);
+  return max(1, min(wanted, per_event));
+}
 
 int launch_bin(const Params& P, const HitBatch& in, int n_batch, cudaStream_t s, cudaEvent_t* ev) {
   int n_max = 0;
   for (int b = 0; b < n_batch; ++b) n_max = max(n_max, in.ev[b].n);
-  const int per_event = max(8, 1184 / n_batch);
-  const dim3 g(max(1, min((n_max + 255) / 256, per_event)), (unsigned)n_batch);
+  const unsigned nb = (unsigned)n_batch;
+  const dim3 g(blocks_per_event((n_max + 255) / 256, n_batch, 8), nb);
   LST_EV(0);
-  k_bin_count<<<g, 256, 0, s>>>(P, in);   // + scan of the bin counts by the event's last block
+  k_reset<<<dim3(blocks_per_event((int)(P.L.reset_bytes / 16 + 255) / 256, n_batch, 8), nb), 256, 0, s>>>(P);
   LST_EV(1);
+  k_bin_count<<<g, 256, 0, s>>>(P, in);   // + scan of the bin counts by the event's last block
   LST_EV(2);
   k_bin_scatter<<<g, 256, 0, s>>>(P, in);
   LST_EV(3);
-  k_bin_order<<<dim3((P.L.n_bins + kOrderWarps - 1) / kOrderWarps, (unsigned)n_batch), kOrderWarps * 32, 0, s>>>(P, in);
+  k_bin_order<<<dim3((max(n_max, P.L.n_modules) + 255) / 256, nb), 256, 0, s>>>(P, in);
   LST_EV(4);
-  return 3;
+  return 4;
 }
 
 int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEvent_t* ev) {
   const unsigned nb = (unsigned)n_batch;
-  // persistent chunk loops of T3 / T5: enough blocks to fill the machine across the batch
-  const int per_event = max(8, 1184 / n_batch);
   LST_EV(0);
   switch (stage) {
-    case LST_MD_: {
-      dim3 g(min(per_event, P.L.n_chunk_hits), nb);
-      k_md<false><<<g, kScanChunk, 0, s>>>(P);
-      LST_EV(1);
-      k_md<true><<<g, kScanChunk, 0, s>>>(P);
+    case LST_MD_:
+      k_md<<<dim3(blocks_per_event((P.L.n_chunk[0] + kWarps - 1) / kWarps, n_batch, 6), nb), kWarps * 32, 0, s>>>(P);
       break;
-    }
-    case LST_SEG_: {
-      dim3 g(min(2 * per_event, P.L.n_chunk_md), nb);   // 128-thread blocks: twice as many per SM
-      k_seg<<<g, kSegThreads, 0, s>>>(P);               // single pass (ticket + look-back)
-      LST_EV(1);
-      LST_EV(2);
-      return 1;
-    }
-    case LST_T3_: {
-      dim3 g(min(per_event, P.L.n_chunk_seg), nb);
-      k_t3<false><<<g, kScanChunk, 0, s>>>(P);
-      LST_EV(1);
-      k_t3<true><<<g, kScanChunk, 0, s>>>(P);
+    case LST_SEG_:
+      k_seg<<<dim3(blocks_per_event((P.L.n_chunk[1] + kSegWarps - 1) / kSegWarps, n_batch, 8), nb), kSegWarps * 32, 0, s>>>(P);
       break;
-    }
-    case LST_T5_: {
-      dim3 g(min(per_event, P.L.n_chunk_t3), nb);
-      k_t5<false><<<g, kScanChunk, 0, s>>>(P);
-      LST_EV(1);
-      k_t5<true><<<g, kScanChunk, 0, s>>>(P);
+    case LST_T3_:
+      k_t3<<<dim3(blocks_per_event((P.L.n_chunk[2] + kWarps - 1) / kWarps, n_batch, 6), nb), kWarps * 32, 0, s>>>(P);
       break;
-    }
+    case LST_T5_:
+      k_t5<<<dim3(blocks_per_event((P.L.n_chunk[3] + kWarps - 1) / kWarps, n_batch, 4), nb), kWarps * 32, 0, s>>>(P);
+      break;
     default:
       return 0;
   }
-  LST_EV(2);
-  return 2;
+  LST_EV(1);
+  return 1;
 }
 
 int launch_gather_hits(const Params& P, int kind, int n, cudaStream_t s) {

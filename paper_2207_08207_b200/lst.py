@@ -20,8 +20,7 @@ LIB_PATH = os.path.join(HERE, "liblst.so")
 N_LAYERS = 6
 MD, SEG, T3, T5 = 0, 1, 2, 3
 KIND_NAMES = ("md", "seg", "t3", "t5")
-KERNEL_NAMES = ("bin_count", "bin_unused", "bin_scatter", "bin_order", "md_count", "md_fill", "seg_count", "seg_fill",
-                "t3_count", "t3_fill", "t5_count", "t5_fill")
+KERNEL_NAMES = ("reset", "bin_count", "bin_scatter", "bin_order", "md", "seg", "t3", "t5")   # lst_stats.kernel_ms[0..7]
 HITS_PER_OBJECT = (2, 4, 6, 10)
 VALUES_PER_OBJECT = (4, 4, 2, 5)
 
@@ -91,7 +90,8 @@ class T5View(C.Structure):
 
 class Stats(C.Structure):
     _fields_ = [("n_hits", C.c_int32), ("needed", C.c_int64 * 4), ("candidates", C.c_int64 * 4),
-                ("evaluated", C.c_int64 * 4), ("overflow", C.c_int32), ("bad_hits", C.c_int32), ("stage_ms", C.c_float * 5), ("kernel_ms", C.c_float * 12)]
+                ("evaluated", C.c_int64 * 4), ("overflow", C.c_int32), ("bad_hits", C.c_int32), ("stage_ms", C.c_float * 5), ("kernel_ms", C.c_float * 12),
+                ("rewalks", C.c_int64 * 4)]
 
 
 # every symbol include/lst.h declares: name -> (restype, argtypes)
@@ -277,7 +277,7 @@ class Lst:
         self._check(self.lib.lst_get_stats(self.h, slot, C.byref(s)), "lst_get_stats")
         return dict(n_hits=int(s.n_hits), needed=[int(v) for v in s.needed], candidates=[int(v) for v in s.candidates],
                     evaluated=[int(v) for v in s.evaluated], overflow=int(s.overflow), bad_hits=int(s.bad_hits), stage_ms=[float(v) for v in s.stage_ms],
-                    kernel_ms=[float(v) for v in s.kernel_ms])
+                    kernel_ms=[float(v) for v in s.kernel_ms], rewalks=[int(v) for v in s.rewalks])
 
     def mds(self, slot: int) -> dict:
         v = MdView()
