@@ -34,7 +34,7 @@ import numpy as np  # noqa: E402
 METRIC = "events/sec at PU200-like density (1 B200)"
 UNIT = "events/s"
 N_EVENTS = 64
-N_STREAMS = 4
+N_STREAMS = int(os.environ.get("LST_BENCH_STREAMS", "4"))   # BASELINE.json configs[2]: 4 streams (override: experiments only)
 # SURVEY.md 8(d) algorithmic bytes per unit (each input read once, each output written once)
 MAP_BYTES = 4 * (69630 + 6121)
 # SPEC operations per candidate (every sqrt and div counted as one)

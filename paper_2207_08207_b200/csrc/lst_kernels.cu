@@ -353,17 +353,24 @@ __device__ __forceinline__ unsigned long long ld_status(const unsigned long long
   asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
   return v;
 }
-// Called by all lanes of a warp. Returns the number of objects of chunks 0 .. c-1.  Only the
-// warp with publish = true writes chunk c's status; the other warps of the block read along.
-__device__ __forceinline__ int lookback_exclusive(unsigned long long* status, int c, int total, bool publish) {
-  const int lane = (int)lane_id();
-  if (publish && lane == 0) st_status(status + c, ((c == 0 ? 2ull : 1ull) << 62) | (unsigned)total);
+// A chunk's total is published as soon as its walk is over (status 1 = total only), so no warp ever
+// waits on another warp's look-back, only on its walk.
+__device__ __forceinline__ void publish_aggregate(unsigned long long* status, int c, int total) {
+  if (lane_id() == 0) st_status(status + c, ((c == 0 ? 2ull : 1ull) << 62) | (unsigned)total);
+}
+// Called by all lanes of a warp, after publish_aggregate(c).  Returns the number of objects of
+// chunks 0 .. c-1 and publishes chunk c's inclusive prefix (status 2).
+__device__ __forceinline__ int resolve_base(unsigned long long* status, int c, int total) {
   if (c == 0) return 0;
+  const int lane = (int)lane_id();
   int sum = 0;
   for (int j = c - 1;; j -= 32) {
     const int idx = j - lane;
     unsigned long long v = (idx >= 0) ? ld_status(status + idx) : (2ull << 62);
-    while (__any_sync(kFull, (v >> 62) == 0)) {
+    unsigned ns = 32;
+    while (__any_sync(kFull, (v >> 62) == 0)) {   // a predecessor is still walking: back off, do not burn issue slots
+      __nanosleep(ns);
+      if (ns < 1024) ns <<= 1;
       if ((v >> 62) == 0) v = ld_status(status + idx);
     }
     const unsigned pmask = __ballot_sync(kFull, (v >> 62) == 2);
@@ -374,32 +381,14 @@ __device__ __forceinline__ int lookback_exclusive(unsigned long long* status, in
     sum += contrib;
     if (pmask) break;
   }
-  if (publish && lane == 0) st_status(status + c, (2ull << 62) | (unsigned)(sum + total));
+  if (lane == 0) st_status(status + c, (2ull << 62) | (unsigned)(sum + total));
   return sum;
 }
-
-// The unit of the ticket and of the look-back is the BLOCK: NW warps take NW consecutive chunks
-// of 32 owners (a "super-chunk"), so an event has few units in flight and the look-back is one
-// or two steps deep.  Two block barriers per super-chunk; everything between them is per warp.
-struct BlockShared {
-  int ticket;
-  int tot[8];
-};
-// Next super-chunk of the block (barrier: also separates the shared-memory use of two rounds).
-__device__ __forceinline__ int block_ticket(unsigned* ticket, BlockShared& bs) {
-  if (threadIdx.x == 0) bs.ticket = (int)atomicAdd(ticket, 1u);
-  __syncthreads();
-  return bs.ticket;
-}
-// Index of the first object of this warp's chunk, given the number of objects `total` it found.
-template <int NW>
-__device__ __forceinline__ int block_base(unsigned long long* status, int C, int total, BlockShared& bs) {
-  const int w = threadIdx.x >> 5, lane = (int)lane_id();
-  if (lane == 0) bs.tot[w] = total;
-  __syncthreads();
-  int block_total;
-  const int ex = warp_excl_scan(lane < NW ? bs.tot[lane] : 0, block_total);
-  return lookback_exclusive(status, C, block_total, w == 0) + __shfl_sync(kFull, ex, w);
+// Next chunk of 32 owners of this warp.
+__device__ __forceinline__ int warp_ticket(unsigned* ticket) {
+  int c = 0;
+  if (lane_id() == 0) c = (int)atomicAdd(ticket, 1u);
+  return __shfl_sync(kFull, c, 0);
 }
 
 constexpr int kWarps = 8;        // warps per block of the MD / T3 / T5 kernels
@@ -413,29 +402,29 @@ constexpr int kQueue = 64;       // queue slots per warp (a push adds <= 32, a d
 constexpr int kMdStash = 96;
 struct MdWarp {
   float4 lo[32];
-  float key[32];
-  int mod[32], layer[32], tab[32], cnt[32];
-  int stI[kMdStash];
-  float stS[kMdStash];
+  int layer[32], tab[32];
+  int cnt[2][32];               // objects per owner, of the chunk being walked / the chunk awaiting its base
+  int stI[2][kMdStash];
+  float stS[2][kMdStash];
 };
 
-__device__ __forceinline__ void md_emit(const Params& P, const Slot& S, const MdWarp& sh, int pos, int i, int ol, int u,
-                                        float sinA) {
+// i = index of the lower hit (owner), u = index of the upper hit.
+__device__ __forceinline__ void md_emit(const Params& P, const Slot& S, int pos, int i, int u, float sinA) {
   if (pos >= P.L.cap_md) return;
-  const float4 lo = sh.lo[ol], up = S.hit4()[u];
+  const float4 lo = S.hit4()[i], up = S.hit4()[u];
   const float dx = up.x - lo.x, dy = up.y - lo.y;
   const float cross = lo.x * dy - lo.y * dx, dot = lo.x * dx + lo.y * dy;   // as in md_select
   S.md_anchor()[pos] = lo;
   S.md_aux()[pos] = make_float2(up.w, sinA);
-  S.md_key()[pos] = sh.key[ol];
+  S.md_key()[pos] = S.hit_key()[i];
   S.md_hits()[pos] = make_int2(S.hit_orig()[i], S.hit_orig()[u]);
   S.md_out()[pos] = make_float2(atan2f(lo.x * up.y - lo.y * up.x, lo.x * up.x + lo.y * up.y), atan2f(cross, dot));
-  S.md_module()[pos] = sh.mod[ol];
+  S.md_module()[pos] = S.hit_module()[i];
 }
 
 template <bool DIRECT>
-__device__ __forceinline__ int md_walk(const Params& P, const Slot& S, MdWarp& sh, int n, int off, int total, int j0,
-                                       int i0, int base) {
+__device__ __forceinline__ int md_walk(const Params& P, const Slot& S, MdWarp& sh, int buf, int n, int off, int total,
+                                       int j0, int i0, int base) {
   const float4* hit4 = S.hit4();
   const int lane = (int)lane_id();
   int running = 0;
@@ -455,10 +444,10 @@ __device__ __forceinline__ int md_walk(const Params& P, const Slot& S, MdWarp& s
     if (pass) {
       const int pos = running + __popc(bal & lanemask_lt());
       if (!DIRECT) {
-        atomicAdd(&sh.cnt[ol], 1);
-        if (pos < kMdStash) { sh.stI[pos] = (ol << 26) | u; sh.stS[pos] = o.sinA; }
+        atomicAdd(&sh.cnt[buf][ol], 1);
+        if (pos < kMdStash) { sh.stI[buf][pos] = (ol << 26) | u; sh.stS[buf][pos] = o.sinA; }
       } else {
-        md_emit(P, S, sh, base + pos, i0 + ol, ol, u, o.sinA);
+        md_emit(P, S, base + pos, i0 + ol, u, o.sinA);
       }
     }
     running += __popc(bal);
@@ -469,12 +458,11 @@ __device__ __forceinline__ int md_walk(const Params& P, const Slot& S, MdWarp& s
 __global__ void __launch_bounds__(kWarps * 32) k_md(const __grid_constant__ Params P) {
   __shared__ MdWarp shw[kWarps];
   __shared__ float s_w[6], s_rmaxU[6];
-  __shared__ BlockShared bsh;
   Slot S(P, blockIdx.y);
   SlotHeader* H = S.hdr();
   const int nmod = P.L.n_modules, cap = P.L.cap_md;
   const int nLower = H->n_lower;
-  const int nSuper = (nLower + kWarps * kChunk - 1) / (kWarps * kChunk);
+  const int nChunks = (nLower + kChunk - 1) / kChunk;
   const int lane = (int)lane_id();
   MdWarp& sh = shw[threadIdx.x >> 5];
   if (threadIdx.x < 6) {
@@ -488,11 +476,46 @@ __global__ void __launch_bounds__(kWarps * 32) k_md(const __grid_constant__ Para
   const int* hmod = S.hit_module();
   int* md_start = S.md_start();
   int* info = reinterpret_cast<int*>(S.mod_info());
+  unsigned long long* status = S.lb(LST_MD_);
   unsigned long long evals = 0;
+
+  // writes what depends on the chunk's base: per-module tables, the grand total (+ the objects
+  // themselves when they sit in the stash)
+  auto finish = [&](int C, int b, int total, int base, bool from_stash) {
+    const int i0 = C * kChunk, i = i0 + lane;
+    if (from_stash)
+      for (int t = lane; t < total; t += 32) {
+        const int v = sh.stI[b][t];
+        md_emit(P, S, base + t, i0 + (int)((unsigned)v >> 26), v & (kMaxCap - 1), sh.stS[b][t]);
+      }
+    int tot;
+    const int first = min(base + warp_excl_scan(sh.cnt[b][lane], tot), cap);
+    if (i < nLower) {
+      // module table: the first lower hit of a module (and the modules without lower hits before it)
+      const int m = hmod[i], m_prev = (i > 0) ? hmod[i - 1] : -1;
+      for (int mm = m_prev + 1; mm <= m; ++mm) {
+        md_start[mm] = first;
+        info[4 * mm] = first;
+        if (mm > 0) info[4 * (mm - 1) + 1] = first;
+      }
+      if (i == nLower - 1) {
+        const int end = min(base + total, cap);
+        for (int mm = m + 1; mm <= nmod; ++mm) {
+          md_start[mm] = end;
+          if (mm < nmod) info[4 * mm] = end;
+          info[4 * (mm - 1) + 1] = end;
+        }
+        publish_total(H, LST_MD_, base + total, cap);
+      }
+    }
+    __syncwarp();
+  };
+
+  int buf = 0, pC = -1, pTotal = 0;   // pC: chunk whose objects wait in stash[buf ^ 1] for their base
   for (;;) {
-    const int C = block_ticket(&H->ticket[LST_MD_], bsh);
-    if (C >= nSuper) {
-      if (C == 0 && threadIdx.x < 32) {  // no lower hits at all: the first ticket publishes the empty result
+    const int C = warp_ticket(&H->ticket[LST_MD_]);
+    if (C >= nChunks) {
+      if (C == 0) {  // no lower hits at all: the first ticket publishes the empty result
         for (int m = lane; m <= nmod; m += 32) {
           md_start[m] = 0;
           if (m < nmod) { info[4 * m] = 0; info[4 * m + 1] = 0; }
@@ -501,17 +524,15 @@ __global__ void __launch_bounds__(kWarps * 32) k_md(const __grid_constant__ Para
       }
       break;
     }
-    const int i0 = (C * kWarps + (int)(threadIdx.x >> 5)) * kChunk, i = i0 + lane;
-    int n = 0, j0 = 0, m = 0;
+    const int i0 = C * kChunk, i = i0 + lane;
+    int n = 0, j0 = 0;
     if (i < nLower) {
-      m = hmod[i];
+      const int m = hmod[i];
       const int layer = P.mod_layer[m];
       const int u0 = (int)bs[nmod + m], u1 = (int)bs[nmod + m + 1];
       const float4 lo = S.hit4()[i];
       const float kl = hkey[i];
       sh.lo[lane] = lo;
-      sh.key[lane] = kl;
-      sh.mod[lane] = m;
       sh.layer[lane] = layer;
       const float w = s_w[layer];
       if (u1 > u0 && w >= 0.0f && s_rmaxU[layer] * 1.000001f >= lo.w) {
@@ -524,47 +545,28 @@ __global__ void __launch_bounds__(kWarps * 32) k_md(const __grid_constant__ Para
         n = j1 - j0;
       }
     }
-    sh.cnt[lane] = 0;
+    sh.cnt[buf][lane] = 0;
     evals += (unsigned long long)n;
     int total_c;
     const int off = warp_excl_scan(n, total_c);
     build_owner_table(n, sh.tab);
-    const int total = md_walk<false>(P, S, sh, n, off, total_c, j0, i0, 0);
-    const int base = block_base<kWarps>(S.lb(LST_MD_), C, total, bsh);
+    const int total = md_walk<false>(P, S, sh, buf, n, off, total_c, j0, i0, 0);
+    publish_aggregate(status, C, total);
     __syncwarp();
+    if (pC >= 0) {   // the previous chunk has had a whole walk of slack: its base is (almost always) there
+      finish(pC, buf ^ 1, pTotal, resolve_base(status, pC, pTotal), true);
+      pC = -1;
+    }
     if (total <= kMdStash) {
-      for (int t = lane; t < total; t += 32) {
-        const int v = sh.stI[t], ol = (int)((unsigned)v >> 26), u = v & (kMaxCap - 1);
-        md_emit(P, S, sh, base + t, i0 + ol, ol, u, sh.stS[t]);
-      }
-    } else {
+      pC = C; pTotal = total; buf ^= 1;
+    } else {           // does not fit the stash: resolve now and walk again, writing directly
       if (lane == 0) atomicAdd(&H->rewalk[LST_MD_], 1ull);
-      md_walk<true>(P, S, sh, n, off, total_c, j0, i0, base);
+      const int base = resolve_base(status, C, total);
+      md_walk<true>(P, S, sh, buf, n, off, total_c, j0, i0, base);
+      finish(C, buf, total, base, false);
     }
-    // module table: the first lower hit of a module (and the modules without lower hits before it)
-    {
-      int tot;
-      const int first = min(base + warp_excl_scan(sh.cnt[lane], tot), cap);
-      if (i < nLower) {
-        const int m_prev = (i > 0) ? hmod[i - 1] : -1;
-        for (int mm = m_prev + 1; mm <= m; ++mm) {
-          md_start[mm] = first;
-          info[4 * mm] = first;
-          if (mm > 0) info[4 * (mm - 1) + 1] = first;
-        }
-        if (i == nLower - 1) {
-          const int end = min(base + total, cap);
-          for (int mm = m + 1; mm <= nmod; ++mm) {
-            md_start[mm] = end;
-            if (mm < nmod) info[4 * mm] = end;
-            info[4 * (mm - 1) + 1] = end;
-          }
-          publish_total(H, LST_MD_, base + total, cap);
-        }
-      }
-    }
-    __syncwarp();
   }
+  if (pC >= 0) finish(pC, buf ^ 1, pTotal, resolve_base(status, pC, pTotal), true);
   evals = warp_sum_ull(evals);
   if (lane == 0 && evals) atomicAdd(&H->eval[LST_MD_], evals);
 }
@@ -583,16 +585,17 @@ struct SegWarp {
   float4 a4[32];
   float2 aux[32];
   float key[32], dlo[32], dhi[32];
-  int layer[32], tab[32], ptab[32], cnt[32];
+  int layer[32], tab[32], ptab[32];
   int2 pq[kQueue], cq[kQueue];
-  int stI[kSegStash];
-  float2 stV[kSegStash];
+  int cnt[2][32];
+  int stI[2][kSegStash];
+  float2 stV[2][kSegStash];
 };
 
-__device__ __forceinline__ void seg_emit(const Params& P, const Slot& S, const SegWarp& sh, int pos, int i, int ol, int o,
-                                         float sinS, float z0) {
+// i / o = index of the inner / outer MD.
+__device__ __forceinline__ void seg_emit(const Params& P, const Slot& S, int pos, int i, int o, float sinS, float z0) {
   if (pos >= P.L.cap_seg) return;
-  const float4 ai = sh.a4[ol], ao = S.md_anchor()[o];
+  const float4 ai = S.md_anchor()[i], ao = S.md_anchor()[o];
   const float dx = ao.x - ai.x, dy = ao.y - ai.y;
   const float cross = ai.x * dy - ai.y * dx, dot = ai.x * dx + ai.y * dy;   // as in seg_select
   S.seg_md()[pos] = make_int2(i, o);
@@ -600,8 +603,8 @@ __device__ __forceinline__ void seg_emit(const Params& P, const Slot& S, const S
 }
 
 template <bool DIRECT>
-__device__ __forceinline__ int seg_walk(const Params& P, const Slot& S, SegWarp& sh, int nt, int off, int nPairs, int row0,
-                                        int i0, int base, unsigned long long& space, unsigned long long& evals) {
+__device__ __forceinline__ int seg_walk(const Params& P, const Slot& S, SegWarp& sh, int buf, int nt, int off, int nPairs,
+                                        int row0, int i0, int base, unsigned long long& space, unsigned long long& evals) {
   const float4* anchor = S.md_anchor();
   const float2* aux = S.md_aux();
   const float* mkey = S.md_key();
@@ -620,10 +623,10 @@ __device__ __forceinline__ int seg_walk(const Params& P, const Slot& S, SegWarp&
     if (pass) {
       const int pos = running + __popc(bal & lanemask_lt());
       if (!DIRECT) {
-        atomicAdd(&sh.cnt[ol], 1);
-        if (pos < kSegStash) { sh.stI[pos] = (ol << 26) | o; sh.stV[pos] = make_float2(so.sinS, so.z0); }
+        atomicAdd(&sh.cnt[buf][ol], 1);
+        if (pos < kSegStash) { sh.stI[buf][pos] = (ol << 26) | o; sh.stV[buf][pos] = make_float2(so.sinS, so.z0); }
       } else {
-        seg_emit(P, S, sh, base + pos, i0 + ol, ol, o, so.sinS, so.z0);
+        seg_emit(P, S, base + pos, i0 + ol, o, so.sinS, so.z0);
       }
     }
     running += __popc(bal);
@@ -714,12 +717,11 @@ __device__ __forceinline__ int seg_walk(const Params& P, const Slot& S, SegWarp&
 __global__ void __launch_bounds__(kSegWarps * 32) k_seg(const __grid_constant__ Params P) {
   __shared__ SegWarp shw[kSegWarps];
   __shared__ float s_rMinO[6], s_rMaxO[6];
-  __shared__ BlockShared bsh;
   Slot S(P, blockIdx.y);
   SlotHeader* H = S.hdr();
   const int cap = P.L.cap_seg;
   const int nMD = H->n[LST_MD_];
-  const int nSuper = (nMD + kSegWarps * kChunk - 1) / (kSegWarps * kChunk);
+  const int nChunks = (nMD + kChunk - 1) / kChunk;
   const int lane = (int)lane_id();
   SegWarp& sh = shw[threadIdx.x >> 5];
   if (threadIdx.x < 6) {
@@ -728,17 +730,38 @@ __global__ void __launch_bounds__(kSegWarps * 32) k_seg(const __grid_constant__ 
   }
   __syncthreads();
   int* seg_start = S.seg_start();
+  unsigned long long* status = S.lb(LST_SEG_);
   unsigned long long space = 0, evals = 0;
+
+  auto finish = [&](int C, int b, int total, int base, bool from_stash) {
+    const int i0 = C * kChunk, i = i0 + lane;
+    if (from_stash)
+      for (int t = lane; t < total; t += 32) {
+        const int v = sh.stI[b][t];
+        const float2 f = sh.stV[b][t];
+        seg_emit(P, S, base + t, i0 + (int)((unsigned)v >> 26), v & (kMaxCap - 1), f.x, f.y);
+      }
+    int tot;
+    const int ex = warp_excl_scan(sh.cnt[b][lane], tot);
+    if (i < nMD) seg_start[i] = min(base + ex, cap);
+    if (i == nMD - 1) {
+      seg_start[nMD] = min(base + total, cap);
+      publish_total(H, LST_SEG_, base + total, cap);
+    }
+    __syncwarp();
+  };
+
+  int buf = 0, pC = -1, pTotal = 0;
   for (;;) {
-    const int C = block_ticket(&H->ticket[LST_SEG_], bsh);
-    if (C >= nSuper) {
-      if (C == 0 && threadIdx.x == 0) {  // no MDs at all: the first ticket publishes the empty result
+    const int C = warp_ticket(&H->ticket[LST_SEG_]);
+    if (C >= nChunks) {
+      if (C == 0 && lane == 0) {  // no MDs at all: the first ticket publishes the empty result
         publish_total(H, LST_SEG_, 0, cap);
         seg_start[0] = 0;
       }
       break;
     }
-    const int i0 = (C * kSegWarps + (int)(threadIdx.x >> 5)) * kChunk, i = i0 + lane;
+    const int i0 = C * kChunk, i = i0 + lane;
     int nt = 0, row0 = 0;
     if (i < nMD) {
       const float4 a = S.md_anchor()[i];
@@ -756,34 +779,27 @@ __global__ void __launch_bounds__(kSegWarps * 32) k_seg(const __grid_constant__ 
       sh.dhi[lane] = dhi;
       sh.layer[lane] = layer;
     }
-    sh.cnt[lane] = 0;
+    sh.cnt[buf][lane] = 0;
     int nPairs;
     const int off = warp_excl_scan(nt, nPairs);
     build_owner_table(nt, sh.tab);
-    const int total = seg_walk<false>(P, S, sh, nt, off, nPairs, row0, i0, 0, space, evals);
-    const int base = block_base<kSegWarps>(S.lb(LST_SEG_), C, total, bsh);
+    const int total = seg_walk<false>(P, S, sh, buf, nt, off, nPairs, row0, i0, 0, space, evals);
+    publish_aggregate(status, C, total);
     __syncwarp();
+    if (pC >= 0) {
+      finish(pC, buf ^ 1, pTotal, resolve_base(status, pC, pTotal), true);
+      pC = -1;
+    }
     if (total <= kSegStash) {
-      for (int t = lane; t < total; t += 32) {
-        const int v = sh.stI[t], ol = (int)((unsigned)v >> 26), o = v & (kMaxCap - 1);
-        const float2 f = sh.stV[t];
-        seg_emit(P, S, sh, base + t, i0 + ol, ol, o, f.x, f.y);
-      }
+      pC = C; pTotal = total; buf ^= 1;
     } else {
       if (lane == 0) atomicAdd(&H->rewalk[LST_SEG_], 1ull);
-      seg_walk<true>(P, S, sh, nt, off, nPairs, row0, i0, base, space, evals);
+      const int base = resolve_base(status, C, total);
+      seg_walk<true>(P, S, sh, buf, nt, off, nPairs, row0, i0, base, space, evals);
+      finish(C, buf, total, base, false);
     }
-    {
-      int tot;
-      const int ex = warp_excl_scan(sh.cnt[lane], tot);
-      if (i < nMD) seg_start[i] = min(base + ex, cap);
-      if (i == nMD - 1) {
-        seg_start[nMD] = min(base + total, cap);
-        publish_total(H, LST_SEG_, base + total, cap);
-      }
-    }
-    __syncwarp();
   }
+  if (pC >= 0) finish(pC, buf ^ 1, pTotal, resolve_base(status, pC, pTotal), true);
   space = warp_sum_ull(space);
   evals = warp_sum_ull(evals);
   if (lane == 0 && space) atomicAdd(&H->cand[LST_SEG_], space);
@@ -797,24 +813,24 @@ __global__ void __launch_bounds__(kSegWarps * 32) k_seg(const __grid_constant__ 
 constexpr int kT3Stash = 128;
 struct T3Warp {
   float4 p1[32], p2[32];
-  int2 md[32];
-  int layer[32], tab[32], cnt[32];
-  int stI[kT3Stash];
-  float2 stV[kT3Stash];
+  int layer[32], tab[32];
+  int cnt[2][32];
+  int stI[2][kT3Stash];
+  float2 stV[2][kT3Stash];
 };
 
-__device__ __forceinline__ void t3_emit(const Params& P, const Slot& S, const T3Warp& sh, int pos, int a, int ol, int b,
-                                        float kappa, float chi2) {
+// a / b = index of the first / second segment.
+__device__ __forceinline__ void t3_emit(const Params& P, const Slot& S, int pos, int a, int b, float kappa, float chi2) {
   if (pos >= P.L.cap_t3) return;
-  const int2 ma = sh.md[ol];
+  const int2 ma = S.seg_md()[a];
   S.t3_pack()[pos] = make_int4(ma.x, ma.y, S.seg_md()[b].y, __float_as_int(kappa));
   S.t3_seg()[pos] = make_int2(a, b);
   S.t3_chi2()[pos] = chi2;
 }
 
 template <bool DIRECT>
-__device__ __forceinline__ int t3_walk(const Params& P, const Slot& S, T3Warp& sh, int n, int off, int total, int b0,
-                                       int a0, int base) {
+__device__ __forceinline__ int t3_walk(const Params& P, const Slot& S, T3Warp& sh, int buf, int n, int off, int total,
+                                       int b0, int a0, int base) {
   const int2* seg_md = S.seg_md();
   const float4* anchor = S.md_anchor();
   const int lane = (int)lane_id();
@@ -831,10 +847,10 @@ __device__ __forceinline__ int t3_walk(const Params& P, const Slot& S, T3Warp& s
     if (pass) {
       const int pos = running + __popc(bal & lanemask_lt());
       if (!DIRECT) {
-        atomicAdd(&sh.cnt[ol], 1);
-        if (pos < kT3Stash) { sh.stI[pos] = (ol << 26) | b; sh.stV[pos] = make_float2(kappa, chi2); }
+        atomicAdd(&sh.cnt[buf][ol], 1);
+        if (pos < kT3Stash) { sh.stI[buf][pos] = (ol << 26) | b; sh.stV[buf][pos] = make_float2(kappa, chi2); }
       } else {
-        t3_emit(P, S, sh, base + pos, a0 + ol, ol, b, kappa, chi2);
+        t3_emit(P, S, base + pos, a0 + ol, b, kappa, chi2);
       }
     }
     running += __popc(bal);
@@ -844,68 +860,80 @@ __device__ __forceinline__ int t3_walk(const Params& P, const Slot& S, T3Warp& s
 
 __global__ void __launch_bounds__(kWarps * 32) k_t3(const __grid_constant__ Params P) {
   __shared__ T3Warp shw[kWarps];
-  __shared__ BlockShared bsh;
   Slot S(P, blockIdx.y);
   SlotHeader* H = S.hdr();
   const int cap = P.L.cap_t3;
   const int nSeg = H->n[LST_SEG_];
-  const int nSuper = (nSeg + kWarps * kChunk - 1) / (kWarps * kChunk);
+  const int nChunks = (nSeg + kChunk - 1) / kChunk;
   const int lane = (int)lane_id();
   T3Warp& sh = shw[threadIdx.x >> 5];
   const int* seg_start = S.seg_start();
   int* t3_start = S.t3_start();
+  unsigned long long* status = S.lb(LST_T3_);
   unsigned long long cand = 0;
+
+  auto finish = [&](int C, int b, int total, int base, bool from_stash) {
+    const int a0 = C * kChunk, a = a0 + lane;
+    if (from_stash)
+      for (int t = lane; t < total; t += 32) {
+        const int v = sh.stI[b][t];
+        const float2 f = sh.stV[b][t];
+        t3_emit(P, S, base + t, a0 + (int)((unsigned)v >> 26), v & (kMaxCap - 1), f.x, f.y);
+      }
+    int tot;
+    const int ex = warp_excl_scan(sh.cnt[b][lane], tot);
+    if (a < nSeg) t3_start[a] = min(base + ex, cap);
+    if (a == nSeg - 1) {
+      t3_start[nSeg] = min(base + total, cap);
+      publish_total(H, LST_T3_, base + total, cap);
+    }
+    __syncwarp();
+  };
+
+  int buf = 0, pC = -1, pTotal = 0;
   for (;;) {
-    const int C = block_ticket(&H->ticket[LST_T3_], bsh);
-    if (C >= nSuper) {
-      if (C == 0 && threadIdx.x == 0) {
+    const int C = warp_ticket(&H->ticket[LST_T3_]);
+    if (C >= nChunks) {
+      if (C == 0 && lane == 0) {
         publish_total(H, LST_T3_, 0, cap);
         t3_start[0] = 0;
       }
       break;
     }
-    const int a0 = (C * kWarps + (int)(threadIdx.x >> 5)) * kChunk, a = a0 + lane;
+    const int a0 = C * kChunk, a = a0 + lane;
     int n = 0, b0 = 0;
     if (a < nSeg) {
       const int2 ma = S.seg_md()[a];
       b0 = seg_start[ma.y];
       n = seg_start[ma.y + 1] - b0;
-      sh.md[lane] = ma;
       if (n > 0) {
         sh.p1[lane] = S.md_anchor()[ma.x];
         sh.p2[lane] = S.md_anchor()[ma.y];
         sh.layer[lane] = P.mod_layer[S.md_module()[ma.x]];
       }
     }
-    sh.cnt[lane] = 0;
+    sh.cnt[buf][lane] = 0;
     cand += (unsigned long long)n;
     int total_c;
     const int off = warp_excl_scan(n, total_c);
     build_owner_table(n, sh.tab);
-    const int total = t3_walk<false>(P, S, sh, n, off, total_c, b0, a0, 0);
-    const int base = block_base<kWarps>(S.lb(LST_T3_), C, total, bsh);
+    const int total = t3_walk<false>(P, S, sh, buf, n, off, total_c, b0, a0, 0);
+    publish_aggregate(status, C, total);
     __syncwarp();
+    if (pC >= 0) {
+      finish(pC, buf ^ 1, pTotal, resolve_base(status, pC, pTotal), true);
+      pC = -1;
+    }
     if (total <= kT3Stash) {
-      for (int t = lane; t < total; t += 32) {
-        const int v = sh.stI[t], ol = (int)((unsigned)v >> 26), b = v & (kMaxCap - 1);
-        const float2 f = sh.stV[t];
-        t3_emit(P, S, sh, base + t, a0 + ol, ol, b, f.x, f.y);
-      }
+      pC = C; pTotal = total; buf ^= 1;
     } else {
       if (lane == 0) atomicAdd(&H->rewalk[LST_T3_], 1ull);
-      t3_walk<true>(P, S, sh, n, off, total_c, b0, a0, base);
+      const int base = resolve_base(status, C, total);
+      t3_walk<true>(P, S, sh, buf, n, off, total_c, b0, a0, base);
+      finish(C, buf, total, base, false);
     }
-    {
-      int tot;
-      const int ex = warp_excl_scan(sh.cnt[lane], tot);
-      if (a < nSeg) t3_start[a] = min(base + ex, cap);
-      if (a == nSeg - 1) {
-        t3_start[nSeg] = min(base + total, cap);
-        publish_total(H, LST_T3_, base + total, cap);
-      }
-    }
-    __syncwarp();
   }
+  if (pC >= 0) finish(pC, buf ^ 1, pTotal, resolve_base(status, pC, pTotal), true);
   cand = warp_sum_ull(cand);
   if (lane == 0 && cand) { atomicAdd(&H->cand[LST_T3_], cand); atomicAdd(&H->eval[LST_T3_], cand); }
 }
@@ -921,10 +949,11 @@ constexpr int kT5Stash = 64;
 struct T5Warp {
   float4 p[3][32];
   float kA[32];
-  int layer[32], tab[32], cnt[32];
+  int layer[32], tab[32];
   int2 q[kQueue];
-  int stI[kT5Stash];
-  float stV[3][kT5Stash];
+  int cnt[2][32];
+  int stI[2][kT5Stash];
+  float stV[2][3][kT5Stash];
 };
 
 __device__ __forceinline__ void t5_emit(const Params& P, const Slot& S, int pos, int A, int B, float kfit, float chi2xy,
@@ -939,8 +968,8 @@ __device__ __forceinline__ void t5_emit(const Params& P, const Slot& S, int pos,
 }
 
 template <bool DIRECT>
-__device__ __forceinline__ int t5_walk(const Params& P, const Slot& S, T5Warp& sh, int n, int off, int total, int B0,
-                                       int A0, int base) {
+__device__ __forceinline__ int t5_walk(const Params& P, const Slot& S, T5Warp& sh, int buf, int n, int off, int total,
+                                       int B0, int A0, int base) {
   const int4* t3_pack = S.t3_pack();
   const float4* anchor = S.md_anchor();
   const int lane = (int)lane_id();
@@ -959,10 +988,10 @@ __device__ __forceinline__ int t5_walk(const Params& P, const Slot& S, T5Warp& s
     if (pass) {
       const int pos = running + __popc(bal & lanemask_lt());
       if (!DIRECT) {
-        atomicAdd(&sh.cnt[ol], 1);
+        atomicAdd(&sh.cnt[buf][ol], 1);
         if (pos < kT5Stash) {
-          sh.stI[pos] = (ol << 26) | Bi;
-          sh.stV[0][pos] = o.kfit; sh.stV[1][pos] = o.chi2xy; sh.stV[2][pos] = o.chi2rz;
+          sh.stI[buf][pos] = (ol << 26) | Bi;
+          sh.stV[buf][0][pos] = o.kfit; sh.stV[buf][1][pos] = o.chi2xy; sh.stV[buf][2][pos] = o.chi2rz;
         }
       } else {
         t5_emit(P, S, base + pos, A0 + ol, Bi, o.kfit, o.chi2xy, o.chi2rz);
@@ -999,28 +1028,48 @@ __device__ __forceinline__ int t5_walk(const Params& P, const Slot& S, T5Warp& s
 
 __global__ void __launch_bounds__(kWarps * 32) k_t5(const __grid_constant__ Params P) {
   __shared__ T5Warp shw[kWarps];
-  __shared__ BlockShared bsh;
   Slot S(P, blockIdx.y);
   SlotHeader* H = S.hdr();
   const int cap = P.L.cap_t5;
   const int nT3 = H->n[LST_T3_];
-  const int nSuper = (nT3 + kWarps * kChunk - 1) / (kWarps * kChunk);
+  const int nChunks = (nT3 + kChunk - 1) / kChunk;
   const int lane = (int)lane_id();
   T5Warp& sh = shw[threadIdx.x >> 5];
   const int* seg_start = S.seg_start();
   const int* t3_start = S.t3_start();
   int* t5_start = S.t5_start();
+  unsigned long long* status = S.lb(LST_T5_);
   unsigned long long cand = 0;
+
+  auto finish = [&](int C, int b, int total, int base, bool from_stash) {
+    const int A0 = C * kChunk, A = A0 + lane;
+    if (from_stash)
+      for (int t = lane; t < total; t += 32) {
+        const int v = sh.stI[b][t];
+        t5_emit(P, S, base + t, A0 + (int)((unsigned)v >> 26), v & (kMaxCap - 1), sh.stV[b][0][t], sh.stV[b][1][t],
+                sh.stV[b][2][t]);
+      }
+    int tot;
+    const int ex = warp_excl_scan(sh.cnt[b][lane], tot);
+    if (A < nT3) t5_start[A] = min(base + ex, cap);
+    if (A == nT3 - 1) {
+      t5_start[nT3] = min(base + total, cap);
+      publish_total(H, LST_T5_, base + total, cap);
+    }
+    __syncwarp();
+  };
+
+  int buf = 0, pC = -1, pTotal = 0;
   for (;;) {
-    const int C = block_ticket(&H->ticket[LST_T5_], bsh);
-    if (C >= nSuper) {
-      if (C == 0 && threadIdx.x == 0) {
+    const int C = warp_ticket(&H->ticket[LST_T5_]);
+    if (C >= nChunks) {
+      if (C == 0 && lane == 0) {
         publish_total(H, LST_T5_, 0, cap);
         t5_start[0] = 0;
       }
       break;
     }
-    const int A0 = (C * kWarps + (int)(threadIdx.x >> 5)) * kChunk, A = A0 + lane;
+    const int A0 = C * kChunk, A = A0 + lane;
     int n = 0, B0 = 0;
     if (A < nT3) {
       const int4 ta = S.t3_pack()[A];
@@ -1036,34 +1085,28 @@ __global__ void __launch_bounds__(kWarps * 32) k_t5(const __grid_constant__ Para
         if (layer > 1) n = 0;   // cannot happen with a valid module map (targets one layer out); t5_select indexes [layer + 4]
       }
     }
-    sh.cnt[lane] = 0;
+    sh.cnt[buf][lane] = 0;
     cand += (unsigned long long)n;
     int total_c;
     const int off = warp_excl_scan(n, total_c);
     build_owner_table(n, sh.tab);
-    const int total = t5_walk<false>(P, S, sh, n, off, total_c, B0, A0, 0);
-    const int base = block_base<kWarps>(S.lb(LST_T5_), C, total, bsh);
+    const int total = t5_walk<false>(P, S, sh, buf, n, off, total_c, B0, A0, 0);
+    publish_aggregate(status, C, total);
     __syncwarp();
+    if (pC >= 0) {
+      finish(pC, buf ^ 1, pTotal, resolve_base(status, pC, pTotal), true);
+      pC = -1;
+    }
     if (total <= kT5Stash) {
-      for (int t = lane; t < total; t += 32) {
-        const int v = sh.stI[t], ol = (int)((unsigned)v >> 26), Bi = v & (kMaxCap - 1);
-        t5_emit(P, S, base + t, A0 + ol, Bi, sh.stV[0][t], sh.stV[1][t], sh.stV[2][t]);
-      }
+      pC = C; pTotal = total; buf ^= 1;
     } else {
       if (lane == 0) atomicAdd(&H->rewalk[LST_T5_], 1ull);
-      t5_walk<true>(P, S, sh, n, off, total_c, B0, A0, base);
+      const int base = resolve_base(status, C, total);
+      t5_walk<true>(P, S, sh, buf, n, off, total_c, B0, A0, base);
+      finish(C, buf, total, base, false);
     }
-    {
-      int tot;
-      const int ex = warp_excl_scan(sh.cnt[lane], tot);
-      if (A < nT3) t5_start[A] = min(base + ex, cap);
-      if (A == nT3 - 1) {
-        t5_start[nT3] = min(base + total, cap);
-        publish_total(H, LST_T5_, base + total, cap);
-      }
-    }
-    __syncwarp();
   }
+  if (pC >= 0) finish(pC, buf ^ 1, pTotal, resolve_base(status, pC, pTotal), true);
   cand = warp_sum_ull(cand);
   if (lane == 0 && cand) { atomicAdd(&H->cand[LST_T5_], cand); atomicAdd(&H->eval[LST_T5_], cand); }
 }
