@@ -39,6 +39,7 @@ N_STREAMS = int(os.environ.get("LST_BENCH_STREAMS", "4"))   # BASELINE.json conf
 MAP_BYTES = 4 * (69630 + 6121)
 # SPEC operations per candidate (every sqrt and div counted as one)
 FLOPS_PER_CAND = (34, 51, 45, 255)
+HEADER_BYTES = 304   # per-slot counter block that lst_sync_batch reads back (csrc/lst_device.cuh SlotHeader)
 
 
 def algorithmic_bytes(stage: int, n_hits, needed):
@@ -249,15 +250,17 @@ def run_ours(args):
     np_in = [[t.numpy() for t in ev] for ev in h_in]
     np_out = [(a.numpy(), b.numpy()) for a, b in h_out]
 
+    idx_bufs = [[np_out[k][0] for k in range(s * per_stream, (s + 1) * per_stream)] for s in range(N_STREAMS)]
+    val_bufs = [[np_out[k][1] for k in range(s * per_stream, (s + 1) * per_stream)] for s in range(N_STREAMS)]
+
     def step_e2e():
-        for s, st in enumerate(streams):
+        for s, st in enumerate(streams):        # H2D of the pinned hit SoA + a0..a4, all asynchronous
             ctx.load_events(s * per_stream, np_in[s * per_stream:(s + 1) * per_stream], stream=st)
             ctx.run_batch(s * per_stream, per_stream, st)
-        for s, st in enumerate(streams):
-            for k in range(s * per_stream, (s + 1) * per_stream):
-                ctx.sync(k, st)
-                ctx.fetch_hit_indices(k, lst.T5, st, out=np_out[k][0])
-                ctx.fetch_values(k, lst.T5, st, out=np_out[k][1])
+        for s, st in enumerate(streams):        # counters back (one sync per stream), then gathers + D2H enqueued
+            ctx.fetch_batch(s * per_stream, lst.T5, idx_bufs[s], val_bufs[s], stream=st, wait=False)
+        for st in streams:
+            st.synchronize()
 
     e2e_steps = max(3, min(args.steps, 10))
     for _ in range(2):
@@ -273,10 +276,11 @@ def run_ours(args):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         e2e_s = float(t.item())
     h2d = sum(sum(t.numel() * t.element_size() for t in ev) for ev in h_in)
-    d2h = needed[3] * (40 + 20) + N_EVENTS * 128
+    d2h = needed[3] * (40 + 20) + N_EVENTS * HEADER_BYTES
     e2e = {"value": world * N_EVENTS * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
            "d2h_bytes_per_step": int(d2h), "steps": e2e_steps,
-           "how": "lst_load_event(host pinned SoA) + lst_run_batch + lst_sync + lst_fetch_{hit_indices,values}(T5) per event"}
+           "how": "per stream: lst_load_events(16 x pinned host SoA) + lst_run_batch + lst_fetch_batch(T5 hit indices + values "
+                  "to pinned host buffers); every step ends with all results on the host"}
 
     # ---- per-kernel times (CUDA events inside the library, timing mode), one 64-event batch ----
     kernel_ms = per_kernel_times(lst, geom, mmap, d_in, local)

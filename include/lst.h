@@ -122,8 +122,9 @@ typedef struct {
 LST_API int lst_default_config(lst_config* cfg);
 
 /* Hit SoA of one event (BASELINE.json configs[1]: "fp32 SoA (x, y, z, module id, sensor side)").
- * All five arrays are HOST pointers (on_device = 0; pinned memory makes the copy asynchronous)
- * or all five DEVICE pointers (on_device = 1).  They are borrowed until the stream has passed
+ * All five arrays are HOST pointers (on_device = 0) or all five DEVICE pointers (on_device = 1).
+ * Pinned (page-locked) host arrays are read by the binning kernel itself over PCIe, once and
+ * coalesced -- no separate copy is enqueued; pageable host arrays go through cudaMemcpyAsync.  They are borrowed until the stream has passed
  * the work enqueued by lst_load_event.  side: 0 = lower sensor (the anchor), 1 = upper. */
 typedef struct {
   int32_t n;
@@ -212,6 +213,12 @@ LST_API int lst_run_stage(lst_ctx* ctx, int first_slot, int n_slots, int stage, 
  * LST_OK, LST_ERR_OVERFLOW, LST_ERR_ARG (bad hits were dropped), LST_ERR_CUDA. */
 LST_API int lst_sync(lst_ctx* ctx, int slot, void* cuda_stream);
 
+/* lst_sync for slots first_slot .. first_slot+n_slots-1 that were enqueued on `cuda_stream`: ONE
+ * strided device-to-host copy of their counters and ONE stream synchronisation.  Returns LST_OK, or
+ * LST_ERR_OVERFLOW if any slot overflowed, else LST_ERR_ARG if any slot dropped bad hits (per-slot
+ * detail: lst_get_stats). */
+LST_API int lst_sync_batch(lst_ctx* ctx, int first_slot, int n_slots, void* cuda_stream);
+
 /* Valid after a successful lst_sync of the slot; LST_ERR_STATE otherwise. */
 LST_API int lst_get_mds(lst_ctx* ctx, int slot, lst_md_view* out);
 LST_API int lst_get_segments(lst_ctx* ctx, int slot, lst_seg_view* out);
@@ -228,6 +235,21 @@ LST_API int lst_fetch_hit_indices(lst_ctx* ctx, int slot, int kind, int32_t* out
 /* Float payload of class `kind` to HOST memory: MD [n][4] sinA, dphi, dphichange, r_anchor;
  * LS [n][4] sinS, z0, dphi, dphichange; T3 [n][2] kappa, chi2rz; T5 [n][5] as lst_t5_view.f. */
 LST_API int lst_fetch_values(lst_ctx* ctx, int slot, int kind, float* out, int64_t cap_objects, void* cuda_stream);
+
+/* Result download for a batch of slots in one call (the end-to-end path of a multi-event
+ * pipeline): synchronises the slots if they are not yet (lst_sync_batch), then
+ * for slot first_slot + b gathers the hit-index tuples of class `kind` on the device and enqueues
+ * their copy to the HOST buffer idx_out[b] ([n][2|4|6|10] int32) and the copy of the float payload
+ * (layout as lst_fetch_values) to val_out[b].  idx_out / val_out may be NULL, and so may single
+ * entries (nothing is copied for them).  cap_objects[b] = rows available in slot b's buffers;
+ * counts[b] (may be NULL) receives the object count.  One gather launch per table for the whole
+ * batch, then one cudaMemcpyAsync per buffer (pinned buffers make them asynchronous).  wait != 0:
+ * returns after the copies have completed; wait == 0: the work is only enqueued and the buffers are
+ * complete once `cuda_stream` has been synchronised by the caller.  Errors: LST_ERR_STATE (a slot not run), LST_ERR_OVERFLOW,
+ * LST_ERR_ARG (a buffer too small: nothing is copied), LST_ERR_CUDA. */
+LST_API int lst_fetch_batch(lst_ctx* ctx, int first_slot, int n_slots, int kind, int32_t* const* idx_out,
+                            float* const* val_out, const int64_t* cap_objects, int32_t* counts, int wait,
+                            void* cuda_stream);
 
 /* Bytes of the arena (all slots) and of one slot. */
 LST_API int lst_arena_bytes(lst_ctx* ctx, int64_t* total, int64_t* per_slot);

@@ -15,6 +15,7 @@
 #include <cstdlib>
 #include <cmath>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -51,6 +52,11 @@ struct lst_ctx {
   size_t arena_bytes = 0;
   std::vector<SlotHost> slots;
   SlotHeader* pinned = nullptr;
+  // Stage-in kernels (k_bin_count reading pinned host memory) of different streams are chained in enqueue
+  // order, as a copy engine would serve copies: each gets the whole PCIe link and the next stream's stage-in
+  // overlaps this stream's compute, instead of all of them sharing the link and finishing together.
+  cudaEvent_t stage_ev = nullptr;
+  std::mutex stage_mu;
   std::atomic<long long> launches{0};
   std::atomic<int> last_cuda{0};
 };
@@ -80,12 +86,11 @@ Layout make_layout(const lst_config& cfg, int n_modules) {
   auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
   L.hdr = take(sizeof(SlotHeader));
   L.bin_start = take(sizeof(int) * (size_t)(L.n_bins + 1));
-  L.bin_cursor = take(sizeof(int) * (size_t)L.n_bins);
   for (int k = 0; k < 4; ++k) L.lb[k] = take(8 * (size_t)(L.n_chunk[k] + 1));
   L.reset_bytes = off - L.hdr;
   const size_t nh = (size_t)cfg.cap_hits, nm = (size_t)cfg.cap_md, ns = (size_t)cfg.cap_seg, n3 = (size_t)cfg.cap_t3, n5 = (size_t)cfg.cap_t5;
   L.in_x = take(4 * nh); L.in_y = take(4 * nh); L.in_z = take(4 * nh); L.in_module = take(4 * nh); L.in_side = take(nh);
-  L.tmp_ki = take(8 * nh); L.tmp_bin = take(4 * nh);
+  L.tmp_kr = take(8 * nh); L.tmp_ki = take(8 * nh); L.tmp_bin = take(4 * nh);
   L.hit4 = take(16 * nh); L.hit_key = take(4 * nh); L.hit_orig = take(4 * nh); L.hit_module = take(4 * nh);
   L.md_start = take(4 * (size_t)(n_modules + 1)); L.mod_info = take(16 * (size_t)n_modules);
   L.md_anchor = take(16 * nm); L.md_aux = take(8 * nm); L.md_key = take(4 * nm); L.md_hits = take(8 * nm);
@@ -96,13 +101,29 @@ Layout make_layout(const lst_config& cfg, int n_modules) {
   L.t3_pack = take(16 * n3); L.t3_seg = take(8 * n3); L.t3_chi2 = take(4 * n3);
   L.t5_start = take(4 * (n3 + 1));
   L.t5_md = take(20 * n5); L.t5_t3 = take(8 * n5); L.t5_f = take(20 * n5);
-  size_t scr = 8 * nm;
+  size_t scr = 16 * nm;   // one gathered table at a time: hit-index tuples (8 / 16 / 24 / 40 B) or packed values (16 / 16 / 8 / 20 B)
   if (16 * ns > scr) scr = 16 * ns;
   if (24 * n3 > scr) scr = 24 * n3;
   if (40 * n5 > scr) scr = 40 * n5;
   L.scratch = take(scr);
   L.slot_bytes = align_up(off, 4096);
   return L;
+}
+
+// Device-visible alias of a pinned (page-locked, mapped) host pointer, or nullptr for pageable memory.
+const void* mapped_alias(const void* p) {
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+  return a.type == cudaMemoryTypeHost ? a.devicePointer : nullptr;
+}
+// True (and the pointers replaced by their device-visible aliases) if all five arrays are pinned host memory.
+bool mapped_host(HitInput& in) {
+  const void* p[5] = {mapped_alias(in.x), mapped_alias(in.y), mapped_alias(in.z), mapped_alias(in.module), mapped_alias(in.side)};
+  for (const void* q : p)
+    if (!q) return false;
+  in.x = static_cast<const float*>(p[0]); in.y = static_cast<const float*>(p[1]); in.z = static_cast<const float*>(p[2]);
+  in.module = static_cast<const int*>(p[3]); in.side = static_cast<const unsigned char*>(p[4]);
+  return true;
 }
 
 bool valid_slot(const lst_ctx* c, int slot) { return c && slot >= 0 && slot < (int)c->slots.size(); }
@@ -229,6 +250,7 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
   if ((e = cudaMemset(c->arena, 0, c->arena_bytes)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   if ((e = cudaMallocHost(&c->pinned, sizeof(SlotHeader) * (size_t)cfg.n_slots)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   std::memset(c->pinned, 0, sizeof(SlotHeader) * (size_t)cfg.n_slots);
+  if ((e = cudaEventCreateWithFlags(&c->stage_ev, cudaEventDisableTiming)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   c->slots.resize(cfg.n_slots);
   for (int s = 0; s < cfg.n_slots; ++s) {
     c->slots[s].hdr = c->pinned + s;
@@ -257,6 +279,7 @@ int lst_destroy(lst_ctx* c) {
   for (auto& s : c->slots)
     for (auto& ev : s.ev)
       if (ev) cudaEventDestroy(ev);
+  if (c->stage_ev) cudaEventDestroy(c->stage_ev);
   if (c->pinned) cudaFreeHost(c->pinned);
   if (c->arena) cudaFree(c->arena);
   if (c->d_map_dphi) cudaFree(c->d_map_dphi);
@@ -281,8 +304,9 @@ int lst_load_events(lst_ctx* c, int first, int n_ev, const lst_hits* hits, void*
   const Layout& L = c->P.L;
   for (int b0 = 0; b0 < n_ev; b0 += kMaxBatch) {
     const int nb = n_ev - b0 < kMaxBatch ? n_ev - b0 : kMaxBatch;
-    HitBatch batch;
-    std::memset(&batch, 0, sizeof(batch));
+    HitBatch src, dev;
+    std::memset(&src, 0, sizeof(src));
+    std::memset(&dev, 0, sizeof(dev));
     for (int b = 0; b < nb; ++b) {
       const int slot = first + b0 + b;
       const lst_hits* h = hits + b0 + b;
@@ -292,26 +316,40 @@ int lst_load_events(lst_ctx* c, int first, int n_ev, const lst_hits* hits, void*
       sh.ev_bin = false;
       for (bool& f : sh.ev_stage) f = false;
       char* base = c->arena + (size_t)slot * c->P.slot_stride;
-      HitInput in{h->x, h->y, h->z, h->module, h->side, h->n};
-      if (!h->on_device && h->n > 0) {
+      HitInput in{h->x, h->y, h->z, h->module, h->side, h->n, 0};
+      HitInput staged{reinterpret_cast<const float*>(base + L.in_x), reinterpret_cast<const float*>(base + L.in_y),
+                      reinterpret_cast<const float*>(base + L.in_z), reinterpret_cast<const int*>(base + L.in_module),
+                      reinterpret_cast<const unsigned char*>(base + L.in_side), h->n, 0};
+      if (h->on_device || h->n == 0) {
+        src.ev[b] = dev.ev[b] = in;
+      } else if (mapped_host(in)) {
+        // pinned host arrays: k_bin_count reads them over PCIe (one coalesced pass) and fills the staging area
+        in.stage = 1;
+        src.ev[b] = in;
+        dev.ev[b] = staged;
+      } else {
+        // pageable host arrays: the driver stages the copies
         const size_t n = (size_t)h->n;
         LST_CUDA(c, cudaMemcpyAsync(base + L.in_x, h->x, 4 * n, cudaMemcpyHostToDevice, s));
         LST_CUDA(c, cudaMemcpyAsync(base + L.in_y, h->y, 4 * n, cudaMemcpyHostToDevice, s));
         LST_CUDA(c, cudaMemcpyAsync(base + L.in_z, h->z, 4 * n, cudaMemcpyHostToDevice, s));
         LST_CUDA(c, cudaMemcpyAsync(base + L.in_module, h->module, 4 * n, cudaMemcpyHostToDevice, s));
         LST_CUDA(c, cudaMemcpyAsync(base + L.in_side, h->side, n, cudaMemcpyHostToDevice, s));
-        in.x = reinterpret_cast<const float*>(base + L.in_x);
-        in.y = reinterpret_cast<const float*>(base + L.in_y);
-        in.z = reinterpret_cast<const float*>(base + L.in_z);
-        in.module = reinterpret_cast<const int*>(base + L.in_module);
-        in.side = reinterpret_cast<const unsigned char*>(base + L.in_side);
+        src.ev[b] = dev.ev[b] = staged;
       }
-      batch.ev[b] = in;
     }
     SlotHost& sh0 = c->slots[first + b0];
     Params P = c->P;
     P.first_slot = first + b0;
-    c->launches += launch_bin(P, batch, nb, s, c->cfg.timing ? sh0.ev : nullptr);
+    bool staged = false;
+    for (int b = 0; b < nb; ++b) staged = staged || src.ev[b].stage;
+    if (staged) {
+      std::lock_guard<std::mutex> lock(c->stage_mu);
+      LST_CUDA(c, cudaStreamWaitEvent(s, c->stage_ev, 0));   // a never-recorded event does not block
+      c->launches += launch_bin(P, src, dev, nb, s, c->cfg.timing ? sh0.ev : nullptr, c->stage_ev);
+    } else {
+      c->launches += launch_bin(P, src, dev, nb, s, c->cfg.timing ? sh0.ev : nullptr, nullptr);
+    }
     LST_CUDA(c, cudaGetLastError());
     sh0.ev_bin = c->cfg.timing != 0;
     for (int b = 0; b < nb; ++b) c->slots[first + b0 + b].loaded = true;
@@ -449,6 +487,86 @@ int lst_get_stats(lst_ctx* c, int slot, lst_stats* o) {
 }
 
 static const int kHitsPerObject[4] = {2, 4, 6, 10};
+static const int kValuesPerObject[4] = {4, 4, 2, 5};
+
+int lst_sync_batch(lst_ctx* c, int first, int n, void* stream) {
+  if (!c || n < 1 || !valid_slot(c, first) || !valid_slot(c, first + n - 1)) return LST_ERR_ARG;
+  for (int s = first; s < first + n; ++s)
+    if (!c->slots[s].loaded) return LST_ERR_STATE;
+  cudaStream_t st = (cudaStream_t)stream;
+  LST_CUDA(c, cudaSetDevice(c->device));
+  // the n headers in ONE strided copy: they sit slot_stride apart on the device, contiguous in the pinned mirror
+  LST_CUDA(c, cudaMemcpy2DAsync(c->pinned + first, sizeof(SlotHeader), c->arena + (size_t)first * c->P.slot_stride + c->P.L.hdr,
+                                c->P.slot_stride, sizeof(SlotHeader), (size_t)n, cudaMemcpyDeviceToHost, st));
+  LST_CUDA(c, cudaStreamSynchronize(st));
+  int status = LST_OK;
+  for (int s = first; s < first + n; ++s) {
+    SlotHost& sh = c->slots[s];
+    sh.synced = true;
+    if (status == LST_OK && sh.hdr->overflow) status = LST_ERR_OVERFLOW;
+  }
+  if (status == LST_OK)
+    for (int s = first; s < first + n; ++s)
+      if (c->slots[s].hdr->bad_hits) { status = LST_ERR_ARG; break; }
+  return status;
+}
+
+int lst_fetch_batch(lst_ctx* c, int first, int n, int kind, int32_t* const* idx_out, float* const* val_out,
+                    const int64_t* cap_objects, int32_t* counts, int wait, void* stream) {
+  if (!c || n < 1 || !valid_slot(c, first) || !valid_slot(c, first + n - 1) || kind < LST_MD || kind > LST_T5 || !cap_objects)
+    return LST_ERR_ARG;
+  for (int s = first; s < first + n; ++s)
+    if (!c->slots[s].loaded || !c->slots[s].ran) return LST_ERR_STATE;
+  bool all_synced = true;
+  for (int s = first; s < first + n; ++s) all_synced = all_synced && c->slots[s].synced;
+  if (!all_synced) {
+    const int r = lst_sync_batch(c, first, n, stream);
+    if (r == LST_ERR_CUDA || r == LST_ERR_STATE) return r;
+  }
+  int n_max = 0;
+  for (int b = 0; b < n; ++b) {
+    const SlotHeader* h = c->slots[first + b].hdr;
+    if (h->overflow) return LST_ERR_OVERFLOW;
+    const int nk = h->n[kind];
+    if (counts) counts[b] = nk;
+    if (nk > cap_objects[b] && ((idx_out && idx_out[b]) || (val_out && val_out[b]))) return LST_ERR_ARG;
+    n_max = nk > n_max ? nk : n_max;
+  }
+  cudaStream_t st = (cudaStream_t)stream;
+  LST_CUDA(c, cudaSetDevice(c->device));
+  const Layout& L = c->P.L;
+  Params P = c->P;
+  P.first_slot = first;
+  // Copies go through the copy engine (they overlap the stage kernels of the other streams without taking
+  // SM slots).  The slot's scratch area holds one gathered table at a time: stream order keeps the second
+  // gather behind the first copy.
+  if (idx_out && n_max > 0) {
+    c->launches += launch_gather_hits(P, kind, n_max, n, st);
+    LST_CUDA(c, cudaGetLastError());
+    for (int b = 0; b < n; ++b) {
+      const int nk = c->slots[first + b].hdr->n[kind];
+      if (!idx_out[b] || nk == 0) continue;
+      const char* base = c->arena + (size_t)(first + b) * c->P.slot_stride;
+      LST_CUDA(c, cudaMemcpyAsync(idx_out[b], base + L.scratch, sizeof(int32_t) * (size_t)nk * kHitsPerObject[kind], cudaMemcpyDeviceToHost, st));
+    }
+  }
+  if (val_out && n_max > 0) {
+    const bool packed = kind == LST_MD || kind == LST_T3;
+    if (packed) {
+      c->launches += launch_pack_values(P, kind, n_max, n, st);
+      LST_CUDA(c, cudaGetLastError());
+    }
+    const size_t src_off = packed ? L.scratch : (kind == LST_SEG ? L.seg_f : L.t5_f);
+    for (int b = 0; b < n; ++b) {
+      const int nk = c->slots[first + b].hdr->n[kind];
+      if (!val_out[b] || nk == 0) continue;
+      const char* base = c->arena + (size_t)(first + b) * c->P.slot_stride;
+      LST_CUDA(c, cudaMemcpyAsync(val_out[b], base + src_off, sizeof(float) * (size_t)nk * kValuesPerObject[kind], cudaMemcpyDeviceToHost, st));
+    }
+  }
+  if (wait) LST_CUDA(c, cudaStreamSynchronize(st));
+  return LST_OK;
+}
 
 int lst_fetch_hit_indices(lst_ctx* c, int slot, int kind, int32_t* out, int64_t cap, void* stream) {
   if (kind < LST_MD || kind > LST_T5) return LST_ERR_ARG;
@@ -457,16 +575,9 @@ int lst_fetch_hit_indices(lst_ctx* c, int slot, int kind, int32_t* out, int64_t 
   const int n = c->slots[slot].hdr->n[kind];
   if (n == 0) return LST_OK;
   if (!out || cap < n) return LST_ERR_ARG;
-  cudaStream_t s = (cudaStream_t)stream;
-  LST_CUDA(c, cudaSetDevice(c->device));
-  Params P = c->P;
-  P.first_slot = slot;
-  c->launches += launch_gather_hits(P, kind, n, s);
-  LST_CUDA(c, cudaGetLastError());
-  const char* b = c->arena + (size_t)slot * c->P.slot_stride;
-  LST_CUDA(c, cudaMemcpyAsync(out, b + P.L.scratch, sizeof(int32_t) * (size_t)n * kHitsPerObject[kind], cudaMemcpyDeviceToHost, s));
-  LST_CUDA(c, cudaStreamSynchronize(s));
-  return LST_OK;
+  int32_t* outs[1] = {out};
+  const int64_t caps[1] = {cap};
+  return lst_fetch_batch(c, slot, 1, kind, outs, nullptr, caps, nullptr, 1, stream);
 }
 
 int lst_fetch_values(lst_ctx* c, int slot, int kind, float* out, int64_t cap, void* stream) {
@@ -476,28 +587,9 @@ int lst_fetch_values(lst_ctx* c, int slot, int kind, float* out, int64_t cap, vo
   const int n = c->slots[slot].hdr->n[kind];
   if (n == 0) return LST_OK;
   if (!out || cap < n) return LST_ERR_ARG;
-  cudaStream_t s = (cudaStream_t)stream;
-  LST_CUDA(c, cudaSetDevice(c->device));
-  Params P = c->P;
-  P.first_slot = slot;
-  const char* b = c->arena + (size_t)slot * c->P.slot_stride;
-  const char* src;
-  size_t width;
-  if (kind == LST_MD || kind == LST_T3) {
-    c->launches += launch_pack_values(P, kind, n, s);
-    LST_CUDA(c, cudaGetLastError());
-    src = b + P.L.scratch;
-    width = kind == LST_MD ? 4 : 2;
-  } else if (kind == LST_SEG) {
-    src = b + P.L.seg_f;
-    width = 4;
-  } else {
-    src = b + P.L.t5_f;
-    width = 5;
-  }
-  LST_CUDA(c, cudaMemcpyAsync(out, src, sizeof(float) * (size_t)n * width, cudaMemcpyDeviceToHost, s));
-  LST_CUDA(c, cudaStreamSynchronize(s));
-  return LST_OK;
+  float* outs[1] = {out};
+  const int64_t caps[1] = {cap};
+  return lst_fetch_batch(c, slot, 1, kind, nullptr, outs, caps, nullptr, 1, stream);
 }
 
 int lst_arena_bytes(lst_ctx* c, int64_t* total, int64_t* per_slot) {

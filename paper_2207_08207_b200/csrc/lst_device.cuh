@@ -69,10 +69,10 @@ struct Layout {
   int cap_hits, cap_md, cap_seg, cap_t3, cap_t5;
   int n_chunk[4];                 // ceil(cap of the OWNER class / kChunk): hits, MD, LS, T3
   // byte offsets from the slot base (all multiples of 256)
-  size_t hdr, bin_start, bin_cursor, lb[4];   // contiguous: zeroed by k_reset at lst_load_event
+  size_t hdr, bin_start, lb[4];               // contiguous: zeroed by k_reset at lst_load_event
   size_t reset_bytes;                         // bytes to zero at lst_load_event, from hdr
   size_t in_x, in_y, in_z, in_module, in_side;// staging of host input
-  size_t tmp_ki, tmp_bin, hit4, hit_key, hit_orig, hit_module;
+  size_t tmp_kr, tmp_ki, tmp_bin, hit4, hit_key, hit_orig, hit_module;
   size_t md_start, mod_info, md_anchor, md_aux, md_key, md_hits, md_out, md_module;
   size_t seg_start, seg_md, seg_f;
   size_t t3_start, t3_pack, t3_seg, t3_chi2;
@@ -105,8 +105,8 @@ struct Slot {
   __device__ __forceinline__ T* at(size_t off) const { return reinterpret_cast<T*>(b + off); }
   __device__ __forceinline__ SlotHeader* hdr() const { return at<SlotHeader>(L.hdr); }
   __device__ __forceinline__ unsigned* bin_start() const { return at<unsigned>(L.bin_start); }
-  __device__ __forceinline__ unsigned* bin_cursor() const { return at<unsigned>(L.bin_cursor); }
   __device__ __forceinline__ unsigned long long* lb(int kind) const { return at<unsigned long long>(L.lb[kind]); }
+  __device__ __forceinline__ int2* tmp_kr() const { return at<int2>(L.tmp_kr); }
   __device__ __forceinline__ int2* tmp_ki() const { return at<int2>(L.tmp_ki); }
   __device__ __forceinline__ int* tmp_bin() const { return at<int>(L.tmp_bin); }
   __device__ __forceinline__ float4* hit4() const { return at<float4>(L.hit4); }
@@ -143,6 +143,7 @@ struct HitInput {
   const int* module;
   const unsigned char* side;
   int n;
+  int stage;   // != 0: the arrays are mapped (pinned) host memory; k_bin_count copies them into the slot's staging area
 };
 // Inputs of a batch of events: slot first_slot + b reads ev[b].
 struct HitBatch {
@@ -151,9 +152,13 @@ struct HitBatch {
 
 // Host-callable launchers (lst_kernels.cu). Each returns the number of kernels it launched.
 // `ev` (optional, timing mode): ev[0] is recorded before the first kernel, ev[k + 1] after kernel k.
-int launch_bin(const Params& P, const HitBatch& in, int n_batch, cudaStream_t s, cudaEvent_t* ev);   // 4 kernels
+// `src`: the arrays k_bin_count reads (device, or mapped host memory with stage = 1); `dev`: the device-resident arrays
+// the later kernels read (the same, or the slot's staging area).
+// `staged_in` (optional) is recorded right after k_bin_count when it read host memory.
+int launch_bin(const Params& P, const HitBatch& src, const HitBatch& dev, int n_batch, cudaStream_t s, cudaEvent_t* ev,
+               cudaEvent_t staged_in);   // 4 kernels
 int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEvent_t* ev);          // 1 kernel
-int launch_gather_hits(const Params& P, int kind, int n, cudaStream_t s);
-int launch_pack_values(const Params& P, int kind, int n, cudaStream_t s);
+int launch_gather_hits(const Params& P, int kind, int n_max, int n_batch, cudaStream_t s);   // slots first_slot .. + n_batch - 1
+int launch_pack_values(const Params& P, int kind, int n_max, int n_batch, cudaStream_t s);
 
 }  // namespace lst

@@ -203,7 +203,7 @@ __device__ __forceinline__ float r_max_of(const SlotHeader* h, int side, int lay
 // a0: load + bin by (side, module) + order by azimuth + derive r
 // blockIdx.y = event of the batch; its input arrays come from the pointer table `B`.
 // ------------------------------------------------------------------------------------------
-// Recycles the slot: zeroes header, bin counters, bin cursors and the look-back status words.
+// Recycles the slot: zeroes header, bin counters and the look-back status words.
 __global__ void __launch_bounds__(256) k_reset(const __grid_constant__ Params P) {
   Slot S(P, blockIdx.y);
   int4* p = S.at<int4>(P.L.hdr);
@@ -211,17 +211,37 @@ __global__ void __launch_bounds__(256) k_reset(const __grid_constant__ Params P)
   for (size_t i = (size_t)blockIdx.x * 256 + threadIdx.x; i < n; i += (size_t)gridDim.x * 256) p[i] = make_int4(0, 0, 0, 0);
 }
 
+// One pass over the caller's arrays: histogram by (side, module); the value the atomic returns is
+// the hit's arrival rank in its bin, kept with its azimuth key so that the scatter needs no second
+// atomic.  If the arrays are mapped host memory (in.stage) this pass IS the host-to-device copy:
+// every array is read once over PCIe, coalesced, and written to the slot's staging area, which is
+// what the later kernels read.  The event's last block turns the counts into bin offsets.
 __global__ void __launch_bounds__(256) k_bin_count(const __grid_constant__ Params P, const __grid_constant__ HitBatch B) {
   Slot S(P, blockIdx.y);
   const HitInput& in = B.ev[blockIdx.y];
   unsigned* cnt = S.bin_start();
+  int2* kr = S.tmp_kr();
   const int nmod = P.L.n_modules;
+  float* sx = S.at<float>(P.L.in_x);
+  float* sy = S.at<float>(P.L.in_y);
+  float* sz = S.at<float>(P.L.in_z);
+  int* sm = S.at<int>(P.L.in_module);
+  unsigned char* ss = S.at<unsigned char>(P.L.in_side);
   int bad = 0;
   for (int h = blockIdx.x * blockDim.x + threadIdx.x; h < in.n; h += gridDim.x * blockDim.x) {
     const int m = in.module[h];
     const unsigned sd = in.side[h];
+    const float x = in.x[h], y = in.y[h];
+    if (in.stage) {
+      sx[h] = x; sy[h] = y; sz[h] = in.z[h]; sm[h] = m; ss[h] = (unsigned char)sd;
+    }
     if (m < 0 || m >= nmod || sd > 1u) { ++bad; continue; }
-    atomicAdd(cnt + ((int)sd * nmod + m), 1u);
+    const float2 cs = P.mod_cs[m];
+    // azimuth relative to the module normal; non-finite hits (they can never pass a cut) go last
+    float k = atan2f(cs.x * y - cs.y * x, cs.x * x + cs.y * y);
+    if (!(fabsf(k) <= 4.0f)) k = 3.0e38f;
+    const unsigned rank = atomicAdd(cnt + ((int)sd * nmod + m), 1u);
+    kr[h] = make_int2(__float_as_int(k), (int)rank);
   }
   if (bad) atomicAdd(&S.hdr()->bad_hits, bad);
   // the last block of the event turns the counts into bin offsets
@@ -242,11 +262,12 @@ __global__ void __launch_bounds__(256) k_bin_count(const __grid_constant__ Param
   }
 }
 
+// (key, original index) of every hit to bin offset + arrival rank.  `B` holds device-resident arrays.
 __global__ void __launch_bounds__(256) k_bin_scatter(const __grid_constant__ Params P, const __grid_constant__ HitBatch B) {
   Slot S(P, blockIdx.y);
   const HitInput& in = B.ev[blockIdx.y];
   const unsigned* start = S.bin_start();
-  unsigned* cur = S.bin_cursor();
+  const int2* kr = S.tmp_kr();
   int2* tki = S.tmp_ki();
   int* tbin = S.tmp_bin();
   const int nmod = P.L.n_modules;
@@ -255,13 +276,9 @@ __global__ void __launch_bounds__(256) k_bin_scatter(const __grid_constant__ Par
     const unsigned sd = in.side[h];
     if (m < 0 || m >= nmod || sd > 1u) continue;
     const int b = (int)sd * nmod + m;
-    const float x = in.x[h], y = in.y[h];
-    const float2 cs = P.mod_cs[m];
-    // azimuth relative to the module normal; non-finite hits (they can never pass a cut) go last
-    float k = atan2f(cs.x * y - cs.y * x, cs.x * x + cs.y * y);
-    if (!(fabsf(k) <= 4.0f)) k = 3.0e38f;
-    const unsigned pos = start[b] + atomicAdd(cur + b, 1u);
-    tki[pos] = make_int2(__float_as_int(k), h);
+    const int2 v = kr[h];
+    const unsigned pos = start[b] + (unsigned)v.y;
+    tki[pos] = make_int2(v.x, h);
     tbin[pos] = b;
   }
 }
@@ -306,10 +323,19 @@ __global__ void __launch_bounds__(256) k_bin_order(const __grid_constant__ Param
       if (rank == 0) info[4 * m + 2] = me.x;
       if (rank == e - s - 1) info[4 * m + 3] = me.x;
     }
-    if (r < 3.0e38f) {
-      const int layer = P.mod_layer[m];
-      atomicMax(&s_rng[side * 6 + layer], 0x7f800000 - __float_as_int(r));
-      atomicMax(&s_rng[12 + side * 6 + layer], __float_as_int(r));
+    // range of r per (side, layer): neighbouring threads sit in the same or the next bin, so a warp
+    // holds one or two (side, layer) groups -- one shared-memory atomic pair per group, not per hit
+    const bool fin = r < 3.0e38f;
+    const unsigned act = __ballot_sync(__activemask(), fin);
+    if (fin) {
+      const int slot = side * 6 + P.mod_layer[m];
+      const unsigned grp = __match_any_sync(act, slot);
+      const int rmax = __reduce_max_sync(grp, __float_as_int(r));
+      const int rinv = __reduce_max_sync(grp, 0x7f800000 - __float_as_int(r));
+      if ((int)lane_id() == __ffs(grp) - 1) {
+        atomicMax(&s_rng[slot], rinv);
+        atomicMax(&s_rng[12 + slot], rmax);
+      }
     }
   }
   if (p < nmod && start[p + 1] == start[p]) {  // no lower hits: an empty key range
@@ -1114,40 +1140,45 @@ __global__ void __launch_bounds__(kWarps * 32) k_t5(const __grid_constant__ Para
 // ------------------------------------------------------------------------------------------
 // output helpers: original-hit-index tuples and float payloads, one thread per object
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_gather_hits(const __grid_constant__ Params P, int kind, int n) {
-  Slot S(P, 0);
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
+// blockIdx.y = slot of the batch; the object count comes from the slot header (clamped to capacity).
+// Destination: the slot's scratch area (lst_fetch_batch copies it to the host from there).
+__global__ void __launch_bounds__(256) k_gather_hits(const __grid_constant__ Params P, int kind) {
+  Slot S(P, blockIdx.y);
+  const int w = kind == LST_MD_ ? 1 : kind == LST_SEG_ ? 2 : kind == LST_T3_ ? 3 : 5;   // MDs per object
+  const size_t m = (size_t)S.hdr()->n[kind] * w;
   const int2* mh = S.md_hits();
   int2* out = reinterpret_cast<int2*>(S.scratch());
-  if (kind == LST_MD_) {
-    out[i] = mh[i];
-  } else if (kind == LST_SEG_) {
-    const int2 s = S.seg_md()[i];
-    out[2 * (size_t)i] = mh[s.x];
-    out[2 * (size_t)i + 1] = mh[s.y];
-  } else if (kind == LST_T3_) {
-    const int4 t = S.t3_pack()[i];
-    out[3 * (size_t)i] = mh[t.x];
-    out[3 * (size_t)i + 1] = mh[t.y];
-    out[3 * (size_t)i + 2] = mh[t.z];
-  } else {
-    const int* md = S.t5_md() + 5 * (size_t)i;
-#pragma unroll
-    for (int k = 0; k < 5; ++k) out[5 * (size_t)i + k] = mh[md[k]];
+  // one thread per (object, MD): a warp writes 256 contiguous bytes whatever the class
+  for (size_t j = (size_t)blockIdx.x * blockDim.x + threadIdx.x; j < m; j += (size_t)gridDim.x * blockDim.x) {
+    int md;
+    if (kind == LST_MD_) {
+      md = (int)j;
+    } else if (kind == LST_SEG_) {
+      md = reinterpret_cast<const int*>(S.seg_md())[j];
+    } else if (kind == LST_T3_) {
+      const size_t i = j / 3;
+      md = reinterpret_cast<const int*>(S.t3_pack())[4 * i + (j - 3 * i)];
+    } else {
+      md = S.t5_md()[j];
+    }
+    out[j] = mh[md];
   }
 }
 
-__global__ void __launch_bounds__(256) k_pack_values(const __grid_constant__ Params P, int kind, int n) {
-  Slot S(P, 0);
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
+// Float payload of the classes whose fields are spread over several arrays (MD, T3), in the layout of
+// lst_fetch_values, to the slot's scratch area.  (LS and T5 payloads are stored in that layout already.)
+__global__ void __launch_bounds__(256) k_pack_values(const __grid_constant__ Params P, int kind) {
+  Slot S(P, blockIdx.y);
+  const int n = S.hdr()->n[kind];
   float* out = reinterpret_cast<float*>(S.scratch());
   if (kind == LST_MD_) {
-    const float2 o = S.md_out()[i];
-    reinterpret_cast<float4*>(out)[i] = make_float4(S.md_aux()[i].y, o.x, o.y, S.md_anchor()[i].w);
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+      const float2 o = S.md_out()[i];
+      reinterpret_cast<float4*>(out)[i] = make_float4(S.md_aux()[i].y, o.x, o.y, S.md_anchor()[i].w);
+    }
   } else if (kind == LST_T3_) {
-    reinterpret_cast<float2*>(out)[i] = make_float2(__int_as_float(S.t3_pack()[i].w), S.t3_chi2()[i]);
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
+      reinterpret_cast<float2*>(out)[i] = make_float2(__int_as_float(S.t3_pack()[i].w), S.t3_chi2()[i]);
   }
 }
 
@@ -1162,19 +1193,26 @@ static int blocks_per_event(int wanted, int n_batch, int resident_per_sm) {
   return max(1, min(wanted, per_event));
 }
 
-int launch_bin(const Params& P, const HitBatch& in, int n_batch, cudaStream_t s, cudaEvent_t* ev) {
+int launch_bin(const Params& P, const HitBatch& src, const HitBatch& dev, int n_batch, cudaStream_t s, cudaEvent_t* ev,
+               cudaEvent_t staged_in) {
   int n_max = 0;
-  for (int b = 0; b < n_batch; ++b) n_max = max(n_max, in.ev[b].n);
+  for (int b = 0; b < n_batch; ++b) n_max = max(n_max, src.ev[b].n);
   const unsigned nb = (unsigned)n_batch;
   const dim3 g(blocks_per_event((n_max + 255) / 256, n_batch, 8), nb);
   LST_EV(0);
   k_reset<<<dim3(blocks_per_event((int)(P.L.reset_bytes / 16 + 255) / 256, n_batch, 8), nb), 256, 0, s>>>(P);
   LST_EV(1);
-  k_bin_count<<<g, 256, 0, s>>>(P, in);   // + scan of the bin counts by the event's last block
+  // Reading mapped host memory the kernel is PCIe bound (~75 KB in flight cover latency x bandwidth): a
+  // small grid leaves the SMs to the other streams' stage kernels.
+  bool staged = false;
+  for (int b = 0; b < n_batch; ++b) staged = staged || src.ev[b].stage;
+  const dim3 gc(staged ? min((int)g.x, 8) : g.x, nb);
+  k_bin_count<<<gc, 256, 0, s>>>(P, src);   // (+ stage-in) + scan of the bin counts by the event's last block
+  if (staged && staged_in) cudaEventRecord(staged_in, s);
   LST_EV(2);
-  k_bin_scatter<<<g, 256, 0, s>>>(P, in);
+  k_bin_scatter<<<g, 256, 0, s>>>(P, dev);
   LST_EV(3);
-  k_bin_order<<<dim3((max(n_max, P.L.n_modules) + 255) / 256, nb), 256, 0, s>>>(P, in);
+  k_bin_order<<<dim3((max(n_max, P.L.n_modules) + 255) / 256, nb), 256, 0, s>>>(P, dev);
   LST_EV(4);
   return 4;
 }
@@ -1202,15 +1240,16 @@ int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEv
   return 1;
 }
 
-int launch_gather_hits(const Params& P, int kind, int n, cudaStream_t s) {
-  if (n <= 0) return 0;
-  k_gather_hits<<<(n + 255) / 256, 256, 0, s>>>(P, kind, n);
+int launch_gather_hits(const Params& P, int kind, int n_max, int n_batch, cudaStream_t s) {
+  if (n_max <= 0 || n_batch <= 0) return 0;
+  const int w = kind == LST_MD_ ? 1 : kind == LST_SEG_ ? 2 : kind == LST_T3_ ? 3 : 5;
+  k_gather_hits<<<dim3(min(256, (n_max * w + 255) / 256), (unsigned)n_batch), 256, 0, s>>>(P, kind);
   return 1;
 }
 
-int launch_pack_values(const Params& P, int kind, int n, cudaStream_t s) {
-  if (n <= 0 || (kind != LST_MD_ && kind != LST_T3_)) return 0;
-  k_pack_values<<<(n + 255) / 256, 256, 0, s>>>(P, kind, n);
+int launch_pack_values(const Params& P, int kind, int n_max, int n_batch, cudaStream_t s) {
+  if (n_max <= 0 || n_batch <= 0 || (kind != LST_MD_ && kind != LST_T3_)) return 0;
+  k_pack_values<<<dim3(min(256, (n_max + 255) / 256), (unsigned)n_batch), 256, 0, s>>>(P, kind);
   return 1;
 }
 

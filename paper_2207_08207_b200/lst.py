@@ -106,6 +106,9 @@ SYMBOLS = {
     "lst_run_batch": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p]),
     "lst_run_stage": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]),
     "lst_sync": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
+    "lst_sync_batch": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p]),
+    "lst_fetch_batch": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, P(C.c_void_p), P(C.c_void_p), P(C.c_int64),
+                                  P(C.c_int32), C.c_int, C.c_void_p]),
     "lst_get_mds": (C.c_int, [C.c_void_p, C.c_int, P(MdView)]),
     "lst_get_segments": (C.c_int, [C.c_void_p, C.c_int, P(SegView)]),
     "lst_get_triplets": (C.c_int, [C.c_void_p, C.c_int, P(T3View)]),
@@ -270,6 +273,34 @@ class Lst:
         if check:
             self._check(st, "lst_sync")
         return st
+
+    def sync_batch(self, first_slot: int, n_slots: int, stream=None, check: bool = True) -> int:
+        st = self.lib.lst_sync_batch(self.h, first_slot, n_slots, _stream(stream))
+        if check:
+            self._check(st, "lst_sync_batch")
+        return st
+
+    def fetch_batch(self, first_slot: int, kind: int, idx_out=None, val_out=None, stream=None, wait: bool = True):
+        """One call for a batch of slots: idx_out / val_out are sequences of host arrays (numpy or pinned
+        torch tensors; entries may be None), slot first_slot + b writes into entry b.  Returns the object
+        counts.  wait=False only enqueues the copies: synchronise the stream before reading the buffers."""
+        bufs = idx_out if idx_out is not None else val_out
+        n = len(bufs)
+        def table(seq):
+            if seq is None:
+                return None
+            arr = (C.c_void_p * n)()
+            for b, a in enumerate(seq):
+                arr[b] = _ptr(a) or None
+            return arr
+        caps = (C.c_int64 * n)()
+        for b in range(n):
+            rows = [int(seq[b].shape[0]) for seq in (idx_out, val_out) if seq is not None and seq[b] is not None]
+            caps[b] = min(rows) if rows else 0
+        counts = (C.c_int32 * n)()
+        self._check(self.lib.lst_fetch_batch(self.h, first_slot, n, kind, table(idx_out), table(val_out), caps, counts,
+                                             1 if wait else 0, _stream(stream)), "lst_fetch_batch")
+        return [int(v) for v in counts]
 
     # ---- results ----------------------------------------------------------------------------
     def stats(self, slot: int) -> dict:

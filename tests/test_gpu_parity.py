@@ -221,3 +221,41 @@ def test_search_windows_never_change_the_result(lstmod, geom, mmap, o32, run_ora
     _, st = check_event(c, o32, run_oracle, ev, label=how)
     assert st["needed"][3] > 500
     c.close()
+
+
+def test_fetch_batch_equals_per_slot_fetch(ctx, geom):
+    """lst_sync_batch + lst_fetch_batch (one call per batch, asynchronous copies into pinned host
+    buffers) return exactly what the per-slot lst_sync + lst_fetch_* calls return, for every class."""
+    import torch
+    evs = [synth.generate_event(geom, 1, 80 + i, n_particles=300 + 400 * i) for i in range(3)]
+    evs.append(synth.Event(*(np.zeros(0, t) for t in (np.float32, np.float32, np.float32, np.int32, np.uint8, np.int32)), {}))
+    stream = torch.cuda.Stream()
+    # pinned host input: the binning kernel reads it over PCIe itself (no memcpy); slot 6 gets the same event as
+    # slot 3 from pageable memory (cudaMemcpyAsync path) and must produce the same arrays
+    pin = lambda a: torch.from_numpy(a).pin_memory().numpy()
+    ctx.load_events(2, [tuple(pin(a) for a in (e.x, e.y, e.z, e.module, e.side)) for e in evs], stream=stream)
+    ctx.run_batch(2, len(evs), stream)
+    assert ctx.sync_batch(2, len(evs), stream) == 0
+    pageable = parity.run_gpu(ctx, evs[1], slot=6, stream=stream)
+    pinned = parity.gpu_tables(ctx, 3, stream)
+    for kind in range(4):
+        assert np.array_equal(pageable[kind][0], pinned[kind][0]) and np.array_equal(pageable[kind][1], pinned[kind][1], equal_nan=True)
+    for kind in range(4):
+        need = [ctx.stats(2 + b)["needed"][kind] for b in range(len(evs))]
+        idx = [torch.full((n + 3, parity_width(kind)[0]), -7, dtype=torch.int32).pin_memory().numpy() for n in need]
+        val = [torch.full((n + 3, parity_width(kind)[1]), -7.0, dtype=torch.float32).pin_memory().numpy() for n in need]
+        counts = ctx.fetch_batch(2, kind, idx, val, stream=stream, wait=False)
+        stream.synchronize()
+        assert counts == need
+        for b, n in enumerate(need):
+            assert np.array_equal(idx[b][:n], ctx.fetch_hit_indices(2 + b, kind, stream))
+            assert np.array_equal(val[b][:n], ctx.fetch_values(2 + b, kind, stream), equal_nan=True)
+            assert (idx[b][n:] == -7).all() and (val[b][n:] == -7.0).all()      # nothing written past the count
+    # a buffer that is too small is refused before anything is copied
+    small = [np.zeros((1, 10), np.int32) for _ in evs]
+    with pytest.raises(Exception):
+        ctx.fetch_batch(2, 3, small, None, stream=stream)
+
+
+def parity_width(kind):
+    return (2, 4, 6, 10)[kind], (4, 4, 2, 5)[kind]
