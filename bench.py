@@ -216,6 +216,7 @@ def run_ours(args):
     needed = [sum(s["needed"][j] for s in stats) for j in range(4)]
     cands = [sum(s["candidates"][j] for s in stats) for j in range(4)]
     evals = [sum(s["evaluated"][j] for s in stats) for j in range(4)]
+    rewalks = [sum(s["rewalks"][j] for s in stats) for j in range(4)]
 
     # ---- the timed region ---------------------------------------------------------------
     sampler = ClockSampler(local)
@@ -295,6 +296,7 @@ def run_ours(args):
            "objects_per_step": dict(hits=n_hits, md=needed[0], ls=needed[1], t3=needed[2], t5=needed[3]),
            "candidates_per_step": dict(md=cands[0], ls=cands[1], t3=cands[2], t5=cands[3]),
            "evaluated_per_step": dict(md=evals[0], ls=evals[1], t3=evals[2], t5=evals[3]),
+           "rewalks_per_step": dict(md=rewalks[0], ls=rewalks[1], t3=rewalks[2], t5=rewalks[3]),
            "arena_mib": ctx.arena_bytes()[0] / 2 ** 20, "impl": "ours"}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         v, dt = oracle_events_per_s(geom, mmap, events)

@@ -481,7 +481,7 @@ __device__ __forceinline__ int md_walk(const Params& P, const Slot& S, MdWarp& s
   return running;
 }
 
-__global__ void __launch_bounds__(kWarps * 32) k_md(const __grid_constant__ Params P) {
+__global__ void __launch_bounds__(kWarps * 32, 6) k_md(const __grid_constant__ Params P) {
   __shared__ MdWarp shw[kWarps];
   __shared__ float s_w[6], s_rmaxU[6];
   Slot S(P, blockIdx.y);
@@ -740,7 +740,7 @@ __device__ __forceinline__ int seg_walk(const Params& P, const Slot& S, SegWarp&
   return running;
 }
 
-__global__ void __launch_bounds__(kSegWarps * 32) k_seg(const __grid_constant__ Params P) {
+__global__ void __launch_bounds__(kSegWarps * 32, 6) k_seg(const __grid_constant__ Params P) {
   __shared__ SegWarp shw[kSegWarps];
   __shared__ float s_rMinO[6], s_rMaxO[6];
   Slot S(P, blockIdx.y);
@@ -836,7 +836,7 @@ __global__ void __launch_bounds__(kSegWarps * 32) k_seg(const __grid_constant__ 
 // a3: triplets.  Owner = first segment a = (m1, m2); candidates are the segments leaving m2, a
 // contiguous range because segments are stored by inner MD.
 // ------------------------------------------------------------------------------------------
-constexpr int kT3Stash = 128;
+constexpr int kT3Stash = 96;
 struct T3Warp {
   float4 p1[32], p2[32];
   int layer[32], tab[32];
@@ -884,7 +884,7 @@ __device__ __forceinline__ int t3_walk(const Params& P, const Slot& S, T3Warp& s
   return running;
 }
 
-__global__ void __launch_bounds__(kWarps * 32) k_t3(const __grid_constant__ Params P) {
+__global__ void __launch_bounds__(kWarps * 32, 6) k_t3(const __grid_constant__ Params P) {
   __shared__ T3Warp shw[kWarps];
   Slot S(P, blockIdx.y);
   SlotHeader* H = S.hdr();
@@ -1052,7 +1052,7 @@ __device__ __forceinline__ int t5_walk(const Params& P, const Slot& S, T5Warp& s
   return running;
 }
 
-__global__ void __launch_bounds__(kWarps * 32) k_t5(const __grid_constant__ Params P) {
+__global__ void __launch_bounds__(kWarps * 32, 4) k_t5(const __grid_constant__ Params P) {
   __shared__ T5Warp shw[kWarps];
   Slot S(P, blockIdx.y);
   SlotHeader* H = S.hdr();
@@ -1225,7 +1225,7 @@ int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEv
       k_md<<<dim3(blocks_per_event((P.L.n_chunk[0] + kWarps - 1) / kWarps, n_batch, 6), nb), kWarps * 32, 0, s>>>(P);
       break;
     case LST_SEG_:
-      k_seg<<<dim3(blocks_per_event((P.L.n_chunk[1] + kSegWarps - 1) / kSegWarps, n_batch, 8), nb), kSegWarps * 32, 0, s>>>(P);
+      k_seg<<<dim3(blocks_per_event((P.L.n_chunk[1] + kSegWarps - 1) / kSegWarps, n_batch, 6), nb), kSegWarps * 32, 0, s>>>(P);
       break;
     case LST_T3_:
       k_t3<<<dim3(blocks_per_event((P.L.n_chunk[2] + kWarps - 1) / kWarps, n_batch, 6), nb), kWarps * 32, 0, s>>>(P);
