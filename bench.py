@@ -99,6 +99,26 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def rank_seed0(rank: int) -> int:
+    """First event seed of a rank: replicas work on disjoint events (rank r: seeds 64 r .. 64 r + 63)."""
+    return rank * N_EVENTS
+
+
+def max_over_ranks(value: float, dist, device) -> float:
+    """The slowest rank's time (the job is over when the last replica is)."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_events_per_s(world: int, steps: int, total_ms: float) -> float:
+    """Events all ranks processed / the slowest rank's time."""
+    return world * N_EVENTS * steps / (total_ms * 1e-3)
+
+
 def make_events(seed0: int, n: int):
     from paper_2207_08207_b200 import synth
     geom = synth.make_geometry()
@@ -166,7 +186,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = torch.device("cuda", local)
 
-    geom, mmap, events = make_events(rank * N_EVENTS, N_EVENTS)
+    geom, mmap, events = make_events(rank_seed0(rank), N_EVENTS)
     per_stream = N_EVENTS // N_STREAMS
     cfg = lst.default_config()
     cfg.device, cfg.n_slots = local, N_EVENTS
@@ -229,12 +249,8 @@ def run_ours(args):
     wall = time.perf_counter() - w0
     launches = ctx.launch_count() - l0
     clocks = sampler.stop()
-    total_ms = sum(ms)
-    if dist:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
-    value = world * N_EVENTS * args.steps / (total_ms * 1e-3)
+    total_ms = max_over_ranks(sum(ms), dist, dev)
+    value = whole_job_events_per_s(world, args.steps, total_ms)
 
     if args.profile:
         if rank == 0:
@@ -271,11 +287,7 @@ def run_ours(args):
     for _ in range(e2e_steps):
         step_e2e()
     torch.cuda.synchronize(dev)
-    e2e_s = time.perf_counter() - t0
-    if dist:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = max_over_ranks(time.perf_counter() - t0, dist, dev)
     h2d = sum(sum(t.numel() * t.element_size() for t in ev) for ev in h_in)
     d2h = needed[3] * (40 + 20) + N_EVENTS * HEADER_BYTES
     e2e = {"value": world * N_EVENTS * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),

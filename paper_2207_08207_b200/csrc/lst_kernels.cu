@@ -721,11 +721,12 @@ __device__ __forceinline__ int seg_walk(const Params& P, const Slot& S, SegWarp&
     float c0 = 0.0f;
     if (q < nPairs) {
       tgt = P.map_targets[e];
+      const float dphi = P.map_dphi[e];   // issued with the target load, not behind the test below
       const int4 info = mod_info[tgt];
       if (!DIRECT) space += (unsigned long long)(info.y - info.x);
       const float dlo = sh.dlo[ol], dhi = sh.dhi[ol];
       if (info.y > info.x && dlo <= dhi) {
-        c0 = sh.key[ol] + P.map_dphi[e];
+        c0 = sh.key[ol] + dphi;
         keep = !(fabsf(c0) + fmaxf(fabsf(dlo), fabsf(dhi)) < 3.0f) ||
                (c0 + dhi >= __int_as_float(info.z) && c0 + dlo <= __int_as_float(info.w));
       }
@@ -1198,7 +1199,8 @@ int launch_bin(const Params& P, const HitBatch& src, const HitBatch& dev, int n_
   int n_max = 0;
   for (int b = 0; b < n_batch; ++b) n_max = max(n_max, src.ev[b].n);
   const unsigned nb = (unsigned)n_batch;
-  const dim3 g(blocks_per_event((n_max + 255) / 256, n_batch, 8), nb);
+  // one hit per thread: the loads, the returning atomic and the scattered stores of all hits are in flight at once
+  const dim3 g(max(1, (n_max + 255) / 256), nb);
   LST_EV(0);
   k_reset<<<dim3(blocks_per_event((int)(P.L.reset_bytes / 16 + 255) / 256, n_batch, 8), nb), 256, 0, s>>>(P);
   LST_EV(1);
@@ -1206,7 +1208,7 @@ int launch_bin(const Params& P, const HitBatch& src, const HitBatch& dev, int n_
   // small grid leaves the SMs to the other streams' stage kernels.
   bool staged = false;
   for (int b = 0; b < n_batch; ++b) staged = staged || src.ev[b].stage;
-  const dim3 gc(staged ? min((int)g.x, 8) : g.x, nb);
+  const dim3 gc(staged ? min((int)g.x, 8) : blocks_per_event((int)g.x, n_batch, 8), nb);   // grid-stride: fewer 'last block' tickets
   k_bin_count<<<gc, 256, 0, s>>>(P, src);   // (+ stage-in) + scan of the bin counts by the event's last block
   if (staged && staged_in) cudaEventRecord(staged_in, s);
   LST_EV(2);

@@ -259,3 +259,33 @@ def test_fetch_batch_equals_per_slot_fetch(ctx, geom):
 
 def parity_width(kind):
     return (2, 4, 6, 10)[kind], (4, 4, 2, 5)[kind]
+
+
+def test_parity_in_the_bench_launch_configuration(lstmod, geom, mmap, o32, run_oracle):
+    """BASELINE.json configs[2] exactly as bench.py times it: 64 PU200-like events (seeds 0..63), device-resident
+    hit SoA, 64 slots, 4 CUDA streams x 16-event batched launches, two passes over the same arena.  Every event:
+    object and candidate counts equal the oracle's; 8 sampled events: every object and float compared."""
+    import torch
+    n_ev, n_streams = 64, 4
+    per = n_ev // n_streams
+    evs = [synth.generate_event(geom, 1, s) for s in range(n_ev)]
+    cfg = lstmod.default_config()
+    cfg.n_slots = n_ev
+    c = lstmod.Lst.from_synth(geom, mmap, cfg)
+    d_in = [[torch.from_numpy(a).cuda() for a in (e.x, e.y, e.z, e.module, e.side)] for e in evs]
+    streams = [torch.cuda.Stream() for _ in range(n_streams)]
+    torch.cuda.synchronize()
+    for _ in range(2):                                  # second pass: slots recycled by k_reset
+        for s, st in enumerate(streams):
+            c.load_events(s * per, d_in[s * per:(s + 1) * per], stream=st)
+            c.run_batch(s * per, per, st)
+    for s, st in enumerate(streams):
+        assert c.sync_batch(s * per, per, st) == 0
+    sampled = {0, 7, 15, 16, 31, 42, 48, 63}            # first / last of a batch, first / last of a stream
+    for k, ev in enumerate(evs):
+        ora = run_oracle(o32, ev)
+        st = c.stats(k)
+        assert st["needed"] == ora.counts and st["candidates"] == ora.candidates and st["n_hits"] == ev.n, (k, st)
+        if k in sampled:
+            parity.compare(parity.gpu_tables(c, k, streams[k // per]), parity.oracle_tables(ora), f"bench slot {k}")
+    c.close()
