@@ -52,10 +52,13 @@ struct lst_ctx {
   size_t arena_bytes = 0;
   std::vector<SlotHost> slots;
   SlotHeader* pinned = nullptr;
-  // Stage-in kernels (k_bin_count reading pinned host memory) of different streams are chained in enqueue
-  // order, as a copy engine would serve copies: each gets the whole PCIe link and the next stream's stage-in
-  // overlaps this stream's compute, instead of all of them sharing the link and finishing together.
-  cudaEvent_t stage_ev = nullptr;
+  // Stage-in kernels (k_bin_count reading pinned host memory) run on the library's own high-priority stream,
+  // forked from and joined to the caller's stream by events: like copies on a copy engine they are served one
+  // after the other at full link speed, and the next batch's stage-in overlaps this batch's stage kernels.
+  static constexpr int kStageEvents = 32;
+  cudaStream_t stage_stream = nullptr;
+  cudaEvent_t stage_ev[kStageEvents] = {};
+  unsigned stage_next = 0;
   std::mutex stage_mu;
   std::atomic<long long> launches{0};
   std::atomic<int> last_cuda{0};
@@ -250,7 +253,13 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
   if ((e = cudaMemset(c->arena, 0, c->arena_bytes)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   if ((e = cudaMallocHost(&c->pinned, sizeof(SlotHeader) * (size_t)cfg.n_slots)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   std::memset(c->pinned, 0, sizeof(SlotHeader) * (size_t)cfg.n_slots);
-  if ((e = cudaEventCreateWithFlags(&c->stage_ev, cudaEventDisableTiming)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
+  {
+    int lo = 0, hi = 0;
+    if ((e = cudaDeviceGetStreamPriorityRange(&lo, &hi)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
+    if ((e = cudaStreamCreateWithPriority(&c->stage_stream, cudaStreamNonBlocking, hi)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
+    for (auto& ev : c->stage_ev)
+      if ((e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
+  }
   c->slots.resize(cfg.n_slots);
   for (int s = 0; s < cfg.n_slots; ++s) {
     c->slots[s].hdr = c->pinned + s;
@@ -279,7 +288,9 @@ int lst_destroy(lst_ctx* c) {
   for (auto& s : c->slots)
     for (auto& ev : s.ev)
       if (ev) cudaEventDestroy(ev);
-  if (c->stage_ev) cudaEventDestroy(c->stage_ev);
+  for (auto& ev : c->stage_ev)
+    if (ev) cudaEventDestroy(ev);
+  if (c->stage_stream) cudaStreamDestroy(c->stage_stream);
   if (c->pinned) cudaFreeHost(c->pinned);
   if (c->arena) cudaFree(c->arena);
   if (c->d_map_dphi) cudaFree(c->d_map_dphi);
@@ -345,8 +356,9 @@ int lst_load_events(lst_ctx* c, int first, int n_ev, const lst_hits* hits, void*
     for (int b = 0; b < nb; ++b) staged = staged || src.ev[b].stage;
     if (staged) {
       std::lock_guard<std::mutex> lock(c->stage_mu);
-      LST_CUDA(c, cudaStreamWaitEvent(s, c->stage_ev, 0));   // a never-recorded event does not block
-      c->launches += launch_bin(P, src, dev, nb, s, c->cfg.timing ? sh0.ev : nullptr, c->stage_ev);
+      StageIn st{c->stage_stream, c->stage_ev[c->stage_next % lst_ctx::kStageEvents], c->stage_ev[(c->stage_next + 1) % lst_ctx::kStageEvents]};
+      c->stage_next += 2;
+      c->launches += launch_bin(P, src, dev, nb, s, c->cfg.timing ? sh0.ev : nullptr, &st);
     } else {
       c->launches += launch_bin(P, src, dev, nb, s, c->cfg.timing ? sh0.ev : nullptr, nullptr);
     }

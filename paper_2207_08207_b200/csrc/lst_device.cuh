@@ -153,10 +153,14 @@ struct HitBatch {
 // Host-callable launchers (lst_kernels.cu). Each returns the number of kernels it launched.
 // `ev` (optional, timing mode): ev[0] is recorded before the first kernel, ev[k + 1] after kernel k.
 // `src`: the arrays k_bin_count reads (device, or mapped host memory with stage = 1); `dev`: the device-resident arrays
-// the later kernels read (the same, or the slot's staging area).
-// `staged_in` (optional) is recorded right after k_bin_count when it read host memory.
+// the later kernels read (the same, or the slot's staging area).  `stage` (non-null when k_bin_count reads host memory):
+// the library's stage-in stream and the two events that fork it from / join it to `s`.
+struct StageIn {
+  cudaStream_t stream;
+  cudaEvent_t before, after;
+};
 int launch_bin(const Params& P, const HitBatch& src, const HitBatch& dev, int n_batch, cudaStream_t s, cudaEvent_t* ev,
-               cudaEvent_t staged_in);   // 4 kernels
+               const StageIn* stage);   // 4 kernels
 int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEvent_t* ev);          // 1 kernel
 int launch_gather_hits(const Params& P, int kind, int n_max, int n_batch, cudaStream_t s);   // slots first_slot .. + n_batch - 1
 int launch_pack_values(const Params& P, int kind, int n_max, int n_batch, cudaStream_t s);

@@ -1195,22 +1195,28 @@ static int blocks_per_event(int wanted, int n_batch, int resident_per_sm) {
 }
 
 int launch_bin(const Params& P, const HitBatch& src, const HitBatch& dev, int n_batch, cudaStream_t s, cudaEvent_t* ev,
-               cudaEvent_t staged_in) {
+               const StageIn* stage) {
   int n_max = 0;
   for (int b = 0; b < n_batch; ++b) n_max = max(n_max, src.ev[b].n);
   const unsigned nb = (unsigned)n_batch;
-  // one hit per thread: the loads, the returning atomic and the scattered stores of all hits are in flight at once
+  // one hit per thread: the loads and the scattered stores of all hits are in flight at once
   const dim3 g(max(1, (n_max + 255) / 256), nb);
   LST_EV(0);
   k_reset<<<dim3(blocks_per_event((int)(P.L.reset_bytes / 16 + 255) / 256, n_batch, 8), nb), 256, 0, s>>>(P);
   LST_EV(1);
-  // Reading mapped host memory the kernel is PCIe bound (~75 KB in flight cover latency x bandwidth): a
-  // small grid leaves the SMs to the other streams' stage kernels.
-  bool staged = false;
-  for (int b = 0; b < n_batch; ++b) staged = staged || src.ev[b].stage;
-  const dim3 gc(staged ? min((int)g.x, 8) : blocks_per_event((int)g.x, n_batch, 8), nb);   // grid-stride: fewer 'last block' tickets
-  k_bin_count<<<gc, 256, 0, s>>>(P, src);   // (+ stage-in) + scan of the bin counts by the event's last block
-  if (staged && staged_in) cudaEventRecord(staged_in, s);
+  if (stage) {
+    // Reading pinned host memory the kernel is PCIe bound (~75 KB in flight cover latency x bandwidth): a small
+    // grid, on the library's own high-priority stream so that its blocks are placed ahead of the other streams'
+    // stage kernels, and so that the stage-ins of all streams run one after the other at full link speed.
+    cudaEventRecord(stage->before, s);
+    cudaStreamWaitEvent(stage->stream, stage->before, 0);
+    k_bin_count<<<dim3(min((int)g.x, 8), nb), 256, 0, stage->stream>>>(P, src);
+    cudaEventRecord(stage->after, stage->stream);
+    cudaStreamWaitEvent(s, stage->after, 0);
+  } else {
+    // grid-stride: fewer 'last block' tickets; + scan of the bin counts by the event's last block
+    k_bin_count<<<dim3(blocks_per_event((int)g.x, n_batch, 8), nb), 256, 0, s>>>(P, src);
+  }
   LST_EV(2);
   k_bin_scatter<<<g, 256, 0, s>>>(P, dev);
   LST_EV(3);
