@@ -308,6 +308,9 @@ def run_ours(args):
            "objects_per_step": dict(hits=n_hits, md=needed[0], ls=needed[1], t3=needed[2], t5=needed[3]),
            "candidates_per_step": dict(md=cands[0], ls=cands[1], t3=cands[2], t5=cands[3]),
            "evaluated_per_step": dict(md=evals[0], ls=evals[1], t3=evals[2], t5=evals[3]),
+           "stage_overlap": {"sum_of_stage_ms_one_stream": sum(v["ms"] for v in per_stage.values()),
+                             "ms_per_step_4_streams": total_ms / args.steps,
+                             "factor": sum(v["ms"] for v in per_stage.values()) / (total_ms / args.steps)},
            "rewalks_per_step": dict(md=rewalks[0], ls=rewalks[1], t3=rewalks[2], t5=rewalks[3]),
            "arena_mib": ctx.arena_bytes()[0] / 2 ** 20, "impl": "ours"}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -381,6 +384,70 @@ def roofline(kernel_ms, n_hits, needed, cands, peaks):
     return roof, per_stage
 
 
+# ------------------------------------------------------------------------------------------
+# BASELINE.json configs[4]: occupancy sweep, a0 + mini-doublet + segment kernels only
+# ------------------------------------------------------------------------------------------
+def run_sweep(args):
+    """One JSON line per size (1 k, 10 k, 100 k, 1 M hits on the configs[0] geometry, 50 % track hits): per-kernel
+    ms (CUDA events around every launch, median of 5 after 2 warm-ups, L2 flushed), algorithmic HBM GB/s and its
+    fraction of the measured peak, evaluated candidates per second.  Capacities are grown from the sizes the
+    library reports as needed (LST_ERR_OVERFLOW -> lst_get_stats.needed), as a caller would."""
+    import torch
+    from paper_2207_08207_b200 import lst, synth
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    geom = synth.make_geometry()
+    mmap = synth.make_module_map(geom)
+    peaks = measured_peaks()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    st = torch.cuda.Stream()
+    for n in (1000, 10000, 100000, 1000000):
+        ev = synth.generate_occupancy_event(geom, n, seed=4)
+        d_in = [torch.from_numpy(a).cuda() for a in (ev.x, ev.y, ev.z, ev.module, ev.side)]
+        caps = dict(cap_hits=max(ev.n, 1024), cap_md=max(2 * ev.n, 1024), cap_seg=max(4 * ev.n, 1024), cap_t3=1024, cap_t5=1024)
+        for _ in range(4):                       # grow the capacities until MD and LS fit
+            cfg = lst.default_config()
+            cfg.n_slots, cfg.timing = 1, 1
+            for k, v in caps.items():
+                setattr(cfg, k, int(v))
+            ctx = lst.Lst.from_synth(geom, mmap, cfg)
+            ctx.load_events(0, [d_in], stream=st)
+            ctx.run_stage(0, 1, lst.MD, st)
+            ctx.run_stage(0, 1, lst.SEG, st)
+            status = ctx.sync(0, st, check=False)
+            need = ctx.stats(0)["needed"]
+            if status == lst.OK:
+                break
+            ctx.close()
+            caps["cap_md"] = max(caps["cap_md"], int(1.1 * need[0]) + 1024)
+            caps["cap_seg"] = max(caps["cap_seg"], int(1.1 * need[1]) + 1024, 4 * caps["cap_md"])
+        assert status == lst.OK, (n, status, need)
+        rows = []
+        for _ in range(7):
+            with torch.cuda.stream(st):
+                flush.zero_()
+            ctx.load_events(0, [d_in], stream=st)
+            ctx.run_stage(0, 1, lst.MD, st)
+            ctx.run_stage(0, 1, lst.SEG, st)
+            ctx.sync(0, st)
+            rows.append(ctx.stats(0)["kernel_ms"][:6])
+        stt = ctx.stats(0)
+        k_ms = dict(zip(lst.KERNEL_NAMES[:6], np.median(np.asarray(rows[2:]), axis=0).tolist()))
+        need, evl, cand = stt["needed"], stt["evaluated"], stt["candidates"]
+        per = {}
+        for name, ks, stage in (("a0_bin", ("reset", "bin_count", "bin_scatter", "bin_order"), 0), ("a1_md", ("md",), 1), ("a2_ls", ("seg",), 2)):
+            ms = sum(k_ms[k] for k in ks)
+            b = algorithmic_bytes(stage, stt["n_hits"], need)
+            per[name] = {"ms": ms, "algorithmic_bytes": int(b), "hbm_gbs": b / (ms * 1e-3) / 1e9,
+                         "hbm_frac": b / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"]}
+            if stage:
+                per[name].update(candidates=cand[stage - 1], evaluated=evl[stage - 1], passed=need[stage - 1],
+                                 evaluated_per_s=evl[stage - 1] / (ms * 1e-3))
+        print(json.dumps({"sweep": "BASELINE.json configs[4]", "hits": ev.n, "kernels_ms": k_ms, "per_stage": per,
+                          "rewalks": stt["rewalks"][:2], "capacities": caps, "peak_hbm_gbs": peaks["hbm_gbs"],
+                          "peak_source": peaks["source"], "arena_mib": ctx.arena_bytes()[0] / 2 ** 20}))
+        ctx.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -390,8 +457,11 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--profile", action="store_true",
                     help="device-resident steps only (no e2e, per-kernel timing or CPU baseline): the command ncu wraps")
+    ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[4]: occupancy sweep of the a0 / MD / LS kernels")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.sweep:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

@@ -206,7 +206,9 @@ LST_API int lst_load_events(lst_ctx* ctx, int first_slot, int n_slots, const lst
  * launches (the batch index is a grid dimension).  Asynchronous; no host synchronisation. */
 LST_API int lst_run(lst_ctx* ctx, int slot, void* cuda_stream);
 LST_API int lst_run_batch(lst_ctx* ctx, int first_slot, int n_slots, void* cuda_stream);
-/* One stage only (LST_MD .. LST_T5) of a slot range; lst_run_batch == the four in order. */
+/* One stage only (LST_MD .. LST_T5) of a slot range; lst_run_batch == the four in order.  A stage needs the
+ * one before it (LST_ERR_STATE otherwise); after a partial run the views / fetches of the classes built so far
+ * are valid (BASELINE.json configs[4] runs the mini-doublet and segment stages only). */
 LST_API int lst_run_stage(lst_ctx* ctx, int first_slot, int n_slots, int stage, void* cuda_stream);
 
 /* Waits for `cuda_stream`, reads the slot's counters back and returns its status:

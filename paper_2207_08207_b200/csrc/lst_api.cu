@@ -30,7 +30,8 @@ static_assert((int)LST_MD == (int)LST_MD_ && (int)LST_SEG == (int)LST_SEG_ && (i
 namespace {
 
 struct SlotHost {
-  bool loaded = false, ran = false, synced = false;
+  bool loaded = false, synced = false;
+  int stages_run = 0;         // stages a1 .. run in order since the load: objects of class k are valid iff stages_run > k
   int n_hits_in = 0;
   SlotHeader* hdr = nullptr;  // pinned host copy of the device header
   cudaEvent_t ev[13] = {};    // timing mode: ev[0..4] around the 4 a0 kernels, ev[5 + 2 s], ev[6 + 2 s] around stage s
@@ -322,7 +323,8 @@ int lst_load_events(lst_ctx* c, int first, int n_ev, const lst_hits* hits, void*
       const int slot = first + b0 + b;
       const lst_hits* h = hits + b0 + b;
       SlotHost& sh = c->slots[slot];
-      sh.loaded = sh.ran = sh.synced = false;
+      sh.loaded = sh.synced = false;
+      sh.stages_run = 0;
       sh.n_hits_in = h->n;
       sh.ev_bin = false;
       for (bool& f : sh.ev_stage) f = false;
@@ -374,7 +376,7 @@ int lst_load_event(lst_ctx* c, int slot, const lst_hits* h, void* stream) { retu
 int lst_run_stage(lst_ctx* c, int first, int n, int stage, void* stream) {
   if (!c || n < 1 || !valid_slot(c, first) || !valid_slot(c, first + n - 1) || stage < LST_MD || stage > LST_T5) return LST_ERR_ARG;
   for (int s = first; s < first + n; ++s)
-    if (!c->slots[s].loaded) return LST_ERR_STATE;
+    if (!c->slots[s].loaded || c->slots[s].stages_run < stage) return LST_ERR_STATE;   // a stage needs the one before it
   cudaStream_t st = (cudaStream_t)stream;
   LST_CUDA(c, cudaSetDevice(c->device));
   SlotHost& sh = c->slots[first];
@@ -383,7 +385,7 @@ int lst_run_stage(lst_ctx* c, int first, int n, int stage, void* stream) {
   c->launches += launch_stage(P, n, stage, st, c->cfg.timing ? sh.ev + 5 + 2 * stage : nullptr);
   LST_CUDA(c, cudaGetLastError());
   if (c->cfg.timing) sh.ev_stage[stage] = true;
-  for (int s = first; s < first + n; ++s) { c->slots[s].synced = false; if (stage == LST_T5) c->slots[s].ran = true; }
+  for (int s = first; s < first + n; ++s) { c->slots[s].synced = false; c->slots[s].stages_run = stage + 1; }
   return LST_OK;
 }
 
@@ -412,16 +414,16 @@ int lst_sync(lst_ctx* c, int slot, void* stream) {
   return LST_OK;
 }
 
-static int view_ready(lst_ctx* c, int slot) {
+static int view_ready(lst_ctx* c, int slot, int kind) {
   if (!valid_slot(c, slot)) return LST_ERR_ARG;
   const SlotHost& sh = c->slots[slot];
-  if (!sh.synced || !sh.ran) return LST_ERR_STATE;
+  if (!sh.synced || sh.stages_run <= kind) return LST_ERR_STATE;
   if (sh.hdr->overflow) return LST_ERR_OVERFLOW;
   return LST_OK;
 }
 
 int lst_get_mds(lst_ctx* c, int slot, lst_md_view* v) {
-  const int r = view_ready(c, slot);
+  const int r = view_ready(c, slot, LST_MD);
   if (r != LST_OK || !v) return r != LST_OK ? r : LST_ERR_ARG;
   const Layout& L = c->P.L;
   const char* b = c->arena + (size_t)slot * c->P.slot_stride;
@@ -436,7 +438,7 @@ int lst_get_mds(lst_ctx* c, int slot, lst_md_view* v) {
 }
 
 int lst_get_segments(lst_ctx* c, int slot, lst_seg_view* v) {
-  const int r = view_ready(c, slot);
+  const int r = view_ready(c, slot, LST_SEG);
   if (r != LST_OK || !v) return r != LST_OK ? r : LST_ERR_ARG;
   const Layout& L = c->P.L;
   const char* b = c->arena + (size_t)slot * c->P.slot_stride;
@@ -448,7 +450,7 @@ int lst_get_segments(lst_ctx* c, int slot, lst_seg_view* v) {
 }
 
 int lst_get_triplets(lst_ctx* c, int slot, lst_t3_view* v) {
-  const int r = view_ready(c, slot);
+  const int r = view_ready(c, slot, LST_T3);
   if (r != LST_OK || !v) return r != LST_OK ? r : LST_ERR_ARG;
   const Layout& L = c->P.L;
   const char* b = c->arena + (size_t)slot * c->P.slot_stride;
@@ -461,7 +463,7 @@ int lst_get_triplets(lst_ctx* c, int slot, lst_t3_view* v) {
 }
 
 int lst_get_quintuplets(lst_ctx* c, int slot, lst_t5_view* v) {
-  const int r = view_ready(c, slot);
+  const int r = view_ready(c, slot, LST_T5);
   if (r != LST_OK || !v) return r != LST_OK ? r : LST_ERR_ARG;
   const Layout& L = c->P.L;
   const char* b = c->arena + (size_t)slot * c->P.slot_stride;
@@ -528,7 +530,7 @@ int lst_fetch_batch(lst_ctx* c, int first, int n, int kind, int32_t* const* idx_
   if (!c || n < 1 || !valid_slot(c, first) || !valid_slot(c, first + n - 1) || kind < LST_MD || kind > LST_T5 || !cap_objects)
     return LST_ERR_ARG;
   for (int s = first; s < first + n; ++s)
-    if (!c->slots[s].loaded || !c->slots[s].ran) return LST_ERR_STATE;
+    if (!c->slots[s].loaded || c->slots[s].stages_run <= kind) return LST_ERR_STATE;
   bool all_synced = true;
   for (int s = first; s < first + n; ++s) all_synced = all_synced && c->slots[s].synced;
   if (!all_synced) {
@@ -582,7 +584,7 @@ int lst_fetch_batch(lst_ctx* c, int first, int n, int kind, int32_t* const* idx_
 
 int lst_fetch_hit_indices(lst_ctx* c, int slot, int kind, int32_t* out, int64_t cap, void* stream) {
   if (kind < LST_MD || kind > LST_T5) return LST_ERR_ARG;
-  const int r = view_ready(c, slot);
+  const int r = view_ready(c, slot, kind);
   if (r != LST_OK) return r;
   const int n = c->slots[slot].hdr->n[kind];
   if (n == 0) return LST_OK;
@@ -594,7 +596,7 @@ int lst_fetch_hit_indices(lst_ctx* c, int slot, int kind, int32_t* out, int64_t 
 
 int lst_fetch_values(lst_ctx* c, int slot, int kind, float* out, int64_t cap, void* stream) {
   if (kind < LST_MD || kind > LST_T5) return LST_ERR_ARG;
-  const int r = view_ready(c, slot);
+  const int r = view_ready(c, slot, kind);
   if (r != LST_OK) return r;
   const int n = c->slots[slot].hdr->n[kind];
   if (n == 0) return LST_OK;

@@ -289,3 +289,72 @@ def test_parity_in_the_bench_launch_configuration(lstmod, geom, mmap, o32, run_o
         if k in sampled:
             parity.compare(parity.gpu_tables(c, k, streams[k // per]), parity.oracle_tables(ora), f"bench slot {k}")
     c.close()
+
+
+def test_occupancy_sweep_1m_hits_sampled(lstmod, geom, mmap, o32):
+    """BASELINE.json configs[4] at its maximum size (1 M hits; mini-doublet and segment stages only), in the launch
+    configuration `bench.py --sweep` times.  The oracle finishes the MD stage (60 M candidates) in seconds: ALL
+    876 k mini-doublets are compared.  The segment stage has 1.8e9 candidates, so segments are checked on sampled
+    inner MDs: for each, the oracle's scalar cut is run over every MD of every connected module and the resulting
+    set of outer MDs (and the float outputs) must equal the GPU's segments of that MD."""
+    import torch
+    ev = synth.generate_occupancy_event(geom, 1000000, seed=4)
+    ora = o32.run(geom.layer, mmap.row_offsets, mmap.targets, ev.x, ev.y, ev.z, ev.module, ev.side, stages=1)
+    cfg = lstmod.default_config()
+    cfg.n_slots, cfg.cap_hits, cfg.cap_md, cfg.cap_seg, cfg.cap_t3, cfg.cap_t5 = 1, ev.n, 2 * ev.n, 20 * ev.n, 1024, 1024
+    c = lstmod.Lst.from_synth(geom, mmap, cfg)
+    st = torch.cuda.Stream()
+    d_in = [torch.from_numpy(a).cuda() for a in (ev.x, ev.y, ev.z, ev.module, ev.side)]
+    c.load_events(0, [d_in], stream=st)
+    c.run_stage(0, 1, lstmod.MD, st)
+    c.run_stage(0, 1, lstmod.SEG, st)
+    assert c.sync(0, st) == 0
+    stats = c.stats(0)
+    assert stats["needed"][0] == ora.counts[0] and stats["candidates"][0] == ora.candidates[0] and stats["n_hits"] == ev.n
+    # every mini-doublet, bit-exact as (lower hit, upper hit), floats within tolerance
+    g_hits = c.fetch_hit_indices(0, lstmod.MD, st)
+    g_vals = c.fetch_values(0, lstmod.MD, st)
+    oh = ora.md_hits()
+    ov = np.stack([ora.md_sinA, ora.md_dphi, ora.md_dphichange, ora.md_r], 1)
+    gh, gv = parity.sort_rows(g_hits, g_vals)
+    oh_s, ov_s = parity.sort_rows(oh, ov)
+    assert np.array_equal(gh, oh_s)
+    for col, (name, floor) in enumerate(parity.VALUE_SPEC[0]):
+        a, b = gv[:, col].astype(np.float64), ov_s[:, col].astype(np.float64)
+        assert np.all(np.abs(a - b) <= parity.REL_TOL * np.maximum(np.abs(a), np.abs(b)) + floor), name
+    # segments of sampled inner MDs
+    key = lambda h: (h[:, 0].astype(np.int64) << 32) | h[:, 1].astype(np.int64)
+    gpu_of = dict(zip(key(g_hits).tolist(), range(len(g_hits))))
+    view = lstmod.SegView()
+    assert c.lib.lst_get_segments(c.h, 0, view) == 0 and view.n == stats["needed"][1]
+    seg_md = lstmod.DeviceArray(view.md, (view.n, 2), "<i4", c).torch().cpu().numpy()
+    seg_f = lstmod.DeviceArray(view.f, (view.n, 4), "<f4", c).torch().cpu().numpy()
+    md_start = lstmod.DeviceArray(view.md_start, (stats["needed"][0] + 1,), "<i4", c).torch().cpu().numpy()
+    assert md_start[0] == 0 and md_start[-1] == view.n and np.all(np.diff(md_start) >= 0)
+    order = np.argsort(ora.md_module, kind="stable")
+    first = np.searchsorted(ora.md_module[order], np.arange(geom.n_modules + 1))
+    rec = lambda i: (ora.md_x[i], ora.md_y[i], ora.md_z[i], ora.md_r[i], ora.md_ur[i], ora.md_sinA[i])
+    rng = np.random.default_rng(11)
+    inner_layers = np.nonzero(geom.layer[ora.md_module] <= 4)[0]
+    n_seg_checked = 0
+    for i in rng.choice(inner_layers, 60, replace=False):
+        A = int(ora.md_module[i])
+        L = int(geom.layer[A])
+        want = {}
+        for B in mmap.targets[mmap.row_offsets[A]:mmap.row_offsets[A + 1]]:
+            for o in order[first[B]:first[B + 1]]:
+                ok, out, _ = o32.seg_cut(L, rec(i), rec(o))
+                if ok:
+                    want[int(key(oh[o:o + 1])[0])] = out
+        g = gpu_of[int(key(oh[i:i + 1])[0])]
+        rows = range(md_start[g], md_start[g + 1])
+        assert all(seg_md[r, 0] == g for r in rows)
+        got = {int(key(g_hits[seg_md[r, 1]:seg_md[r, 1] + 1])[0]): seg_f[r] for r in rows}
+        assert set(got) == set(want), (i, len(got), len(want))
+        for k, out in want.items():
+            for col, (name, floor) in enumerate(parity.VALUE_SPEC[1]):
+                a, b = float(got[k][col]), float(out[name.split("_")[1]])
+                assert abs(a - b) <= parity.REL_TOL * max(abs(a), abs(b)) + floor, (name, a, b)
+        n_seg_checked += len(want)
+    assert n_seg_checked > 300
+    c.close()
