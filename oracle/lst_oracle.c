@@ -569,6 +569,66 @@ lsto_event* lsto_run(const lsto_config* cfg, int32_t n_modules, const int8_t* la
   return ev;
 }
 
+/* ------------------------------------------------------------------------------------ */
+/* [D] duplicate cleaning of quintuplets  (DESIGN.md section 1 [D])      */
+/* ------------------------------------------------------------------------------------ */
+/* The paper cleans duplicates when the track-candidate collection is assembled (PAPER.md:67
+ * "cross-clean", :105 "efficient cross-cleaning ... duplicate rates are quite low") and gives no
+ * rule for quintuplets among themselves; the rule here is DESIGN.md reading 24:
+ *   score(q)  = chi2xy(q) + chi2rz(q)                        (one addition in `real`)
+ *   shared(a, b) = number of original hit indices the two quintuplets have in common
+ *   b beats a  iff  score(b) < score(a), or the scores are equal and b's hit tuple (10 indices,
+ *                   in layer order: MD1 lower, MD1 upper, ...) is lexicographically smaller
+ *   a is REMOVED iff some b != a has shared(a, b) >= min_shared and b beats a
+ * (removed quintuplets still remove others: the rule is one pass over all pairs, independent of
+ * any processing order).  This is the plain definition: every pair is looked at; the common hits
+ * of a pair are counted by merging the two sorted copies of the tuples (the 10 hits of a
+ * quintuplet are distinct, pin P9).
+ * hits: [n][10] original hit indices; keep: [n] out, 1 = kept.  Returns the number kept. */
+static int cmp_i32(const void* a, const void* b) {
+  const int32_t x = *(const int32_t*)a, y = *(const int32_t*)b;
+  return (x > y) - (x < y);
+}
+int64_t lsto_t5_clean(int64_t n, const int32_t* hits, const real* chi2xy, const real* chi2rz, int min_shared,
+                      uint8_t* keep) {
+  int64_t a, b, kept = 0;
+  int k;
+  int32_t* sorted = malloc((size_t)(n > 0 ? n : 1) * 10 * sizeof(int32_t));
+  real* score = malloc((size_t)(n > 0 ? n : 1) * sizeof(real));
+  for (a = 0; a < n; ++a) {
+    for (k = 0; k < 10; ++k) sorted[10 * a + k] = hits[10 * a + k];
+    qsort(sorted + 10 * a, 10, sizeof(int32_t), cmp_i32);
+    score[a] = chi2xy[a] + chi2rz[a];
+    keep[a] = 1;
+  }
+  for (a = 0; a < n; ++a) {
+    for (b = 0; b < n; ++b) {
+      int i = 0, j = 0, shared = 0, beats;
+      const int32_t *sa = sorted + 10 * a, *sb = sorted + 10 * b;
+      if (b == a) continue;
+      while (i < 10 && j < 10) {
+        if (sa[i] < sb[j]) ++i;
+        else if (sa[i] > sb[j]) ++j;
+        else { ++shared; ++i; ++j; }
+      }
+      if (shared < min_shared) continue;
+      if (score[b] < score[a]) beats = 1;
+      else if (score[b] > score[a]) beats = 0;
+      else {
+        beats = 0;
+        for (k = 0; k < 10; ++k) {
+          if (hits[10 * b + k] != hits[10 * a + k]) { beats = hits[10 * b + k] < hits[10 * a + k]; break; }
+        }
+      }
+      if (beats) { keep[a] = 0; break; }
+    }
+    kept += keep[a];
+  }
+  free(sorted);
+  free(score);
+  return kept;
+}
+
 /* ---- accessors for the ctypes wrapper ---- */
 int64_t lsto_count(const lsto_event* ev, int kind) {
   switch (kind) { case 0: return ev->n_md; case 1: return ev->n_seg; case 2: return ev->n_t3; case 3: return ev->n_t5; }

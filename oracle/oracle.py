@@ -88,6 +88,8 @@ class OracleLib:
         lib.lsto_t5_cut.argtypes = [P(self.Config), C.c_int, r, r, P(r), P(r), P(r)]
         for f in (lib.lsto_md_cut, lib.lsto_seg_cut, lib.lsto_t3_cut, lib.lsto_t5_cut):
             f.restype = C.c_int
+        lib.lsto_t5_clean.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
+        lib.lsto_t5_clean.restype = C.c_int64
 
     # ---- configuration -------------------------------------------------------------------
     def default_config(self):
@@ -133,6 +135,19 @@ class OracleLib:
         ok = self.lib.lsto_t5_cut(C.byref(cfg), int(layer1), self.real(float(kappa_a)), self.real(float(kappa_b)),
                                   self._arr(flat), out, mar)
         return bool(ok), dict(zip(("kfit", "chi2xy", "chi2rz"), list(out))), list(mar)
+
+    def t5_clean(self, hits, chi2xy, chi2rz, min_shared: int = 7) -> np.ndarray:
+        """[D] duplicate cleaning: hits [n][10] original hit indices -> keep [n] bool (all-pairs definition)."""
+        hits = np.ascontiguousarray(hits, np.int32).reshape(-1, 10)
+        n = len(hits)
+        cx = np.ascontiguousarray(chi2xy, self.np_real)
+        cz = np.ascontiguousarray(chi2rz, self.np_real)
+        assert len(cx) == n and len(cz) == n
+        keep = np.zeros(max(n, 1), np.uint8)
+        ptr = lambda a: a.ctypes.data_as(C.c_void_p)
+        kept = self.lib.lsto_t5_clean(C.c_int64(n), ptr(hits), ptr(cx), ptr(cz), int(min_shared), ptr(keep))
+        assert kept == int(keep[:n].sum())
+        return keep[:n].astype(bool)
 
     # ---- whole event -----------------------------------------------------------------------
     def run(self, layer, row_offsets, targets, x, y, z, module, side, mode=0, stages=4, cfg=None) -> "OracleResult":
