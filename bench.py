@@ -39,7 +39,7 @@ N_STREAMS = int(os.environ.get("LST_BENCH_STREAMS", "4"))   # BASELINE.json conf
 MAP_BYTES = 4 * (69630 + 6121)
 # SPEC operations per candidate (every sqrt and div counted as one)
 FLOPS_PER_CAND = (34, 51, 45, 255)
-HEADER_BYTES = 304   # per-slot counter block that lst_sync_batch reads back (csrc/lst_device.cuh SlotHeader)
+HEADER_BYTES = 312   # per-slot counter block that lst_sync_batch reads back (csrc/lst_device.cuh SlotHeader)
 
 
 def algorithmic_bytes(stage: int, n_hits, needed):
@@ -297,8 +297,25 @@ def run_ours(args):
 
     # ---- per-kernel times (CUDA events inside the library, timing mode), one 64-event batch ----
     kernel_ms = per_kernel_times(lst, geom, mmap, d_in, local)
+    clean_ms = {k: kernel_ms.pop(k) for k in lst.KERNEL_NAMES[8:]}
     peaks = measured_peaks()
     roof, per_stage = roofline(kernel_ms, n_hits, needed, evals, peaks)
+
+    # ---- the path followed by the optional duplicate-cleaning stage [D], same timing rules ----
+    def step_device_clean():
+        for s, st in enumerate(streams):
+            ctx.load_events(s * per_stream, d_in[s * per_stream:(s + 1) * per_stream], stream=st)
+            ctx.run_batch(s * per_stream, per_stream, st)
+            ctx.run_stage(s * per_stream, per_stream, lst.CLEAN, st)
+    timed(step_device_clean, 3)
+    clean_total_ms = max_over_ranks(sum(timed(step_device_clean, args.steps)), dist, dev)
+    for s, st in enumerate(streams):
+        ctx.sync_batch(s * per_stream, per_stream, st)
+    kept = sum(ctx.stats(k)["n_kept"] for k in range(N_EVENTS))
+    clean = {"events_per_s_with_clean": whole_job_events_per_s(world, args.steps, clean_total_ms),
+             "ms_per_step_with_clean": clean_total_ms / args.steps, "kernels_ms_one_stream": clean_ms,
+             "t5_in": needed[3], "t5_kept": kept,
+             "what": "a0..a4 + LST_CLEAN per step; `value` above is a0..a4 only (the BASELINE.json path)"}
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
            "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -311,6 +328,7 @@ def run_ours(args):
            "stage_overlap": {"sum_of_stage_ms_one_stream": sum(v["ms"] for v in per_stage.values()),
                              "ms_per_step_4_streams": total_ms / args.steps,
                              "factor": sum(v["ms"] for v in per_stage.values()) / (total_ms / args.steps)},
+           "duplicate_cleaning": clean,
            "rewalks_per_step": dict(md=rewalks[0], ls=rewalks[1], t3=rewalks[2], t5=rewalks[3]),
            "arena_mib": ctx.arena_bytes()[0] / 2 ** 20, "impl": "ours"}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -339,12 +357,13 @@ def per_kernel_times(lst, geom, mmap, d_in, local, reps=5):
             flush.zero_()
         ctx.load_events(0, d_in, stream=st)
         ctx.run_batch(0, N_EVENTS, st)
+        ctx.run_stage(0, N_EVENTS, lst.CLEAN, st)          # optional stage [D], reported beside the path, not in it
         ctx.sync(0, st)
-        k_ms = np.zeros(8)
+        k_ms = np.zeros(12)
         for k in range(0, N_EVENTS, 16):                  # a0 runs in launches of 16 events
             ctx.sync(k, st)
             k_ms[:4] += np.asarray(ctx.stats(k)["kernel_ms"][:4])
-        k_ms[4:] = np.asarray(ctx.stats(0)["kernel_ms"][4:8])
+        k_ms[4:] = np.asarray(ctx.stats(0)["kernel_ms"][4:12])
         rows.append(k_ms)
     ctx.close()
     return dict(zip(lst.KERNEL_NAMES, np.median(np.asarray(rows[2:]), axis=0).tolist()))

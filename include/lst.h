@@ -56,7 +56,8 @@ enum {
   LST_ERR_NOMEM = -5     /* arena allocation failed in lst_create                                  */
 };
 
-enum { LST_MD = 0, LST_SEG = 1, LST_T3 = 2, LST_T5 = 3 };
+enum { LST_MD = 0, LST_SEG = 1, LST_T3 = 2, LST_T5 = 3,
+       LST_CLEAN = 4 /* optional stage after LST_T5: duplicate cleaning of the quintuplets (lst_run_stage only) */ };
 
 typedef struct lst_ctx lst_ctx;
 
@@ -115,6 +116,8 @@ typedef struct {
   int32_t cap_t5;
   int32_t timing;     /* != 0: record CUDA events around every kernel (lst_get_stats.stage_ms /
                          kernel_ms; for a batch they are kept on its first slot) */
+  int32_t t5_dup_min_shared; /* [D] D4: quintuplets sharing at least this many of their 10 original hits
+                         are duplicates (7) */
 } lst_config;
 
 /* Fills *cfg with the frozen SPEC constants, device 0, 4 slots and capacities that hold the
@@ -170,6 +173,16 @@ typedef struct {
   const int32_t* t3_start; /* [n_t3 + 1] quintuplets with inner triplet A are [start[A], start[A+1]) */
 } lst_t5_view;
 
+/* Result of the optional duplicate-cleaning stage (DESIGN.md section 1 [D]): the
+ * quintuplets that no better quintuplet sharing >= t5_dup_min_shared original hits removes -- the T5-only
+ * track-candidate list. */
+typedef struct {
+  int32_t n;            /* quintuplets kept                                                       */
+  const int32_t* t5;    /* [n] their indices into lst_t5_view, ascending                          */
+  const uint8_t* keep;  /* [n_t5] 1 = kept                                                        */
+  const float* score;   /* [n_t5] chi2xy + chi2rz                                                 */
+} lst_tc_view;
+
 typedef struct {
   int32_t n_hits;
   int64_t needed[4];     /* objects that passed per class (may exceed the capacity on overflow) */
@@ -182,8 +195,10 @@ typedef struct {
   int32_t overflow;      /* bit k set: capacity of class k exceeded                              */
   int32_t bad_hits;      /* hits dropped because module id / side was out of range               */
   float stage_ms[5];     /* a0 .. a4; zeros unless lst_config.timing                              */
-  float kernel_ms[12];   /* a0: reset, bin count + scan, scatter, order; then the MD, LS, T3, T5 kernel; rest 0 */
+  float kernel_ms[12];   /* a0: reset, bin count + scan, scatter, order; then the MD, LS, T3, T5 kernel; then the four
+                            kernels of LST_CLEAN (prepare, count + scan, fill, mark + list) */
   int64_t rewalks[4];    /* chunks of 32 owners whose objects exceeded the on-chip stash and were walked twice */
+  int32_t n_kept;        /* quintuplets kept by LST_CLEAN (0 if the stage was not run)                         */
 } lst_stats;
 
 /* Validates geometry and map, uploads the per-module tables, allocates the arena (the only
@@ -208,7 +223,9 @@ LST_API int lst_run(lst_ctx* ctx, int slot, void* cuda_stream);
 LST_API int lst_run_batch(lst_ctx* ctx, int first_slot, int n_slots, void* cuda_stream);
 /* One stage only (LST_MD .. LST_T5) of a slot range; lst_run_batch == the four in order.  A stage needs the
  * one before it (LST_ERR_STATE otherwise); after a partial run the views / fetches of the classes built so far
- * are valid (BASELINE.json configs[4] runs the mini-doublet and segment stages only). */
+ * are valid (BASELINE.json configs[4] runs the mini-doublet and segment stages only).  LST_CLEAN (duplicate
+ * cleaning of the quintuplets, DESIGN.md section 1 [D]) is not part of lst_run / lst_run_batch: run it with
+ * lst_run_stage after LST_T5. */
 LST_API int lst_run_stage(lst_ctx* ctx, int first_slot, int n_slots, int stage, void* cuda_stream);
 
 /* Waits for `cuda_stream`, reads the slot's counters back and returns its status:
@@ -226,6 +243,11 @@ LST_API int lst_get_mds(lst_ctx* ctx, int slot, lst_md_view* out);
 LST_API int lst_get_segments(lst_ctx* ctx, int slot, lst_seg_view* out);
 LST_API int lst_get_triplets(lst_ctx* ctx, int slot, lst_t3_view* out);
 LST_API int lst_get_quintuplets(lst_ctx* ctx, int slot, lst_t5_view* out);
+/* Valid after LST_CLEAN was run (lst_run_stage) and the slot synced. */
+LST_API int lst_get_track_candidates(lst_ctx* ctx, int slot, lst_tc_view* out);
+/* Indices (into the quintuplet arrays, ascending) of the kept quintuplets to HOST memory: out[n_kept];
+ * LST_ERR_ARG if cap < n_kept.  Synchronises `cuda_stream`. */
+LST_API int lst_fetch_kept(lst_ctx* ctx, int slot, int32_t* out, int64_t cap, void* cuda_stream);
 /* Valid after any lst_sync of the slot (also after an overflow). */
 LST_API int lst_get_stats(lst_ctx* ctx, int slot, lst_stats* out);
 

@@ -25,7 +25,7 @@
 using namespace lst;
 
 static_assert((int)LST_MD == (int)LST_MD_ && (int)LST_SEG == (int)LST_SEG_ && (int)LST_T3 == (int)LST_T3_ &&
-                  (int)LST_T5 == (int)LST_T5_, "stage ids");
+                  (int)LST_T5 == (int)LST_T5_ && (int)LST_CLEAN == (int)LST_CLEAN_, "stage ids");
 
 namespace {
 
@@ -34,8 +34,8 @@ struct SlotHost {
   int stages_run = 0;         // stages a1 .. run in order since the load: objects of class k are valid iff stages_run > k
   int n_hits_in = 0;
   SlotHeader* hdr = nullptr;  // pinned host copy of the device header
-  cudaEvent_t ev[13] = {};    // timing mode: ev[0..4] around the 4 a0 kernels, ev[5 + 2 s], ev[6 + 2 s] around stage s
-  bool ev_bin = false, ev_stage[4] = {false, false, false, false};
+  cudaEvent_t ev[18] = {};    // timing mode: ev[0..4] around the 4 a0 kernels, ev[5 + 2 s], ev[6 + 2 s] around stage s, ev[13..17] around the 4 cleaning kernels
+  bool ev_bin = false, ev_stage[5] = {false, false, false, false, false};
 };
 
 }  // namespace
@@ -105,6 +105,8 @@ Layout make_layout(const lst_config& cfg, int n_modules) {
   L.t3_pack = take(16 * n3); L.t3_seg = take(8 * n3); L.t3_chi2 = take(4 * n3);
   L.t5_start = take(4 * (n3 + 1));
   L.t5_md = take(20 * n5); L.t5_t3 = take(8 * n5); L.t5_f = take(20 * n5);
+  L.t5_hits = take(40 * n5); L.t5_score = take(4 * n5); L.t5_keep = take(n5); L.tc_list = take(4 * n5);
+  L.inc_start = take(4 * (nm + 8)); L.inc_cur = take(4 * (nm + 8)); L.inc_list = take(40 * n5);
   size_t scr = 16 * nm;   // one gathered table at a time: hit-index tuples (8 / 16 / 24 / 40 B) or packed values (16 / 16 / 8 / 20 B)
   if (16 * ns > scr) scr = 16 * ns;
   if (24 * n3 > scr) scr = 24 * n3;
@@ -187,6 +189,7 @@ int lst_default_config(lst_config* c) {
   c->cap_t3 = 384 * 1024;
   c->cap_t5 = 128 * 1024;
   c->timing = 0;
+  c->t5_dup_min_shared = 7;
   return LST_OK;
 }
 
@@ -199,6 +202,7 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
   if (n <= 0 || n > (1 << 24) || m->n_modules != n || !g->layer || !g->phi || !m->row_offsets) return LST_ERR_ARG;
   /* object indices are packed into 26 bits, module ids into 24 bits by the stage kernels */
   if (cfg.cap_hits > kMaxCap || cfg.cap_md > kMaxCap || cfg.cap_seg > kMaxCap || cfg.cap_t3 > kMaxCap || cfg.cap_t5 > kMaxCap) return LST_ERR_ARG;
+  if (cfg.t5_dup_min_shared < 1 || cfg.t5_dup_min_shared > 10) return LST_ERR_ARG;
   if (cfg.n_slots < 1 || cfg.cap_hits < 1 || cfg.cap_md < 1 || cfg.cap_seg < 1 || cfg.cap_t3 < 1 || cfg.cap_t5 < 1) return LST_ERR_ARG;
   for (int i = 0; i < n; ++i)
     if (g->layer[i] < 0 || g->layer[i] >= LST_N_LAYERS) return LST_ERR_ARG;
@@ -278,6 +282,7 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
   c->P.map_targets = c->d_map_targets;
   c->P.map_dphi = c->d_map_dphi;
   c->P.first_slot = 0;
+  c->P.dup_min_shared = cfg.t5_dup_min_shared;
   if ((e = cudaDeviceSynchronize()) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   *out = c;
   return LST_OK;
@@ -374,7 +379,7 @@ int lst_load_events(lst_ctx* c, int first, int n_ev, const lst_hits* hits, void*
 int lst_load_event(lst_ctx* c, int slot, const lst_hits* h, void* stream) { return lst_load_events(c, slot, 1, h, stream); }
 
 int lst_run_stage(lst_ctx* c, int first, int n, int stage, void* stream) {
-  if (!c || n < 1 || !valid_slot(c, first) || !valid_slot(c, first + n - 1) || stage < LST_MD || stage > LST_T5) return LST_ERR_ARG;
+  if (!c || n < 1 || !valid_slot(c, first) || !valid_slot(c, first + n - 1) || stage < LST_MD || stage > LST_CLEAN) return LST_ERR_ARG;
   for (int s = first; s < first + n; ++s)
     if (!c->slots[s].loaded || c->slots[s].stages_run < stage) return LST_ERR_STATE;   // a stage needs the one before it
   cudaStream_t st = (cudaStream_t)stream;
@@ -382,7 +387,10 @@ int lst_run_stage(lst_ctx* c, int first, int n, int stage, void* stream) {
   SlotHost& sh = c->slots[first];
   Params P = c->P;
   P.first_slot = first;
-  c->launches += launch_stage(P, n, stage, st, c->cfg.timing ? sh.ev + 5 + 2 * stage : nullptr);
+  if (stage == LST_CLEAN)
+    c->launches += launch_clean(P, n, st, c->cfg.timing ? sh.ev + 13 : nullptr);
+  else
+    c->launches += launch_stage(P, n, stage, st, c->cfg.timing ? sh.ev + 5 + 2 * stage : nullptr);
   LST_CUDA(c, cudaGetLastError());
   if (c->cfg.timing) sh.ev_stage[stage] = true;
   for (int s = first; s < first + n; ++s) { c->slots[s].synced = false; c->slots[s].stages_run = stage + 1; }
@@ -475,6 +483,32 @@ int lst_get_quintuplets(lst_ctx* c, int slot, lst_t5_view* v) {
   return LST_OK;
 }
 
+int lst_get_track_candidates(lst_ctx* c, int slot, lst_tc_view* v) {
+  const int r = view_ready(c, slot, LST_CLEAN);
+  if (r != LST_OK || !v) return r != LST_OK ? r : LST_ERR_ARG;
+  const Layout& L = c->P.L;
+  const char* b = c->arena + (size_t)slot * c->P.slot_stride;
+  v->n = c->slots[slot].hdr->n_kept;
+  v->t5 = (const int32_t*)(b + L.tc_list);
+  v->keep = (const uint8_t*)(b + L.t5_keep);
+  v->score = (const float*)(b + L.t5_score);
+  return LST_OK;
+}
+
+int lst_fetch_kept(lst_ctx* c, int slot, int32_t* out, int64_t cap, void* stream) {
+  const int r = view_ready(c, slot, LST_CLEAN);
+  if (r != LST_OK) return r;
+  const int n = c->slots[slot].hdr->n_kept;
+  if (n == 0) return LST_OK;
+  if (!out || cap < n) return LST_ERR_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  LST_CUDA(c, cudaSetDevice(c->device));
+  const char* b = c->arena + (size_t)slot * c->P.slot_stride;
+  LST_CUDA(c, cudaMemcpyAsync(out, b + c->P.L.tc_list, sizeof(int32_t) * (size_t)n, cudaMemcpyDeviceToHost, s));
+  LST_CUDA(c, cudaStreamSynchronize(s));
+  return LST_OK;
+}
+
 int lst_get_stats(lst_ctx* c, int slot, lst_stats* o) {
   if (!valid_slot(c, slot) || !o) return LST_ERR_ARG;
   SlotHost& sh = c->slots[slot];
@@ -484,11 +518,14 @@ int lst_get_stats(lst_ctx* c, int slot, lst_stats* o) {
   for (int k = 0; k < 4; ++k) { o->needed[k] = (int64_t)sh.hdr->needed[k]; o->candidates[k] = (int64_t)sh.hdr->cand[k]; o->evaluated[k] = (int64_t)sh.hdr->eval[k]; o->rewalks[k] = (int64_t)sh.hdr->rewalk[k]; }
   o->overflow = sh.hdr->overflow;
   o->bad_hits = sh.hdr->bad_hits;
+  o->n_kept = sh.stages_run > LST_CLEAN ? sh.hdr->n_kept : 0;
   if (c->cfg.timing) {
     if (sh.ev_bin) {
       cudaEventElapsedTime(&o->stage_ms[0], sh.ev[0], sh.ev[4]);
       for (int k = 0; k < 4; ++k) cudaEventElapsedTime(&o->kernel_ms[k], sh.ev[k], sh.ev[k + 1]);
     }
+    if (sh.ev_stage[4])
+      for (int k = 0; k < 4; ++k) cudaEventElapsedTime(&o->kernel_ms[8 + k], sh.ev[13 + k], sh.ev[14 + k]);
     for (int st = 0; st < 4; ++st)
       if (sh.ev_stage[st]) {
         cudaEvent_t* e = sh.ev + 5 + 2 * st;

@@ -44,7 +44,7 @@ constexpr int kChunk = 32;        // owners (lower hits / MDs / segments / tripl
 constexpr int kMaxBatch = 16;     // events per launch of the a0 kernels (pointer table in the launch parameters)
 constexpr int kMaxRow = 64;       // longest module-map row accepted
 constexpr int kMaxCap = 1 << 26;  // largest per-slot capacity: object indices are packed into 26 bits
-enum { LST_MD_ = 0, LST_SEG_ = 1, LST_T3_ = 2, LST_T5_ = 3 };  // == LST_MD .. LST_T5 of lst.h
+enum { LST_MD_ = 0, LST_SEG_ = 1, LST_T3_ = 2, LST_T5_ = 3, LST_CLEAN_ = 4 };  // == LST_MD .. LST_CLEAN of lst.h
 
 struct SlotHeader {
   int n_hits;                     // valid hits binned
@@ -62,6 +62,8 @@ struct SlotHeader {
   int r_max[2][6];
   unsigned int done[8];           // "last block done" tickets, self-resetting
   unsigned int ticket[4];         // next chunk of the single-pass kernels (zeroed with the header)
+  int n_kept;                     // quintuplets kept by the duplicate cleaning (stage LST_CLEAN)
+  int pad_;
 };
 
 struct Layout {
@@ -77,6 +79,7 @@ struct Layout {
   size_t seg_start, seg_md, seg_f;
   size_t t3_start, t3_pack, t3_seg, t3_chi2;
   size_t t5_start, t5_md, t5_t3, t5_f;
+  size_t t5_hits, t5_score, t5_keep, tc_list, inc_start, inc_cur, inc_list;   // duplicate cleaning
   size_t scratch;
   size_t slot_bytes;
 };
@@ -93,6 +96,7 @@ struct Params {
   const int* map_targets;        // [map_offsets[n_modules]] ascending per row
   const float* map_dphi;         // [map_offsets[n_modules]] azimuth(source normal) - azimuth(target normal), in (-pi, pi]
   int first_slot;
+  int dup_min_shared;            // [D] D4: quintuplets sharing at least this many original hits are duplicates
 };
 
 // Typed access to one slot.
@@ -132,6 +136,13 @@ struct Slot {
   __device__ __forceinline__ int* t5_md() const { return at<int>(L.t5_md); }
   __device__ __forceinline__ int2* t5_t3() const { return at<int2>(L.t5_t3); }
   __device__ __forceinline__ float* t5_f() const { return at<float>(L.t5_f); }
+  __device__ __forceinline__ int* t5_hits() const { return at<int>(L.t5_hits); }
+  __device__ __forceinline__ float* t5_score() const { return at<float>(L.t5_score); }
+  __device__ __forceinline__ unsigned char* t5_keep() const { return at<unsigned char>(L.t5_keep); }
+  __device__ __forceinline__ int* tc_list() const { return at<int>(L.tc_list); }
+  __device__ __forceinline__ int* inc_start() const { return at<int>(L.inc_start); }
+  __device__ __forceinline__ int* inc_cur() const { return at<int>(L.inc_cur); }
+  __device__ __forceinline__ int2* inc_list() const { return at<int2>(L.inc_list); }
   __device__ __forceinline__ int* scratch() const { return at<int>(L.scratch); }
 };
 
@@ -162,6 +173,8 @@ struct StageIn {
 int launch_bin(const Params& P, const HitBatch& src, const HitBatch& dev, int n_batch, cudaStream_t s, cudaEvent_t* ev,
                const StageIn* stage);   // 4 kernels
 int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEvent_t* ev);          // 1 kernel
+// Duplicate cleaning [D]: 4 kernels; ev[k] before kernel k, ev[4] after the last.
+int launch_clean(const Params& P, int n_batch, cudaStream_t s, cudaEvent_t* ev);
 int launch_gather_hits(const Params& P, int kind, int n_max, int n_batch, cudaStream_t s);   // slots first_slot .. + n_batch - 1
 int launch_pack_values(const Params& P, int kind, int n_max, int n_batch, cudaStream_t s);
 

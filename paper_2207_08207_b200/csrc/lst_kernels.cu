@@ -1139,6 +1139,210 @@ __global__ void __launch_bounds__(kWarps * 32, 4) k_t5(const __grid_constant__ P
 }
 
 // ------------------------------------------------------------------------------------------
+// [D] duplicate cleaning of quintuplets (DESIGN.md section 1 [D]; optional stage LST_CLEAN).
+// Two quintuplets that share >= 7 of their 10 original hits share a mini-doublet (a mini-doublet is a
+// pair of hits of one module: without a common MD at most one hit per common layer can coincide), so the
+// partners of a quintuplet are found through an MD -> quintuplets incidence table (counting sort over the
+// MDs: count, scan, fill), and every (quintuplet, partner) pair goes through the exact rule D2-D4.
+// The result does not depend on the order of the incidence lists: D4 is an "exists" over the partners.
+// ------------------------------------------------------------------------------------------
+// score, hit tuple in layer order; zero the incidence counters
+__global__ void __launch_bounds__(256) k_clean_prepare(const __grid_constant__ Params P) {
+  Slot S(P, blockIdx.y);
+  const SlotHeader* H = S.hdr();
+  const int n5 = H->n[LST_T5_], nmd = H->n[LST_MD_];
+  int* cnt = S.inc_start();
+  int* cur = S.inc_cur();
+  const int2* mh = S.md_hits();
+  const int nz = (nmd + 1 + 3) / 4 * 4;   // the in-place scan reads whole int4s
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < max(n5, nz); i += gridDim.x * blockDim.x) {
+    if (i < nz) { cnt[i] = 0; cur[i] = 0; }
+    if (i < n5) {
+      const float* f = S.t5_f() + 5 * (size_t)i;
+      S.t5_score()[i] = f[3] + f[4];                       // D1
+      S.t5_keep()[i] = 1;
+      const int* md = S.t5_md() + 5 * (size_t)i;
+      int2* out = reinterpret_cast<int2*>(S.t5_hits()) + 5 * (size_t)i;
+#pragma unroll
+      for (int k = 0; k < 5; ++k) out[k] = mh[md[k]];
+    }
+  }
+}
+
+// quintuplets per MD; the event's last block turns the counts into offsets
+__global__ void __launch_bounds__(256) k_clean_count(const __grid_constant__ Params P) {
+  Slot S(P, blockIdx.y);
+  SlotHeader* H = S.hdr();
+  const int n5 = H->n[LST_T5_], nmd = H->n[LST_MD_];
+  int* cnt = S.inc_start();
+  const int* md = S.t5_md();
+  for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < 5 * n5; j += gridDim.x * blockDim.x) atomicAdd(cnt + md[j], 1);
+  if (!last_block_done(&H->done[5], gridDim.x)) return;
+  block_scan_array4<256>(cnt, nmd);
+}
+
+__global__ void __launch_bounds__(256) k_clean_fill(const __grid_constant__ Params P) {
+  Slot S(P, blockIdx.y);
+  const int n5 = S.hdr()->n[LST_T5_];
+  const int* start = S.inc_start();
+  int* cur = S.inc_cur();
+  int2* list = S.inc_list();
+  const int* md = S.t5_md();
+  for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < 5 * n5; j += gridDim.x * blockDim.x) {
+    const int m = md[j];
+    list[start[m] + atomicAdd(cur + m, 1)] = make_int2(j / 5, m);
+  }
+}
+
+// A hit belongs to one layer and one sensor side, so it can sit at one position only of a quintuplet's tuple:
+// with OFF = (position of a common MD in q) - (its position in b), MD i of q can only equal MD i - OFF of b and
+// hit k of q only hit k - 2 OFF of b.  Quintuplets span 5 of the 6 layers, so OFF is -1, 0 or 1.
+template <int OFF>
+__device__ __forceinline__ void common_mds(const int (&qm)[5], const int (&bm)[5], int pos, int& n_md, bool& earlier) {
+  n_md = 0;
+  earlier = false;
+#pragma unroll
+  for (int i = 0; i < 5; ++i) {
+    if (i - OFF < 0 || i - OFF >= 5) continue;
+    const bool eq = qm[i] == bm[i - OFF];
+    n_md += eq;
+    earlier = earlier || (eq && i < pos);
+  }
+}
+template <int OFF>
+__device__ __forceinline__ int common_hits(const int (&a)[10], const int (&h)[10]) {
+  int shared = 0;
+#pragma unroll
+  for (int k = 0; k < 10; ++k)
+    if (k - 2 * OFF >= 0 && k - 2 * OFF < 10) shared += (a[k] == h[k - 2 * OFF]);
+  return shared;
+}
+
+// One thread per entry of the incidence table = (quintuplet q, one of its five MDs): rule D2-D4 against every
+// quintuplet in that MD's list.  Threads are taken in TABLE order, so neighbouring threads walk the same list
+// (same trip count, the partners' records served from L1).
+// A removal is an idempotent store of 0 (k_clean_prepare set every flag to 1).  The event's last block then
+// lists the kept quintuplets in ascending order (the T5-only track-candidate list).
+__global__ void __launch_bounds__(256) k_clean_mark(const __grid_constant__ Params P) {
+  __shared__ int s_warp[8];
+  __shared__ int s_base;
+  Slot S(P, blockIdx.y);
+  SlotHeader* H = S.hdr();
+  const int n5 = H->n[LST_T5_];
+  const int* start = S.inc_start();
+  const int2* list = S.inc_list();
+  const int* md = S.t5_md();
+  const int* hits = S.t5_hits();
+  const float* score = S.t5_score();
+  unsigned char* keep = S.t5_keep();
+  const int K = P.dup_min_shared;
+  for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < 5 * n5; t += gridDim.x * blockDim.x) {
+    const int2 entry = list[t];
+    const int q = entry.x, m = entry.y;
+    const int j0 = start[m], j1 = start[m + 1];
+    if (j1 - j0 < 2) continue;                              // the list holds q itself only
+    int qm[5];
+#pragma unroll
+    for (int k = 0; k < 5; ++k) qm[k] = md[5 * (size_t)q + k];
+    int pos = 0;
+#pragma unroll
+    for (int k = 1; k < 5; ++k) pos = (qm[k] == m) ? k : pos;
+    const float sq = score[q];
+    bool removed = false;
+    for (int j = j0; j < j1 && !removed; ++j) {
+      const int b = list[j].x;
+      if (b == q) continue;
+      // common MDs first: a common MD is two common hits, and a layer without a common MD holds at most one
+      // common hit, so  2 * n_md <= shared <= n_md + 5 : most pairs are decided without looking at the hits
+      int bm[5];
+#pragma unroll
+      for (int k = 0; k < 5; ++k) bm[k] = md[5 * (size_t)b + k];
+      int kpos = 0;
+#pragma unroll
+      for (int k = 1; k < 5; ++k) kpos = (bm[k] == m) ? k : kpos;
+      const int off = pos - kpos;
+      int n_md = 0;
+      bool earlier = false;
+      if (off == 0) common_mds<0>(qm, bm, pos, n_md, earlier);
+      else if (off == 1) common_mds<1>(qm, bm, pos, n_md, earlier);
+      else if (off == -1) common_mds<-1>(qm, bm, pos, n_md, earlier);
+      else {   // not reachable with 6 layers; the position-free form
+#pragma unroll
+        for (int k = 0; k < 5; ++k)
+#pragma unroll
+          for (int i = 0; i < 5; ++i) {
+            const bool eq = qm[i] == bm[k];
+            n_md += eq;
+            earlier = earlier || (eq && i < pos);
+          }
+      }
+      if (earlier) continue;                                // the thread of the earlier common MD handles this pair
+      bool dup = 2 * n_md >= K;
+      const bool need_hits = !dup && n_md + 5 >= K;
+      const float sb = score[b];
+      if (!need_hits && (!dup || sb != sq)) {               // decided by the MDs and the scores alone
+        removed = dup && sb < sq;
+        continue;
+      }
+      int a[10], h[10];
+#pragma unroll
+      for (int k = 0; k < 10; ++k) { a[k] = hits[10 * (size_t)q + k]; h[k] = hits[10 * (size_t)b + k]; }
+      if (need_hits) {
+        int shared = 0;                                     // D2: the 10 hits of a quintuplet are distinct
+        if (off == 0) shared = common_hits<0>(a, h);
+        else if (off == 1) shared = common_hits<1>(a, h);
+        else if (off == -1) shared = common_hits<-1>(a, h);
+        else {
+#pragma unroll
+          for (int i = 0; i < 10; ++i)
+#pragma unroll
+            for (int k = 0; k < 10; ++k) shared += (a[i] == h[k]);
+        }
+        dup = shared >= K;
+      }
+      if (!dup) continue;
+      bool beats = sb < sq;                                 // D3
+      if (sb == sq) {
+#pragma unroll
+        for (int k = 9; k >= 0; --k)
+          if (h[k] != a[k]) beats = h[k] < a[k];            // the first differing position decides
+      }
+      removed = beats;
+    }
+    if (removed) keep[q] = 0;
+  }
+  if (!last_block_done(&H->done[6], gridDim.x)) return;
+  // ordered list of the kept ones: 8 flags per thread and step
+  int* tc = S.tc_list();
+  if (threadIdx.x == 0) s_base = 0;
+  __syncthreads();
+  for (int q0 = 0; q0 < n5; q0 += 2048) {
+    const int q = q0 + 8 * threadIdx.x;
+    unsigned long long f = 0;
+    if (q < n5) f = __ldcg(reinterpret_cast<const unsigned long long*>(keep + q));   // the array is padded to 256 B
+    if (q + 8 > n5) f &= (q < n5) ? ((1ull << (8 * (n5 - q))) - 1ull) : 0ull;
+    const int mine = __popcll(f & 0x0101010101010101ull);
+    const int incl = warp_incl_scan(mine);
+    if (lane_id() == 31) s_warp[threadIdx.x >> 5] = incl;
+    __syncthreads();
+    int before = s_base, total = 0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) {
+      before += (w < (int)(threadIdx.x >> 5)) ? s_warp[w] : 0;
+      total += s_warp[w];
+    }
+    int pos = before + incl - mine;
+#pragma unroll
+    for (int k = 0; k < 8; ++k)
+      if ((f >> (8 * k)) & 1ull) tc[pos++] = q + k;
+    __syncthreads();
+    if (threadIdx.x == 0) s_base += total;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) H->n_kept = s_base;
+}
+
+// ------------------------------------------------------------------------------------------
 // output helpers: original-hit-index tuples and float payloads, one thread per object
 // ------------------------------------------------------------------------------------------
 // blockIdx.y = slot of the batch; the object count comes from the slot header (clamped to capacity).
@@ -1246,6 +1450,20 @@ int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEv
   }
   LST_EV(1);
   return 1;
+}
+
+int launch_clean(const Params& P, int n_batch, cudaStream_t s, cudaEvent_t* ev) {
+  const dim3 g(blocks_per_event((P.L.cap_t5 + 255) / 256, n_batch, 4), (unsigned)n_batch);
+  LST_EV(0);
+  k_clean_prepare<<<g, 256, 0, s>>>(P);
+  LST_EV(1);
+  k_clean_count<<<g, 256, 0, s>>>(P);
+  LST_EV(2);
+  k_clean_fill<<<g, 256, 0, s>>>(P);
+  LST_EV(3);
+  k_clean_mark<<<dim3(blocks_per_event((5 * P.L.cap_t5 + 255) / 256, n_batch, 8), (unsigned)n_batch), 256, 0, s>>>(P);
+  LST_EV(4);
+  return 4;
 }
 
 int launch_gather_hits(const Params& P, int kind, int n_max, int n_batch, cudaStream_t s) {

@@ -19,8 +19,10 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "liblst.so")
 N_LAYERS = 6
 MD, SEG, T3, T5 = 0, 1, 2, 3
+CLEAN = 4                                      # optional stage: duplicate cleaning of the quintuplets (run_stage only)
 KIND_NAMES = ("md", "seg", "t3", "t5")
-KERNEL_NAMES = ("reset", "bin_count", "bin_scatter", "bin_order", "md", "seg", "t3", "t5")   # lst_stats.kernel_ms[0..7]
+KERNEL_NAMES = ("reset", "bin_count", "bin_scatter", "bin_order", "md", "seg", "t3", "t5",
+                "clean_prepare", "clean_count", "clean_fill", "clean_mark")   # lst_stats.kernel_ms[0..11]
 HITS_PER_OBJECT = (2, 4, 6, 10)
 VALUES_PER_OBJECT = (4, 4, 2, 5)
 
@@ -51,7 +53,8 @@ class Config(C.Structure):
                 ("t5_chi2rz_max", C.c_float * 2), ("t5_chi2xy_max", C.c_float), ("t5_sigma_xy2_scaled", C.c_float),
                 ("t5_kappa_max", C.c_float),
                 ("device", C.c_int32), ("n_slots", C.c_int32), ("cap_hits", C.c_int32), ("cap_md", C.c_int32),
-                ("cap_seg", C.c_int32), ("cap_t3", C.c_int32), ("cap_t5", C.c_int32), ("timing", C.c_int32)]
+                ("cap_seg", C.c_int32), ("cap_t3", C.c_int32), ("cap_t5", C.c_int32), ("timing", C.c_int32),
+                ("t5_dup_min_shared", C.c_int32)]
 
     CUT_FIELDS = ("half_kappa_max", "z_lum", "md_cos_eps", "md_sin_eps", "md_dz_res", "md_eps", "seg_cos_eps",
                   "seg_sin_eps", "seg_z0_max", "t3_kappa_max", "t3_chi2rz_max", "sigma_z2", "inv_sigma_z2",
@@ -91,7 +94,11 @@ class T5View(C.Structure):
 class Stats(C.Structure):
     _fields_ = [("n_hits", C.c_int32), ("needed", C.c_int64 * 4), ("candidates", C.c_int64 * 4),
                 ("evaluated", C.c_int64 * 4), ("overflow", C.c_int32), ("bad_hits", C.c_int32), ("stage_ms", C.c_float * 5), ("kernel_ms", C.c_float * 12),
-                ("rewalks", C.c_int64 * 4)]
+                ("rewalks", C.c_int64 * 4), ("n_kept", C.c_int32)]
+
+
+class TcView(C.Structure):
+    _fields_ = [("n", C.c_int32), ("t5", C.c_void_p), ("keep", C.c_void_p), ("score", C.c_void_p)]
 
 
 # every symbol include/lst.h declares: name -> (restype, argtypes)
@@ -114,6 +121,8 @@ SYMBOLS = {
     "lst_get_triplets": (C.c_int, [C.c_void_p, C.c_int, P(T3View)]),
     "lst_get_quintuplets": (C.c_int, [C.c_void_p, C.c_int, P(T5View)]),
     "lst_get_stats": (C.c_int, [C.c_void_p, C.c_int, P(Stats)]),
+    "lst_get_track_candidates": (C.c_int, [C.c_void_p, C.c_int, P(TcView)]),
+    "lst_fetch_kept": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_int64, C.c_void_p]),
     "lst_fetch_hit_indices": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int64, C.c_void_p]),
     "lst_fetch_values": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int64, C.c_void_p]),
     "lst_arena_bytes": (C.c_int, [C.c_void_p, P(C.c_int64), P(C.c_int64)]),
@@ -165,7 +174,7 @@ class DeviceArray:
     def torch(self):
         import torch
         if 0 in self.shape:
-            return torch.empty(self.shape, dtype={"<i4": torch.int32, "<f4": torch.float32}[self.__cuda_array_interface__["typestr"]], device="cuda")
+            return torch.empty(self.shape, dtype={"<i4": torch.int32, "<f4": torch.float32, "|u1": torch.uint8}[self.__cuda_array_interface__["typestr"]], device="cuda")
         return torch.as_tensor(self, device="cuda")
 
 
@@ -308,7 +317,7 @@ class Lst:
         self._check(self.lib.lst_get_stats(self.h, slot, C.byref(s)), "lst_get_stats")
         return dict(n_hits=int(s.n_hits), needed=[int(v) for v in s.needed], candidates=[int(v) for v in s.candidates],
                     evaluated=[int(v) for v in s.evaluated], overflow=int(s.overflow), bad_hits=int(s.bad_hits), stage_ms=[float(v) for v in s.stage_ms],
-                    kernel_ms=[float(v) for v in s.kernel_ms], rewalks=[int(v) for v in s.rewalks])
+                    kernel_ms=[float(v) for v in s.kernel_ms], rewalks=[int(v) for v in s.rewalks], n_kept=int(s.n_kept))
 
     def mds(self, slot: int) -> dict:
         v = MdView()
@@ -339,6 +348,20 @@ class Lst:
         n_t3 = self.stats(slot)["needed"][T3]
         return dict(n=v.n, md=DeviceArray(v.md, (v.n, 5), "<i4", self), t3=DeviceArray(v.t3, (v.n, 2), "<i4", self),
                     f=DeviceArray(v.f, (v.n, 5), "<f4", self), t3_start=DeviceArray(v.t3_start, (n_t3 + 1,), "<i4", self))
+
+    def track_candidates(self, slot: int) -> dict:
+        """After run_stage(..., CLEAN) and sync: the kept quintuplets (device arrays)."""
+        v = TcView()
+        self._check(self.lib.lst_get_track_candidates(self.h, slot, C.byref(v)), "lst_get_track_candidates")
+        n5 = self.stats(slot)["needed"][T5]
+        return dict(n=v.n, t5=DeviceArray(v.t5, (v.n,), "<i4", self), keep=DeviceArray(v.keep, (n5,), "|u1", self),
+                    score=DeviceArray(v.score, (n5,), "<f4", self))
+
+    def fetch_kept(self, slot: int, stream=None) -> np.ndarray:
+        """Indices of the kept quintuplets (ascending), host numpy."""
+        out = np.empty(max(self.stats(slot)["n_kept"], 1), np.int32)
+        self._check(self.lib.lst_fetch_kept(self.h, slot, _ptr(out), out.shape[0], _stream(stream)), "lst_fetch_kept")
+        return out[:self.stats(slot)["n_kept"]]
 
     def fetch_hit_indices(self, slot: int, kind: int, stream=None, out=None) -> np.ndarray:
         """[n][2|4|6|10] original hit indices of every object of class ``kind`` (host numpy)."""

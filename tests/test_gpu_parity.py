@@ -358,3 +358,67 @@ def test_occupancy_sweep_1m_hits_sampled(lstmod, geom, mmap, o32):
         n_seg_checked += len(want)
     assert n_seg_checked > 300
     c.close()
+
+
+@pytest.mark.parametrize("config,seed,n_particles", [(0, 0, None), (0, 3, None), (1, 21, 900), (1, 0, None)])
+def test_duplicate_cleaning_parity(ctx, lstmod, o32, run_oracle, geom, config, seed, n_particles):
+    """Stage LST_CLEAN (DESIGN.md section 1 [D]) against the oracle's all-pairs definition: the kept set must be
+    IDENTICAL (as hit tuples; the decision is taken on both sides on the same fp32 score), the kept list ascending and
+    consistent with the flags; incl. the full PU200-like event (10.5 k quintuplets, 110 M pairs in the oracle)."""
+    import torch
+    ev = synth.generate_event(geom, config, seed) if n_particles is None else synth.generate_event(geom, config, seed, n_particles=n_particles)
+    st = torch.cuda.Stream()
+    gpu = parity.run_gpu(ctx, ev, slot=1, stream=st)
+    with pytest.raises(lstmod.LstError):
+        ctx.track_candidates(1)                                   # stage not run yet -> LST_ERR_STATE
+    ctx.run_stage(1, 1, lstmod.CLEAN, st)
+    ctx.sync(1, st)
+    ora = run_oracle(o32, ev)
+    keep_o = o32.t5_clean(ora.t5_hits(), ora.t5_chi2xy, ora.t5_chi2rz, 7)
+    tc = ctx.track_candidates(1)
+    keep_g = tc["keep"].torch().cpu().numpy().astype(bool)
+    kept_idx = ctx.fetch_kept(1, st)
+    g_hits = gpu[3][0]
+    assert len(keep_g) == len(g_hits) == len(keep_o) and tc["n"] == ctx.stats(1)["n_kept"] == int(keep_g.sum())
+    assert np.array_equal(kept_idx, np.nonzero(keep_g)[0])
+    assert np.array_equal(tc["t5"].torch().cpu().numpy(), kept_idx)
+    as_set = lambda h: set(map(tuple, h.tolist()))
+    assert as_set(g_hits[keep_g]) == as_set(ora.t5_hits()[keep_o])
+    # scores: the same fp32 addition on both sides
+    score_g = tc["score"].torch().cpu().numpy()
+    gs, _ = parity.sort_rows(g_hits, score_g.reshape(-1, 1))
+    order_g = np.lexsort(g_hits.T[::-1]); order_o = np.lexsort(ora.t5_hits().T[::-1])
+    assert np.array_equal(score_g[order_g], (ora.t5_chi2xy + ora.t5_chi2rz).astype(np.float32)[order_o])
+    assert 0 < keep_g.sum() < len(keep_g)
+
+
+def test_duplicate_cleaning_batch_empty_and_ties(lstmod, geom, mmap, o32, run_oracle):
+    """A batch of slots through one set of LST_CLEAN launches (incl. an empty event and an event without quintuplets),
+    a second threshold (t5_dup_min_shared = 5), and the stage order check."""
+    import torch
+    cfg = lstmod.default_config()
+    cfg.n_slots, cfg.t5_dup_min_shared = 4, 5
+    c = lstmod.Lst.from_synth(geom, mmap, cfg)
+    st = torch.cuda.Stream()
+    full = synth.generate_event(geom, 1, 8, n_particles=600)
+    lower_only = np.nonzero(full.side == 0)[0]
+    sub = synth.Event(full.x[lower_only], full.y[lower_only], full.z[lower_only], full.module[lower_only], full.side[lower_only],
+                      full.truth[lower_only], {})
+    empty = synth.Event(*(np.zeros(0, t) for t in (np.float32, np.float32, np.float32, np.int32, np.uint8, np.int32)), {})
+    evs = [full, empty, sub, synth.generate_event(geom, 0, 9)]
+    c.load_events(0, [(e.x, e.y, e.z, e.module, e.side) for e in evs], stream=st)
+    c.run_stage(0, 4, lstmod.MD, st)
+    with pytest.raises(lstmod.LstError):
+        c.run_stage(0, 4, lstmod.CLEAN, st)                       # needs the quintuplets first
+    for stage in (lstmod.SEG, lstmod.T3, lstmod.T5, lstmod.CLEAN):
+        c.run_stage(0, 4, stage, st)
+    assert c.sync_batch(0, 4, st) == 0
+    for k, ev in enumerate(evs):
+        ora = run_oracle(o32, ev)
+        keep_o = o32.t5_clean(ora.t5_hits(), ora.t5_chi2xy, ora.t5_chi2rz, 5)
+        hits = c.fetch_hit_indices(k, lstmod.T5, st)
+        kept = c.fetch_kept(k, st)
+        assert c.stats(k)["n_kept"] == int(keep_o.sum()) == len(kept)
+        assert set(map(tuple, hits[kept].tolist())) == set(map(tuple, ora.t5_hits()[keep_o].tolist()))
+    assert c.stats(1)["n_kept"] == 0 and c.stats(2)["n_kept"] == 0
+    c.close()
