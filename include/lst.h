@@ -195,8 +195,8 @@ typedef struct {
   int32_t overflow;      /* bit k set: capacity of class k exceeded                              */
   int32_t bad_hits;      /* hits dropped because module id / side was out of range               */
   float stage_ms[5];     /* a0 .. a4; zeros unless lst_config.timing                              */
-  float kernel_ms[12];   /* a0: reset, bin count + scan, scatter, order; then the MD, LS, T3, T5 kernel; then the four
-                            kernels of LST_CLEAN (prepare, count + scan, fill, mark + list) */
+  float kernel_ms[12];   /* a0: reset, bin count + offsets scan (2 launches), scatter, order; then the MD, LS, T3, T5 kernel; then the four
+                            steps of LST_CLEAN (prepare, count + offsets scan, fill, mark + list) */
   int64_t rewalks[4];    /* chunks of 32 owners whose objects exceeded the on-chip stash and were walked twice */
   int32_t n_kept;        /* quintuplets kept by LST_CLEAN (0 if the stage was not run)                         */
 } lst_stats;

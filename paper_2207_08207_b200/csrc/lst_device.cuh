@@ -171,9 +171,9 @@ struct StageIn {
   cudaEvent_t before, after;
 };
 int launch_bin(const Params& P, const HitBatch& src, const HitBatch& dev, int n_batch, cudaStream_t s, cudaEvent_t* ev,
-               const StageIn* stage);   // 4 kernels
+               const StageIn* stage);   // 5 kernels
 int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEvent_t* ev);          // 1 kernel
-// Duplicate cleaning [D]: 4 kernels; ev[k] before kernel k, ev[4] after the last.
+// Duplicate cleaning [D]: 5 kernels (prepare, count, scan, fill, mark); ev[0..4] around the four steps.
 int launch_clean(const Params& P, int n_batch, cudaStream_t s, cudaEvent_t* ev);
 int launch_gather_hits(const Params& P, int kind, int n_max, int n_batch, cudaStream_t s);   // slots first_slot .. + n_batch - 1
 int launch_pack_values(const Params& P, int kind, int n_max, int n_batch, cudaStream_t s);

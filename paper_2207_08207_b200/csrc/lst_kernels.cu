@@ -63,45 +63,49 @@ __device__ __forceinline__ unsigned long long warp_sum_ull(unsigned long long v)
 }
 
 // In-place exclusive scan of the ints a[0 .. n] (a[n] must be 0 on entry and receives the total)
-// by the whole block, 16 bytes per lane and coalesced.  The array is padded with zeros to a
-// multiple of 4 ints (the slot layout rounds every array up to 256 bytes).  The values were
-// written by other blocks: ld.cg.  Returns the total.
-template <int NT>
+// by the whole block.  The array is padded with zeros to a multiple of 4 ints (the slot layout rounds
+// every array up to 256 bytes).  The values were written by other blocks: ld.cg.  Returns the total.
+// One block runs this while the rest of the event's grid has retired, so what counts is its latency: a
+// tile of NT x kPer int4 is loaded with all loads in flight at once (kPer independent 16-byte loads per
+// thread, blocked layout; 1024 x 3 covers the 12 241 bin counters of the BASELINE geometry in one tile), scanned in registers + one block scan, and written back.
+template <int NT, int kPer>
 __device__ int block_scan_array4(int* a, int n) {
-  __shared__ int warp_tot[NT / 32];
   constexpr int W = NT / 32;
+  __shared__ int warp_tot[W];
+  __shared__ int s_carry;
   int4* a4 = reinterpret_cast<int4*>(a);
-  const int n4 = (n + 1 + 3) / 4, per = (n4 + W - 1) / W;
+  const int n4 = (n + 1 + 3) / 4;
   const int w = threadIdx.x >> 5, lane = (int)lane_id();
-  const int lo = min(n4, w * per), hi = min(n4, lo + per);
-  int s = 0;
-  for (int j = lo + lane; j < hi; j += 32) {
-    const int4 v = __ldcg(a4 + j);
-    s += (v.x + v.y) + (v.z + v.w);
-  }
-#pragma unroll
-  for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(kFull, s, d);
-  if (lane == 0) warp_tot[w] = s;
+  if (threadIdx.x == 0) s_carry = 0;
   __syncthreads();
-  int carry = 0, total = 0;
+  for (int t0 = 0; t0 < n4; t0 += NT * kPer) {
+    const int j0 = t0 + (int)threadIdx.x * kPer;
+    int4 v[kPer];
 #pragma unroll
-  for (int i = 0; i < W; ++i) {
-    const int v = warp_tot[i];
-    carry += (i < w) ? v : 0;
-    total += v;
+    for (int k = 0; k < kPer; ++k) v[k] = (j0 + k < n4) ? __ldcg(a4 + j0 + k) : make_int4(0, 0, 0, 0);
+    int mine = 0;
+#pragma unroll
+    for (int k = 0; k < kPer; ++k) mine += (v[k].x + v[k].y) + (v[k].z + v[k].w);
+    const int incl = warp_incl_scan(mine);
+    if (lane == 31) warp_tot[w] = incl;
+    __syncthreads();
+    int ex = s_carry + incl - mine, tile_total = 0;
+#pragma unroll 8
+    for (int i = 0; i < W; ++i) {
+      const int t = warp_tot[i];
+      ex += (i < w) ? t : 0;
+      tile_total += t;
+    }
+#pragma unroll
+    for (int k = 0; k < kPer; ++k) {
+      if (j0 + k < n4) a4[j0 + k] = make_int4(ex, ex + v[k].x, ex + v[k].x + v[k].y, ex + v[k].x + v[k].y + v[k].z);
+      ex += (v[k].x + v[k].y) + (v[k].z + v[k].w);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) s_carry += tile_total;
+    __syncthreads();
   }
-  for (int j0 = lo; j0 < hi; j0 += 32) {
-    const int j = j0 + lane;
-    int4 v = make_int4(0, 0, 0, 0);
-    if (j < hi) v = __ldcg(a4 + j);
-    const int t = (v.x + v.y) + (v.z + v.w);
-    const int incl = warp_incl_scan(t);
-    const int ex = carry + incl - t;
-    if (j < hi) a4[j] = make_int4(ex, ex + v.x, ex + v.x + v.y, ex + v.x + v.y + v.z);
-    carry += __shfl_sync(kFull, incl, 31);
-  }
-  __syncthreads();
-  return total;
+  return s_carry;
 }
 
 // Ticket: true in every thread of the block that finishes last among `n_blocks`.
@@ -215,7 +219,7 @@ __global__ void __launch_bounds__(256) k_reset(const __grid_constant__ Params P)
 // the hit's arrival rank in its bin, kept with its azimuth key so that the scatter needs no second
 // atomic.  If the arrays are mapped host memory (in.stage) this pass IS the host-to-device copy:
 // every array is read once over PCIe, coalesced, and written to the slot's staging area, which is
-// what the later kernels read.  The event's last block turns the counts into bin offsets.
+// what the later kernels read.  k_scan then turns the counts into bin offsets.
 __global__ void __launch_bounds__(256) k_bin_count(const __grid_constant__ Params P, const __grid_constant__ HitBatch B) {
   Slot S(P, blockIdx.y);
   const HitInput& in = B.ev[blockIdx.y];
@@ -244,21 +248,22 @@ __global__ void __launch_bounds__(256) k_bin_count(const __grid_constant__ Param
     kr[h] = make_int2(__float_as_int(k), (int)rank);
   }
   if (bad) atomicAdd(&S.hdr()->bad_hits, bad);
-  // the last block of the event turns the counts into bin offsets
-  if (!last_block_done(&S.hdr()->done[4], gridDim.x)) return;
-  int* start = reinterpret_cast<int*>(cnt);
-  // search space of the MD stage: sum over modules of (#lower hits) x (#upper hits)
-  unsigned long long c = 0;
-#pragma unroll 4
-  for (int m = threadIdx.x; m < nmod; m += 256)
-    c += (unsigned long long)__ldcg(start + m) * (unsigned long long)__ldcg(start + nmod + m);
-  c = warp_sum_ull(c);
-  if (lane_id() == 0 && c) atomicAdd(&S.hdr()->cand[LST_MD_], c);
-  __syncthreads();
-  const int total = block_scan_array4<256>(start, P.L.n_bins);
-  if (threadIdx.x == 0) {
-    S.hdr()->n_hits = total;
-    S.hdr()->n_lower = start[nmod];
+}
+
+// Counters to offsets, one block of 1024 threads per event: which = 0 the (side, module) bins of a0 (also
+// publishes the hit counts), which = 1 the MD -> quintuplet incidence counters of the cleaning stage.
+__global__ void __launch_bounds__(1024) k_scan(const __grid_constant__ Params P, int which) {
+  Slot S(P, blockIdx.y);
+  SlotHeader* H = S.hdr();
+  if (which == 0) {
+    int* start = reinterpret_cast<int*>(S.bin_start());
+    const int total = block_scan_array4<1024, 3>(start, P.L.n_bins);
+    if (threadIdx.x == 0) {
+      H->n_hits = total;
+      H->n_lower = start[P.L.n_modules];
+    }
+  } else {
+    block_scan_array4<1024, 3>(S.inc_start(), H->n[LST_MD_]);
   }
 }
 
@@ -341,6 +346,13 @@ __global__ void __launch_bounds__(256) k_bin_order(const __grid_constant__ Param
   if (p < nmod && start[p + 1] == start[p]) {  // no lower hits: an empty key range
     info[4 * p + 2] = __float_as_int(3.0e38f);
     info[4 * p + 3] = __float_as_int(-3.0e38f);
+  }
+  // search space of the MD stage: sum over modules of (#lower hits) x (#upper hits)
+  if (blockIdx.x * 256 < (unsigned)nmod) {
+    unsigned long long c = 0;
+    if (p < nmod) c = (unsigned long long)(start[p + 1] - start[p]) * (unsigned long long)(start[nmod + p + 1] - start[nmod + p]);
+    c = warp_sum_ull(c);
+    if (lane_id() == 0 && c) atomicAdd(&H->cand[LST_MD_], c);
   }
   __syncthreads();
   if (threadIdx.x < 24 && s_rng[threadIdx.x]) atomicMax(&H->r_min_inv[0][0] + threadIdx.x, s_rng[threadIdx.x]);
@@ -1169,16 +1181,13 @@ __global__ void __launch_bounds__(256) k_clean_prepare(const __grid_constant__ P
   }
 }
 
-// quintuplets per MD; the event's last block turns the counts into offsets
+// quintuplets per MD (k_scan turns the counts into offsets)
 __global__ void __launch_bounds__(256) k_clean_count(const __grid_constant__ Params P) {
   Slot S(P, blockIdx.y);
-  SlotHeader* H = S.hdr();
-  const int n5 = H->n[LST_T5_], nmd = H->n[LST_MD_];
+  const int n5 = S.hdr()->n[LST_T5_];
   int* cnt = S.inc_start();
   const int* md = S.t5_md();
   for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < 5 * n5; j += gridDim.x * blockDim.x) atomicAdd(cnt + md[j], 1);
-  if (!last_block_done(&H->done[5], gridDim.x)) return;
-  block_scan_array4<256>(cnt, nmd);
 }
 
 __global__ void __launch_bounds__(256) k_clean_fill(const __grid_constant__ Params P) {
@@ -1415,18 +1424,19 @@ int launch_bin(const Params& P, const HitBatch& src, const HitBatch& dev, int n_
     cudaEventRecord(stage->before, s);
     cudaStreamWaitEvent(stage->stream, stage->before, 0);
     k_bin_count<<<dim3(min((int)g.x, 8), nb), 256, 0, stage->stream>>>(P, src);
+    k_scan<<<dim3(1, nb), 1024, 0, stage->stream>>>(P, 0);
     cudaEventRecord(stage->after, stage->stream);
     cudaStreamWaitEvent(s, stage->after, 0);
   } else {
-    // grid-stride: fewer 'last block' tickets; + scan of the bin counts by the event's last block
-    k_bin_count<<<dim3(blocks_per_event((int)g.x, n_batch, 8), nb), 256, 0, s>>>(P, src);
+    k_bin_count<<<dim3(blocks_per_event((int)g.x, n_batch, 6), nb), 256, 0, s>>>(P, src);   // 40 registers: 6 blocks per SM
+    k_scan<<<dim3(1, nb), 1024, 0, s>>>(P, 0);
   }
   LST_EV(2);
   k_bin_scatter<<<g, 256, 0, s>>>(P, dev);
   LST_EV(3);
   k_bin_order<<<dim3((max(n_max, P.L.n_modules) + 255) / 256, nb), 256, 0, s>>>(P, dev);
   LST_EV(4);
-  return 4;
+  return 5;
 }
 
 int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEvent_t* ev) {
@@ -1458,12 +1468,13 @@ int launch_clean(const Params& P, int n_batch, cudaStream_t s, cudaEvent_t* ev) 
   k_clean_prepare<<<g, 256, 0, s>>>(P);
   LST_EV(1);
   k_clean_count<<<g, 256, 0, s>>>(P);
+  k_scan<<<dim3(1, (unsigned)n_batch), 1024, 0, s>>>(P, 1);
   LST_EV(2);
   k_clean_fill<<<g, 256, 0, s>>>(P);
   LST_EV(3);
   k_clean_mark<<<dim3(blocks_per_event((5 * P.L.cap_t5 + 255) / 256, n_batch, 8), (unsigned)n_batch), 256, 0, s>>>(P);
   LST_EV(4);
-  return 4;
+  return 5;
 }
 
 int launch_gather_hits(const Params& P, int kind, int n_max, int n_batch, cudaStream_t s) {
