@@ -296,10 +296,22 @@ def run_ours(args):
                   "to pinned host buffers); every step ends with all results on the host"}
 
     # ---- per-kernel times (CUDA events inside the library, timing mode), one 64-event batch ----
-    kernel_ms = per_kernel_times(lst, geom, mmap, d_in, local)
-    clean_ms = {k: kernel_ms.pop(k) for k in lst.KERNEL_NAMES[8:]}
+    kernel_ms, launches_per_step = per_kernel_times(lst, geom, mmap, d_in, local)
+    for k in lst.KERNEL_NAMES[8:]:
+        kernel_ms.pop(k)
+    with_clean_ms, _ = per_kernel_times(lst, geom, mmap, d_in, local, with_clean=True)
+    clean_ms = {k: with_clean_ms[k] for k in lst.KERNEL_NAMES[8:]}
     peaks = measured_peaks()
-    roof, per_stage = roofline(kernel_ms, n_hits, needed, evals, peaks)
+    lp = launches_per_step                      # per-launch quantities: one launch covers 64 / lp events
+    roof, per_stage = roofline(kernel_ms, n_hits / lp, [v / lp for v in needed], [v / lp for v in evals], peaks, N_EVENTS // lp)
+    spec_flops_step = sum(evals[i] * FLOPS_PER_CAND[i] for i in range(4))
+    alu_peak = 148 * 128 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    path = {"what": "whole path a0..a4 over the timed region: SPEC flops of all evaluated candidates and algorithmic bytes "
+                    "of all stages per step / ms_per_step",
+            "alu_tflops": spec_flops_step / (total_ms / args.steps * 1e-3) / 1e12, "alu_peak_tflops": alu_peak,
+            "alu_frac": spec_flops_step / (total_ms / args.steps * 1e-3) / 1e12 / alu_peak,
+            "hbm_gbs": sum(algorithmic_bytes(i, n_hits, needed) for i in range(5)) / (total_ms / args.steps * 1e-3) / 1e9,
+            "hbm_frac": sum(algorithmic_bytes(i, n_hits, needed) for i in range(5)) / (total_ms / args.steps * 1e-3) / 1e9 / peaks["hbm_gbs"]}
 
     # ---- the path followed by the optional duplicate-cleaning stage [D], same timing rules ----
     def step_device_clean():
@@ -313,7 +325,7 @@ def run_ours(args):
         ctx.sync_batch(s * per_stream, per_stream, st)
     kept = sum(ctx.stats(k)["n_kept"] for k in range(N_EVENTS))
     clean = {"events_per_s_with_clean": whole_job_events_per_s(world, args.steps, clean_total_ms),
-             "ms_per_step_with_clean": clean_total_ms / args.steps, "kernels_ms_one_stream": clean_ms,
+             "ms_per_step_with_clean": clean_total_ms / args.steps, "kernels_ms_per_launch": clean_ms,
              "t5_in": needed[3], "t5_kept": kept,
              "what": "a0..a4 + LST_CLEAN per step; `value` above is a0..a4 only (the BASELINE.json path)"}
 
@@ -325,9 +337,12 @@ def run_ours(args):
            "objects_per_step": dict(hits=n_hits, md=needed[0], ls=needed[1], t3=needed[2], t5=needed[3]),
            "candidates_per_step": dict(md=cands[0], ls=cands[1], t3=cands[2], t5=cands[3]),
            "evaluated_per_step": dict(md=evals[0], ls=evals[1], t3=evals[2], t5=evals[3]),
-           "stage_overlap": {"sum_of_stage_ms_one_stream": sum(v["ms"] for v in per_stage.values()),
+           "roofline_path": path,
+           "stage_overlap": {"sum_of_launch_ms_per_step": launches_per_step * sum(v["ms"] for v in per_stage.values()),
                              "ms_per_step_4_streams": total_ms / args.steps,
-                             "factor": sum(v["ms"] for v in per_stage.values()) / (total_ms / args.steps)},
+                             "factor": launches_per_step * sum(v["ms"] for v in per_stage.values()) / (total_ms / args.steps),
+                             "what": "sum over the step's launches of their CUDA-event durations / the step: > 1 = kernels of "
+                                     "different streams run side by side"},
            "duplicate_cleaning": clean,
            "rewalks_per_step": dict(md=rewalks[0], ls=rewalks[1], t3=rewalks[2], t5=rewalks[3]),
            "arena_mib": ctx.arena_bytes()[0] / 2 ** 20, "impl": "ours"}
@@ -342,34 +357,37 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
-def per_kernel_times(lst, geom, mmap, d_in, local, reps=5):
-    """Median per-kernel duration (ms) for ONE batch of all 64 events on one stream, from CUDA
-    events recorded by the library around every launch (lst_config.timing)."""
+def per_kernel_times(lst, geom, mmap, d_in, local, with_clean=False, reps=6):
+    """Average duration (ms) of ONE launch of every kernel in the configuration the timed region uses: 4 streams x
+    16-event launches running concurrently, CUDA events recorded by the library around every launch on the stream it
+    is launched on (lst_config.timing), L2 flushed before every step.  (Concurrent kernels share the SMs, so the
+    durations of one step add up to more than the step.)  The optional cleaning stage [D] is timed the same way."""
     import torch
     cfg = lst.default_config()
     cfg.device, cfg.n_slots, cfg.timing = local, N_EVENTS, 1
     ctx = lst.Lst.from_synth(geom, mmap, cfg)
-    st = torch.cuda.Stream()
+    streams = [torch.cuda.Stream() for _ in range(N_STREAMS)]
+    per = N_EVENTS // N_STREAMS
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     rows = []
-    for _ in range(reps + 2):
-        with torch.cuda.stream(st):
-            flush.zero_()
-        ctx.load_events(0, d_in, stream=st)
-        ctx.run_batch(0, N_EVENTS, st)
-        ctx.run_stage(0, N_EVENTS, lst.CLEAN, st)          # optional stage [D], reported beside the path, not in it
-        ctx.sync(0, st)
-        k_ms = np.zeros(12)
-        for k in range(0, N_EVENTS, 16):                  # a0 runs in launches of 16 events
-            ctx.sync(k, st)
-            k_ms[:4] += np.asarray(ctx.stats(k)["kernel_ms"][:4])
-        k_ms[4:] = np.asarray(ctx.stats(0)["kernel_ms"][4:12])
-        rows.append(k_ms)
+    for rep in range(reps + 2):
+        flush.zero_()
+        torch.cuda.synchronize()
+        for s, st in enumerate(streams):
+            ctx.load_events(s * per, d_in[s * per:(s + 1) * per], stream=st)
+            ctx.run_batch(s * per, per, st)
+            if with_clean:                                  # optional stage [D], reported beside the path, not in it
+                ctx.run_stage(s * per, per, lst.CLEAN, st)
+        for s, st in enumerate(streams):
+            ctx.sync_batch(s * per, per, st)
+            for k in range(s * per, (s + 1) * per, 16):    # one set of launches per 16 events; times kept on its first slot
+                if rep >= 2:
+                    rows.append(ctx.stats(k)["kernel_ms"][:12])
     ctx.close()
-    return dict(zip(lst.KERNEL_NAMES, np.median(np.asarray(rows[2:]), axis=0).tolist()))
+    return dict(zip(lst.KERNEL_NAMES, np.mean(np.asarray(rows), axis=0).tolist())), max(1, per // 16) * N_STREAMS
 
 
-def roofline(kernel_ms, n_hits, needed, cands, peaks):
+def roofline(kernel_ms, n_hits, needed, cands, peaks, events_per_launch):
     """Per-stage table and the `roofline` object for the dominant kernel. Two lower bounds per stage:
     HBM (algorithmic bytes / measured copy bandwidth) and ALU (SPEC flops of all candidates / fp32
     non-FMA peak = 148 SMs x 128 lanes x sm_max clock; FMA is excluded by the SPEC's arithmetic)."""
@@ -397,7 +415,8 @@ def roofline(kernel_ms, n_hits, needed, cands, peaks):
     else:
         roof = {"bound": "hbm", "achieved": b / (ms * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s"}
     roof.update({"frac": roof["achieved"] / roof["peak"], "traffic": None, "kernel": top, "kernel_ms": ms,
-                 "launch": f"one launch over all {N_EVENTS} events (grid.y = event)", "peak_source": peaks["source"],
+                 "launch": f"one launch = {events_per_launch} events (grid.y = event), timed inside the 4-stream step; "
+                           "flops / bytes are those of one launch", "peak_source": peaks["source"],
                  "hbm_view": {"achieved_gbs": b / (ms * 1e-3) / 1e9, "peak_gbs": peaks["hbm_gbs"],
                               "frac": b / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"], "algorithmic_bytes": int(b)}})
     return roof, per_stage

@@ -1402,8 +1402,13 @@ __global__ void __launch_bounds__(256) k_pack_values(const __grid_constant__ Par
 #define LST_EV(k) do { if (ev) cudaEventRecord(ev[k], s); } while (0)
 
 // blocks per event of a grid-stride / persistent kernel: enough to fill the machine across the batch
-static int blocks_per_event(int wanted, int n_batch, int resident_per_sm) {
-  const int per_event = max(8, 148 * resident_per_sm / n_batch);
+// The stage kernels are sized for HALF of what the machine holds: the kernels of two streams then run side by
+// side, each event gets fewer warps (a stage's throughput per event stops growing long before a 16-event batch
+// fills 148 SMs: ticket order and the ordered output bound it) and one stream's tail is filled by the other's body
+// (measured: 44.0k -> 47.4k events/s on the 4 x 16 workload; a third or a quarter is no better).
+constexpr int kGridShare = 2;
+static int blocks_per_event(int wanted, int n_batch, int resident_per_sm, int share = 1) {
+  const int per_event = max(8, 148 * resident_per_sm / (n_batch * share));
   return max(1, min(wanted, per_event));
 }
 
@@ -1444,16 +1449,16 @@ int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEv
   LST_EV(0);
   switch (stage) {
     case LST_MD_:
-      k_md<<<dim3(blocks_per_event((P.L.n_chunk[0] + kWarps - 1) / kWarps, n_batch, 6), nb), kWarps * 32, 0, s>>>(P);
+      k_md<<<dim3(blocks_per_event((P.L.n_chunk[0] + kWarps - 1) / kWarps, n_batch, 6, kGridShare), nb), kWarps * 32, 0, s>>>(P);
       break;
     case LST_SEG_:
-      k_seg<<<dim3(blocks_per_event((P.L.n_chunk[1] + kSegWarps - 1) / kSegWarps, n_batch, 6), nb), kSegWarps * 32, 0, s>>>(P);
+      k_seg<<<dim3(blocks_per_event((P.L.n_chunk[1] + kSegWarps - 1) / kSegWarps, n_batch, 6, kGridShare), nb), kSegWarps * 32, 0, s>>>(P);
       break;
     case LST_T3_:
-      k_t3<<<dim3(blocks_per_event((P.L.n_chunk[2] + kWarps - 1) / kWarps, n_batch, 6), nb), kWarps * 32, 0, s>>>(P);
+      k_t3<<<dim3(blocks_per_event((P.L.n_chunk[2] + kWarps - 1) / kWarps, n_batch, 6, kGridShare), nb), kWarps * 32, 0, s>>>(P);
       break;
     case LST_T5_:
-      k_t5<<<dim3(blocks_per_event((P.L.n_chunk[3] + kWarps - 1) / kWarps, n_batch, 4), nb), kWarps * 32, 0, s>>>(P);
+      k_t5<<<dim3(blocks_per_event((P.L.n_chunk[3] + kWarps - 1) / kWarps, n_batch, 4, kGridShare), nb), kWarps * 32, 0, s>>>(P);
       break;
     default:
       return 0;
