@@ -189,7 +189,7 @@ def run_ours(args):
     geom, mmap, events = make_events(rank_seed0(rank), N_EVENTS)
     per_stream = N_EVENTS // N_STREAMS
     cfg = lst.default_config()
-    cfg.device, cfg.n_slots = local, N_EVENTS
+    cfg.device, cfg.n_slots = local, 2 * N_EVENTS          # second half: the other buffer set of the end-to-end pipeline
     ctx = lst.Lst.from_synth(geom, mmap, cfg)
     streams = [torch.cuda.Stream(dev) for _ in range(N_STREAMS)]
     main = torch.cuda.current_stream(dev)
@@ -262,38 +262,60 @@ def run_ours(args):
     # ---- end to end: pinned host hits in, quintuplets out, through the C-ABI -------------
     h_in = [[torch.from_numpy(a).pin_memory() for a in (e.x, e.y, e.z, e.module, e.side)] for e in events]
     cap5 = max(s["needed"][3] for s in stats) * 2 + 1024
-    h_out = [(torch.empty((cap5, 10), dtype=torch.int32).pin_memory(), torch.empty((cap5, 5), dtype=torch.float32).pin_memory())
-             for _ in range(N_EVENTS)]
     np_in = [[t.numpy() for t in ev] for ev in h_in]
-    np_out = [(a.numpy(), b.numpy()) for a, b in h_out]
+    # Two buffer sets (slots, streams, pinned result buffers): step i + 1 is loaded and run while the results of
+    # step i travel back -- H2D and D2H share the PCIe link in opposite directions, as in a continuously fed pipeline.
+    sets = []
+    for p in range(2):
+        out = [(torch.empty((cap5, 10), dtype=torch.int32).pin_memory().numpy(), torch.empty((cap5, 5), dtype=torch.float32).pin_memory().numpy())
+               for _ in range(N_EVENTS)]
+        sets.append({"base": p * N_EVENTS, "streams": streams if p == 0 else [torch.cuda.Stream(dev) for _ in range(N_STREAMS)],
+                     "idx": [[out[k][0] for k in range(s * per_stream, (s + 1) * per_stream)] for s in range(N_STREAMS)],
+                     "val": [[out[k][1] for k in range(s * per_stream, (s + 1) * per_stream)] for s in range(N_STREAMS)],
+                     "counts": None})
 
-    idx_bufs = [[np_out[k][0] for k in range(s * per_stream, (s + 1) * per_stream)] for s in range(N_STREAMS)]
-    val_bufs = [[np_out[k][1] for k in range(s * per_stream, (s + 1) * per_stream)] for s in range(N_STREAMS)]
+    def e2e_launch(i):                              # H2D of the pinned hit SoA + a0..a4 of step i, all asynchronous
+        S = sets[i % 2]
+        for s, st in enumerate(S["streams"]):
+            ctx.load_events(S["base"] + s * per_stream, np_in[s * per_stream:(s + 1) * per_stream], stream=st)
+            ctx.run_batch(S["base"] + s * per_stream, per_stream, st)
 
-    def step_e2e():
-        for s, st in enumerate(streams):        # H2D of the pinned hit SoA + a0..a4, all asynchronous
-            ctx.load_events(s * per_stream, np_in[s * per_stream:(s + 1) * per_stream], stream=st)
-            ctx.run_batch(s * per_stream, per_stream, st)
-        for s, st in enumerate(streams):        # counters back (one sync per stream), then gathers + D2H enqueued
-            ctx.fetch_batch(s * per_stream, lst.T5, idx_bufs[s], val_bufs[s], stream=st, wait=False)
-        for st in streams:
-            st.synchronize()
+    def e2e_collect(i):                             # counters back (one sync per stream), then gathers + D2H enqueued
+        S = sets[i % 2]
+        S["counts"] = [ctx.fetch_batch(S["base"] + s * per_stream, lst.T5, S["idx"][s], S["val"][s], stream=st, wait=False)
+                       for s, st in enumerate(S["streams"])]
 
-    e2e_steps = max(3, min(args.steps, 10))
-    for _ in range(2):
-        step_e2e()
+    def e2e_run(n):
+        e2e_launch(0)
+        for i in range(1, n):
+            e2e_launch(i)
+            e2e_collect(i - 1)
+        e2e_collect(n - 1)
+        for S in sets:
+            for st in S["streams"]:
+                st.synchronize()
+
+    e2e_steps = max(4, min(args.steps, 10))
+    e2e_run(3)
     barrier()
     t0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        step_e2e()
+    e2e_run(e2e_steps)
     torch.cuda.synchronize(dev)
     e2e_s = max_over_ranks(time.perf_counter() - t0, dist, dev)
+    # the results are on the host: both buffer sets hold every event's quintuplets (counts and tuples of two events checked)
+    for S in sets:
+        got = [c for per in S["counts"] for c in per]
+        assert got == [st_["needed"][3] for st_ in stats], "end-to-end results incomplete"
+        for k in (0, N_EVENTS - 1):
+            ref = ctx.fetch_hit_indices(S["base"] + k, lst.T5, S["streams"][k // per_stream])
+            assert np.array_equal(S["idx"][k // per_stream][k % per_stream][:len(ref)], ref)
     h2d = sum(sum(t.numel() * t.element_size() for t in ev) for ev in h_in)
     d2h = needed[3] * (40 + 20) + N_EVENTS * HEADER_BYTES
     e2e = {"value": world * N_EVENTS * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
            "d2h_bytes_per_step": int(d2h), "steps": e2e_steps,
            "how": "per stream: lst_load_events(16 x pinned host SoA) + lst_run_batch + lst_fetch_batch(T5 hit indices + values "
-                  "to pinned host buffers); every step ends with all results on the host"}
+                  "to pinned host buffers); two buffer sets, step i + 1 is loaded and run while step i's results travel back; "
+                  "the timed region ends with every step's results on the host"}
 
     # ---- per-kernel times (CUDA events inside the library, timing mode), one 64-event batch ----
     kernel_ms, launches_per_step = per_kernel_times(lst, geom, mmap, d_in, local)
@@ -387,6 +409,22 @@ def per_kernel_times(lst, geom, mmap, d_in, local, with_clean=False, reps=6):
     return dict(zip(lst.KERNEL_NAMES, np.mean(np.asarray(rows), axis=0).tolist())), max(1, per // 16) * N_STREAMS
 
 
+def ncu_traffic_bytes(kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed `ncu --set full`
+    summary of the same launch configuration (profiles/r1d_ncu_full_summary.csv; 16-event launches), or None."""
+    import csv
+    path = os.path.join(ROOT, "profiles", "r1d_ncu_full_summary.csv")
+    name = {"seg": "k_seg", "md": "k_md", "t3": "k_t3", "t5": "k_t5"}.get(kernel, "k_" + kernel)
+    try:
+        rows = list(csv.reader(open(path)))
+        h = rows[0]
+        vals = [(float(r[h.index("dram__bytes_read.sum")]) + float(r[h.index("dram__bytes_write.sum")])) * 1e6
+                for r in rows[2:] if r[h.index("Kernel Name")].startswith(name + "(")]
+        return sum(vals) / len(vals) if vals else None
+    except Exception:
+        return None
+
+
 def roofline(kernel_ms, n_hits, needed, cands, peaks, events_per_launch):
     """Per-stage table and the `roofline` object for the dominant kernel. Two lower bounds per stage:
     HBM (algorithmic bytes / measured copy bandwidth) and ALU (SPEC flops of all candidates / fp32
@@ -414,7 +452,8 @@ def roofline(kernel_ms, n_hits, needed, cands, peaks, events_per_launch):
         roof = {"bound": "alu", "achieved": fl / (ms * 1e-3) / 1e12, "peak": alu_peak_tflops, "unit": "TFLOP/s"}
     else:
         roof = {"bound": "hbm", "achieved": b / (ms * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s"}
-    roof.update({"frac": roof["achieved"] / roof["peak"], "traffic": None, "kernel": top, "kernel_ms": ms,
+    roof.update({"frac": roof["achieved"] / roof["peak"], "traffic": ncu_traffic_bytes(top) if events_per_launch == 16 else None,
+                 "traffic_source": "profiles/r1d_ncu_full_summary.csv (bytes per 16-event launch)", "kernel": top, "kernel_ms": ms,
                  "launch": f"one launch = {events_per_launch} events (grid.y = event), timed inside the 4-stream step; "
                            "flops / bytes are those of one launch", "peak_source": peaks["source"],
                  "hbm_view": {"achieved_gbs": b / (ms * 1e-3) / 1e9, "peak_gbs": peaks["hbm_gbs"],
