@@ -422,3 +422,64 @@ def test_duplicate_cleaning_batch_empty_and_ties(lstmod, geom, mmap, o32, run_or
         assert set(map(tuple, hits[kept].tolist())) == set(map(tuple, ora.t5_hits()[keep_o].tolist()))
     assert c.stats(1)["n_kept"] == 0 and c.stats(2)["n_kept"] == 0
     c.close()
+
+
+def test_cuda_graph_capture_and_replay(ctx, o32, run_oracle, geom):
+    """include/lst.h: lst_load_event(s) (device input) + lst_run_batch only enqueue work, so the sequence can be captured
+    into a CUDA graph.  Capture once over fixed device buffers, then replay with two different events copied into
+    those buffers: each replay must give that event's oracle result."""
+    import torch
+    evs = [synth.generate_event(geom, 1, 90 + i, n_particles=1000) for i in range(2)]
+    n_max = max(e.n for e in evs)
+    bufs = [torch.zeros(n_max, dtype=dt, device="cuda") for dt in (torch.float32, torch.float32, torch.float32, torch.int32, torch.uint8)]
+    st = torch.cuda.Stream()
+
+    def fill(ev):          # pad with hits of an invalid side? no: the graph is captured for a fixed n, so replay events are cut to it
+        n = min(e.n for e in evs)
+        for b, a in zip(bufs, (ev.x, ev.y, ev.z, ev.module, ev.side)):
+            b[:n].copy_(torch.from_numpy(a[:n]))
+        return synth.Event(ev.x[:n], ev.y[:n], ev.z[:n], ev.module[:n], ev.side[:n], ev.truth[:n], {})
+
+    n = min(e.n for e in evs)
+    view = [b[:n] for b in bufs]
+    fill(evs[0])
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=st):
+        ctx.load_events(3, [view], stream=st)
+        ctx.run_batch(3, 1, st)
+    for ev in (evs[1], evs[0]):
+        cut = fill(ev)
+        torch.cuda.synchronize()
+        g.replay()
+        torch.cuda.synchronize()
+        ctx.sync(3, st)
+        parity.compare(parity.gpu_tables(ctx, 3, st), parity.oracle_tables(run_oracle(o32, cut)), "graph replay")
+
+
+def test_slots_driven_from_host_threads(ctx, o32, run_oracle, geom):
+    """include/lst.h: distinct slots may be driven from distinct host threads (each with its own stream)."""
+    import threading
+    import torch
+    evs = [synth.generate_event(geom, 1, 95 + i, n_particles=700) for i in range(4)]
+    pin = lambda a: torch.from_numpy(a).pin_memory().numpy()
+    out, err = {}, []
+
+    def work(k):
+        try:
+            st = torch.cuda.Stream()
+            e = evs[k]
+            for _ in range(3):
+                ctx.load_event(k, *(pin(a) for a in (e.x, e.y, e.z, e.module, e.side)), st)   # stage-in path (shared internal stream)
+                ctx.run(k, st)
+                ctx.sync(k, st)
+            out[k] = parity.gpu_tables(ctx, k, st)
+        except Exception as ex:       # noqa: BLE001
+            err.append(ex)
+
+    ts = [threading.Thread(target=work, args=(k,)) for k in range(4)]
+    [t.start() for t in ts]
+    [t.join() for t in ts]
+    assert not err, err
+    for k in range(4):
+        parity.compare(out[k], parity.oracle_tables(run_oracle(o32, evs[k])), f"thread {k}")
