@@ -369,9 +369,12 @@ def run_ours(args):
            "rewalks_per_step": dict(md=rewalks[0], ls=rewalks[1], t3=rewalks[2], t5=rewalks[3]),
            "arena_mib": ctx.arena_bytes()[0] / 2 ** 20, "impl": "ours"}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        v, dt = oracle_events_per_s(geom, mmap, events)
-        out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
-                               "sample": f"all {N_EVENTS} events of the workload once, single thread, {dt:.1f} s"}
+        n_pass, t_cpu = 0, 0.0
+        while t_cpu < 12.0 and n_pass < 8:          # a bounded sample: whole passes over the workload, >= 12 s of CPU work
+            t_cpu += oracle_events_per_s(geom, mmap, events)[1]
+            n_pass += 1
+        out["cpu_baseline"] = {"value": n_pass * N_EVENTS / t_cpu, "unit": UNIT, "cores": 1, "kind": "oracle",
+                               "sample": f"all {N_EVENTS} events of the workload x {n_pass} passes, single thread, {t_cpu:.1f} s"}
     ctx.close()
     if rank == 0:
         print(json.dumps(out))
