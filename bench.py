@@ -375,6 +375,20 @@ def run_ours(args):
             n_pass += 1
         out["cpu_baseline"] = {"value": n_pass * N_EVENTS / t_cpu, "unit": UNIT, "cores": 1, "kind": "oracle",
                                "sample": f"all {N_EVENTS} events of the workload x {n_pass} passes, single thread, {t_cpu:.1f} s"}
+        # the same oracle on every host core: events are independent (SURVEY 8(d) "all host cores" figure)
+        from concurrent.futures import ThreadPoolExecutor
+        from oracle import oracle as _oracle
+        o = _oracle.load("f32")
+        n_thr = os.cpu_count() or 1
+        def _one(ev):
+            o.run(geom.layer, mmap.row_offsets, mmap.targets, ev.x, ev.y, ev.z, ev.module, ev.side)   # ctypes releases the GIL
+        work = events * max(1, (2 * n_thr + N_EVENTS - 1) // N_EVENTS)
+        t0 = time.perf_counter()
+        with ThreadPoolExecutor(n_thr) as pool:
+            list(pool.map(_one, work))
+        dt = time.perf_counter() - t0
+        out["cpu_baseline"]["all_cores"] = {"value": len(work) / dt, "unit": UNIT, "cores": n_thr,
+                                            "sample": f"{len(work)} events on {n_thr} threads, {dt:.1f} s"}
     ctx.close()
     if rank == 0:
         print(json.dumps(out))
