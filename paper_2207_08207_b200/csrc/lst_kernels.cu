@@ -43,6 +43,17 @@ __device__ __forceinline__ unsigned lanemask_le() {
   return m;
 }
 
+// Order-preserving map of a float's bit pattern to an unsigned integer (and back): (key, original index) then
+// compares as ONE 64-bit integer in the ranking loop of k_bin_order.  Keys are finite or the 3e38 sentinel; -0 sorts
+// just before +0, which only permutes hits whose azimuths are equal.
+__device__ __forceinline__ unsigned sortable_of(float f) {
+  const unsigned b = __float_as_uint(f);
+  return b ^ ((unsigned)((int)b >> 31) | 0x80000000u);
+}
+__device__ __forceinline__ float float_of_sortable(unsigned u) {
+  return __uint_as_float(u ^ ((u & 0x80000000u) ? 0x80000000u : 0xffffffffu));
+}
+
 __device__ __forceinline__ int warp_incl_scan(int v) {
 #pragma unroll
   for (int d = 1; d < 32; d <<= 1) {
@@ -305,7 +316,7 @@ __global__ void __launch_bounds__(256) k_bin_scatter(const __grid_constant__ Par
     const int b = (int)sd * nmod + m;
     const int2 v = kr[h];
     const unsigned pos = start[b] + (unsigned)v.y;
-    tki[pos] = make_int2(v.x, h);
+    tki[pos] = make_int2(h, (int)sortable_of(__int_as_float(v.x)));   // little endian: (index, key) = key in the high word
     tbin[pos] = b;
   }
 }
@@ -330,14 +341,12 @@ __global__ void __launch_bounds__(256) k_bin_order(const __grid_constant__ Param
   if (p < nh) {
     const int b = S.tmp_bin()[p];
     const int s = (int)start[b], e = (int)start[b + 1];
-    const int2 me = tki[p];
+    const unsigned long long* tk = reinterpret_cast<const unsigned long long*>(tki);
+    const unsigned long long mine = tk[p];                   // (sortable key << 32) | original index
+    const int2 me = make_int2(__float_as_int(float_of_sortable((unsigned)(mine >> 32))), (int)(unsigned)mine);
     const float key = __int_as_float(me.x);
     int rank = 0;
-    for (int j = s; j < e; ++j) {
-      const int2 o = tki[j];
-      const float kj = __int_as_float(o.x);
-      rank += (kj < key) || (kj == key && o.y < me.y);
-    }
+    for (int j = s; j < e; ++j) rank += tk[j] < mine;
     const int side = b >= nmod, m = b - side * nmod;
     const float x = in.x[me.y], y = in.y[me.y], z = in.z[me.y];
     const float r = sqrtf(x * x + y * y);
