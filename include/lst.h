@@ -126,8 +126,11 @@ LST_API int lst_default_config(lst_config* cfg);
 
 /* Hit SoA of one event (BASELINE.json configs[1]: "fp32 SoA (x, y, z, module id, sensor side)").
  * All five arrays are HOST pointers (on_device = 0) or all five DEVICE pointers (on_device = 1).
- * Pinned (page-locked) host arrays are read by the binning kernel itself over PCIe, once and
- * coalesced -- no separate copy is enqueued; pageable host arrays go through cudaMemcpyAsync.  They are borrowed until the stream has passed
+ * Fastest host form ("packed"): the five arrays back to back in ONE pinned block, each starting on a
+ * 256-byte boundary (y = x + A, z = x + 2A, module = x + 3A, side = x + 4A as byte addresses, A = 4 n
+ * rounded up to 256): the event travels as one copy-engine transfer at link speed.  Other pinned
+ * (page-locked) host arrays are read by the binning kernel itself over PCIe, once and coalesced;
+ * pageable host arrays go through five cudaMemcpyAsync.  They are borrowed until the stream has passed
  * the work enqueued by lst_load_event.  side: 0 = lower sensor (the anchor), 1 = upper. */
 typedef struct {
   int32_t n;
@@ -267,9 +270,10 @@ LST_API int lst_fetch_values(lst_ctx* ctx, int slot, int kind, float* out, int64
  * (layout as lst_fetch_values) to val_out[b].  idx_out / val_out may be NULL, and so may single
  * entries (nothing is copied for them).  cap_objects[b] = rows available in slot b's buffers;
  * counts[b] (may be NULL) receives the object count.  One gather launch per table for the whole
- * batch, then one cudaMemcpyAsync per buffer (pinned buffers make them asynchronous).  wait != 0:
- * returns after the copies have completed; wait == 0: the work is only enqueued and the buffers are
- * complete once `cuda_stream` has been synchronised by the caller.  Errors: LST_ERR_STATE (a slot not run), LST_ERR_OVERFLOW,
+ * batch.  Pinned (page-locked) host buffers are written by ONE kernel per 16 slots directly over PCIe
+ * (coalesced, each byte once); pageable ones through the slot's scratch area and one cudaMemcpyAsync
+ * per buffer.  wait != 0: returns after the copies have completed; wait == 0: the work is only
+ * enqueued and the buffers are complete once `cuda_stream` has been synchronised by the caller.  Errors: LST_ERR_STATE (a slot not run), LST_ERR_OVERFLOW,
  * LST_ERR_ARG (a buffer too small: nothing is copied), LST_ERR_CUDA. */
 LST_API int lst_fetch_batch(lst_ctx* ctx, int first_slot, int n_slots, int kind, int32_t* const* idx_out,
                             float* const* val_out, const int64_t* cap_objects, int32_t* counts, int wait,

@@ -338,8 +338,23 @@ int lst_load_events(lst_ctx* c, int first, int n_ev, const lst_hits* hits, void*
       HitInput staged{reinterpret_cast<const float*>(base + L.in_x), reinterpret_cast<const float*>(base + L.in_y),
                       reinterpret_cast<const float*>(base + L.in_z), reinterpret_cast<const int*>(base + L.in_module),
                       reinterpret_cast<const unsigned char*>(base + L.in_side), h->n, 0};
+      // "packed" host layout: the five arrays back to back in ONE block, each starting on a 256-byte boundary
+      // (x at p, y at p + A, z at p + 2 A, module at p + 3 A, side at p + 4 A, A = 4 n rounded up to 256)
+      const size_t A = align_up(4 * (size_t)h->n, 256);
+      const char* px = reinterpret_cast<const char*>(h->x);
+      const bool packed = !h->on_device && h->n > 0 && reinterpret_cast<const char*>(h->y) == px + A &&
+                          reinterpret_cast<const char*>(h->z) == px + 2 * A && reinterpret_cast<const char*>(h->module) == px + 3 * A &&
+                          reinterpret_cast<const char*>(h->side) == px + 4 * A;
       if (h->on_device || h->n == 0) {
         src.ev[b] = dev.ev[b] = in;
+      } else if (packed) {
+        // one copy-engine transfer of the whole event (1.3 MB at PU200 density runs at link speed, five 300 kB ones do
+        // not), into the same layout in the slot's staging area; no SM involved, full duplex with the result copies
+        char* d = base + L.in_x;
+        LST_CUDA(c, cudaMemcpyAsync(d, px, 4 * A + (size_t)h->n, cudaMemcpyHostToDevice, s));
+        src.ev[b] = dev.ev[b] = HitInput{reinterpret_cast<const float*>(d), reinterpret_cast<const float*>(d + A),
+                                         reinterpret_cast<const float*>(d + 2 * A), reinterpret_cast<const int*>(d + 3 * A),
+                                         reinterpret_cast<const unsigned char*>(d + 4 * A), h->n, 0};
       } else if (mapped_host(in)) {
         // pinned host arrays: k_bin_count reads them over PCIe (one coalesced pass) and fills the staging area
         in.stage = 1;
@@ -588,9 +603,38 @@ int lst_fetch_batch(lst_ctx* c, int first, int n, int kind, int32_t* const* idx_
   const Layout& L = c->P.L;
   Params P = c->P;
   P.first_slot = first;
-  // Copies go through the copy engine (they overlap the stage kernels of the other streams without taking
-  // SM slots).  The slot's scratch area holds one gathered table at a time: stream order keeps the second
-  // gather behind the first copy.
+  // Pinned (mapped) host buffers are written by ONE kernel per 16 slots (k_fetch_direct); what is left (pageable
+  // buffers) goes through the slot's scratch area and the copy engine, below.
+  std::vector<int32_t*> idx_dma(idx_out ? idx_out : nullptr, idx_out ? idx_out + n : nullptr);
+  std::vector<float*> val_dma(val_out ? val_out : nullptr, val_out ? val_out + n : nullptr);
+  for (int b0 = 0; b0 < n && n_max > 0; b0 += kMaxBatch) {
+    const int nb = n - b0 < kMaxBatch ? n - b0 : kMaxBatch;
+    OutTable T;
+    std::memset(&T, 0, sizeof(T));
+    bool any = false;
+    for (int b = 0; b < nb; ++b) {
+      if (c->slots[first + b0 + b].hdr->n[kind] == 0) continue;
+      if (idx_out && idx_out[b0 + b])
+        if (void* a = const_cast<void*>(mapped_alias(idx_out[b0 + b]))) { T.idx[b] = static_cast<int*>(a); idx_dma[b0 + b] = nullptr; any = true; }
+      if (val_out && val_out[b0 + b])
+        if (void* a = const_cast<void*>(mapped_alias(val_out[b0 + b]))) { T.val[b] = static_cast<float*>(a); val_dma[b0 + b] = nullptr; any = true; }
+    }
+    if (!any) continue;
+    Params Pd = c->P;
+    Pd.first_slot = first + b0;
+    c->launches += launch_fetch_direct(Pd, T, kind, nb, st);
+    LST_CUDA(c, cudaGetLastError());
+  }
+  bool idx_left = false, val_left = false;
+  for (int b = 0; b < n; ++b) {
+    const bool has = c->slots[first + b].hdr->n[kind] > 0;
+    idx_left = idx_left || (has && idx_out && idx_dma[b]);
+    val_left = val_left || (has && val_out && val_dma[b]);
+  }
+  idx_out = idx_left ? idx_dma.data() : nullptr;
+  val_out = val_left ? val_dma.data() : nullptr;
+  // The slot's scratch area holds one gathered table at a time: stream order keeps the second gather behind the
+  // first copy.
   if (idx_out && n_max > 0) {
     c->launches += launch_gather_hits(P, kind, n_max, n, st);
     LST_CUDA(c, cudaGetLastError());

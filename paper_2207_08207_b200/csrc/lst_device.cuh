@@ -175,6 +175,13 @@ int launch_bin(const Params& P, const HitBatch& src, const HitBatch& dev, int n_
 int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEvent_t* ev);          // 1 kernel
 // Duplicate cleaning [D]: 5 kernels (prepare, count, scan, fill, mark); ev[0..4] around the four steps.
 int launch_clean(const Params& P, int n_batch, cudaStream_t s, cudaEvent_t* ev);
+// Per slot of a batch: device-visible aliases of pinned host buffers for the hit-index tuples / the float payload
+// (null = that table is not wanted there, or goes through the scratch area and the copy engine).
+struct OutTable {
+  int* idx[kMaxBatch];
+  float* val[kMaxBatch];
+};
+int launch_fetch_direct(const Params& P, const OutTable& T, int kind, int n_batch, cudaStream_t s);
 int launch_gather_hits(const Params& P, int kind, int n_max, int n_batch, cudaStream_t s);   // slots first_slot .. + n_batch - 1
 int launch_pack_values(const Params& P, int kind, int n_max, int n_batch, cudaStream_t s);
 

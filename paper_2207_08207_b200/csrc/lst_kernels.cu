@@ -1432,6 +1432,43 @@ __global__ void __launch_bounds__(256) k_pack_values(const __grid_constant__ Par
   }
 }
 
+// Both tables of every slot of a batch straight into pinned (mapped) host buffers: the kernel IS the device-to-host
+// copy -- each byte crosses PCIe once, in coalesced 128 / 256-byte writes -- and replaces two copy-engine calls per
+// slot by ONE launch per batch.  Small grid: the kernel is bound by the link, not by the SMs.
+__global__ void __launch_bounds__(256) k_fetch_direct(const __grid_constant__ Params P, const __grid_constant__ OutTable T, int kind) {
+  Slot S(P, blockIdx.y);
+  const int n = S.hdr()->n[kind];
+  const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (size_t)gridDim.x * blockDim.x;
+  if (int2* out = reinterpret_cast<int2*>(T.idx[blockIdx.y])) {
+    const int w = kind == LST_MD_ ? 1 : kind == LST_SEG_ ? 2 : kind == LST_T3_ ? 3 : 5;
+    const size_t m = (size_t)n * w;
+    const int2* mh = S.md_hits();
+    for (size_t j = tid; j < m; j += nth) {
+      int md;
+      if (kind == LST_MD_) md = (int)j;
+      else if (kind == LST_SEG_) md = reinterpret_cast<const int*>(S.seg_md())[j];
+      else if (kind == LST_T3_) { const size_t i = j / 3; md = reinterpret_cast<const int*>(S.t3_pack())[4 * i + (j - 3 * i)]; }
+      else md = S.t5_md()[j];
+      out[j] = mh[md];
+    }
+  }
+  if (float* out = T.val[blockIdx.y]) {
+    if (kind == LST_MD_) {
+      for (size_t i = tid; i < (size_t)n; i += nth) {
+        const float2 o = S.md_out()[i];
+        reinterpret_cast<float4*>(out)[i] = make_float4(S.md_aux()[i].y, o.x, o.y, S.md_anchor()[i].w);
+      }
+    } else if (kind == LST_T3_) {
+      for (size_t i = tid; i < (size_t)n; i += nth)
+        reinterpret_cast<float2*>(out)[i] = make_float2(__int_as_float(S.t3_pack()[i].w), S.t3_chi2()[i]);
+    } else {   // LS [n][4] and T5 [n][5] are stored in the output layout: a flat copy
+      const float* src = kind == LST_SEG_ ? reinterpret_cast<const float*>(S.seg_f()) : S.t5_f();
+      const size_t m = (size_t)n * (kind == LST_SEG_ ? 4 : 5);
+      for (size_t i = tid; i < m; i += nth) out[i] = src[i];
+    }
+  }
+}
+
 // ------------------------------------------------------------------------------------------
 // launchers
 // ------------------------------------------------------------------------------------------
@@ -1516,6 +1553,11 @@ int launch_clean(const Params& P, int n_batch, cudaStream_t s, cudaEvent_t* ev) 
   k_clean_mark<<<dim3(blocks_per_event((5 * P.L.cap_t5 + 255) / 256, n_batch, 8), (unsigned)n_batch), 256, 0, s>>>(P);
   LST_EV(4);
   return 5;
+}
+
+int launch_fetch_direct(const Params& P, const OutTable& T, int kind, int n_batch, cudaStream_t s) {
+  k_fetch_direct<<<dim3(8, (unsigned)n_batch), 256, 0, s>>>(P, T, kind);
+  return 1;
 }
 
 int launch_gather_hits(const Params& P, int kind, int n_max, int n_batch, cudaStream_t s) {

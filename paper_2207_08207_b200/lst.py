@@ -196,6 +196,21 @@ def _stream(s) -> int:
     return int(s)
 
 
+def packed_event_buffers(n: int):
+    """Five numpy arrays (x, y, z, module, side) of length ``n`` inside ONE pinned host block in the "packed" layout of
+    include/lst.h (each array on a 256-byte boundary, back to back): an event loaded from them travels as a single
+    copy-engine transfer.  Fill them in place.  (torch is used for the pinned allocation only.)"""
+    import torch
+    a = (4 * n + 255) // 256 * 256
+    block = torch.empty(4 * a + max(n, 1), dtype=torch.uint8).pin_memory()
+    raw = block.numpy()
+    out = (raw[0:4 * n].view(np.float32), raw[a:a + 4 * n].view(np.float32), raw[2 * a:2 * a + 4 * n].view(np.float32),
+           raw[3 * a:3 * a + 4 * n].view(np.int32), raw[4 * a:4 * a + n])
+    for v in out:
+        v.flags.writeable = True
+    return out + (block,)          # keep the last element alive as long as the views are used
+
+
 class Lst:
     """One library context: geometry + module map + arena of event slots (lst_create)."""
 

@@ -223,7 +223,7 @@ def test_search_windows_never_change_the_result(lstmod, geom, mmap, o32, run_ora
     c.close()
 
 
-def test_fetch_batch_equals_per_slot_fetch(ctx, geom):
+def test_fetch_batch_equals_per_slot_fetch(ctx, lstmod, geom):
     """lst_sync_batch + lst_fetch_batch (one call per batch, asynchronous copies into pinned host
     buffers) return exactly what the per-slot lst_sync + lst_fetch_* calls return, for every class."""
     import torch
@@ -238,6 +238,16 @@ def test_fetch_batch_equals_per_slot_fetch(ctx, geom):
     assert ctx.sync_batch(2, len(evs), stream) == 0
     pageable = parity.run_gpu(ctx, evs[1], slot=6, stream=stream)
     pinned = parity.gpu_tables(ctx, 3, stream)
+    # "packed" host layout (one pinned block, arrays on 256-byte boundaries): one copy-engine transfer per event
+    pk = lstmod.packed_event_buffers(evs[1].n)
+    for dst, src in zip(pk[:5], (evs[1].x, evs[1].y, evs[1].z, evs[1].module, evs[1].side)):
+        dst[:] = src
+    ctx.load_event(7, *pk[:5], stream)
+    ctx.run(7, stream)
+    ctx.sync(7, stream)
+    packed = parity.gpu_tables(ctx, 7, stream)
+    for kind in range(4):
+        assert np.array_equal(packed[kind][0], pinned[kind][0]) and np.array_equal(packed[kind][1], pinned[kind][1], equal_nan=True)
     for kind in range(4):
         assert np.array_equal(pageable[kind][0], pinned[kind][0]) and np.array_equal(pageable[kind][1], pinned[kind][1], equal_nan=True)
     for kind in range(4):
