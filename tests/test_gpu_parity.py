@@ -493,3 +493,36 @@ def test_slots_driven_from_host_threads(ctx, o32, run_oracle, geom):
     assert not err, err
     for k in range(4):
         parity.compare(out[k], parity.oracle_tables(run_oracle(o32, evs[k])), f"thread {k}")
+
+
+def test_fuzz_small_events(ctx, o32, run_oracle, geom):
+    """Seeded random small events of adversarial structure (noise only; all hits in a handful of modules; duplicated
+    hits; coordinates scaled far off the detector; mixtures): sets, counts and floats equal the oracle's every time."""
+    rng = np.random.default_rng(2024)
+    n_obj = np.zeros(4, np.int64)
+    for trial in range(24):
+        kind = trial % 6
+        base = synth.generate_event(geom, 1, 700 + trial, n_particles=12 if kind == 3 else int(rng.integers(20, 400)))
+        x, y, z, mod, side = (a.copy() for a in (base.x, base.y, base.z, base.module, base.side))
+        if kind == 1:       # noise only: positions scrambled among the hits of each (module, side) -- keeps them on the sensors
+            p = rng.permutation(len(x)); order = np.lexsort((p, side, mod)); src = np.lexsort((np.arange(len(x)), side, mod))
+            x[src], y[src], z[src] = x[order], y[order], z[order]
+        elif kind == 2:     # everything folded into 12 modules of consecutive layers (heavy bins, long lists)
+            keep = np.isin(mod, np.concatenate([np.arange(0, 3), 408 + np.arange(0, 3), 1008 + np.arange(0, 3), 1848 + np.arange(0, 3)]))
+            if keep.sum() < 4:
+                keep[:] = True
+            x, y, z, mod, side = x[keep], y[keep], z[keep], mod[keep], side[keep]
+        elif kind == 3:     # every hit twice (equal keys: ties by original index; a T5 becomes 2^10 of them)
+            x, y, z, mod, side = (np.tile(a, 2) for a in (x, y, z, mod, side))
+        elif kind == 4:     # a tenth of the hits far away / tiny / negative radius direction
+            m = rng.random(len(x)) < 0.1
+            x[m] *= rng.choice([1e-6, 1e4, -1.0], m.sum()).astype(np.float32)
+            z[m] *= np.float32(50.0)
+        elif kind == 5:     # sides swapped for a third of the modules
+            m = (mod % 3) == 0
+            side[m] = 1 - side[m]
+        ev = synth.Event(x.astype(np.float32), y.astype(np.float32), z.astype(np.float32), mod.astype(np.int32), side.astype(np.uint8),
+                         np.full(len(x), -1, np.int32), {})
+        _, st = check_event(ctx, o32, run_oracle, ev, slot=trial % 8, label=f"fuzz{trial}/kind{kind}")
+        n_obj += np.asarray(st["needed"])
+    assert n_obj[0] > 5000 and n_obj[3] > 50, n_obj
