@@ -524,7 +524,7 @@ __device__ __forceinline__ int md_walk(const Params& P, const Slot& S, MdWarp& s
   return running;
 }
 
-__global__ void __launch_bounds__(kWarps * 32, 5) k_md(const __grid_constant__ Params P) {
+__global__ void __launch_bounds__(kWarps * 32, 6) k_md(const __grid_constant__ Params P) {
   __shared__ MdWarp shw[kWarps];
   __shared__ float s_w[6], s_rmaxU[6];
   Slot S(P, blockIdx.y);
@@ -789,7 +789,7 @@ __device__ __forceinline__ int seg_walk(const Params& P, const Slot& S, SegWarp&
   return running;
 }
 
-__global__ void __launch_bounds__(kSegWarps * 32, 6) k_seg(const __grid_constant__ Params P) {
+__global__ void __launch_bounds__(kSegWarps * 32, 7) k_seg(const __grid_constant__ Params P) {
   __shared__ SegWarp shw[kSegWarps];
   __shared__ float s_rMinO[6], s_rMaxO[6];
   Slot S(P, blockIdx.y);
@@ -933,7 +933,7 @@ __device__ __forceinline__ int t3_walk(const Params& P, const Slot& S, T3Warp& s
   return running;
 }
 
-__global__ void __launch_bounds__(kWarps * 32, 5) k_t3(const __grid_constant__ Params P) {
+__global__ void __launch_bounds__(kWarps * 32, 6) k_t3(const __grid_constant__ Params P) {
   __shared__ T3Warp shw[kWarps];
   Slot S(P, blockIdx.y);
   SlotHeader* H = S.hdr();
