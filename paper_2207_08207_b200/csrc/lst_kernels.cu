@@ -758,23 +758,45 @@ __device__ __forceinline__ int seg_walk(const Params& P, const Slot& S, SegWarp&
       __syncwarp();
     }
   };
-  // A: all (inner MD, connected module) pairs of the chunk
-  for (int tb = 0; tb < nPairs; tb += 32) {
+  // A: all (inner MD, connected module) pairs of the chunk.  The loads of tile t + 1 (target, azimuth offset, the
+  // target's module record: two dependent round trips) are issued before tile t is processed, so they travel while
+  // the queues of tile t are drained.
+  struct ATile {
+    int ol, tgt;
+    float dphi;
+    int4 info;
+    bool valid;
+  };
+  auto loadA = [&](int tb) {
+    ATile t;
     const int rk = tile_owner(nt, off, tb);
     const int q = tb + lane;
-    const int ol = (q < nPairs) ? sh.tab[rk] : 0;
-    const int e = __shfl_sync(kFull, row0, ol) + (q - __shfl_sync(kFull, off, ol));
+    t.valid = q < nPairs;
+    t.ol = t.valid ? sh.tab[rk] : 0;
+    const int e = __shfl_sync(kFull, row0, t.ol) + (q - __shfl_sync(kFull, off, t.ol));
+    t.tgt = 0;
+    t.dphi = 0.0f;
+    t.info = make_int4(0, 0, 0, 0);
+    if (t.valid) {
+      t.tgt = P.map_targets[e];
+      t.dphi = P.map_dphi[e];
+      t.info = mod_info[t.tgt];
+    }
+    return t;
+  };
+  ATile cur = loadA(0);
+  for (int tb = 0; tb < nPairs; tb += 32) {
+    ATile nxt = cur;
+    if (tb + 32 < nPairs) nxt = loadA(tb + 32);
+    const int ol = cur.ol, tgt = cur.tgt;
     bool keep = false;
-    int tgt = 0;
     float c0 = 0.0f;
-    if (q < nPairs) {
-      tgt = P.map_targets[e];
-      const float dphi = P.map_dphi[e];   // issued with the target load, not behind the test below
-      const int4 info = mod_info[tgt];
+    if (cur.valid) {
+      const int4 info = cur.info;
       if (!DIRECT) space += (unsigned long long)(info.y - info.x);
       const float dlo = sh.dlo[ol], dhi = sh.dhi[ol];
       if (info.y > info.x && dlo <= dhi) {
-        c0 = sh.key[ol] + dphi;
+        c0 = sh.key[ol] + cur.dphi;
         keep = !(fabsf(c0) + fmaxf(fabsf(dlo), fabsf(dhi)) < 3.0f) ||
                (c0 + dhi >= __int_as_float(info.z) && c0 + dlo <= __int_as_float(info.w));
       }
@@ -783,6 +805,7 @@ __device__ __forceinline__ int seg_walk(const Params& P, const Slot& S, SegWarp&
     if (keep) sh.pq[(pt + __popc(bal & lanemask_lt())) & (kQueue - 1)] = make_int2((ol << 26) | tgt, __float_as_int(c0));
     pt += __popc(bal);
     drainB(false);
+    cur = nxt;
   }
   drainB(true);
   drainC(true);
