@@ -428,7 +428,7 @@ def per_kernel_times(lst, geom, mmap, d_in, local, with_clean=False, reps=6):
 
 def ncu_traffic_bytes(kernel: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed `ncu --set full`
-    summary of the same launch configuration (profiles/r1e_ncu_full_summary.csv; 16-event launches), or None."""
+    summary of the same launch configuration (profiles/r1f_ncu_full_summary.csv; 16-event launches), or None."""
     import csv
     path = os.path.join(ROOT, "profiles", "r1d_ncu_full_summary.csv")
     name = {"seg": "k_seg", "md": "k_md", "t3": "k_t3", "t5": "k_t5"}.get(kernel, "k_" + kernel)
@@ -470,7 +470,7 @@ def roofline(kernel_ms, n_hits, needed, cands, peaks, events_per_launch):
     else:
         roof = {"bound": "hbm", "achieved": b / (ms * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s"}
     roof.update({"frac": roof["achieved"] / roof["peak"], "traffic": ncu_traffic_bytes(top) if events_per_launch == 16 else None,
-                 "traffic_source": "profiles/r1e_ncu_full_summary.csv (bytes per 16-event launch)", "kernel": top, "kernel_ms": ms,
+                 "traffic_source": "profiles/r1f_ncu_full_summary.csv (bytes per 16-event launch)", "kernel": top, "kernel_ms": ms,
                  "launch": f"one launch = {events_per_launch} events (grid.y = event), timed inside the 4-stream step; "
                            "flops / bytes are those of one launch", "peak_source": peaks["source"],
                  "hbm_view": {"achieved_gbs": b / (ms * 1e-3) / 1e9, "peak_gbs": peaks["hbm_gbs"],
