@@ -430,7 +430,7 @@ def ncu_traffic_bytes(kernel: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed `ncu --set full`
     summary of the same launch configuration (profiles/r1f_ncu_full_summary.csv; 16-event launches), or None."""
     import csv
-    path = os.path.join(ROOT, "profiles", "r1d_ncu_full_summary.csv")
+    path = os.path.join(ROOT, "profiles", "r1f_ncu_full_summary.csv")
     name = {"seg": "k_seg", "md": "k_md", "t3": "k_t3", "t5": "k_t5"}.get(kernel, "k_" + kernel)
     try:
         rows = list(csv.reader(open(path)))
