@@ -16,7 +16,12 @@
 //     queue and the expensive selection runs on full tiles of survivors;
 //   * what passes is kept, in (owner, candidate) order, in a shared-memory stash until a
 //     decoupled look-back over the chunk totals has told the warp where its objects start;
-//     objects are then written once, contiguous per owner (CSR), in a deterministic order.
+//     objects are then written once, contiguous per owner (CSR), in a deterministic order.  The
+//     emit is DEFERRED by one chunk: the total is published right after the walk, the warp walks
+//     its next chunk, and only then resolves the base of the previous one (second stash), so the
+//     ordered-output wait has a whole walk of slack (two walks of slack, or an extra non-blocking
+//     attempt right after the walk, measured slower: the inclusive prefixes come later / cost a
+//     round trip);
 // No global atomic is issued per candidate or per object, and no block-wide barrier is used:
 // warps are independent, compaction is ballot + popc.
 //
