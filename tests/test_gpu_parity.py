@@ -526,3 +526,31 @@ def test_fuzz_small_events(ctx, o32, run_oracle, geom):
         _, st = check_event(ctx, o32, run_oracle, ev, slot=trial % 8, label=f"fuzz{trial}/kind{kind}")
         n_obj += np.asarray(st["needed"])
     assert n_obj[0] > 5000 and n_obj[3] > 50, n_obj
+
+
+def test_parity_with_non_default_cut_constants(lstmod, geom, mmap, o32):
+    """Every threshold comes from lst_config, none is baked into a kernel: with tightened / loosened constants on BOTH
+    sides (same fp32 values) the object sets and floats still agree, and differ from the default result."""
+    changes = dict(z_lum=10.0, seg_cos_eps=0.999998, seg_sin_eps=0.0015, t3_kappa_max=0.012, t5_dkappa_max=0.0004,
+                   t5_chi2xy_max=60.0, t5_kappa_max=0.0125)
+    arrays = dict(md_dz_res=0.8, seg_z0_max=0.7, t3_chi2rz_max=0.5, t5_chi2rz_max=1.5, md_eps=0.9)
+    cfg = lstmod.default_config()
+    cfg.n_slots = 1
+    ocfg = o32.default_config()
+    for k, v in changes.items():
+        setattr(cfg, k, v)
+        setattr(ocfg, k, v)
+    for k, f in arrays.items():
+        a, b = getattr(cfg, k), getattr(ocfg, k)
+        for i in range(len(a)):
+            a[i] = np.float32(a[i] * f)
+            b[i] = a[i]
+    c = lstmod.Lst.from_synth(geom, mmap, cfg)
+    ev = synth.generate_event(geom, 1, 55, n_particles=1500)
+    gpu = parity.run_gpu(c, ev)
+    ora = o32.run(geom.layer, mmap.row_offsets, mmap.targets, ev.x, ev.y, ev.z, ev.module, ev.side, cfg=ocfg)
+    parity.compare(gpu, parity.oracle_tables(ora), "custom cuts")
+    assert c.stats(0)["needed"] == ora.counts
+    default = o32.run(geom.layer, mmap.row_offsets, mmap.targets, ev.x, ev.y, ev.z, ev.module, ev.side)
+    assert all(a != b for a, b in zip(default.counts, ora.counts)), (default.counts, ora.counts)
+    c.close()
