@@ -554,3 +554,41 @@ def test_parity_with_non_default_cut_constants(lstmod, geom, mmap, o32):
     default = o32.run(geom.layer, mmap.row_offsets, mmap.targets, ev.x, ev.y, ev.z, ev.module, ev.side)
     assert all(a != b for a, b in zip(default.counts, ora.counts)), (default.counts, ora.counts)
     c.close()
+
+
+@pytest.mark.parametrize("how", ["thinned", "fat"])
+def test_parity_with_other_module_maps(lstmod, geom, mmap, o32, how):
+    """The module map is an INPUT that defines the search space (reading 6): a map with 30 % of its connections
+    removed, and a fat one (every module of the next layer within +-3 rings and +-3 azimuth steps: rows of up to 49
+    targets, more than one warp tile per owner) must give the oracle's sets for that same map."""
+    rng = np.random.default_rng(17)
+    if how == "thinned":
+        rows = [np.asarray(mmap.targets[mmap.row_offsets[a]:mmap.row_offsets[a + 1]]) for a in range(geom.n_modules)]
+        rows = [r[rng.random(len(r)) > 0.3] for r in rows]
+    else:
+        nphi = {l: int((geom.layer == l).sum()) // 24 for l in range(6)}
+        base = {l: int(np.nonzero(geom.layer == l)[0][0]) for l in range(6)}
+        rows = []
+        for a in range(geom.n_modules):
+            l = int(geom.layer[a])
+            if l == 5:
+                rows.append(np.zeros(0, np.int64))
+                continue
+            ring, i = divmod(a - base[l], nphi[l])
+            i2 = int(round(i * nphi[l + 1] / nphi[l]))
+            t = [base[l + 1] + r * nphi[l + 1] + (i2 + d) % nphi[l + 1] for r in range(max(0, ring - 3), min(24, ring + 4)) for d in range(-3, 4)]
+            rows.append(np.unique(t))
+        assert max(len(r) for r in rows) > 32
+    offs = np.zeros(geom.n_modules + 1, np.int32)
+    offs[1:] = np.cumsum([len(r) for r in rows])
+    tg = np.concatenate(rows).astype(np.int32)
+    cfg = lstmod.default_config()
+    cfg.n_slots = 1
+    c = lstmod.Lst(geom.layer, offs, tg, cfg, phi=geom.phi)
+    ev = synth.generate_event(geom, 1, 66, n_particles=1500)
+    gpu = parity.run_gpu(c, ev)
+    ora = o32.run(geom.layer, offs, tg, ev.x, ev.y, ev.z, ev.module, ev.side)
+    parity.compare(gpu, parity.oracle_tables(ora), how)
+    st = c.stats(0)
+    assert st["needed"] == ora.counts and st["candidates"] == ora.candidates and ora.counts[3] > 100
+    c.close()
