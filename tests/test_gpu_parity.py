@@ -592,3 +592,24 @@ def test_parity_with_other_module_maps(lstmod, geom, mmap, o32, how):
     st = c.stats(0)
     assert st["needed"] == ora.counts and st["candidates"] == ora.candidates and ora.counts[3] > 100
     c.close()
+
+
+def test_create_destroy_returns_the_arena(lstmod, geom, mmap):
+    """lst_create makes ONE arena allocation (plus the small tables); lst_destroy gives everything back: 20 create / run /
+    destroy cycles leave the device's free memory where it was."""
+    import torch
+    torch.cuda.synchronize()
+    ev = synth.generate_event(geom, 0, 4)
+    free0 = torch.cuda.mem_get_info()[0]
+    for _ in range(20):
+        cfg = lstmod.default_config()
+        cfg.n_slots = 3
+        c = lstmod.Lst.from_synth(geom, mmap, cfg)
+        total, per_slot = c.arena_bytes()
+        assert total == 3 * per_slot and torch.cuda.mem_get_info()[0] <= free0 - total
+        c.load_event(2, ev.x, ev.y, ev.z, ev.module, ev.side)
+        c.run(2)
+        assert c.sync(2) == 0
+        c.close()
+    torch.cuda.synchronize()
+    assert abs(torch.cuda.mem_get_info()[0] - free0) <= 64 << 20
