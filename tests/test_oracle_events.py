@@ -208,3 +208,22 @@ def test_p10_truth_sanity_and_p6_statistics(geom, o32, run_oracle, c1):
     chi2xy = loose.t5_chi2xy[one]
     assert 1.6 < chi2xy.mean() < 2.4 and 1.0 < np.median(chi2xy) < 1.7     # mean 2, median 1.386
     assert np.quantile(chi2xy, 0.99) < 13.0                                # chi2(2): 9.21
+
+
+def test_golden_oracle_counts():
+    """tests/golden/oracle_counts.txt (written by tests/golden/make_oracle_counts.py from the oracle alone): the oracle as
+    it stands reproduces the stored counts and quintuplet digests on the seeded events."""
+    import importlib.util
+    import os
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("make_oracle_counts", os.path.join(here, "make_oracle_counts.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    stored = [ln.strip() for ln in open(os.path.join(here, "oracle_counts.txt")) if ln.strip()]
+    mod.CASES = tuple(c for c in mod.CASES if c[0] in ("C0", "C1small"))        # the cheap cases: a few seconds
+    now = {ln.split(" |")[0]: ln for ln in mod.lines() if not ln.startswith("#")}
+    assert now, "no case ran"
+    for ln in stored:
+        key = ln.split(" |")[0]
+        if key in now:
+            assert now[key] == ln, (now[key], ln)
