@@ -295,7 +295,7 @@ def run_ours(args):
             for st in S["streams"]:
                 st.synchronize()
 
-    e2e_steps = max(4, min(args.steps, 10))
+    e2e_steps = max(4, min(args.steps, 40))
     e2e_run(3)
     barrier()
     t0 = time.perf_counter()
@@ -382,7 +382,7 @@ def run_ours(args):
         n_thr = os.cpu_count() or 1
         def _one(ev):
             o.run(geom.layer, mmap.row_offsets, mmap.targets, ev.x, ev.y, ev.z, ev.module, ev.side)   # ctypes releases the GIL
-        work = events * max(1, (8 * n_thr + N_EVENTS - 1) // N_EVENTS)        # ~8 events per thread: a few seconds
+        work = events * max(2, (64 * n_thr + N_EVENTS - 1) // N_EVENTS)       # ~64 events per thread: several seconds
         t0 = time.perf_counter()
         with ThreadPoolExecutor(n_thr) as pool:
             list(pool.map(_one, work))
@@ -545,7 +545,7 @@ def run_sweep(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
