@@ -631,6 +631,68 @@ int64_t lsto_t5_clean(int64_t n, const int32_t* hits, const real* chi2xy, const 
   return kept;
 }
 
+/* ------------------------------------------------------------------------------------ */
+/* [B] module-map builder  (DESIGN.md section 1 [B])        */
+/* ------------------------------------------------------------------------------------ */
+/* "derived from first principles by computing the possible track trajectories as helices that can start
+ * from the edges of a given module that are compatible with the pT threshold, and then listing all the
+ * modules in the adjacent layer that intersect these helices".  The paper gives no
+ * formula; the reading (reading 25) is the closed-form envelope of those
+ * helices, always in double precision, for a source module A and a module B of the next layer:
+ *   radii reached on A / B:  r_lo = rho_A - gap_A/2, r_hi = hypot(rho_A + gap_A/2, hw_A),
+ *                            r'_lo = rho_B - gap_B/2, r'_hi = hypot(rho_B + gap_B/2, hw_B)
+ *   tightest helix:          R_m = pt_min / (k B), a(r) = asin(min(1, r / (2 R_m)))
+ *   azimuth:  |wrap(phi_B - phi_A)| <= atan(hw_A / r_lo) + atan(hw_B / r'_lo) + (a(r'_hi) - a(r_lo)) + pad_phi
+ *   z:        the interval spanned by z0 + (z_A - z0) * ratio over z0 in {-z0_max, +z0_max},
+ *             z_A in {zlo_A - pad_z, zhi_A + pad_z}, ratio in {r'_lo / r_hi (straight, shortest lever),
+ *             a(r'_hi) / a(r_lo) (tightest helix, arc-length ratio)} must meet [zlo_B, zhi_B].
+ * rows come out ascending.  counts[n] / targets: the caller passes targets == NULL to count only.
+ * Returns the number of connections. */
+int64_t lsto_build_map(int32_t n, const int8_t* layer, const double* phi, const double* rho, const double* gap,
+                       const double* hw, const double* zlo, const double* zhi, double pt_min, double b_tesla,
+                       double z0_max, double pad_phi, double pad_z, int32_t* row_offsets, int32_t* targets) {
+  const double kGeV = 2.99792458e-3, kPi = 3.14159265358979323846;
+  const double Rm = pt_min / (kGeV * b_tesla);
+  int64_t total = 0;
+  int32_t A, B;
+  for (A = 0; A < n; ++A) {
+    row_offsets[A] = (int32_t)total;
+    for (B = 0; B < n; ++B) {
+      double r_lo, r_hi, rp_lo, rp_hi, a_out, a_in, tol, d, ratio[2], z_lo = 0, z_hi = 0;
+      int iz0, iza, ir, first = 1;
+      if (layer[B] != layer[A] + 1) continue;
+      r_lo = rho[A] - gap[A] / 2;
+      r_hi = hypot(rho[A] + gap[A] / 2, hw[A]);
+      rp_lo = rho[B] - gap[B] / 2;
+      rp_hi = hypot(rho[B] + gap[B] / 2, hw[B]);
+      a_out = asin(fmin(1.0, rp_hi / (2 * Rm)));
+      a_in = asin(fmin(1.0, r_lo / (2 * Rm)));
+      tol = atan(hw[A] / r_lo) + atan(hw[B] / rp_lo) + (a_out - a_in) + pad_phi;
+      d = fmod(phi[B] - phi[A], 2 * kPi);            /* into (-pi, pi] */
+      if (d > kPi) d -= 2 * kPi;
+      if (d <= -kPi) d += 2 * kPi;
+      if (!(fabs(d) <= tol)) continue;
+      ratio[0] = rp_lo / r_hi;
+      ratio[1] = a_out / a_in;
+      for (iz0 = 0; iz0 < 2; ++iz0)
+        for (iza = 0; iza < 2; ++iza)
+          for (ir = 0; ir < 2; ++ir) {
+            const double z0 = iz0 ? z0_max : -z0_max;
+            const double za = iza ? zhi[A] + pad_z : zlo[A] - pad_z;
+            const double zp = z0 + (za - z0) * ratio[ir];
+            if (first || zp < z_lo) z_lo = zp;
+            if (first || zp > z_hi) z_hi = zp;
+            first = 0;
+          }
+      if (!(z_hi >= zlo[B] && z_lo <= zhi[B])) continue;
+      if (targets) targets[total] = B;
+      ++total;
+    }
+  }
+  row_offsets[n] = (int32_t)total;
+  return total;
+}
+
 /* ---- accessors for the ctypes wrapper ---- */
 int64_t lsto_count(const lsto_event* ev, int kind) {
   switch (kind) { case 0: return ev->n_md; case 1: return ev->n_seg; case 2: return ev->n_t3; case 3: return ev->n_t5; }

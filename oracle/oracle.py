@@ -149,6 +149,21 @@ class OracleLib:
         assert kept == int(keep[:n].sum())
         return keep[:n].astype(bool)
 
+    def build_map(self, layer, phi, rho, gap, hw, zlo, zhi, pt_min=0.8, b_tesla=3.8, z0_max=15.0, pad_phi=0.01, pad_z=1.0):
+        """[B] module-map builder (always double precision). Returns (row_offsets, targets)."""
+        layer = np.ascontiguousarray(layer, np.int8)
+        arrs = [np.ascontiguousarray(a, np.float64) for a in (phi, rho, gap, hw, zlo, zhi)]
+        n = len(layer)
+        ptr = lambda a: a.ctypes.data_as(C.c_void_p)
+        f = self.lib.lsto_build_map
+        f.restype = C.c_int64
+        f.argtypes = [C.c_int32] + [C.c_void_p] * 7 + [C.c_double] * 5 + [C.c_void_p, C.c_void_p]
+        offs = np.zeros(n + 1, np.int32)
+        total = f(n, ptr(layer), *[ptr(a) for a in arrs], pt_min, b_tesla, z0_max, pad_phi, pad_z, ptr(offs), None)
+        tg = np.zeros(max(int(total), 1), np.int32)
+        f(n, ptr(layer), *[ptr(a) for a in arrs], pt_min, b_tesla, z0_max, pad_phi, pad_z, ptr(offs), ptr(tg))
+        return offs, tg[:total]
+
     # ---- whole event -----------------------------------------------------------------------
     def run(self, layer, row_offsets, targets, x, y, z, module, side, mode=0, stages=4, cfg=None) -> "OracleResult":
         cfg = cfg or self.default_config()

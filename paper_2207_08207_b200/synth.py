@@ -135,6 +135,16 @@ def make_module_map(geom: Geometry) -> ModuleMap:
     return ModuleMap(geom.n_modules, row_offsets, targets.astype(np.int32))
 
 
+def map_geometry(geom: Geometry) -> dict:
+    """Per-module inputs of the module-map builder [B] (float64): azimuth of the normal, normal distance of the
+    mid-plane, sensor gap, half width in r-phi, z range.  Input data only, none of the builder's arithmetic."""
+    l = geom.layer.astype(np.int64)
+    zlo = -Z_MAX + RING_LEN * geom.ring.astype(np.float64)
+    return dict(layer=geom.layer.astype(np.int8), phi=geom.phi.astype(np.float64), rho=np.asarray(LAYER_R, np.float64)[l],
+                gap=np.asarray(SENSOR_GAP, np.float64)[l], hw=np.full(geom.n_modules, MODULE_HALF_W, np.float64),
+                zlo=zlo, zhi=zlo + RING_LEN)
+
+
 # ----------------------------------------------------------------------------------------
 # Events
 # ----------------------------------------------------------------------------------------
