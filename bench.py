@@ -351,6 +351,16 @@ def run_ours(args):
              "t5_in": needed[3], "t5_kept": kept,
              "what": "a0..a4 + LST_CLEAN per step; `value` above is a0..a4 only (the BASELINE.json path)"}
 
+    # ---- the step before the path: module-map builder [B], built once per geometry ----
+    from paper_2207_08207_b200 import synth as _synth
+    mg = _synth.map_geometry(geom)
+    margs = (mg["layer"], mg["phi"], mg["rho"], mg["gap"], mg["hw"], mg["zlo"], mg["zhi"])
+    lst.build_module_map(*margs, device=local)
+    b_offs, b_tg, b_ms = lst.build_module_map(*margs, device=local)
+    map_builder = {"kernels_ms": {"count": b_ms[0], "fill": b_ms[1]}, "modules": int(geom.n_modules), "connections": int(len(b_tg)),
+                   "pair_tests_per_s": 2 * geom.n_modules ** 2 / ((b_ms[0] + b_ms[1]) * 1e-3),
+                   "equals_input_map": bool(np.array_equal(b_offs, mmap.row_offsets) and np.array_equal(b_tg, mmap.targets))}
+
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
            "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "f32", "data": "synthetic", "config": workload_config(), "clocks": clocks, "e2e": e2e,
@@ -365,7 +375,7 @@ def run_ours(args):
                              "factor": launches_per_step * sum(v["ms"] for v in per_stage.values()) / (total_ms / args.steps),
                              "what": "sum over the step's launches of their CUDA-event durations / the step: > 1 = kernels of "
                                      "different streams run side by side"},
-           "duplicate_cleaning": clean,
+           "duplicate_cleaning": clean, "module_map_builder": map_builder,
            "rewalks_per_step": dict(md=rewalks[0], ls=rewalks[1], t3=rewalks[2], t5=rewalks[3]),
            "arena_mib": ctx.arena_bytes()[0] / 2 ** 20, "impl": "ours"}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -387,6 +397,9 @@ def run_ours(args):
         with ThreadPoolExecutor(n_thr) as pool:
             list(pool.map(_one, work))
         dt = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        o.build_map(*margs)
+        map_builder["oracle_s_one_thread"] = time.perf_counter() - t0
         out["cpu_baseline"]["all_cores"] = {"value": len(work) / dt, "unit": UNIT, "cores": n_thr,
                                             "sample": f"{len(work)} events on {n_thr} threads, {dt:.1f} s"}
     ctx.close()

@@ -279,6 +279,36 @@ LST_API int lst_fetch_batch(lst_ctx* ctx, int first_slot, int n_slots, int kind,
                             float* const* val_out, const int64_t* cap_objects, int32_t* counts, int wait,
                             void* cuda_stream);
 
+/* ---- module-map builder: the step before the path (DESIGN.md section 1 [B]) ---------------- */
+/* Per-module inputs, HOST pointers, binary64: azimuth of the module normal, normal distance of the module
+ * mid-plane from the beam line, distance between the two sensors, half width in r-phi, z range. */
+typedef struct {
+  int32_t n_modules;
+  const int8_t* layer;      /* [n_modules] 0 .. LST_N_LAYERS-1 */
+  const double* phi;
+  const double* rho;
+  const double* gap;
+  const double* half_width;
+  const double* z_lo;
+  const double* z_hi;
+} lst_map_geometry;
+typedef struct {
+  double pt_min;   /* GeV  (0.8: the paper's threshold) */
+  double b_tesla;  /* T    (3.8) */
+  double z0_max;   /* cm   (15)  */
+  double pad_phi;  /* rad  (0.01) */
+  double pad_z;    /* cm   (1)   */
+} lst_map_params;
+LST_API int lst_default_map_params(lst_map_params* params);
+/* Builds the module map on `device`: module B of the next layer is connected to A iff the closed-form envelope
+ * of the pT >= pt_min helices from A's edges meets B (rule B1-B4).  row_offsets: HOST [n_modules + 1], always
+ * written; targets: HOST [cap_targets], rows ascending; *n_targets = number of connections.  params = NULL means
+ * lst_default_map_params.  kernel_ms (may be NULL): [2] durations of the count and the fill kernel.
+ * Errors: LST_ERR_ARG; LST_ERR_OVERFLOW if cap_targets is too small (row_offsets and *n_targets are valid: call
+ * again with a buffer of *n_targets entries); LST_ERR_NOMEM; LST_ERR_CUDA. */
+LST_API int lst_build_module_map(const lst_map_geometry* geom, const lst_map_params* params, int device, int32_t* row_offsets,
+                                 int32_t* targets, int64_t cap_targets, int64_t* n_targets, float* kernel_ms);
+
 /* Bytes of the arena (all slots) and of one slot. */
 LST_API int lst_arena_bytes(lst_ctx* ctx, int64_t* total, int64_t* per_slot);
 /* Kernels launched by this context so far (for bench.py's gpu_launches). */

@@ -15,7 +15,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblst.so")
-SOURCES = ["lst_kernels.cu", "lst_api.cu"]
+SOURCES = ["lst_kernels.cu", "lst_api.cu", "lst_map.cu"]
 HEADERS = ["lst_cuts.cuh", "lst_device.cuh", os.path.join("..", "..", "include", "lst.h")]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

@@ -97,6 +97,16 @@ class Stats(C.Structure):
                 ("rewalks", C.c_int64 * 4), ("n_kept", C.c_int32)]
 
 
+class MapGeometry(C.Structure):
+    _fields_ = [("n_modules", C.c_int32), ("layer", C.c_void_p), ("phi", C.c_void_p), ("rho", C.c_void_p), ("gap", C.c_void_p),
+                ("half_width", C.c_void_p), ("z_lo", C.c_void_p), ("z_hi", C.c_void_p)]
+
+
+class MapParams(C.Structure):
+    _fields_ = [("pt_min", C.c_double), ("b_tesla", C.c_double), ("z0_max", C.c_double), ("pad_phi", C.c_double),
+                ("pad_z", C.c_double)]
+
+
 class TcView(C.Structure):
     _fields_ = [("n", C.c_int32), ("t5", C.c_void_p), ("keep", C.c_void_p), ("score", C.c_void_p)]
 
@@ -125,6 +135,9 @@ SYMBOLS = {
     "lst_fetch_kept": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_int64, C.c_void_p]),
     "lst_fetch_hit_indices": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int64, C.c_void_p]),
     "lst_fetch_values": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int64, C.c_void_p]),
+    "lst_default_map_params": (C.c_int, [P(MapParams)]),
+    "lst_build_module_map": (C.c_int, [P(MapGeometry), P(MapParams), C.c_int, C.c_void_p, C.c_void_p, C.c_int64, P(C.c_int64),
+                                       P(C.c_float)]),
     "lst_arena_bytes": (C.c_int, [C.c_void_p, P(C.c_int64), P(C.c_int64)]),
     "lst_launch_count": (C.c_int64, [C.c_void_p]),
     "lst_last_cuda_error": (C.c_int, [C.c_void_p]),
@@ -194,6 +207,31 @@ def _stream(s) -> int:
     if hasattr(s, "cuda_stream"):
         return int(s.cuda_stream)
     return int(s)
+
+
+def build_module_map(layer, phi, rho, gap, half_width, z_lo, z_hi, device: int = 0, **params):
+    """Module-map builder [B] on the GPU (lst_build_module_map). Arrays: per module, host. Keyword parameters override
+    lst_default_map_params (pt_min, b_tesla, z0_max, pad_phi, pad_z). Returns (row_offsets, targets, kernel_ms[2])."""
+    lib = load_library()
+    layer = np.ascontiguousarray(layer, np.int8)
+    arrs = [np.ascontiguousarray(a, np.float64) for a in (phi, rho, gap, half_width, z_lo, z_hi)]
+    n = len(layer)
+    g = MapGeometry(n, _ptr(layer), *[_ptr(a) for a in arrs])
+    p = MapParams()
+    lib.lst_default_map_params(C.byref(p))
+    for k, v in params.items():
+        setattr(p, k, float(v))
+    offs = np.zeros(n + 1, np.int32)
+    total = C.c_int64(0)
+    ms = (C.c_float * 2)()
+    targets = np.zeros(1, np.int32)
+    st = lib.lst_build_module_map(C.byref(g), C.byref(p), device, _ptr(offs), _ptr(targets), 0, C.byref(total), ms)
+    if st == ERR_OVERFLOW:                       # the size is known now: second call with the buffer it asks for
+        targets = np.zeros(max(int(total.value), 1), np.int32)
+        st = lib.lst_build_module_map(C.byref(g), C.byref(p), device, _ptr(offs), _ptr(targets), len(targets), C.byref(total), ms)
+    if st != OK:
+        raise LstError(st, "lst_build_module_map")
+    return offs, targets[:int(total.value)], [float(ms[0]), float(ms[1])]
 
 
 def packed_event_buffers(n: int):

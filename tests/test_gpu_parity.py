@@ -613,3 +613,46 @@ def test_create_destroy_returns_the_arena(lstmod, geom, mmap):
         c.close()
     torch.cuda.synchronize()
     assert abs(torch.cuda.mem_get_info()[0] - free0) <= 64 << 20
+
+
+def test_module_map_builder_parity(lstmod, geom, mmap, o64):
+    """lst_build_module_map [B] against the oracle (binary64 on both sides): identical CSR (offsets and ascending
+    targets) on the BASELINE geometry, with other parameters, and on a jittered geometry; the two-call size protocol;
+    and the map it builds drives the path to the same result as the test-side map."""
+    import ctypes as C
+    mg = synth.map_geometry(geom)
+    args = (mg["layer"], mg["phi"], mg["rho"], mg["gap"], mg["hw"], mg["zlo"], mg["zhi"])
+    offs, tg, ms = lstmod.build_module_map(*args)
+    o_offs, o_tg = o64.build_map(*args)
+    assert np.array_equal(offs, o_offs) and np.array_equal(tg, o_tg) and len(tg) == 69630
+    assert np.array_equal(offs, mmap.row_offsets) and np.array_equal(tg, mmap.targets)
+    print(f"map builder: count {ms[0]:.3f} ms, fill {ms[1]:.3f} ms for {geom.n_modules} modules, {len(tg)} connections")
+    for kw in (dict(pt_min=0.6), dict(pt_min=1.5, z0_max=5.0), dict(pad_phi=0.0, pad_z=0.0), dict(b_tesla=2.0)):
+        g_o, g_t, _ = lstmod.build_module_map(*args, **kw)
+        r_o, r_t = o64.build_map(*args, **kw)
+        assert np.array_equal(g_o, r_o) and np.array_equal(g_t, r_t), kw
+    rng = np.random.default_rng(8)                                   # another detector: jittered radii, gaps, widths, azimuths
+    jit = (mg["layer"], mg["phi"] + rng.normal(0, 0.02, geom.n_modules), mg["rho"] * rng.uniform(0.97, 1.03, geom.n_modules),
+           mg["gap"] * rng.uniform(0.5, 1.5, geom.n_modules), mg["hw"] * rng.uniform(0.6, 1.2, geom.n_modules),
+           mg["zlo"] + rng.normal(0, 0.5, geom.n_modules), mg["zhi"] + rng.normal(0, 0.5, geom.n_modules))
+    g_o, g_t, _ = lstmod.build_module_map(*jit)
+    r_o, r_t = o64.build_map(*jit)
+    assert np.array_equal(g_o, r_o) and np.array_equal(g_t, r_t) and len(g_t) != 69630
+    # size protocol and argument errors through the C-ABI
+    lib = lstmod.load_library()
+    keep = [np.ascontiguousarray(a) for a in args]
+    g = lstmod.MapGeometry(geom.n_modules, *[lstmod._ptr(a) for a in keep])
+    ro = np.zeros(geom.n_modules + 1, np.int32)
+    small = np.zeros(10, np.int32)
+    total = C.c_int64(0)
+    st = lib.lst_build_module_map(C.byref(g), None, 0, lstmod._ptr(ro), lstmod._ptr(small), 10, C.byref(total), None)
+    assert st == lstmod.ERR_OVERFLOW and total.value == 69630 and np.array_equal(ro, o_offs) and not small.any()
+    bad = lstmod.MapGeometry(geom.n_modules, lstmod._ptr(keep[0]), 0, *[lstmod._ptr(a) for a in keep[2:]])
+    assert lib.lst_build_module_map(C.byref(bad), None, 0, lstmod._ptr(ro), lstmod._ptr(small), 10, C.byref(total), None) == lstmod.ERR_ARG
+    # the built map feeds lst_create
+    c = lstmod.Lst(geom.layer, offs, tg, phi=geom.phi)
+    ev = synth.generate_event(geom, 0, 2)
+    c.load_event(0, ev.x, ev.y, ev.z, ev.module, ev.side)
+    c.run(0)
+    assert c.sync(0) == 0 and c.stats(0)["needed"][3] > 50
+    c.close()
