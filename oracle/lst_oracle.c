@@ -27,7 +27,9 @@
  * single-helix recovery (P4), library least-squares / circumradius reductions (P5),
  * chi2 statistics (P6), symmetries (P7), threshold flips (P8), structure (P9), truth (P10);
  * duplicate cleaning [D] (tests/test_oracle_clean.py): single helix (P11), set-based restatement (P12),
- * implied properties and order independence (P13), truth statistics (P14).
+ * implied properties and order independence (P13), truth statistics (P14); module-map builder [B]
+ * (tests/test_oracle_map.py): simulated tracks stay inside the map (P15), the test-side generator (P16),
+ * symmetries and monotonicity (P17).
  * The paper prints no worked numerical example, so no value is pinned to the paper itself.
  */
 #include <math.h>
