@@ -173,9 +173,11 @@ def workload_config():
 # ------------------------------------------------------------------------------------------
 def run_ours(args):
     import torch
-    from paper_2207_08207_b200 import lst
+    from paper_2207_08207_b200 import build as lst_build, lst
 
     rank = int(os.environ.get("RANK", "0"))
+    if int(os.environ.get("LOCAL_RANK", "0")) == 0:
+        lst_build.build()                       # no-op when liblst.so is up to date (it travels in-tree); never a fallback
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"

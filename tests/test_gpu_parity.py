@@ -16,7 +16,8 @@ pytestmark = pytest.mark.gpu
 def lstmod():
     import torch
     assert torch.cuda.is_available(), "GPU tests need a CUDA device"
-    from paper_2207_08207_b200 import lst
+    from paper_2207_08207_b200 import build as lst_build, lst
+    lst_build.build()           # no-op when liblst.so is up to date; compiles it (nvcc, sm_100a) on a fresh checkout
     lst.load_library()          # raises if liblst.so is missing: no fallback
     return lst
 
