@@ -276,15 +276,19 @@ def run_ours(args):
                      "val": [[out[k][1] for k in range(s * per_stream, (s + 1) * per_stream)] for s in range(N_STREAMS)],
                      "counts": None})
 
+    e2e_kind = [lst.T5]                             # lst.CLEAN: the path + cleaning stage, only the kept quintuplets travel back
+
     def e2e_launch(i):                              # H2D of the pinned hit SoA + a0..a4 of step i, all asynchronous
         S = sets[i % 2]
         for s, st in enumerate(S["streams"]):
             ctx.load_events(S["base"] + s * per_stream, np_in[s * per_stream:(s + 1) * per_stream], stream=st)
             ctx.run_batch(S["base"] + s * per_stream, per_stream, st)
+            if e2e_kind[0] == lst.CLEAN:
+                ctx.run_stage(S["base"] + s * per_stream, per_stream, lst.CLEAN, st)
 
     def e2e_collect(i):                             # counters back (one sync per stream), then gathers + D2H enqueued
         S = sets[i % 2]
-        S["counts"] = [ctx.fetch_batch(S["base"] + s * per_stream, lst.T5, S["idx"][s], S["val"][s], stream=st, wait=False)
+        S["counts"] = [ctx.fetch_batch(S["base"] + s * per_stream, e2e_kind[0], S["idx"][s], S["val"][s], stream=st, wait=False)
                        for s, st in enumerate(S["streams"])]
 
     def e2e_run(n):
@@ -311,13 +315,26 @@ def run_ours(args):
         for k in (0, N_EVENTS - 1):
             ref = ctx.fetch_hit_indices(S["base"] + k, lst.T5, S["streams"][k // per_stream])
             assert np.array_equal(S["idx"][k // per_stream][k % per_stream][:len(ref)], ref)
+    # the same with the cleaning stage [D] in the step and only the kept quintuplets (the track candidates) downloaded
+    e2e_kind[0] = lst.CLEAN
+    e2e_run(3)
+    barrier()
+    t0 = time.perf_counter()
+    e2e_run(e2e_steps)
+    torch.cuda.synchronize(dev)
+    e2e_tc_s = max_over_ranks(time.perf_counter() - t0, dist, dev)
+    kept_e2e = sum(c for S in sets[:1] for per in S["counts"] for c in per)
+    e2e_kind[0] = lst.T5
     h2d = sum(sum(t.numel() * t.element_size() for t in ev) for ev in h_in)
     d2h = needed[3] * (40 + 20) + N_EVENTS * HEADER_BYTES
     e2e = {"value": world * N_EVENTS * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
            "d2h_bytes_per_step": int(d2h), "steps": e2e_steps,
            "how": "per stream: lst_load_events(16 x pinned host SoA) + lst_run_batch + lst_fetch_batch(T5 hit indices + values "
                   "to pinned host buffers); two buffer sets, step i + 1 is loaded and run while step i's results travel back; "
-                  "the timed region ends with every step's results on the host"}
+                  "the timed region ends with every step's results on the host",
+           "track_candidates": {"value": world * N_EVENTS * e2e_steps / e2e_tc_s, "unit": UNIT, "d2h_bytes_per_step": int(kept_e2e * 60 + N_EVENTS * HEADER_BYTES),
+                                "what": "the same pipeline with LST_CLEAN in the step and lst_fetch_batch(kind = LST_CLEAN): only the kept "
+                                        "quintuplets (T5-only track candidates) travel back"}}
 
     # ---- per-kernel times (CUDA events inside the library, timing mode), one 64-event batch ----
     kernel_ms, launches_per_step = per_kernel_times(lst, geom, mmap, d_in, local)

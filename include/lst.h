@@ -265,7 +265,8 @@ LST_API int lst_fetch_values(lst_ctx* ctx, int slot, int kind, float* out, int64
 
 /* Result download for a batch of slots in one call (the end-to-end path of a multi-event
  * pipeline): synchronises the slots if they are not yet (lst_sync_batch), then
- * for slot first_slot + b gathers the hit-index tuples of class `kind` on the device and enqueues
+ * for slot first_slot + b gathers the hit-index tuples of class `kind` (LST_MD .. LST_T5, or LST_CLEAN =
+ * the quintuplets kept by the cleaning stage only, in the layout of LST_T5) on the device and enqueues
  * their copy to the HOST buffer idx_out[b] ([n][2|4|6|10] int32) and the copy of the float payload
  * (layout as lst_fetch_values) to val_out[b].  idx_out / val_out may be NULL, and so may single
  * entries (nothing is copied for them).  cap_objects[b] = rows available in slot b's buffers;

@@ -552,8 +552,8 @@ int lst_get_stats(lst_ctx* c, int slot, lst_stats* o) {
   return LST_OK;
 }
 
-static const int kHitsPerObject[4] = {2, 4, 6, 10};
-static const int kValuesPerObject[4] = {4, 4, 2, 5};
+static const int kHitsPerObject[5] = {2, 4, 6, 10, 10};     // [4]: the kept quintuplets (LST_CLEAN)
+static const int kValuesPerObject[5] = {4, 4, 2, 5, 5};
 
 int lst_sync_batch(lst_ctx* c, int first, int n, void* stream) {
   if (!c || n < 1 || !valid_slot(c, first) || !valid_slot(c, first + n - 1)) return LST_ERR_ARG;
@@ -577,9 +577,11 @@ int lst_sync_batch(lst_ctx* c, int first, int n, void* stream) {
   return status;
 }
 
+static inline int count_of(const SlotHeader* h, int kind) { return kind == LST_CLEAN ? h->n_kept : h->n[kind]; }
+
 int lst_fetch_batch(lst_ctx* c, int first, int n, int kind, int32_t* const* idx_out, float* const* val_out,
                     const int64_t* cap_objects, int32_t* counts, int wait, void* stream) {
-  if (!c || n < 1 || !valid_slot(c, first) || !valid_slot(c, first + n - 1) || kind < LST_MD || kind > LST_T5 || !cap_objects)
+  if (!c || n < 1 || !valid_slot(c, first) || !valid_slot(c, first + n - 1) || kind < LST_MD || kind > LST_CLEAN || !cap_objects)
     return LST_ERR_ARG;
   for (int s = first; s < first + n; ++s)
     if (!c->slots[s].loaded || c->slots[s].stages_run <= kind) return LST_ERR_STATE;
@@ -593,7 +595,7 @@ int lst_fetch_batch(lst_ctx* c, int first, int n, int kind, int32_t* const* idx_
   for (int b = 0; b < n; ++b) {
     const SlotHeader* h = c->slots[first + b].hdr;
     if (h->overflow) return LST_ERR_OVERFLOW;
-    const int nk = h->n[kind];
+    const int nk = count_of(h, kind);
     if (counts) counts[b] = nk;
     if (nk > cap_objects[b] && ((idx_out && idx_out[b]) || (val_out && val_out[b]))) return LST_ERR_ARG;
     n_max = nk > n_max ? nk : n_max;
@@ -613,7 +615,7 @@ int lst_fetch_batch(lst_ctx* c, int first, int n, int kind, int32_t* const* idx_
     std::memset(&T, 0, sizeof(T));
     bool any = false;
     for (int b = 0; b < nb; ++b) {
-      if (c->slots[first + b0 + b].hdr->n[kind] == 0) continue;
+      if (count_of(c->slots[first + b0 + b].hdr, kind) == 0) continue;
       if (idx_out && idx_out[b0 + b])
         if (void* a = const_cast<void*>(mapped_alias(idx_out[b0 + b]))) { T.idx[b] = static_cast<int*>(a); idx_dma[b0 + b] = nullptr; any = true; }
       if (val_out && val_out[b0 + b])
@@ -627,7 +629,7 @@ int lst_fetch_batch(lst_ctx* c, int first, int n, int kind, int32_t* const* idx_
   }
   bool idx_left = false, val_left = false;
   for (int b = 0; b < n; ++b) {
-    const bool has = c->slots[first + b].hdr->n[kind] > 0;
+    const bool has = count_of(c->slots[first + b].hdr, kind) > 0;
     idx_left = idx_left || (has && idx_out && idx_dma[b]);
     val_left = val_left || (has && val_out && val_dma[b]);
   }
@@ -639,21 +641,21 @@ int lst_fetch_batch(lst_ctx* c, int first, int n, int kind, int32_t* const* idx_
     c->launches += launch_gather_hits(P, kind, n_max, n, st);
     LST_CUDA(c, cudaGetLastError());
     for (int b = 0; b < n; ++b) {
-      const int nk = c->slots[first + b].hdr->n[kind];
+      const int nk = count_of(c->slots[first + b].hdr, kind);
       if (!idx_out[b] || nk == 0) continue;
       const char* base = c->arena + (size_t)(first + b) * c->P.slot_stride;
       LST_CUDA(c, cudaMemcpyAsync(idx_out[b], base + L.scratch, sizeof(int32_t) * (size_t)nk * kHitsPerObject[kind], cudaMemcpyDeviceToHost, st));
     }
   }
   if (val_out && n_max > 0) {
-    const bool packed = kind == LST_MD || kind == LST_T3;
+    const bool packed = kind == LST_MD || kind == LST_T3 || kind == LST_CLEAN;
     if (packed) {
       c->launches += launch_pack_values(P, kind, n_max, n, st);
       LST_CUDA(c, cudaGetLastError());
     }
     const size_t src_off = packed ? L.scratch : (kind == LST_SEG ? L.seg_f : L.t5_f);
     for (int b = 0; b < n; ++b) {
-      const int nk = c->slots[first + b].hdr->n[kind];
+      const int nk = count_of(c->slots[first + b].hdr, kind);
       if (!val_out[b] || nk == 0) continue;
       const char* base = c->arena + (size_t)(first + b) * c->P.slot_stride;
       LST_CUDA(c, cudaMemcpyAsync(val_out[b], base + src_off, sizeof(float) * (size_t)nk * kValuesPerObject[kind], cudaMemcpyDeviceToHost, st));

@@ -1423,7 +1423,7 @@ __global__ void __launch_bounds__(256) k_clean_mark(const __grid_constant__ Para
 __global__ void __launch_bounds__(256) k_gather_hits(const __grid_constant__ Params P, int kind) {
   Slot S(P, blockIdx.y);
   const int w = kind == LST_MD_ ? 1 : kind == LST_SEG_ ? 2 : kind == LST_T3_ ? 3 : 5;   // MDs per object
-  const size_t m = (size_t)S.hdr()->n[kind] * w;
+  const size_t m = (size_t)(kind == LST_CLEAN_ ? S.hdr()->n_kept : S.hdr()->n[kind]) * w;
   const int2* mh = S.md_hits();
   int2* out = reinterpret_cast<int2*>(S.scratch());
   // one thread per (object, MD): a warp writes 256 contiguous bytes whatever the class
@@ -1436,8 +1436,11 @@ __global__ void __launch_bounds__(256) k_gather_hits(const __grid_constant__ Par
     } else if (kind == LST_T3_) {
       const size_t i = j / 3;
       md = reinterpret_cast<const int*>(S.t3_pack())[4 * i + (j - 3 * i)];
-    } else {
+    } else if (kind == LST_T5_) {
       md = S.t5_md()[j];
+    } else {
+      const size_t i = j / 5;
+      md = S.t5_md()[5 * (size_t)S.tc_list()[i] + (j - 5 * i)];
     }
     out[j] = mh[md];
   }
@@ -1447,9 +1450,14 @@ __global__ void __launch_bounds__(256) k_gather_hits(const __grid_constant__ Par
 // lst_fetch_values, to the slot's scratch area.  (LS and T5 payloads are stored in that layout already.)
 __global__ void __launch_bounds__(256) k_pack_values(const __grid_constant__ Params P, int kind) {
   Slot S(P, blockIdx.y);
-  const int n = S.hdr()->n[kind];
+  const int n = kind == LST_CLEAN_ ? S.hdr()->n_kept : S.hdr()->n[kind];
   float* out = reinterpret_cast<float*>(S.scratch());
-  if (kind == LST_MD_) {
+  if (kind == LST_CLEAN_) {
+    for (size_t j = (size_t)blockIdx.x * blockDim.x + threadIdx.x; j < (size_t)n * 5; j += (size_t)gridDim.x * blockDim.x) {
+      const size_t i = j / 5;
+      out[j] = S.t5_f()[5 * (size_t)S.tc_list()[i] + (j - 5 * i)];
+    }
+  } else if (kind == LST_MD_) {
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
       const float2 o = S.md_out()[i];
       reinterpret_cast<float4*>(out)[i] = make_float4(S.md_aux()[i].y, o.x, o.y, S.md_anchor()[i].w);
@@ -1465,7 +1473,7 @@ __global__ void __launch_bounds__(256) k_pack_values(const __grid_constant__ Par
 // slot by ONE launch per batch.  Small grid: the kernel is bound by the link, not by the SMs.
 __global__ void __launch_bounds__(256) k_fetch_direct(const __grid_constant__ Params P, const __grid_constant__ OutTable T, int kind) {
   Slot S(P, blockIdx.y);
-  const int n = S.hdr()->n[kind];
+  const int n = kind == LST_CLEAN_ ? S.hdr()->n_kept : S.hdr()->n[kind];   // LST_CLEAN_: the kept quintuplets only
   const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (size_t)gridDim.x * blockDim.x;
   if (int2* out = reinterpret_cast<int2*>(T.idx[blockIdx.y])) {
     const int w = kind == LST_MD_ ? 1 : kind == LST_SEG_ ? 2 : kind == LST_T3_ ? 3 : 5;
@@ -1476,12 +1484,15 @@ __global__ void __launch_bounds__(256) k_fetch_direct(const __grid_constant__ Pa
       if (kind == LST_MD_) md = (int)j;
       else if (kind == LST_SEG_) md = reinterpret_cast<const int*>(S.seg_md())[j];
       else if (kind == LST_T3_) { const size_t i = j / 3; md = reinterpret_cast<const int*>(S.t3_pack())[4 * i + (j - 3 * i)]; }
-      else md = S.t5_md()[j];
+      else if (kind == LST_T5_) md = S.t5_md()[j];
+      else { const size_t i = j / 5; md = S.t5_md()[5 * (size_t)S.tc_list()[i] + (j - 5 * i)]; }
       out[j] = mh[md];
     }
   }
   if (float* out = T.val[blockIdx.y]) {
-    if (kind == LST_MD_) {
+    if (kind == LST_CLEAN_) {
+      for (size_t j = tid; j < (size_t)n * 5; j += nth) { const size_t i = j / 5; out[j] = S.t5_f()[5 * (size_t)S.tc_list()[i] + (j - 5 * i)]; }
+    } else if (kind == LST_MD_) {
       for (size_t i = tid; i < (size_t)n; i += nth) {
         const float2 o = S.md_out()[i];
         reinterpret_cast<float4*>(out)[i] = make_float4(S.md_aux()[i].y, o.x, o.y, S.md_anchor()[i].w);
@@ -1596,7 +1607,7 @@ int launch_gather_hits(const Params& P, int kind, int n_max, int n_batch, cudaSt
 }
 
 int launch_pack_values(const Params& P, int kind, int n_max, int n_batch, cudaStream_t s) {
-  if (n_max <= 0 || n_batch <= 0 || (kind != LST_MD_ && kind != LST_T3_)) return 0;
+  if (n_max <= 0 || n_batch <= 0 || (kind != LST_MD_ && kind != LST_T3_ && kind != LST_CLEAN_)) return 0;
   k_pack_values<<<dim3(min(256, (n_max + 255) / 256), (unsigned)n_batch), 256, 0, s>>>(P, kind);
   return 1;
 }

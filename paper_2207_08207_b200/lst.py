@@ -23,8 +23,8 @@ CLEAN = 4                                      # optional stage: duplicate clean
 KIND_NAMES = ("md", "seg", "t3", "t5")
 KERNEL_NAMES = ("reset", "bin_count", "bin_scatter", "bin_order", "md", "seg", "t3", "t5",
                 "clean_prepare", "clean_count", "clean_fill", "clean_mark")   # lst_stats.kernel_ms[0..11]
-HITS_PER_OBJECT = (2, 4, 6, 10)
-VALUES_PER_OBJECT = (4, 4, 2, 5)
+HITS_PER_OBJECT = (2, 4, 6, 10, 10)       # [CLEAN]: the kept quintuplets
+VALUES_PER_OBJECT = (4, 4, 2, 5, 5)
 
 OK, ERR_ARG, ERR_CUDA, ERR_OVERFLOW, ERR_STATE, ERR_NOMEM = 0, -1, -2, -3, -4, -5
 

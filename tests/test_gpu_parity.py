@@ -432,6 +432,17 @@ def test_duplicate_cleaning_batch_empty_and_ties(lstmod, geom, mmap, o32, run_or
         assert c.stats(k)["n_kept"] == int(keep_o.sum()) == len(kept)
         assert set(map(tuple, hits[kept].tolist())) == set(map(tuple, ora.t5_hits()[keep_o].tolist()))
     assert c.stats(1)["n_kept"] == 0 and c.stats(2)["n_kept"] == 0
+    # lst_fetch_batch(kind = LST_CLEAN): the kept quintuplets only, pinned (kernel writes) and pageable (copy engine) buffers
+    for pinned in (True, False):
+        mk = (lambda shape, dt: torch.zeros(shape, dtype=dt).pin_memory().numpy()) if pinned else (lambda shape, dt: np.zeros(shape, {torch.int32: np.int32, torch.float32: np.float32}[dt]))
+        idx = [mk((c.stats(k)["n_kept"] + 2, 10), torch.int32) for k in range(4)]
+        val = [mk((c.stats(k)["n_kept"] + 2, 5), torch.float32) for k in range(4)]
+        counts = c.fetch_batch(0, lstmod.CLEAN, idx, val, stream=st, wait=True)
+        for k in range(4):
+            kept = c.fetch_kept(k, st)
+            assert counts[k] == len(kept)
+            assert np.array_equal(idx[k][:len(kept)], c.fetch_hit_indices(k, lstmod.T5, st)[kept])
+            assert np.array_equal(val[k][:len(kept)], c.fetch_values(k, lstmod.T5, st)[kept])
     c.close()
 
 
