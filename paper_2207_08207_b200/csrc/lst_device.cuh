@@ -173,7 +173,7 @@ struct StageIn {
 int launch_bin(const Params& P, const HitBatch& src, const HitBatch& dev, int n_batch, cudaStream_t s, cudaEvent_t* ev,
                const StageIn* stage);   // 5 kernels
 int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEvent_t* ev);          // 1 kernel
-// Duplicate cleaning [D]: 5 kernels (prepare, count, scan, fill, mark); ev[0..4] around the four steps.
+// Duplicate cleaning [D]: 6 kernels (prepare, count, scan, fill, mark, list); ev[0..4] around the four steps.
 int launch_clean(const Params& P, int n_batch, cudaStream_t s, cudaEvent_t* ev);
 // Per slot of a batch: device-visible aliases of pinned host buffers for the hit-index tuples / the float payload
 // (null = that table is not wanted there, or goes through the scratch area and the copy engine).

@@ -1294,11 +1294,8 @@ __device__ __forceinline__ int common_hits(const int (&a)[10], const int (&h)[10
 // One thread per entry of the incidence table = (quintuplet q, one of its five MDs): rule D2-D4 against every
 // quintuplet in that MD's list.  Threads are taken in TABLE order, so neighbouring threads walk the same list
 // (same trip count, the partners' records served from L1).
-// A removal is an idempotent store of 0 (k_clean_prepare set every flag to 1).  The event's last block then
-// lists the kept quintuplets in ascending order (the T5-only track-candidate list).
+// A removal is an idempotent store of 0 (k_clean_prepare set every flag to 1); k_clean_list then lists the kept ones.
 __global__ void __launch_bounds__(256) k_clean_mark(const __grid_constant__ Params P) {
-  __shared__ int s_warp[8];
-  __shared__ int s_base;
   Slot S(P, blockIdx.y);
   SlotHeader* H = S.hdr();
   const int n5 = H->n[LST_T5_];
@@ -1384,25 +1381,35 @@ __global__ void __launch_bounds__(256) k_clean_mark(const __grid_constant__ Para
     }
     if (removed) keep[q] = 0;
   }
-  if (!last_block_done(&H->done[6], gridDim.x)) return;
-  // ordered list of the kept ones: 8 flags per thread and step
+}
+
+// The kept quintuplets in ascending order (the T5-only track-candidate list): one block of 1024 threads per event,
+// 8 flags per thread and step.
+__global__ void __launch_bounds__(1024) k_clean_list(const __grid_constant__ Params P) {
+  __shared__ int s_warp[32];
+  __shared__ int s_base;
+  Slot S(P, blockIdx.y);
+  SlotHeader* H = S.hdr();
+  const int n5 = H->n[LST_T5_];
+  const unsigned char* keep = S.t5_keep();
   int* tc = S.tc_list();
+  const int w = threadIdx.x >> 5;
   if (threadIdx.x == 0) s_base = 0;
   __syncthreads();
-  for (int q0 = 0; q0 < n5; q0 += 2048) {
+  for (int q0 = 0; q0 < n5; q0 += 8192) {
     const int q = q0 + 8 * threadIdx.x;
     unsigned long long f = 0;
-    if (q < n5) f = __ldcg(reinterpret_cast<const unsigned long long*>(keep + q));   // the array is padded to 256 B
+    if (q < n5) f = *reinterpret_cast<const unsigned long long*>(keep + q);   // the array is padded to 256 B
     if (q + 8 > n5) f &= (q < n5) ? ((1ull << (8 * (n5 - q))) - 1ull) : 0ull;
     const int mine = __popcll(f & 0x0101010101010101ull);
     const int incl = warp_incl_scan(mine);
-    if (lane_id() == 31) s_warp[threadIdx.x >> 5] = incl;
+    if (lane_id() == 31) s_warp[w] = incl;
     __syncthreads();
     int before = s_base, total = 0;
-#pragma unroll
-    for (int w = 0; w < 8; ++w) {
-      before += (w < (int)(threadIdx.x >> 5)) ? s_warp[w] : 0;
-      total += s_warp[w];
+#pragma unroll 8
+    for (int i = 0; i < 32; ++i) {
+      before += (i < w) ? s_warp[i] : 0;
+      total += s_warp[i];
     }
     int pos = before + incl - mine;
 #pragma unroll
@@ -1590,8 +1597,9 @@ int launch_clean(const Params& P, int n_batch, cudaStream_t s, cudaEvent_t* ev) 
   k_clean_fill<<<g, 256, 0, s>>>(P);
   LST_EV(3);
   k_clean_mark<<<dim3(blocks_per_event((5 * P.L.cap_t5 + 255) / 256, n_batch, 8), (unsigned)n_batch), 256, 0, s>>>(P);
+  k_clean_list<<<dim3(1, (unsigned)n_batch), 1024, 0, s>>>(P);
   LST_EV(4);
-  return 5;
+  return 6;
 }
 
 int launch_fetch_direct(const Params& P, const OutTable& T, int kind, int n_batch, cudaStream_t s) {
