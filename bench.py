@@ -119,11 +119,25 @@ def whole_job_events_per_s(world: int, steps: int, total_ms: float) -> float:
     return world * N_EVENTS * steps / (total_ms * 1e-3)
 
 
-def make_events(seed0: int, n: int):
+def make_map(geom, device=None):
+    """The module map (rule [B]), the step before the path: our arm builds it with the library's own GPU
+    builder (lst_build_module_map), the reference arm with the oracle's (device=None)."""
+    from paper_2207_08207_b200 import synth
+    mg = synth.map_geometry(geom)
+    margs = (mg["layer"], mg["phi"], mg["rho"], mg["gap"], mg["hw"], mg["zlo"], mg["zhi"])
+    if device is None:
+        from oracle import oracle
+        offs, tg = oracle.load("f64").build_map(*margs)
+    else:
+        from paper_2207_08207_b200 import lst
+        offs, tg, _ = lst.build_module_map(*margs, device=device)
+    return synth.ModuleMap(geom.n_modules, offs, tg)
+
+
+def make_events(seed0: int, n: int, device=None):
     from paper_2207_08207_b200 import synth
     geom = synth.make_geometry()
-    mmap = synth.make_module_map(geom)
-    return geom, mmap, [synth.generate_event(geom, 1, seed0 + i) for i in range(n)]
+    return geom, make_map(geom, device), [synth.generate_event(geom, 1, seed0 + i) for i in range(n)]
 
 
 # ------------------------------------------------------------------------------------------
@@ -188,7 +202,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = torch.device("cuda", local)
 
-    geom, mmap, events = make_events(rank_seed0(rank), N_EVENTS)
+    geom, mmap, events = make_events(rank_seed0(rank), N_EVENTS, device=local)
     per_stream = N_EVENTS // N_STREAMS
     cfg = lst.default_config()
     cfg.device, cfg.n_slots = local, 2 * N_EVENTS          # second half: the other buffer set of the end-to-end pipeline
@@ -522,7 +536,7 @@ def run_sweep(args):
     from paper_2207_08207_b200 import lst, synth
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
     geom = synth.make_geometry()
-    mmap = synth.make_module_map(geom)
+    mmap = make_map(geom, device=0)
     peaks = measured_peaks()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     st = torch.cuda.Stream()

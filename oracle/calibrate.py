@@ -38,7 +38,8 @@ def one_particle(truth_rows, pt):
 def main():
     o = oracle.load("f32")
     geom = synth.make_geometry()
-    mm = synth.make_module_map(geom)
+    mg = synth.map_geometry(geom)                # the oracle's own module map [B]
+    mm = synth.ModuleMap(geom.n_modules, *o.build_map(mg["layer"], mg["phi"], mg["rho"], mg["gap"], mg["hw"], mg["zlo"], mg["zhi"]))
     cfg = o.default_config()
     for i in range(4):
         cfg.t3_chi2rz_max[i] = HUGE

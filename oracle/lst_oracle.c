@@ -23,13 +23,16 @@
  *                                formulas against closed forms / library fits tightly, and
  *                                to measure how ill-conditioned a quantity is in fp32.
  *
- * Pins (tests/test_oracle_pins.py): helix closed forms (P1, P2), brute force vs map (P3),
- * single-helix recovery (P4), library least-squares / circumradius reductions (P5),
- * chi2 statistics (P6), symmetries (P7), threshold flips (P8), structure (P9), truth (P10);
+ * Pins (tests/test_oracle_pins.py, tests/test_oracle_events.py): helix closed forms (P1, P2), brute force vs
+ * map (P3), single-helix recovery (P4), library least-squares / circumradius reductions (P5),
+ * chi2 statistics (P6), symmetries (P7), threshold flips (P8), structure (P9), truth (P10), M3 closed form
+ * and flip (P18), per-layer threshold indices (P19), the Q5 cut (P20);
  * duplicate cleaning [D] (tests/test_oracle_clean.py): single helix (P11), set-based restatement (P12),
  * implied properties and order independence (P13), truth statistics (P14); module-map builder [B]
- * (tests/test_oracle_map.py): simulated tracks stay inside the map (P15), the test-side generator (P16),
- * symmetries and monotonicity (P17).
+ * (tests/test_oracle_map.py): simulated tracks stay inside the map (P15), the test-side generator (P16: a
+ * restatement, pins nothing on its own), symmetries and monotonicity (P17), two-module special cases by
+ * similar triangles / arc lengths (P18), helices propagated from the module edges: soundness and tightness (P19).
+ * Every pin was checked to bite by mutating this file (a dropped term, a wrong index, a removed cut).
  * The paper prints no worked numerical example, so no value is pinned to the paper itself.
  */
 #include <math.h>

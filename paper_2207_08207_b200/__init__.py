@@ -2,8 +2,9 @@
 
 Sub-modules
 -----------
-synth   seeded synthetic geometry / module map / event generators (numpy only, none of
-        the method's arithmetic; shared by the oracle tests and the CUDA path's tests).
+synth   seeded synthetic geometry / event generators (numpy only, none of the method's
+        arithmetic -- the module map is built by ``lst.build_module_map`` --; shared by
+        the oracle tests and the CUDA path's tests).
 lst     thin ctypes binding over the C-ABI library ``liblst.so`` (include/lst.h).
 build   nvcc build of ``csrc/`` for sm_100a.
 

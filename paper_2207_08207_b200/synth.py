@@ -1,10 +1,13 @@
-"""Seeded synthetic inputs for the LST hot path: detector geometry, module map, events.
+"""Seeded synthetic inputs for the LST hot path: detector geometry and events.
 
 This module produces INPUTS only (BASELINE.json ``configs[0..4]``; recipe in DESIGN.md
 section "Input recipe", formulas from SURVEY.md Appendix A).  It holds none of the
-method's arithmetic (no mini-doublet / segment / triplet / quintuplet selection): the
-CPU oracle and the CUDA path (``csrc/``) both receive what is generated here as
-plain arrays, and neither of them is imported from here.
+method's arithmetic: no mini-doublet / segment / triplet / quintuplet selection, no
+duplicate cleaning, and no module-map derivation (rule [B] is a step of the method: the
+CUDA library builds the map with ``lst_build_module_map``, the oracle with ``lsto_build_map``,
+and the tests keep a third, numpy statement of it in ``tests/mapgen.py``).  The CPU oracle
+and the CUDA path (``csrc/``) both receive what is generated here as plain arrays, and
+neither of them is imported from here.
 
 The paper measures on CMS tt-bar + PU200 simulation, which is not
 available; these events stand in for it (same gross shape: barrel pT modules, soft
@@ -88,51 +91,14 @@ def _wrap(a):
 
 
 # ----------------------------------------------------------------------------------------
-# Module map (helices at the pT threshold from the module edges -> list of
-# adjacent-layer modules they can reach). CSR, rows sorted ascending.
+# Module map container (module -> connectable modules of the next layer). CSR, rows
+# sorted ascending.  The derivation itself is not here (see the module docstring).
 # ----------------------------------------------------------------------------------------
 @dataclasses.dataclass(frozen=True)
 class ModuleMap:
     n_modules: int
     row_offsets: np.ndarray   # int32 [n_modules+1]
     targets: np.ndarray       # int32 [row_offsets[-1]]
-
-
-def make_module_map(geom: Geometry) -> ModuleMap:
-    r_m = MAP_PT / (K_GEV_PER_T_CM * B_TESLA)
-    rows = [[] for _ in range(geom.n_modules)]
-    for l in range(N_LAYERS - 1):
-        r_lo = LAYER_R[l] - SENSOR_GAP[l] / 2
-        r_hi = math.hypot(LAYER_R[l] + SENSOR_GAP[l] / 2, MODULE_HALF_W)
-        rp_lo = LAYER_R[l + 1] - SENSOR_GAP[l + 1] / 2
-        rp_hi = math.hypot(LAYER_R[l + 1] + SENSOR_GAP[l + 1] / 2, MODULE_HALF_W)
-        a_out = math.asin(min(1.0, rp_hi / (2 * r_m)))
-        a_in = math.asin(r_lo / (2 * r_m))
-        dphi_max = a_out - a_in
-        h_a = math.atan(MODULE_HALF_W / r_lo)
-        h_b = math.atan(MODULE_HALF_W / rp_lo)
-        phi_tol = h_a + h_b + dphi_max + MAP_PAD_PHI
-        ratios = (rp_lo / r_hi, a_out / a_in)
-        n_a, n_b = int(geom.n_phi[l]), int(geom.n_phi[l + 1])
-        phi_a = 2 * np.pi * np.arange(n_a) / n_a
-        phi_b = 2 * np.pi * np.arange(n_b) / n_b
-        phi_ok = np.abs(_wrap(phi_b[None, :] - phi_a[:, None])) <= phi_tol       # [n_a, n_b]
-        for j in range(N_RINGS):
-            za = (-Z_MAX + RING_LEN * j - MAP_PAD_Z, -Z_MAX + RING_LEN * (j + 1) + MAP_PAD_Z)
-            zs = [z0 + (z - z0) * rt for z0 in (-MAP_Z0, MAP_Z0) for z in za for rt in ratios]
-            z_lo, z_hi = min(zs), max(zs)
-            ring_lo = -Z_MAX + RING_LEN * np.arange(N_RINGS)
-            rings_b = np.nonzero((z_hi >= ring_lo) & (z_lo <= ring_lo + RING_LEN))[0]
-            for i in range(n_a):
-                src = int(geom.base[l]) + j * n_a + i
-                ib = np.nonzero(phi_ok[i])[0]
-                t = (int(geom.base[l + 1]) + rings_b[:, None] * n_b + ib[None, :]).ravel()
-                rows[src] = np.sort(t)
-    counts = np.array([len(r) for r in rows], dtype=np.int64)
-    row_offsets = np.concatenate([[0], np.cumsum(counts)]).astype(np.int32)
-    targets = (np.concatenate([np.asarray(r, dtype=np.int32) for r in rows if len(r)])
-               if counts.sum() else np.zeros(0, np.int32))
-    return ModuleMap(geom.n_modules, row_offsets, targets.astype(np.int32))
 
 
 def map_geometry(geom: Geometry) -> dict:
@@ -205,7 +171,7 @@ def propagate(geom: Geometry, z0, q, pt, phi0, eta, du=None, dz=None):
                 x, y, z = helix_point(pt, q, phi0, eta, z0, theta)
                 u = -x * np.sin(Phi) + y * np.cos(Phi)
                 ok &= (np.abs(u) <= MODULE_HALF_W) & (z >= -Z_MAX) & (z < Z_MAX)
-                ring = np.floor((z + Z_MAX) / RING_LEN).astype(np.int64)
+                ring = np.minimum(np.floor((z + Z_MAX) / RING_LEN).astype(np.int64), N_RINGS - 1)   # z one ulp below Z_MAX
                 if du is not None:
                     u = u + du[:, l, side, c]
                     z = z + dz[:, l, side, c]

@@ -7,6 +7,9 @@ import pytest
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
+HERE = os.path.dirname(os.path.abspath(__file__))
+if HERE not in sys.path:
+    sys.path.insert(0, HERE)
 
 
 def pytest_configure(config):
@@ -21,8 +24,9 @@ def geom():
 
 @pytest.fixture(scope="session")
 def mmap(geom):
-    from paper_2207_08207_b200 import synth
-    return synth.make_module_map(geom)
+    """The module map used as INPUT by the oracle and GPU tests: the test-side generator (tests/mapgen.py)."""
+    import mapgen
+    return mapgen.make_module_map(geom)
 
 
 @pytest.fixture(scope="session")

@@ -23,8 +23,9 @@ CASES = (("C0", 0, 0, None), ("C0", 0, 1, None), ("C1", 1, 0, None), ("C1small",
 
 def lines():
     geom = synth.make_geometry()
-    mmap = synth.make_module_map(geom)
     o = oracle.load("f32")
+    mg = synth.map_geometry(geom)                # the oracle's own module map [B] (69 630 connections on this geometry)
+    mmap = synth.ModuleMap(geom.n_modules, *o.build_map(mg["layer"], mg["phi"], mg["rho"], mg["gap"], mg["hw"], mg["zlo"], mg["zhi"]))
     yield "# case config seed n_particles | hits | MD LS T3 T5 | candidates MD LS T3 T5 | kept by [D] (K = 7) | sha256(sorted T5 hit tuples)[:16]"
     for name, cfg, seed, npart in CASES:
         ev = synth.generate_event(geom, cfg, seed) if npart is None else synth.generate_event(geom, cfg, seed, n_particles=npart)

@@ -227,3 +227,67 @@ def test_golden_oracle_counts():
         key = ln.split(" |")[0]
         if key in now:
             assert now[key] == ln, (now[key], ln)
+
+
+# ----------------------------------------------------------------------------------------
+# P19: per-layer threshold indices ("for different categories", PAPER.md:55) and P20: the Q5 cut
+# ----------------------------------------------------------------------------------------
+@pytest.fixture(scope="module")
+def c1small(geom, o32, run_oracle):
+    ev = synth.generate_event(geom, 1, 5, n_particles=1200)
+    return ev, run_oracle(o32, ev)
+
+
+def _layers(geom, ev, hits):
+    """[n][k] hit tuples -> [n][k/2] layer of every MD of the object."""
+    return geom.layer[ev.module[np.asarray(hits)[:, ::2]]].astype(int)
+
+
+INDEX_CASES = (
+    [("md_dz_res", l, 1, "md", "any") for l in range(6)] +           # M3: md_dz_res[layer]
+    [("md_thr", l, 1, "md", "any") for l in range(6)] +              # M2: md_cos_eps / md_sin_eps[layer]
+    [("seg_z0_max", l, 2, "seg", "first") for l in range(5)] +       # S3: by inner layer
+    [("md_eps", l, 2, "seg", "any") for l in range(6)] +             # S4: [inner layer] for the inner MD, [inner + 1] for the outer
+    [("t3_chi2rz_max", l, 3, "t3", "first") for l in range(4)] +     # T3: by innermost layer
+    [("t5_chi2rz_max", l, 4, "t5", "first") for l in range(2)])      # Q3: by innermost layer
+
+
+@pytest.mark.parametrize("field,l,stages,cls,who", INDEX_CASES)
+def test_p19_threshold_entry_l_removes_exactly_the_objects_of_layer_l(geom, o32, run_oracle, c1small, field, l, stages, cls, who):
+    """Closing ONE entry of a per-layer threshold array removes exactly the objects that the SPEC says read that entry
+    -- those whose innermost layer is l ("first"), or any of whose mini-doublets sits in layer l ("any": an MD in its own
+    layer; S4 reads md_eps[inner layer] for the inner and md_eps[inner layer + 1] for the outer mini-doublet) -- and leaves
+    every other object of that class in place.  An off-by-one or a constant index in the oracle fails this."""
+    ev, base = c1small
+    cfg = o32.default_config()
+    if field == "md_thr":                         # SINTHR = t cosE + sqrt(1 - t^2) sinE < 0: nothing passes M2
+        cfg.md_cos_eps[l], cfg.md_sin_eps[l] = 0.0, -1.0
+    else:
+        getattr(cfg, field)[l] = -1.0e30 if field == "md_dz_res" else -1.0
+    got = run_oracle(o32, ev, stages=stages, cfg=cfg)
+    name = {"md": "md_hits", "seg": "seg_hits", "t3": "t3_hits", "t5": "t5_hits"}[cls]
+    before = getattr(base, name)()
+    lay = _layers(geom, ev, before)
+    hit = (lay[:, 0] == l) if who == "first" else (lay == l).any(1)
+    assert 0 < hit.sum() < len(before), (field, l, hit.sum())
+    assert as_set(getattr(got, name)()) == as_set(before[~hit]), (field, l)
+
+
+def test_p20_q5_fitted_curvature_cut(geom, o32, run_oracle):
+    """Q5 (DESIGN.md SPEC [Q] step 4): |kFit| <= t5_kappa_max.  kFit of a noiseless helix is -q/R = -q k B / pT (pin P1), so with
+    the threshold moved to the curvature of a 2 GeV track (and the other quintuplet cuts left as they are: they pass
+    exact helices) both quintuplets of every 1.5 GeV helix disappear and both of every 3 GeV helix stay."""
+    kb = synth.K_GEV_PER_T_CM * synth.B_TESLA
+    cfg = o32.default_config()
+    cfg.t5_kappa_max = kb / 2.0
+    rng = np.random.default_rng(20)
+    done = {1.5: 0, 3.0: 0}
+    while min(done.values()) < 12:
+        pt = 1.5 if done[1.5] <= done[3.0] else 3.0
+        q, phi0, eta, z0 = rng.choice([-1.0, 1.0]), rng.uniform(-np.pi, np.pi), rng.uniform(-0.6, 0.6), rng.normal(0, 4.0)
+        ev = synth.single_helix_event(geom, pt, q, phi0, eta, z0)
+        if run_oracle(o32, ev).counts != [6, 5, 4, 2]:
+            continue                               # crosses an overlap or leaves the barrel: not the clean case
+        r = run_oracle(o32, ev, cfg=cfg)
+        assert r.counts[:3] == [6, 5, 4] and r.counts[3] == (0 if pt == 1.5 else 2), (pt, q, r.counts)
+        done[pt] += 1

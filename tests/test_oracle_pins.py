@@ -261,3 +261,45 @@ def test_boundary_semantics(o32):
     cfg.seg_z0_max[0] = float(np.nextafter(np.float32(abs(mar[2])), np.float32(0)))
     assert not o32.seg_cut(0, inner, (35.57, 0.0, 11.0, 35.57, 35.83, 0.0), cfg=cfg)[0]
     assert z0 == z0
+
+
+# ----------------------------------------------------------------------------------------
+# P18: M3 (the luminous-region term of the mini-doublet cut) in closed form + flip
+# ----------------------------------------------------------------------------------------
+def test_p18_m3_closed_form_and_flip(geom, o64):
+    """M3 ("error terms ... take into account ... the luminous region size"; DESIGN.md SPEC [M] step 3) on
+    noiseless helices, fp64 build.  A helix from (0, 0, z0) has z(r) = z0 + sinh(eta) s(r) with the arc length
+    s(r) = 2R asin(r / 2R), so both sides of the inequality are known from the helix parameters and the two radii:
+        lhs = |sinh(eta) (s_u - s_l) - (z0 + sinh(eta) s_l) (r_u - r_l) / r_l|,   rhs = z_lum |r_u - r_l| / r_l + 4 sqrt2 sigma_z[L].
+    Flip: with md_dz_res = 0 the cut passes iff z0 lies within z_lum of a/b (a = sinh(eta) (s_u - s_l - s_l dr / r_l),
+    b = dr / r_l): helices displaced to a/b +- z_lum (1 -+ 1e-3) pass, to a/b +- z_lum (1 +- 1e-3) fail."""
+    rng = np.random.default_rng(18)
+    z_lum = 15.0
+    cfg0 = o64.default_config()
+    for l in range(6):
+        cfg0.md_dz_res[l] = 0.0
+    n_flip = 0
+    for _ in range(40):
+        h, mds = clean_helix(geom, rng, eta_max=0.5)
+        R, sh, z0 = h["R"], math.sinh(h["eta"]), h["z0"]
+        for l in range(6):
+            (xl, yl, _), (xu, yu, _) = mds[l][0], mds[l][1]
+            rl, ru = math.hypot(xl, yl), math.hypot(xu, yu)
+            sl, su = arc(rl, R), arc(ru, R)
+            ok, _, mar = o64.md_cut(l, mds[l][0], mds[l][1])
+            assert mar[2] == pytest.approx(abs(sh * (su - sl) - (z0 + sh * sl) * (ru - rl) / rl), abs=1e-9)
+            assert mar[3] == pytest.approx(z_lum * abs(ru - rl) / rl + 4.0 * math.sqrt(2.0) * SIG_Z[l], rel=1e-7)   # the constant is typed as the nearest binary32
+            assert ok == (mar[2] <= mar[3])
+            # flip: the same trajectory in x-y displaced along the beam line
+            b = (ru - rl) / rl
+            centre = sh * (su - sl - sl * b) / b
+            for edge in (+1.0, -1.0):
+                for inside in (True, False):
+                    z0n = centre + edge * z_lum * (1.0 - 1e-3 if inside else 1.0 + 1e-3)
+                    lo = (xl, yl, z0n + sh * sl)
+                    up = (xu, yu, z0n + sh * su)
+                    ok, _, mar = o64.md_cut(l, lo, up, cfg=cfg0)
+                    assert ok == inside, (l, edge, inside, mar)
+                    assert mar[2] / mar[3] == pytest.approx(1.0 - 1e-3 if inside else 1.0 + 1e-3, rel=1e-6)
+                    n_flip += 1
+    assert n_flip == 40 * 6 * 4
