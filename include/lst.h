@@ -117,7 +117,9 @@ typedef struct {
   int32_t timing;     /* != 0: record CUDA events around every kernel (lst_get_stats.stage_ms /
                          kernel_ms; for a batch they are kept on its first slot) */
   int32_t t5_dup_min_shared; /* [D] D4: quintuplets sharing at least this many of their 10 original hits
-                         are duplicates (7) */
+                         are duplicates (7).  Accepted range 6 .. 10 (lst_create returns LST_ERR_ARG otherwise): the
+                         stage finds partners through a common mini-doublet, which >= 6 common hits imply and
+                         <= 5 do not */
 } lst_config;
 
 /* Fills *cfg with the frozen SPEC constants, device 0, 4 slots and capacities that hold the

@@ -202,7 +202,9 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
   if (n <= 0 || n > (1 << 24) || m->n_modules != n || !g->layer || !g->phi || !m->row_offsets) return LST_ERR_ARG;
   /* object indices are packed into 26 bits, module ids into 24 bits by the stage kernels */
   if (cfg.cap_hits > kMaxCap || cfg.cap_md > kMaxCap || cfg.cap_seg > kMaxCap || cfg.cap_t3 > kMaxCap || cfg.cap_t5 > kMaxCap) return LST_ERR_ARG;
-  if (cfg.t5_dup_min_shared < 1 || cfg.t5_dup_min_shared > 10) return LST_ERR_ARG;
+  /* [D]: partners are found through a common mini-doublet, which two quintuplets sharing >= 6 of their 10 hits always
+     have (five common layers with one common hit each give at most 5): smaller thresholds are refused, not approximated */
+  if (cfg.t5_dup_min_shared < 6 || cfg.t5_dup_min_shared > 10) return LST_ERR_ARG;
   if (cfg.n_slots < 1 || cfg.cap_hits < 1 || cfg.cap_md < 1 || cfg.cap_seg < 1 || cfg.cap_t3 < 1 || cfg.cap_t5 < 1) return LST_ERR_ARG;
   for (int i = 0; i < n; ++i)
     if (g->layer[i] < 0 || g->layer[i] >= LST_N_LAYERS) return LST_ERR_ARG;

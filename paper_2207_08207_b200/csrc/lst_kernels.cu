@@ -1216,8 +1216,9 @@ __global__ void __launch_bounds__(kWarps * 32, 4) k_t5(const __grid_constant__ P
 
 // ------------------------------------------------------------------------------------------
 // [D] duplicate cleaning of quintuplets (DESIGN.md section 1 [D]; optional stage LST_CLEAN).
-// Two quintuplets that share >= 7 of their 10 original hits share a mini-doublet (a mini-doublet is a
-// pair of hits of one module: without a common MD at most one hit per common layer can coincide), so the
+// Two quintuplets that share >= 6 of their 10 original hits share a mini-doublet (a mini-doublet is a
+// pair of hits of one module: without a common MD at most one hit per common layer can coincide, 5 in all;
+// lst_create refuses t5_dup_min_shared < 6), so the
 // partners of a quintuplet are found through an MD -> quintuplets incidence table (counting sort over the
 // MDs: count, scan, fill), and every (quintuplet, partner) pair goes through the exact rule D2-D4.
 // The result does not depend on the order of the incidence lists: D4 is an "exists" over the partners.

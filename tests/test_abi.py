@@ -76,6 +76,9 @@ def test_create_rejects_bad_arguments_before_any_cuda_call(lst_mod, geom, mmap):
     assert status(row_offsets=bad_r) == lst_mod.ERR_ARG
     cfg = lst_mod.default_config(); cfg.n_slots = 0
     assert status(config=cfg) == lst_mod.ERR_ARG
+    for k in (0, 5, 11):                                           # [D]: thresholds outside 6 .. 10 are refused (include/lst.h)
+        cfg = lst_mod.default_config(); cfg.t5_dup_min_shared = k
+        assert status(config=cfg) == lst_mod.ERR_ARG, k
     assert status(phi=None) == lst_mod.ERR_ARG                     # module azimuths are required
     bad_phi = geom.phi.copy(); bad_phi[7] = np.nan
     assert status(phi=bad_phi) == lst_mod.ERR_ARG
