@@ -18,7 +18,7 @@ LIB = os.path.join(HERE, "liblst.so")
 SOURCES = ["lst_kernels.cu", "lst_api.cu", "lst_map.cu"]
 HEADERS = ["lst_cuts.cuh", "lst_device.cuh", os.path.join("..", "..", "include", "lst.h")]
 NVCC_FLAGS = [
-    "-O3", "-std=c++17", *(["-DLST_DEBUG"] if os.environ.get("LST_DEBUG") else []), "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+    "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
     "--fmad=false", "--prec-div=true", "--prec-sqrt=true", "--ftz=false",
     "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "-shared", "-cudart", "static",
 ]

@@ -27,9 +27,6 @@
 //
 // blockIdx.y = index of the event within the batch (lst_run_batch): all events of a batch go
 // through one launch per kernel.
-#include <cstdio>
-#include <cstdlib>
-
 #include "lst_device.cuh"
 
 namespace lst {
@@ -913,315 +910,6 @@ __global__ void __launch_bounds__(kSegWarps * 32, 7) k_seg(const __grid_constant
 }
 
 // ------------------------------------------------------------------------------------------
-// a2: segments, module-owner walk.  Owners are still handed out as chunks of 32 consecutive inner
-// MDs (ticket order = CSR order), but a chunk is walked PIECE by piece, a piece being the MDs of the chunk that sit in
-// one module A (MDs are stored by module, so a piece is a lane range; a module with more than 32 MDs is split over
-// chunks, i.e. over warps).  Everything that depends on A only is done once per piece instead of once per MD:
-//   stage  the row of the module map: per connected module B its MD slice (first, count) and the azimuth offset
-//          between the two module frames, to shared memory; the slices of the row form the piece's OUTER LIST;
-//   scan   the outer list in tiles of 32: lane = one outer MD, its azimuth key (moved into A's frame) in a register;
-//          the owners' windows are broadcast from shared memory one after the other and each lane collects a bit
-//          mask of the owners whose window holds it -- a flat compare, no search, no dependent load, no branch;
-//   queue  the (owner, outer MD) pairs of the masks -> closed-form pre-filter on full tiles -> exact SPEC selection
-//          on full tiles of survivors -> stash, as before.
-// For one owner the outer MDs are met in ascending order whatever the interleaving between owners, so a segment's
-// place in the CSR output is  chunk base + (segments of the owners before it) + (its arrival rank within its owner),
-// which is what the stash keeps.
-// ------------------------------------------------------------------------------------------
-constexpr int kSegQ = 128;       // slots of the candidate queue (a push adds <= kSegPush, a drain leaves < 32)
-constexpr int kSegPush = 96;
-struct Seg2Warp {
-  float4 a4[32];
-  float2 aux[32];
-  float lo[32], hi[32];          // the owner's azimuth window in its own module frame: key + dlo, key + dhi (lo > hi: nothing passes)
-  int layer[32];
-  int tfirst[kMaxRow];           // per connected module of the piece: first MD,
-  int toff[kMaxRow + 1];         //   offset of its slice in the piece's outer list (toff[nt] = length of the list),
-  float tdphi[kMaxRow];          //   azimuth(A's normal) - azimuth(its normal)
-  int2 cq[kSegQ], dq[kQueue];    // window candidates / pre-filter survivors: (owner lane, outer MD)
-  int cnt[2][32], ex[32], cur[32];
-  int stI[2][kSegStash], stR[2][kSegStash];
-  float2 stV[2][kSegStash];
-};
-
-// The cut variables of S3 / S4 in fast arithmetic straight from the two anchors (|error| ~ 1e-6, from the cancellation
-// in the cross product and the fast reciprocal square root / division), tested with slack that is orders of magnitude
-// above it (0.1 % + 0.5 mm on z0; 2e-3 on thresholds of 0.057 / 0.092): necessary conditions only, the exact
-// selection keeps the last word.
-__device__ __forceinline__ bool seg_prefilter2(const Cuts& c, int layer_in, const float4& ai, const float2& auxi,
-                                               const float4& ao, const float2& auxo) {
-  const float dr = ao.w - ai.w;
-  const float z0 = ai.z - ai.w * __fdividef(ao.z - ai.z, dr);
-  if (fabsf(z0) > c.seg_z0_max[layer_in] * 1.001f + 0.05f) return false;      // S3 (a NaN goes on to the exact test)
-  const float dx = ao.x - ai.x, dy = ao.y - ai.y;
-  const float cross = ai.x * dy - ai.y * dx;
-  const float n2 = (ai.w * ai.w) * (dx * dx + dy * dy);
-  if (!(n2 > 0.0f)) return true;
-  const float q = __fdividef(cross * rsqrtf(n2), ao.w);                       // sinS / r_o
-  if (fabsf(auxo.y - q * auxo.x) > c.md_eps[layer_in + 1] + 2e-3f) return false;   // S4, outer mini-doublet
-  return !(fabsf(auxi.y - q * auxi.x) > c.md_eps[layer_in] + 2e-3f);               // S4, inner mini-doublet
-}
-
-// modA / row0 / nt: module of this lane's MD and its row of the module map; wbits: bits of |key| + window reach (0 if no
-// window); okw: the lane has a window.  nValid lanes hold MDs (a prefix of the warp).
-template <bool DIRECT>
-__device__ __forceinline__ int seg2_walk(const Params& P, const Slot& S, Seg2Warp& sh, int buf, int modA, int row0, int nt,
-                                         int wbits, bool okw, int nValid, int i0, int base, unsigned long long& space,
-                                         unsigned long long& evals) {
-  const float4* anchor = S.md_anchor();
-  const float2* aux = S.md_aux();
-  const float* mkey = S.md_key();
-  const int4* mod_info = S.mod_info();
-  const int lane = (int)lane_id();
-  int* ctr = DIRECT ? sh.cur : sh.cnt[buf];
-  int running = 0;
-  int ch = 0, ct = 0, dh = 0, dt = 0;   // heads / tails of the candidate and the survivor queue
-
-  // exact selection on up to 32 survivors
-  auto drainD = [&](bool all) {
-    while (dt - dh >= 32 || (all && dt > dh)) {
-      __syncwarp();
-      const int n = min(32, dt - dh);
-      bool pass = false;
-      SegOut so;
-      int ol = 0, o = 0;
-      if (lane < n) {
-        const int2 it = sh.dq[(dh + lane) & (kQueue - 1)];
-        ol = it.x; o = it.y;
-        pass = seg_select(P.cuts, sh.layer[ol], sh.a4[ol], sh.aux[ol], anchor[o], aux[o], so);
-      }
-      const unsigned bal = __ballot_sync(kFull, pass);
-      if (pass) {
-        // arrival rank within the owner: lanes of one owner sit in ascending order of the outer MD
-        const unsigned peers = __match_any_sync(bal, ol);
-        const int r = ctr[ol] + __popc(peers & lanemask_lt());
-        __syncwarp(bal);
-        if ((peers & lanemask_lt()) == 0) ctr[ol] = r + __popc(peers);
-        if (!DIRECT) {
-          const int slot = running + __popc(bal & lanemask_lt());
-          if (slot < kSegStash) { sh.stI[buf][slot] = (ol << 26) | o; sh.stR[buf][slot] = r; sh.stV[buf][slot] = make_float2(so.sinS, so.z0); }
-        } else {
-          seg_emit(P, S, base + sh.ex[ol] + r, i0 + ol, o, so.sinS, so.z0);
-        }
-      }
-      running += __popc(bal);
-      dh += n;
-      __syncwarp();
-    }
-  };
-  // pre-filter on up to 32 window candidates
-  auto drainC = [&](bool all) {
-    while (ct - ch >= 32 || (all && ct > ch)) {
-      __syncwarp();
-      const int n = min(32, ct - ch);
-      bool keep = false;
-      int2 it = make_int2(0, 0);
-      if (lane < n) {
-        it = sh.cq[(ch + lane) & (kSegQ - 1)];
-        keep = seg_prefilter2(P.cuts, sh.layer[it.x], sh.a4[it.x], sh.aux[it.x], anchor[it.y], aux[it.y]);
-      }
-      const unsigned bal = __ballot_sync(kFull, keep);
-      if (keep) sh.dq[(dt + __popc(bal & lanemask_lt())) & (kQueue - 1)] = it;
-      dt += __popc(bal);
-      ch += n;
-      drainD(false);
-      __syncwarp();
-    }
-  };
-
-  const int modPrev = __shfl_up_sync(kFull, modA, 1);
-  unsigned heads = __ballot_sync(kFull, lane < nValid && (lane == 0 || modA != modPrev));
-  while (heads) {
-    const int la = __ffs(heads) - 1;
-    heads &= heads - 1;
-    const int lb = heads ? __ffs(heads) - 1 : nValid;
-    const int pr0 = __shfl_sync(kFull, row0, la), pnt = __shfl_sync(kFull, nt, la);
-    if (pnt == 0) continue;
-    // stage the row: MD slices of the connected modules, their offsets in the outer list, the frame offsets
-    int nO = 0, dbits = 0;
-    for (int tb = 0; tb < pnt; tb += 32) {
-      const int t = tb + lane;
-      int first = 0, c = 0;
-      float dphi = 0.0f;
-      if (t < pnt) {
-        const int4 info = mod_info[P.map_targets[pr0 + t]];
-        dphi = P.map_dphi[pr0 + t];
-        first = info.x;
-        c = info.y - info.x;
-      }
-      int tot;
-      const int off = warp_excl_scan(c, tot);
-      if (t < pnt) { sh.tfirst[t] = first; sh.toff[t] = nO + off; sh.tdphi[t] = dphi; }
-      dbits = max(dbits, __reduce_max_sync(kFull, __float_as_int(fabsf(dphi))));
-      nO += tot;
-    }
-    if (lane == 0) sh.toff[pnt] = nO;
-    if (!DIRECT && lane == 0) space += (unsigned long long)(lb - la) * (unsigned long long)nO;
-    if (nO == 0) continue;
-    const bool mine_piece = lane >= la && lane < lb;
-    // azimuth wrap possible for some (owner, connected module) of the piece (never with a sane geometry): every pair
-    // of an owner that has a window becomes a candidate
-    const int reach = __reduce_max_sync(kFull, mine_piece ? wbits : 0);
-    if (!(__int_as_float(reach) + __int_as_float(dbits) < 3.0f) && mine_piece) {
-      sh.lo[lane] = okw ? -3.0e38f : 1.0f;
-      sh.hi[lane] = okw ? 3.0e38f : -1.0f;
-    }
-    __syncwarp();
-    int t0 = 0;   // connected module that holds position p0 of the outer list
-    for (int p0 = 0; p0 < nO; p0 += 32) {
-      const int p = p0 + lane;
-      int t = t0, tn = t0;
-      for (int j = t0 + 1; j < pnt; ++j) {
-        const int oj = sh.toff[j];
-        if (oj > p0 + 32) break;
-        t += (oj <= p);
-        tn += 1;
-      }
-      t0 = tn;
-      int o = 0;
-      float rk = 0.0f;
-      if (p < nO) {
-        o = sh.tfirst[t] + (p - sh.toff[t]);
-#ifdef LST_DEBUG
-        if (t < 0 || t >= pnt || o < 0 || o >= S.hdr()->n[LST_MD_]) { printf("seg2: bad o %d t %d p %d nO %d pnt %d la %d lb %d toff %d first %d\n", o, t, p, nO, pnt, la, lb, sh.toff[t < 0 ? 0 : t], sh.tfirst[t < 0 ? 0 : t]); o = 0; }
-#endif
-        rk = mkey[o] - sh.tdphi[t];
-      }
-      unsigned mine = 0;
-#pragma unroll 4
-      for (int i = la; i < lb; ++i)
-        if (rk >= sh.lo[i] && rk <= sh.hi[i]) mine |= 1u << i;
-      if (p >= nO) mine = 0;
-      int tot;
-      const int off = warp_excl_scan(__popc(mine), tot);
-      if (tot == 0) continue;
-      if (!DIRECT && lane == 0) evals += (unsigned long long)tot;
-      int j = 0;
-      for (int done = 0; done < tot; done += kSegPush) {
-        while (mine && off + j < done + kSegPush) {
-          const int b = __ffs(mine) - 1;
-          mine &= mine - 1;
-          sh.cq[(ct + off + j - done) & (kSegQ - 1)] = make_int2(b, o);
-          ++j;
-        }
-        ct += min(kSegPush, tot - done);
-        drainC(false);
-      }
-    }
-  }
-  drainC(true);
-  drainD(true);
-  return running;
-}
-
-__global__ void __launch_bounds__(kSegWarps * 32, 6) k_seg_v2(const __grid_constant__ Params P) {
-  __shared__ Seg2Warp shw[kSegWarps];
-  __shared__ float s_rMinO[6], s_rMaxO[6];
-  Slot S(P, blockIdx.y);
-  SlotHeader* H = S.hdr();
-  const int cap = P.L.cap_seg;
-  const int nMD = H->n[LST_MD_];
-  const int nChunks = (nMD + kChunk - 1) / kChunk;
-  const int lane = (int)lane_id();
-  Seg2Warp& sh = shw[threadIdx.x >> 5];
-  if (threadIdx.x < 6) {
-    s_rMinO[threadIdx.x] = r_min_of(H, 0, threadIdx.x);
-    s_rMaxO[threadIdx.x] = r_max_of(H, 0, threadIdx.x);
-  }
-  __syncthreads();
-  int* seg_start = S.seg_start();
-  unsigned long long* status = S.lb(LST_SEG_);
-  unsigned long long space = 0, evals = 0;
-
-  // per-owner offsets of chunk C (buffer b) from its counts, left in sh.ex; returns the lane's own
-  auto offsets = [&](int b) {
-    int tot;
-    const int ex = warp_excl_scan(sh.cnt[b][lane], tot);
-    sh.ex[lane] = ex;
-    __syncwarp();
-    return ex;
-  };
-  auto finish = [&](int C, int b, int total, int base, int ex, bool from_stash) {
-    const int i0 = C * kChunk, i = i0 + lane;
-    if (from_stash)
-      for (int t = lane; t < total; t += 32) {
-        const int v = sh.stI[b][t], ol = (int)((unsigned)v >> 26);
-        const float2 f = sh.stV[b][t];
-        seg_emit(P, S, base + sh.ex[ol] + sh.stR[b][t], i0 + ol, v & (kMaxCap - 1), f.x, f.y);
-      }
-    if (i < nMD) seg_start[i] = min(base + ex, cap);
-    if (i == nMD - 1) {
-      seg_start[nMD] = min(base + total, cap);
-      publish_total(H, LST_SEG_, base + total, cap);
-    }
-    __syncwarp();
-  };
-
-  int buf = 0, pC = -1, pTotal = 0;
-  for (;;) {
-    const int C = warp_ticket(&H->ticket[LST_SEG_]);
-    if (C >= nChunks) {
-      if (C == 0 && lane == 0) {  // no MDs at all: the first ticket publishes the empty result
-        publish_total(H, LST_SEG_, 0, cap);
-        seg_start[0] = 0;
-      }
-      break;
-    }
-    const int i0 = C * kChunk, i = i0 + lane;
-    int nt = 0, row0 = 0, modA = -1, wbits = 0;
-    bool okw = false;
-    if (i < nMD) {
-      const float4 a = S.md_anchor()[i];
-      const float2 x = S.md_aux()[i];
-      const float key = S.md_key()[i];
-      modA = S.md_module()[i];
-      row0 = P.map_offsets[modA];
-      nt = P.map_offsets[modA + 1] - row0;
-      const int layer = P.mod_layer[modA];
-      float dlo = 1.0f, dhi = -1.0f;
-      if (nt > 0) seg_window(P.cuts, layer, a.w, x.x, x.y, s_rMinO[layer + 1], s_rMaxO[layer + 1], dlo, dhi);
-      okw = dlo <= dhi;
-      sh.a4[lane] = a;
-      sh.aux[lane] = x;
-      sh.lo[lane] = okw ? key + dlo : 1.0f;
-      sh.hi[lane] = okw ? key + dhi : -1.0f;
-      sh.layer[lane] = layer;
-      if (okw) wbits = __float_as_int(fabsf(key) + fmaxf(fabsf(dlo), fabsf(dhi)));
-    }
-    sh.cnt[buf][lane] = 0;
-    __syncwarp();
-    const int nValid = min(kChunk, nMD - i0);
-    const int total = seg2_walk<false>(P, S, sh, buf, modA, row0, nt, wbits, okw, nValid, i0, 0, space, evals);
-    publish_aggregate(status, C, total);
-    __syncwarp();
-    if (pC >= 0) {
-      const int ex = offsets(buf ^ 1);
-      finish(pC, buf ^ 1, pTotal, resolve_base(status, pC, pTotal), ex, true);
-      pC = -1;
-    }
-    if (total <= kSegStash) {
-      pC = C; pTotal = total; buf ^= 1;
-    } else {
-      if (lane == 0) atomicAdd(&H->rewalk[LST_SEG_], 1ull);
-      const int base = resolve_base(status, C, total);
-      const int ex = offsets(buf);
-      sh.cur[lane] = 0;
-      __syncwarp();
-      seg2_walk<true>(P, S, sh, buf, modA, row0, nt, wbits, okw, nValid, i0, base, space, evals);
-      finish(C, buf, total, base, ex, false);
-    }
-  }
-  if (pC >= 0) {
-    const int ex = offsets(buf ^ 1);
-    finish(pC, buf ^ 1, pTotal, resolve_base(status, pC, pTotal), ex, true);
-  }
-  space = warp_sum_ull(space);
-  evals = warp_sum_ull(evals);
-  if (lane == 0 && space) atomicAdd(&H->cand[LST_SEG_], space);
-  if (lane == 0 && evals) atomicAdd(&H->eval[LST_SEG_], evals);
-}
-
-// ------------------------------------------------------------------------------------------
 // a3: triplets.  Owner = first segment a = (m1, m2); candidates are the segments leaving m2, a
 // contiguous range because segments are stored by inner MD.
 // ------------------------------------------------------------------------------------------
@@ -1883,14 +1571,10 @@ int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEv
     case LST_MD_:
       k_md<<<dim3(blocks_per_event((P.L.n_chunk[0] + kWarps - 1) / kWarps, n_batch, 6, kGridShare), nb), kWarps * 32, 0, s>>>(P);
       break;
-    case LST_SEG_: {
-      // A/B of round 2 (profiles/r2_seg_ab.md): LST_SEG_V2=1 selects the module-owner walk, which lost
-      static const bool v2 = getenv("LST_SEG_V2") != nullptr;
-      const dim3 g(blocks_per_event((P.L.n_chunk[1] + kSegWarps - 1) / kSegWarps, n_batch, 6, kGridShare), nb);
-      if (v2) k_seg_v2<<<g, kSegWarps * 32, 0, s>>>(P);
-      else k_seg<<<g, kSegWarps * 32, 0, s>>>(P);
+    case LST_SEG_:
+      // (a module-owner walk with a flat on-chip key-window compare was built and measured in round 2: it lost, profiles/r2_seg_ab.md)
+      k_seg<<<dim3(blocks_per_event((P.L.n_chunk[1] + kSegWarps - 1) / kSegWarps, n_batch, 6, kGridShare), nb), kSegWarps * 32, 0, s>>>(P);
       break;
-    }
     case LST_T3_:
       k_t3<<<dim3(blocks_per_event((P.L.n_chunk[2] + kWarps - 1) / kWarps, n_batch, 6, kGridShare), nb), kWarps * 32, 0, s>>>(P);
       break;
