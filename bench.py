@@ -40,6 +40,7 @@ MAP_BYTES = 4 * (69630 + 6121)
 # SPEC operations per candidate (every sqrt and div counted as one)
 FLOPS_PER_CAND = (34, 51, 45, 255)
 HEADER_BYTES = 312   # per-slot counter block that lst_sync_batch reads back (csrc/lst_device.cuh SlotHeader)
+A0_KERNELS = ("bin_count", "bin_scatter", "bin_order")               # lst_stats.kernel_ms[0..2]
 
 
 def algorithmic_bytes(stage: int, n_hits, needed):
@@ -143,13 +144,20 @@ def make_events(seed0: int, n: int, device=None):
 # ------------------------------------------------------------------------------------------
 # reference arm: the CPU oracle, as it stands, on a bounded sample
 # ------------------------------------------------------------------------------------------
-def oracle_events_per_s(geom, mmap, events):
+def oracle_events_per_s(geom, mmap, events, check=None):
+    """Times the oracle over `events`.  check: per event, the quintuplet hit tuples the GPU arm downloaded end to end; they
+    are compared with the oracle's (outside the timed intervals)."""
     from oracle import oracle
     o = oracle.load("f32")
-    t0 = time.perf_counter()
-    for ev in events:
-        o.run(geom.layer, mmap.row_offsets, mmap.targets, ev.x, ev.y, ev.z, ev.module, ev.side)
-    dt = time.perf_counter() - t0
+    dt = 0.0
+    for k, ev in enumerate(events):
+        t0 = time.perf_counter()
+        r = o.run(geom.layer, mmap.row_offsets, mmap.targets, ev.x, ev.y, ev.z, ev.module, ev.side)
+        dt += time.perf_counter() - t0
+        if check is not None:
+            want, got = r.t5_hits(), check[k]
+            assert got.shape == want.shape and set(map(tuple, got.tolist())) == set(map(tuple, want.tolist())), \
+                f"end-to-end quintuplets of event {k} differ from the oracle's"
     return len(events) / dt, dt
 
 
@@ -276,9 +284,23 @@ def run_ours(args):
         return
 
     # ---- end to end: pinned host hits in, quintuplets out, through the C-ABI -------------
-    h_in = [[torch.from_numpy(a).pin_memory() for a in (e.x, e.y, e.z, e.module, e.side)] for e in events]
+    # Host input in the "packed" layout of include/lst.h (the five arrays of an event in ONE pinned block): an event
+    # travels as one copy-engine transfer while the results come back through k_fetch_direct (SM writes over PCIe), so
+    # the two directions do not queue on one engine.  LST_BENCH_E2E_INPUT=arrays: five separate pinned arrays per event
+    # (read by the binning kernel itself), for comparison.
+    e2e_input = os.environ.get("LST_BENCH_E2E_INPUT", "packed")
+    if e2e_input == "packed":
+        keep_blocks, np_in = [], []
+        for e in events:
+            bufs = lst.packed_event_buffers(e.n)
+            for dst, src in zip(bufs[:5], (e.x, e.y, e.z, e.module, e.side)):
+                dst[:] = src
+            np_in.append(list(bufs[:5]))
+            keep_blocks.append(bufs[5])
+    else:
+        h_in = [[torch.from_numpy(a).pin_memory() for a in (e.x, e.y, e.z, e.module, e.side)] for e in events]
+        np_in = [[t.numpy() for t in ev] for ev in h_in]
     cap5 = max(s["needed"][3] for s in stats) * 2 + 1024
-    np_in = [[t.numpy() for t in ev] for ev in h_in]
     # Two buffer sets (slots, streams, pinned result buffers): step i + 1 is loaded and run while the results of
     # step i travel back -- H2D and D2H share the PCIe link in opposite directions, as in a continuously fed pipeline.
     sets = []
@@ -322,13 +344,12 @@ def run_ours(args):
     e2e_run(e2e_steps)
     torch.cuda.synchronize(dev)
     e2e_s = max_over_ranks(time.perf_counter() - t0, dist, dev)
-    # the results are on the host: both buffer sets hold every event's quintuplets (counts and tuples of two events checked)
+    # the results are on the host: both buffer sets hold every event's quintuplets (all counts checked here; every tuple is
+    # compared with the ORACLE's in the cpu_baseline leg below, where the oracle runs over these events anyway)
     for S in sets:
         got = [c for per in S["counts"] for c in per]
         assert got == [st_["needed"][3] for st_ in stats], "end-to-end results incomplete"
-        for k in (0, N_EVENTS - 1):
-            ref = ctx.fetch_hit_indices(S["base"] + k, lst.T5, S["streams"][k // per_stream])
-            assert np.array_equal(S["idx"][k // per_stream][k % per_stream][:len(ref)], ref)
+    e2e_tuples = [np.array(sets[0]["idx"][k // per_stream][k % per_stream][:stats[k]["needed"][3]]) for k in range(N_EVENTS)]
     # the same with the cleaning stage [D] in the step and only the kept quintuplets (the track candidates) downloaded
     e2e_kind[0] = lst.CLEAN
     e2e_run(3)
@@ -339,26 +360,36 @@ def run_ours(args):
     e2e_tc_s = max_over_ranks(time.perf_counter() - t0, dist, dev)
     kept_e2e = sum(c for S in sets[:1] for per in S["counts"] for c in per)
     e2e_kind[0] = lst.T5
-    h2d = sum(sum(t.numel() * t.element_size() for t in ev) for ev in h_in)
+    h2d = sum(sum(a.nbytes for a in ev) for ev in np_in)
     d2h = needed[3] * (40 + 20) + N_EVENTS * HEADER_BYTES
+    # What the link itself allows for these byte counts: the same number and sizes of transfers as plain copies, both
+    # directions at once on two streams, nothing else on the GPU (same box, same pinned buffers).
+    pcie = pcie_ceiling(torch, dev, [[blk] for blk in keep_blocks] if e2e_input == "packed" else np_in,
+                        [(stats[k]["needed"][3] * 40, stats[k]["needed"][3] * 20) for k in range(N_EVENTS)], sets[0])
+    step_s = e2e_s / e2e_steps
     e2e = {"value": world * N_EVENTS * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
-           "d2h_bytes_per_step": int(d2h), "steps": e2e_steps,
-           "how": "per stream: lst_load_events(16 x pinned host SoA) + lst_run_batch + lst_fetch_batch(T5 hit indices + values "
-                  "to pinned host buffers); two buffer sets, step i + 1 is loaded and run while step i's results travel back; "
-                  "the timed region ends with every step's results on the host",
+           "d2h_bytes_per_step": int(d2h), "steps": e2e_steps, "ms_per_step": 1e3 * step_s,
+           "h2d_gbs": h2d / step_s / 1e9, "d2h_gbs": d2h / step_s / 1e9, "input_layout": e2e_input,
+           "pcie_ceiling": pcie,
+           "how": "per stream: lst_load_events(16 x pinned host event, packed layout: one copy-engine transfer each) + lst_run_batch + "
+                  "lst_fetch_batch(T5 hit indices + values to pinned host buffers); two buffer sets, step i + 1 is loaded and run while "
+                  "step i's results travel back; the timed region ends with every step's results on the host",
            "track_candidates": {"value": world * N_EVENTS * e2e_steps / e2e_tc_s, "unit": UNIT, "d2h_bytes_per_step": int(kept_e2e * 60 + N_EVENTS * HEADER_BYTES),
                                 "what": "the same pipeline with LST_CLEAN in the step and lst_fetch_batch(kind = LST_CLEAN): only the kept "
                                         "quintuplets (T5-only track candidates) travel back"}}
 
     # ---- per-kernel times (CUDA events inside the library, timing mode), one 64-event batch ----
     kernel_ms, launches_per_step = per_kernel_times(lst, geom, mmap, d_in, local)
-    for k in lst.KERNEL_NAMES[8:]:
+    alone_ms, _ = per_kernel_times(lst, geom, mmap, d_in, local, alone=True)
+    for k in lst.KERNEL_NAMES[7:]:
         kernel_ms.pop(k)
+        alone_ms.pop(k)
     with_clean_ms, _ = per_kernel_times(lst, geom, mmap, d_in, local, with_clean=True)
-    clean_ms = {k: with_clean_ms[k] for k in lst.KERNEL_NAMES[8:]}
+    clean_alone_ms, _ = per_kernel_times(lst, geom, mmap, d_in, local, with_clean=True, alone=True, reps=3)
+    clean_ms = {k: {"in_step": with_clean_ms[k], "alone": clean_alone_ms[k]} for k in lst.KERNEL_NAMES[7:]}
     peaks = measured_peaks()
     lp = launches_per_step                      # per-launch quantities: one launch covers 64 / lp events
-    roof, per_stage = roofline(kernel_ms, n_hits / lp, [v / lp for v in needed], [v / lp for v in evals], peaks, N_EVENTS // lp)
+    roof, per_stage = roofline(kernel_ms, alone_ms, n_hits / lp, [v / lp for v in needed], [v / lp for v in evals], peaks, N_EVENTS // lp)
     spec_flops_step = sum(evals[i] * FLOPS_PER_CAND[i] for i in range(4))
     alu_peak = 148 * 128 * peaks["sm_max_mhz"] * 1e6 / 1e12
     path = {"what": "whole path a0..a4 over the timed region: SPEC flops of all evaluated candidates and algorithmic bytes "
@@ -404,18 +435,24 @@ def run_ours(args):
            "evaluated_per_step": dict(md=evals[0], ls=evals[1], t3=evals[2], t5=evals[3]),
            "roofline_path": path,
            "stage_overlap": {"sum_of_launch_ms_per_step": launches_per_step * sum(v["ms"] for v in per_stage.values()),
+                             "sum_of_alone_ms_per_step": launches_per_step * sum(v["alone"]["ms"] for v in per_stage.values()),
                              "ms_per_step_4_streams": total_ms / args.steps,
                              "factor": launches_per_step * sum(v["ms"] for v in per_stage.values()) / (total_ms / args.steps),
-                             "what": "sum over the step's launches of their CUDA-event durations / the step: > 1 = kernels of "
-                                     "different streams run side by side"},
+                             "alone_factor": launches_per_step * sum(v["alone"]["ms"] for v in per_stage.values()) / (total_ms / args.steps),
+                             "what": "launches per step x (sum of the kernels' durations) / the step. `factor` uses the durations inside the "
+                                     "4-stream step (kernels of different streams run side by side and stretch one another), `alone_factor` "
+                                     "the durations with the GPU otherwise idle: what the 4-stream pipeline gains over running the same "
+                                     "launches back to back"},
+           "csrc_digest": csrc_digest(),
            "duplicate_cleaning": clean, "module_map_builder": map_builder,
            "rewalks_per_step": dict(md=rewalks[0], ls=rewalks[1], t3=rewalks[2], t5=rewalks[3]),
            "arena_mib": ctx.arena_bytes()[0] / 2 ** 20, "impl": "ours"}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         n_pass, t_cpu = 0, 0.0
         while t_cpu < 12.0 and n_pass < 8:          # a bounded sample: whole passes over the workload, >= 12 s of CPU work
-            t_cpu += oracle_events_per_s(geom, mmap, events)[1]
+            t_cpu += oracle_events_per_s(geom, mmap, events, check=e2e_tuples if n_pass == 0 else None)[1]
             n_pass += 1
+        out["e2e"]["verified"] = f"the quintuplets of all {N_EVENTS} events as downloaded by the end-to-end arm equal the oracle's (sets of 10 hit indices)"
         out["cpu_baseline"] = {"value": n_pass * N_EVENTS / t_cpu, "unit": UNIT, "cores": 1, "kind": "oracle",
                                "sample": f"all {N_EVENTS} events of the workload x {n_pass} passes, single thread, {t_cpu:.1f} s"}
         # the same oracle on every host core: events are independent (SURVEY 8(d) "all host cores" figure)
@@ -442,11 +479,58 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
-def per_kernel_times(lst, geom, mmap, d_in, local, with_clean=False, reps=6):
-    """Average duration (ms) of ONE launch of every kernel in the configuration the timed region uses: 4 streams x
-    16-event launches running concurrently, CUDA events recorded by the library around every launch on the stream it
-    is launched on (lst_config.timing), L2 flushed before every step.  (Concurrent kernels share the SMs, so the
-    durations of one step add up to more than the step.)  The optional cleaning stage [D] is timed the same way."""
+def pcie_ceiling(torch, dev, np_in, out_bytes, S, reps=10):
+    """Plain copies of the end-to-end arm's byte counts, both directions at once: per step the host->device transfers the
+    library makes (np_in: per event the list of pinned host tensors that travel -- ONE block in the packed layout, five arrays
+    otherwise) on one stream and 128 device->host transfers (hit tuples and values of every event) on another, from / to the
+    same pinned buffers.  Returns the step time and what it would allow in events/s."""
+    h_src = [[a if hasattr(a, "data_ptr") else torch.from_numpy(a) for a in ev] for ev in np_in]
+    d_dst = [[torch.empty(t.numel(), dtype=t.dtype, device=dev) for t in ev] for ev in h_src]
+    per = N_EVENTS // N_STREAMS
+    h_out = [(torch.from_numpy(S["idx"][k // per][k % per]).view(torch.uint8).reshape(-1), torch.from_numpy(S["val"][k // per][k % per]).view(torch.uint8).reshape(-1))
+             for k in range(N_EVENTS)]
+    d_src = torch.empty(max(max(a, b) for a, b in out_bytes) + 16, dtype=torch.uint8, device=dev)
+    up, down = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+
+    def step(do_up=True, do_down=True):
+        if do_up:
+            with torch.cuda.stream(up):
+                for hs, ds in zip(h_src, d_dst):
+                    for h, d in zip(hs, ds):
+                        d.copy_(h, non_blocking=True)
+        if do_down:
+            with torch.cuda.stream(down):
+                for (hi, hv), (nb_i, nb_v) in zip(h_out, out_bytes):
+                    hi[:nb_i].copy_(d_src[:nb_i], non_blocking=True)
+                    hv[:nb_v].copy_(d_src[:nb_v], non_blocking=True)
+
+    def timed(**kw):
+        for _ in range(2):
+            step(**kw)
+        torch.cuda.synchronize(dev)
+        t0 = time.perf_counter()
+        for _ in range(reps):
+            step(**kw)
+        torch.cuda.synchronize(dev)
+        return (time.perf_counter() - t0) / reps
+
+    both, only_up, only_down = timed(), timed(do_down=False), timed(do_up=False)
+    h2d = sum(t.numel() * t.element_size() for ev in h_src for t in ev)
+    d2h = sum(a + b for a, b in out_bytes)
+    return {"ms_per_step_both_directions": 1e3 * both, "events_per_s": N_EVENTS / both, "h2d_alone_gbs": h2d / only_up / 1e9,
+            "d2h_alone_gbs": d2h / only_down / 1e9, "h2d_gbs_duplex": h2d / both / 1e9, "d2h_gbs_duplex": d2h / both / 1e9,
+            "h2d_transfers_per_step": sum(len(ev) for ev in h_src), "d2h_transfers_per_step": 2 * N_EVENTS,
+            "what": "cudaMemcpyAsync (torch copy_) of the end-to-end arm's transfers only, two streams, same pinned buffers, same box; "
+                    "no kernel running"}
+
+
+def per_kernel_times(lst, geom, mmap, d_in, local, with_clean=False, reps=6, alone=False):
+    """Average duration (ms) of ONE launch of every kernel, from CUDA events recorded by the library around every launch on
+    the stream it is launched on (lst_config.timing), L2 flushed before every step.
+    alone=False: the configuration the timed region uses -- 4 streams x 16-event launches running concurrently (concurrent
+    kernels share the SMs, so the durations of one step add up to more than the step).
+    alone=True: the same 16-event launches one batch at a time on one stream, the GPU otherwise idle.
+    The optional cleaning stage [D] is timed the same way."""
     import torch
     cfg = lst.default_config()
     cfg.device, cfg.n_slots, cfg.timing = local, N_EVENTS, 1
@@ -455,72 +539,120 @@ def per_kernel_times(lst, geom, mmap, d_in, local, with_clean=False, reps=6):
     per = N_EVENTS // N_STREAMS
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     rows = []
+
+    def enqueue(s, st):
+        ctx.load_events(s * per, d_in[s * per:(s + 1) * per], stream=st)
+        ctx.run_batch(s * per, per, st)
+        if with_clean:                                  # optional stage [D], reported beside the path, not in it
+            ctx.run_stage(s * per, per, lst.CLEAN, st)
+
+    def collect(s, st, keep):
+        ctx.sync_batch(s * per, per, st)
+        for k in range(s * per, (s + 1) * per, 16):    # one set of launches per 16 events; times kept on its first slot
+            if keep:
+                rows.append(ctx.stats(k)["kernel_ms"][:11])
+
     for rep in range(reps + 2):
-        flush.zero_()
-        torch.cuda.synchronize()
-        for s, st in enumerate(streams):
-            ctx.load_events(s * per, d_in[s * per:(s + 1) * per], stream=st)
-            ctx.run_batch(s * per, per, st)
-            if with_clean:                                  # optional stage [D], reported beside the path, not in it
-                ctx.run_stage(s * per, per, lst.CLEAN, st)
-        for s, st in enumerate(streams):
-            ctx.sync_batch(s * per, per, st)
-            for k in range(s * per, (s + 1) * per, 16):    # one set of launches per 16 events; times kept on its first slot
-                if rep >= 2:
-                    rows.append(ctx.stats(k)["kernel_ms"][:12])
+        if alone:
+            for s in range(N_STREAMS):
+                flush.zero_()
+                torch.cuda.synchronize()
+                enqueue(s, streams[0])
+                collect(s, streams[0], rep >= 2)
+        else:
+            flush.zero_()
+            torch.cuda.synchronize()
+            for s, st in enumerate(streams):
+                enqueue(s, st)
+            for s, st in enumerate(streams):
+                collect(s, st, rep >= 2)
     ctx.close()
     return dict(zip(lst.KERNEL_NAMES, np.mean(np.asarray(rows), axis=0).tolist())), max(1, per // 16) * N_STREAMS
 
 
+def csrc_digest() -> str:
+    """sha256 over the CUDA sources and the header the library is built from: ties a committed ncu summary to the code it
+    was taken on (there is no .git on the GPU box)."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2207_08207_b200", "csrc")
+    for f in sorted(os.listdir(d)) + [os.path.join("..", "..", "include", "lst.h")]:
+        if f.endswith((".cu", ".cuh", ".h")):
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+NCU_SUMMARY = os.path.join("profiles", "r2_ncu_full_summary.csv")      # its .json sidecar holds the csrc digest of the capture
+
+
 def ncu_traffic_bytes(kernel: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed `ncu --set full`
-    summary of the same launch configuration (profiles/r1f_ncu_full_summary.csv; 16-event launches), or None."""
+    """(bytes, note): dram__bytes_read.sum + dram__bytes_write.sum per 16-event launch of `kernel` from the committed
+    `ncu --set full` summary -- a CITATION of that capture, not a measurement of this run; refused (None) when the CUDA
+    sources have changed since the capture was taken."""
     import csv
-    path = os.path.join(ROOT, "profiles", "r1f_ncu_full_summary.csv")
-    name = {"seg": "k_seg", "md": "k_md", "t3": "k_t3", "t5": "k_t5"}.get(kernel, "k_" + kernel)
+    path = os.path.join(ROOT, NCU_SUMMARY)
     try:
+        meta = json.load(open(path[:-4] + ".json"))
+        if meta.get("csrc_digest") != csrc_digest():
+            return None, f"{NCU_SUMMARY} is stale: taken at csrc digest {meta.get('csrc_digest')}, this run is {csrc_digest()}"
         rows = list(csv.reader(open(path)))
         h = rows[0]
-        vals = [(float(r[h.index("dram__bytes_read.sum")]) + float(r[h.index("dram__bytes_write.sum")])) * 1e6
-                for r in rows[2:] if r[h.index("Kernel Name")].startswith(name + "(")]
-        return sum(vals) / len(vals) if vals else None
-    except Exception:
-        return None
+        unit = {"Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0, "Gbyte": 1e9}
+        def col(r, name):
+            i = h.index(name)
+            return float(r[i]) * unit[rows[1][i]]
+        vals = [col(r, "dram__bytes_read.sum") + col(r, "dram__bytes_write.sum")
+                for r in rows[2:] if r[h.index("Kernel Name")].startswith("k_" + kernel + "(")]
+        if not vals:
+            return None, f"{NCU_SUMMARY} has no row for k_{kernel}"
+        return sum(vals) / len(vals), (f"cited from {NCU_SUMMARY} (ncu --set full of this code, csrc digest {meta['csrc_digest']}, "
+                                      f"commit {meta.get('commit', '?')}; bytes per 16-event launch, kernel alone)")
+    except Exception as e:                       # noqa: BLE001
+        return None, f"no usable {NCU_SUMMARY}: {e}"
 
 
-def roofline(kernel_ms, n_hits, needed, cands, peaks, events_per_launch):
-    """Per-stage table and the `roofline` object for the dominant kernel. Two lower bounds per stage:
-    HBM (algorithmic bytes / measured copy bandwidth) and ALU (SPEC flops of all candidates / fp32
-    non-FMA peak = 148 SMs x 128 lanes x sm_max clock; FMA is excluded by the SPEC's arithmetic)."""
+def roofline(kernel_ms, alone_ms, n_hits, needed, cands, peaks, events_per_launch):
+    """Per-stage table and the `roofline` object (achieved HBM fraction) for the dominant kernel.
+    kernel_ms: average duration of one launch inside the timed 4-stream configuration (kernels of other streams share the
+    SMs); alone_ms: the same launch with nothing else on the GPU.  Both from CUDA events the library records around every
+    launch on the stream it is launched on.  Bytes / flops are those of ONE launch (`events_per_launch` events).
+    The ALU view (SPEC flops of the evaluated candidates / non-FMA fp32 peak = 148 SMs x 128 lanes x sm_max clock; the
+    SPEC forbids FMA contraction) is kept beside the HBM view: this path is not bandwidth bound."""
     alu_peak_tflops = 148 * 128 * peaks["sm_max_mhz"] * 1e6 / 1e12
-    groups = (("a0_bin", ("reset", "bin_count", "bin_scatter", "bin_order")), ("a1_md", ("md",)),
-              ("a2_ls", ("seg",)), ("a3_t3", ("t3",)), ("a4_t5", ("t5",)))
+    groups = (("a0_bin", A0_KERNELS), ("a1_md", ("md",)), ("a2_ls", ("seg",)), ("a3_t3", ("t3",)), ("a4_t5", ("t5",)))
+
+    def views(b, fl, ms):
+        if not ms:
+            return {"ms": ms}
+        return {"ms": ms, "hbm_gbs": b / (ms * 1e-3) / 1e9, "hbm_frac": b / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                "alu_tflops": fl / (ms * 1e-3) / 1e12, "alu_frac": fl / (ms * 1e-3) / 1e12 / alu_peak_tflops}
+
     per_stage = {}
     for i, (name, ks) in enumerate(groups):
-        ms = sum(kernel_ms[k] for k in ks)
         b = algorithmic_bytes(i, n_hits, needed)
         fl = cands[i - 1] * FLOPS_PER_CAND[i - 1] if i else 0
-        per_stage[name] = {"ms": ms, "kernels_ms": {k: kernel_ms[k] for k in ks}, "algorithmic_bytes": int(b),
-                           "hbm_gbs": b / (ms * 1e-3) / 1e9 if ms else None,
-                           "hbm_frac": b / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"] if ms else None,
-                           "spec_flops": int(fl), "alu_tflops": fl / (ms * 1e-3) / 1e12 if ms else None,
-                           "alu_frac": fl / (ms * 1e-3) / 1e12 / alu_peak_tflops if ms else None}
+        per_stage[name] = {"algorithmic_bytes": int(b), "spec_flops": int(fl),
+                           "kernels_ms_in_step": {k: kernel_ms[k] for k in ks}, "kernels_ms_alone": {k: alone_ms[k] for k in ks},
+                           "in_step": views(b, fl, sum(kernel_ms[k] for k in ks)), "alone": views(b, fl, sum(alone_ms[k] for k in ks))}
+        per_stage[name]["ms"] = per_stage[name]["in_step"]["ms"]
     top = max(kernel_ms, key=kernel_ms.get)
     si = next(i for i, (_, ks) in enumerate(groups) if top in ks)
-    ms = kernel_ms[top]
     b = algorithmic_bytes(si, n_hits, needed)
     fl = cands[si - 1] * FLOPS_PER_CAND[si - 1] if si else 0
-    t_hbm, t_alu = b / (peaks["hbm_gbs"] * 1e9), fl / (alu_peak_tflops * 1e12)
-    if t_alu > t_hbm:
-        roof = {"bound": "alu", "achieved": fl / (ms * 1e-3) / 1e12, "peak": alu_peak_tflops, "unit": "TFLOP/s"}
-    else:
-        roof = {"bound": "hbm", "achieved": b / (ms * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s"}
-    roof.update({"frac": roof["achieved"] / roof["peak"], "traffic": ncu_traffic_bytes(top) if events_per_launch == 16 else None,
-                 "traffic_source": "profiles/r1f_ncu_full_summary.csv (bytes per 16-event launch)", "kernel": top, "kernel_ms": ms,
-                 "launch": f"one launch = {events_per_launch} events (grid.y = event), timed inside the 4-stream step; "
-                           "flops / bytes are those of one launch", "peak_source": peaks["source"],
-                 "hbm_view": {"achieved_gbs": b / (ms * 1e-3) / 1e9, "peak_gbs": peaks["hbm_gbs"],
-                              "frac": b / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"], "algorithmic_bytes": int(b)}})
+    ins, alo = views(b, fl, kernel_ms[top]), views(b, fl, alone_ms[top])
+    traffic, note = ncu_traffic_bytes(top) if events_per_launch == 16 else (None, "launch is not 16 events")
+    roof = {"bound": "hbm", "achieved": ins["hbm_gbs"], "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ins["hbm_frac"],
+            "traffic": traffic, "traffic_source": note, "kernel": "k_" + top, "algorithmic_bytes": int(b),
+            "kernel_ms": kernel_ms[top], "kernel_ms_alone": alone_ms[top], "peak_source": peaks["source"],
+            "launch": f"one launch = {events_per_launch} events (grid.y = event); kernel_ms = average launch duration inside the timed "
+                      "4-stream configuration (CUDA events on the launching stream), kernel_ms_alone = the same launch with the GPU "
+                      "otherwise idle; achieved = algorithmic_bytes / kernel_ms",
+            "alone": {"achieved": alo["hbm_gbs"], "frac": alo["hbm_frac"]},
+            "alu_view": {"what": "secondary bound: SPEC flops of the evaluated candidates / non-FMA fp32 peak", "spec_flops": int(fl),
+                         "peak_tflops": alu_peak_tflops, "in_step": {"achieved_tflops": ins["alu_tflops"], "frac": ins["alu_frac"]},
+                         "alone": {"achieved_tflops": alo["alu_tflops"], "frac": alo["alu_frac"]}},
+            "why_low": "the path is latency / issue bound, not bandwidth bound: a 16-event batch is L2 resident (traffic < algorithmic "
+                       "bytes) and the search is a gather; DESIGN.md section 7"}
     return roof, per_stage
 
 
@@ -569,12 +701,12 @@ def run_sweep(args):
             ctx.run_stage(0, 1, lst.MD, st)
             ctx.run_stage(0, 1, lst.SEG, st)
             ctx.sync(0, st)
-            rows.append(ctx.stats(0)["kernel_ms"][:6])
+            rows.append(ctx.stats(0)["kernel_ms"][:5])
         stt = ctx.stats(0)
-        k_ms = dict(zip(lst.KERNEL_NAMES[:6], np.median(np.asarray(rows[2:]), axis=0).tolist()))
+        k_ms = dict(zip(lst.KERNEL_NAMES[:5], np.median(np.asarray(rows[2:]), axis=0).tolist()))
         need, evl, cand = stt["needed"], stt["evaluated"], stt["candidates"]
         per = {}
-        for name, ks, stage in (("a0_bin", ("reset", "bin_count", "bin_scatter", "bin_order"), 0), ("a1_md", ("md",), 1), ("a2_ls", ("seg",), 2)):
+        for name, ks, stage in (("a0_bin", A0_KERNELS, 0), ("a1_md", ("md",), 1), ("a2_ls", ("seg",), 2)):
             ms = sum(k_ms[k] for k in ks)
             b = algorithmic_bytes(stage, stt["n_hits"], need)
             per[name] = {"ms": ms, "algorithmic_bytes": int(b), "hbm_gbs": b / (ms * 1e-3) / 1e9,

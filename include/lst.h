@@ -200,14 +200,15 @@ typedef struct {
   int32_t overflow;      /* bit k set: capacity of class k exceeded                              */
   int32_t bad_hits;      /* hits dropped because module id / side was out of range               */
   float stage_ms[5];     /* a0 .. a4; zeros unless lst_config.timing                              */
-  float kernel_ms[12];   /* a0: reset, bin count + offsets scan (2 launches), scatter, order; then the MD, LS, T3, T5 kernel; then the four
-                            steps of LST_CLEAN (prepare, count + offsets scan, fill, mark + list) */
+  float kernel_ms[12];   /* [0..2] a0: count (+ bin offsets and the slot's fresh header, by its last block), scatter, order;
+                            [3..6] the MD, LS, T3, T5 kernel; [7..10] the four steps of LST_CLEAN (prepare, count + offsets
+                            scan, fill, mark + list); [11] unused */
   int64_t rewalks[4];    /* chunks of 32 owners whose objects exceeded the on-chip stash and were walked twice */
   int32_t n_kept;        /* quintuplets kept by LST_CLEAN (0 if the stage was not run)                         */
 } lst_stats;
 
-/* Validates geometry and map, uploads the per-module tables, allocates the arena (the only
- * cudaMalloc of the library's lifetime).  cfg = NULL means lst_default_config.
+/* Validates geometry and map, uploads the per-module tables, allocates the arena (the library allocates
+ * here and nowhere else: nothing is allocated or freed per event).  cfg = NULL means lst_default_config.
  * Errors: LST_ERR_ARG (with nothing allocated), LST_ERR_NOMEM, LST_ERR_CUDA. */
 LST_API int lst_create(const lst_geometry* geom, const lst_module_map* map, const lst_config* cfg, lst_ctx** out);
 LST_API int lst_destroy(lst_ctx* ctx);

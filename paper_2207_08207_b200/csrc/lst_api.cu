@@ -1,9 +1,10 @@
 // lst_api.cu -- host side of liblst.so: the C-ABI of include/lst.h, the arena and the slots.
 //
 // Runtime design:
-//  * ONE cudaMalloc in lst_create covers every slot's input staging, hit store, object store,
-//    CSR offsets and scratch ("arena"); per event nothing is allocated or freed, the slot is
-//    recycled by one small kernel (k_reset) that zeroes its header, bin counters and look-back words.
+//  * lst_create allocates once: the arena (every slot's input staging, hit store, object store, CSR offsets and
+//    scratch) and five small geometry / map tables; per event nothing is allocated or freed, and a slot recycles
+//    itself inside the a0 kernels (bin counters cleared by the block that scans them, a fresh header written by the
+//    same block, look-back words cleared by the scatter kernel): no reset launch.
 //  * lst_load_event / lst_run* only enqueue work on the caller's stream; sizes that are only
 //    known on the device (object counts) never come back to the host between stages: grids
 //    are fixed by the geometry / capacities and kernels read the counts from the slot header.
@@ -34,7 +35,7 @@ struct SlotHost {
   int stages_run = 0;         // stages a1 .. run in order since the load: objects of class k are valid iff stages_run > k
   int n_hits_in = 0;
   SlotHeader* hdr = nullptr;  // pinned host copy of the device header
-  cudaEvent_t ev[18] = {};    // timing mode: ev[0..4] around the 4 a0 kernels, ev[5 + 2 s], ev[6 + 2 s] around stage s, ev[13..17] around the 4 cleaning kernels
+  cudaEvent_t ev[17] = {};    // timing mode: ev[0..3] around the 3 a0 kernels, ev[4 + 2 s], ev[5 + 2 s] around stage s, ev[12..16] around the 4 cleaning steps
   bool ev_bin = false, ev_stage[5] = {false, false, false, false, false};
 };
 
@@ -89,12 +90,14 @@ Layout make_layout(const lst_config& cfg, int n_modules) {
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
   L.hdr = take(sizeof(SlotHeader));
+  L.bin_cnt = take(sizeof(int) * (size_t)(L.n_bins + 1));
   L.bin_start = take(sizeof(int) * (size_t)(L.n_bins + 1));
   for (int k = 0; k < 4; ++k) L.lb[k] = take(8 * (size_t)(L.n_chunk[k] + 1));
-  L.reset_bytes = off - L.hdr;
+  L.lb_bytes = off - L.lb[0];
   const size_t nh = (size_t)cfg.cap_hits, nm = (size_t)cfg.cap_md, ns = (size_t)cfg.cap_seg, n3 = (size_t)cfg.cap_t3, n5 = (size_t)cfg.cap_t5;
   L.in_x = take(4 * nh); L.in_y = take(4 * nh); L.in_z = take(4 * nh); L.in_module = take(4 * nh); L.in_side = take(nh);
-  L.tmp_kr = take(8 * nh); L.tmp_ki = take(8 * nh); L.tmp_bin = take(4 * nh);
+  L.rec4 = take(16 * nh); L.recb = take(8 * nh); L.reck = take(4 * nh);
+  L.tmp_ki = take(8 * nh); L.tmp_bin = take(4 * nh);
   L.hit4 = take(16 * nh); L.hit_key = take(4 * nh); L.hit_orig = take(4 * nh); L.hit_module = take(4 * nh);
   L.md_start = take(4 * (size_t)(n_modules + 1)); L.mod_info = take(16 * (size_t)n_modules);
   L.md_anchor = take(16 * nm); L.md_aux = take(8 * nm); L.md_key = take(4 * nm); L.md_hits = take(8 * nm);
@@ -323,9 +326,8 @@ int lst_load_events(lst_ctx* c, int first, int n_ev, const lst_hits* hits, void*
   const Layout& L = c->P.L;
   for (int b0 = 0; b0 < n_ev; b0 += kMaxBatch) {
     const int nb = n_ev - b0 < kMaxBatch ? n_ev - b0 : kMaxBatch;
-    HitBatch src, dev;
+    HitBatch src;
     std::memset(&src, 0, sizeof(src));
-    std::memset(&dev, 0, sizeof(dev));
     for (int b = 0; b < nb; ++b) {
       const int slot = first + b0 + b;
       const lst_hits* h = hits + b0 + b;
@@ -337,9 +339,9 @@ int lst_load_events(lst_ctx* c, int first, int n_ev, const lst_hits* hits, void*
       for (bool& f : sh.ev_stage) f = false;
       char* base = c->arena + (size_t)slot * c->P.slot_stride;
       HitInput in{h->x, h->y, h->z, h->module, h->side, h->n, 0};
-      HitInput staged{reinterpret_cast<const float*>(base + L.in_x), reinterpret_cast<const float*>(base + L.in_y),
-                      reinterpret_cast<const float*>(base + L.in_z), reinterpret_cast<const int*>(base + L.in_module),
-                      reinterpret_cast<const unsigned char*>(base + L.in_side), h->n, 0};
+      const HitInput staged{reinterpret_cast<const float*>(base + L.in_x), reinterpret_cast<const float*>(base + L.in_y),
+                            reinterpret_cast<const float*>(base + L.in_z), reinterpret_cast<const int*>(base + L.in_module),
+                            reinterpret_cast<const unsigned char*>(base + L.in_side), h->n, 0};
       // "packed" host layout: the five arrays back to back in ONE block, each starting on a 256-byte boundary
       // (x at p, y at p + A, z at p + 2 A, module at p + 3 A, side at p + 4 A, A = 4 n rounded up to 256)
       const size_t A = align_up(4 * (size_t)h->n, 256);
@@ -348,20 +350,19 @@ int lst_load_events(lst_ctx* c, int first, int n_ev, const lst_hits* hits, void*
                           reinterpret_cast<const char*>(h->z) == px + 2 * A && reinterpret_cast<const char*>(h->module) == px + 3 * A &&
                           reinterpret_cast<const char*>(h->side) == px + 4 * A;
       if (h->on_device || h->n == 0) {
-        src.ev[b] = dev.ev[b] = in;
+        src.ev[b] = in;
       } else if (packed) {
         // one copy-engine transfer of the whole event (1.3 MB at PU200 density runs at link speed, five 300 kB ones do
-        // not), into the same layout in the slot's staging area; no SM involved, full duplex with the result copies
+        // not), into the same layout in the slot's copy area; no SM involved, full duplex with the result copies
         char* d = base + L.in_x;
         LST_CUDA(c, cudaMemcpyAsync(d, px, 4 * A + (size_t)h->n, cudaMemcpyHostToDevice, s));
-        src.ev[b] = dev.ev[b] = HitInput{reinterpret_cast<const float*>(d), reinterpret_cast<const float*>(d + A),
-                                         reinterpret_cast<const float*>(d + 2 * A), reinterpret_cast<const int*>(d + 3 * A),
-                                         reinterpret_cast<const unsigned char*>(d + 4 * A), h->n, 0};
+        src.ev[b] = HitInput{reinterpret_cast<const float*>(d), reinterpret_cast<const float*>(d + A),
+                             reinterpret_cast<const float*>(d + 2 * A), reinterpret_cast<const int*>(d + 3 * A),
+                             reinterpret_cast<const unsigned char*>(d + 4 * A), h->n, 0};
       } else if (mapped_host(in)) {
-        // pinned host arrays: k_bin_count reads them over PCIe (one coalesced pass) and fills the staging area
+        // pinned host arrays: k_bin_count reads them over PCIe (one coalesced pass); nothing else ever reads them
         in.stage = 1;
         src.ev[b] = in;
-        dev.ev[b] = staged;
       } else {
         // pageable host arrays: the driver stages the copies
         const size_t n = (size_t)h->n;
@@ -370,7 +371,7 @@ int lst_load_events(lst_ctx* c, int first, int n_ev, const lst_hits* hits, void*
         LST_CUDA(c, cudaMemcpyAsync(base + L.in_z, h->z, 4 * n, cudaMemcpyHostToDevice, s));
         LST_CUDA(c, cudaMemcpyAsync(base + L.in_module, h->module, 4 * n, cudaMemcpyHostToDevice, s));
         LST_CUDA(c, cudaMemcpyAsync(base + L.in_side, h->side, n, cudaMemcpyHostToDevice, s));
-        src.ev[b] = dev.ev[b] = staged;
+        src.ev[b] = staged;
       }
     }
     SlotHost& sh0 = c->slots[first + b0];
@@ -382,9 +383,9 @@ int lst_load_events(lst_ctx* c, int first, int n_ev, const lst_hits* hits, void*
       std::lock_guard<std::mutex> lock(c->stage_mu);
       StageIn st{c->stage_stream, c->stage_ev[c->stage_next % lst_ctx::kStageEvents], c->stage_ev[(c->stage_next + 1) % lst_ctx::kStageEvents]};
       c->stage_next += 2;
-      c->launches += launch_bin(P, src, dev, nb, s, c->cfg.timing ? sh0.ev : nullptr, &st);
+      c->launches += launch_bin(P, src, nb, s, c->cfg.timing ? sh0.ev : nullptr, &st);
     } else {
-      c->launches += launch_bin(P, src, dev, nb, s, c->cfg.timing ? sh0.ev : nullptr, nullptr);
+      c->launches += launch_bin(P, src, nb, s, c->cfg.timing ? sh0.ev : nullptr, nullptr);
     }
     LST_CUDA(c, cudaGetLastError());
     sh0.ev_bin = c->cfg.timing != 0;
@@ -405,9 +406,9 @@ int lst_run_stage(lst_ctx* c, int first, int n, int stage, void* stream) {
   Params P = c->P;
   P.first_slot = first;
   if (stage == LST_CLEAN)
-    c->launches += launch_clean(P, n, st, c->cfg.timing ? sh.ev + 13 : nullptr);
+    c->launches += launch_clean(P, n, st, c->cfg.timing ? sh.ev + 12 : nullptr);
   else
-    c->launches += launch_stage(P, n, stage, st, c->cfg.timing ? sh.ev + 5 + 2 * stage : nullptr);
+    c->launches += launch_stage(P, n, stage, st, c->cfg.timing ? sh.ev + 4 + 2 * stage : nullptr);
   LST_CUDA(c, cudaGetLastError());
   if (c->cfg.timing) sh.ev_stage[stage] = true;
   for (int s = first; s < first + n; ++s) { c->slots[s].synced = false; c->slots[s].stages_run = stage + 1; }
@@ -538,16 +539,16 @@ int lst_get_stats(lst_ctx* c, int slot, lst_stats* o) {
   o->n_kept = sh.stages_run > LST_CLEAN ? sh.hdr->n_kept : 0;
   if (c->cfg.timing) {
     if (sh.ev_bin) {
-      cudaEventElapsedTime(&o->stage_ms[0], sh.ev[0], sh.ev[4]);
-      for (int k = 0; k < 4; ++k) cudaEventElapsedTime(&o->kernel_ms[k], sh.ev[k], sh.ev[k + 1]);
+      cudaEventElapsedTime(&o->stage_ms[0], sh.ev[0], sh.ev[3]);
+      for (int k = 0; k < 3; ++k) cudaEventElapsedTime(&o->kernel_ms[k], sh.ev[k], sh.ev[k + 1]);
     }
     if (sh.ev_stage[4])
-      for (int k = 0; k < 4; ++k) cudaEventElapsedTime(&o->kernel_ms[8 + k], sh.ev[13 + k], sh.ev[14 + k]);
+      for (int k = 0; k < 4; ++k) cudaEventElapsedTime(&o->kernel_ms[7 + k], sh.ev[12 + k], sh.ev[13 + k]);
     for (int st = 0; st < 4; ++st)
       if (sh.ev_stage[st]) {
-        cudaEvent_t* e = sh.ev + 5 + 2 * st;
+        cudaEvent_t* e = sh.ev + 4 + 2 * st;
         cudaEventElapsedTime(&o->stage_ms[1 + st], e[0], e[1]);
-        o->kernel_ms[4 + st] = o->stage_ms[1 + st];
+        o->kernel_ms[3 + st] = o->stage_ms[1 + st];
       }
     cudaGetLastError();
   }

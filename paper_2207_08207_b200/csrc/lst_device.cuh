@@ -1,6 +1,6 @@
 // lst_device.cuh -- device-side data layout of one event slot and the kernel launch parameters.
 //
-// One arena (a single cudaMalloc in lst_create) holds n_slots identical slots;
+// One arena (allocated once in lst_create) holds n_slots identical slots;
 // every array of a slot sits at a fixed byte offset from the slot base (struct Layout), so a
 // kernel finds slot s at arena + s * slot_stride and needs no per-slot pointer table.  The
 // batch index (which slot of a batch) is blockIdx.y of every kernel.
@@ -60,10 +60,10 @@ struct SlotHeader {
   // r_min is stored as 0x7f800000 - bits so that the zeroed header means "+inf"
   int r_min_inv[2][6];
   int r_max[2][6];
-  unsigned int done[8];           // "last block done" tickets, self-resetting
+  unsigned int done[8];           // "last block done" tickets, self-resetting (never zeroed with the header)
   unsigned int ticket[4];         // next chunk of the single-pass kernels (zeroed with the header)
   int n_kept;                     // quintuplets kept by the duplicate cleaning (stage LST_CLEAN)
-  int pad_;
+  unsigned int bad_acc;           // invalid hits seen by k_bin_count so far; moved to bad_hits and cleared by its last block
 };
 
 struct Layout {
@@ -71,10 +71,12 @@ struct Layout {
   int cap_hits, cap_md, cap_seg, cap_t3, cap_t5;
   int n_chunk[4];                 // ceil(cap of the OWNER class / kChunk): hits, MD, LS, T3
   // byte offsets from the slot base (all multiples of 256)
-  size_t hdr, bin_start, lb[4];               // contiguous: zeroed by k_reset at lst_load_event
-  size_t reset_bytes;                         // bytes to zero at lst_load_event, from hdr
-  size_t in_x, in_y, in_z, in_module, in_side;// staging of host input
-  size_t tmp_kr, tmp_ki, tmp_bin, hit4, hit_key, hit_orig, hit_module;
+  size_t hdr, bin_cnt, bin_start, lb[4];      // header; bin counters (self-cleaning); bin offsets; look-back words (contiguous)
+  size_t lb_bytes;                            // bytes of the four look-back arrays, zeroed by k_bin_scatter
+  size_t in_x, in_y, in_z, in_module, in_side;// destination of host -> device copies of the caller's arrays (copy-engine paths)
+  size_t rec4, recb, reck;                    // per input hit: (x, y, z, key), (bin, arrival rank in the bin), key again (dense)
+  size_t tmp_ki, tmp_bin;                     // per hit at its unsorted place in the bin: (original index, sortable key), bin
+  size_t hit4, hit_key, hit_orig, hit_module;
   size_t md_start, mod_info, md_anchor, md_aux, md_key, md_hits, md_out, md_module;
   size_t seg_start, seg_md, seg_f;
   size_t t3_start, t3_pack, t3_seg, t3_chi2;
@@ -108,9 +110,12 @@ struct Slot {
   template <class T>
   __device__ __forceinline__ T* at(size_t off) const { return reinterpret_cast<T*>(b + off); }
   __device__ __forceinline__ SlotHeader* hdr() const { return at<SlotHeader>(L.hdr); }
+  __device__ __forceinline__ unsigned* bin_cnt() const { return at<unsigned>(L.bin_cnt); }
   __device__ __forceinline__ unsigned* bin_start() const { return at<unsigned>(L.bin_start); }
   __device__ __forceinline__ unsigned long long* lb(int kind) const { return at<unsigned long long>(L.lb[kind]); }
-  __device__ __forceinline__ int2* tmp_kr() const { return at<int2>(L.tmp_kr); }
+  __device__ __forceinline__ float4* rec4() const { return at<float4>(L.rec4); }
+  __device__ __forceinline__ int2* recb() const { return at<int2>(L.recb); }
+  __device__ __forceinline__ float* reck() const { return at<float>(L.reck); }
   __device__ __forceinline__ int2* tmp_ki() const { return at<int2>(L.tmp_ki); }
   __device__ __forceinline__ int* tmp_bin() const { return at<int>(L.tmp_bin); }
   __device__ __forceinline__ float4* hit4() const { return at<float4>(L.hit4); }
@@ -146,7 +151,7 @@ struct Slot {
   __device__ __forceinline__ int* scratch() const { return at<int>(L.scratch); }
 };
 
-// Raw input arrays of one event (caller's device pointers, or the slot's staging area).
+// Raw input arrays of one event (caller's device pointers, mapped host memory, or the slot's copy destination).
 struct HitInput {
   const float* x;
   const float* y;
@@ -154,7 +159,7 @@ struct HitInput {
   const int* module;
   const unsigned char* side;
   int n;
-  int stage;   // != 0: the arrays are mapped (pinned) host memory; k_bin_count copies them into the slot's staging area
+  int stage;   // != 0: the arrays are mapped (pinned) host memory, read by k_bin_count over PCIe
 };
 // Inputs of a batch of events: slot first_slot + b reads ev[b].
 struct HitBatch {
@@ -163,15 +168,15 @@ struct HitBatch {
 
 // Host-callable launchers (lst_kernels.cu). Each returns the number of kernels it launched.
 // `ev` (optional, timing mode): ev[0] is recorded before the first kernel, ev[k + 1] after kernel k.
-// `src`: the arrays k_bin_count reads (device, or mapped host memory with stage = 1); `dev`: the device-resident arrays
-// the later kernels read (the same, or the slot's staging area).  `stage` (non-null when k_bin_count reads host memory):
-// the library's stage-in stream and the two events that fork it from / join it to `s`.
+// `src`: the arrays k_bin_count reads (device, or mapped host memory with stage = 1); it is the only kernel that touches
+// them.  `stage` (non-null when k_bin_count reads host memory): the library's stage-in stream and the two events that fork it
+// from / join it to `s`.
 struct StageIn {
   cudaStream_t stream;
   cudaEvent_t before, after;
 };
-int launch_bin(const Params& P, const HitBatch& src, const HitBatch& dev, int n_batch, cudaStream_t s, cudaEvent_t* ev,
-               const StageIn* stage);   // 5 kernels
+int launch_bin(const Params& P, const HitBatch& src, int n_batch, cudaStream_t s, cudaEvent_t* ev,
+               const StageIn* stage);   // 3 kernels
 int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEvent_t* ev);          // 1 kernel
 // Duplicate cleaning [D]: 6 kernels (prepare, count, scan, fill, mark, list); ev[0..4] around the four steps.
 int launch_clean(const Params& P, int n_batch, cudaStream_t s, cudaEvent_t* ev);

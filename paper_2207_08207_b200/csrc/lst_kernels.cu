@@ -27,6 +27,8 @@
 //
 // blockIdx.y = index of the event within the batch (lst_run_batch): all events of a batch go
 // through one launch per kernel.
+#include <cstddef>
+
 #include "lst_device.cuh"
 
 namespace lst {
@@ -127,9 +129,9 @@ __device__ int block_scan_array4(int* a, int n) {
 // Ticket: true in every thread of the block that finishes last among `n_blocks`.
 __device__ __forceinline__ bool last_block_done(unsigned* counter, unsigned n_blocks) {
   __shared__ bool is_last;
-  __threadfence();
   __syncthreads();
   if (threadIdx.x == 0) {
+    __threadfence();   // release: cumulative over what the block's threads wrote before the barrier (as in a grid-wide sync)
     const unsigned t = atomicAdd(counter, 1u);
     is_last = (t == n_blocks - 1);
     if (is_last) atomicExch(counter, 0u);
@@ -244,125 +246,174 @@ __device__ __forceinline__ float r_max_of(const SlotHeader* h, int side, int lay
 // ------------------------------------------------------------------------------------------
 // a0: load + bin by (side, module) + order by azimuth + derive r
 // blockIdx.y = event of the batch; its input arrays come from the pointer table `B`.
+// Three launches.  The caller's arrays are read ONCE, by k_bin_count, which leaves a 28-byte record per hit; the other two
+// kernels work from records.  The slot recycles itself: the last block of k_bin_count turns the bin counters into offsets,
+// clears them for the next event and writes a fresh header; k_bin_scatter clears the look-back words on the side.
 // ------------------------------------------------------------------------------------------
-// Recycles the slot: zeroes header, bin counters and the look-back status words.
-__global__ void __launch_bounds__(256) k_reset(const __grid_constant__ Params P) {
-  Slot S(P, blockIdx.y);
-  int4* p = S.at<int4>(P.L.hdr);
-  const size_t n = P.L.reset_bytes / 16;
-  for (size_t i = (size_t)blockIdx.x * 256 + threadIdx.x; i < n; i += (size_t)gridDim.x * 256) p[i] = make_int4(0, 0, 0, 0);
+// Counters cnt[0 .. n] -> exclusive offsets start[0 .. n] (start[n] = total), counters cleared, by the whole block; the
+// counters were incremented by other blocks (ld.cg).  Arrays are padded with zeros to a multiple of 4 ints (the slot layout
+// rounds every array up to 256 bytes).  One block does this while the rest of the event's grid has retired, so what
+// counts is its latency: a tile of NT x kPer int4 is loaded with all loads in flight at once.  Returns the total.
+template <int NT, int kPer>
+__device__ int block_offsets_from_counts(unsigned* cnt, unsigned* start, int n) {
+  constexpr int W = NT / 32;
+  __shared__ int warp_tot[W];
+  __shared__ int s_carry;
+  int4* c4 = reinterpret_cast<int4*>(cnt);
+  int4* s4 = reinterpret_cast<int4*>(start);
+  const int n4 = (n + 1 + 3) / 4;
+  const int w = threadIdx.x >> 5, lane = (int)lane_id();
+  if (threadIdx.x == 0) s_carry = 0;
+  __syncthreads();
+  for (int t0 = 0; t0 < n4; t0 += NT * kPer) {
+    const int j0 = t0 + (int)threadIdx.x * kPer;
+    int4 v[kPer];
+#pragma unroll
+    for (int k = 0; k < kPer; ++k) v[k] = (j0 + k < n4) ? __ldcg(c4 + j0 + k) : make_int4(0, 0, 0, 0);
+    int mine = 0;
+#pragma unroll
+    for (int k = 0; k < kPer; ++k) mine += (v[k].x + v[k].y) + (v[k].z + v[k].w);
+    const int incl = warp_incl_scan(mine);
+    if (lane == 31) warp_tot[w] = incl;
+    __syncthreads();
+    int ex = s_carry + incl - mine, tile_total = 0;
+#pragma unroll
+    for (int i = 0; i < W; ++i) {
+      const int t = warp_tot[i];
+      ex += (i < w) ? t : 0;
+      tile_total += t;
+    }
+#pragma unroll
+    for (int k = 0; k < kPer; ++k) {
+      if (j0 + k < n4) {
+        s4[j0 + k] = make_int4(ex, ex + v[k].x, ex + v[k].x + v[k].y, ex + v[k].x + v[k].y + v[k].z);
+        c4[j0 + k] = make_int4(0, 0, 0, 0);
+      }
+      ex += (v[k].x + v[k].y) + (v[k].z + v[k].w);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) s_carry += tile_total;
+    __syncthreads();
+  }
+  return s_carry;
 }
 
-// One pass over the caller's arrays: histogram by (side, module); the value the atomic returns is
-// the hit's arrival rank in its bin, kept with its azimuth key so that the scatter needs no second
-// atomic.  If the arrays are mapped host memory (in.stage) this pass IS the host-to-device copy:
-// every array is read once over PCIe, coalesced, and written to the slot's staging area, which is
-// what the later kernels read.  k_scan then turns the counts into bin offsets.
+// One pass over the caller's arrays -- the only one: per hit its azimuth key and, from the atomic on its (side, module)
+// counter, its arrival rank in the bin, kept with the coordinates as a record (16 + 8 + 4 bytes: the key is stored twice,
+// densely for the scatter and beside the coordinates for the final gather).  If the arrays are mapped host
+// memory (in.stage) this pass IS the host-to-device copy: every array is read once over PCIe, coalesced.
+// The block that finishes last in the event turns the counters into bin offsets (clearing them for the next event) and
+// writes the header afresh: hit counts, dropped hits, every accumulator and ticket of the stage kernels at zero.
 __global__ void __launch_bounds__(256) k_bin_count(const __grid_constant__ Params P, const __grid_constant__ HitBatch B) {
   Slot S(P, blockIdx.y);
   const HitInput& in = B.ev[blockIdx.y];
-  unsigned* cnt = S.bin_start();
-  int2* kr = S.tmp_kr();
+  SlotHeader* H = S.hdr();
+  unsigned* cnt = S.bin_cnt();
+  float4* rec4 = S.rec4();
+  int2* recb = S.recb();
+  float* reck = S.reck();
   const int nmod = P.L.n_modules;
-  float* sx = S.at<float>(P.L.in_x);
-  float* sy = S.at<float>(P.L.in_y);
-  float* sz = S.at<float>(P.L.in_z);
-  int* sm = S.at<int>(P.L.in_module);
-  unsigned char* ss = S.at<unsigned char>(P.L.in_side);
   int bad = 0;
   for (int h = blockIdx.x * blockDim.x + threadIdx.x; h < in.n; h += gridDim.x * blockDim.x) {
     const int m = in.module[h];
     const unsigned sd = in.side[h];
-    const float x = in.x[h], y = in.y[h];
-    if (in.stage) {
-      sx[h] = x; sy[h] = y; sz[h] = in.z[h]; sm[h] = m; ss[h] = (unsigned char)sd;
+    const float x = in.x[h], y = in.y[h], z = in.z[h];
+    int bin = -1, rank = 0;
+    float k = 0.0f;
+    if (m < 0 || m >= nmod || sd > 1u) {
+      ++bad;
+    } else {
+      const float2 cs = P.mod_cs[m];
+      // azimuth relative to the module normal; non-finite hits (they can never pass a cut) go last
+      k = atan2f(cs.x * y - cs.y * x, cs.x * x + cs.y * y);
+      if (!(fabsf(k) <= 4.0f)) k = 3.0e38f;
+      bin = (int)sd * nmod + m;
+      rank = (int)atomicAdd(cnt + bin, 1u);
     }
-    if (m < 0 || m >= nmod || sd > 1u) { ++bad; continue; }
-    const float2 cs = P.mod_cs[m];
-    // azimuth relative to the module normal; non-finite hits (they can never pass a cut) go last
-    float k = atan2f(cs.x * y - cs.y * x, cs.x * x + cs.y * y);
-    if (!(fabsf(k) <= 4.0f)) k = 3.0e38f;
-    const unsigned rank = atomicAdd(cnt + ((int)sd * nmod + m), 1u);
-    kr[h] = make_int2(__float_as_int(k), (int)rank);
+    rec4[h] = make_float4(x, y, z, k);
+    recb[h] = make_int2(bin, rank);
+    reck[h] = k;
   }
-  if (bad) atomicAdd(&S.hdr()->bad_hits, bad);
+  if (bad) atomicAdd(&H->bad_acc, (unsigned)bad);
+  if (!last_block_done(&H->done[0], gridDim.x)) return;
+  unsigned* start = S.bin_start();
+  const int total = block_offsets_from_counts<256, 2>(cnt, start, P.L.n_bins);   // small tiles: the tail must not set the kernel's register count
+  // fresh header: everything but the self-resetting tickets
+  int* hw = reinterpret_cast<int*>(H);
+  constexpr int kDone0 = offsetof(SlotHeader, done) / 4, kDone1 = offsetof(SlotHeader, ticket) / 4, kBad = offsetof(SlotHeader, bad_acc) / 4;
+  for (int i = threadIdx.x; i < (int)(sizeof(SlotHeader) / 4); i += blockDim.x)
+    if ((i < kDone0 || i >= kDone1) && i != kBad) hw[i] = 0;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    H->n_hits = total;
+    H->n_lower = (int)start[nmod];
+    H->bad_hits = (int)H->bad_acc;
+    H->bad_acc = 0;
+  }
 }
 
-// Counters to offsets, one block of 1024 threads per event: which = 0 the (side, module) bins of a0 (also
-// publishes the hit counts), which = 1 the MD -> quintuplet incidence counters of the cleaning stage.
-__global__ void __launch_bounds__(1024) k_scan(const __grid_constant__ Params P, int which) {
+// Counters to offsets for the MD -> quintuplet incidence table of the cleaning stage: one block of 1024 threads per event.
+__global__ void __launch_bounds__(1024) k_scan(const __grid_constant__ Params P) {
   Slot S(P, blockIdx.y);
-  SlotHeader* H = S.hdr();
-  if (which == 0) {
-    int* start = reinterpret_cast<int*>(S.bin_start());
-    const int total = block_scan_array4<1024, 3>(start, P.L.n_bins);
-    if (threadIdx.x == 0) {
-      H->n_hits = total;
-      H->n_lower = start[P.L.n_modules];
-    }
-  } else {
-    block_scan_array4<1024, 3>(S.inc_start(), H->n[LST_MD_]);
-  }
+  block_scan_array4<1024, 3>(S.inc_start(), S.hdr()->n[LST_MD_]);
 }
 
-// (key, original index) of every hit to bin offset + arrival rank.  `B` holds device-resident arrays.
+// (original index, key) of every hit to its (unsorted) place in its bin: bin offset + arrival rank -- no second atomic.
+// On the side: the look-back words of the stage kernels are cleared for this event.
 __global__ void __launch_bounds__(256) k_bin_scatter(const __grid_constant__ Params P, const __grid_constant__ HitBatch B) {
   Slot S(P, blockIdx.y);
-  const HitInput& in = B.ev[blockIdx.y];
+  const int n = B.ev[blockIdx.y].n;
   const unsigned* start = S.bin_start();
-  const int2* kr = S.tmp_kr();
+  const int2* recb = S.recb();
+  const float* reck = S.reck();
   int2* tki = S.tmp_ki();
   int* tbin = S.tmp_bin();
-  const int nmod = P.L.n_modules;
-  for (int h = blockIdx.x * blockDim.x + threadIdx.x; h < in.n; h += gridDim.x * blockDim.x) {
-    const int m = in.module[h];
-    const unsigned sd = in.side[h];
-    if (m < 0 || m >= nmod || sd > 1u) continue;
-    const int b = (int)sd * nmod + m;
-    const int2 v = kr[h];
-    const unsigned pos = start[b] + (unsigned)v.y;
-    tki[pos] = make_int2(h, (int)sortable_of(__int_as_float(v.x)));   // little endian: (index, key) = key in the high word
-    tbin[pos] = b;
+  const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
+  int4* lb = S.at<int4>(P.L.lb[0]);
+  for (int i = tid; i < (int)(P.L.lb_bytes / 16); i += nth) lb[i] = make_int4(0, 0, 0, 0);
+  for (int h = tid; h < n; h += nth) {
+    const int2 b = recb[h];
+    if (b.x < 0) continue;
+    const unsigned pos = start[b.x] + (unsigned)b.y;
+    tki[pos] = make_int2(h, (int)sortable_of(reck[h]));   // little endian: (index, key) = key in the high word
+    tbin[pos] = b.x;
   }
 }
 
-// One thread per hit: its rank inside the bin by (key, original index) is the number of hits
-// of the bin that come before it -- a loop over the bin (6 hits on average, all lanes busy
-// whatever the bin sizes; neighbouring threads sit in the same or the next bin).  Then gather the
-// coordinates, derive r, and keep the range of r per (side, layer) and the key range per module.
-__global__ void __launch_bounds__(256) k_bin_order(const __grid_constant__ Params P, const __grid_constant__ HitBatch B) {
+// One thread per hit: its rank inside the bin by (key, original index) is the number of hits of the bin that come
+// before it -- a loop over the bin (6 hits on average, all lanes busy whatever the bin sizes; neighbouring threads sit
+// in the same or the next bin).  Then fetch the hit's record (one 16-byte gather), derive r, and keep the range of r per
+// (side, layer) and the key range per module.
+__global__ void __launch_bounds__(256) k_bin_order(const __grid_constant__ Params P) {
   __shared__ int s_rng[24];
   Slot S(P, blockIdx.y);
-  const HitInput& in = B.ev[blockIdx.y];
   SlotHeader* H = S.hdr();
   const int nmod = P.L.n_modules;
   if (threadIdx.x < 24) s_rng[threadIdx.x] = 0;
   __syncthreads();
   const int nh = H->n_hits;
   const unsigned* start = S.bin_start();
-  const int2* tki = S.tmp_ki();
+  const unsigned long long* tk = reinterpret_cast<const unsigned long long*>(S.tmp_ki());
   int* info = reinterpret_cast<int*>(S.mod_info());
   const int p = blockIdx.x * 256 + threadIdx.x;
   if (p < nh) {
     const int b = S.tmp_bin()[p];
     const int s = (int)start[b], e = (int)start[b + 1];
-    const unsigned long long* tk = reinterpret_cast<const unsigned long long*>(tki);
     const unsigned long long mine = tk[p];                   // (sortable key << 32) | original index
-    const int2 me = make_int2(__float_as_int(float_of_sortable((unsigned)(mine >> 32))), (int)(unsigned)mine);
-    const float key = __int_as_float(me.x);
+    const int orig = (int)(unsigned)mine;
+    const float4 v = S.rec4()[orig];                         // (x, y, z, key)
     int rank = 0;
     for (int j = s; j < e; ++j) rank += tk[j] < mine;
     const int side = b >= nmod, m = b - side * nmod;
-    const float x = in.x[me.y], y = in.y[me.y], z = in.z[me.y];
-    const float r = sqrtf(x * x + y * y);
+    const float r = sqrtf(v.x * v.x + v.y * v.y);
     const int dst = s + rank;
-    S.hit4()[dst] = make_float4(x, y, z, r);
-    S.hit_key()[dst] = key;
-    S.hit_orig()[dst] = me.y;
+    S.hit4()[dst] = make_float4(v.x, v.y, v.z, r);
+    S.hit_key()[dst] = v.w;
+    S.hit_orig()[dst] = orig;
     S.hit_module()[dst] = m;
     if (!side) {
-      if (rank == 0) info[4 * m + 2] = me.x;
-      if (rank == e - s - 1) info[4 * m + 3] = me.x;
+      if (rank == 0) info[4 * m + 2] = __float_as_int(v.w);
+      if (rank == e - s - 1) info[4 * m + 3] = __float_as_int(v.w);
     }
     // range of r per (side, layer): neighbouring threads sit in the same or the next bin, so a warp
     // holds one or two (side, layer) groups -- one shared-memory atomic pair per group, not per hit
@@ -1532,16 +1583,13 @@ static int blocks_per_event(int wanted, int n_batch, int resident_per_sm, int sh
   return max(1, min(wanted, per_event));
 }
 
-int launch_bin(const Params& P, const HitBatch& src, const HitBatch& dev, int n_batch, cudaStream_t s, cudaEvent_t* ev,
-               const StageIn* stage) {
+int launch_bin(const Params& P, const HitBatch& src, int n_batch, cudaStream_t s, cudaEvent_t* ev, const StageIn* stage) {
   int n_max = 0;
   for (int b = 0; b < n_batch; ++b) n_max = max(n_max, src.ev[b].n);
   const unsigned nb = (unsigned)n_batch;
-  // one hit per thread: the loads and the scattered stores of all hits are in flight at once
+  // one hit per thread: the loads, the atomics and the scattered stores of all hits are in flight at once
   const dim3 g(max(1, (n_max + 255) / 256), nb);
   LST_EV(0);
-  k_reset<<<dim3(blocks_per_event((int)(P.L.reset_bytes / 16 + 255) / 256, n_batch, 8), nb), 256, 0, s>>>(P);
-  LST_EV(1);
   if (stage) {
     // Reading pinned host memory the kernel is PCIe bound (~75 KB in flight cover latency x bandwidth): a small
     // grid, on the library's own high-priority stream so that its blocks are placed ahead of the other streams'
@@ -1549,19 +1597,19 @@ int launch_bin(const Params& P, const HitBatch& src, const HitBatch& dev, int n_
     cudaEventRecord(stage->before, s);
     cudaStreamWaitEvent(stage->stream, stage->before, 0);
     k_bin_count<<<dim3(min((int)g.x, 8), nb), 256, 0, stage->stream>>>(P, src);
-    k_scan<<<dim3(1, nb), 1024, 0, stage->stream>>>(P, 0);
     cudaEventRecord(stage->after, stage->stream);
     cudaStreamWaitEvent(s, stage->after, 0);
   } else {
-    k_bin_count<<<dim3(blocks_per_event((int)g.x, n_batch, 6), nb), 256, 0, s>>>(P, src);   // 40 registers: 6 blocks per SM
-    k_scan<<<dim3(1, nb), 1024, 0, s>>>(P, 0);
+    // grid-stride with about one wave of blocks: a block ends with a release fence (last_block_done) that waits for
+    // its stores and atomics, so fewer, longer-lived blocks beat one hit per thread
+    k_bin_count<<<dim3(blocks_per_event((int)g.x, n_batch, 8), nb), 256, 0, s>>>(P, src);
   }
+  LST_EV(1);
+  k_bin_scatter<<<g, 256, 0, s>>>(P, src);
   LST_EV(2);
-  k_bin_scatter<<<g, 256, 0, s>>>(P, dev);
+  k_bin_order<<<dim3((max(n_max, P.L.n_modules) + 255) / 256, nb), 256, 0, s>>>(P);
   LST_EV(3);
-  k_bin_order<<<dim3((max(n_max, P.L.n_modules) + 255) / 256, nb), 256, 0, s>>>(P, dev);
-  LST_EV(4);
-  return 5;
+  return 3;
 }
 
 int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEvent_t* ev) {
@@ -1594,7 +1642,7 @@ int launch_clean(const Params& P, int n_batch, cudaStream_t s, cudaEvent_t* ev) 
   k_clean_prepare<<<g, 256, 0, s>>>(P);
   LST_EV(1);
   k_clean_count<<<g, 256, 0, s>>>(P);
-  k_scan<<<dim3(1, (unsigned)n_batch), 1024, 0, s>>>(P, 1);
+  k_scan<<<dim3(1, (unsigned)n_batch), 1024, 0, s>>>(P);
   LST_EV(2);
   k_clean_fill<<<g, 256, 0, s>>>(P);
   LST_EV(3);

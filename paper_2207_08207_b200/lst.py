@@ -21,8 +21,8 @@ N_LAYERS = 6
 MD, SEG, T3, T5 = 0, 1, 2, 3
 CLEAN = 4                                      # optional stage: duplicate cleaning of the quintuplets (run_stage only)
 KIND_NAMES = ("md", "seg", "t3", "t5")
-KERNEL_NAMES = ("reset", "bin_count", "bin_scatter", "bin_order", "md", "seg", "t3", "t5",
-                "clean_prepare", "clean_count", "clean_fill", "clean_mark")   # lst_stats.kernel_ms[0..11]
+KERNEL_NAMES = ("bin_count", "bin_scatter", "bin_order", "md", "seg", "t3", "t5",
+                "clean_prepare", "clean_count", "clean_fill", "clean_mark")   # lst_stats.kernel_ms[0..10]
 HITS_PER_OBJECT = (2, 4, 6, 10, 10)       # [CLEAN]: the kept quintuplets
 VALUES_PER_OBJECT = (4, 4, 2, 5, 5)
 
