@@ -310,21 +310,25 @@ def run_ours(args):
         sets.append({"base": p * N_EVENTS, "streams": streams if p == 0 else [torch.cuda.Stream(dev) for _ in range(N_STREAMS)],
                      "idx": [[out[k][0] for k in range(s * per_stream, (s + 1) * per_stream)] for s in range(N_STREAMS)],
                      "val": [[out[k][1] for k in range(s * per_stream, (s + 1) * per_stream)] for s in range(N_STREAMS)],
+                     # the same pinned memory seen as binary16 rows, for the reduced-precision store
+                     "val_h": [[out[k][1].view(np.float16).reshape(-1)[:cap5 * 5].reshape(cap5, 5) for k in range(s * per_stream, (s + 1) * per_stream)]
+                               for s in range(N_STREAMS)],
                      "counts": None})
 
     e2e_kind = [lst.T5]                             # lst.CLEAN: the path + cleaning stage, only the kept quintuplets travel back
+    e2e_ctx = [ctx, "val"]                          # the context the end-to-end arm drives and the result buffers it fills
 
     def e2e_launch(i):                              # H2D of the pinned hit SoA + a0..a4 of step i, all asynchronous
         S = sets[i % 2]
         for s, st in enumerate(S["streams"]):
-            ctx.load_events(S["base"] + s * per_stream, np_in[s * per_stream:(s + 1) * per_stream], stream=st)
-            ctx.run_batch(S["base"] + s * per_stream, per_stream, st)
+            e2e_ctx[0].load_events(S["base"] + s * per_stream, np_in[s * per_stream:(s + 1) * per_stream], stream=st)
+            e2e_ctx[0].run_batch(S["base"] + s * per_stream, per_stream, st)
             if e2e_kind[0] == lst.CLEAN:
-                ctx.run_stage(S["base"] + s * per_stream, per_stream, lst.CLEAN, st)
+                e2e_ctx[0].run_stage(S["base"] + s * per_stream, per_stream, lst.CLEAN, st)
 
     def e2e_collect(i):                             # counters back (one sync per stream), then gathers + D2H enqueued
         S = sets[i % 2]
-        S["counts"] = [ctx.fetch_batch(S["base"] + s * per_stream, e2e_kind[0], S["idx"][s], S["val"][s], stream=st, wait=False)
+        S["counts"] = [e2e_ctx[0].fetch_batch(S["base"] + s * per_stream, e2e_kind[0], S["idx"][s], S[e2e_ctx[1]][s], stream=st, wait=False)
                        for s, st in enumerate(S["streams"])]
 
     def e2e_run(n):
@@ -415,6 +419,45 @@ def run_ours(args):
              "t5_in": needed[3], "t5_kept": kept,
              "what": "a0..a4 + LST_CLEAN per step; `value` above is a0..a4 only (the BASELINE.json path)"}
 
+    arena_mib = ctx.arena_bytes()[0] / 2 ** 20
+    # ---- reduced-precision object store [H]: the same measurements with
+    # lst_config.store_half: output floats that no selection reads kept as binary16, everything else unchanged ----
+    ctx.close()
+    cfg_h = lst.default_config()
+    cfg_h.device, cfg_h.n_slots, cfg_h.store_half = local, 2 * N_EVENTS, 1
+    ctx_h = lst.Lst.from_synth(geom, mmap, cfg_h)
+
+    def step_device_half():
+        for s, st in enumerate(streams):
+            ctx_h.load_events(s * per_stream, d_in[s * per_stream:(s + 1) * per_stream], stream=st)
+            ctx_h.run_batch(s * per_stream, per_stream, st)
+    timed(step_device_half, 3)
+    half_total_ms = max_over_ranks(sum(timed(step_device_half, args.steps)), dist, dev)
+    for s, st in enumerate(streams):
+        ctx_h.sync_batch(s * per_stream, per_stream, st)
+    assert [ctx_h.stats(k)["needed"] for k in range(N_EVENTS)] == [st_["needed"] for st_ in stats], "half store changed the object counts"
+    e2e_ctx[0], e2e_ctx[1] = ctx_h, "val_h"
+    e2e_run(3)
+    barrier()
+    t0 = time.perf_counter()
+    e2e_run(e2e_steps)
+    torch.cuda.synchronize(dev)
+    e2e_h_s = max_over_ranks(time.perf_counter() - t0, dist, dev)
+    ctx_h.close()
+    half_ms, _ = per_kernel_times(lst, geom, mmap, d_in, local, store_half=True)
+    half_alone_ms, _ = per_kernel_times(lst, geom, mmap, d_in, local, alone=True, reps=3, store_half=True)
+    stored = lambda h: needed[0] * (8, 4)[h] + needed[1] * (16, 8)[h] + needed[2] * (4, 2)[h] + needed[3] * ((20, 10)[h] + 4)
+    half = {"what": "lst_config.store_half = 1: MD (dphi, dphichange), LS (sinS, z0, dphi, dphichange), T3 chi2rz, T5 (5 values) stored and "
+                    "downloaded as binary16 (round to nearest even of the fp32 result); selections, sets and [D] unchanged (DESIGN.md [H])",
+            "events_per_s": whole_job_events_per_s(world, args.steps, half_total_ms), "events_per_s_fp32": value,
+            "ms_per_step": half_total_ms / args.steps, "ms_per_step_fp32": total_ms / args.steps,
+            "kernels_ms_in_step": {k: {"fp32": kernel_ms[k], "half": half_ms[k]} for k in ("md", "seg", "t3", "t5")},
+            "kernels_ms_alone": {k: {"fp32": alone_ms[k], "half": half_alone_ms[k]} for k in ("md", "seg", "t3", "t5")},
+            "output_float_bytes_per_step": {"fp32": int(stored(0)), "half": int(stored(1))},
+            "algorithmic_bytes_per_step_fp32": int(sum(algorithmic_bytes(i, n_hits, needed) for i in range(5))),
+            "e2e": {"value": world * N_EVENTS * e2e_steps / e2e_h_s, "value_fp32": e2e["value"], "unit": UNIT,
+                    "d2h_bytes_per_step": int(needed[3] * (40 + 10) + N_EVENTS * HEADER_BYTES), "d2h_bytes_per_step_fp32": int(d2h)}}
+
     # ---- the step before the path: module-map builder [B], built once per geometry ----
     from paper_2207_08207_b200 import synth as _synth
     mg = _synth.map_geometry(geom)
@@ -444,9 +487,9 @@ def run_ours(args):
                                      "the durations with the GPU otherwise idle: what the 4-stream pipeline gains over running the same "
                                      "launches back to back"},
            "csrc_digest": csrc_digest(),
-           "duplicate_cleaning": clean, "module_map_builder": map_builder,
+           "duplicate_cleaning": clean, "reduced_precision_store": half, "module_map_builder": map_builder,
            "rewalks_per_step": dict(md=rewalks[0], ls=rewalks[1], t3=rewalks[2], t5=rewalks[3]),
-           "arena_mib": ctx.arena_bytes()[0] / 2 ** 20, "impl": "ours"}
+           "arena_mib": arena_mib, "impl": "ours"}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         n_pass, t_cpu = 0, 0.0
         while t_cpu < 12.0 and n_pass < 8:          # a bounded sample: whole passes over the workload, >= 12 s of CPU work
@@ -524,7 +567,7 @@ def pcie_ceiling(torch, dev, np_in, out_bytes, S, reps=10):
                     "no kernel running"}
 
 
-def per_kernel_times(lst, geom, mmap, d_in, local, with_clean=False, reps=6, alone=False):
+def per_kernel_times(lst, geom, mmap, d_in, local, with_clean=False, reps=6, alone=False, store_half=False):
     """Average duration (ms) of ONE launch of every kernel, from CUDA events recorded by the library around every launch on
     the stream it is launched on (lst_config.timing), L2 flushed before every step.
     alone=False: the configuration the timed region uses -- 4 streams x 16-event launches running concurrently (concurrent
@@ -533,7 +576,7 @@ def per_kernel_times(lst, geom, mmap, d_in, local, with_clean=False, reps=6, alo
     The optional cleaning stage [D] is timed the same way."""
     import torch
     cfg = lst.default_config()
-    cfg.device, cfg.n_slots, cfg.timing = local, N_EVENTS, 1
+    cfg.device, cfg.n_slots, cfg.timing, cfg.store_half = local, N_EVENTS, 1, int(store_half)
     ctx = lst.Lst.from_synth(geom, mmap, cfg)
     streams = [torch.cuda.Stream() for _ in range(N_STREAMS)]
     per = N_EVENTS // N_STREAMS

@@ -116,6 +116,12 @@ typedef struct {
   int32_t cap_t5;
   int32_t timing;     /* != 0: record CUDA events around every kernel (lst_get_stats.stage_ms /
                          kernel_ms; for a batch they are kept on its first slot) */
+  int32_t store_half; /* != 0: reduced-precision object store ("exploring data types such as half precision
+                         floats"; DESIGN.md section 1 [H]): the per-object OUTPUT floats that no later selection reads -- MD
+                         (dphi, dphichange), LS (sinS, z0, dphi, dphichange), T3 chi2rz, T5 (kappa_in, kappa_out, kappa_fit,
+                         chi2xy, chi2rz) -- are stored as IEEE binary16, rounded to nearest even from the fp32 value; all
+                         arithmetic and everything a selection reads stay fp32, so the object sets do not change.  The views
+                         then expose these arrays through their *_h members and the fetched float payloads are binary16 */
   int32_t t5_dup_min_shared; /* [D] D4: quintuplets sharing at least this many of their 10 original hits
                          are duplicates (7).  Accepted range 6 .. 10 (lst_create returns LST_ERR_ARG otherwise): the
                          stage finds partners through a common mini-doublet, which >= 6 common hits imply and
@@ -151,31 +157,35 @@ typedef struct {
   const int32_t* module;       /* [n]                                                         */
   const float* anchor;         /* [n][4] x, y, z, r of the anchor (lower) hit, 16-B aligned   */
   const float* ur_sina;        /* [n][2] r of the upper hit, sinA                             */
-  const float* dphi_dphichange;/* [n][2]                                                      */
+  const float* dphi_dphichange;/* [n][2]  (NULL when lst_config.store_half)                   */
   const int32_t* module_start; /* [n_modules + 1] MDs of module m are [start[m], start[m+1])  */
+  const uint16_t* dphi_dphichange_h; /* [n][2] binary16 (NULL unless lst_config.store_half)   */
 } lst_md_view;
 
 typedef struct {
   int32_t n;
   const int32_t* md;       /* [n][2] inner MD, outer MD                                        */
-  const float* f;          /* [n][4] sinS, z0, dphi, dphichange                                */
+  const float* f;          /* [n][4] sinS, z0, dphi, dphichange (NULL when store_half)         */
   const int32_t* md_start; /* [n_md + 1] segments with inner MD i are [start[i], start[i+1])   */
+  const uint16_t* f_h;     /* [n][4] the same as binary16 (NULL unless store_half)              */
 } lst_seg_view;
 
 typedef struct {
   int32_t n;
   const int32_t* md_kappa; /* [n][4] MD1, MD2, MD3, bit pattern of kappa (fp32)                 */
   const int32_t* seg;      /* [n][2] first segment, second segment                              */
-  const float* chi2rz;     /* [n]                                                               */
+  const float* chi2rz;     /* [n] (NULL when store_half)                                        */
   const int32_t* seg_start;/* [n_seg + 1] triplets with first segment a are [start[a], start[a+1]) */
+  const uint16_t* chi2rz_h;/* [n] binary16 (NULL unless store_half)                             */
 } lst_t3_view;
 
 typedef struct {
   int32_t n;
   const int32_t* md;       /* [n][5] MD1 .. MD5                                                 */
   const int32_t* t3;       /* [n][2] inner triplet, outer triplet                               */
-  const float* f;          /* [n][5] kappa_in, kappa_out, kappa_fit, chi2xy, chi2rz             */
+  const float* f;          /* [n][5] kappa_in, kappa_out, kappa_fit, chi2xy, chi2rz (NULL when store_half) */
   const int32_t* t3_start; /* [n_t3 + 1] quintuplets with inner triplet A are [start[A], start[A+1]) */
+  const uint16_t* f_h;     /* [n][5] the same as binary16 (NULL unless store_half)              */
 } lst_t5_view;
 
 /* Result of the optional duplicate-cleaning stage (DESIGN.md section 1 [D]): the
@@ -185,7 +195,7 @@ typedef struct {
   int32_t n;            /* quintuplets kept                                                       */
   const int32_t* t5;    /* [n] their indices into lst_t5_view, ascending                          */
   const uint8_t* keep;  /* [n_t5] 1 = kept                                                        */
-  const float* score;   /* [n_t5] chi2xy + chi2rz                                                 */
+  const float* score;   /* [n_t5] chi2xy + chi2rz, the fp32 sum of the fp32 values (also when store_half)  */
 } lst_tc_view;
 
 typedef struct {
@@ -263,15 +273,17 @@ LST_API int lst_get_stats(lst_ctx* ctx, int slot, lst_stats* out);
  * Synchronises `cuda_stream`. */
 LST_API int lst_fetch_hit_indices(lst_ctx* ctx, int slot, int kind, int32_t* out, int64_t cap_objects, void* cuda_stream);
 /* Float payload of class `kind` to HOST memory: MD [n][4] sinA, dphi, dphichange, r_anchor;
- * LS [n][4] sinS, z0, dphi, dphichange; T3 [n][2] kappa, chi2rz; T5 [n][5] as lst_t5_view.f. */
-LST_API int lst_fetch_values(lst_ctx* ctx, int slot, int kind, float* out, int64_t cap_objects, void* cuda_stream);
+ * LS [n][4] sinS, z0, dphi, dphichange; T3 [n][2] kappa, chi2rz; T5 [n][5] as lst_t5_view.f.
+ * fp32 values, or -- with lst_config.store_half -- binary16 values in the same order ([n][k] uint16_t; columns that are kept
+ * in fp32 for the selections, e.g. sinA or kappa, are rounded to nearest even on the way out). */
+LST_API int lst_fetch_values(lst_ctx* ctx, int slot, int kind, void* out, int64_t cap_objects, void* cuda_stream);
 
 /* Result download for a batch of slots in one call (the end-to-end path of a multi-event
  * pipeline): synchronises the slots if they are not yet (lst_sync_batch), then
  * for slot first_slot + b gathers the hit-index tuples of class `kind` (LST_MD .. LST_T5, or LST_CLEAN =
  * the quintuplets kept by the cleaning stage only, in the layout of LST_T5) on the device and enqueues
  * their copy to the HOST buffer idx_out[b] ([n][2|4|6|10] int32) and the copy of the float payload
- * (layout as lst_fetch_values) to val_out[b].  idx_out / val_out may be NULL, and so may single
+ * (layout and element type as lst_fetch_values: fp32, or binary16 with lst_config.store_half) to val_out[b].  idx_out / val_out may be NULL, and so may single
  * entries (nothing is copied for them).  cap_objects[b] = rows available in slot b's buffers;
  * counts[b] (may be NULL) receives the object count.  One gather launch per table for the whole
  * batch.  Pinned (page-locked) host buffers are written by ONE kernel per 16 slots directly over PCIe
@@ -280,7 +292,7 @@ LST_API int lst_fetch_values(lst_ctx* ctx, int slot, int kind, float* out, int64
  * enqueued and the buffers are complete once `cuda_stream` has been synchronised by the caller.  Errors: LST_ERR_STATE (a slot not run), LST_ERR_OVERFLOW,
  * LST_ERR_ARG (a buffer too small: nothing is copied), LST_ERR_CUDA. */
 LST_API int lst_fetch_batch(lst_ctx* ctx, int first_slot, int n_slots, int kind, int32_t* const* idx_out,
-                            float* const* val_out, const int64_t* cap_objects, int32_t* counts, int wait,
+                            void* const* val_out, const int64_t* cap_objects, int32_t* counts, int wait,
                             void* cuda_stream);
 
 /* ---- module-map builder: the step before the path (DESIGN.md section 1 [B]) ---------------- */

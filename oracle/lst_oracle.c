@@ -698,6 +698,45 @@ int64_t lsto_build_map(int32_t n, const int8_t* layer, const double* phi, const 
   return total;
 }
 
+/* ------------------------------------------------------------------------------------ */
+/* [H] reduced-precision object store  (DESIGN.md section 1 [H])        */
+/* ------------------------------------------------------------------------------------ */
+/* The paper names half precision as future work ("exploring data types such as half precision
+ * floats"); the reading (reading 27) stores the per-object OUTPUT floats that no later selection reads as
+ * IEEE 754 binary16, each the value nearest to the fp32 result, ties to even; overflow goes to infinity, values
+ * below the smallest subnormal to (signed) zero, NaN stays NaN.  This is that rounding, on the bit patterns, so that it
+ * does not depend on the compiler's or the CPU's half-precision support.  Pin P21: equals numpy's float32 -> float16
+ * conversion on every binary16 value, on every tie and on random inputs (tests/test_oracle_half.py). */
+uint16_t lsto_half_bits(float f) {
+  uint32_t x, sign, e, m, q, rem, half;
+  int shift;
+  memcpy(&x, &f, 4);
+  sign = (x >> 16) & 0x8000u;
+  x &= 0x7fffffffu;
+  if (x > 0x7f800000u) return (uint16_t)(sign | 0x7e00u | ((x >> 13) & 0x1ffu));   /* NaN (quiet, payload kept) */
+  if (x >= 0x477ff000u) return (uint16_t)(sign | 0x7c00u);   /* >= 65520 = max half + half an ulp: infinity */
+  e = x >> 23;
+  if (e < 113u) {                                             /* below 2^-14: subnormal half, unit 2^-24 */
+    if (e < 102u) return (uint16_t)sign;                      /* below 2^-25: zero */
+    m = (x & 0x7fffffu) | 0x800000u;
+    shift = (int)(126u - e);                                  /* 14 .. 24 */
+    q = m >> shift;
+    rem = m & ((1u << shift) - 1u);
+    half = 1u << (shift - 1);
+  } else {
+    m = x & 0x7fffffu;
+    q = ((e - 112u) << 10) | (m >> 13);
+    rem = m & 0x1fffu;
+    half = 0x1000u;
+  }
+  if (rem > half || (rem == half && (q & 1u))) ++q;           /* nearest, ties to even; a carry moves to the next binade */
+  return (uint16_t)(sign | q);
+}
+void lsto_half_bits_array(int64_t n, const float* in, uint16_t* out) {
+  int64_t i;
+  for (i = 0; i < n; ++i) out[i] = lsto_half_bits(in[i]);
+}
+
 /* ---- accessors for the ctypes wrapper ---- */
 int64_t lsto_count(const lsto_event* ev, int kind) {
   switch (kind) { case 0: return ev->n_md; case 1: return ev->n_seg; case 2: return ev->n_t3; case 3: return ev->n_t5; }

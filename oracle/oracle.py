@@ -90,6 +90,8 @@ class OracleLib:
             f.restype = C.c_int
         lib.lsto_t5_clean.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
         lib.lsto_t5_clean.restype = C.c_int64
+        lib.lsto_half_bits_array.argtypes = [C.c_int64, C.c_void_p, C.c_void_p]
+        lib.lsto_half_bits_array.restype = None
 
     # ---- configuration -------------------------------------------------------------------
     def default_config(self):
@@ -148,6 +150,13 @@ class OracleLib:
         kept = self.lib.lsto_t5_clean(C.c_int64(n), ptr(hits), ptr(cx), ptr(cz), int(min_shared), ptr(keep))
         assert kept == int(keep[:n].sum())
         return keep[:n].astype(bool)
+
+    def half_bits(self, values) -> np.ndarray:
+        """[H] binary16 bit patterns (uint16) of fp32 values, round to nearest even (reduced-precision object store)."""
+        v = np.ascontiguousarray(values, np.float32)
+        out = np.zeros(v.shape, np.uint16)
+        self.lib.lsto_half_bits_array(C.c_int64(v.size), v.ctypes.data_as(C.c_void_p), out.ctypes.data_as(C.c_void_p))
+        return out
 
     def build_map(self, layer, phi, rho, gap, hw, zlo, zhi, pt_min=0.8, b_tesla=3.8, z0_max=15.0, pad_phi=0.01, pad_z=1.0):
         """[B] module-map builder (always double precision). Returns (row_offsets, targets)."""

@@ -43,7 +43,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and up_to_date():
         return LIB
     tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [nvcc(), *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []),
+    cmd = [nvcc(), *NVCC_FLAGS, *os.environ.get("LST_NVCC_EXTRA", "").split(), *(["-Xptxas", "-v"] if verbose else []),
            *[os.path.join(CSRC, s) for s in SOURCES], "-o", tmp]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or r.returncode:

@@ -193,6 +193,7 @@ int lst_default_config(lst_config* c) {
   c->cap_t5 = 128 * 1024;
   c->timing = 0;
   c->t5_dup_min_shared = 7;
+  c->store_half = 0;
   return LST_OK;
 }
 
@@ -288,6 +289,7 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
   c->P.map_dphi = c->d_map_dphi;
   c->P.first_slot = 0;
   c->P.dup_min_shared = cfg.t5_dup_min_shared;
+  c->P.store_half = cfg.store_half != 0;
   if ((e = cudaDeviceSynchronize()) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   *out = c;
   return LST_OK;
@@ -458,7 +460,8 @@ int lst_get_mds(lst_ctx* c, int slot, lst_md_view* v) {
   v->module = (const int32_t*)(b + L.md_module);
   v->anchor = (const float*)(b + L.md_anchor);
   v->ur_sina = (const float*)(b + L.md_aux);
-  v->dphi_dphichange = (const float*)(b + L.md_out);
+  v->dphi_dphichange = c->P.store_half ? nullptr : (const float*)(b + L.md_out);
+  v->dphi_dphichange_h = c->P.store_half ? (const uint16_t*)(b + L.md_out) : nullptr;
   v->module_start = (const int32_t*)(b + L.md_start);
   return LST_OK;
 }
@@ -470,7 +473,8 @@ int lst_get_segments(lst_ctx* c, int slot, lst_seg_view* v) {
   const char* b = c->arena + (size_t)slot * c->P.slot_stride;
   v->n = c->slots[slot].hdr->n[LST_SEG];
   v->md = (const int32_t*)(b + L.seg_md);
-  v->f = (const float*)(b + L.seg_f);
+  v->f = c->P.store_half ? nullptr : (const float*)(b + L.seg_f);
+  v->f_h = c->P.store_half ? (const uint16_t*)(b + L.seg_f) : nullptr;
   v->md_start = (const int32_t*)(b + L.seg_start);
   return LST_OK;
 }
@@ -483,7 +487,8 @@ int lst_get_triplets(lst_ctx* c, int slot, lst_t3_view* v) {
   v->n = c->slots[slot].hdr->n[LST_T3];
   v->md_kappa = (const int32_t*)(b + L.t3_pack);
   v->seg = (const int32_t*)(b + L.t3_seg);
-  v->chi2rz = (const float*)(b + L.t3_chi2);
+  v->chi2rz = c->P.store_half ? nullptr : (const float*)(b + L.t3_chi2);
+  v->chi2rz_h = c->P.store_half ? (const uint16_t*)(b + L.t3_chi2) : nullptr;
   v->seg_start = (const int32_t*)(b + L.t3_start);
   return LST_OK;
 }
@@ -496,7 +501,8 @@ int lst_get_quintuplets(lst_ctx* c, int slot, lst_t5_view* v) {
   v->n = c->slots[slot].hdr->n[LST_T5];
   v->md = (const int32_t*)(b + L.t5_md);
   v->t3 = (const int32_t*)(b + L.t5_t3);
-  v->f = (const float*)(b + L.t5_f);
+  v->f = c->P.store_half ? nullptr : (const float*)(b + L.t5_f);
+  v->f_h = c->P.store_half ? (const uint16_t*)(b + L.t5_f) : nullptr;
   v->t3_start = (const int32_t*)(b + L.t5_start);
   return LST_OK;
 }
@@ -582,7 +588,7 @@ int lst_sync_batch(lst_ctx* c, int first, int n, void* stream) {
 
 static inline int count_of(const SlotHeader* h, int kind) { return kind == LST_CLEAN ? h->n_kept : h->n[kind]; }
 
-int lst_fetch_batch(lst_ctx* c, int first, int n, int kind, int32_t* const* idx_out, float* const* val_out,
+int lst_fetch_batch(lst_ctx* c, int first, int n, int kind, int32_t* const* idx_out, void* const* val_out,
                     const int64_t* cap_objects, int32_t* counts, int wait, void* stream) {
   if (!c || n < 1 || !valid_slot(c, first) || !valid_slot(c, first + n - 1) || kind < LST_MD || kind > LST_CLEAN || !cap_objects)
     return LST_ERR_ARG;
@@ -611,7 +617,7 @@ int lst_fetch_batch(lst_ctx* c, int first, int n, int kind, int32_t* const* idx_
   // Pinned (mapped) host buffers are written by ONE kernel per 16 slots (k_fetch_direct); what is left (pageable
   // buffers) goes through the slot's scratch area and the copy engine, below.
   std::vector<int32_t*> idx_dma(idx_out ? idx_out : nullptr, idx_out ? idx_out + n : nullptr);
-  std::vector<float*> val_dma(val_out ? val_out : nullptr, val_out ? val_out + n : nullptr);
+  std::vector<void*> val_dma(val_out ? val_out : nullptr, val_out ? val_out + n : nullptr);
   for (int b0 = 0; b0 < n && n_max > 0; b0 += kMaxBatch) {
     const int nb = n - b0 < kMaxBatch ? n - b0 : kMaxBatch;
     OutTable T;
@@ -622,7 +628,7 @@ int lst_fetch_batch(lst_ctx* c, int first, int n, int kind, int32_t* const* idx_
       if (idx_out && idx_out[b0 + b])
         if (void* a = const_cast<void*>(mapped_alias(idx_out[b0 + b]))) { T.idx[b] = static_cast<int*>(a); idx_dma[b0 + b] = nullptr; any = true; }
       if (val_out && val_out[b0 + b])
-        if (void* a = const_cast<void*>(mapped_alias(val_out[b0 + b]))) { T.val[b] = static_cast<float*>(a); val_dma[b0 + b] = nullptr; any = true; }
+        if (void* a = const_cast<void*>(mapped_alias(val_out[b0 + b]))) { T.val[b] = a; val_dma[b0 + b] = nullptr; any = true; }
     }
     if (!any) continue;
     Params Pd = c->P;
@@ -651,17 +657,19 @@ int lst_fetch_batch(lst_ctx* c, int first, int n, int kind, int32_t* const* idx_
     }
   }
   if (val_out && n_max > 0) {
+    // LS and T5 payloads are stored in the output layout (in either precision): copied straight from the store
     const bool packed = kind == LST_MD || kind == LST_T3 || kind == LST_CLEAN;
     if (packed) {
       c->launches += launch_pack_values(P, kind, n_max, n, st);
       LST_CUDA(c, cudaGetLastError());
     }
     const size_t src_off = packed ? L.scratch : (kind == LST_SEG ? L.seg_f : L.t5_f);
+    const size_t elem = c->P.store_half ? 2 : 4;
     for (int b = 0; b < n; ++b) {
       const int nk = count_of(c->slots[first + b].hdr, kind);
       if (!val_out[b] || nk == 0) continue;
       const char* base = c->arena + (size_t)(first + b) * c->P.slot_stride;
-      LST_CUDA(c, cudaMemcpyAsync(val_out[b], base + src_off, sizeof(float) * (size_t)nk * kValuesPerObject[kind], cudaMemcpyDeviceToHost, st));
+      LST_CUDA(c, cudaMemcpyAsync(val_out[b], base + src_off, elem * (size_t)nk * kValuesPerObject[kind], cudaMemcpyDeviceToHost, st));
     }
   }
   if (wait) LST_CUDA(c, cudaStreamSynchronize(st));
@@ -680,14 +688,14 @@ int lst_fetch_hit_indices(lst_ctx* c, int slot, int kind, int32_t* out, int64_t 
   return lst_fetch_batch(c, slot, 1, kind, outs, nullptr, caps, nullptr, 1, stream);
 }
 
-int lst_fetch_values(lst_ctx* c, int slot, int kind, float* out, int64_t cap, void* stream) {
+int lst_fetch_values(lst_ctx* c, int slot, int kind, void* out, int64_t cap, void* stream) {
   if (kind < LST_MD || kind > LST_T5) return LST_ERR_ARG;
   const int r = view_ready(c, slot, kind);
   if (r != LST_OK) return r;
   const int n = c->slots[slot].hdr->n[kind];
   if (n == 0) return LST_OK;
   if (!out || cap < n) return LST_ERR_ARG;
-  float* outs[1] = {out};
+  void* outs[1] = {out};
   const int64_t caps[1] = {cap};
   return lst_fetch_batch(c, slot, 1, kind, nullptr, outs, caps, nullptr, 1, stream);
 }

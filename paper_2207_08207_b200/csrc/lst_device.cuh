@@ -17,18 +17,20 @@
 // are always read together, packed to 8 or 16 bytes so one vector load fetches the group
 // (PAPER.md:139-141 argues for SoA on V100; on sm_100a the unit that matters is the 16-B
 // vector / 32-B sector):
+// Fields marked [h] are pure outputs (no later selection reads them): with Params::store_half they are stored as IEEE
+// binary16 (round to nearest even of the fp32 value) in the first half of the same array (DESIGN.md section 1 [H]).
 //   MD     md_anchor  = (x, y, z, r) of anchor  float4   ordered by (module, key of anchor hit)
 //          md_aux     = (r_upper, sinA)         float2
 //          md_key     = key of the anchor hit   float    (the segment search window runs on it)
 //          md_hits    = (orig lower, orig upper)int2
-//          md_out     = (dphi, dphichange)      float2
+//          md_out     = (dphi, dphichange)      float2   [h]
 //          md_module                            int
 //   LS     seg_md     = (inner MD, outer MD)    int2
-//          seg_f      = (sinS, z0, dphi, dphichange) float4
+//          seg_f      = (sinS, z0, dphi, dphichange) float4   [h]
 //   T3     t3_pack    = (MD1, MD2, MD3, kappa)  int4 (kappa as bits)
 //          t3_seg     = (seg a, seg b)          int2
-//          t3_chi2                              float
-//   T5     t5_md[5], t5_t3 = (A, B) int2, t5_f[5] = kA, kB, kfit, chi2xy, chi2rz
+//          t3_chi2                              float    [h]
+//   T5     t5_md[5], t5_t3 = (A, B) int2, t5_f[5] = kA, kB, kfit, chi2xy, chi2rz [h], t5_score = chi2xy + chi2rz (fp32, read by [D])
 // CSR offsets: bin_start[2*n_modules+1], md_start[n_modules+1], seg_start[cap_md+1] (by inner
 // MD), t3_start[cap_seg+1] (by first segment), t5_start[cap_t3+1] (by inner triplet).
 // mod_info[m] = (first MD, end MD, smallest key, largest key of the module's lower hits).
@@ -99,6 +101,7 @@ struct Params {
   const float* map_dphi;         // [map_offsets[n_modules]] azimuth(source normal) - azimuth(target normal), in (-pi, pi]
   int first_slot;
   int dup_min_shared;            // [D] D4: quintuplets sharing at least this many original hits are duplicates
+  int store_half;                // [H] output floats that no selection reads are stored as binary16
 };
 
 // Typed access to one slot.
@@ -184,7 +187,7 @@ int launch_clean(const Params& P, int n_batch, cudaStream_t s, cudaEvent_t* ev);
 // (null = that table is not wanted there, or goes through the scratch area and the copy engine).
 struct OutTable {
   int* idx[kMaxBatch];
-  float* val[kMaxBatch];
+  void* val[kMaxBatch];          // fp32 values, or binary16 when Params::store_half
 };
 int launch_fetch_direct(const Params& P, const OutTable& T, int kind, int n_batch, cudaStream_t s);
 int launch_gather_hits(const Params& P, int kind, int n_max, int n_batch, cudaStream_t s);   // slots first_slot .. + n_batch - 1

@@ -27,6 +27,8 @@
 //
 // blockIdx.y = index of the event within the batch (lst_run_batch): all events of a batch go
 // through one launch per kernel.
+#include <cuda_fp16.h>
+
 #include <cstddef>
 
 #include "lst_device.cuh"
@@ -516,6 +518,12 @@ __device__ __forceinline__ int warp_ticket(unsigned* ticket) {
   return __shfl_sync(kFull, c, 0);
 }
 
+#ifndef LST_MD_BLOCKS
+#define LST_MD_BLOCKS 6          // resident blocks per SM the launch bounds ask for (A/B of round 2: profiles/r2_summary.md)
+#endif
+#ifndef LST_T5_BLOCKS
+#define LST_T5_BLOCKS 4
+#endif
 constexpr int kWarps = 8;        // warps per block of the MD / T3 / T5 kernels
 constexpr int kSegWarps = 4;     // of the segment kernel (more shared memory per warp)
 constexpr int kQueue = 64;       // queue slots per warp (a push adds <= 32, a drain starts at >= 32)
@@ -543,7 +551,9 @@ __device__ __forceinline__ void md_emit(const Params& P, const Slot& S, int pos,
   S.md_aux()[pos] = make_float2(up.w, sinA);
   S.md_key()[pos] = S.hit_key()[i];
   S.md_hits()[pos] = make_int2(S.hit_orig()[i], S.hit_orig()[u]);
-  S.md_out()[pos] = make_float2(atan2f(lo.x * up.y - lo.y * up.x, lo.x * up.x + lo.y * up.y), atan2f(cross, dot));
+  const float dphi = atan2f(lo.x * up.y - lo.y * up.x, lo.x * up.x + lo.y * up.y), dphichange = atan2f(cross, dot);
+  if (P.store_half) reinterpret_cast<__half2*>(S.md_out())[pos] = __floats2half2_rn(dphi, dphichange);   // [H]
+  else S.md_out()[pos] = make_float2(dphi, dphichange);
   S.md_module()[pos] = S.hit_module()[i];
 }
 
@@ -580,7 +590,7 @@ __device__ __forceinline__ int md_walk(const Params& P, const Slot& S, MdWarp& s
   return running;
 }
 
-__global__ void __launch_bounds__(kWarps * 32, 6) k_md(const __grid_constant__ Params P) {
+__global__ void __launch_bounds__(kWarps * 32, LST_MD_BLOCKS) k_md(const __grid_constant__ Params P) {
   __shared__ MdWarp shw[kWarps];
   __shared__ float s_w[6], s_rmaxU[6];
   Slot S(P, blockIdx.y);
@@ -724,7 +734,13 @@ __device__ __forceinline__ void seg_emit(const Params& P, const Slot& S, int pos
   const float dx = ao.x - ai.x, dy = ao.y - ai.y;
   const float cross = ai.x * dy - ai.y * dx, dot = ai.x * dx + ai.y * dy;   // as in seg_select
   S.seg_md()[pos] = make_int2(i, o);
-  S.seg_f()[pos] = make_float4(sinS, z0, atan2f(ai.x * ao.y - ai.y * ao.x, ai.x * ao.x + ai.y * ao.y), atan2f(cross, dot));
+  const float dphi = atan2f(ai.x * ao.y - ai.y * ao.x, ai.x * ao.x + ai.y * ao.y), dphichange = atan2f(cross, dot);
+  if (P.store_half) {   // [H]
+    const __half2 a = __floats2half2_rn(sinS, z0), b = __floats2half2_rn(dphi, dphichange);
+    reinterpret_cast<uint2*>(S.seg_f())[pos] = make_uint2(*reinterpret_cast<const unsigned*>(&a), *reinterpret_cast<const unsigned*>(&b));
+  } else {
+    S.seg_f()[pos] = make_float4(sinS, z0, dphi, dphichange);
+  }
 }
 
 template <bool DIRECT>
@@ -979,7 +995,8 @@ __device__ __forceinline__ void t3_emit(const Params& P, const Slot& S, int pos,
   const int2 ma = S.seg_md()[a];
   S.t3_pack()[pos] = make_int4(ma.x, ma.y, S.seg_md()[b].y, __float_as_int(kappa));
   S.t3_seg()[pos] = make_int2(a, b);
-  S.t3_chi2()[pos] = chi2;
+  if (P.store_half) reinterpret_cast<__half*>(S.t3_chi2())[pos] = __float2half_rn(chi2);   // [H]
+  else S.t3_chi2()[pos] = chi2;
 }
 
 template <bool DIRECT>
@@ -1117,8 +1134,15 @@ __device__ __forceinline__ void t5_emit(const Params& P, const Slot& S, int pos,
   int* md = S.t5_md() + 5 * (size_t)pos;
   md[0] = ta.x; md[1] = ta.y; md[2] = ta.z; md[3] = tb.y; md[4] = tb.z;
   S.t5_t3()[pos] = make_int2(A, B);
-  float* f = S.t5_f() + 5 * (size_t)pos;
-  f[0] = __int_as_float(ta.w); f[1] = __int_as_float(tb.w); f[2] = kfit; f[3] = chi2xy; f[4] = chi2rz;
+  S.t5_score()[pos] = chi2xy + chi2rz;   // [D] D1, one fp32 addition of the fp32 values whatever the store
+  if (P.store_half) {   // [H]
+    __half* f = reinterpret_cast<__half*>(S.t5_f()) + 5 * (size_t)pos;
+    f[0] = __float2half_rn(__int_as_float(ta.w)); f[1] = __float2half_rn(__int_as_float(tb.w)); f[2] = __float2half_rn(kfit);
+    f[3] = __float2half_rn(chi2xy); f[4] = __float2half_rn(chi2rz);
+  } else {
+    float* f = S.t5_f() + 5 * (size_t)pos;
+    f[0] = __int_as_float(ta.w); f[1] = __int_as_float(tb.w); f[2] = kfit; f[3] = chi2xy; f[4] = chi2rz;
+  }
 }
 
 template <bool DIRECT>
@@ -1180,7 +1204,7 @@ __device__ __forceinline__ int t5_walk(const Params& P, const Slot& S, T5Warp& s
   return running;
 }
 
-__global__ void __launch_bounds__(kWarps * 32, 4) k_t5(const __grid_constant__ Params P) {
+__global__ void __launch_bounds__(kWarps * 32, LST_T5_BLOCKS) k_t5(const __grid_constant__ Params P) {
   __shared__ T5Warp shw[kWarps];
   Slot S(P, blockIdx.y);
   SlotHeader* H = S.hdr();
@@ -1274,7 +1298,7 @@ __global__ void __launch_bounds__(kWarps * 32, 4) k_t5(const __grid_constant__ P
 // MDs: count, scan, fill), and every (quintuplet, partner) pair goes through the exact rule D2-D4.
 // The result does not depend on the order of the incidence lists: D4 is an "exists" over the partners.
 // ------------------------------------------------------------------------------------------
-// score, hit tuple in layer order; zero the incidence counters
+// hit tuple in layer order (the score was stored by the quintuplet kernel); zero the incidence counters
 __global__ void __launch_bounds__(256) k_clean_prepare(const __grid_constant__ Params P) {
   Slot S(P, blockIdx.y);
   const SlotHeader* H = S.hdr();
@@ -1286,8 +1310,6 @@ __global__ void __launch_bounds__(256) k_clean_prepare(const __grid_constant__ P
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < max(n5, nz); i += gridDim.x * blockDim.x) {
     if (i < nz) { cnt[i] = 0; cur[i] = 0; }
     if (i < n5) {
-      const float* f = S.t5_f() + 5 * (size_t)i;
-      S.t5_score()[i] = f[3] + f[4];                       // D1
       S.t5_keep()[i] = 1;
       const int* md = S.t5_md() + 5 * (size_t)i;
       int2* out = reinterpret_cast<int2*>(S.t5_hits()) + 5 * (size_t)i;
@@ -1505,26 +1527,44 @@ __global__ void __launch_bounds__(256) k_gather_hits(const __grid_constant__ Par
   }
 }
 
-// Float payload of the classes whose fields are spread over several arrays (MD, T3), in the layout of
-// lst_fetch_values, to the slot's scratch area.  (LS and T5 payloads are stored in that layout already.)
+// Float payload of object i of class `kind`, column c, in the order of lst_fetch_values, read from either store.
+// HALF: the binary16 payload (bits); otherwise the fp32 value.  Columns that the selections need in fp32 (sinA, r, kappa of a
+// triplet) are rounded on the way out in the binary16 case.
+template <bool HALF>
+__device__ __forceinline__ auto payload(const Slot& S, int kind, size_t i, int c) {
+  if constexpr (HALF) {
+    const __half* mo = reinterpret_cast<const __half*>(S.md_out());
+    if (kind == LST_MD_) return c == 0 ? __float2half_rn(S.md_aux()[i].y) : c == 3 ? __float2half_rn(S.md_anchor()[i].w) : mo[2 * i + (c - 1)];
+    if (kind == LST_SEG_) return reinterpret_cast<const __half*>(S.seg_f())[4 * i + c];
+    if (kind == LST_T3_) return c == 0 ? __float2half_rn(__int_as_float(S.t3_pack()[i].w)) : reinterpret_cast<const __half*>(S.t3_chi2())[i];
+    return reinterpret_cast<const __half*>(S.t5_f())[5 * i + c];
+  } else {
+    if (kind == LST_MD_) return c == 0 ? S.md_aux()[i].y : c == 3 ? S.md_anchor()[i].w : reinterpret_cast<const float*>(S.md_out())[2 * i + (c - 1)];
+    if (kind == LST_SEG_) return reinterpret_cast<const float*>(S.seg_f())[4 * i + c];
+    if (kind == LST_T3_) return c == 0 ? __int_as_float(S.t3_pack()[i].w) : S.t3_chi2()[i];
+    return S.t5_f()[5 * i + c];
+  }
+}
+// The whole payload table [n][w] of a slot to `out`, one element per thread and step (coalesced writes).
+template <bool HALF, class T>
+__device__ __forceinline__ void write_payload(const Slot& S, int kind, int n, T* out, size_t tid, size_t nth) {
+  const int src_kind = kind == LST_CLEAN_ ? LST_T5_ : kind;
+  const int w = src_kind == LST_T3_ ? 2 : src_kind == LST_T5_ ? 5 : 4;
+  const size_t m = (size_t)n * w;
+  for (size_t j = tid; j < m; j += nth) {
+    const size_t i = j / w;
+    const int c = (int)(j - i * w);
+    out[j] = payload<HALF>(S, src_kind, kind == LST_CLEAN_ ? (size_t)S.tc_list()[i] : i, c);
+  }
+}
+
+// Float payload of a class in the layout of lst_fetch_values to the slot's scratch area (pageable destination buffers).
 __global__ void __launch_bounds__(256) k_pack_values(const __grid_constant__ Params P, int kind) {
   Slot S(P, blockIdx.y);
   const int n = kind == LST_CLEAN_ ? S.hdr()->n_kept : S.hdr()->n[kind];
-  float* out = reinterpret_cast<float*>(S.scratch());
-  if (kind == LST_CLEAN_) {
-    for (size_t j = (size_t)blockIdx.x * blockDim.x + threadIdx.x; j < (size_t)n * 5; j += (size_t)gridDim.x * blockDim.x) {
-      const size_t i = j / 5;
-      out[j] = S.t5_f()[5 * (size_t)S.tc_list()[i] + (j - 5 * i)];
-    }
-  } else if (kind == LST_MD_) {
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-      const float2 o = S.md_out()[i];
-      reinterpret_cast<float4*>(out)[i] = make_float4(S.md_aux()[i].y, o.x, o.y, S.md_anchor()[i].w);
-    }
-  } else if (kind == LST_T3_) {
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
-      reinterpret_cast<float2*>(out)[i] = make_float2(__int_as_float(S.t3_pack()[i].w), S.t3_chi2()[i]);
-  }
+  const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (size_t)gridDim.x * blockDim.x;
+  if (P.store_half) write_payload<true>(S, kind, n, reinterpret_cast<__half*>(S.scratch()), tid, nth);
+  else write_payload<false>(S, kind, n, reinterpret_cast<float*>(S.scratch()), tid, nth);
 }
 
 // Both tables of every slot of a batch straight into pinned (mapped) host buffers: the kernel IS the device-to-host
@@ -1548,22 +1588,9 @@ __global__ void __launch_bounds__(256) k_fetch_direct(const __grid_constant__ Pa
       out[j] = mh[md];
     }
   }
-  if (float* out = T.val[blockIdx.y]) {
-    if (kind == LST_CLEAN_) {
-      for (size_t j = tid; j < (size_t)n * 5; j += nth) { const size_t i = j / 5; out[j] = S.t5_f()[5 * (size_t)S.tc_list()[i] + (j - 5 * i)]; }
-    } else if (kind == LST_MD_) {
-      for (size_t i = tid; i < (size_t)n; i += nth) {
-        const float2 o = S.md_out()[i];
-        reinterpret_cast<float4*>(out)[i] = make_float4(S.md_aux()[i].y, o.x, o.y, S.md_anchor()[i].w);
-      }
-    } else if (kind == LST_T3_) {
-      for (size_t i = tid; i < (size_t)n; i += nth)
-        reinterpret_cast<float2*>(out)[i] = make_float2(__int_as_float(S.t3_pack()[i].w), S.t3_chi2()[i]);
-    } else {   // LS [n][4] and T5 [n][5] are stored in the output layout: a flat copy
-      const float* src = kind == LST_SEG_ ? reinterpret_cast<const float*>(S.seg_f()) : S.t5_f();
-      const size_t m = (size_t)n * (kind == LST_SEG_ ? 4 : 5);
-      for (size_t i = tid; i < m; i += nth) out[i] = src[i];
-    }
+  if (void* out = T.val[blockIdx.y]) {
+    if (P.store_half) write_payload<true>(S, kind, n, reinterpret_cast<__half*>(out), tid, nth);
+    else write_payload<false>(S, kind, n, reinterpret_cast<float*>(out), tid, nth);
   }
 }
 
@@ -1617,7 +1644,7 @@ int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEv
   LST_EV(0);
   switch (stage) {
     case LST_MD_:
-      k_md<<<dim3(blocks_per_event((P.L.n_chunk[0] + kWarps - 1) / kWarps, n_batch, 6, kGridShare), nb), kWarps * 32, 0, s>>>(P);
+      k_md<<<dim3(blocks_per_event((P.L.n_chunk[0] + kWarps - 1) / kWarps, n_batch, LST_MD_BLOCKS, kGridShare), nb), kWarps * 32, 0, s>>>(P);
       break;
     case LST_SEG_:
       // (a module-owner walk with a flat on-chip key-window compare was built and measured in round 2: it lost, profiles/r2_seg_ab.md)
@@ -1627,7 +1654,7 @@ int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEv
       k_t3<<<dim3(blocks_per_event((P.L.n_chunk[2] + kWarps - 1) / kWarps, n_batch, 6, kGridShare), nb), kWarps * 32, 0, s>>>(P);
       break;
     case LST_T5_:
-      k_t5<<<dim3(blocks_per_event((P.L.n_chunk[3] + kWarps - 1) / kWarps, n_batch, 4, kGridShare), nb), kWarps * 32, 0, s>>>(P);
+      k_t5<<<dim3(blocks_per_event((P.L.n_chunk[3] + kWarps - 1) / kWarps, n_batch, LST_T5_BLOCKS, kGridShare), nb), kWarps * 32, 0, s>>>(P);
       break;
     default:
       return 0;
@@ -1665,7 +1692,7 @@ int launch_gather_hits(const Params& P, int kind, int n_max, int n_batch, cudaSt
 }
 
 int launch_pack_values(const Params& P, int kind, int n_max, int n_batch, cudaStream_t s) {
-  if (n_max <= 0 || n_batch <= 0 || (kind != LST_MD_ && kind != LST_T3_ && kind != LST_CLEAN_)) return 0;
+  if (n_max <= 0 || n_batch <= 0) return 0;
   k_pack_values<<<dim3(min(256, (n_max + 255) / 256), (unsigned)n_batch), 256, 0, s>>>(P, kind);
   return 1;
 }

@@ -54,7 +54,7 @@ class Config(C.Structure):
                 ("t5_kappa_max", C.c_float),
                 ("device", C.c_int32), ("n_slots", C.c_int32), ("cap_hits", C.c_int32), ("cap_md", C.c_int32),
                 ("cap_seg", C.c_int32), ("cap_t3", C.c_int32), ("cap_t5", C.c_int32), ("timing", C.c_int32),
-                ("t5_dup_min_shared", C.c_int32)]
+                ("store_half", C.c_int32), ("t5_dup_min_shared", C.c_int32)]
 
     CUT_FIELDS = ("half_kappa_max", "z_lum", "md_cos_eps", "md_sin_eps", "md_dz_res", "md_eps", "seg_cos_eps",
                   "seg_sin_eps", "seg_z0_max", "t3_kappa_max", "t3_chi2rz_max", "sigma_z2", "inv_sigma_z2",
@@ -75,20 +75,22 @@ class Hits(C.Structure):
 
 class MdView(C.Structure):
     _fields_ = [("n", C.c_int32), ("hits", C.c_void_p), ("module", C.c_void_p), ("anchor", C.c_void_p),
-                ("ur_sina", C.c_void_p), ("dphi_dphichange", C.c_void_p), ("module_start", C.c_void_p)]
+                ("ur_sina", C.c_void_p), ("dphi_dphichange", C.c_void_p), ("module_start", C.c_void_p),
+                ("dphi_dphichange_h", C.c_void_p)]
 
 
 class SegView(C.Structure):
-    _fields_ = [("n", C.c_int32), ("md", C.c_void_p), ("f", C.c_void_p), ("md_start", C.c_void_p)]
+    _fields_ = [("n", C.c_int32), ("md", C.c_void_p), ("f", C.c_void_p), ("md_start", C.c_void_p), ("f_h", C.c_void_p)]
 
 
 class T3View(C.Structure):
     _fields_ = [("n", C.c_int32), ("md_kappa", C.c_void_p), ("seg", C.c_void_p), ("chi2rz", C.c_void_p),
-                ("seg_start", C.c_void_p)]
+                ("seg_start", C.c_void_p), ("chi2rz_h", C.c_void_p)]
 
 
 class T5View(C.Structure):
-    _fields_ = [("n", C.c_int32), ("md", C.c_void_p), ("t3", C.c_void_p), ("f", C.c_void_p), ("t3_start", C.c_void_p)]
+    _fields_ = [("n", C.c_int32), ("md", C.c_void_p), ("t3", C.c_void_p), ("f", C.c_void_p), ("t3_start", C.c_void_p),
+                ("f_h", C.c_void_p)]
 
 
 class Stats(C.Structure):
@@ -187,7 +189,7 @@ class DeviceArray:
     def torch(self):
         import torch
         if 0 in self.shape:
-            return torch.empty(self.shape, dtype={"<i4": torch.int32, "<f4": torch.float32, "|u1": torch.uint8}[self.__cuda_array_interface__["typestr"]], device="cuda")
+            return torch.empty(self.shape, dtype={"<i4": torch.int32, "<f4": torch.float32, "<f2": torch.float16, "|u1": torch.uint8}[self.__cuda_array_interface__["typestr"]], device="cuda")
         return torch.as_tensor(self, device="cuda")
 
 
@@ -274,6 +276,7 @@ class Lst:
         self.h = h
         self.n_modules = len(layer)
         self.n_slots = int(self.cfg.n_slots)
+        self.store_half = bool(self.cfg.store_half)          # [H]: output floats are binary16 in views and fetches
         self._borrowed = {}
 
     @classmethod
@@ -372,20 +375,24 @@ class Lst:
                     evaluated=[int(v) for v in s.evaluated], overflow=int(s.overflow), bad_hits=int(s.bad_hits), stage_ms=[float(v) for v in s.stage_ms],
                     kernel_ms=[float(v) for v in s.kernel_ms], rewalks=[int(v) for v in s.rewalks], n_kept=int(s.n_kept))
 
+    def _payload(self, p32, p16, shape):
+        """The fp32 array of a view, or its binary16 twin when the context was created with store_half."""
+        return DeviceArray(p16, shape, "<f2", self) if self.store_half else DeviceArray(p32, shape, "<f4", self)
+
     def mds(self, slot: int) -> dict:
         v = MdView()
         self._check(self.lib.lst_get_mds(self.h, slot, C.byref(v)), "lst_get_mds")
         n = v.n
         return dict(n=n, hits=DeviceArray(v.hits, (n, 2), "<i4", self), module=DeviceArray(v.module, (n,), "<i4", self),
                     anchor=DeviceArray(v.anchor, (n, 4), "<f4", self), ur_sina=DeviceArray(v.ur_sina, (n, 2), "<f4", self),
-                    dphi_dphichange=DeviceArray(v.dphi_dphichange, (n, 2), "<f4", self),
+                    dphi_dphichange=self._payload(v.dphi_dphichange, v.dphi_dphichange_h, (n, 2)),
                     module_start=DeviceArray(v.module_start, (self.n_modules + 1,), "<i4", self))
 
     def segments(self, slot: int) -> dict:
         v = SegView()
         self._check(self.lib.lst_get_segments(self.h, slot, C.byref(v)), "lst_get_segments")
         n_md = self.stats(slot)["needed"][MD]
-        return dict(n=v.n, md=DeviceArray(v.md, (v.n, 2), "<i4", self), f=DeviceArray(v.f, (v.n, 4), "<f4", self),
+        return dict(n=v.n, md=DeviceArray(v.md, (v.n, 2), "<i4", self), f=self._payload(v.f, v.f_h, (v.n, 4)),
                     md_start=DeviceArray(v.md_start, (n_md + 1,), "<i4", self))
 
     def triplets(self, slot: int) -> dict:
@@ -393,14 +400,14 @@ class Lst:
         self._check(self.lib.lst_get_triplets(self.h, slot, C.byref(v)), "lst_get_triplets")
         n_seg = self.stats(slot)["needed"][SEG]
         return dict(n=v.n, md_kappa=DeviceArray(v.md_kappa, (v.n, 4), "<i4", self), seg=DeviceArray(v.seg, (v.n, 2), "<i4", self),
-                    chi2rz=DeviceArray(v.chi2rz, (v.n,), "<f4", self), seg_start=DeviceArray(v.seg_start, (n_seg + 1,), "<i4", self))
+                    chi2rz=self._payload(v.chi2rz, v.chi2rz_h, (v.n,)), seg_start=DeviceArray(v.seg_start, (n_seg + 1,), "<i4", self))
 
     def quintuplets(self, slot: int) -> dict:
         v = T5View()
         self._check(self.lib.lst_get_quintuplets(self.h, slot, C.byref(v)), "lst_get_quintuplets")
         n_t3 = self.stats(slot)["needed"][T3]
         return dict(n=v.n, md=DeviceArray(v.md, (v.n, 5), "<i4", self), t3=DeviceArray(v.t3, (v.n, 2), "<i4", self),
-                    f=DeviceArray(v.f, (v.n, 5), "<f4", self), t3_start=DeviceArray(v.t3_start, (n_t3 + 1,), "<i4", self))
+                    f=self._payload(v.f, v.f_h, (v.n, 5)), t3_start=DeviceArray(v.t3_start, (n_t3 + 1,), "<i4", self))
 
     def track_candidates(self, slot: int) -> dict:
         """After run_stage(..., CLEAN) and sync: the kept quintuplets (device arrays)."""
@@ -430,7 +437,7 @@ class Lst:
         n = self.stats(slot)["needed"][kind]
         w = VALUES_PER_OBJECT[kind]
         if out is None:
-            out = np.empty((n, w), np.float32)
+            out = np.empty((n, w), np.float16 if self.store_half else np.float32)
         self._check(self.lib.lst_fetch_values(self.h, slot, kind, _ptr(out), out.shape[0], _stream(stream)),
                     "lst_fetch_values")
         return out[:n]

@@ -65,3 +65,45 @@ def run_gpu(lst, ev, slot=0, stream=None):
     lst.run(slot, stream)
     lst.sync(slot, stream)
     return gpu_tables(lst, slot, stream)
+
+
+# ---- reduced-precision object store [H] (DESIGN.md section 1 [H]) -----------------------------------------------
+# columns of lst_fetch_values that come out of atan2f (libm and CUDA differ by an fp32 ulp or two, which can move
+# the binary16 rounding by one binary16 ulp); every other column is the RNE rounding of a bit-identical fp32 value
+ATAN_COLUMNS = {0: (1, 2), 1: (2, 3), 2: (), 3: ()}
+
+
+def half_steps(a_bits, b_bits):
+    """Distance in binary16 ulps between two arrays of bit patterns (sign-magnitude -> ordered integers)."""
+    def ordered(u):
+        u = u.astype(np.int32)
+        return np.where(u & 0x8000, -(u & 0x7fff), u & 0x7fff)
+    return np.abs(ordered(a_bits) - ordered(b_bits))
+
+
+def compare_half(gpu, ora, o32, label=""):
+    """Relaxed parity rule of the reduced-precision store: object sets IDENTICAL (nothing a selection reads is reduced);
+    every fetched value equals the oracle's fp32 value rounded to binary16 (round to nearest even) bit for bit, except the
+    atan2f outputs, which may differ by one binary16 ulp; and, against the unrounded fp32 oracle value, every value is
+    within 2^-11 relative + 2^-25 absolute (half an ulp of binary16, subnormal spacing included)."""
+    n_off = 0
+    for k in range(4):
+        gh, gv = sort_rows(*gpu[k])
+        oh, ov = sort_rows(*ora[k])
+        assert gv.dtype == np.float16, (label, k, gv.dtype)
+        assert gh.shape == oh.shape and np.array_equal(gh, oh), f"{label} class {k}: object sets differ"
+        if len(gh) == 0:
+            continue
+        want = o32.half_bits(ov.astype(np.float32))
+        got = np.ascontiguousarray(gv).view(np.uint16)
+        for c in range(gv.shape[1]):
+            d = half_steps(got[:, c], want[:, c])
+            if c in ATAN_COLUMNS[k]:
+                assert d.max() <= 1, f"{label} class {k} column {c}: {d.max()} binary16 ulps"
+                n_off += int((d > 0).sum())
+            else:
+                assert d.max() == 0, f"{label} class {k} column {c}: not the RNE rounding of the fp32 value ({int((d > 0).sum())} off)"
+            a, b = gv[:, c].astype(np.float64), ov[:, c].astype(np.float64)
+            tol = 2.0 ** -11 * np.abs(b) + 2.0 ** -25 + (2.0 ** -10 * np.abs(b) if c in ATAN_COLUMNS[k] else 0.0)
+            assert np.all(np.abs(a - b) <= tol), f"{label} class {k} column {c}: beyond half an ulp of binary16"
+    return n_off

@@ -706,3 +706,47 @@ def test_soak_mixed_sizes_repeatable(lstmod, geom, mmap, o32, run_oracle):
         assert list(ref[k]) == ora.counts
         parity.compare(parity.gpu_tables(c, k, streams[k // 4]), parity.oracle_tables(ora), f"soak slot {k}")
     c.close()
+
+
+@pytest.mark.parametrize("config,seed", [(0, 0), (1, 0), (3, 0)])
+def test_reduced_precision_store_parity(lstmod, geom, mmap, o32, run_oracle, config, seed):
+    """lst_config.store_half (DESIGN.md section 1 [H]): the output floats no selection reads are kept as
+    binary16.  Relaxed parity rule (parity.compare_half): identical object sets and candidate counts; every fetched value is
+    the round-to-nearest-even binary16 of the oracle's fp32 value (atan2f outputs: within one binary16 ulp); the duplicate
+    cleaning, which reads chi2xy + chi2rz, still equals the fp32 oracle's kept set because its score is kept in fp32."""
+    import torch
+    cfg = lstmod.default_config()
+    cfg.n_slots, cfg.store_half = 2, 1
+    c = lstmod.Lst.from_synth(geom, mmap, cfg)
+    st = torch.cuda.Stream()
+    ev = synth.generate_event(geom, config, seed)
+    gpu = parity.run_gpu(c, ev, slot=1, stream=st)
+    ora = run_oracle(o32, ev)
+    n_off = parity.compare_half(gpu, parity.oracle_tables(ora), o32, f"half C{config}")
+    stt = c.stats(1)
+    assert stt["needed"] == ora.counts and stt["candidates"] == ora.candidates
+    # views expose the binary16 arrays; they hold what the fetch returns
+    t5 = c.quintuplets(1)
+    assert t5["f"].torch().dtype == torch.float16
+    order = np.lexsort(gpu[3][0].T[::-1])
+    assert np.array_equal(t5["f"].torch().cpu().numpy()[order].view(np.uint16), parity.sort_rows(*gpu[3])[1].view(np.uint16))
+    seg = c.segments(1)
+    assert np.array_equal(seg["f"].torch().cpu().numpy().view(np.uint16), gpu[1][1].view(np.uint16))
+    # cleaning: same kept set as the fp32 oracle
+    if config != 3:
+        c.run_stage(1, 1, lstmod.CLEAN, st)
+        c.sync(1, st)
+        keep_o = o32.t5_clean(ora.t5_hits(), ora.t5_chi2xy, ora.t5_chi2rz, 7)
+        kept = c.fetch_kept(1, st)
+        as_set = lambda h: set(map(tuple, h.tolist()))
+        assert as_set(gpu[3][0][kept]) == as_set(ora.t5_hits()[keep_o])
+        # lst_fetch_batch of the kept quintuplets: binary16 rows of the same table, pinned and pageable buffers
+        for pinned in (True, False):
+            idx = np.zeros((len(kept) + 1, 10), np.int32)
+            val = np.zeros((len(kept) + 1, 5), np.float16)
+            if pinned:
+                idx, val = torch.from_numpy(idx).pin_memory().numpy(), torch.from_numpy(val).pin_memory().numpy()
+            assert c.fetch_batch(1, lstmod.CLEAN, [idx], [val], stream=st, wait=True) == [len(kept)]
+            assert np.array_equal(idx[:len(kept)], gpu[3][0][kept]) and np.array_equal(val[:len(kept)].view(np.uint16), gpu[3][1][kept].view(np.uint16))
+    print(f"half store C{config}: {stt['needed']} objects, {n_off} atan2f outputs one binary16 ulp off")
+    c.close()
