@@ -106,6 +106,12 @@ typedef struct {
   float t5_chi2xy_max;
   float t5_sigma_xy2_scaled;
   float t5_kappa_max;
+  /* [P] pixel line segments -> pixel triplets [0] / pixel quintuplets [1] (DESIGN.md section 1 [P]) */
+  float pix_dkappa_max[2];
+  float pix_inv_var_xy[LST_N_LAYERS];
+  float pix_inv_var_rz[LST_N_LAYERS];
+  float pix_chi2xy_max[2];
+  float pix_chi2rz_max[2];
   /* runtime */
   int32_t device;     /* CUDA device ordinal */
   int32_t n_slots;    /* event slots in the arena (>= 1) */

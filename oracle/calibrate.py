@@ -84,5 +84,41 @@ def main():
           f"frozen={d['t5_dkappa_max']/kappa_max:.5f}")
 
 
+def main_pixel():
+    """[P] pixel links (python -m oracle.calibrate pixel): with the frozen [M]..[Q] cuts and the [P] thresholds opened, the
+    maximum of |kappa_obj - kappa_seed|, chi2xy and chi2rz over the links whose outer object and seed come from the same
+    generated particle (pT >= 0.8 GeV); threshold = smallest multiple of 5 (chi2) / of 1e-4 cm^-1 (curvature) >= 1.5 x max."""
+    o = oracle.load("f32")
+    geom = synth.make_geometry()
+    mg = synth.map_geometry(geom)
+    mm = synth.ModuleMap(geom.n_modules, *o.build_map(mg["layer"], mg["phi"], mg["rho"], mg["gap"], mg["hw"], mg["zlo"], mg["zhi"]))
+    cfg = o.default_config()
+    for k in range(2):
+        cfg.pix_dkappa_max[k] = cfg.pix_chi2xy_max[k] = cfg.pix_chi2rz_max[k] = HUGE
+    mx = {name: np.zeros(2) for name in ("dkappa", "chi2xy", "chi2rz")}
+    n = np.zeros(2, int)
+    for seed in SEEDS:
+        ev = synth.generate_event(geom, 1, seed, n_particles=2000)       # the full product seeds x objects is the search space: a third of an event keeps this to a minute
+        sd = synth.generate_seeds(ev, seed)
+        r = o.run(geom.layer, mm.row_offsets, mm.targets, ev.x, ev.y, ev.z, ev.module, ev.side, cfg=cfg, seeds=sd.arrays())
+        pt = ev.particles["pt"]
+        for kind in (0, 1):
+            d = r.pix[kind]
+            tr = ev.truth[(r.t5_hits() if kind else r.t3_hits())[d["obj"]]]
+            same = (tr == tr[:, :1]).all(1) & (tr[:, 0] >= 0) & (tr[:, 0] == sd.truth[d["seed"]])
+            same[same] = pt[tr[same, 0]] >= 0.8
+            n[kind] += same.sum()
+            for name in mx:
+                mx[name][kind] = max(mx[name][kind], np.abs(d[name][same]).max())
+        print(f"seed {seed}: hits {ev.n} seeds {sd.n} counts {r.counts}", flush=True)
+    d = o.config_dict()
+    for kind, what in enumerate(("pixel triplets", "pixel quintuplets")):
+        print(f"{what}: n={n[kind]}")
+        print(f"  |dkappa| max={mx['dkappa'][kind]:.6f} x1.5={1.5 * mx['dkappa'][kind]:.6f} frozen={d['pix_dkappa_max'][kind]}")
+        print(f"  chi2xy   max={mx['chi2xy'][kind]:.3f} x1.5={1.5 * mx['chi2xy'][kind]:.3f} frozen={d['pix_chi2xy_max'][kind]}")
+        print(f"  chi2rz   max={mx['chi2rz'][kind]:.3f} x1.5={1.5 * mx['chi2rz'][kind]:.3f} frozen={d['pix_chi2rz_max'][kind]}")
+
+
 if __name__ == "__main__":
-    main()
+    import sys
+    main_pixel() if "pixel" in sys.argv[1:] else main()

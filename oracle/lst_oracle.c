@@ -80,6 +80,12 @@ typedef struct {
   real t5_chi2xy_max;
   real t5_sigma_xy2_scaled;     /* (sigma_rphi/32)^2                                          */
   real t5_kappa_max;            /* 1.05 * KAPPA_MAX                                           */
+  /* [P] pixel line segments -> pT3 / pT5; index [0] = pixel triplets, [1] = pixel quintuplets */
+  real pix_dkappa_max[2];       /* |kappa of the outer object - kappa of the seed|            */
+  real pix_inv_var_xy[N_LAYERS];/* 1 / (x-y variance of an anchor of layer l about the seed's circle) */
+  real pix_inv_var_rz[N_LAYERS];/* 1 / (z variance of an anchor of layer l about the seed's line)     */
+  real pix_chi2xy_max[2];
+  real pix_chi2rz_max[2];
 } lsto_config;
 
 void lsto_default_config(lsto_config* c) {
@@ -107,6 +113,13 @@ void lsto_default_config(lsto_config* c) {
   c->t5_chi2xy_max = C(35.0);
   c->t5_sigma_xy2_scaled = C(6.6015625e-09);
   c->t5_kappa_max = C(0.0149521492);
+  c->pix_dkappa_max[0] = C(0.0008); c->pix_dkappa_max[1] = C(0.0007);
+  c->pix_inv_var_xy[0] = C(809.479);   c->pix_inv_var_xy[1] = C(187.19363); c->pix_inv_var_xy[2] = C(51.984085);
+  c->pix_inv_var_xy[3] = C(16.645065); c->pix_inv_var_xy[4] = C(6.149085);  c->pix_inv_var_xy[5] = C(2.8425808);
+  c->pix_inv_var_rz[0] = C(229.09508);  c->pix_inv_var_rz[1] = C(136.11072); c->pix_inv_var_rz[2] = C(79.544624);
+  c->pix_inv_var_rz[3] = C(0.50524855); c->pix_inv_var_rz[4] = C(0.5020406); c->pix_inv_var_rz[5] = C(0.4982422);
+  c->pix_chi2xy_max[0] = C(85.0); c->pix_chi2xy_max[1] = C(145.0);
+  c->pix_chi2rz_max[0] = C(25.0); c->pix_chi2rz_max[1] = C(35.0);
 }
 
 int lsto_is_f64(void) { return LSTO_F64; }
@@ -349,6 +362,61 @@ int lsto_t5_cut(const lsto_config* c, int layer1, real kappaA, real kappaB,
 }
 
 /* ------------------------------------------------------------------------------------ */
+/* [P] pixel line segment + outer object -> pixel triplet / pixel quintuplet */
+/* ------------------------------------------------------------------------------------ */
+/* "Selections similar to that used for the Quintuplets are used here, the difference being that the straight lines
+ * and circles in the r-z and x-y plane, respectively, are not fit but rather the estimates from the pixel detector
+ * are used and the consistency of the outer hits to this hypothesis is checked".  Reading (DESIGN.md
+ * SPEC [P], reading 28): a pixel line segment is the inner tracker's estimate of a prompt helix,
+ *     seed = (kappa, cos phi0, sin phi0, z0, t):  signed curvature (sign as the triplet's kappa), direction of the
+ *     momentum at the beam line, z at the beam line, t = cot(theta) = dz / d(arc length);
+ * the outer object brings n = 3 (triplet) or 5 (quintuplet) anchors p_i on layers layer1 .. layer1 + n - 1 and its own
+ * curvature kappa_obj (circumcurvature of the triplet / fitted curvature of the quintuplet).
+ *   P1  |kappa_obj - kappa| <= pix_dkappa_max[kind]                  ("radii close to each other", with the seed's)
+ *   P2  x-y: the seed's circle goes through the beam line with that direction and curvature; a point p lies on it iff
+ *       e(p) = (kappa / 2) r^2 + x sin phi0 - y cos phi0 = 0, and e is the signed distance from the circle to first
+ *       order (its gradient has unit length on the circle).  chi2xy = sum_i e_i^2 / var_xy[layer_i] <= pix_chi2xy_max[kind]
+ *   P3  r-z: the seed's line is z = z0 + t s, s the arc length in the transverse plane at radius r,
+ *       s = (2 / kappa) asin(kappa r / 2), taken by its power series in u^2 = (kappa r / 2)^2 up to u^10 (no
+ *       transcendental function in a cut variable; remainder < 0.035 u^12 r for u <= 0.77, the largest value in this geometry).  d_i = (z_i - z0) - t s_i;
+ *       chi2rz = sum_i d_i^2 / var_rz[layer_i] <= pix_chi2rz_max[kind]
+ * kind: 0 = pixel triplet, 1 = pixel quintuplet.  p = [n][4] x, y, z, r.
+ * out[0] = chi2xy, out[1] = chi2rz, out[2] = kappa_obj - kappa; margin = {value, threshold} of P1, P2, P3. */
+int lsto_pix_cut(const lsto_config* c, int kind, int layer1, int n, const real* seed /* kappa, cphi, sphi, z0, t */,
+                 real kappa_obj, const real* p, real* out, real* margin) {
+  const real kappa = seed[0], cphi = seed[1], sphi = seed[2], z0 = seed[3], t = seed[4];
+  const real hk = C(0.5) * kappa;
+  real dk, chi2xy = C(0.0), chi2rz = C(0.0);
+  int i;
+  /* P1 */
+  dk = kappa_obj - kappa;
+  if (margin) { margin[0] = R_ABS(dk); margin[1] = c->pix_dkappa_max[kind]; }
+  if (!(R_ABS(dk) <= c->pix_dkappa_max[kind])) return 0;
+  /* P2 */
+  for (i = 0; i < n; ++i) {
+    const real x = p[4 * i + 0], y = p[4 * i + 1], r = p[4 * i + 3];
+    const real e = (hk * (r * r) + x * sphi) - y * cphi;
+    chi2xy = chi2xy + (e * e) * c->pix_inv_var_xy[layer1 + i];
+  }
+  if (margin) { margin[2] = chi2xy; margin[3] = c->pix_chi2xy_max[kind]; }
+  if (!(chi2xy <= c->pix_chi2xy_max[kind])) return 0;
+  /* P3 */
+  for (i = 0; i < n; ++i) {
+    const real z = p[4 * i + 2], r = p[4 * i + 3];
+    const real u = hk * r, u2 = u * u;
+    const real s = r * (C(1.0) + u2 * (C(0.16666667) + u2 * (C(0.075) + u2 * (C(0.04464286) + u2 * (C(0.030381944) + u2 * C(0.022372158))))));
+    const real d = (z - z0) - t * s;
+    chi2rz = chi2rz + (d * d) * c->pix_inv_var_rz[layer1 + i];
+  }
+  if (margin) { margin[4] = chi2rz; margin[5] = c->pix_chi2rz_max[kind]; }
+  if (!(chi2rz <= c->pix_chi2rz_max[kind])) return 0;
+  out[0] = chi2xy;
+  out[1] = chi2rz;
+  out[2] = dk;
+  return 1;
+}
+
+/* ------------------------------------------------------------------------------------ */
 /* Event-level driver                                                                      */
 /* ------------------------------------------------------------------------------------ */
 typedef struct {
@@ -370,6 +438,10 @@ typedef struct {
   real *t5_kfit, *t5_chi2xy, *t5_chi2rz;
   /* candidates examined per stage */
   int64_t cand[4];
+  /* [P] pixel links of kind 0 (pT3) / 1 (pT5): seed index, index of the outer object, chi2xy, chi2rz, kappa_obj - kappa */
+  int64_t n_pix[2], cap_pix[2], cand_pix[2];
+  int32_t *pix_seed[2], *pix_obj[2];
+  real *pix_chi2xy[2], *pix_chi2rz[2], *pix_dk[2];
 } lsto_event;
 
 static void* grow(void* p, int64_t n, size_t sz) { return realloc(p, (size_t)(n > 0 ? n : 1) * sz); }
@@ -406,6 +478,7 @@ void lsto_free(lsto_event* ev) {
   free(ev->seg_dphi); free(ev->seg_dphichange);
   free(ev->t3_a); free(ev->t3_b); free(ev->t3_kappa); free(ev->t3_chi2rz);
   free(ev->t5_a); free(ev->t5_b); free(ev->t5_kfit); free(ev->t5_chi2xy); free(ev->t5_chi2rz);
+  { int k; for (k = 0; k < 2; ++k) { free(ev->pix_seed[k]); free(ev->pix_obj[k]); free(ev->pix_chi2xy[k]); free(ev->pix_chi2rz[k]); free(ev->pix_dk[k]); } }
   free(ev);
 }
 
@@ -574,6 +647,64 @@ lsto_event* lsto_run(const lsto_config* cfg, int32_t n_modules, const int8_t* la
     free(byFirst); free(lst); free(cur);
   }
   return ev;
+}
+
+/* [P] event level: every (outer object, seed) pair is a candidate -- the search space is the full product, there is no
+ * map for seeds -- for the triplets whose innermost layer is 0 or 1 (kind 0) and for all quintuplets (kind 1).  Links come
+ * out ordered by (outer object, seed).  Adds to `ev` (built up to stage 3 resp. 4 by lsto_run); returns the number of links. */
+int64_t lsto_pixel_link(const lsto_config* cfg, lsto_event* ev, const int8_t* layer, int kind, int32_t n_seeds,
+                        const float* kappa, const float* cphi, const float* sphi, const float* z0, const float* t) {
+  const int n = kind ? 5 : 3;
+  const int64_t n_obj = kind ? ev->n_t5 : ev->n_t3;
+  int64_t o;
+  int32_t s;
+  ev->n_pix[kind] = 0;
+  ev->cand_pix[kind] = 0;
+  for (o = 0; o < n_obj; ++o) {
+    int32_t md[5];
+    real p[20], kobj;
+    int j, layer1;
+    if (kind) {
+      const int32_t A = ev->t5_a[o], B = ev->t5_b[o];
+      md[0] = ev->seg_in[ev->t3_a[A]]; md[1] = ev->seg_out[ev->t3_a[A]]; md[2] = ev->seg_out[ev->t3_b[A]];
+      md[3] = ev->seg_out[ev->t3_a[B]]; md[4] = ev->seg_out[ev->t3_b[B]];
+      kobj = ev->t5_kfit[o];
+    } else {
+      md[0] = ev->seg_in[ev->t3_a[o]]; md[1] = ev->seg_out[ev->t3_a[o]]; md[2] = ev->seg_out[ev->t3_b[o]];
+      kobj = ev->t3_kappa[o];
+    }
+    layer1 = layer[ev->md_module[md[0]]];
+    if (layer1 > 1) continue;
+    for (j = 0; j < n; ++j) {
+      p[4 * j + 0] = ev->md_x[md[j]]; p[4 * j + 1] = ev->md_y[md[j]];
+      p[4 * j + 2] = ev->md_z[md[j]]; p[4 * j + 3] = ev->md_r[md[j]];
+    }
+    for (s = 0; s < n_seeds; ++s) {
+      real seed[5], out[3];
+      seed[0] = kappa[s]; seed[1] = cphi[s]; seed[2] = sphi[s]; seed[3] = z0[s]; seed[4] = t[s];
+      ev->cand_pix[kind]++;
+      if (lsto_pix_cut(cfg, kind, layer1, n, seed, kobj, p, out, NULL)) {
+        if (ev->n_pix[kind] == ev->cap_pix[kind]) {
+          const int64_t c = ev->cap_pix[kind] ? 2 * ev->cap_pix[kind] : 1024;
+          ev->pix_seed[kind] = grow(ev->pix_seed[kind], c, 4); ev->pix_obj[kind] = grow(ev->pix_obj[kind], c, 4);
+          ev->pix_chi2xy[kind] = grow(ev->pix_chi2xy[kind], c, sizeof(real)); ev->pix_chi2rz[kind] = grow(ev->pix_chi2rz[kind], c, sizeof(real));
+          ev->pix_dk[kind] = grow(ev->pix_dk[kind], c, sizeof(real));
+          ev->cap_pix[kind] = c;
+        }
+        ev->pix_seed[kind][ev->n_pix[kind]] = s; ev->pix_obj[kind][ev->n_pix[kind]] = (int32_t)o;
+        ev->pix_chi2xy[kind][ev->n_pix[kind]] = out[0]; ev->pix_chi2rz[kind][ev->n_pix[kind]] = out[1];
+        ev->pix_dk[kind][ev->n_pix[kind]] = out[2];
+        ev->n_pix[kind]++;
+      }
+    }
+  }
+  return ev->n_pix[kind];
+}
+int64_t lsto_pix_count(const lsto_event* ev, int kind) { return ev->n_pix[kind]; }
+int64_t lsto_pix_candidates(const lsto_event* ev, int kind) { return ev->cand_pix[kind]; }
+const int32_t* lsto_pix_i32(const lsto_event* ev, int kind, int field) { return field ? ev->pix_obj[kind] : ev->pix_seed[kind]; }
+const real* lsto_pix_real(const lsto_event* ev, int kind, int field) {
+  return field == 0 ? ev->pix_chi2xy[kind] : field == 1 ? ev->pix_chi2rz[kind] : ev->pix_dk[kind];
 }
 
 /* ------------------------------------------------------------------------------------ */

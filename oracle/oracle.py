@@ -31,6 +31,7 @@ _CONFIG_FIELDS = [
     ("md_eps", 6), ("seg_cos_eps", 1), ("seg_sin_eps", 1), ("seg_z0_max", 5), ("t3_kappa_max", 1),
     ("t3_chi2rz_max", 4), ("sigma_z2", 6), ("inv_sigma_z2", 6), ("t5_dkappa_max", 1),
     ("t5_chi2rz_max", 2), ("t5_chi2xy_max", 1), ("t5_sigma_xy2_scaled", 1), ("t5_kappa_max", 1),
+    ("pix_dkappa_max", 2), ("pix_inv_var_xy", 6), ("pix_inv_var_rz", 6), ("pix_chi2xy_max", 2), ("pix_chi2rz_max", 2),
 ]
 
 
@@ -92,6 +93,15 @@ class OracleLib:
         lib.lsto_t5_clean.restype = C.c_int64
         lib.lsto_half_bits_array.argtypes = [C.c_int64, C.c_void_p, C.c_void_p]
         lib.lsto_half_bits_array.restype = None
+        lib.lsto_pix_cut.argtypes = [P(self.Config), C.c_int, C.c_int, C.c_int, P(r), r, P(r), P(r), P(r)]
+        lib.lsto_pix_cut.restype = C.c_int
+        lib.lsto_pixel_link.argtypes = [P(self.Config), C.c_void_p, C.c_void_p, C.c_int, C.c_int32] + [C.c_void_p] * 5
+        lib.lsto_pixel_link.restype = C.c_int64
+        lib.lsto_pix_count.argtypes = lib.lsto_pix_candidates.argtypes = [C.c_void_p, C.c_int]
+        lib.lsto_pix_count.restype = lib.lsto_pix_candidates.restype = C.c_int64
+        lib.lsto_pix_i32.argtypes = lib.lsto_pix_real.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        lib.lsto_pix_i32.restype = P(C.c_int32)
+        lib.lsto_pix_real.restype = P(self.real)
 
     # ---- configuration -------------------------------------------------------------------
     def default_config(self):
@@ -138,6 +148,16 @@ class OracleLib:
                                   self._arr(flat), out, mar)
         return bool(ok), dict(zip(("kfit", "chi2xy", "chi2rz"), list(out))), list(mar)
 
+    def pix_cut(self, kind, layer1, seed, kappa_obj, pts, cfg=None):
+        """[P] seed = (kappa, cos phi0, sin phi0, z0, t); pts = 3 (kind 0) or 5 (kind 1) anchors (x, y, z, r).
+        Returns (passed, dict(chi2xy, chi2rz, dkappa), margins[6])."""
+        cfg = cfg or self.default_config()
+        out, mar = self._arr([np.nan] * 3), self._arr([np.nan] * 6)
+        flat = [v for p in pts for v in p]
+        ok = self.lib.lsto_pix_cut(C.byref(cfg), int(kind), int(layer1), len(pts), self._arr(seed), self.real(float(kappa_obj)),
+                                   self._arr(flat), out, mar)
+        return bool(ok), dict(zip(("chi2xy", "chi2rz", "dkappa"), list(out))), list(mar)
+
     def t5_clean(self, hits, chi2xy, chi2rz, min_shared: int = 7) -> np.ndarray:
         """[D] duplicate cleaning: hits [n][10] original hit indices -> keep [n] bool (all-pairs definition)."""
         hits = np.ascontiguousarray(hits, np.int32).reshape(-1, 10)
@@ -174,7 +194,7 @@ class OracleLib:
         return offs, tg[:total]
 
     # ---- whole event -----------------------------------------------------------------------
-    def run(self, layer, row_offsets, targets, x, y, z, module, side, mode=0, stages=4, cfg=None) -> "OracleResult":
+    def run(self, layer, row_offsets, targets, x, y, z, module, side, mode=0, stages=4, cfg=None, seeds=None) -> "OracleResult":
         cfg = cfg or self.default_config()
         layer = np.ascontiguousarray(layer, np.int8)
         row_offsets = np.ascontiguousarray(row_offsets, np.int32)
@@ -190,7 +210,12 @@ class OracleLib:
         if not h:
             raise ValueError("oracle: invalid input (module id / side / module map)")
         try:
-            return OracleResult(self, h)
+            if seeds is not None:         # [P]: seeds = (kappa, cphi, sphi, z0, t) fp32 arrays -> pixel triplets and quintuplets
+                sd = [np.ascontiguousarray(a, np.float32) for a in seeds]
+                for kind in (0, 1):
+                    if stages >= 3 + kind:
+                        self.lib.lsto_pixel_link(C.byref(cfg), h, ptr(layer), kind, len(sd[0]), *[ptr(a) for a in sd])
+            return OracleResult(self, h, pixel=seeds is not None, stages=stages)
         finally:
             self.lib.lsto_free(h)
 
@@ -205,8 +230,18 @@ _REAL = dict(md_x=(0, 0), md_y=(1, 0), md_z=(2, 0), md_r=(3, 0), md_ur=(4, 0), m
 class OracleResult:
     """numpy copies of every output array, plus hit-index tuples per object class."""
 
-    def __init__(self, o: OracleLib, h):
+    def __init__(self, o: OracleLib, h, pixel=False, stages=4):
         lib = o.lib
+        self.pix = {}
+        if pixel:
+            for kind in (0, 1):
+                if stages < 3 + kind:
+                    continue
+                n = int(lib.lsto_pix_count(h, kind))
+                get_i = lambda f: np.ctypeslib.as_array(lib.lsto_pix_i32(h, kind, f), (n,)).copy() if n else np.zeros(0, np.int32)
+                get_r = lambda f: np.ctypeslib.as_array(lib.lsto_pix_real(h, kind, f), (n,)).copy() if n else np.zeros(0, o.np_real)
+                self.pix[kind] = dict(n=n, candidates=int(lib.lsto_pix_candidates(h, kind)), seed=get_i(0), obj=get_i(1),
+                                      chi2xy=get_r(0), chi2rz=get_r(1), dkappa=get_r(2))
         self.counts = [int(lib.lsto_count(h, k)) for k in range(4)]
         self.candidates = [int(lib.lsto_candidates(h, k)) for k in range(4)]
         for name, (f, kind) in _I32.items():
@@ -242,6 +277,12 @@ class OracleResult:
 
     def t5_hits(self):
         return self._hits(self.t5_mds())
+
+    def pix_tuples(self, kind):
+        """[P] identity of a pixel link: (seed index, the 6 / 10 original hit indices of its outer object)."""
+        hits = self.t5_hits() if kind else self.t3_hits()
+        d = self.pix[kind]
+        return np.concatenate([d["seed"].reshape(-1, 1), hits[d["obj"]].reshape(len(d["obj"]), 10 if kind else 6)], 1)
 
 
 def load(precision: str = "f32") -> OracleLib:

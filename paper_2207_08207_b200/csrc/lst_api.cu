@@ -184,6 +184,12 @@ int lst_default_config(lst_config* c) {
   c->t5_chi2xy_max = 35.0f;
   c->t5_sigma_xy2_scaled = 6.6015625e-09f;
   c->t5_kappa_max = 0.0149521492f;
+  c->pix_dkappa_max[0] = 0.0008f; c->pix_dkappa_max[1] = 0.0007f;
+  const float pvx[6] = {809.479f, 187.19363f, 51.984085f, 16.645065f, 6.149085f, 2.8425808f};
+  const float pvz[6] = {229.09508f, 136.11072f, 79.544624f, 0.50524855f, 0.5020406f, 0.4982422f};
+  for (int l = 0; l < LST_N_LAYERS; ++l) { c->pix_inv_var_xy[l] = pvx[l]; c->pix_inv_var_rz[l] = pvz[l]; }
+  c->pix_chi2xy_max[0] = 85.0f; c->pix_chi2xy_max[1] = 145.0f;
+  c->pix_chi2rz_max[0] = 25.0f; c->pix_chi2rz_max[1] = 35.0f;
   c->device = 0;
   c->n_slots = 4;
   c->cap_hits = 192 * 1024;

@@ -52,13 +52,16 @@ class Config(C.Structure):
                 ("sigma_z2", C.c_float * 6), ("inv_sigma_z2", C.c_float * 6), ("t5_dkappa_max", C.c_float),
                 ("t5_chi2rz_max", C.c_float * 2), ("t5_chi2xy_max", C.c_float), ("t5_sigma_xy2_scaled", C.c_float),
                 ("t5_kappa_max", C.c_float),
+                ("pix_dkappa_max", C.c_float * 2), ("pix_inv_var_xy", C.c_float * 6), ("pix_inv_var_rz", C.c_float * 6),
+                ("pix_chi2xy_max", C.c_float * 2), ("pix_chi2rz_max", C.c_float * 2),
                 ("device", C.c_int32), ("n_slots", C.c_int32), ("cap_hits", C.c_int32), ("cap_md", C.c_int32),
                 ("cap_seg", C.c_int32), ("cap_t3", C.c_int32), ("cap_t5", C.c_int32), ("timing", C.c_int32),
                 ("store_half", C.c_int32), ("t5_dup_min_shared", C.c_int32)]
 
     CUT_FIELDS = ("half_kappa_max", "z_lum", "md_cos_eps", "md_sin_eps", "md_dz_res", "md_eps", "seg_cos_eps",
                   "seg_sin_eps", "seg_z0_max", "t3_kappa_max", "t3_chi2rz_max", "sigma_z2", "inv_sigma_z2",
-                  "t5_dkappa_max", "t5_chi2rz_max", "t5_chi2xy_max", "t5_sigma_xy2_scaled", "t5_kappa_max")
+                  "t5_dkappa_max", "t5_chi2rz_max", "t5_chi2xy_max", "t5_sigma_xy2_scaled", "t5_kappa_max",
+                  "pix_dkappa_max", "pix_inv_var_xy", "pix_inv_var_rz", "pix_chi2xy_max", "pix_chi2rz_max")
 
     def cuts_dict(self) -> dict:
         out = {}

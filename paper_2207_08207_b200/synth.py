@@ -335,3 +335,71 @@ def transform_event(ev: Event, rot: float = 0.0, mirror_z: bool = False) -> Even
     y = (ev.x.astype(np.float64) * s + ev.y.astype(np.float64) * c).astype(np.float32)
     z = -ev.z if mirror_z else ev.z.copy()
     return Event(x, y, z, ev.module.copy(), ev.side.copy(), ev.truth.copy(), ev.particles)
+
+
+# ----------------------------------------------------------------------------------------
+# Pixel line segments: inner-tracker seeds.  The CMS seeds are not available; this is a stand-in seed
+# model: every generated particle above the seeding threshold gives, with some efficiency, the
+# inner tracker's ESTIMATE of its helix -- the true parameters smeared with fixed resolutions -- plus fake seeds with
+# random parameters.  Input data only: the consistency selection [P] is in the oracle and in the CUDA library.
+# ----------------------------------------------------------------------------------------
+SEED_PT_MIN = 0.8
+SEED_EFFICIENCY = 0.9
+SEED_FAKE_FRACTION = 0.2
+SEED_SIGMA_KAPPA_REL = 0.01          # relative curvature (pT) resolution ...
+SEED_SIGMA_KAPPA_ABS = 2.0e-5        # ... and its floor, cm^-1
+SEED_SIGMA_PHI = 5.0e-4              # rad
+SEED_SIGMA_Z0 = 0.01                 # cm
+SEED_SIGMA_T = 1.0e-3                # cot(theta)
+
+
+@dataclasses.dataclass
+class Seeds:
+    """Pixel line segments as the library receives them (fp32 SoA) + generator truth."""
+    kappa: np.ndarray        # signed curvature, cm^-1; sign convention of the triplet curvature: -q / R
+    cphi: np.ndarray         # cos / sin of the azimuth of the momentum at the beam line
+    sphi: np.ndarray
+    z0: np.ndarray           # z at the beam line, cm
+    t: np.ndarray            # cot(theta) = sinh(eta) = dz / d(transverse arc length)
+    truth: np.ndarray        # int32 particle index, -1 = fake seed
+
+    @property
+    def n(self) -> int:
+        return int(self.kappa.shape[0])
+
+    def arrays(self):
+        return self.kappa, self.cphi, self.sphi, self.z0, self.t
+
+
+def generate_seeds(ev: Event, seed: int = 0, *, efficiency=SEED_EFFICIENCY, fake_fraction=SEED_FAKE_FRACTION, smear: bool = True,
+                   shuffle: bool = True) -> Seeds:
+    """Draw order (fixed; generator PCG64(seed + 7919)): kept mask [P]; smearing of kappa, phi0, z0, t [n_true each];
+    fake kappa, phi0, z0, eta [n_fake each]; final permutation."""
+    rng = np.random.Generator(np.random.PCG64(seed + 7919))
+    par = ev.particles
+    P = len(par["pt"])
+    keep = (par["pt"] >= SEED_PT_MIN) & (rng.uniform(0.0, 1.0, P) < efficiency)
+    idx = np.nonzero(keep)[0]
+    n = len(idx)
+    R = par["pt"][idx] / (K_GEV_PER_T_CM * B_TESLA)
+    kappa = -par["q"][idx] / R
+    phi0, z0, t = par["phi0"][idx].copy(), par["z0"][idx].copy(), np.sinh(par["eta"][idx])
+    g = rng.normal(0.0, 1.0, (4, n))
+    if smear:
+        kappa = kappa + g[0] * np.hypot(SEED_SIGMA_KAPPA_REL * kappa, SEED_SIGMA_KAPPA_ABS)
+        phi0 = phi0 + g[1] * SEED_SIGMA_PHI
+        z0 = z0 + g[2] * SEED_SIGMA_Z0
+        t = t + g[3] * SEED_SIGMA_T
+    n_fake = int(math.floor(fake_fraction * n))
+    kmax = K_GEV_PER_T_CM * B_TESLA / SEED_PT_MIN
+    fk = rng.uniform(-kmax, kmax, n_fake)
+    fp = rng.uniform(-np.pi, np.pi, n_fake)
+    fz = rng.normal(0.0, 5.0, n_fake)
+    ft = np.sinh(rng.uniform(-1.2, 1.2, n_fake))
+    kappa, phi0, z0, t = (np.concatenate(a) for a in ((kappa, fk), (phi0, fp), (z0, fz), (t, ft)))
+    truth = np.concatenate([idx.astype(np.int32), np.full(n_fake, -1, np.int32)])
+    if shuffle:
+        perm = rng.permutation(len(kappa))
+        kappa, phi0, z0, t, truth = (a[perm] for a in (kappa, phi0, z0, t, truth))
+    f = lambda a: np.ascontiguousarray(a, np.float32)
+    return Seeds(f(kappa), f(np.cos(phi0)), f(np.sin(phi0)), f(z0), f(t), truth.astype(np.int32))
