@@ -372,6 +372,9 @@ int lsto_t5_cut(const lsto_config* c, int layer1, real kappaA, real kappaB,
  *     momentum at the beam line, z at the beam line, t = cot(theta) = dz / d(arc length);
  * the outer object brings n = 3 (triplet) or 5 (quintuplet) anchors p_i on layers layer1 .. layer1 + n - 1 and its own
  * curvature kappa_obj (circumcurvature of the triplet / fitted curvature of the quintuplet).
+ *   P0  the first anchor lies ahead of the seed: x_1 cos phi0 + y_1 sin phi0 > 0 (a circle through the beam line passes
+ *       every radius twice, going out and coming back; e(p) below vanishes on both arcs, the outer tracker's hits of a
+ *       prompt particle sit on the outgoing one)
  *   P1  |kappa_obj - kappa| <= pix_dkappa_max[kind]                  ("radii close to each other", with the seed's)
  *   P2  x-y: the seed's circle goes through the beam line with that direction and curvature; a point p lies on it iff
  *       e(p) = (kappa / 2) r^2 + x sin phi0 - y cos phi0 = 0, and e is the signed distance from the circle to first
@@ -388,6 +391,8 @@ int lsto_pix_cut(const lsto_config* c, int kind, int layer1, int n, const real* 
   const real hk = C(0.5) * kappa;
   real dk, chi2xy = C(0.0), chi2rz = C(0.0);
   int i;
+  /* P0 */
+  if (!(p[0] * cphi + p[1] * sphi > C(0.0))) return 0;
   /* P1 */
   dk = kappa_obj - kappa;
   if (margin) { margin[0] = R_ABS(dk); margin[1] = c->pix_dkappa_max[kind]; }

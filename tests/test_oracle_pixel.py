@@ -109,6 +109,29 @@ def test_p23_distance_from_the_circle_and_arc_length(o64):
         assert lo * (1 - 1e-9) <= out["chi2rz"] <= hi * (1 + 1e-9)
 
 
+def test_p22b_the_returning_arc_is_excluded(geom, o64):
+    """P0: a seed pointing the opposite way describes the same straight line (for a circle: its returning arc), so the x-y
+    residuals of a stiff track vanish for it too; the forward requirement on the first anchor rejects it."""
+    rng = np.random.default_rng(27)
+    cfg = open_cfg(o64)
+    n = 0
+    for _ in range(20):
+        h, mds = clean_helix(geom, rng, pt_lo=200.0, pt_hi=1000.0, eta_max=0.05)
+        t = [md_tuple(o64, l, mds[l])[0] for l in range(6)]
+        seed = helix_seed(h)
+        back = [seed[0], -seed[1], -seed[2], seed[3], seed[4]]
+        pts = [t[k][:4] for k in range(5)]
+        ok, out, mar = o64.pix_cut(1, 0, seed, seed[0], pts, cfg=cfg)
+        assert ok and out["chi2xy"] < 1e-12
+        cfg2 = open_cfg(o64)
+        ok_back, _, _ = o64.pix_cut(1, 0, back, seed[0], pts, cfg=cfg2)
+        assert not ok_back
+        e_back = [(back[0] / 2) * p[3] ** 2 + p[0] * back[2] - p[1] * back[1] for p in pts]
+        assert max(abs(e) for e in e_back) < 0.6            # the residuals alone would not have rejected it (stiff track: 2 kappa r^2 / 2)
+        n += 1
+    assert n == 20
+
+
 @pytest.fixture(scope="module")
 def small(geom, o32, run_oracle):
     ev = synth.generate_event(geom, 1, 5, n_particles=1200)
