@@ -57,7 +57,9 @@ enum {
 };
 
 enum { LST_MD = 0, LST_SEG = 1, LST_T3 = 2, LST_T5 = 3,
-       LST_CLEAN = 4 /* optional stage after LST_T5: duplicate cleaning of the quintuplets (lst_run_stage only) */ };
+       LST_CLEAN = 4, /* optional stage after LST_T5: duplicate cleaning of the quintuplets (lst_run_stage only) */
+       LST_PIXEL = 5  /* optional stage after LST_T5 (with or without LST_CLEAN): pixel line segments -> pixel triplets and
+                         pixel quintuplets (lst_load_seeds first; lst_run_stage only) */ };
 
 typedef struct lst_ctx lst_ctx;
 
@@ -132,6 +134,9 @@ typedef struct {
                          are duplicates (7).  Accepted range 6 .. 10 (lst_create returns LST_ERR_ARG otherwise): the
                          stage finds partners through a common mini-doublet, which >= 6 common hits imply and
                          <= 5 do not */
+  int32_t cap_seeds;  /* [P] per-slot capacities: pixel line segments (16 k), pixel triplets (64 k), pixel quintuplets (64 k) */
+  int32_t cap_pt3;
+  int32_t cap_pt5;
 } lst_config;
 
 /* Fills *cfg with the frozen SPEC constants, device 0, 4 slots and capacities that hold the
@@ -155,6 +160,23 @@ typedef struct {
   const uint8_t* side;
   int32_t on_device;
 } lst_hits;
+
+/* Pixel line segments of one event ("pixel-based seeds ... line segments"; DESIGN.md section 1 [P]): the inner
+ * tracker's estimate of a prompt helix per seed, fp32 SoA.  kappa: signed curvature in 1/cm with the sign convention of the
+ * triplet curvature (lst_t3_view.md_kappa); (cphi, sphi): direction of the momentum at the beam line (a unit vector; seeds
+ * whose direction is not one are still evaluated exactly, only slower); z0: z at the beam line, cm; t: cot(theta) = dz per
+ * unit of transverse arc length.  All five HOST pointers (on_device = 0; pinned arrays are read by the kernel over PCIe,
+ * pageable ones copied first) or all five DEVICE pointers (on_device = 1); borrowed until the stream has passed the work
+ * enqueued by lst_load_seeds. */
+typedef struct {
+  int32_t n;
+  const float* kappa;
+  const float* cphi;
+  const float* sphi;
+  const float* z0;
+  const float* t;
+  int32_t on_device;
+} lst_seeds;
 
 /* Views: DEVICE pointers into the slot's object store + the object count. */
 typedef struct {
@@ -204,6 +226,17 @@ typedef struct {
   const float* score;   /* [n_t5] chi2xy + chi2rz, the fp32 sum of the fp32 values (also when store_half)  */
 } lst_tc_view;
 
+/* Result of the optional stage LST_PIXEL for kind 0 (pixel triplets: seed + triplet whose first MD is on layer 0 or 1) or
+ * kind 1 (pixel quintuplets: seed + quintuplet): every (outer object, seed) pair that passes rule P0-P3, ordered by
+ * (outer object, seed index).  Always fp32 (also with lst_config.store_half). */
+typedef struct {
+  int32_t n;
+  const int32_t* link;         /* [n][2] seed index (position in the caller's seed arrays), index of the outer object
+                                  (into lst_t3_view for kind 0, lst_t5_view for kind 1)                              */
+  const float* f;              /* [n][3] chi2xy, chi2rz, kappa_object - kappa_seed                                   */
+  const int32_t* object_start; /* [n_objects + 1] links of outer object o are [start[o], start[o+1])                 */
+} lst_pix_view;
+
 typedef struct {
   int32_t n_hits;
   int64_t needed[4];     /* objects that passed per class (may exceed the capacity on overflow) */
@@ -221,6 +254,14 @@ typedef struct {
                             scan, fill, mark + list); [11] unused */
   int64_t rewalks[4];    /* chunks of 32 owners whose objects exceeded the on-chip stash and were walked twice */
   int32_t n_kept;        /* quintuplets kept by LST_CLEAN (0 if the stage was not run)                         */
+  /* [P], index 0 = pixel triplets, 1 = pixel quintuplets (zeros unless LST_PIXEL was run) */
+  int32_t n_seeds;       /* seeds loaded by lst_load_seeds                                                      */
+  int64_t pix_needed[2];     /* links that passed (may exceed the capacity: overflow bits 4, 5)                 */
+  int64_t pix_candidates[2]; /* the method's search space: (outer objects starting on layer 0 or 1) x seeds     */
+  int64_t pix_evaluated[2];  /* pairs inside the azimuth window of the object's first anchor, all of which went
+                                through the selection                                                           */
+  int64_t pix_rewalks[2];
+  float pix_ms[3];       /* seed binning kernel, pixel-triplet kernel, pixel-quintuplet kernel (lst_config.timing) */
 } lst_stats;
 
 /* Validates geometry and map, uploads the per-module tables, allocates the arena (the library allocates
@@ -239,6 +280,12 @@ LST_API int lst_destroy(lst_ctx* ctx);
 LST_API int lst_load_event(lst_ctx* ctx, int slot, const lst_hits* hits, void* cuda_stream);
 LST_API int lst_load_events(lst_ctx* ctx, int first_slot, int n_slots, const lst_hits* hits, void* cuda_stream);
 
+/* [P] Loads the pixel line segments of slots first_slot .. first_slot+n_slots-1 (seeds[b] into slot first_slot + b) and
+ * orders them for the search (one kernel per 16 events).  Call it AFTER lst_load_event(s) of the same slots, on the same
+ * stream (loading hits resets the slot, its seeds included).  Asynchronous.
+ * Errors: LST_ERR_ARG, LST_ERR_STATE (slot not loaded), LST_ERR_OVERFLOW (n > cap_seeds). */
+LST_API int lst_load_seeds(lst_ctx* ctx, int first_slot, int n_slots, const lst_seeds* seeds, void* cuda_stream);
+
 /* Steps a1..a4 for one slot / for slots first_slot .. first_slot+n_slots-1 in ONE set of
  * launches (the batch index is a grid dimension).  Asynchronous; no host synchronisation. */
 LST_API int lst_run(lst_ctx* ctx, int slot, void* cuda_stream);
@@ -247,7 +294,8 @@ LST_API int lst_run_batch(lst_ctx* ctx, int first_slot, int n_slots, void* cuda_
  * one before it (LST_ERR_STATE otherwise); after a partial run the views / fetches of the classes built so far
  * are valid (BASELINE.json configs[4] runs the mini-doublet and segment stages only).  LST_CLEAN (duplicate
  * cleaning of the quintuplets, DESIGN.md section 1 [D]) is not part of lst_run / lst_run_batch: run it with
- * lst_run_stage after LST_T5. */
+ * lst_run_stage after LST_T5.  LST_PIXEL (DESIGN.md section 1 [P]) likewise: after LST_T5 and lst_load_seeds
+ * (LST_ERR_STATE otherwise), independent of LST_CLEAN. */
 LST_API int lst_run_stage(lst_ctx* ctx, int first_slot, int n_slots, int stage, void* cuda_stream);
 
 /* Waits for `cuda_stream`, reads the slot's counters back and returns its status:
@@ -267,6 +315,11 @@ LST_API int lst_get_triplets(lst_ctx* ctx, int slot, lst_t3_view* out);
 LST_API int lst_get_quintuplets(lst_ctx* ctx, int slot, lst_t5_view* out);
 /* Valid after LST_CLEAN was run (lst_run_stage) and the slot synced. */
 LST_API int lst_get_track_candidates(lst_ctx* ctx, int slot, lst_tc_view* out);
+/* Valid after LST_PIXEL was run and the slot synced; kind 0 = pixel triplets, 1 = pixel quintuplets. */
+LST_API int lst_get_pixel_links(lst_ctx* ctx, int slot, int kind, lst_pix_view* out);
+/* The same to HOST memory: link_out[n][2] (seed, outer object), f_out[n][3]; either may be NULL.  LST_ERR_ARG if
+ * cap < n (lst_get_stats.pix_needed).  Synchronises `cuda_stream`. */
+LST_API int lst_fetch_pixel_links(lst_ctx* ctx, int slot, int kind, int32_t* link_out, float* f_out, int64_t cap, void* cuda_stream);
 /* Indices (into the quintuplet arrays, ascending) of the kept quintuplets to HOST memory: out[n_kept];
  * LST_ERR_ARG if cap < n_kept.  Synchronises `cuda_stream`. */
 LST_API int lst_fetch_kept(lst_ctx* ctx, int slot, int32_t* out, int64_t cap, void* cuda_stream);

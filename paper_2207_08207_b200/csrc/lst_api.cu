@@ -26,7 +26,7 @@
 using namespace lst;
 
 static_assert((int)LST_MD == (int)LST_MD_ && (int)LST_SEG == (int)LST_SEG_ && (int)LST_T3 == (int)LST_T3_ &&
-                  (int)LST_T5 == (int)LST_T5_ && (int)LST_CLEAN == (int)LST_CLEAN_, "stage ids");
+                  (int)LST_T5 == (int)LST_T5_ && (int)LST_CLEAN == (int)LST_CLEAN_ && (int)LST_PIXEL == (int)LST_PIXEL_, "stage ids");
 
 namespace {
 
@@ -35,8 +35,10 @@ struct SlotHost {
   int stages_run = 0;         // stages a1 .. run in order since the load: objects of class k are valid iff stages_run > k
   int n_hits_in = 0;
   SlotHeader* hdr = nullptr;  // pinned host copy of the device header
-  cudaEvent_t ev[17] = {};    // timing mode: ev[0..3] around the 3 a0 kernels, ev[4 + 2 s], ev[5 + 2 s] around stage s, ev[12..16] around the 4 cleaning steps
-  bool ev_bin = false, ev_stage[5] = {false, false, false, false, false};
+  bool seeds_loaded = false, pixel_run = false;   // [P]: lst_load_seeds since the last lst_load_event; LST_PIXEL since then
+  int n_seeds_in = 0;
+  cudaEvent_t ev[22] = {};    // timing mode: ev[0..3] around the 3 a0 kernels, ev[4 + 2 s], ev[5 + 2 s] around stage s, ev[12..16] around the 4 cleaning steps, ev[17..18] around k_seed_bin, ev[19..21] around the two link kernels
+  bool ev_bin = false, ev_stage[5] = {false, false, false, false, false}, ev_seed = false, ev_pix = false;
 };
 
 }  // namespace
@@ -85,6 +87,8 @@ Layout make_layout(const lst_config& cfg, int n_modules) {
   L.n_modules = n_modules;
   L.n_bins = 2 * n_modules;
   L.cap_hits = cfg.cap_hits; L.cap_md = cfg.cap_md; L.cap_seg = cfg.cap_seg; L.cap_t3 = cfg.cap_t3; L.cap_t5 = cfg.cap_t5;
+  L.cap_seeds = cfg.cap_seeds; L.cap_pix[0] = cfg.cap_pt3; L.cap_pix[1] = cfg.cap_pt5;
+  L.n_chunk_pix[0] = (cfg.cap_t3 + kChunk - 1) / kChunk; L.n_chunk_pix[1] = (cfg.cap_t5 + kChunk - 1) / kChunk;
   const int owner_cap[4] = {cfg.cap_hits, cfg.cap_md, cfg.cap_seg, cfg.cap_t3};
   for (int k = 0; k < 4; ++k) L.n_chunk[k] = (owner_cap[k] + kChunk - 1) / kChunk;
   size_t off = 0;
@@ -107,9 +111,22 @@ Layout make_layout(const lst_config& cfg, int n_modules) {
   L.t3_start = take(4 * (ns + 1));
   L.t3_pack = take(16 * n3); L.t3_seg = take(8 * n3); L.t3_chi2 = take(4 * n3);
   L.t5_start = take(4 * (n3 + 1));
-  L.t5_md = take(20 * n5); L.t5_t3 = take(8 * n5); L.t5_f = take(20 * n5);
+  L.t5_md = take(20 * n5); L.t5_t3 = take(8 * n5); L.t5_f = take(20 * n5); L.t5_kfit = take(4 * n5);
   L.t5_hits = take(40 * n5); L.t5_score = take(4 * n5); L.t5_keep = take(n5); L.tc_list = take(4 * n5);
   L.inc_start = take(4 * (nm + 8)); L.inc_cur = take(4 * (nm + 8)); L.inc_list = take(40 * n5);
+  {  // [P]
+    const size_t nsd = (size_t)cfg.cap_seeds;
+    L.seed_in = take(20 * nsd); L.seed_rec4 = take(16 * nsd); L.seed_rec2 = take(8 * nsd);
+    L.seed_bin_start = take(4 * (size_t)(kSeedBins + 3));
+    for (int k = 0; k < 2; ++k) L.lb_pix[k] = take(8 * (size_t)(L.n_chunk_pix[k] + 1));
+    L.lb_pix_bytes = off - L.lb_pix[0];
+    const size_t nobj[2] = {n3, n5};
+    for (int k = 0; k < 2; ++k) {
+      L.pix_start[k] = take(4 * (nobj[k] + 1));
+      L.pix_link[k] = take(8 * (size_t)L.cap_pix[k]);
+      L.pix_f[k] = take(12 * (size_t)L.cap_pix[k]);
+    }
+  }
   size_t scr = 16 * nm;   // one gathered table at a time: hit-index tuples (8 / 16 / 24 / 40 B) or packed values (16 / 16 / 8 / 20 B)
   if (16 * ns > scr) scr = 16 * ns;
   if (24 * n3 > scr) scr = 24 * n3;
@@ -150,6 +167,8 @@ void copy_cuts(Cuts& d, const lst_config& s) {
   d.t5_dkappa_max = s.t5_dkappa_max;
   for (int i = 0; i < 2; ++i) d.t5_chi2rz_max[i] = s.t5_chi2rz_max[i];
   d.t5_chi2xy_max = s.t5_chi2xy_max; d.t5_sigma_xy2_scaled = s.t5_sigma_xy2_scaled; d.t5_kappa_max = s.t5_kappa_max;
+  for (int i = 0; i < 2; ++i) { d.pix_dkappa_max[i] = s.pix_dkappa_max[i]; d.pix_chi2xy_max[i] = s.pix_chi2xy_max[i]; d.pix_chi2rz_max[i] = s.pix_chi2rz_max[i]; }
+  for (int i = 0; i < 6; ++i) { d.pix_inv_var_xy[i] = s.pix_inv_var_xy[i]; d.pix_inv_var_rz[i] = s.pix_inv_var_rz[i]; }
 }
 
 }  // namespace
@@ -200,6 +219,9 @@ int lst_default_config(lst_config* c) {
   c->timing = 0;
   c->t5_dup_min_shared = 7;
   c->store_half = 0;
+  c->cap_seeds = 16 * 1024;
+  c->cap_pt3 = 64 * 1024;
+  c->cap_pt5 = 64 * 1024;
   return LST_OK;
 }
 
@@ -216,6 +238,7 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
      have (five common layers with one common hit each give at most 5): smaller thresholds are refused, not approximated */
   if (cfg.t5_dup_min_shared < 6 || cfg.t5_dup_min_shared > 10) return LST_ERR_ARG;
   if (cfg.n_slots < 1 || cfg.cap_hits < 1 || cfg.cap_md < 1 || cfg.cap_seg < 1 || cfg.cap_t3 < 1 || cfg.cap_t5 < 1) return LST_ERR_ARG;
+  if (cfg.cap_seeds < 1 || cfg.cap_pt3 < 1 || cfg.cap_pt5 < 1 || cfg.cap_seeds > kMaxCap || cfg.cap_pt3 > kMaxCap || cfg.cap_pt5 > kMaxCap) return LST_ERR_ARG;
   for (int i = 0; i < n; ++i)
     if (g->layer[i] < 0 || g->layer[i] >= LST_N_LAYERS) return LST_ERR_ARG;
   if (m->row_offsets[0] != 0) return LST_ERR_ARG;
@@ -345,6 +368,7 @@ int lst_load_events(lst_ctx* c, int first, int n_ev, const lst_hits* hits, void*
       sh.n_hits_in = h->n;
       sh.ev_bin = false;
       for (bool& f : sh.ev_stage) f = false;
+      sh.seeds_loaded = sh.pixel_run = sh.ev_seed = sh.ev_pix = false;
       char* base = c->arena + (size_t)slot * c->P.slot_stride;
       HitInput in{h->x, h->y, h->z, h->module, h->side, h->n, 0};
       const HitInput staged{reinterpret_cast<const float*>(base + L.in_x), reinterpret_cast<const float*>(base + L.in_y),
@@ -405,14 +429,24 @@ int lst_load_events(lst_ctx* c, int first, int n_ev, const lst_hits* hits, void*
 int lst_load_event(lst_ctx* c, int slot, const lst_hits* h, void* stream) { return lst_load_events(c, slot, 1, h, stream); }
 
 int lst_run_stage(lst_ctx* c, int first, int n, int stage, void* stream) {
-  if (!c || n < 1 || !valid_slot(c, first) || !valid_slot(c, first + n - 1) || stage < LST_MD || stage > LST_CLEAN) return LST_ERR_ARG;
-  for (int s = first; s < first + n; ++s)
-    if (!c->slots[s].loaded || c->slots[s].stages_run < stage) return LST_ERR_STATE;   // a stage needs the one before it
+  if (!c || n < 1 || !valid_slot(c, first) || !valid_slot(c, first + n - 1) || stage < LST_MD || stage > LST_PIXEL) return LST_ERR_ARG;
+  for (int s = first; s < first + n; ++s) {
+    const SlotHost& h = c->slots[s];
+    if (!h.loaded || h.stages_run < (stage == LST_PIXEL ? (int)LST_T5 + 1 : stage)) return LST_ERR_STATE;   // a stage needs the one before it
+    if (stage == LST_PIXEL && !h.seeds_loaded) return LST_ERR_STATE;
+  }
   cudaStream_t st = (cudaStream_t)stream;
   LST_CUDA(c, cudaSetDevice(c->device));
   SlotHost& sh = c->slots[first];
   Params P = c->P;
   P.first_slot = first;
+  if (stage == LST_PIXEL) {   // beside the linear chain: stages_run stays
+    c->launches += launch_pixel(P, n, st, c->cfg.timing ? sh.ev + 19 : nullptr);
+    LST_CUDA(c, cudaGetLastError());
+    sh.ev_pix = c->cfg.timing != 0;
+    for (int s = first; s < first + n; ++s) { c->slots[s].synced = false; c->slots[s].pixel_run = true; }
+    return LST_OK;
+  }
   if (stage == LST_CLEAN)
     c->launches += launch_clean(P, n, st, c->cfg.timing ? sh.ev + 12 : nullptr);
   else
@@ -420,6 +454,54 @@ int lst_run_stage(lst_ctx* c, int first, int n, int stage, void* stream) {
   LST_CUDA(c, cudaGetLastError());
   if (c->cfg.timing) sh.ev_stage[stage] = true;
   for (int s = first; s < first + n; ++s) { c->slots[s].synced = false; c->slots[s].stages_run = stage + 1; }
+  return LST_OK;
+}
+
+int lst_load_seeds(lst_ctx* c, int first, int n_ev, const lst_seeds* seeds, void* stream) {
+  if (!c || n_ev < 1 || !valid_slot(c, first) || !valid_slot(c, first + n_ev - 1) || !seeds) return LST_ERR_ARG;
+  for (int b = 0; b < n_ev; ++b) {
+    const lst_seeds* q = seeds + b;
+    if (q->n < 0) return LST_ERR_ARG;
+    if (q->n > 0 && (!q->kappa || !q->cphi || !q->sphi || !q->z0 || !q->t)) return LST_ERR_ARG;
+    if (!c->slots[first + b].loaded) return LST_ERR_STATE;
+    if (q->n > c->cfg.cap_seeds) return LST_ERR_OVERFLOW;
+  }
+  cudaStream_t s = (cudaStream_t)stream;
+  LST_CUDA(c, cudaSetDevice(c->device));
+  const Layout& L = c->P.L;
+  for (int b0 = 0; b0 < n_ev; b0 += kMaxBatch) {
+    const int nb = n_ev - b0 < kMaxBatch ? n_ev - b0 : kMaxBatch;
+    SeedBatch src;
+    std::memset(&src, 0, sizeof(src));
+    for (int b = 0; b < nb; ++b) {
+      const lst_seeds* q = seeds + b0 + b;
+      SlotHost& sh = c->slots[first + b0 + b];
+      sh.seeds_loaded = sh.pixel_run = sh.synced = false;
+      sh.n_seeds_in = q->n;
+      const float* in[5] = {q->kappa, q->cphi, q->sphi, q->z0, q->t};
+      if (!q->on_device && q->n > 0) {
+        // pinned host arrays are read by the binning kernel over PCIe (100 kB per event); pageable ones are copied first
+        const void* al[5];
+        bool mapped = true;
+        for (int k = 0; k < 5; ++k) { al[k] = mapped_alias(in[k]); mapped = mapped && al[k]; }
+        float* stage = reinterpret_cast<float*>(c->arena + (size_t)(first + b0 + b) * c->P.slot_stride + L.seed_in);
+        for (int k = 0; k < 5; ++k) {
+          if (mapped) { in[k] = static_cast<const float*>(al[k]); continue; }
+          float* d = stage + (size_t)k * (size_t)c->cfg.cap_seeds;
+          LST_CUDA(c, cudaMemcpyAsync(d, in[k], 4 * (size_t)q->n, cudaMemcpyHostToDevice, s));
+          in[k] = d;
+        }
+      }
+      src.ev[b] = SeedInput{in[0], in[1], in[2], in[3], in[4], q->n};
+    }
+    Params P = c->P;
+    P.first_slot = first + b0;
+    SlotHost& s0 = c->slots[first + b0];
+    c->launches += launch_seed_bin(P, src, nb, s, c->cfg.timing ? s0.ev + 17 : nullptr);
+    LST_CUDA(c, cudaGetLastError());
+    s0.ev_seed = c->cfg.timing != 0;
+    for (int b = 0; b < nb; ++b) c->slots[first + b0 + b].seeds_loaded = true;
+  }
   return LST_OK;
 }
 
@@ -525,6 +607,41 @@ int lst_get_track_candidates(lst_ctx* c, int slot, lst_tc_view* v) {
   return LST_OK;
 }
 
+static int pixel_ready(lst_ctx* c, int slot, int kind) {
+  if (!valid_slot(c, slot) || kind < 0 || kind > 1) return LST_ERR_ARG;
+  const SlotHost& sh = c->slots[slot];
+  if (!sh.synced || !sh.pixel_run) return LST_ERR_STATE;
+  if (sh.hdr->overflow) return LST_ERR_OVERFLOW;
+  return LST_OK;
+}
+
+int lst_get_pixel_links(lst_ctx* c, int slot, int kind, lst_pix_view* v) {
+  const int r = pixel_ready(c, slot, kind);
+  if (r != LST_OK || !v) return r != LST_OK ? r : LST_ERR_ARG;
+  const Layout& L = c->P.L;
+  const char* b = c->arena + (size_t)slot * c->P.slot_stride;
+  v->n = c->slots[slot].hdr->n_pix[kind];
+  v->link = (const int32_t*)(b + L.pix_link[kind]);
+  v->f = (const float*)(b + L.pix_f[kind]);
+  v->object_start = (const int32_t*)(b + L.pix_start[kind]);
+  return LST_OK;
+}
+
+int lst_fetch_pixel_links(lst_ctx* c, int slot, int kind, int32_t* link_out, float* f_out, int64_t cap, void* stream) {
+  const int r = pixel_ready(c, slot, kind);
+  if (r != LST_OK) return r;
+  const int n = c->slots[slot].hdr->n_pix[kind];
+  if (n == 0) return LST_OK;
+  if (cap < n) return LST_ERR_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  LST_CUDA(c, cudaSetDevice(c->device));
+  const char* b = c->arena + (size_t)slot * c->P.slot_stride;
+  if (link_out) LST_CUDA(c, cudaMemcpyAsync(link_out, b + c->P.L.pix_link[kind], 8 * (size_t)n, cudaMemcpyDeviceToHost, s));
+  if (f_out) LST_CUDA(c, cudaMemcpyAsync(f_out, b + c->P.L.pix_f[kind], 12 * (size_t)n, cudaMemcpyDeviceToHost, s));
+  LST_CUDA(c, cudaStreamSynchronize(s));
+  return LST_OK;
+}
+
 int lst_fetch_kept(lst_ctx* c, int slot, int32_t* out, int64_t cap, void* stream) {
   const int r = view_ready(c, slot, LST_CLEAN);
   if (r != LST_OK) return r;
@@ -549,6 +666,12 @@ int lst_get_stats(lst_ctx* c, int slot, lst_stats* o) {
   o->overflow = sh.hdr->overflow;
   o->bad_hits = sh.hdr->bad_hits;
   o->n_kept = sh.stages_run > LST_CLEAN ? sh.hdr->n_kept : 0;
+  if (sh.seeds_loaded) o->n_seeds = sh.hdr->n_seeds;
+  if (sh.pixel_run)
+    for (int k = 0; k < 2; ++k) {
+      o->pix_needed[k] = (int64_t)sh.hdr->needed_pix[k]; o->pix_candidates[k] = (int64_t)sh.hdr->cand_pix[k];
+      o->pix_evaluated[k] = (int64_t)sh.hdr->eval_pix[k]; o->pix_rewalks[k] = (int64_t)sh.hdr->rewalk_pix[k];
+    }
   if (c->cfg.timing) {
     if (sh.ev_bin) {
       cudaEventElapsedTime(&o->stage_ms[0], sh.ev[0], sh.ev[3]);
@@ -556,6 +679,8 @@ int lst_get_stats(lst_ctx* c, int slot, lst_stats* o) {
     }
     if (sh.ev_stage[4])
       for (int k = 0; k < 4; ++k) cudaEventElapsedTime(&o->kernel_ms[7 + k], sh.ev[12 + k], sh.ev[13 + k]);
+    if (sh.ev_seed) cudaEventElapsedTime(&o->pix_ms[0], sh.ev[17], sh.ev[18]);
+    if (sh.ev_pix) { cudaEventElapsedTime(&o->pix_ms[1], sh.ev[19], sh.ev[20]); cudaEventElapsedTime(&o->pix_ms[2], sh.ev[20], sh.ev[21]); }
     for (int st = 0; st < 4; ++st)
       if (sh.ev_stage[st]) {
         cudaEvent_t* e = sh.ev + 4 + 2 * st;

@@ -29,6 +29,12 @@ struct Cuts {
   float t5_chi2xy_max;
   float t5_sigma_xy2_scaled;
   float t5_kappa_max;
+  // [P] pixel line segment + outer object; index [0] = pixel triplets, [1] = pixel quintuplets
+  float pix_dkappa_max[2];
+  float pix_inv_var_xy[6];
+  float pix_inv_var_rz[6];
+  float pix_chi2xy_max[2];
+  float pix_chi2rz_max[2];
 };
 
 // SINTHR(r, cosE, sinE) = sin(asin(min(1, r * kappa_max / 2)) + eps)
@@ -224,6 +230,48 @@ __device__ __forceinline__ bool t5_select(const Cuts& c, int layer1, float kappa
   o.kfit = kfit;
   o.chi2xy = chi2xy;
   o.chi2rz = chi2rz;
+  return true;
+}
+
+// ---- [P] pixel line segment + outer object -------------------------------
+// "the straight lines and circles in the r-z and x-y plane, respectively, are not fit but rather the estimates from the
+// pixel detector are used and the consistency of the outer hits to this hypothesis is checked".
+// seed = (kappa, cos phi0, sin phi0, z0, t); the outer object brings N = 3 (triplet, kind 0) or 5 (quintuplet, kind 1)
+// anchors on layers layer1 .. layer1 + N - 1 and its own curvature kobj.
+struct PixOut {
+  float chi2xy, chi2rz, dk;
+};
+template <int N>
+__device__ __forceinline__ bool pix_select(const Cuts& c, int kind, int layer1, float kappa, float cphi, float sphi,
+                                           float z0, float t, float kobj, const float4 (&p)[N], PixOut& o) {
+  const float hk = 0.5f * kappa;
+  // P0: the first anchor lies ahead of the seed (the outgoing arc of the circle)
+  if (!(p[0].x * cphi + p[0].y * sphi > 0.0f)) return false;
+  // P1
+  const float dk = kobj - kappa;
+  if (!(fabsf(dk) <= c.pix_dkappa_max[kind])) return false;
+  // P2: distance of the anchors from the seed's circle through the beam line
+  float chi2xy = 0.0f;
+#pragma unroll
+  for (int i = 0; i < N; ++i) {
+    const float e = (hk * (p[i].w * p[i].w) + p[i].x * sphi) - p[i].y * cphi;
+    chi2xy = chi2xy + (e * e) * c.pix_inv_var_xy[layer1 + i];
+  }
+  if (!(chi2xy <= c.pix_chi2xy_max[kind])) return false;
+  // P3: distance of the anchors from the seed's line z = z0 + t s, s = arc length by its power series in (kappa r / 2)^2
+  float chi2rz = 0.0f;
+#pragma unroll
+  for (int i = 0; i < N; ++i) {
+    const float r = p[i].w;
+    const float u = hk * r, u2 = u * u;
+    const float s = r * (1.0f + u2 * (0.16666667f + u2 * (0.075f + u2 * (0.04464286f + u2 * (0.030381944f + u2 * 0.022372158f)))));
+    const float d = (p[i].z - z0) - t * s;
+    chi2rz = chi2rz + (d * d) * c.pix_inv_var_rz[layer1 + i];
+  }
+  if (!(chi2rz <= c.pix_chi2rz_max[kind])) return false;
+  o.chi2xy = chi2xy;
+  o.chi2rz = chi2rz;
+  o.dk = dk;
   return true;
 }
 

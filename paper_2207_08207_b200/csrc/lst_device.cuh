@@ -46,7 +46,11 @@ constexpr int kChunk = 32;        // owners (lower hits / MDs / segments / tripl
 constexpr int kMaxBatch = 16;     // events per launch of the a0 kernels (pointer table in the launch parameters)
 constexpr int kMaxRow = 64;       // longest module-map row accepted
 constexpr int kMaxCap = 1 << 26;  // largest per-slot capacity: object indices are packed into 26 bits
-enum { LST_MD_ = 0, LST_SEG_ = 1, LST_T3_ = 2, LST_T5_ = 3, LST_CLEAN_ = 4 };  // == LST_MD .. LST_CLEAN of lst.h
+enum { LST_MD_ = 0, LST_SEG_ = 1, LST_T3_ = 2, LST_T5_ = 3, LST_CLEAN_ = 4, LST_PIXEL_ = 5 };  // == LST_MD .. LST_PIXEL of lst.h
+// [P] pixel line segments (seeds) are binned by the azimuth of their direction at the beam line: kSeedBins uniform bins
+// over (-pi, pi], then bin kSeedBins = seeds whose (cos, sin) is not a unit vector (no azimuth window can be derived for
+// them: every object looks at them), then bin kSeedBins + 1 = seeds that no object can accept (non-finite or zero direction).
+constexpr int kSeedBins = 1024;
 
 struct SlotHeader {
   int n_hits;                     // valid hits binned
@@ -66,12 +70,19 @@ struct SlotHeader {
   unsigned int ticket[4];         // next chunk of the single-pass kernels (zeroed with the header)
   int n_kept;                     // quintuplets kept by the duplicate cleaning (stage LST_CLEAN)
   unsigned int bad_acc;           // invalid hits seen by k_bin_count so far; moved to bad_hits and cleared by its last block
+  // [P] pixel links, index 0 = pixel triplets (seed + T3), 1 = pixel quintuplets (seed + T5); written by k_seed_bin / k_pix
+  int n_seeds;                    // seeds loaded (lst_load_seeds)
+  int n_pix[2];                   // links stored (clamped to capacity); overflow bits 4, 5
+  unsigned int ticket_pix[2];
+  unsigned long long needed_pix[2], cand_pix[2], eval_pix[2], rewalk_pix[2];
 };
 
 struct Layout {
   int n_modules, n_bins;
   int cap_hits, cap_md, cap_seg, cap_t3, cap_t5;
+  int cap_seeds, cap_pix[2];      // [P] seeds per slot; pixel triplets / pixel quintuplets per slot
   int n_chunk[4];                 // ceil(cap of the OWNER class / kChunk): hits, MD, LS, T3
+  int n_chunk_pix[2];             // owners of the pixel stage: T3, T5
   // byte offsets from the slot base (all multiples of 256)
   size_t hdr, bin_cnt, bin_start, lb[4];      // header; bin counters (self-cleaning); bin offsets; look-back words (contiguous)
   size_t lb_bytes;                            // bytes of the four look-back arrays, zeroed by k_bin_scatter
@@ -83,7 +94,13 @@ struct Layout {
   size_t seg_start, seg_md, seg_f;
   size_t t3_start, t3_pack, t3_seg, t3_chi2;
   size_t t5_start, t5_md, t5_t3, t5_f;
+  size_t t5_kfit;                             // fitted curvature in fp32 whatever the store ([P] P1 reads it)
   size_t t5_hits, t5_score, t5_keep, tc_list, inc_start, inc_cur, inc_list;   // duplicate cleaning
+  // [P]: copy destination of host seed arrays (5 x cap_seeds floats); seeds ordered by azimuth bin: (kappa, cos, sin, z0),
+  // (t, original index); bin offsets [kSeedBins + 3]; look-back words of the two link kernels (contiguous, cleared by
+  // k_seed_bin); per kind: CSR offsets by outer object, links (seed, object), values (chi2xy, chi2rz, kappa_obj - kappa)
+  size_t seed_in, seed_rec4, seed_rec2, seed_bin_start, lb_pix[2], lb_pix_bytes;
+  size_t pix_start[2], pix_link[2], pix_f[2];
   size_t scratch;
   size_t slot_bytes;
 };
@@ -146,12 +163,20 @@ struct Slot {
   __device__ __forceinline__ float* t5_f() const { return at<float>(L.t5_f); }
   __device__ __forceinline__ int* t5_hits() const { return at<int>(L.t5_hits); }
   __device__ __forceinline__ float* t5_score() const { return at<float>(L.t5_score); }
+  __device__ __forceinline__ float* t5_kfit() const { return at<float>(L.t5_kfit); }
   __device__ __forceinline__ unsigned char* t5_keep() const { return at<unsigned char>(L.t5_keep); }
   __device__ __forceinline__ int* tc_list() const { return at<int>(L.tc_list); }
   __device__ __forceinline__ int* inc_start() const { return at<int>(L.inc_start); }
   __device__ __forceinline__ int* inc_cur() const { return at<int>(L.inc_cur); }
   __device__ __forceinline__ int2* inc_list() const { return at<int2>(L.inc_list); }
   __device__ __forceinline__ int* scratch() const { return at<int>(L.scratch); }
+  __device__ __forceinline__ float4* seed_rec4() const { return at<float4>(L.seed_rec4); }
+  __device__ __forceinline__ float2* seed_rec2() const { return at<float2>(L.seed_rec2); }
+  __device__ __forceinline__ int* seed_bin_start() const { return at<int>(L.seed_bin_start); }
+  __device__ __forceinline__ unsigned long long* lb_pix(int kind) const { return at<unsigned long long>(L.lb_pix[kind]); }
+  __device__ __forceinline__ int* pix_start(int kind) const { return at<int>(L.pix_start[kind]); }
+  __device__ __forceinline__ int2* pix_link(int kind) const { return at<int2>(L.pix_link[kind]); }
+  __device__ __forceinline__ float* pix_f(int kind) const { return at<float>(L.pix_f[kind]); }
 };
 
 // Raw input arrays of one event (caller's device pointers, mapped host memory, or the slot's copy destination).
@@ -169,6 +194,19 @@ struct HitBatch {
   HitInput ev[kMaxBatch];
 };
 
+// Seed arrays of one event (caller's device pointers, mapped host memory, or the slot's copy destination).
+struct SeedInput {
+  const float* kappa;
+  const float* cphi;
+  const float* sphi;
+  const float* z0;
+  const float* t;
+  int n;
+};
+struct SeedBatch {
+  SeedInput ev[kMaxBatch];
+};
+
 // Host-callable launchers (lst_kernels.cu). Each returns the number of kernels it launched.
 // `ev` (optional, timing mode): ev[0] is recorded before the first kernel, ev[k + 1] after kernel k.
 // `src`: the arrays k_bin_count reads (device, or mapped host memory with stage = 1); it is the only kernel that touches
@@ -183,6 +221,9 @@ int launch_bin(const Params& P, const HitBatch& src, int n_batch, cudaStream_t s
 int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEvent_t* ev);          // 1 kernel
 // Duplicate cleaning [D]: 6 kernels (prepare, count, scan, fill, mark, list); ev[0..4] around the four steps.
 int launch_clean(const Params& P, int n_batch, cudaStream_t s, cudaEvent_t* ev);
+// [P]: seeds of a batch to azimuth bins (1 kernel; ev[0..1]); pixel triplets + pixel quintuplets (2 kernels; ev[0..2]).
+int launch_seed_bin(const Params& P, const SeedBatch& src, int n_batch, cudaStream_t s, cudaEvent_t* ev);
+int launch_pixel(const Params& P, int n_batch, cudaStream_t s, cudaEvent_t* ev);
 // Per slot of a batch: device-visible aliases of pinned host buffers for the hit-index tuples / the float payload
 // (null = that table is not wanted there, or goes through the scratch area and the copy engine).
 struct OutTable {

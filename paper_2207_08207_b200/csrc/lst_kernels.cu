@@ -1135,6 +1135,7 @@ __device__ __forceinline__ void t5_emit(const Params& P, const Slot& S, int pos,
   md[0] = ta.x; md[1] = ta.y; md[2] = ta.z; md[3] = tb.y; md[4] = tb.z;
   S.t5_t3()[pos] = make_int2(A, B);
   S.t5_score()[pos] = chi2xy + chi2rz;   // [D] D1, one fp32 addition of the fp32 values whatever the store
+  S.t5_kfit()[pos] = kfit;               // [P] P1 reads the fitted curvature in fp32 whatever the store
   if (P.store_half) {   // [H]
     __half* f = reinterpret_cast<__half*>(S.t5_f()) + 5 * (size_t)pos;
     f[0] = __float2half_rn(__int_as_float(ta.w)); f[1] = __float2half_rn(__int_as_float(tb.w)); f[2] = __float2half_rn(kfit);
@@ -1497,6 +1498,351 @@ __global__ void __launch_bounds__(1024) k_clean_list(const __grid_constant__ Par
 }
 
 // ------------------------------------------------------------------------------------------
+// [P] pixel line segments -> pixel triplets / pixel quintuplets (DESIGN.md section 1 [P]; optional
+// stage LST_PIXEL).  The method's search space is the full product (outer object, seed); here the seeds are binned by the
+// azimuth of their direction at the beam line, and an object looks only at the bins its first anchor allows:
+// with phi_p the azimuth of the first anchor (x, y, r) and delta = phi0 - phi_p, the P2 term of that anchor is
+//     e = (kappa / 2) r^2 + x sin phi0 - y cos phi0 = (kappa / 2) r^2 + n r sin(delta),   n = |(cos phi0, sin phi0)|,
+// P2 needs e^2 / var_xy[layer] <= chi2xy_max (every term of the sum is >= 0), P1 confines kappa to kappa_obj +- dkappa_max
+// and P0 confines delta to (-pi/2, pi/2): an interval of sin(delta), hence of phi0.  Every seed inside the window goes
+// through the exact selection, so the link set does not depend on the window.  Seeds whose direction is not a unit vector
+// (|n^2 - 1| > 1e-3) have no such window: they sit in a bin of their own that every object looks at.
+// ------------------------------------------------------------------------------------------
+constexpr float kPiF = 3.14159274f;
+constexpr float kSeedBinScale = 162.974663f;   // kSeedBins / (2 pi)
+static_assert(kSeedBins == 1024, "k_seed_bin scans one azimuth bin per thread");
+
+__device__ __forceinline__ int seed_bin_of(float c, float s) {
+  // no object can accept it: a non-finite direction makes e infinite or NaN, a zero direction fails P0
+  if (!(fabsf(c) <= 3.4028235e38f) || !(fabsf(s) <= 3.4028235e38f) || (c == 0.0f && s == 0.0f)) return kSeedBins + 1;
+  const float n2 = c * c + s * s;
+  if (!(fabsf(n2 - 1.0f) <= 1e-3f)) return kSeedBins;
+  const int b = (int)floorf((atan2f(s, c) + kPiF) * kSeedBinScale);
+  return min(kSeedBins - 1, max(0, b));
+}
+
+// One block per event: histogram over the azimuth bins in shared memory, scan, scatter of the records (kappa, cos, sin, z0),
+// (t, original index).  The order inside a bin is the arrival order (it never reaches the output: links carry the original
+// seed index and are ordered by it).  Also clears the look-back words and the counters of the two link kernels.
+__global__ void __launch_bounds__(1024) k_seed_bin(const __grid_constant__ Params P, const __grid_constant__ SeedBatch B) {
+  __shared__ int s_cnt[kSeedBins + 2], s_cur[kSeedBins + 2], s_warp[32];
+  Slot S(P, blockIdx.y);
+  SlotHeader* H = S.hdr();
+  const SeedInput& in = B.ev[blockIdx.y];
+  const int n = min(in.n, P.L.cap_seeds);
+  const int tid = (int)threadIdx.x, lane = (int)lane_id();
+  for (int i = tid; i < kSeedBins + 2; i += 1024) s_cnt[i] = 0;
+  int4* lb = S.at<int4>(P.L.lb_pix[0]);
+  for (int i = tid; i < (int)(P.L.lb_pix_bytes / 16); i += 1024) lb[i] = make_int4(0, 0, 0, 0);
+  __syncthreads();
+  for (int i = tid; i < n; i += 1024) atomicAdd(&s_cnt[seed_bin_of(in.cphi[i], in.sphi[i])], 1);
+  __syncthreads();
+  const int v = s_cnt[tid];
+  const int incl = warp_incl_scan(v);
+  if (lane == 31) s_warp[tid >> 5] = incl;
+  __syncthreads();
+  if (tid < 32) {
+    const int w = s_warp[tid];
+    s_warp[tid] = warp_incl_scan(w) - w;
+  }
+  __syncthreads();
+  const int ex = s_warp[tid >> 5] + incl - v;
+  int* start = S.seed_bin_start();
+  s_cur[tid] = ex;
+  start[tid] = ex;
+  if (tid == kSeedBins - 1) {
+    const int n_binned = ex + v, n_live = n_binned + s_cnt[kSeedBins];
+    s_cur[kSeedBins] = n_binned;
+    s_cur[kSeedBins + 1] = n_live;
+    start[kSeedBins] = n_binned;
+    start[kSeedBins + 1] = n_live;
+    start[kSeedBins + 2] = n_live + s_cnt[kSeedBins + 1];
+  }
+  __syncthreads();
+  float4* rec4 = S.seed_rec4();
+  float2* rec2 = S.seed_rec2();
+  for (int i = tid; i < n; i += 1024) {
+    const float c = in.cphi[i], sn = in.sphi[i];
+    const int pos = atomicAdd(&s_cur[seed_bin_of(c, sn)], 1);
+    rec4[pos] = make_float4(in.kappa[i], c, sn, in.z0[i]);
+    rec2[pos] = make_float2(in.t[i], __int_as_float(i));
+  }
+  if (tid == 0) {
+    H->n_seeds = n;
+    atomicAnd(&H->overflow, ~0x30);
+    for (int k = 0; k < 2; ++k) {
+      H->n_pix[k] = 0;
+      H->ticket_pix[k] = 0u;
+      H->needed_pix[k] = H->cand_pix[k] = H->eval_pix[k] = H->rewalk_pix[k] = 0ull;
+    }
+  }
+}
+
+constexpr int kPixWarps = 4;
+constexpr int kPixStash = 64;
+template <int N>
+struct PixWarp {
+  float4 p[N][32];
+  float kobj[32];
+  int layer[32], tab[32];
+  int2 q[kQueue];
+  int cnt[2][32];
+  int stSeed[2][kPixStash], stOl[2][kPixStash];
+  float stV[2][3][kPixStash];
+};
+
+template <int KIND>
+__device__ __forceinline__ void pix_emit(const Params& P, const Slot& S, int pos, int obj, int seed, float chi2xy, float chi2rz,
+                                         float dk) {
+  if (pos >= P.L.cap_pix[KIND]) return;
+  S.pix_link(KIND)[pos] = make_int2(seed, obj);
+  float* f = S.pix_f(KIND) + 3 * (size_t)pos;
+  f[0] = chi2xy; f[1] = chi2rz; f[2] = dk;
+}
+
+// Owner lane: `n` candidates = nMain binned seeds starting at position `first` of the bin-ordered seed list (cyclic over
+// the nBinned binned seeds: the azimuth window may straddle +-pi) followed by all seeds of the non-unit bin.
+// Two levels: P1, P0 and the first anchor's term of P2 on every candidate (one 16-byte load), survivors compacted
+// into a queue; the full selection on full tiles of survivors.
+template <int KIND, bool DIRECT>
+__device__ __forceinline__ int pix_walk(const Params& P, const Slot& S, PixWarp<(KIND ? 5 : 3)>& sh, int buf, int n, int off,
+                                        int total, int first, int nMain, int nBinned, int A0, int base) {
+  constexpr int N = KIND ? 5 : 3;
+  const float4* rec4 = S.seed_rec4();
+  const float2* rec2 = S.seed_rec2();
+  const int lane = (int)lane_id();
+  const float dkmax = P.cuts.pix_dkappa_max[KIND], cxy = P.cuts.pix_chi2xy_max[KIND];
+  int running = 0, qh = 0, qt = 0;
+  auto full = [&](bool valid, int2 it) {
+    bool pass = false;
+    PixOut o;
+    int orig = 0;
+    const int ol = it.x;
+    if (valid) {
+      const float4 a = rec4[it.y];
+      const float2 b = rec2[it.y];
+      orig = __float_as_int(b.y);
+      float4 p[N];
+#pragma unroll
+      for (int i = 0; i < N; ++i) p[i] = sh.p[i][ol];
+      pass = pix_select<N>(P.cuts, KIND, sh.layer[ol], a.x, a.y, a.z, a.w, b.x, sh.kobj[ol], p, o);
+    }
+    const unsigned bal = __ballot_sync(kFull, pass);
+    if (pass) {
+      const int pos = running + __popc(bal & lanemask_lt());
+      if (!DIRECT) {
+        atomicAdd(&sh.cnt[buf][ol], 1);
+        if (pos < kPixStash) {
+          sh.stSeed[buf][pos] = orig; sh.stOl[buf][pos] = ol;
+          sh.stV[buf][0][pos] = o.chi2xy; sh.stV[buf][1][pos] = o.chi2rz; sh.stV[buf][2][pos] = o.dk;
+        }
+      } else {
+        pix_emit<KIND>(P, S, base + pos, A0 + ol, orig, o.chi2xy, o.chi2rz, o.dk);
+      }
+    }
+    running += __popc(bal);
+  };
+  auto drain = [&](bool all) {
+    while (qt - qh >= 32 || (all && qt > qh)) {
+      __syncwarp();
+      const bool valid = lane < qt - qh;
+      int2 it = make_int2(0, 0);
+      if (valid) it = sh.q[(qh + lane) & (kQueue - 1)];
+      full(valid, it);
+      qh += min(32, qt - qh);
+      __syncwarp();
+    }
+  };
+  for (int tb = 0; tb < total; tb += 32) {
+    const int rk = tile_owner(n, off, tb);
+    const int j = tb + lane;
+    const int ol = (j < total) ? sh.tab[rk] : 0;
+    const int jj = j - __shfl_sync(kFull, off, ol);
+    const int f0 = __shfl_sync(kFull, first, ol), nm = __shfl_sync(kFull, nMain, ol);
+    int idx = f0 + jj;
+    if (jj >= nm) idx = nBinned + (jj - nm);
+    else if (idx >= nBinned) idx -= nBinned;
+    bool keep = false;
+    if (j < total) {
+      const float4 a = rec4[idx];                     // kappa, cos, sin, z0
+      const float4 p0 = sh.p[0][ol];
+      const float hk = 0.5f * a.x;
+      const float e = (hk * (p0.w * p0.w) + p0.x * a.z) - p0.y * a.y;    // the i = 0 term of P2, exactly as pix_select
+      keep = fabsf(sh.kobj[ol] - a.x) <= dkmax && p0.x * a.y + p0.y * a.z > 0.0f &&
+             (e * e) * P.cuts.pix_inv_var_xy[sh.layer[ol]] <= cxy;
+    }
+    const unsigned bal = __ballot_sync(kFull, keep);
+    if (keep) sh.q[(qt + __popc(bal & lanemask_lt())) & (kQueue - 1)] = make_int2(ol, idx);
+    qt += __popc(bal);
+    drain(false);
+  }
+  drain(true);
+  return running;
+}
+
+template <int KIND>
+__global__ void __launch_bounds__(kPixWarps * 32, 6) k_pix(const __grid_constant__ Params P) {
+  constexpr int N = KIND ? 5 : 3;
+  __shared__ PixWarp<N> shw[kPixWarps];
+  __shared__ float s_E[2];
+  Slot S(P, blockIdx.y);
+  SlotHeader* H = S.hdr();
+  const int cap = P.L.cap_pix[KIND];
+  const int nObj = H->n[KIND ? LST_T5_ : LST_T3_];
+  const int nChunks = (nObj + kChunk - 1) / kChunk;
+  const int nSeeds = H->n_seeds;
+  const int lane = (int)lane_id();
+  PixWarp<N>& sh = shw[threadIdx.x >> 5];
+  const int* bs = S.seed_bin_start();
+  const int nBinned = bs[kSeedBins], nWild = bs[kSeedBins + 1] - nBinned;
+  int* pix_start = S.pix_start(KIND);
+  unsigned long long* status = S.lb_pix(KIND);
+  unsigned long long cand = 0, evals = 0;
+  // largest |e| the first anchor may have, by its layer, with slack far above the rounding of e
+  if (threadIdx.x < 2) s_E[threadIdx.x] = sqrtf(P.cuts.pix_chi2xy_max[KIND] / P.cuts.pix_inv_var_xy[threadIdx.x]) * 1.0001f + 1e-4f;
+  __syncthreads();
+
+  auto publish = [&](int total) {
+    H->needed_pix[KIND] = (unsigned long long)total;
+    H->n_pix[KIND] = min(total, cap);
+    if (total > cap) atomicOr(&H->overflow, 16 << KIND);
+  };
+  // the links of one object in ascending ORIGINAL seed index (the order of the method's loop over the seeds): an
+  // object has one or two links, so an insertion sort by its owner lane
+  auto finish = [&](int C, int b, int total, int base, bool from_stash) {
+    const int A0 = C * kChunk, A = A0 + lane;
+    const int mine = sh.cnt[b][lane];
+    int tot;
+    const int ex = warp_excl_scan(mine, tot);
+    if (from_stash) {
+      for (int i = ex + 1; i < ex + mine; ++i) {
+        const int key = sh.stSeed[b][i];
+        const float v0 = sh.stV[b][0][i], v1 = sh.stV[b][1][i], v2 = sh.stV[b][2][i];
+        int j = i - 1;
+        for (; j >= ex && sh.stSeed[b][j] > key; --j) {
+          sh.stSeed[b][j + 1] = sh.stSeed[b][j];
+          sh.stV[b][0][j + 1] = sh.stV[b][0][j]; sh.stV[b][1][j + 1] = sh.stV[b][1][j]; sh.stV[b][2][j + 1] = sh.stV[b][2][j];
+        }
+        sh.stSeed[b][j + 1] = key;
+        sh.stV[b][0][j + 1] = v0; sh.stV[b][1][j + 1] = v1; sh.stV[b][2][j + 1] = v2;
+      }
+      __syncwarp();
+      for (int t = lane; t < total; t += 32)
+        pix_emit<KIND>(P, S, base + t, A0 + sh.stOl[b][t], sh.stSeed[b][t], sh.stV[b][0][t], sh.stV[b][1][t], sh.stV[b][2][t]);
+    } else {
+      __syncwarp();   // the direct walk's stores of the other lanes
+      int2* link = S.pix_link(KIND);
+      float* f = S.pix_f(KIND);
+      const int lo = min(base + ex, cap), hi = min(base + ex + mine, cap);
+      for (int i = lo + 1; i < hi; ++i) {
+        const int2 key = link[i];
+        const float v0 = f[3 * (size_t)i], v1 = f[3 * (size_t)i + 1], v2 = f[3 * (size_t)i + 2];
+        int j = i - 1;
+        for (; j >= lo && link[j].x > key.x; --j) {
+          link[j + 1] = link[j];
+          f[3 * (size_t)(j + 1)] = f[3 * (size_t)j]; f[3 * (size_t)(j + 1) + 1] = f[3 * (size_t)j + 1]; f[3 * (size_t)(j + 1) + 2] = f[3 * (size_t)j + 2];
+        }
+        link[j + 1] = key;
+        f[3 * (size_t)(j + 1)] = v0; f[3 * (size_t)(j + 1) + 1] = v1; f[3 * (size_t)(j + 1) + 2] = v2;
+      }
+    }
+    if (A < nObj) pix_start[A] = min(base + ex, cap);
+    if (A == nObj - 1) {
+      pix_start[nObj] = min(base + total, cap);
+      publish(base + total);
+    }
+    __syncwarp();
+  };
+
+  int buf = 0, pC = -1, pTotal = 0;
+  for (;;) {
+    const int C = warp_ticket(&H->ticket_pix[KIND]);
+    if (C >= nChunks) {
+      if (C == 0 && lane == 0) {
+        publish(0);
+        pix_start[0] = 0;
+      }
+      break;
+    }
+    const int A0 = C * kChunk, A = A0 + lane;
+    int n = 0, first = 0, nMain = 0;
+    if (A < nObj) {
+      int md[N];
+      float kobj;
+      if (KIND) {
+        const int* m5 = S.t5_md() + 5 * (size_t)A;
+#pragma unroll
+        for (int i = 0; i < N; ++i) md[i] = m5[i];
+        kobj = S.t5_kfit()[A];
+      } else {
+        const int4 ta = S.t3_pack()[A];
+        md[0] = ta.x; md[1] = ta.y; md[2] = ta.z;
+        kobj = __int_as_float(ta.w);
+      }
+      const int layer = P.mod_layer[S.md_module()[md[0]]];
+      if (layer <= 1) {     // the first anchor of a pixel-linked object sits on one of the two innermost layers
+        const float4 p0 = S.md_anchor()[md[0]];
+        sh.p[0][lane] = p0;
+#pragma unroll
+        for (int i = 1; i < N; ++i) sh.p[i][lane] = S.md_anchor()[md[i]];
+        sh.kobj[lane] = kobj;
+        sh.layer[lane] = layer;
+        cand += (unsigned long long)nSeeds;
+        const float E = s_E[layer], r = p0.w;
+        bool whole = !(E < 1.0e30f);
+        if (!whole) {
+          const float dk = P.cuts.pix_dkappa_max[KIND] * 1.001f + 1e-7f;
+          const float hlo = 0.5f * (kobj - dk), hhi = 0.5f * (kobj + dk);
+          float a = -E / r - hhi * r, b = E / r - hlo * r;     // range of n sin(delta)
+          a -= fabsf(a) * 2e-3f + 1e-5f;
+          b += fabsf(b) * 2e-3f + 1e-5f;
+          if (a <= b && a <= 1.0f && b >= -1.0f) {
+            const float phip = atan2f(p0.y, p0.x);
+            const float lo = phip + asinf(fmaxf(a, -1.0f)) - 1e-4f, hi = phip + asinf(fminf(b, 1.0f)) + 1e-4f;
+            int blo = (int)floorf((lo + kPiF) * kSeedBinScale) - 1, bhi = (int)floorf((hi + kPiF) * kSeedBinScale) + 1;
+            if (bhi - blo + 1 >= kSeedBins) {
+              whole = true;
+            } else {
+              blo = ((blo % kSeedBins) + kSeedBins) % kSeedBins;
+              bhi = ((bhi % kSeedBins) + kSeedBins) % kSeedBins;
+              first = bs[blo];
+              nMain = (blo <= bhi) ? bs[bhi + 1] - first : (nBinned - first) + bs[bhi + 1];
+            }
+          }
+        }
+        if (whole) { first = 0; nMain = nBinned; }
+        n = nMain + nWild;
+      }
+    }
+    sh.cnt[buf][lane] = 0;
+    evals += (unsigned long long)n;
+    int total_c;
+    const int off = warp_excl_scan(n, total_c);
+    build_owner_table(n, sh.tab);
+    const int total = pix_walk<KIND, false>(P, S, sh, buf, n, off, total_c, first, nMain, nBinned, A0, 0);
+    publish_aggregate(status, C, total);
+    __syncwarp();
+    if (pC >= 0) {
+      finish(pC, buf ^ 1, pTotal, resolve_base(status, pC, pTotal), true);
+      pC = -1;
+    }
+    if (total <= kPixStash) {
+      pC = C; pTotal = total; buf ^= 1;
+    } else {
+      if (lane == 0) atomicAdd(&H->rewalk_pix[KIND], 1ull);
+      const int base = resolve_base(status, C, total);
+      pix_walk<KIND, true>(P, S, sh, buf, n, off, total_c, first, nMain, nBinned, A0, base);
+      finish(C, buf, total, base, false);
+    }
+  }
+  if (pC >= 0) finish(pC, buf ^ 1, pTotal, resolve_base(status, pC, pTotal), true);
+  cand = warp_sum_ull(cand);
+  evals = warp_sum_ull(evals);
+  if (lane == 0 && cand) atomicAdd(&H->cand_pix[KIND], cand);
+  if (lane == 0 && evals) atomicAdd(&H->eval_pix[KIND], evals);
+}
+
+// ------------------------------------------------------------------------------------------
 // output helpers: original-hit-index tuples and float payloads, one thread per object
 // ------------------------------------------------------------------------------------------
 // blockIdx.y = slot of the batch; the object count comes from the slot header (clamped to capacity).
@@ -1677,6 +2023,23 @@ int launch_clean(const Params& P, int n_batch, cudaStream_t s, cudaEvent_t* ev) 
   k_clean_list<<<dim3(1, (unsigned)n_batch), 1024, 0, s>>>(P);
   LST_EV(4);
   return 6;
+}
+
+int launch_seed_bin(const Params& P, const SeedBatch& src, int n_batch, cudaStream_t s, cudaEvent_t* ev) {
+  LST_EV(0);
+  k_seed_bin<<<dim3(1, (unsigned)n_batch), 1024, 0, s>>>(P, src);
+  LST_EV(1);
+  return 1;
+}
+
+int launch_pixel(const Params& P, int n_batch, cudaStream_t s, cudaEvent_t* ev) {
+  const unsigned nb = (unsigned)n_batch;
+  LST_EV(0);
+  k_pix<0><<<dim3(blocks_per_event((P.L.n_chunk_pix[0] + kPixWarps - 1) / kPixWarps, n_batch, 6, kGridShare), nb), kPixWarps * 32, 0, s>>>(P);
+  LST_EV(1);
+  k_pix<1><<<dim3(blocks_per_event((P.L.n_chunk_pix[1] + kPixWarps - 1) / kPixWarps, n_batch, 6, kGridShare), nb), kPixWarps * 32, 0, s>>>(P);
+  LST_EV(2);
+  return 2;
 }
 
 int launch_fetch_direct(const Params& P, const OutTable& T, int kind, int n_batch, cudaStream_t s) {

@@ -20,6 +20,8 @@ LIB_PATH = os.path.join(HERE, "liblst.so")
 N_LAYERS = 6
 MD, SEG, T3, T5 = 0, 1, 2, 3
 CLEAN = 4                                      # optional stage: duplicate cleaning of the quintuplets (run_stage only)
+PIXEL = 5                                      # optional stage: pixel line segments -> pixel triplets / quintuplets (run_stage only)
+PT3, PT5 = 0, 1                                # kinds of pixel links
 KIND_NAMES = ("md", "seg", "t3", "t5")
 KERNEL_NAMES = ("bin_count", "bin_scatter", "bin_order", "md", "seg", "t3", "t5",
                 "clean_prepare", "clean_count", "clean_fill", "clean_mark")   # lst_stats.kernel_ms[0..10]
@@ -56,7 +58,8 @@ class Config(C.Structure):
                 ("pix_chi2xy_max", C.c_float * 2), ("pix_chi2rz_max", C.c_float * 2),
                 ("device", C.c_int32), ("n_slots", C.c_int32), ("cap_hits", C.c_int32), ("cap_md", C.c_int32),
                 ("cap_seg", C.c_int32), ("cap_t3", C.c_int32), ("cap_t5", C.c_int32), ("timing", C.c_int32),
-                ("store_half", C.c_int32), ("t5_dup_min_shared", C.c_int32)]
+                ("store_half", C.c_int32), ("t5_dup_min_shared", C.c_int32),
+                ("cap_seeds", C.c_int32), ("cap_pt3", C.c_int32), ("cap_pt5", C.c_int32)]
 
     CUT_FIELDS = ("half_kappa_max", "z_lum", "md_cos_eps", "md_sin_eps", "md_dz_res", "md_eps", "seg_cos_eps",
                   "seg_sin_eps", "seg_z0_max", "t3_kappa_max", "t3_chi2rz_max", "sigma_z2", "inv_sigma_z2",
@@ -74,6 +77,15 @@ class Config(C.Structure):
 class Hits(C.Structure):
     _fields_ = [("n", C.c_int32), ("x", C.c_void_p), ("y", C.c_void_p), ("z", C.c_void_p),
                 ("module", C.c_void_p), ("side", C.c_void_p), ("on_device", C.c_int32)]
+
+
+class Seeds(C.Structure):
+    _fields_ = [("n", C.c_int32), ("kappa", C.c_void_p), ("cphi", C.c_void_p), ("sphi", C.c_void_p), ("z0", C.c_void_p),
+                ("t", C.c_void_p), ("on_device", C.c_int32)]
+
+
+class PixView(C.Structure):
+    _fields_ = [("n", C.c_int32), ("link", C.c_void_p), ("f", C.c_void_p), ("object_start", C.c_void_p)]
 
 
 class MdView(C.Structure):
@@ -99,7 +111,9 @@ class T5View(C.Structure):
 class Stats(C.Structure):
     _fields_ = [("n_hits", C.c_int32), ("needed", C.c_int64 * 4), ("candidates", C.c_int64 * 4),
                 ("evaluated", C.c_int64 * 4), ("overflow", C.c_int32), ("bad_hits", C.c_int32), ("stage_ms", C.c_float * 5), ("kernel_ms", C.c_float * 12),
-                ("rewalks", C.c_int64 * 4), ("n_kept", C.c_int32)]
+                ("rewalks", C.c_int64 * 4), ("n_kept", C.c_int32), ("n_seeds", C.c_int32), ("pix_needed", C.c_int64 * 2),
+                ("pix_candidates", C.c_int64 * 2), ("pix_evaluated", C.c_int64 * 2), ("pix_rewalks", C.c_int64 * 2),
+                ("pix_ms", C.c_float * 3)]
 
 
 class MapGeometry(C.Structure):
@@ -124,6 +138,9 @@ SYMBOLS = {
     "lst_destroy": (C.c_int, [C.c_void_p]),
     "lst_load_event": (C.c_int, [C.c_void_p, C.c_int, P(Hits), C.c_void_p]),
     "lst_load_events": (C.c_int, [C.c_void_p, C.c_int, C.c_int, P(Hits), C.c_void_p]),
+    "lst_load_seeds": (C.c_int, [C.c_void_p, C.c_int, C.c_int, P(Seeds), C.c_void_p]),
+    "lst_get_pixel_links": (C.c_int, [C.c_void_p, C.c_int, C.c_int, P(PixView)]),
+    "lst_fetch_pixel_links": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]),
     "lst_run": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
     "lst_run_batch": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p]),
     "lst_run_stage": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]),
@@ -327,6 +344,18 @@ class Lst:
             self._borrowed[first_slot + b] = keep
         return self._check(self.lib.lst_load_events(self.h, first_slot, len(events), arr, _stream(stream)), "lst_load_events")
 
+    def load_seeds(self, first_slot: int, seeds, stream=None):
+        """[P] seeds: sequence of (kappa, cphi, sphi, z0, t) tuples (all numpy / pinned host, or all torch CUDA tensors, f32);
+        entry b goes to slot first_slot + b.  After load_event(s) of the same slots, on the same stream."""
+        arr = (Seeds * len(seeds))()
+        for b, sd in enumerate(seeds):
+            on_device = hasattr(sd[0], "data_ptr") and getattr(sd[0], "is_cuda", False)
+            if not hasattr(sd[0], "data_ptr"):
+                sd = tuple(np.ascontiguousarray(a, np.float32) for a in sd)
+            self._borrowed[("seeds", first_slot + b)] = sd
+            arr[b] = Seeds(int(sd[0].shape[0]), *[_ptr(a) for a in sd], 1 if on_device else 0)
+        return self._check(self.lib.lst_load_seeds(self.h, first_slot, len(seeds), arr, _stream(stream)), "lst_load_seeds")
+
     def run(self, slot: int, stream=None):
         return self._check(self.lib.lst_run(self.h, slot, _stream(stream)), "lst_run")
 
@@ -376,7 +405,10 @@ class Lst:
         self._check(self.lib.lst_get_stats(self.h, slot, C.byref(s)), "lst_get_stats")
         return dict(n_hits=int(s.n_hits), needed=[int(v) for v in s.needed], candidates=[int(v) for v in s.candidates],
                     evaluated=[int(v) for v in s.evaluated], overflow=int(s.overflow), bad_hits=int(s.bad_hits), stage_ms=[float(v) for v in s.stage_ms],
-                    kernel_ms=[float(v) for v in s.kernel_ms], rewalks=[int(v) for v in s.rewalks], n_kept=int(s.n_kept))
+                    kernel_ms=[float(v) for v in s.kernel_ms], rewalks=[int(v) for v in s.rewalks], n_kept=int(s.n_kept),
+                    n_seeds=int(s.n_seeds), pix_needed=[int(v) for v in s.pix_needed], pix_candidates=[int(v) for v in s.pix_candidates],
+                    pix_evaluated=[int(v) for v in s.pix_evaluated], pix_rewalks=[int(v) for v in s.pix_rewalks],
+                    pix_ms=[float(v) for v in s.pix_ms])
 
     def _payload(self, p32, p16, shape):
         """The fp32 array of a view, or its binary16 twin when the context was created with store_half."""
@@ -419,6 +451,21 @@ class Lst:
         n5 = self.stats(slot)["needed"][T5]
         return dict(n=v.n, t5=DeviceArray(v.t5, (v.n,), "<i4", self), keep=DeviceArray(v.keep, (n5,), "|u1", self),
                     score=DeviceArray(v.score, (n5,), "<f4", self))
+
+    def pixel_links(self, slot: int, kind: int) -> dict:
+        """After run_stage(..., PIXEL) and sync: links of kind PT3 / PT5 (device arrays)."""
+        v = PixView()
+        self._check(self.lib.lst_get_pixel_links(self.h, slot, kind, C.byref(v)), "lst_get_pixel_links")
+        n_obj = self.stats(slot)["needed"][T5 if kind else T3]
+        return dict(n=v.n, link=DeviceArray(v.link, (v.n, 2), "<i4", self), f=DeviceArray(v.f, (v.n, 3), "<f4", self),
+                    object_start=DeviceArray(v.object_start, (n_obj + 1,), "<i4", self))
+
+    def fetch_pixel_links(self, slot: int, kind: int, stream=None):
+        """(link [n][2] = seed index, outer object index; f [n][3] = chi2xy, chi2rz, kappa_obj - kappa_seed), host numpy."""
+        n = self.stats(slot)["pix_needed"][kind]
+        link, f = np.empty((n, 2), np.int32), np.empty((n, 3), np.float32)
+        self._check(self.lib.lst_fetch_pixel_links(self.h, slot, kind, _ptr(link), _ptr(f), n, _stream(stream)), "lst_fetch_pixel_links")
+        return link, f
 
     def fetch_kept(self, slot: int, stream=None) -> np.ndarray:
         """Indices of the kept quintuplets (ascending), host numpy."""
