@@ -39,7 +39,7 @@ N_STREAMS = int(os.environ.get("LST_BENCH_STREAMS", "4"))   # BASELINE.json conf
 MAP_BYTES = 4 * (69630 + 6121)
 # SPEC operations per candidate (every sqrt and div counted as one)
 FLOPS_PER_CAND = (34, 51, 45, 255)
-HEADER_BYTES = 312   # per-slot counter block that lst_sync_batch reads back (csrc/lst_device.cuh SlotHeader)
+HEADER_BYTES = 400   # per-slot counter block that lst_sync_batch reads back (csrc/lst_device.cuh SlotHeader)
 A0_KERNELS = ("bin_count", "bin_scatter", "bin_order")               # lst_stats.kernel_ms[0..2]
 
 
@@ -159,6 +159,11 @@ def oracle_events_per_s(geom, mmap, events, check=None):
             assert got.shape == want.shape and set(map(tuple, got.tolist())) == set(map(tuple, want.tolist())), \
                 f"end-to-end quintuplets of event {k} differ from the oracle's"
     return len(events) / dt, dt
+
+
+def _oracle_with_seeds(geom, mmap, ev, sd):
+    from oracle import oracle
+    return oracle.load("f32").run(geom.layer, mmap.row_offsets, mmap.targets, ev.x, ev.y, ev.z, ev.module, ev.side, seeds=sd.arrays())
 
 
 def run_reference(args):
@@ -384,6 +389,7 @@ def run_ours(args):
 
     # ---- per-kernel times (CUDA events inside the library, timing mode), one 64-event batch ----
     kernel_ms, launches_per_step = per_kernel_times(lst, geom, mmap, d_in, local)
+    lp = launches_per_step                      # per-launch quantities: one launch covers 64 / lp events
     alone_ms, _ = per_kernel_times(lst, geom, mmap, d_in, local, alone=True)
     for k in lst.KERNEL_NAMES[7:]:
         kernel_ms.pop(k)
@@ -392,7 +398,6 @@ def run_ours(args):
     clean_alone_ms, _ = per_kernel_times(lst, geom, mmap, d_in, local, with_clean=True, alone=True, reps=3)
     clean_ms = {k: {"in_step": with_clean_ms[k], "alone": clean_alone_ms[k]} for k in lst.KERNEL_NAMES[7:]}
     peaks = measured_peaks()
-    lp = launches_per_step                      # per-launch quantities: one launch covers 64 / lp events
     roof, per_stage = roofline(kernel_ms, alone_ms, n_hits / lp, [v / lp for v in needed], [v / lp for v in evals], peaks, N_EVENTS // lp)
     spec_flops_step = sum(evals[i] * FLOPS_PER_CAND[i] for i in range(4))
     alu_peak = 148 * 128 * peaks["sm_max_mhz"] * 1e6 / 1e12
@@ -418,6 +423,45 @@ def run_ours(args):
              "ms_per_step_with_clean": clean_total_ms / args.steps, "kernels_ms_per_launch": clean_ms,
              "t5_in": needed[3], "t5_kept": kept,
              "what": "a0..a4 + LST_CLEAN per step; `value` above is a0..a4 only (the BASELINE.json path)"}
+
+    # ---- the path followed by the optional pixel-linking stage [P]: the stand-in seed
+    # model of DESIGN.md section 3, seeds resident in HBM like the hits, same timing rules ----
+    from paper_2207_08207_b200 import synth as _synth
+    seeds = [_synth.generate_seeds(e, rank_seed0(rank) + i) for i, e in enumerate(events)]
+    d_seeds = [[torch.from_numpy(a).to(dev) for a in sd.arrays()] for sd in seeds]
+
+    def step_device_pixel():
+        for s, st in enumerate(streams):
+            ctx.load_events(s * per_stream, d_in[s * per_stream:(s + 1) * per_stream], stream=st)
+            ctx.load_seeds(s * per_stream, d_seeds[s * per_stream:(s + 1) * per_stream], stream=st)
+            ctx.run_batch(s * per_stream, per_stream, st)
+            ctx.run_stage(s * per_stream, per_stream, lst.PIXEL, st)
+    timed(step_device_pixel, 3)
+    pix_total_ms = max_over_ranks(sum(timed(step_device_pixel, args.steps)), dist, dev)
+    for s, st in enumerate(streams):
+        ctx.sync_batch(s * per_stream, per_stream, st)
+    pst = [ctx.stats(k) for k in range(N_EVENTS)]
+    pix_links0 = [ctx.fetch_pixel_links(0, kind)[0] for kind in (0, 1)]
+    pix_objs0 = [ctx.fetch_hit_indices(0, lst.T3), ctx.fetch_hit_indices(0, lst.T5)]
+    pix_in, _ = per_kernel_times(lst, geom, mmap, d_in, local, d_seeds=d_seeds)
+    pix_alone, _ = per_kernel_times(lst, geom, mmap, d_in, local, d_seeds=d_seeds, alone=True, reps=3)
+    pix_sum = lambda key, k: int(sum(q[key][k] for q in pst))
+    n_seeds_step = int(sum(q["n_seeds"] for q in pst))
+    # algorithmic bytes (each input read once, each output written once): seeds 20 B in + 24 B ordered; per outer object its
+    # record (T3 16 B, T5 20 + 4 B) + 16 B per anchor + 4 B offset; 20 B per link
+    pix_bytes = [(16 + 3 * 16 + 4) * needed[2] + 20 * pix_sum("pix_needed", 0) + 44 * n_seeds_step,
+                 (24 + 5 * 16 + 4) * needed[3] + 20 * pix_sum("pix_needed", 1) + 24 * n_seeds_step]
+    pixel = {"events_per_s_with_pixel": whole_job_events_per_s(world, args.steps, pix_total_ms), "ms_per_step_with_pixel": pix_total_ms / args.steps,
+             "seeds_per_step": n_seeds_step,
+             "links_per_step": {"pt3": pix_sum("pix_needed", 0), "pt5": pix_sum("pix_needed", 1)},
+             "candidates_per_step": {"pt3": pix_sum("pix_candidates", 0), "pt5": pix_sum("pix_candidates", 1)},
+             "evaluated_per_step": {"pt3": pix_sum("pix_evaluated", 0), "pt5": pix_sum("pix_evaluated", 1)},
+             "rewalks_per_step": {"pt3": pix_sum("pix_rewalks", 0), "pt5": pix_sum("pix_rewalks", 1)},
+             "kernels_ms_per_launch": {k: {"in_step": pix_in[k], "alone": pix_alone[k]} for k in ("seed_bin", "pt3", "pt5")},
+             "hbm_frac_alone": {k: pix_bytes[i] / lp / (pix_alone[k] * 1e-3) / 1e9 / measured_peaks()["hbm_gbs"] for i, k in enumerate(("pt3", "pt5"))},
+             "what": "a0..a4 + lst_load_seeds + LST_PIXEL per step (hits and seeds resident in HBM); `value` above is a0..a4 only. The method's "
+                     "search space is the full (outer object, seed) product (candidates); the kernels evaluate the window of each "
+                     "object's first anchor (evaluated) and link sets equal the oracle's (tests/test_gpu_pixel.py)"}
 
     arena_mib = ctx.arena_bytes()[0] / 2 ** 20
     # ---- reduced-precision object store [H]: the same measurements with
@@ -487,7 +531,7 @@ def run_ours(args):
                                      "the durations with the GPU otherwise idle: what the 4-stream pipeline gains over running the same "
                                      "launches back to back"},
            "csrc_digest": csrc_digest(),
-           "duplicate_cleaning": clean, "reduced_precision_store": half, "module_map_builder": map_builder,
+           "duplicate_cleaning": clean, "pixel_linking": pixel, "reduced_precision_store": half, "module_map_builder": map_builder,
            "rewalks_per_step": dict(md=rewalks[0], ls=rewalks[1], t3=rewalks[2], t5=rewalks[3]),
            "arena_mib": arena_mib, "impl": "ours"}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -495,6 +539,12 @@ def run_ours(args):
         while t_cpu < 12.0 and n_pass < 8:          # a bounded sample: whole passes over the workload, >= 12 s of CPU work
             t_cpu += oracle_events_per_s(geom, mmap, events, check=e2e_tuples if n_pass == 0 else None)[1]
             n_pass += 1
+        # [P]: the links of event 0 as the timed step left them, against the oracle's full product
+        r0 = _oracle_with_seeds(geom, mmap, events[0], seeds[0])
+        for kind in (0, 1):
+            got = np.concatenate([pix_links0[kind][:, :1], pix_objs0[kind][pix_links0[kind][:, 1]].reshape(len(pix_links0[kind]), -1)], 1)
+            assert set(map(tuple, got.tolist())) == set(map(tuple, r0.pix_tuples(kind).tolist())), "pixel links of event 0 differ from the oracle's"
+        out["pixel_linking"]["verified"] = "pixel triplets and quintuplets of event 0 after the timed steps equal the oracle's (seed index + hit indices)"
         out["e2e"]["verified"] = f"the quintuplets of all {N_EVENTS} events as downloaded by the end-to-end arm equal the oracle's (sets of 10 hit indices)"
         out["cpu_baseline"] = {"value": n_pass * N_EVENTS / t_cpu, "unit": UNIT, "cores": 1, "kind": "oracle",
                                "sample": f"all {N_EVENTS} events of the workload x {n_pass} passes, single thread, {t_cpu:.1f} s"}
@@ -567,13 +617,14 @@ def pcie_ceiling(torch, dev, np_in, out_bytes, S, reps=10):
                     "no kernel running"}
 
 
-def per_kernel_times(lst, geom, mmap, d_in, local, with_clean=False, reps=6, alone=False, store_half=False):
+def per_kernel_times(lst, geom, mmap, d_in, local, with_clean=False, reps=6, alone=False, store_half=False, d_seeds=None):
     """Average duration (ms) of ONE launch of every kernel, from CUDA events recorded by the library around every launch on
     the stream it is launched on (lst_config.timing), L2 flushed before every step.
     alone=False: the configuration the timed region uses -- 4 streams x 16-event launches running concurrently (concurrent
     kernels share the SMs, so the durations of one step add up to more than the step).
     alone=True: the same 16-event launches one batch at a time on one stream, the GPU otherwise idle.
-    The optional cleaning stage [D] is timed the same way."""
+    The optional cleaning stage [D] is timed the same way; with d_seeds the step also loads the seeds and runs LST_PIXEL and
+    the three [P] kernels are returned instead."""
     import torch
     cfg = lst.default_config()
     cfg.device, cfg.n_slots, cfg.timing, cfg.store_half = local, N_EVENTS, 1, int(store_half)
@@ -588,12 +639,15 @@ def per_kernel_times(lst, geom, mmap, d_in, local, with_clean=False, reps=6, alo
         ctx.run_batch(s * per, per, st)
         if with_clean:                                  # optional stage [D], reported beside the path, not in it
             ctx.run_stage(s * per, per, lst.CLEAN, st)
+        if d_seeds is not None:                         # optional stage [P]
+            ctx.load_seeds(s * per, d_seeds[s * per:(s + 1) * per], stream=st)
+            ctx.run_stage(s * per, per, lst.PIXEL, st)
 
     def collect(s, st, keep):
         ctx.sync_batch(s * per, per, st)
         for k in range(s * per, (s + 1) * per, 16):    # one set of launches per 16 events; times kept on its first slot
             if keep:
-                rows.append(ctx.stats(k)["kernel_ms"][:11])
+                rows.append(ctx.stats(k)["pix_ms"] if d_seeds is not None else ctx.stats(k)["kernel_ms"][:11])
 
     for rep in range(reps + 2):
         if alone:
@@ -610,7 +664,8 @@ def per_kernel_times(lst, geom, mmap, d_in, local, with_clean=False, reps=6, alo
             for s, st in enumerate(streams):
                 collect(s, st, rep >= 2)
     ctx.close()
-    return dict(zip(lst.KERNEL_NAMES, np.mean(np.asarray(rows), axis=0).tolist())), max(1, per // 16) * N_STREAMS
+    names = ("seed_bin", "pt3", "pt5") if d_seeds is not None else lst.KERNEL_NAMES
+    return dict(zip(names, np.mean(np.asarray(rows), axis=0).tolist())), max(1, per // 16) * N_STREAMS
 
 
 def csrc_digest() -> str:

@@ -28,6 +28,8 @@ using namespace lst;
 static_assert((int)LST_MD == (int)LST_MD_ && (int)LST_SEG == (int)LST_SEG_ && (int)LST_T3 == (int)LST_T3_ &&
                   (int)LST_T5 == (int)LST_T5_ && (int)LST_CLEAN == (int)LST_CLEAN_ && (int)LST_PIXEL == (int)LST_PIXEL_, "stage ids");
 
+static_assert(sizeof(SlotHeader) == 400, "bench.py HEADER_BYTES counts the header lst_sync_batch reads back");
+
 namespace {
 
 struct SlotHost {
