@@ -281,6 +281,19 @@ def run_ours(args):
     total_ms = max_over_ranks(sum(ms), dist, dev)
     value = whole_job_events_per_s(world, args.steps, total_ms)
 
+    if args.profile and args.with_optional:
+        # the optional stages [D] and [P] in the profiled step too, so that one ncu capture covers every kernel
+        from paper_2207_08207_b200 import synth as _synth
+        d_sd = [[torch.from_numpy(a).to(dev) for a in _synth.generate_seeds(e, rank_seed0(rank) + i).arrays()] for i, e in enumerate(events)]
+
+        def step_all():
+            for s, st in enumerate(streams):
+                ctx.load_events(s * per_stream, d_in[s * per_stream:(s + 1) * per_stream], stream=st)
+                ctx.load_seeds(s * per_stream, d_sd[s * per_stream:(s + 1) * per_stream], stream=st)
+                ctx.run_batch(s * per_stream, per_stream, st)
+                ctx.run_stage(s * per_stream, per_stream, lst.CLEAN, st)
+                ctx.run_stage(s * per_stream, per_stream, lst.PIXEL, st)
+        timed(step_all, 2)
     if args.profile:
         if rank == 0:
             print(json.dumps({"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -827,6 +840,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--profile", action="store_true",
                     help="device-resident steps only (no e2e, per-kernel timing or CPU baseline): the command ncu wraps")
+    ap.add_argument("--with-optional", action="store_true", help="with --profile: two more steps that also run LST_CLEAN and LST_PIXEL")
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[4]: occupancy sweep of the a0 / MD / LS kernels")
     args = ap.parse_args()
     if args.sweep:

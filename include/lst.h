@@ -384,6 +384,15 @@ LST_API int lst_default_map_params(lst_map_params* params);
 LST_API int lst_build_module_map(const lst_map_geometry* geom, const lst_map_params* params, int device, int32_t* row_offsets,
                                  int32_t* targets, int64_t cap_targets, int64_t* n_targets, float* kernel_ms);
 
+/* Overflow recovery (BASELINE.json configs[3] "candidate-buffer overflow handling"; PAPER.md:143 sizes its buffers from the
+ * data too): after lst_sync* returned LST_ERR_OVERFLOW for `slot`, fills *out with the context's configuration in which every
+ * capacity that was exceeded is replaced by what the slot needed (lst_get_stats) times 1.25, rounded up to a multiple of 1024;
+ * capacities that sufficed are kept.  A stage that overflowed feeds the later stages a clamped input, so their needs are
+ * lower bounds: create a context from *out, run the event again, and repeat while it still overflows (at most once per
+ * object class).  Returns LST_OK (also when nothing overflowed: *out is then the current configuration), LST_ERR_STATE if the
+ * slot was not synced, LST_ERR_ARG. */
+LST_API int lst_grown_config(lst_ctx* ctx, int slot, lst_config* out);
+
 /* Bytes of the arena (all slots) and of one slot. */
 LST_API int lst_arena_bytes(lst_ctx* ctx, int64_t* total, int64_t* per_slot);
 /* Kernels launched by this context so far (for bench.py's gpu_launches). */

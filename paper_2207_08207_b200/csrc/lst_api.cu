@@ -118,7 +118,8 @@ Layout make_layout(const lst_config& cfg, int n_modules) {
   L.inc_start = take(4 * (nm + 8)); L.inc_cur = take(4 * (nm + 8)); L.inc_list = take(40 * n5);
   {  // [P]
     const size_t nsd = (size_t)cfg.cap_seeds;
-    L.seed_in = take(20 * nsd); L.seed_rec4 = take(16 * nsd); L.seed_rec2 = take(8 * nsd);
+    L.seed_in = take(20 * nsd);
+    L.seed_rec4 = take(16 * nsd * kSeedBands); L.seed_rec2 = take(8 * nsd * kSeedBands);   // a seed is filed once per curvature band it can match
     L.seed_bin_start = take(4 * (size_t)(kSeedBins + 3));
     for (int k = 0; k < 2; ++k) L.lb_pix[k] = take(8 * (size_t)(L.n_chunk_pix[k] + 1));
     L.lb_pix_bytes = off - L.lb_pix[0];
@@ -321,6 +322,13 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
   c->P.first_slot = 0;
   c->P.dup_min_shared = cfg.t5_dup_min_shared;
   c->P.store_half = cfg.store_half != 0;
+  {  // [P]: are the modules of layers 0 and 1 a prefix of the module ids?
+    int live = 0;
+    while (live < n && g->layer[live] <= 1) ++live;
+    bool prefix = true;
+    for (int i = live; i < n; ++i) prefix = prefix && g->layer[i] > 1;
+    c->P.pix_live_modules = prefix ? live : n;
+  }
   if ((e = cudaDeviceSynchronize()) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   *out = c;
   return LST_OK;
@@ -831,6 +839,28 @@ int lst_fetch_values(lst_ctx* c, int slot, int kind, void* out, int64_t cap, voi
   void* outs[1] = {out};
   const int64_t caps[1] = {cap};
   return lst_fetch_batch(c, slot, 1, kind, nullptr, outs, caps, nullptr, 1, stream);
+}
+
+int lst_grown_config(lst_ctx* c, int slot, lst_config* out) {
+  if (!valid_slot(c, slot) || !out) return LST_ERR_ARG;
+  const SlotHost& sh = c->slots[slot];
+  if (!sh.synced) return LST_ERR_STATE;
+  *out = c->cfg;
+  auto grow = [](int32_t& cap, unsigned long long needed) {
+    if (needed <= (unsigned long long)cap) return;
+    unsigned long long want = (needed + needed / 4 + 1023) / 1024 * 1024;
+    if (want > (unsigned long long)kMaxCap) want = (unsigned long long)kMaxCap;
+    cap = (int32_t)want;
+  };
+  grow(out->cap_md, sh.hdr->needed[LST_MD]);
+  grow(out->cap_seg, sh.hdr->needed[LST_SEG]);
+  grow(out->cap_t3, sh.hdr->needed[LST_T3]);
+  grow(out->cap_t5, sh.hdr->needed[LST_T5]);
+  if (sh.pixel_run) {
+    grow(out->cap_pt3, sh.hdr->needed_pix[0]);
+    grow(out->cap_pt5, sh.hdr->needed_pix[1]);
+  }
+  return LST_OK;
 }
 
 int lst_arena_bytes(lst_ctx* c, int64_t* total, int64_t* per_slot) {

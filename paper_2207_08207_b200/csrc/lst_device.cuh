@@ -47,10 +47,11 @@ constexpr int kMaxBatch = 16;     // events per launch of the a0 kernels (pointe
 constexpr int kMaxRow = 64;       // longest module-map row accepted
 constexpr int kMaxCap = 1 << 26;  // largest per-slot capacity: object indices are packed into 26 bits
 enum { LST_MD_ = 0, LST_SEG_ = 1, LST_T3_ = 2, LST_T5_ = 3, LST_CLEAN_ = 4, LST_PIXEL_ = 5 };  // == LST_MD .. LST_PIXEL of lst.h
-// [P] pixel line segments (seeds) are binned by the azimuth of their direction at the beam line: kSeedBins uniform bins
-// over (-pi, pi], then bin kSeedBins = seeds whose (cos, sin) is not a unit vector (no azimuth window can be derived for
-// them: every object looks at them), then bin kSeedBins + 1 = seeds that no object can accept (non-finite or zero direction).
-constexpr int kSeedBins = 1024;
+// [P] pixel line segments (seeds) are binned by (curvature band, azimuth of their direction at the beam line): kSeedBands bands
+// x kSeedPhiBins uniform azimuth bins over (-pi, pi], a seed filed under every band an object within pix_dkappa_max of it can
+// sit in; then bin kSeedBins = seeds whose (cos, sin) is not a unit vector (no azimuth window can be derived for them: every
+// object looks at them), then bin kSeedBins + 1 = seeds that no object can accept (non-finite or zero direction, NaN curvature).
+constexpr int kSeedPhiBins = 512, kSeedBands = 16, kSeedBins = kSeedPhiBins * kSeedBands;
 
 struct SlotHeader {
   int n_hits;                     // valid hits binned
@@ -119,6 +120,7 @@ struct Params {
   int first_slot;
   int dup_min_shared;            // [D] D4: quintuplets sharing at least this many original hits are duplicates
   int store_half;                // [H] output floats that no selection reads are stored as binary16
+  int pix_live_modules;          // [P] modules 0 .. pix_live_modules-1 are exactly those on layers 0 and 1 (module ids ordered by layer); n_modules if they are not
 };
 
 // Typed access to one slot.

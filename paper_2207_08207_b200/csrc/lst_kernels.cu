@@ -1506,39 +1506,66 @@ __global__ void __launch_bounds__(1024) k_clean_list(const __grid_constant__ Par
 // P2 needs e^2 / var_xy[layer] <= chi2xy_max (every term of the sum is >= 0), P1 confines kappa to kappa_obj +- dkappa_max
 // and P0 confines delta to (-pi/2, pi/2): an interval of sin(delta), hence of phi0.  Every seed inside the window goes
 // through the exact selection, so the link set does not depend on the window.  Seeds whose direction is not a unit vector
-// (|n^2 - 1| > 1e-3) have no such window: they sit in a bin of their own that every object looks at.
+// (|n^2 - 1| > 1e-3) have no such window: they sit in a bin of their own that every object looks at.  The bins are
+// (curvature band, azimuth): P1 is the second window (seed_band_of below).
 // ------------------------------------------------------------------------------------------
 constexpr float kPiF = 3.14159274f;
-constexpr float kSeedBinScale = 162.974663f;   // kSeedBins / (2 pi)
-static_assert(kSeedBins == 1024, "k_seed_bin scans one azimuth bin per thread");
+constexpr float kSeedBinScale = 81.4873309f;   // kSeedPhiBins / (2 pi)
+// Curvature bands: band(kappa) = clamp(floor((kappa + 0.016) * 500), 0, kSeedBands - 1): width 0.002 per cm, the two edge bands
+// open-ended; monotone in kappa.  A seed is filed under every band from band(kappa - dkw) to band(kappa + dkw), dkw = the larger
+// pix_dkappa_max with slack, so the ONE band of an object's own curvature holds every seed P1 can accept for it.
+constexpr float kBandOffset = 0.016f, kBandScale = 500.0f;
+static_assert(kSeedPhiBins == 512 && kSeedBands == 16 && kSeedBins == 8192, "k_seed_bin scans eight bins per thread");
 
-__device__ __forceinline__ int seed_bin_of(float c, float s) {
-  // no object can accept it: a non-finite direction makes e infinite or NaN, a zero direction fails P0
-  if (!(fabsf(c) <= 3.4028235e38f) || !(fabsf(s) <= 3.4028235e38f) || (c == 0.0f && s == 0.0f)) return kSeedBins + 1;
+__device__ __forceinline__ int seed_band_of(float kappa) {
+  return (int)fminf(fmaxf(floorf((kappa + kBandOffset) * kBandScale), 0.0f), (float)(kSeedBands - 1));
+}
+__device__ __forceinline__ float seed_band_reach(const Cuts& c) {
+  const float d = fmaxf(c.pix_dkappa_max[0], c.pix_dkappa_max[1]) * 1.001f + 1e-7f;
+  return d >= 0.0f ? d : 0.0f;
+}
+// kSeedBins + 1: no object can accept the seed (a non-finite direction makes e infinite or NaN, a zero direction fails P0, a NaN
+// curvature fails P1); kSeedBins: direction not a unit vector; else the azimuth bin.
+__device__ __forceinline__ int seed_phi_bin_of(float kappa, float c, float s) {
+  if (!(fabsf(c) <= 3.4028235e38f) || !(fabsf(s) <= 3.4028235e38f) || (c == 0.0f && s == 0.0f) || kappa != kappa) return kSeedBins + 1;
   const float n2 = c * c + s * s;
   if (!(fabsf(n2 - 1.0f) <= 1e-3f)) return kSeedBins;
   const int b = (int)floorf((atan2f(s, c) + kPiF) * kSeedBinScale);
-  return min(kSeedBins - 1, max(0, b));
+  return min(kSeedPhiBins - 1, max(0, b));
 }
 
-// One block per event: histogram over the azimuth bins in shared memory, scan, scatter of the records (kappa, cos, sin, z0),
-// (t, original index).  The order inside a bin is the arrival order (it never reaches the output: links carry the original
-// seed index and are ordered by it).  Also clears the look-back words and the counters of the two link kernels.
+// One block per event: histogram over the (band, azimuth) bins in shared memory, scan, scatter of the records (kappa, cos, sin,
+// z0), (t, original index) -- once per band the seed is filed under.  The order inside a bin is the arrival order (it never
+// reaches the output: links carry the original seed index and are ordered by it).  Also clears the look-back words and the
+// counters of the two link kernels.
 __global__ void __launch_bounds__(1024) k_seed_bin(const __grid_constant__ Params P, const __grid_constant__ SeedBatch B) {
-  __shared__ int s_cnt[kSeedBins + 2], s_cur[kSeedBins + 2], s_warp[32];
+  __shared__ int s_cnt[kSeedBins + 2], s_warp[32];
   Slot S(P, blockIdx.y);
   SlotHeader* H = S.hdr();
   const SeedInput& in = B.ev[blockIdx.y];
   const int n = min(in.n, P.L.cap_seeds);
   const int tid = (int)threadIdx.x, lane = (int)lane_id();
+  const float reach = seed_band_reach(P.cuts);
   for (int i = tid; i < kSeedBins + 2; i += 1024) s_cnt[i] = 0;
   int4* lb = S.at<int4>(P.L.lb_pix[0]);
   for (int i = tid; i < (int)(P.L.lb_pix_bytes / 16); i += 1024) lb[i] = make_int4(0, 0, 0, 0);
   __syncthreads();
-  for (int i = tid; i < n; i += 1024) atomicAdd(&s_cnt[seed_bin_of(in.cphi[i], in.sphi[i])], 1);
+  for (int i = tid; i < n; i += 1024) {
+    const float k = in.kappa[i];
+    const int pb = seed_phi_bin_of(k, in.cphi[i], in.sphi[i]);
+    if (pb >= kSeedBins) {
+      atomicAdd(&s_cnt[pb], 1);
+    } else {
+      const int b1 = seed_band_of(k + reach);
+      for (int b = seed_band_of(k - reach); b <= b1; ++b) atomicAdd(&s_cnt[b * kSeedPhiBins + pb], 1);
+    }
+  }
   __syncthreads();
-  const int v = s_cnt[tid];
-  const int incl = warp_incl_scan(v);
+  // exclusive scan of the kSeedBins counters, eight per thread; the counters become the scatter cursors
+  int v[8], mine = 0;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) { v[k] = s_cnt[8 * tid + k]; mine += v[k]; }
+  const int incl = warp_incl_scan(mine);
   if (lane == 31) s_warp[tid >> 5] = incl;
   __syncthreads();
   if (tid < 32) {
@@ -1546,26 +1573,42 @@ __global__ void __launch_bounds__(1024) k_seed_bin(const __grid_constant__ Param
     s_warp[tid] = warp_incl_scan(w) - w;
   }
   __syncthreads();
-  const int ex = s_warp[tid >> 5] + incl - v;
+  int ex = s_warp[tid >> 5] + incl - mine;
   int* start = S.seed_bin_start();
-  s_cur[tid] = ex;
-  start[tid] = ex;
-  if (tid == kSeedBins - 1) {
-    const int n_binned = ex + v, n_live = n_binned + s_cnt[kSeedBins];
-    s_cur[kSeedBins] = n_binned;
-    s_cur[kSeedBins + 1] = n_live;
-    start[kSeedBins] = n_binned;
-    start[kSeedBins + 1] = n_live;
-    start[kSeedBins + 2] = n_live + s_cnt[kSeedBins + 1];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) {
+    s_cnt[8 * tid + k] = ex;
+    start[8 * tid + k] = ex;
+    ex += v[k];
+  }
+  if (tid == 1023) {
+    const int n_wild = s_cnt[kSeedBins], n_dead = s_cnt[kSeedBins + 1];
+    s_cnt[kSeedBins] = ex;
+    s_cnt[kSeedBins + 1] = ex + n_wild;
+    start[kSeedBins] = ex;
+    start[kSeedBins + 1] = ex + n_wild;
+    start[kSeedBins + 2] = ex + n_wild + n_dead;
   }
   __syncthreads();
   float4* rec4 = S.seed_rec4();
   float2* rec2 = S.seed_rec2();
   for (int i = tid; i < n; i += 1024) {
-    const float c = in.cphi[i], sn = in.sphi[i];
-    const int pos = atomicAdd(&s_cur[seed_bin_of(c, sn)], 1);
-    rec4[pos] = make_float4(in.kappa[i], c, sn, in.z0[i]);
-    rec2[pos] = make_float2(in.t[i], __int_as_float(i));
+    const float k = in.kappa[i], c = in.cphi[i], sn = in.sphi[i];
+    const float4 a = make_float4(k, c, sn, in.z0[i]);
+    const float2 b2 = make_float2(in.t[i], __int_as_float(i));
+    const int pb = seed_phi_bin_of(k, c, sn);
+    if (pb >= kSeedBins) {
+      const int pos = atomicAdd(&s_cnt[pb], 1);
+      rec4[pos] = a;
+      rec2[pos] = b2;
+    } else {
+      const int b1 = seed_band_of(k + reach);
+      for (int b = seed_band_of(k - reach); b <= b1; ++b) {
+        const int pos = atomicAdd(&s_cnt[b * kSeedPhiBins + pb], 1);
+        rec4[pos] = a;
+        rec2[pos] = b2;
+      }
+    }
   }
   if (tid == 0) {
     H->n_seeds = n;
@@ -1600,13 +1643,14 @@ __device__ __forceinline__ void pix_emit(const Params& P, const Slot& S, int pos
   f[0] = chi2xy; f[1] = chi2rz; f[2] = dk;
 }
 
-// Owner lane: `n` candidates = nMain binned seeds starting at position `first` of the bin-ordered seed list (cyclic over
-// the nBinned binned seeds: the azimuth window may straddle +-pi) followed by all seeds of the non-unit bin.
+// Owner lane: `n` candidates = n1 binned seeds starting at position `first` of the bin-ordered seed list, then nMain - n1
+// starting at `second` (the azimuth window may straddle +-pi: the tail and the head of the band), then all seeds of the
+// non-unit bin, which starts at `wild0`.
 // Two levels: P1, P0 and the first anchor's term of P2 on every candidate (one 16-byte load), survivors compacted
 // into a queue; the full selection on full tiles of survivors.
 template <int KIND, bool DIRECT>
 __device__ __forceinline__ int pix_walk(const Params& P, const Slot& S, PixWarp<(KIND ? 5 : 3)>& sh, int buf, int n, int off,
-                                        int total, int first, int nMain, int nBinned, int A0, int base) {
+                                        int total, int first, int n1, int second, int nMain, int wild0, int A0, int base) {
   constexpr int N = KIND ? 5 : 3;
   const float4* rec4 = S.seed_rec4();
   const float2* rec2 = S.seed_rec2();
@@ -1658,10 +1702,9 @@ __device__ __forceinline__ int pix_walk(const Params& P, const Slot& S, PixWarp<
     const int j = tb + lane;
     const int ol = (j < total) ? sh.tab[rk] : 0;
     const int jj = j - __shfl_sync(kFull, off, ol);
-    const int f0 = __shfl_sync(kFull, first, ol), nm = __shfl_sync(kFull, nMain, ol);
-    int idx = f0 + jj;
-    if (jj >= nm) idx = nBinned + (jj - nm);
-    else if (idx >= nBinned) idx -= nBinned;
+    const int f0 = __shfl_sync(kFull, first, ol), m1 = __shfl_sync(kFull, n1, ol);
+    const int f1 = __shfl_sync(kFull, second, ol), nm = __shfl_sync(kFull, nMain, ol);
+    const int idx = jj < m1 ? f0 + jj : jj < nm ? f1 + (jj - m1) : wild0 + (jj - nm);
     bool keep = false;
     if (j < total) {
       const float4 a = rec4[idx];                     // kappa, cos, sin, z0
@@ -1688,13 +1731,19 @@ __global__ void __launch_bounds__(kPixWarps * 32, 6) k_pix(const __grid_constant
   Slot S(P, blockIdx.y);
   SlotHeader* H = S.hdr();
   const int cap = P.L.cap_pix[KIND];
-  const int nObj = H->n[KIND ? LST_T5_ : LST_T3_];
+  const int nAll = H->n[KIND ? LST_T5_ : LST_T3_];
+  // Triplets are numbered by first segment, segments by inner MD, MDs by module: when the module ids are ordered by layer
+  // (P.pix_live_modules = number of leading modules on layers 0 and 1) the triplets that can be linked are a prefix of the
+  // triplet list, found through the CSR offsets; only they are walked, the rest just get their (empty) CSR entry.
+  int nObj = nAll;
+  if (!KIND && P.pix_live_modules < P.L.n_modules && !H->overflow)
+    nObj = min(nAll, S.t3_start()[S.seg_start()[S.md_start()[P.pix_live_modules]]]);
   const int nChunks = (nObj + kChunk - 1) / kChunk;
   const int nSeeds = H->n_seeds;
   const int lane = (int)lane_id();
   PixWarp<N>& sh = shw[threadIdx.x >> 5];
   const int* bs = S.seed_bin_start();
-  const int nBinned = bs[kSeedBins], nWild = bs[kSeedBins + 1] - nBinned;
+  const int wild0 = bs[kSeedBins], nWild = bs[kSeedBins + 1] - wild0;
   int* pix_start = S.pix_start(KIND);
   unsigned long long* status = S.lb_pix(KIND);
   unsigned long long cand = 0, evals = 0;
@@ -1747,9 +1796,10 @@ __global__ void __launch_bounds__(kPixWarps * 32, 6) k_pix(const __grid_constant
       }
     }
     if (A < nObj) pix_start[A] = min(base + ex, cap);
-    if (A == nObj - 1) {
-      pix_start[nObj] = min(base + total, cap);
-      publish(base + total);
+    if (A0 + 31 >= nObj - 1) {      // the last chunk: the end of the CSR array, for the objects not walked too
+      const int end = min(base + total, cap);
+      for (int i = nObj + lane; i <= nAll; i += 32) pix_start[i] = end;
+      if (A == nObj - 1) publish(base + total);
     }
     __syncwarp();
   };
@@ -1758,14 +1808,14 @@ __global__ void __launch_bounds__(kPixWarps * 32, 6) k_pix(const __grid_constant
   for (;;) {
     const int C = warp_ticket(&H->ticket_pix[KIND]);
     if (C >= nChunks) {
-      if (C == 0 && lane == 0) {
-        publish(0);
-        pix_start[0] = 0;
+      if (C == 0) {
+        for (int i = lane; i <= nAll; i += 32) pix_start[i] = 0;
+        if (lane == 0) publish(0);
       }
       break;
     }
     const int A0 = C * kChunk, A = A0 + lane;
-    int n = 0, first = 0, nMain = 0;
+    int n = 0, first = 0, n1 = 0, second = 0, nMain = 0;
     if (A < nObj) {
       int md[N];
       float kobj;
@@ -1800,17 +1850,28 @@ __global__ void __launch_bounds__(kPixWarps * 32, 6) k_pix(const __grid_constant
             const float phip = atan2f(p0.y, p0.x);
             const float lo = phip + asinf(fmaxf(a, -1.0f)) - 1e-4f, hi = phip + asinf(fminf(b, 1.0f)) + 1e-4f;
             int blo = (int)floorf((lo + kPiF) * kSeedBinScale) - 1, bhi = (int)floorf((hi + kPiF) * kSeedBinScale) + 1;
-            if (bhi - blo + 1 >= kSeedBins) {
+            if (bhi - blo + 1 >= kSeedPhiBins) {
               whole = true;
             } else {
-              blo = ((blo % kSeedBins) + kSeedBins) % kSeedBins;
-              bhi = ((bhi % kSeedBins) + kSeedBins) % kSeedBins;
-              first = bs[blo];
-              nMain = (blo <= bhi) ? bs[bhi + 1] - first : (nBinned - first) + bs[bhi + 1];
+              const int* band = bs + seed_band_of(kobj) * kSeedPhiBins;
+              blo = ((blo % kSeedPhiBins) + kSeedPhiBins) % kSeedPhiBins;
+              bhi = ((bhi % kSeedPhiBins) + kSeedPhiBins) % kSeedPhiBins;
+              first = band[blo];
+              if (blo <= bhi) {
+                n1 = nMain = band[bhi + 1] - first;
+              } else {
+                n1 = band[kSeedPhiBins] - first;
+                second = band[0];
+                nMain = n1 + (band[bhi + 1] - second);
+              }
             }
           }
         }
-        if (whole) { first = 0; nMain = nBinned; }
+        if (whole) {
+          const int* band = bs + seed_band_of(kobj) * kSeedPhiBins;
+          first = band[0];
+          n1 = nMain = band[kSeedPhiBins] - first;
+        }
         n = nMain + nWild;
       }
     }
@@ -1819,7 +1880,7 @@ __global__ void __launch_bounds__(kPixWarps * 32, 6) k_pix(const __grid_constant
     int total_c;
     const int off = warp_excl_scan(n, total_c);
     build_owner_table(n, sh.tab);
-    const int total = pix_walk<KIND, false>(P, S, sh, buf, n, off, total_c, first, nMain, nBinned, A0, 0);
+    const int total = pix_walk<KIND, false>(P, S, sh, buf, n, off, total_c, first, n1, second, nMain, wild0, A0, 0);
     publish_aggregate(status, C, total);
     __syncwarp();
     if (pC >= 0) {
@@ -1831,7 +1892,7 @@ __global__ void __launch_bounds__(kPixWarps * 32, 6) k_pix(const __grid_constant
     } else {
       if (lane == 0) atomicAdd(&H->rewalk_pix[KIND], 1ull);
       const int base = resolve_base(status, C, total);
-      pix_walk<KIND, true>(P, S, sh, buf, n, off, total_c, first, nMain, nBinned, A0, base);
+      pix_walk<KIND, true>(P, S, sh, buf, n, off, total_c, first, n1, second, nMain, wild0, A0, base);
       finish(C, buf, total, base, false);
     }
   }

@@ -160,6 +160,7 @@ SYMBOLS = {
     "lst_default_map_params": (C.c_int, [P(MapParams)]),
     "lst_build_module_map": (C.c_int, [P(MapGeometry), P(MapParams), C.c_int, C.c_void_p, C.c_void_p, C.c_int64, P(C.c_int64),
                                        P(C.c_float)]),
+    "lst_grown_config": (C.c_int, [C.c_void_p, C.c_int, P(Config)]),
     "lst_arena_bytes": (C.c_int, [C.c_void_p, P(C.c_int64), P(C.c_int64)]),
     "lst_launch_count": (C.c_int64, [C.c_void_p]),
     "lst_last_cuda_error": (C.c_int, [C.c_void_p]),
@@ -491,6 +492,12 @@ class Lst:
         self._check(self.lib.lst_fetch_values(self.h, slot, kind, _ptr(out), out.shape[0], _stream(stream)),
                     "lst_fetch_values")
         return out[:n]
+
+    def grown_config(self, slot: int) -> Config:
+        """After an overflow: this context's configuration with the exceeded capacities raised to what the slot needed x 1.25."""
+        cfg = Config()
+        self._check(self.lib.lst_grown_config(self.h, slot, C.byref(cfg)), "lst_grown_config")
+        return cfg
 
     def arena_bytes(self):
         t, p = C.c_int64(), C.c_int64()

@@ -190,6 +190,37 @@ def test_overflow_and_bad_input_are_reported(lstmod, geom, mmap, o32, run_oracle
     c.close()
 
 
+def test_overflow_recovery_by_regrowing(lstmod, geom, mmap, o32, run_oracle):
+    """BASELINE.json configs[3] "candidate-buffer overflow handling", the recovery half: start from capacities far too small
+    for the PU300-like stress event, follow lst_grown_config until the event fits (a stage that overflowed hands the next one
+    a clamped input, so it can take one round per object class), and the result equals the oracle's."""
+    ev = synth.generate_event(geom, 3, 0)
+    cfg = lstmod.default_config()
+    cfg.n_slots = 1
+    cfg.cap_hits, cfg.cap_md, cfg.cap_seg, cfg.cap_t3, cfg.cap_t5 = 160 * 1024, 8 * 1024, 8 * 1024, 8 * 1024, 1024
+    rounds = 0
+    while True:
+        c = lstmod.Lst.from_synth(geom, mmap, cfg)
+        c.load_event(0, ev.x, ev.y, ev.z, ev.module, ev.side)
+        c.run(0)
+        status = c.sync(0, check=False)
+        if status == lstmod.OK:
+            break
+        assert status == lstmod.ERR_OVERFLOW and rounds < 5
+        new = c.grown_config(0)
+        assert any(getattr(new, f) > getattr(cfg, f) for f in ("cap_md", "cap_seg", "cap_t3", "cap_t5"))
+        assert all(getattr(new, f) >= getattr(cfg, f) for f in ("cap_hits", "cap_md", "cap_seg", "cap_t3", "cap_t5"))
+        c.close()
+        cfg = new
+        rounds += 1
+    assert 1 <= rounds <= 4
+    ora = run_oracle(o32, ev)
+    parity.compare(parity.gpu_tables(c, 0), parity.oracle_tables(ora), "regrown")
+    same = c.grown_config(0)
+    assert [getattr(same, f) for f in ("cap_md", "cap_seg", "cap_t3", "cap_t5")] == [getattr(cfg, f) for f in ("cap_md", "cap_seg", "cap_t3", "cap_t5")]
+    c.close()
+
+
 def test_multi_stream_pipeline(ctx, o32, run_oracle, geom):
     """BASELINE.json configs[2] in miniature: 8 events on 4 streams, slots recycled, arena reused."""
     import torch

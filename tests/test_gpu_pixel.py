@@ -281,3 +281,92 @@ def test_pixel_in_the_bench_launch_configuration(lstmod, geom, mmap, o32, run_or
         ora = run_oracle(o32, evs[i], seeds=sds[i].arrays())
         compare_links(c, lstmod, ora, slot=i, label=f"batch event {i}")
     c.close()
+
+
+def test_pixel_seeds_on_the_window_edges(lstmod, geom, mmap, o32):
+    """Seeds constructed to sit on the edges of the search windows of real triplets: curvature at kappa_obj +- pix_dkappa_max
+    (1 -+ 1e-6) (the P1 boundary and the curvature bands) and direction such that the first anchor's P2 term is at
+    +- its largest admissible value (1 -+ 1e-5) (the azimuth window).  With the x-y weights of all layers but the first
+    made negligible and the r-z cut opened, pass / fail flips right there, so a window that were too tight by a few ulps would
+    lose links the oracle's full product finds.  Objects starting on layer 1 then have no azimuth window at all (weight ~ 0)."""
+    ev = synth.generate_event(geom, 1, 41, n_particles=600)
+    base = o32.run(geom.layer, mmap.row_offsets, mmap.targets, ev.x, ev.y, ev.z, ev.module, ev.side)
+    t3m = base.t3_mds()
+    lay = geom.layer[base.md_module][t3m[:, 0]]
+    pick = np.nonzero(lay == 0)[0][::3][:400]
+    w0, chi_max, dk_max = 809.479, 85.0, 0.0008
+    E = np.sqrt(chi_max / w0)
+    K, C_, S_, Z0, T = [], [], [], [], []
+    for j in pick:
+        m = t3m[j, 0]
+        x, y, r = float(base.md_x[m]), float(base.md_y[m]), float(base.md_r[m])
+        kobj, phip = float(base.t3_kappa[j]), np.arctan2(y, x)
+        for sk in (-1.0, 1.0):
+            for dkr in (-1e-6, 0.0, 1e-6):
+                kap = np.float32(kobj + sk * dk_max * (1.0 + dkr))
+                for se in (-1.0, 1.0):
+                    for der in (-1e-5, 0.0, 1e-5):
+                        arg = (se * E * (1.0 + der) - 0.5 * float(kap) * r * r) / r
+                        if abs(arg) >= 1.0:
+                            continue
+                        phi0 = phip + np.arcsin(arg)
+                        K.append(kap); C_.append(np.cos(phi0)); S_.append(np.sin(phi0)); Z0.append(0.0); T.append(0.0)
+    seeds = tuple(np.asarray(a, np.float32) for a in (K, C_, S_, Z0, T))
+    assert 2500 < len(seeds[0]) <= 16384
+    cfg = lstmod.default_config()
+    cfg.n_slots = 1
+    cfg.cap_pt3 = cfg.cap_pt5 = 1 << 20
+    ocfg = o32.default_config()
+    for c in (cfg, ocfg):
+        for l in range(1, 6):
+            c.pix_inv_var_xy[l] = 1e-9
+        for k in range(2):
+            c.pix_chi2rz_max[k] = 1e30
+            c.pix_chi2xy_max[k] = chi_max
+            c.pix_dkappa_max[k] = dk_max
+    c = lstmod.Lst.from_synth(geom, mmap, cfg)
+    run_pixel(c, lstmod, ev, seeds)
+    ora = o32.run(geom.layer, mmap.row_offsets, mmap.targets, ev.x, ev.y, ev.z, ev.module, ev.side, cfg=ocfg, seeds=seeds)
+    compare_links(c, lstmod, ora, label="edge seeds")
+    # both outcomes occur at the edges, in numbers: the construction does sit on the boundary
+    own = ora.pix[0]["n"]
+    assert 0.2 * len(seeds[0]) < own, own
+    c.close()
+
+
+def test_module_ids_in_any_order(lstmod, geom, mmap, o32):
+    """The library assumes nothing about how module ids are numbered: the same detector with its module ids randomly
+    permuted (geometry tables, module map rows and targets, the hits' module column) gives the oracle's sets for that
+    numbering -- objects and pixel links.  (With ids ordered by layer, as in the BASELINE geometry, the pixel-triplet kernel
+    walks only the leading triplets; here it cannot.)"""
+    rng = np.random.default_rng(11)
+    n = geom.n_modules
+    perm = rng.permutation(n).astype(np.int32)          # old id -> new id
+    inv = np.argsort(perm)
+    layer, phi = geom.layer[inv], geom.phi[inv]
+    rows = [np.sort(perm[mmap.targets[mmap.row_offsets[a]:mmap.row_offsets[a + 1]]]) for a in inv]
+    offs = np.zeros(n + 1, np.int32)
+    offs[1:] = np.cumsum([len(r) for r in rows])
+    targets = np.concatenate(rows).astype(np.int32)
+    ev = synth.generate_event(geom, 1, 77, n_particles=1500)
+    sd = synth.generate_seeds(ev, 77)
+    module = perm[ev.module]
+    cfg = lstmod.default_config()
+    cfg.n_slots = 1
+    c = lstmod.Lst(layer, offs, targets, cfg, phi=phi)
+    c.load_event(0, ev.x, ev.y, ev.z, module, ev.side)
+    c.load_seeds(0, [sd.arrays()])
+    c.run(0)
+    c.run_stage(0, 1, lstmod.PIXEL)
+    c.run_stage(0, 1, lstmod.CLEAN)
+    c.sync(0)
+    ora = o32.run(layer, offs, targets, ev.x, ev.y, ev.z, module, ev.side, seeds=sd.arrays())
+    parity.compare(parity.gpu_tables(c, 0), parity.oracle_tables(ora), "permuted ids")
+    compare_links(c, lstmod, ora, label="permuted ids")
+    keep = o32.t5_clean(ora.t5_hits(), ora.t5_chi2xy, ora.t5_chi2rz)
+    got = c.fetch_hit_indices(0, lstmod.T5)[c.fetch_kept(0)]
+    assert set(map(tuple, got.tolist())) == set(map(tuple, ora.t5_hits()[keep.astype(bool)].tolist()))
+    # the same objects as with the original numbering (identity is by hit index)
+    ref = o32.run(geom.layer, mmap.row_offsets, mmap.targets, ev.x, ev.y, ev.z, ev.module, ev.side)
+    assert set(map(tuple, ref.t5_hits().tolist())) == set(map(tuple, ora.t5_hits().tolist()))
+    c.close()
