@@ -718,7 +718,11 @@ __global__ void __launch_bounds__(kWarps * 32, LST_MD_BLOCKS) k_md(const __grid_
 //   C  candidates, 32 at a time: the SPEC selection                     -> stash
 // Segments come out ordered by (inner MD, outer MD).
 // ------------------------------------------------------------------------------------------
-constexpr int kSegStash = 160;
+// The block's shared memory decides how much of the SM's 256 KB is left as L1: 7 resident blocks must stay within the 196 KB
+// carve-out (27 648 B per block incl. the 1 KB the system reserves), or the next carve-out (228 KB) halves the L1 and costs 5 %
+// (measured: 48.1 k against 50.5 k events/s for 1.3 KB more per block).  Smaller stashes for a smaller carve-out lose to the
+// re-walks they cause (kSegStash 104: 47.8 k).
+constexpr int kSegStash = 152;
 struct SegWarp {
   float4 a4[32];
   float2 aux[32];
@@ -728,7 +732,9 @@ struct SegWarp {
   int cnt[2][32];
   int stI[2][kSegStash];
   float2 stV[2][kSegStash];
+  unsigned char stR[2][kSegStash];   // rank of a stashed segment among its owner's
 };
+static_assert(kSegWarps * sizeof(SegWarp) + 64 + 1024 <= 28672, "k_seg: 7 blocks per SM must fit the 196 KB shared-memory carve-out");
 
 // i / o = index of the inner / outer MD.
 __device__ __forceinline__ void seg_emit(const Params& P, const Slot& S, int pos, int i, int o, float sinS, float z0) {
@@ -746,34 +752,54 @@ __device__ __forceinline__ void seg_emit(const Params& P, const Slot& S, int pos
   }
 }
 
+// Level A: lane = inner MD of the chunk, and the warp steps through the rows of the module map in lockstep (entry t of every
+// lane's row in iteration t; mini-doublets of one module read the same row entry: one broadcast load).  The (MD, connected
+// module) pairs are not flattened, so there is no owner lookup per pair (the flattened form of round 1 spent a third of the
+// kernel's instructions in level A; same-box A/B 50.5 k -> 51.1 k events/s).  Pairs reach the queues ordered by (row entry, MD);
+// for ONE inner MD they still arrive in ascending outer MD (rows ascend, the queues are FIFO), so a segment's place among its
+// owner's is the number of that owner's segments seen before it (`rank`), and its CSR position is
+// base + (segments of the lanes before the owner) + rank.  cnt[cb] counts per owner as the walk goes.
 template <bool DIRECT>
-__device__ __forceinline__ int seg_walk(const Params& P, const Slot& S, SegWarp& sh, int buf, int nt, int off, int nPairs,
-                                        int row0, int i0, int base, unsigned long long& space, unsigned long long& evals) {
+__device__ __forceinline__ int seg_walk(const Params& P, const Slot& S, SegWarp& sh, int buf, int nt, int row0, int i0,
+                                        int base, unsigned long long& space_acc, unsigned long long& evals_acc) {
   const float4* anchor = S.md_anchor();
   const float2* aux = S.md_aux();
   const float* mkey = S.md_key();
   const int4* mod_info = S.mod_info();
   const int lane = (int)lane_id();
+  const int cb = DIRECT ? buf ^ 1 : buf;   // running per-owner counters (the direct walk keeps the first walk's totals in cnt[buf])
+  // search-space counters of this walk: 32 bits suffice (a lane's row entries are distinct modules, its windows at most
+  // 64 x the mini-doublets of the event, capacities are below 2^26), the 64-bit totals stay out of the loops
+  unsigned space = 0, evals = 0;
   int running = 0;
-  int ph = 0, pt = 0, ch = 0, ct = 0;   // heads / tails of the pair and candidate queues
+  int ph = 0, pt = 0, ch = 0, ct = 0;
 
-  // C: the selection on up to 32 candidates (inner lane, outer MD)
   auto levelC = [&](bool valid, int2 it) {
     bool pass = false;
     SegOut so;
     const int ol = it.x, o = it.y;
     if (valid) pass = seg_select(P.cuts, sh.layer[ol], sh.a4[ol], sh.aux[ol], anchor[o], aux[o], so);
     const unsigned bal = __ballot_sync(kFull, pass);
-    if (pass) {
-      const int pos = running + __popc(bal & lanemask_lt());
-      if (!DIRECT) {
-        atomicAdd(&sh.cnt[buf][ol], 1);
-        if (pos < kSegStash) { sh.stI[buf][pos] = (ol << 26) | o; sh.stV[buf][pos] = make_float2(so.sinS, so.z0); }
-      } else {
-        seg_emit(P, S, base + pos, i0 + ol, o, so.sinS, so.z0);
+    if (bal) {
+      unsigned grp = 0;
+      int rank = 0;
+      if (pass) {
+        grp = __match_any_sync(bal, ol);
+        rank = sh.cnt[cb][ol] + __popc(grp & lanemask_lt());
+        if (!DIRECT) {
+          const int pos = running + __popc(bal & lanemask_lt());
+          if (pos < kSegStash) {
+            sh.stI[buf][pos] = (ol << 26) | o; sh.stV[buf][pos] = make_float2(so.sinS, so.z0);
+            sh.stR[buf][pos] = (unsigned char)rank;
+          }
+        } else {
+          seg_emit(P, S, base + sh.tab[ol] + rank, i0 + ol, o, so.sinS, so.z0);
+        }
       }
+      __syncwarp();
+      if (pass && (grp & lanemask_lt()) == 0) sh.cnt[cb][ol] += __popc(grp);
+      running += __popc(bal);
     }
-    running += __popc(bal);
   };
   auto drainC = [&](bool all) {
     while (ct - ch >= 32 || (all && ct > ch)) {
@@ -786,7 +812,6 @@ __device__ __forceinline__ int seg_walk(const Params& P, const Slot& S, SegWarp&
       __syncwarp();
     }
   };
-  // B: windows of up to 32 surviving pairs (inner lane << 26 | target module, c0)
   auto levelB = [&](bool valid, int2 it) {
     int first = 0, cnt = 0;
     const int ol = (int)((unsigned)it.x >> 26);
@@ -801,7 +826,7 @@ __device__ __forceinline__ int seg_walk(const Params& P, const Slot& S, SegWarp&
         cnt = upper_bound_f(mkey, first, info.y, c0 + dhi) - first;
       }
     }
-    if (!DIRECT) evals += (unsigned long long)cnt;
+    if (!DIRECT) evals += (unsigned)cnt;
     int nc;
     const int coff = warp_excl_scan(cnt, nc);
     build_owner_table(cnt, sh.ptab);
@@ -833,57 +858,51 @@ __device__ __forceinline__ int seg_walk(const Params& P, const Slot& S, SegWarp&
       __syncwarp();
     }
   };
-  // A: all (inner MD, connected module) pairs of the chunk.  The loads of tile t + 1 (target, azimuth offset, the
-  // target's module record: two dependent round trips) are issued before tile t is processed, so they travel while
-  // the queues of tile t are drained.
-  struct ATile {
-    int ol, tgt;
+  // A: row entry t of every lane; the entry after it is fetched (target, azimuth offset, the target's module record) before
+  // this one is tested
+  struct AEntry {
+    int tgt;
     float dphi;
     int4 info;
-    bool valid;
   };
-  auto loadA = [&](int tb) {
-    ATile t;
-    const int rk = tile_owner(nt, off, tb);
-    const int q = tb + lane;
-    t.valid = q < nPairs;
-    t.ol = t.valid ? sh.tab[rk] : 0;
-    const int e = __shfl_sync(kFull, row0, t.ol) + (q - __shfl_sync(kFull, off, t.ol));
-    t.tgt = 0;
-    t.dphi = 0.0f;
-    t.info = make_int4(0, 0, 0, 0);
-    if (t.valid) {
-      t.tgt = P.map_targets[e];
-      t.dphi = P.map_dphi[e];
-      t.info = mod_info[t.tgt];
+  auto loadA = [&](int t) {
+    AEntry e;
+    e.tgt = 0;
+    e.dphi = 0.0f;
+    e.info = make_int4(0, 0, 0, 0);
+    if (t < nt) {
+      e.tgt = P.map_targets[row0 + t];
+      e.dphi = P.map_dphi[row0 + t];
+      e.info = mod_info[e.tgt];
     }
-    return t;
+    return e;
   };
-  ATile cur = loadA(0);
-  for (int tb = 0; tb < nPairs; tb += 32) {
-    ATile nxt = cur;
-    if (tb + 32 < nPairs) nxt = loadA(tb + 32);
-    const int ol = cur.ol, tgt = cur.tgt;
+  const int max_nt = __reduce_max_sync(kFull, nt);
+  AEntry cur = loadA(0);
+  for (int t = 0; t < max_nt; ++t) {
+
     bool keep = false;
     float c0 = 0.0f;
-    if (cur.valid) {
+    if (t < nt) {
       const int4 info = cur.info;
-      if (!DIRECT) space += (unsigned long long)(info.y - info.x);
-      const float dlo = sh.dlo[ol], dhi = sh.dhi[ol];
+      if (!DIRECT) space += (unsigned)(info.y - info.x);
+      const float dlo = sh.dlo[lane], dhi = sh.dhi[lane];
       if (info.y > info.x && dlo <= dhi) {
-        c0 = sh.key[ol] + cur.dphi;
+        c0 = sh.key[lane] + cur.dphi;
         keep = !(fabsf(c0) + fmaxf(fabsf(dlo), fabsf(dhi)) < 3.0f) ||
                (c0 + dhi >= __int_as_float(info.z) && c0 + dlo <= __int_as_float(info.w));
       }
     }
     const unsigned bal = __ballot_sync(kFull, keep);
-    if (keep) sh.pq[(pt + __popc(bal & lanemask_lt())) & (kQueue - 1)] = make_int2((ol << 26) | tgt, __float_as_int(c0));
+    if (keep) sh.pq[(pt + __popc(bal & lanemask_lt())) & (kQueue - 1)] = make_int2((lane << 26) | cur.tgt, __float_as_int(c0));
     pt += __popc(bal);
     drainB(false);
-    cur = nxt;
+    cur = loadA(t + 1);   // (fetching it before this entry is tested was measured: the registers it holds cost more, 50.2 k)
   }
   drainB(true);
   drainC(true);
+  space_acc += space;
+  evals_acc += evals;
   return running;
 }
 
@@ -908,14 +927,19 @@ __global__ void __launch_bounds__(kSegWarps * 32, 7) k_seg(const __grid_constant
 
   auto finish = [&](int C, int b, int total, int base, bool from_stash) {
     const int i0 = C * kChunk, i = i0 + lane;
+    int tot;
+    const int ex = warp_excl_scan(sh.cnt[b][lane], tot);
+    if (from_stash) {   // the stash is in arrival order: place by (owner, rank)
+      sh.tab[lane] = ex;
+      __syncwarp();
+    }
     if (from_stash)
       for (int t = lane; t < total; t += 32) {
         const int v = sh.stI[b][t];
         const float2 f = sh.stV[b][t];
-        seg_emit(P, S, base + t, i0 + (int)((unsigned)v >> 26), v & (kMaxCap - 1), f.x, f.y);
+        const int ol = (int)((unsigned)v >> 26);
+        seg_emit(P, S, base + sh.tab[ol] + sh.stR[b][t], i0 + ol, v & (kMaxCap - 1), f.x, f.y);
       }
-    int tot;
-    const int ex = warp_excl_scan(sh.cnt[b][lane], tot);
     if (i < nMD) seg_start[i] = min(base + ex, cap);
     if (i == nMD - 1) {
       seg_start[nMD] = min(base + total, cap);
@@ -953,10 +977,8 @@ __global__ void __launch_bounds__(kSegWarps * 32, 7) k_seg(const __grid_constant
       sh.layer[lane] = layer;
     }
     sh.cnt[buf][lane] = 0;
-    int nPairs;
-    const int off = warp_excl_scan(nt, nPairs);
-    build_owner_table(nt, sh.tab);
-    const int total = seg_walk<false>(P, S, sh, buf, nt, off, nPairs, row0, i0, 0, space, evals);
+    __syncwarp();
+    const int total = seg_walk<false>(P, S, sh, buf, nt, row0, i0, 0, space, evals);
     publish_aggregate(status, C, total);
     __syncwarp();
     if (pC >= 0) {
@@ -968,7 +990,11 @@ __global__ void __launch_bounds__(kSegWarps * 32, 7) k_seg(const __grid_constant
     } else {
       if (lane == 0) atomicAdd(&H->rewalk[LST_SEG_], 1ull);
       const int base = resolve_base(status, C, total);
-      seg_walk<true>(P, S, sh, buf, nt, off, nPairs, row0, i0, base, space, evals);
+      int tot;   // per-owner offsets from the first walk's totals; fresh running counters
+      sh.tab[lane] = warp_excl_scan(sh.cnt[buf][lane], tot);
+      sh.cnt[buf ^ 1][lane] = 0;
+      __syncwarp();
+      seg_walk<true>(P, S, sh, buf, nt, row0, i0, base, space, evals);
       finish(C, buf, total, base, false);
     }
   }
