@@ -2041,6 +2041,10 @@ __global__ void __launch_bounds__(256) k_fetch_direct(const __grid_constant__ Pa
 // fills 148 SMs: ticket order and the ordered output bound it) and one stream's tail is filled by the other's body
 // (measured: 44.0k -> 47.4k events/s on the 4 x 16 workload; a third or a quarter is no better).
 constexpr int kGridShare = 2;
+// Blocks per SM the grids are sized for (before the halving), from same-box sweeps in the 4-stream configuration; not the
+// launch bounds (those set the register budget).  Segment kernel 4 / 5 / 6 / 7 / 8: 46.0 / 50.0 / 51.2 / 47.8 / 49.0 k events/s;
+// the others are flat within 1 % (MD 5, T3 5, T5 6 together: 51.2 -> 51.6 k).
+constexpr int kMdGrid = 5, kSegGrid = 6, kT3Grid = 5, kT5Grid = 6;
 static int blocks_per_event(int wanted, int n_batch, int resident_per_sm, int share = 1) {
   const int per_event = max(8, 148 * resident_per_sm / (n_batch * share));
   return max(1, min(wanted, per_event));
@@ -2080,17 +2084,17 @@ int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEv
   LST_EV(0);
   switch (stage) {
     case LST_MD_:
-      k_md<<<dim3(blocks_per_event((P.L.n_chunk[0] + kWarps - 1) / kWarps, n_batch, LST_MD_BLOCKS, kGridShare), nb), kWarps * 32, 0, s>>>(P);
+      k_md<<<dim3(blocks_per_event((P.L.n_chunk[0] + kWarps - 1) / kWarps, n_batch, kMdGrid, kGridShare), nb), kWarps * 32, 0, s>>>(P);
       break;
     case LST_SEG_:
       // (a module-owner walk with a flat on-chip key-window compare was built and measured in round 2: it lost, profiles/r2_seg_ab.md)
-      k_seg<<<dim3(blocks_per_event((P.L.n_chunk[1] + kSegWarps - 1) / kSegWarps, n_batch, 6, kGridShare), nb), kSegWarps * 32, 0, s>>>(P);
+      k_seg<<<dim3(blocks_per_event((P.L.n_chunk[1] + kSegWarps - 1) / kSegWarps, n_batch, kSegGrid, kGridShare), nb), kSegWarps * 32, 0, s>>>(P);
       break;
     case LST_T3_:
-      k_t3<<<dim3(blocks_per_event((P.L.n_chunk[2] + kWarps - 1) / kWarps, n_batch, 6, kGridShare), nb), kWarps * 32, 0, s>>>(P);
+      k_t3<<<dim3(blocks_per_event((P.L.n_chunk[2] + kWarps - 1) / kWarps, n_batch, kT3Grid, kGridShare), nb), kWarps * 32, 0, s>>>(P);
       break;
     case LST_T5_:
-      k_t5<<<dim3(blocks_per_event((P.L.n_chunk[3] + kWarps - 1) / kWarps, n_batch, LST_T5_BLOCKS, kGridShare), nb), kWarps * 32, 0, s>>>(P);
+      k_t5<<<dim3(blocks_per_event((P.L.n_chunk[3] + kWarps - 1) / kWarps, n_batch, kT5Grid, kGridShare), nb), kWarps * 32, 0, s>>>(P);
       break;
     default:
       return 0;
