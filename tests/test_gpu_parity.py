@@ -708,9 +708,9 @@ def test_module_map_builder_parity(lstmod, geom, mmap, o64):
 @pytest.mark.timeout(300)
 def test_soak_mixed_sizes_repeatable(lstmod, geom, mmap, o32, run_oracle):
     """400 back-to-back steps of 16 slots on 4 streams with events of very different sizes in one batch (tiny, PU200-like,
-    PU300-like, empty), the cleaning stage every third step: no hang of the ordered-output waits, identical counts at
-    every check, and the last state still equals the oracle.  (A two-minute run of the same loop, 77 k steps / 4.9 M
-    events, is recorded in DESIGN.md.)"""
+    PU300-like, empty), the cleaning stage every third step and the pixel stage every other step: no hang of the
+    ordered-output waits, identical counts at every check, and the last state still equals the oracle.  (A two-minute run of
+    the round-1 loop, 77 k steps / 4.9 M events, is recorded in DESIGN.md.)"""
     import torch
     evs = [synth.generate_event(geom, 1, 300 + i, n_particles=n) for i, n in enumerate((30, 6000, 0, 900, 2500, 1, 400, 5000))]
     evs += [synth.generate_event(geom, 3, 2), synth.generate_event(geom, 0, 5)] + [synth.generate_event(geom, 1, 310 + i, n_particles=1500) for i in range(6)]
@@ -719,23 +719,31 @@ def test_soak_mixed_sizes_repeatable(lstmod, geom, mmap, o32, run_oracle):
     c = lstmod.Lst.from_synth(geom, mmap, cfg)
     streams = [torch.cuda.Stream() for _ in range(4)]
     d_in = [[torch.from_numpy(a).cuda() for a in (e.x, e.y, e.z, e.module, e.side)] for e in evs]
+    sds = [synth.generate_seeds(e, 300 + i) for i, e in enumerate(evs)]
+    d_sd = [[torch.from_numpy(a).cuda() for a in sd.arrays()] for sd in sds]
     ref = None
     for step in range(400):
         for s, st in enumerate(streams):
             c.load_events(4 * s, d_in[4 * s:4 * s + 4], stream=st)
+            if step % 2 == 1:
+                c.load_seeds(4 * s, d_sd[4 * s:4 * s + 4], stream=st)
             c.run_batch(4 * s, 4, st)
             if step % 3 == 0:
                 c.run_stage(4 * s, 4, lstmod.CLEAN, st)
+            if step % 2 == 1:
+                c.run_stage(4 * s, 4, lstmod.PIXEL, st)
         if step % 100 == 99:
             for s, st in enumerate(streams):
                 assert c.sync_batch(4 * s, 4, st) == 0
-            cur = [tuple(c.stats(k)["needed"]) for k in range(16)]
+            cur = [tuple(c.stats(k)["needed"]) + tuple(c.stats(k)["pix_needed"]) for k in range(16)]
             ref = ref or cur
             assert cur == ref
     for k in (1, 8, 9):
         ora = run_oracle(o32, evs[k])
-        assert list(ref[k]) == ora.counts
+        assert list(ref[k][:4]) == ora.counts
         parity.compare(parity.gpu_tables(c, k, streams[k // 4]), parity.oracle_tables(ora), f"soak slot {k}")
+    ora = run_oracle(o32, evs[4], seeds=sds[4].arrays())
+    assert list(ref[4][4:]) == [ora.pix[0]["n"], ora.pix[1]["n"]] and ora.pix[0]["n"] > 1000
     c.close()
 
 
