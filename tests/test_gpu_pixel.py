@@ -370,3 +370,42 @@ def test_module_ids_in_any_order(lstmod, geom, mmap, o32):
     ref = o32.run(geom.layer, mmap.row_offsets, mmap.targets, ev.x, ev.y, ev.z, ev.module, ev.side)
     assert set(map(tuple, ref.t5_hits().tolist())) == set(map(tuple, ora.t5_hits().tolist()))
     c.close()
+
+
+def test_pixel_stage_in_a_cuda_graph(ctx, lstmod, o32, run_oracle, geom):
+    """lst_load_seeds (device input) and LST_PIXEL only enqueue work: the whole sequence load hits -> load seeds -> a1..a4 ->
+    LST_CLEAN -> LST_PIXEL is captured once over fixed device buffers and replayed with other contents."""
+    import torch
+    evs = [synth.generate_event(geom, 1, 190 + i, n_particles=1200) for i in range(2)]
+    sds = [synth.generate_seeds(e, 190 + i) for i, e in enumerate(evs)]
+    n, ns = min(e.n for e in evs), min(s.n for s in sds)
+    hb = [torch.zeros(n, dtype=dt, device="cuda") for dt in (torch.float32, torch.float32, torch.float32, torch.int32, torch.uint8)]
+    sb = [torch.zeros(ns, dtype=torch.float32, device="cuda") for _ in range(5)]
+    st = torch.cuda.Stream()
+
+    def fill(ev, sd):
+        for b, a in zip(hb, (ev.x, ev.y, ev.z, ev.module, ev.side)):
+            b.copy_(torch.from_numpy(a[:n]))
+        for b, a in zip(sb, sd.arrays()):
+            b.copy_(torch.from_numpy(a[:ns]))
+        return (synth.Event(ev.x[:n], ev.y[:n], ev.z[:n], ev.module[:n], ev.side[:n], ev.truth[:n], {}), tuple(a[:ns] for a in sd.arrays()))
+
+    fill(evs[0], sds[0])
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=st):
+        ctx.load_events(2, [hb], stream=st)
+        ctx.load_seeds(2, [sb], stream=st)
+        ctx.run_batch(2, 1, st)
+        ctx.run_stage(2, 1, lstmod.CLEAN, st)
+        ctx.run_stage(2, 1, lstmod.PIXEL, st)
+    for k in (1, 0, 1):
+        cut, seeds = fill(evs[k], sds[k])
+        torch.cuda.synchronize()
+        g.replay()
+        torch.cuda.synchronize()
+        ctx.sync(2, st)
+        ora = run_oracle(o32, cut, seeds=seeds)
+        compare_links(ctx, lstmod, ora, slot=2, label=f"graph replay {k}")
+        keep = o32.t5_clean(ora.t5_hits(), ora.t5_chi2xy, ora.t5_chi2rz)
+        assert ctx.stats(2)["n_kept"] == int(keep.sum())
