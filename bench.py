@@ -39,7 +39,7 @@ N_STREAMS = int(os.environ.get("LST_BENCH_STREAMS", "4"))   # BASELINE.json conf
 MAP_BYTES = 4 * (69630 + 6121)
 # SPEC operations per candidate (every sqrt and div counted as one)
 FLOPS_PER_CAND = (34, 51, 45, 255)
-HEADER_BYTES = 400   # per-slot counter block that lst_sync_batch reads back (csrc/lst_device.cuh SlotHeader)
+HEADER_BYTES = 424   # per-slot counter block that lst_sync_batch reads back (csrc/lst_device.cuh SlotHeader)
 A0_KERNELS = ("bin_count", "bin_scatter", "bin_order")               # lst_stats.kernel_ms[0..2]
 
 

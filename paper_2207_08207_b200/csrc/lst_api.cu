@@ -28,7 +28,7 @@ using namespace lst;
 static_assert((int)LST_MD == (int)LST_MD_ && (int)LST_SEG == (int)LST_SEG_ && (int)LST_T3 == (int)LST_T3_ &&
                   (int)LST_T5 == (int)LST_T5_ && (int)LST_CLEAN == (int)LST_CLEAN_ && (int)LST_PIXEL == (int)LST_PIXEL_, "stage ids");
 
-static_assert(sizeof(SlotHeader) == 400, "bench.py HEADER_BYTES counts the header lst_sync_batch reads back");
+static_assert(sizeof(SlotHeader) == 424, "bench.py HEADER_BYTES counts the header lst_sync_batch reads back");
 
 namespace {
 
@@ -252,6 +252,7 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
   const double kPi = 3.14159265358979323846;
   const int n_conn = m->row_offsets[n];
   std::vector<float> map_dphi((size_t)n_conn + 1, 0.0f);
+  std::vector<int> map_tgt((size_t)n_conn + 1, 0);   // rows re-ordered by (azimuth offset, target) for the segment kernel
   std::vector<float2> mod_cs(n);
   for (int a = 0; a < n; ++a) {
     if (!std::isfinite(g->phi[a])) return LST_ERR_ARG;
@@ -266,6 +267,19 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
       if (d > kPi) d -= 2.0 * kPi;
       if (d <= -kPi) d += 2.0 * kPi;
       map_dphi[k] = (float)d;
+      map_tgt[k] = t;
+    }
+    // insertion sort of the row (at most kMaxRow entries) by (azimuth offset, target)
+    for (int k = m->row_offsets[a] + 1; k < m->row_offsets[a + 1]; ++k) {
+      const float d = map_dphi[k];
+      const int t = map_tgt[k];
+      int j = k - 1;
+      for (; j >= m->row_offsets[a] && (map_dphi[j] > d || (map_dphi[j] == d && map_tgt[j] > t)); --j) {
+        map_dphi[j + 1] = map_dphi[j];
+        map_tgt[j + 1] = map_tgt[j];
+      }
+      map_dphi[j + 1] = d;
+      map_tgt[j + 1] = t;
     }
   }
 
@@ -291,7 +305,7 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
   if ((e = cudaMemcpy(c->d_layer, g->layer, n, cudaMemcpyHostToDevice)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   if ((e = cudaMemcpy(c->d_mod_cs, mod_cs.data(), sizeof(float2) * n, cudaMemcpyHostToDevice)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   if ((e = cudaMemcpy(c->d_map_offsets, m->row_offsets, sizeof(int) * (n + 1), cudaMemcpyHostToDevice)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
-  if (n_conn > 0 && (e = cudaMemcpy(c->d_map_targets, m->targets, sizeof(int) * (size_t)n_conn, cudaMemcpyHostToDevice)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
+  if (n_conn > 0 && (e = cudaMemcpy(c->d_map_targets, map_tgt.data(), sizeof(int) * (size_t)n_conn, cudaMemcpyHostToDevice)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   if (n_conn > 0 && (e = cudaMemcpy(c->d_map_dphi, map_dphi.data(), sizeof(float) * (size_t)n_conn, cudaMemcpyHostToDevice)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   if ((e = cudaMemset(c->arena, 0, c->arena_bytes)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   if ((e = cudaMallocHost(&c->pinned, sizeof(SlotHeader) * (size_t)cfg.n_slots)) != cudaSuccess) return bail(LST_ERR_CUDA, e);

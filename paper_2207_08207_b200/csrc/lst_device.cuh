@@ -67,6 +67,7 @@ struct SlotHeader {
   // r_min is stored as 0x7f800000 - bits so that the zeroed header means "+inf"
   int r_min_inv[2][6];
   int r_max[2][6];
+  int key_absmax[6];              // per layer: largest |key| of the finite lower-sensor hits, as float bits (directly after r_max: one flush loop)
   unsigned int done[8];           // "last block done" tickets, self-resetting (never zeroed with the header)
   unsigned int ticket[4];         // next chunk of the single-pass kernels (zeroed with the header)
   int n_kept;                     // quintuplets kept by the duplicate cleaning (stage LST_CLEAN)
@@ -115,8 +116,8 @@ struct Params {
   const signed char* mod_layer;  // [n_modules]
   const float2* mod_cs;          // [n_modules] (cos, sin) of the azimuth of the module normal
   const int* map_offsets;        // [n_modules + 1] module map, CSR
-  const int* map_targets;        // [map_offsets[n_modules]] ascending per row
-  const float* map_dphi;         // [map_offsets[n_modules]] azimuth(source normal) - azimuth(target normal), in (-pi, pi]
+  const int* map_targets;        // [map_offsets[n_modules]] rows ordered by (map_dphi, target): the entries an inner MD can reach are one run
+  const float* map_dphi;         // [map_offsets[n_modules]] azimuth(source normal) - azimuth(target normal), in (-pi, pi], ascending per row
   int first_slot;
   int dup_min_shared;            // [D] D4: quintuplets sharing at least this many original hits are duplicates
   int store_half;                // [H] output floats that no selection reads are stored as binary16

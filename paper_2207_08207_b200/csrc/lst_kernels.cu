@@ -179,6 +179,21 @@ __device__ __forceinline__ int upper_bound_f(const float* a, int lo, int hi, flo
   return lo;
 }
 
+// [first, first + count) = the entries of the ascending array a[lo .. hi) inside [vlo, vhi]: lower_bound(vlo) and
+// upper_bound(vhi) searched in ONE loop, so that the two chains of dependent loads travel together (these kernels are bound
+// by the latency along a warp's serial chain, not by instruction count: profiles/r2_summary.md).
+__device__ __forceinline__ int window_of(const float* a, int lo, int hi, float vlo, float vhi, int& first) {
+  int l0 = lo, h0 = hi, l1 = lo, h1 = hi;
+  while (l0 < h0 || l1 < h1) {
+    const int m0 = (l0 + h0) >> 1, m1 = (l1 + h1) >> 1;
+    const float k0 = a[min(m0, hi - 1)], k1 = a[min(m1, hi - 1)];
+    if (l0 < h0) { if (k0 < vlo) l0 = m0 + 1; else h0 = m0; }
+    if (l1 < h1) { if (k1 <= vhi) l1 = m1 + 1; else h1 = m1; }
+  }
+  first = l0;
+  return max(l1 - l0, 0);
+}
+
 // M2 bounds |sinA| by thr(r_u) <= thr(r_max_upper); M1 (dot > 0) gives r_u > r_l.  The window
 // shrinks as r_l grows, so evaluated at the smallest r of the layer's lower hits it covers them all.
 // Returns the half width of the azimuth window around the lower hit, < 0 if nothing can pass.
@@ -387,11 +402,11 @@ __global__ void __launch_bounds__(256) k_bin_scatter(const __grid_constant__ Par
 // in the same or the next bin).  Then fetch the hit's record (one 16-byte gather), derive r, and keep the range of r per
 // (side, layer) and the key range per module.
 __global__ void __launch_bounds__(256) k_bin_order(const __grid_constant__ Params P) {
-  __shared__ int s_rng[24];
+  __shared__ int s_rng[30];
   Slot S(P, blockIdx.y);
   SlotHeader* H = S.hdr();
   const int nmod = P.L.n_modules;
-  if (threadIdx.x < 24) s_rng[threadIdx.x] = 0;
+  if (threadIdx.x < 30) s_rng[threadIdx.x] = 0;
   __syncthreads();
   const int nh = H->n_hits;
   const unsigned* start = S.bin_start();
@@ -422,13 +437,15 @@ __global__ void __launch_bounds__(256) k_bin_order(const __grid_constant__ Param
     const bool fin = r < 3.0e38f;
     const unsigned act = __ballot_sync(__activemask(), fin);
     if (fin) {
-      const int slot = side * 6 + P.mod_layer[m];
+      const int layer = P.mod_layer[m], slot = side * 6 + layer;
       const unsigned grp = __match_any_sync(act, slot);
       const int rmax = __reduce_max_sync(grp, __float_as_int(r));
       const int rinv = __reduce_max_sync(grp, 0x7f800000 - __float_as_int(r));
+      const int kabs = __reduce_max_sync(grp, __float_as_int(fabsf(v.w)));     // |key| <= 4: finite here
       if ((int)lane_id() == __ffs(grp) - 1) {
         atomicMax(&s_rng[slot], rinv);
         atomicMax(&s_rng[12 + slot], rmax);
+        if (!side) atomicMax(&s_rng[24 + layer], kabs);      // the segment kernel bounds every module's key range by it
       }
     }
   }
@@ -444,7 +461,7 @@ __global__ void __launch_bounds__(256) k_bin_order(const __grid_constant__ Param
     if (lane_id() == 0 && c) atomicAdd(&H->cand[LST_MD_], c);
   }
   __syncthreads();
-  if (threadIdx.x < 24 && s_rng[threadIdx.x]) atomicMax(&H->r_min_inv[0][0] + threadIdx.x, s_rng[threadIdx.x]);
+  if (threadIdx.x < 30 && s_rng[threadIdx.x]) atomicMax(&H->r_min_inv[0][0] + threadIdx.x, s_rng[threadIdx.x]);   // r_min_inv, r_max, key_absmax
 }
 
 // ------------------------------------------------------------------------------------------
@@ -674,13 +691,9 @@ __global__ void __launch_bounds__(kWarps * 32, LST_MD_BLOCKS) k_md(const __grid_
       sh.layer[lane] = layer;
       const float w = s_w[layer];
       if (u1 > u0 && w >= 0.0f && s_rmaxU[layer] * 1.000001f >= lo.w) {
-        int j1 = u1;
         j0 = u0;
-        if (fabsf(kl) + w < 1.5f) {
-          j0 = lower_bound_f(hkey, u0, u1, kl - w);
-          j1 = upper_bound_f(hkey, j0, u1, kl + w);
-        }
-        n = j1 - j0;
+        n = u1 - u0;
+        if (fabsf(kl) + w < 1.5f) n = window_of(hkey, u0, u1, kl - w, kl + w, j0);
       }
     }
     sh.cnt[buf][lane] = 0;
@@ -761,16 +774,16 @@ __device__ __forceinline__ void seg_emit(const Params& P, const Slot& S, int pos
 // base + (segments of the lanes before the owner) + rank.  cnt[cb] counts per owner as the walk goes.
 template <bool DIRECT>
 __device__ __forceinline__ int seg_walk(const Params& P, const Slot& S, SegWarp& sh, int buf, int nt, int row0, int i0,
-                                        int base, unsigned long long& space_acc, unsigned long long& evals_acc) {
+                                        int base, unsigned long long& evals_acc) {
   const float4* anchor = S.md_anchor();
   const float2* aux = S.md_aux();
   const float* mkey = S.md_key();
   const int4* mod_info = S.mod_info();
   const int lane = (int)lane_id();
   const int cb = DIRECT ? buf ^ 1 : buf;   // running per-owner counters (the direct walk keeps the first walk's totals in cnt[buf])
-  // search-space counters of this walk: 32 bits suffice (a lane's row entries are distinct modules, its windows at most
-  // 64 x the mini-doublets of the event, capacities are below 2^26), the 64-bit totals stay out of the loops
-  unsigned space = 0, evals = 0;
+  // windows evaluated in this walk: 32 bits suffice (at most 64 x the mini-doublets of the event per lane, capacities are
+  // below 2^26), the 64-bit total stays out of the loops
+  unsigned evals = 0;
   int running = 0;
   int ph = 0, pt = 0, ch = 0, ct = 0;
 
@@ -822,8 +835,7 @@ __device__ __forceinline__ int seg_walk(const Params& P, const Slot& S, SegWarp&
         first = info.x;  // azimuth wrap possible (never with a sane geometry): no window
         cnt = info.y - info.x;
       } else {
-        first = lower_bound_f(mkey, info.x, info.y, c0 + dlo);
-        cnt = upper_bound_f(mkey, first, info.y, c0 + dhi) - first;
+        cnt = window_of(mkey, info.x, info.y, c0 + dlo, c0 + dhi, first);
       }
     }
     if (!DIRECT) evals += (unsigned)cnt;
@@ -885,7 +897,6 @@ __device__ __forceinline__ int seg_walk(const Params& P, const Slot& S, SegWarp&
     float c0 = 0.0f;
     if (t < nt) {
       const int4 info = cur.info;
-      if (!DIRECT) space += (unsigned)(info.y - info.x);
       const float dlo = sh.dlo[lane], dhi = sh.dhi[lane];
       if (info.y > info.x && dlo <= dhi) {
         c0 = sh.key[lane] + cur.dphi;
@@ -901,7 +912,6 @@ __device__ __forceinline__ int seg_walk(const Params& P, const Slot& S, SegWarp&
   }
   drainB(true);
   drainC(true);
-  space_acc += space;
   evals_acc += evals;
   return running;
 }
@@ -916,14 +926,36 @@ __global__ void __launch_bounds__(kSegWarps * 32, 7) k_seg(const __grid_constant
   const int nChunks = (nMD + kChunk - 1) / kChunk;
   const int lane = (int)lane_id();
   SegWarp& sh = shw[threadIdx.x >> 5];
+  __shared__ float s_keyMax[6];
   if (threadIdx.x < 6) {
     s_rMinO[threadIdx.x] = r_min_of(H, 0, threadIdx.x);
     s_rMaxO[threadIdx.x] = r_max_of(H, 0, threadIdx.x);
+    s_keyMax[threadIdx.x] = __int_as_float(H->key_absmax[threadIdx.x]);   // every module's key range lies within +- this
   }
   __syncthreads();
   int* seg_start = S.seg_start();
   unsigned long long* status = S.lb(LST_SEG_);
-  unsigned long long space = 0, evals = 0;
+  unsigned long long evals = 0;
+  {
+    // The method's search space (lst_stats.candidates): every pair of an MD with an MD of a connected module, summed per
+    // MODULE here (MDs of a module x MDs of its row), a slice of the modules per block -- the walk below only looks at the
+    // part of a row an MD's window can reach and cannot count it.
+    const int* md_start = S.md_start();
+    const int4* mod_info = S.mod_info();
+    unsigned long long space = 0;
+    for (int m = blockIdx.x * blockDim.x + threadIdx.x; m < P.L.n_modules; m += gridDim.x * blockDim.x) {
+      const int n_in = md_start[m + 1] - md_start[m];
+      if (n_in <= 0) continue;
+      int n_out = 0;
+      for (int e = P.map_offsets[m]; e < P.map_offsets[m + 1]; ++e) {
+        const int4 info = mod_info[P.map_targets[e]];
+        n_out += info.y - info.x;
+      }
+      space += (unsigned long long)n_in * (unsigned long long)n_out;
+    }
+    space = warp_sum_ull(space);
+    if (lane == 0 && space) atomicAdd(&H->cand[LST_SEG_], space);
+  }
 
   auto finish = [&](int C, int b, int total, int base, bool from_stash) {
     const int i0 = C * kChunk, i = i0 + lane;
@@ -940,6 +972,31 @@ __global__ void __launch_bounds__(kSegWarps * 32, 7) k_seg(const __grid_constant
         const int ol = (int)((unsigned)v >> 26);
         seg_emit(P, S, base + sh.tab[ol] + sh.stR[b][t], i0 + ol, v & (kMaxCap - 1), f.x, f.y);
       }
+    // An owner's segments were found in the order of its row (by azimuth offset), not by outer MD: the owner lane puts its
+    // one to three segments in ascending outer MD (insertion sort of the stored records; the other lanes' stores first)
+    __syncwarp();
+    {
+      const int mine = sh.cnt[b][lane];
+      const int lo = min(base + ex, cap), hi = min(base + ex + mine, cap);
+      int2* smd = S.seg_md();
+      for (int k = lo + 1; k < hi; ++k) {
+        const int2 key = smd[k];
+        if (smd[k - 1].y <= key.y) continue;
+        if (P.store_half) {
+          uint2* sf = reinterpret_cast<uint2*>(S.seg_f());
+          const uint2 val = sf[k];
+          int j = k - 1;
+          for (; j >= lo && smd[j].y > key.y; --j) { smd[j + 1] = smd[j]; sf[j + 1] = sf[j]; }
+          smd[j + 1] = key; sf[j + 1] = val;
+        } else {
+          float4* sf = S.seg_f();
+          const float4 val = sf[k];
+          int j = k - 1;
+          for (; j >= lo && smd[j].y > key.y; --j) { smd[j + 1] = smd[j]; sf[j + 1] = sf[j]; }
+          smd[j + 1] = key; sf[j + 1] = val;
+        }
+      }
+    }
     if (i < nMD) seg_start[i] = min(base + ex, cap);
     if (i == nMD - 1) {
       seg_start[nMD] = min(base + total, cap);
@@ -967,18 +1024,33 @@ __global__ void __launch_bounds__(kSegWarps * 32, 7) k_seg(const __grid_constant
       row0 = P.map_offsets[A];
       nt = P.map_offsets[A + 1] - row0;
       const int layer = P.mod_layer[A];
+      const float key = S.md_key()[i];
       float dlo = 1.0f, dhi = -1.0f;
       if (nt > 0) seg_window(P.cuts, layer, a.w, x.x, x.y, s_rMinO[layer + 1], s_rMaxO[layer + 1], dlo, dhi);
+      if (!(dlo <= dhi)) {
+        nt = 0;
+      } else if (nt > 0) {
+        // The part of the row this MD can reach.  A connected module's key range lies within +-W (the largest |key| of the
+        // outer layer's hits), and level A needs key + offset + dhi >= kmin and key + offset + dlo <= kmax, so the offset
+        // lies in [-W - key - dhi, W - key - dlo]: one run of the row, which is ordered by offset (1e-4 rad of slack
+        // against the rounding of these sums).  Where an azimuth wrap is possible the whole row stays.
+        const float W = s_keyMax[layer + 1];
+        if (W + fabsf(key) + fmaxf(fabsf(dlo), fabsf(dhi)) < 1.5f) {
+          int t0;
+          nt = window_of(P.map_dphi, row0, row0 + nt, (-W - key - dhi) - 1e-4f, (W - key - dlo) + 1e-4f, t0);
+          row0 = t0;
+        }
+      }
       sh.a4[lane] = a;
       sh.aux[lane] = x;
-      sh.key[lane] = S.md_key()[i];
+      sh.key[lane] = key;
       sh.dlo[lane] = dlo;
       sh.dhi[lane] = dhi;
       sh.layer[lane] = layer;
     }
     sh.cnt[buf][lane] = 0;
     __syncwarp();
-    const int total = seg_walk<false>(P, S, sh, buf, nt, row0, i0, 0, space, evals);
+    const int total = seg_walk<false>(P, S, sh, buf, nt, row0, i0, 0, evals);
     publish_aggregate(status, C, total);
     __syncwarp();
     if (pC >= 0) {
@@ -994,14 +1066,12 @@ __global__ void __launch_bounds__(kSegWarps * 32, 7) k_seg(const __grid_constant
       sh.tab[lane] = warp_excl_scan(sh.cnt[buf][lane], tot);
       sh.cnt[buf ^ 1][lane] = 0;
       __syncwarp();
-      seg_walk<true>(P, S, sh, buf, nt, row0, i0, base, space, evals);
+      seg_walk<true>(P, S, sh, buf, nt, row0, i0, base, evals);
       finish(C, buf, total, base, false);
     }
   }
   if (pC >= 0) finish(pC, buf ^ 1, pTotal, resolve_base(status, pC, pTotal), true);
-  space = warp_sum_ull(space);
   evals = warp_sum_ull(evals);
-  if (lane == 0 && space) atomicAdd(&H->cand[LST_SEG_], space);
   if (lane == 0 && evals) atomicAdd(&H->eval[LST_SEG_], evals);
 }
 
