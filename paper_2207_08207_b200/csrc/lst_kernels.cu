@@ -11,6 +11,8 @@
 //   * the ranges are flattened: a warp scan numbers the candidates, and every tile of 32
 //     candidates finds its owners with one redux + popc (no search, no barrier), so all 32 lanes
 //     evaluate one candidate each whatever the occupancy skew between owners;
+//     (the segment kernel's first level is the exception: lane = owner, the warp steps through the
+//     owners' map rows in lockstep);
 //   * where a cheap test removes most candidates (module key ranges and windows for segments, the
 //     curvature match for quintuplets) survivors are compacted into a small shared-memory
 //     queue and the expensive selection runs on full tiles of survivors;
@@ -724,12 +726,15 @@ __global__ void __launch_bounds__(kWarps * 32, LST_MD_BLOCKS) k_md(const __grid_
 
 // ------------------------------------------------------------------------------------------
 // a2: segments.  Owner = inner MD.  Three levels, each compacted before the next:
-//   A  every (inner MD, connected module) pair: module has MDs and its key range meets the
-//      MD's azimuth window?                                             -> pair queue
-//   B  surviving pairs: window of outer MDs by two binary searches in the module's key-ordered
-//      MD list; the windows are flattened into candidates               -> candidate queue
-//   C  candidates, 32 at a time: the SPEC selection                     -> stash
-// Segments come out ordered by (inner MD, outer MD).
+//   A  lane = inner MD; the (inner MD, connected module) pairs of the part of the map row the MD's
+//      window can reach (rows are ordered by azimuth offset: one run, found by a search): module
+//      has MDs and its key range meets the MD's azimuth window?         -> pair queue
+//   B  surviving pairs: window of outer MDs by a search (both bounds in one loop) in the module's
+//      key-ordered MD list; the windows are flattened into candidates, closed-form pre-filter
+//                                                                        -> candidate queue
+//   C  candidates, 32 at a time: the SPEC selection                     -> stash (arrival order + rank)
+// Segments come out ordered by (inner MD, outer MD): placed by (owner, arrival rank), then every
+// owner's few segments are put in ascending outer MD.
 // ------------------------------------------------------------------------------------------
 // The block's shared memory decides how much of the SM's 256 KB is left as L1: 7 resident blocks must stay within the 196 KB
 // carve-out (27 648 B per block incl. the 1 KB the system reserves), or the next carve-out (228 KB) halves the L1 and costs 5 %
