@@ -422,7 +422,16 @@ __global__ void __launch_bounds__(256) k_bin_order(const __grid_constant__ Param
     const int orig = (int)(unsigned)mine;
     const float4 v = S.rec4()[orig];                         // (x, y, z, key)
     int rank = 0;
-    for (int j = s; j < e; ++j) rank += tk[j] < mine;
+    {   // two entries per 16-byte load once the position is even (the array is 16-byte aligned)
+      int j = s;
+      if ((j & 1) && j < e) { rank += tk[j] < mine; ++j; }
+      const ulonglong2* tk2 = reinterpret_cast<const ulonglong2*>(tk);
+      for (; j + 1 < e; j += 2) {
+        const ulonglong2 t = tk2[j >> 1];
+        rank += (t.x < mine) + (t.y < mine);
+      }
+      if (j < e) rank += tk[j] < mine;
+    }
     const int side = b >= nmod, m = b - side * nmod;
     const float r = sqrtf(v.x * v.x + v.y * v.y);
     const int dst = s + rank;
