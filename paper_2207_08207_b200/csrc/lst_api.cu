@@ -336,12 +336,13 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
   c->P.first_slot = 0;
   c->P.dup_min_shared = cfg.t5_dup_min_shared;
   c->P.store_half = cfg.store_half != 0;
-  {  // [P]: are the modules of layers 0 and 1 a prefix of the module ids?
+  for (int k = 0; k < 2; ++k) {  // are the modules of layers <= 1 / <= 3 a prefix of the module ids?
+    const int max_layer = k ? 3 : 1;
     int live = 0;
-    while (live < n && g->layer[live] <= 1) ++live;
+    while (live < n && g->layer[live] <= max_layer) ++live;
     bool prefix = true;
-    for (int i = live; i < n; ++i) prefix = prefix && g->layer[i] > 1;
-    c->P.pix_live_modules = prefix ? live : n;
+    for (int i = live; i < n; ++i) prefix = prefix && g->layer[i] > max_layer;
+    c->P.live_modules[k] = prefix ? live : n;
   }
   if ((e = cudaDeviceSynchronize()) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   *out = c;

@@ -1149,6 +1149,10 @@ __global__ void __launch_bounds__(kWarps * 32, 6) k_t3(const __grid_constant__ P
   const int cap = P.L.cap_t3;
   const int nSeg = H->n[LST_SEG_];
   const int nChunks = (nSeg + kChunk - 1) / kChunk;
+  // segments whose inner MD sits on layer 4 cannot start a triplet; with module ids ordered by layer they are the tail of the
+  // segment list (P.live_modules[1] = leading modules on layers 0..3): no candidates, known without a load
+  int nLive = nSeg;
+  if (P.live_modules[1] < P.L.n_modules && !H->overflow) nLive = min(nSeg, S.seg_start()[S.md_start()[P.live_modules[1]]]);
   const int lane = (int)lane_id();
   T3Warp& sh = shw[threadIdx.x >> 5];
   const int* seg_start = S.seg_start();
@@ -1186,7 +1190,7 @@ __global__ void __launch_bounds__(kWarps * 32, 6) k_t3(const __grid_constant__ P
     }
     const int a0 = C * kChunk, a = a0 + lane;
     int n = 0, b0 = 0;
-    if (a < nSeg) {
+    if (a < nLive) {
       const int2 ma = S.seg_md()[a];
       b0 = seg_start[ma.y];
       n = seg_start[ma.y + 1] - b0;
@@ -1325,6 +1329,11 @@ __global__ void __launch_bounds__(kWarps * 32, LST_T5_BLOCKS) k_t5(const __grid_
   const int cap = P.L.cap_t5;
   const int nT3 = H->n[LST_T3_];
   const int nChunks = (nT3 + kChunk - 1) / kChunk;
+  // only triplets starting on layer 0 or 1 can be the inner half of a quintuplet: a prefix of the triplet list when module ids
+  // are ordered by layer (P.live_modules[0]); the owners behind it have no candidates, known without a load
+  int nLive = nT3;
+  if (P.live_modules[0] < P.L.n_modules && !H->overflow)
+    nLive = min(nT3, S.t3_start()[S.seg_start()[S.md_start()[P.live_modules[0]]]]);
   const int lane = (int)lane_id();
   T5Warp& sh = shw[threadIdx.x >> 5];
   const int* seg_start = S.seg_start();
@@ -1363,7 +1372,7 @@ __global__ void __launch_bounds__(kWarps * 32, LST_T5_BLOCKS) k_t5(const __grid_
     }
     const int A0 = C * kChunk, A = A0 + lane;
     int n = 0, B0 = 0;
-    if (A < nT3) {
+    if (A < nLive) {
       const int4 ta = S.t3_pack()[A];
       B0 = t3_start[seg_start[ta.z]];
       n = t3_start[seg_start[ta.z + 1]] - B0;
@@ -1844,13 +1853,13 @@ __global__ void __launch_bounds__(kPixWarps * 32, 6) k_pix(const __grid_constant
   Slot S(P, blockIdx.y);
   SlotHeader* H = S.hdr();
   const int cap = P.L.cap_pix[KIND];
-  const int nAll = H->n[KIND ? LST_T5_ : LST_T3_];
+  const int nObj = H->n[KIND ? LST_T5_ : LST_T3_];
   // Triplets are numbered by first segment, segments by inner MD, MDs by module: when the module ids are ordered by layer
-  // (P.pix_live_modules = number of leading modules on layers 0 and 1) the triplets that can be linked are a prefix of the
-  // triplet list, found through the CSR offsets; only they are walked, the rest just get their (empty) CSR entry.
-  int nObj = nAll;
-  if (!KIND && P.pix_live_modules < P.L.n_modules && !H->overflow)
-    nObj = min(nAll, S.t3_start()[S.seg_start()[S.md_start()[P.pix_live_modules]]]);
+  // (P.live_modules[0] = number of leading modules on layers 0 and 1) the triplets that can be linked are a prefix of the
+  // triplet list, found through the CSR offsets; the owners behind it are known to have no candidates without a load.
+  int nLive = nObj;
+  if (!KIND && P.live_modules[0] < P.L.n_modules && !H->overflow)
+    nLive = min(nObj, S.t3_start()[S.seg_start()[S.md_start()[P.live_modules[0]]]]);
   const int nChunks = (nObj + kChunk - 1) / kChunk;
   const int nSeeds = H->n_seeds;
   const int lane = (int)lane_id();
@@ -1909,10 +1918,9 @@ __global__ void __launch_bounds__(kPixWarps * 32, 6) k_pix(const __grid_constant
       }
     }
     if (A < nObj) pix_start[A] = min(base + ex, cap);
-    if (A0 + 31 >= nObj - 1) {      // the last chunk: the end of the CSR array, for the objects not walked too
-      const int end = min(base + total, cap);
-      for (int i = nObj + lane; i <= nAll; i += 32) pix_start[i] = end;
-      if (A == nObj - 1) publish(base + total);
+    if (A == nObj - 1) {
+      pix_start[nObj] = min(base + total, cap);
+      publish(base + total);
     }
     __syncwarp();
   };
@@ -1921,15 +1929,15 @@ __global__ void __launch_bounds__(kPixWarps * 32, 6) k_pix(const __grid_constant
   for (;;) {
     const int C = warp_ticket(&H->ticket_pix[KIND]);
     if (C >= nChunks) {
-      if (C == 0) {
-        for (int i = lane; i <= nAll; i += 32) pix_start[i] = 0;
-        if (lane == 0) publish(0);
+      if (C == 0 && lane == 0) {
+        publish(0);
+        pix_start[0] = 0;
       }
       break;
     }
     const int A0 = C * kChunk, A = A0 + lane;
     int n = 0, first = 0, n1 = 0, second = 0, nMain = 0;
-    if (A < nObj) {
+    if (A < nLive) {
       int md[N];
       float kobj;
       if (KIND) {
