@@ -336,8 +336,8 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
   c->P.first_slot = 0;
   c->P.dup_min_shared = cfg.t5_dup_min_shared;
   c->P.store_half = cfg.store_half != 0;
-  for (int k = 0; k < 2; ++k) {  // are the modules of layers <= 1 / <= 3 a prefix of the module ids?
-    const int max_layer = k ? 3 : 1;
+  for (int k = 0; k < 3; ++k) {  // are the modules of layers <= 1 / <= 3 / <= 4 a prefix of the module ids?
+    const int max_layer = k == 0 ? 1 : k == 1 ? 3 : 4;
     int live = 0;
     while (live < n && g->layer[live] <= max_layer) ++live;
     bool prefix = true;

@@ -121,9 +121,9 @@ struct Params {
   int first_slot;
   int dup_min_shared;            // [D] D4: quintuplets sharing at least this many original hits are duplicates
   int store_half;                // [H] output floats that no selection reads are stored as binary16
-  int live_modules[2];           // modules 0 .. live_modules[k]-1 are exactly those on layers <= 1 (k = 0) / <= 3 (k = 1) when the module
-                                 // ids are ordered by layer, else n_modules: owners of the triplet / quintuplet / pixel kernels behind the
-                                 // corresponding CSR prefix have no candidates
+  int live_modules[3];           // modules 0 .. live_modules[k]-1 are exactly those on layers <= 1 (k = 0) / <= 3 (k = 1) / <= 4 (k = 2) when the
+                                 // module ids are ordered by layer, else n_modules: owners of the quintuplet and pixel / triplet / segment
+                                 // kernel behind the corresponding CSR prefix have no candidates
 };
 
 // Typed access to one slot.

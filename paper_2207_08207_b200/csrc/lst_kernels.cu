@@ -550,7 +550,7 @@ __device__ __forceinline__ int warp_ticket(unsigned* ticket) {
 }
 
 // a[lo .. hi) = v by one warp: 16-byte stores over the aligned middle (the arrays start on 256-byte boundaries).
-__device__ __forceinline__ void fill_ints(int* a, int lo, int hi, int v) {
+__device__ __noinline__ void fill_ints(int* a, int lo, int hi, int v) {
   const int lane = (int)lane_id();
   const int mid0 = min((lo + 3) & ~3, hi), mid1 = max(hi & ~3, mid0);
   for (int i = lo + lane; i < mid0; i += 32) a[i] = v;
@@ -946,7 +946,11 @@ __global__ void __launch_bounds__(kSegWarps * 32, 7) k_seg(const __grid_constant
   Slot S(P, blockIdx.y);
   SlotHeader* H = S.hdr();
   const int cap = P.L.cap_seg;
-  const int nMD = H->n[LST_MD_];
+  const int nAll = H->n[LST_MD_];
+  // mini-doublets of the outermost layer have no map row: with module ids ordered by layer (P.live_modules[2] = leading modules
+  // on layers 0..4) they are the tail of the MD list; only the MDs before it are walked
+  int nMD = nAll;
+  if (P.live_modules[2] < P.L.n_modules && !H->overflow) nMD = min(nAll, S.md_start()[P.live_modules[2]]);
   const int nChunks = (nMD + kChunk - 1) / kChunk;
   const int lane = (int)lane_id();
   SegWarp& sh = shw[threadIdx.x >> 5];
@@ -1022,9 +1026,9 @@ __global__ void __launch_bounds__(kSegWarps * 32, 7) k_seg(const __grid_constant
       }
     }
     if (i < nMD) seg_start[i] = min(base + ex, cap);
-    if (i == nMD - 1) {
-      seg_start[nMD] = min(base + total, cap);
-      publish_total(H, LST_SEG_, base + total, cap);
+    if (i0 + 31 >= nMD - 1) {
+      fill_ints(seg_start, nMD, nAll + 1, min(base + total, cap));
+      if (i == nMD - 1) publish_total(H, LST_SEG_, base + total, cap);
     }
     __syncwarp();
   };
@@ -1033,9 +1037,9 @@ __global__ void __launch_bounds__(kSegWarps * 32, 7) k_seg(const __grid_constant
   for (;;) {
     const int C = warp_ticket(&H->ticket[LST_SEG_]);
     if (C >= nChunks) {
-      if (C == 0 && lane == 0) {  // no MDs at all: the first ticket publishes the empty result
-        publish_total(H, LST_SEG_, 0, cap);
-        seg_start[0] = 0;
+      if (C == 0) {  // no MDs with a map row at all: the first ticket publishes the empty result
+        fill_ints(seg_start, 0, nAll + 1, 0);
+        if (lane == 0) publish_total(H, LST_SEG_, 0, cap);
       }
       break;
     }
