@@ -409,3 +409,35 @@ def test_pixel_stage_in_a_cuda_graph(ctx, lstmod, o32, run_oracle, geom):
         compare_links(ctx, lstmod, ora, slot=2, label=f"graph replay {k}")
         keep = o32.t5_clean(ora.t5_hits(), ora.t5_chi2xy, ora.t5_chi2rz)
         assert ctx.stats(2)["n_kept"] == int(keep.sum())
+
+
+@pytest.mark.parametrize("first_layer", [1, 2, 4, 5])
+def test_events_without_inner_layers(ctx, lstmod, o32, run_oracle, geom, first_layer):
+    """The stage kernels walk only the owners that can have candidates (a CSR prefix when module ids are ordered by layer) and
+    fill the CSR entries of the rest: events whose hits start at layer 1, 2 (no quintuplet and no pixel link can exist, but
+    triplets do), 4 (segments, no triplets) and 5 (mini-doublets only) exercise the empty-prefix paths."""
+    ev = synth.generate_event(geom, 1, 123, n_particles=1500)
+    keep = geom.layer[ev.module] >= first_layer
+    cut = synth.Event(ev.x[keep], ev.y[keep], ev.z[keep], ev.module[keep], ev.side[keep], ev.truth[keep], {})
+    sd = synth.generate_seeds(ev, 123)
+    run_pixel(ctx, lstmod, cut, sd.arrays(), slot=3)
+    ctx.run_stage(3, 1, lstmod.CLEAN)
+    ctx.sync(3)
+    ora = run_oracle(o32, cut, seeds=sd.arrays())
+    parity.compare(parity.gpu_tables(ctx, 3), parity.oracle_tables(ora), f"from layer {first_layer}")
+    compare_links(ctx, lstmod, ora, slot=3, label=f"from layer {first_layer}")
+    st = ctx.stats(3)
+    assert st["needed"] == ora.counts and st["candidates"] == ora.candidates
+    if first_layer >= 2:
+        assert ora.counts[3] == 0 and ora.pix[0]["n"] == 0 and st["n_kept"] == 0
+    if first_layer == 2:
+        assert ora.counts[2] > 100
+    if first_layer == 4:
+        assert ora.counts[1] > 100 and ora.counts[2] == 0
+    if first_layer == 5:
+        assert ora.counts[0] > 100 and ora.counts[1] == 0
+    # the CSR arrays are complete: every entry of the owners that were not walked equals the total
+    for view, key, n_owner in ((ctx.segments(3), "md_start", st["needed"][0]), (ctx.triplets(3), "seg_start", st["needed"][1]),
+                               (ctx.quintuplets(3), "t3_start", st["needed"][2])):
+        start = view[key].torch().cpu().numpy()
+        assert len(start) == n_owner + 1 and start[0] == 0 and start[-1] == view["n"] and np.all(np.diff(start) >= 0)
