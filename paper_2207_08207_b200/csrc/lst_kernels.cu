@@ -243,16 +243,18 @@ __device__ __forceinline__ void seg_window(const Cuts& c, int layer, float r_i, 
 // event 320 k window candidates -> 55.5 k segments: S3 rejects a third, S4-outer most of the rest.
 __device__ __forceinline__ bool seg_prefilter(const Cuts& c, int layer_in, const float4& ai, const float4& ao,
                                               const float2& auxo, float delta) {
+  // both tests are evaluated without a branch between them, so that the gathers of the outer record (anchor, aux) travel
+  // together instead of the second waiting for the first test
   const float dr = ao.w - ai.w;
   const float z0 = ai.z - ai.w * __fdividef(ao.z - ai.z, dr);
-  if (fabsf(z0) > c.seg_z0_max[layer_in] * 1.001f + 0.05f) return false;      // S3 (a NaN goes on to the exact test)
+  const bool s3_fails = fabsf(z0) > c.seg_z0_max[layer_in] * 1.001f + 0.05f;   // S3 (a NaN goes on to the exact test)
   float sd, cd;
   __sincosf(delta, &sd, &cd);
   const float den2 = (ao.w * ao.w + ai.w * ai.w) - 2.0f * ai.w * ao.w * cd;
-  if (!(den2 > 0.0f)) return true;
   const float s = ao.w * sd * rsqrtf(den2);
   const float e2 = fabsf(auxo.y - s * __fdividef(auxo.x, ao.w));
-  return !(e2 > c.md_eps[layer_in + 1] + 2e-3f);                               // S4, outer mini-doublet
+  const bool s4_fails = den2 > 0.0f && e2 > c.md_eps[layer_in + 1] + 2e-3f;    // S4, outer mini-doublet
+  return !(s3_fails | s4_fails);
 }
 
 __device__ __forceinline__ float r_min_of(const SlotHeader* h, int side, int layer) {
@@ -1206,14 +1208,17 @@ __global__ void __launch_bounds__(kWarps * 32, 6) k_t3(const __grid_constant__ P
     const int a0 = C * kChunk, a = a0 + lane;
     int n = 0, b0 = 0;
     if (a < nSeg) {
+      // every load of the owner's record is issued before any is needed (also for owners that turn out to have no
+      // candidates): the chains travel together
       const int2 ma = S.seg_md()[a];
-      b0 = seg_start[ma.y];
-      n = seg_start[ma.y + 1] - b0;
-      if (n > 0) {
-        sh.p1[lane] = S.md_anchor()[ma.x];
-        sh.p2[lane] = S.md_anchor()[ma.y];
-        sh.layer[lane] = P.mod_layer[S.md_module()[ma.x]];
-      }
+      const int s0 = seg_start[ma.y], s1 = seg_start[ma.y + 1];
+      const float4 p1 = S.md_anchor()[ma.x], p2 = S.md_anchor()[ma.y];
+      const int layer = P.mod_layer[S.md_module()[ma.x]];
+      b0 = s0;
+      n = s1 - s0;
+      sh.p1[lane] = p1;
+      sh.p2[lane] = p2;
+      sh.layer[lane] = layer;
     }
     sh.cnt[buf][lane] = 0;
     cand += (unsigned long long)n;
@@ -1389,18 +1394,19 @@ __global__ void __launch_bounds__(kWarps * 32, LST_T5_BLOCKS) k_t5(const __grid_
     const int A0 = C * kChunk, A = A0 + lane;
     int n = 0, B0 = 0;
     if (A < nT3) {
+      // every load of the owner's record is issued before any is needed: the chains travel together
       const int4 ta = S.t3_pack()[A];
-      B0 = t3_start[seg_start[ta.z]];
-      n = t3_start[seg_start[ta.z + 1]] - B0;
-      if (n > 0) {
-        sh.p[0][lane] = S.md_anchor()[ta.x];
-        sh.p[1][lane] = S.md_anchor()[ta.y];
-        sh.p[2][lane] = S.md_anchor()[ta.z];
-        sh.kA[lane] = __int_as_float(ta.w);
-        const int layer = P.mod_layer[S.md_module()[ta.x]];
-        sh.layer[lane] = layer;
-        if (layer > 1) n = 0;   // cannot happen with a valid module map (targets one layer out); t5_select indexes [layer + 4]
-      }
+      const int g0 = seg_start[ta.z], g1 = seg_start[ta.z + 1];
+      const float4 q0 = S.md_anchor()[ta.x], q1 = S.md_anchor()[ta.y], q2 = S.md_anchor()[ta.z];
+      const int layer = P.mod_layer[S.md_module()[ta.x]];
+      B0 = t3_start[g0];
+      n = t3_start[g1] - B0;
+      sh.p[0][lane] = q0;
+      sh.p[1][lane] = q1;
+      sh.p[2][lane] = q2;
+      sh.kA[lane] = __int_as_float(ta.w);
+      sh.layer[lane] = layer;
+      if (layer > 1) n = 0;   // cannot happen with a valid module map (targets one layer out); t5_select indexes [layer + 4]
     }
     sh.cnt[buf][lane] = 0;
     cand += (unsigned long long)n;
