@@ -81,31 +81,30 @@ struct SegOut {
 // ai / ao = anchor (x, y, z, r) of the inner / outer MD; aux = (ur, sinA) of each.
 __device__ __forceinline__ bool seg_select(const Cuts& c, int layer_in, const float4& ai, const float2& auxi,
                                            const float4& ao, const float2& auxo, SegOut& o) {
+  // Every value is computed by the SPEC expression; the tests are combined at the end instead of returning early (nine in ten
+  // candidates that reach this point pass, and without branches all operands are fetched up front).  A division by zero
+  // gives an infinity or a NaN, and a NaN fails its `<=` as the SPEC demands.
   const float dx = ao.x - ai.x, dy = ao.y - ai.y;
   // S2
   const float cross = ai.x * dy - ai.y * dx;
   const float dot = ai.x * dx + ai.y * dy;
   const float n2 = (ai.x * ai.x + ai.y * ai.y) * (dx * dx + dy * dy);
-  if (!(n2 > 0.0f)) return false;
   const float sinS = cross / sqrtf(n2);
-  if (!(dot > 0.0f)) return false;
   const float thr = sin_threshold(c, ao.w, c.seg_cos_eps, c.seg_sin_eps);
-  if (!(fabsf(sinS) <= thr)) return false;
+  bool ok = (n2 > 0.0f) & (dot > 0.0f) & (fabsf(sinS) <= thr);
   // S3
   const float dr = ao.w - ai.w;
-  if (!(dr > 0.0f)) return false;
   const float z0 = ai.z - ai.w * (ao.z - ai.z) / dr;
-  if (!(fabsf(z0) <= c.seg_z0_max[layer_in])) return false;
+  ok = ok & (dr > 0.0f) & (fabsf(z0) <= c.seg_z0_max[layer_in]);
   // S4
   const float e1 = fabsf(auxi.y - sinS * (auxi.x / ao.w));
-  if (!(e1 <= c.md_eps[layer_in])) return false;
   const float e2 = fabsf(auxo.y - sinS * (auxo.x / ao.w));
-  if (!(e2 <= c.md_eps[layer_in + 1])) return false;
+  ok = ok & (e1 <= c.md_eps[layer_in]) & (e2 <= c.md_eps[layer_in + 1]);
   o.sinS = sinS;
   o.z0 = z0;
   o.cross = cross;
   o.dot = dot;
-  return true;
+  return ok;
 }
 
 // ---- [T] triplet ------------------------------------------------------------

@@ -587,17 +587,20 @@ struct MdWarp {
 // i = index of the lower hit (owner), u = index of the upper hit.
 __device__ __forceinline__ void md_emit(const Params& P, const Slot& S, int pos, int i, int u, float sinA) {
   if (pos >= P.L.cap_md) return;
+  // all gathers first (a store that needs a loaded value holds up the loads behind it), then the stores
   const float4 lo = S.hit4()[i], up = S.hit4()[u];
+  const float key = S.hit_key()[i];
+  const int orig_lo = S.hit_orig()[i], orig_up = S.hit_orig()[u], module = S.hit_module()[i];
   const float dx = up.x - lo.x, dy = up.y - lo.y;
   const float cross = lo.x * dy - lo.y * dx, dot = lo.x * dx + lo.y * dy;   // as in md_select
+  const float dphi = atan2f(lo.x * up.y - lo.y * up.x, lo.x * up.x + lo.y * up.y), dphichange = atan2f(cross, dot);
   S.md_anchor()[pos] = lo;
   S.md_aux()[pos] = make_float2(up.w, sinA);
-  S.md_key()[pos] = S.hit_key()[i];
-  S.md_hits()[pos] = make_int2(S.hit_orig()[i], S.hit_orig()[u]);
-  const float dphi = atan2f(lo.x * up.y - lo.y * up.x, lo.x * up.x + lo.y * up.y), dphichange = atan2f(cross, dot);
+  S.md_key()[pos] = key;
+  S.md_hits()[pos] = make_int2(orig_lo, orig_up);
   if (P.store_half) reinterpret_cast<__half2*>(S.md_out())[pos] = __floats2half2_rn(dphi, dphichange);   // [H]
   else S.md_out()[pos] = make_float2(dphi, dphichange);
-  S.md_module()[pos] = S.hit_module()[i];
+  S.md_module()[pos] = module;
 }
 
 template <bool DIRECT>
@@ -1121,8 +1124,8 @@ struct T3Warp {
 // a / b = index of the first / second segment.
 __device__ __forceinline__ void t3_emit(const Params& P, const Slot& S, int pos, int a, int b, float kappa, float chi2) {
   if (pos >= P.L.cap_t3) return;
-  const int2 ma = S.seg_md()[a];
-  S.t3_pack()[pos] = make_int4(ma.x, ma.y, S.seg_md()[b].y, __float_as_int(kappa));
+  const int2 ma = S.seg_md()[a], mb = S.seg_md()[b];
+  S.t3_pack()[pos] = make_int4(ma.x, ma.y, mb.y, __float_as_int(kappa));
   S.t3_seg()[pos] = make_int2(a, b);
   if (P.store_half) reinterpret_cast<__half*>(S.t3_chi2())[pos] = __float2half_rn(chi2);   // [H]
   else S.t3_chi2()[pos] = chi2;
@@ -1974,12 +1977,14 @@ __global__ void __launch_bounds__(kPixWarps * 32, 6) k_pix(const __grid_constant
         md[0] = ta.x; md[1] = ta.y; md[2] = ta.z;
         kobj = __int_as_float(ta.w);
       }
+      float4 pa[N];          // the anchors are fetched while the layer is looked up (two dependent loads)
+#pragma unroll
+      for (int i = 0; i < N; ++i) pa[i] = S.md_anchor()[md[i]];
       const int layer = P.mod_layer[S.md_module()[md[0]]];
       if (layer <= 1) {     // the first anchor of a pixel-linked object sits on one of the two innermost layers
-        const float4 p0 = S.md_anchor()[md[0]];
-        sh.p[0][lane] = p0;
+        const float4 p0 = pa[0];
 #pragma unroll
-        for (int i = 1; i < N; ++i) sh.p[i][lane] = S.md_anchor()[md[i]];
+        for (int i = 0; i < N; ++i) sh.p[i][lane] = pa[i];
         sh.kobj[lane] = kobj;
         sh.layer[lane] = layer;
         cand += (unsigned long long)nSeeds;
