@@ -51,27 +51,25 @@ struct MdOut {
 // lower = (x, y, z, r) of the side-0 hit, upper likewise for side 1. r = sqrtf(x*x + y*y) was
 // derived at load time with that exact expression.
 __device__ __forceinline__ bool md_select(const Cuts& c, int layer, const float4& lo, const float4& up, MdOut& o) {
+  // no early return (see seg_select): the tests are combined at the end, a NaN fails its `<=`
   const float dx = up.x - lo.x, dy = up.y - lo.y;
   // M1: SINANG(xl, yl, dx, dy)
   const float cross = lo.x * dy - lo.y * dx;
   const float dot = lo.x * dx + lo.y * dy;
   const float n2 = (lo.x * lo.x + lo.y * lo.y) * (dx * dx + dy * dy);
-  if (!(n2 > 0.0f)) return false;
   const float sinA = cross / sqrtf(n2);
-  if (!(dot > 0.0f)) return false;
   // M2
   const float thr = sin_threshold(c, up.w, c.md_cos_eps[layer], c.md_sin_eps[layer]);
-  if (!(fabsf(sinA) <= thr)) return false;
+  bool ok = (n2 > 0.0f) & (dot > 0.0f) & (fabsf(sinA) <= thr);
   // M3
-  if (!(lo.w > 0.0f)) return false;
   const float dr = up.w - lo.w;
   const float lhs = fabsf((up.z - lo.z) - lo.z * dr / lo.w);
   const float rhs = c.z_lum * fabsf(dr) / lo.w + c.md_dz_res[layer];
-  if (!(lhs <= rhs)) return false;
+  ok = ok & (lo.w > 0.0f) & (lhs <= rhs);
   o.sinA = sinA;
   o.cross = cross;
   o.dot = dot;
-  return true;
+  return ok;
 }
 
 // ---- [S] segment --------------------------------------------------------
@@ -110,27 +108,26 @@ __device__ __forceinline__ bool seg_select(const Cuts& c, int layer_in, const fl
 // ---- [T] triplet ------------------------------------------------------------
 __device__ __forceinline__ bool t3_select(const Cuts& c, int layer1, const float4& p1, const float4& p2,
                                           const float4& p3, float& kappa, float& chi2rz) {
+  // no early return (see seg_select)
   const float ax = p2.x - p1.x, ay = p2.y - p1.y;
   const float bx = p3.x - p1.x, by = p3.y - p1.y;
   const float cx = p3.x - p2.x, cy = p3.y - p2.y;
   // T2
   const float cross = ax * by - ay * bx;
   const float den2 = ((ax * ax + ay * ay) * (bx * bx + by * by)) * (cx * cx + cy * cy);
-  if (!(den2 > 0.0f)) return false;
   const float k = (2.0f * cross) / sqrtf(den2);
-  if (!(fabsf(k) <= c.t3_kappa_max)) return false;
+  bool ok = (den2 > 0.0f) & (fabsf(k) <= c.t3_kappa_max);
   // T3
   const float d31 = p3.w - p1.w;
-  if (!(d31 > 0.0f)) return false;
   const float w1 = (p3.w - p2.w) / d31;
   const float w3 = (p2.w - p1.w) / d31;
   const float delta = (p2.z - p1.z) - w3 * (p3.z - p1.z);
   const float var = (c.sigma_z2[layer1 + 1] + (w1 * w1) * c.sigma_z2[layer1]) + (w3 * w3) * c.sigma_z2[layer1 + 2];
   const float chi2 = (delta * delta) / var;
-  if (!(chi2 <= c.t3_chi2rz_max[layer1])) return false;
+  ok = ok & (d31 > 0.0f) & (chi2 <= c.t3_chi2rz_max[layer1]);
   kappa = k;
   chi2rz = chi2;
-  return true;
+  return ok;
 }
 
 // ---- [Q] quintuplet ---------------------------------------------------------
