@@ -136,9 +136,10 @@ struct T5Out {
 };
 __device__ __forceinline__ bool t5_select(const Cuts& c, int layer1, float kappaA, float kappaB,
                                           const float4 (&p)[5], T5Out& o) {
+  // no early return (see seg_select): the tests are combined at the end
   // Q2
   const float dk = fabsf(kappaA - kappaB);
-  if (!(dk <= c.t5_dkappa_max)) return false;
+  bool ok = dk <= c.t5_dkappa_max;
   // Q3: weighted straight line z = a + b r through the five anchors, relative to anchor 2
   float chi2rz;
   {
@@ -159,7 +160,7 @@ __device__ __forceinline__ bool t5_select(const Cuts& c, int layer1, float kappa
       Srz = Srz + (w[i] * rho[i]) * zeta[i];
     }
     const float D = Sw * Srr - Sr * Sr;
-    if (!(D > 0.0f)) return false;
+    ok = ok & (D > 0.0f);
     const float b = (Sw * Srz - Sr * Sz) / D;
     const float a = (Sz - b * Sr) / Sw;
     float chi2 = 0.0f;
@@ -168,13 +169,13 @@ __device__ __forceinline__ bool t5_select(const Cuts& c, int layer1, float kappa
       const float e = zeta[i] - (a + b * rho[i]);
       chi2 = chi2 + w[i] * (e * e);
     }
-    if (!(chi2 <= c.t5_chi2rz_max[layer1])) return false;
+    ok = ok & (chi2 <= c.t5_chi2rz_max[layer1]);
     chi2rz = chi2;
   }
   // Q4: circle fit in the chord frame, lengths scaled by 1/32
   float ex = p[4].x - p[0].x, ey = p[4].y - p[0].y;
   const float len = sqrtf(ex * ex + ey * ey);
-  if (!(len > 0.0f)) return false;
+  ok = ok & (len > 0.0f);
   ex = ex / len;
   ey = ey / len;
   float u[5], v[5], q[5];
@@ -206,7 +207,7 @@ __device__ __forceinline__ bool t5_select(const Cuts& c, int layer1, float kappa
   const float c12 = Squ * Sq - Sqq * Su;
   const float c22 = Sqq * Suu - Squ * Squ;
   const float det = (Sqq * c00 + Squ * c01) + Sq * c02;
-  if (!(det > 0.0f)) return false;
+  ok = ok & (det > 0.0f);
   const float A = ((c00 * Sqv + c01 * Suv) + c02 * Sv) / det;
   const float B = ((c01 * Sqv + c11 * Suv) + c12 * Sv) / det;
   const float C = ((c02 * Sqv + c12 * Suv) + c22 * Sv) / det;
@@ -217,16 +218,15 @@ __device__ __forceinline__ bool t5_select(const Cuts& c, int layer1, float kappa
     ss = ss + e * e;
   }
   const float chi2xy = ss / c.t5_sigma_xy2_scaled;
-  if (!(chi2xy <= c.t5_chi2xy_max)) return false;
+  ok = ok & (chi2xy <= c.t5_chi2xy_max);
   // Q5
   const float disc = (1.0f + B * B) - (4.0f * A) * C;
-  if (!(disc > 0.0f)) return false;
   const float kfit = ((2.0f * A) / sqrtf(disc)) * 0.03125f;
-  if (!(fabsf(kfit) <= c.t5_kappa_max)) return false;
+  ok = ok & (disc > 0.0f) & (fabsf(kfit) <= c.t5_kappa_max);
   o.kfit = kfit;
   o.chi2xy = chi2xy;
   o.chi2rz = chi2rz;
-  return true;
+  return ok;
 }
 
 // ---- [P] pixel line segment + outer object -------------------------------
@@ -241,11 +241,12 @@ template <int N>
 __device__ __forceinline__ bool pix_select(const Cuts& c, int kind, int layer1, float kappa, float cphi, float sphi,
                                            float z0, float t, float kobj, const float4 (&p)[N], PixOut& o) {
   const float hk = 0.5f * kappa;
+  // no early return (see seg_select)
   // P0: the first anchor lies ahead of the seed (the outgoing arc of the circle)
-  if (!(p[0].x * cphi + p[0].y * sphi > 0.0f)) return false;
+  bool ok = p[0].x * cphi + p[0].y * sphi > 0.0f;
   // P1
   const float dk = kobj - kappa;
-  if (!(fabsf(dk) <= c.pix_dkappa_max[kind])) return false;
+  ok = ok & (fabsf(dk) <= c.pix_dkappa_max[kind]);
   // P2: distance of the anchors from the seed's circle through the beam line
   float chi2xy = 0.0f;
 #pragma unroll
@@ -253,7 +254,7 @@ __device__ __forceinline__ bool pix_select(const Cuts& c, int kind, int layer1, 
     const float e = (hk * (p[i].w * p[i].w) + p[i].x * sphi) - p[i].y * cphi;
     chi2xy = chi2xy + (e * e) * c.pix_inv_var_xy[layer1 + i];
   }
-  if (!(chi2xy <= c.pix_chi2xy_max[kind])) return false;
+  ok = ok & (chi2xy <= c.pix_chi2xy_max[kind]);
   // P3: distance of the anchors from the seed's line z = z0 + t s, s = arc length by its power series in (kappa r / 2)^2
   float chi2rz = 0.0f;
 #pragma unroll
@@ -264,11 +265,11 @@ __device__ __forceinline__ bool pix_select(const Cuts& c, int kind, int layer1, 
     const float d = (p[i].z - z0) - t * s;
     chi2rz = chi2rz + (d * d) * c.pix_inv_var_rz[layer1 + i];
   }
-  if (!(chi2rz <= c.pix_chi2rz_max[kind])) return false;
+  ok = ok & (chi2rz <= c.pix_chi2rz_max[kind]);
   o.chi2xy = chi2xy;
   o.chi2rz = chi2rz;
   o.dk = dk;
-  return true;
+  return ok;
 }
 
 }  // namespace lst
