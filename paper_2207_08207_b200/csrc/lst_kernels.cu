@@ -922,17 +922,13 @@ __device__ __forceinline__ int seg_walk(const Params& P, const Slot& S, SegWarp&
   AEntry cur = loadA(0);
   for (int t = 0; t < max_nt; ++t) {
 
-    bool keep = false;
-    float c0 = 0.0f;
-    if (t < nt) {
-      const int4 info = cur.info;
-      const float dlo = sh.dlo[lane], dhi = sh.dhi[lane];
-      if (info.y > info.x && dlo <= dhi) {
-        c0 = sh.key[lane] + cur.dphi;
-        keep = !(fabsf(c0) + fmaxf(fabsf(dlo), fabsf(dhi)) < 3.0f) ||
-               (c0 + dhi >= __int_as_float(info.z) && c0 + dlo <= __int_as_float(info.w));
-      }
-    }
+    // no branches (an entry beyond the lane's run is all zeros: an empty module)
+    const int4 info = cur.info;
+    const float dlo = sh.dlo[lane], dhi = sh.dhi[lane];
+    const float c0 = sh.key[lane] + cur.dphi;
+    const bool wrap = !(fabsf(c0) + fmaxf(fabsf(dlo), fabsf(dhi)) < 3.0f);
+    const bool meets = (c0 + dhi >= __int_as_float(info.z)) & (c0 + dlo <= __int_as_float(info.w));
+    const bool keep = (t < nt) & (info.y > info.x) & (dlo <= dhi) & (wrap | meets);
     const unsigned bal = __ballot_sync(kFull, keep);
     if (keep) sh.pq[(pt + __popc(bal & lanemask_lt())) & (kQueue - 1)] = make_int2((lane << 26) | cur.tgt, __float_as_int(c0));
     pt += __popc(bal);
