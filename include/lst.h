@@ -282,7 +282,10 @@ LST_API int lst_load_events(lst_ctx* ctx, int first_slot, int n_slots, const lst
 
 /* [P] Loads the pixel line segments of slots first_slot .. first_slot+n_slots-1 (seeds[b] into slot first_slot + b) and
  * orders them for the search (one kernel per 16 events).  Call it AFTER lst_load_event(s) of the same slots, on the same
- * stream (loading hits resets the slot, its seeds included).  Asynchronous.
+ * stream (loading hits resets the slot, its seeds included).  Asynchronous.  The ordering kernel is forked onto a stream of
+ * the library's own (after the work already enqueued on `cuda_stream`) so that it runs beside the stage kernels; LST_PIXEL,
+ * lst_sync* and the next lst_load_event(s) of the slot join it again -- inside a stream capture one of them has to follow in the
+ * same capture.
  * Errors: LST_ERR_ARG, LST_ERR_STATE (slot not loaded), LST_ERR_OVERFLOW (n > cap_seeds). */
 LST_API int lst_load_seeds(lst_ctx* ctx, int first_slot, int n_slots, const lst_seeds* seeds, void* cuda_stream);
 

@@ -39,6 +39,8 @@ struct SlotHost {
   SlotHeader* hdr = nullptr;  // pinned host copy of the device header
   bool seeds_loaded = false, pixel_run = false;   // [P]: lst_load_seeds since the last lst_load_event; LST_PIXEL since then
   int n_seeds_in = 0;
+  int seed_owner = -1;        // >= 0: the seed binning of this slot runs on a side stream and has not been joined yet; the slot whose seed_done event marks its end
+  cudaEvent_t seed_fork = nullptr, seed_done = nullptr;
   cudaEvent_t ev[22] = {};    // timing mode: ev[0..3] around the 3 a0 kernels, ev[4 + 2 s], ev[5 + 2 s] around stage s, ev[12..16] around the 4 cleaning steps, ev[17..18] around k_seed_bin, ev[19..21] around the two link kernels
   bool ev_bin = false, ev_stage[5] = {false, false, false, false, false}, ev_seed = false, ev_pix = false;
 };
@@ -66,6 +68,11 @@ struct lst_ctx {
   cudaEvent_t stage_ev[kStageEvents] = {};
   unsigned stage_next = 0;
   std::mutex stage_mu;
+  // [P] The seed binning (one latency-bound block per event) depends on nothing but the slot's fresh header, and only the link
+  // kernels need it: lst_load_seeds forks it onto one of these streams so that it runs beside a0 .. a4 of the same batch, and
+  // LST_PIXEL (or the next load / sync of the slot) joins it.
+  static constexpr int kSeedStreams = 4;
+  cudaStream_t seed_stream[kSeedStreams] = {};
   std::atomic<long long> launches{0};
   std::atomic<int> last_cuda{0};
 };
@@ -156,6 +163,22 @@ bool mapped_host(HitInput& in) {
 }
 
 bool valid_slot(const lst_ctx* c, int slot) { return c && slot >= 0 && slot < (int)c->slots.size(); }
+
+// Makes `s` wait for the seed binning of slots first .. first + n - 1 that still runs on a side stream (one wait per batch).
+cudaError_t join_seeds(lst_ctx* c, int first, int n, cudaStream_t s) {
+  int last_owner = -1;
+  for (int k = first; k < first + n; ++k) {
+    SlotHost& sh = c->slots[k];
+    if (sh.seed_owner < 0) continue;
+    if (sh.seed_owner != last_owner) {
+      const cudaError_t e = cudaStreamWaitEvent(s, c->slots[sh.seed_owner].seed_done, 0);
+      if (e != cudaSuccess) return e;
+      last_owner = sh.seed_owner;
+    }
+    sh.seed_owner = -1;
+  }
+  return cudaSuccess;
+}
 
 void copy_cuts(Cuts& d, const lst_config& s) {
   d.half_kappa_max = s.half_kappa_max; d.z_lum = s.z_lum;
@@ -317,9 +340,13 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
     for (auto& ev : c->stage_ev)
       if ((e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   }
+  for (auto& st : c->seed_stream)
+    if ((e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   c->slots.resize(cfg.n_slots);
   for (int s = 0; s < cfg.n_slots; ++s) {
     c->slots[s].hdr = c->pinned + s;
+    if ((e = cudaEventCreateWithFlags(&c->slots[s].seed_fork, cudaEventDisableTiming)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
+    if ((e = cudaEventCreateWithFlags(&c->slots[s].seed_done, cudaEventDisableTiming)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
     if (cfg.timing)
       for (auto& ev : c->slots[s].ev)
         if ((e = cudaEventCreate(&ev)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
@@ -352,9 +379,14 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
 int lst_destroy(lst_ctx* c) {
   if (!c) return LST_ERR_ARG;
   cudaSetDevice(c->device);
-  for (auto& s : c->slots)
+  for (auto& s : c->slots) {
     for (auto& ev : s.ev)
       if (ev) cudaEventDestroy(ev);
+    if (s.seed_fork) cudaEventDestroy(s.seed_fork);
+    if (s.seed_done) cudaEventDestroy(s.seed_done);
+  }
+  for (auto& st : c->seed_stream)
+    if (st) cudaStreamDestroy(st);
   for (auto& ev : c->stage_ev)
     if (ev) cudaEventDestroy(ev);
   if (c->stage_stream) cudaStreamDestroy(c->stage_stream);
@@ -379,6 +411,7 @@ int lst_load_events(lst_ctx* c, int first, int n_ev, const lst_hits* hits, void*
   }
   cudaStream_t s = (cudaStream_t)stream;
   LST_CUDA(c, cudaSetDevice(c->device));
+  LST_CUDA(c, join_seeds(c, first, n_ev, s));   // a seed binning still in flight on these slots must not meet the new header
   const Layout& L = c->P.L;
   for (int b0 = 0; b0 < n_ev; b0 += kMaxBatch) {
     const int nb = n_ev - b0 < kMaxBatch ? n_ev - b0 : kMaxBatch;
@@ -466,6 +499,7 @@ int lst_run_stage(lst_ctx* c, int first, int n, int stage, void* stream) {
   Params P = c->P;
   P.first_slot = first;
   if (stage == LST_PIXEL) {   // beside the linear chain: stages_run stays
+    LST_CUDA(c, join_seeds(c, first, n, st));
     c->launches += launch_pixel(P, n, st, c->cfg.timing ? sh.ev + 19 : nullptr);
     LST_CUDA(c, cudaGetLastError());
     sh.ev_pix = c->cfg.timing != 0;
@@ -522,10 +556,18 @@ int lst_load_seeds(lst_ctx* c, int first, int n_ev, const lst_seeds* seeds, void
     Params P = c->P;
     P.first_slot = first + b0;
     SlotHost& s0 = c->slots[first + b0];
-    c->launches += launch_seed_bin(P, src, nb, s, c->cfg.timing ? s0.ev + 17 : nullptr);
+    LST_CUDA(c, join_seeds(c, first + b0, nb, s));   // seeds loaded twice: the earlier binning first
+    cudaStream_t side = c->seed_stream[((first + b0) / kMaxBatch) % lst_ctx::kSeedStreams];
+    LST_CUDA(c, cudaEventRecord(s0.seed_fork, s));
+    LST_CUDA(c, cudaStreamWaitEvent(side, s0.seed_fork, 0));
+    c->launches += launch_seed_bin(P, src, nb, side, c->cfg.timing ? s0.ev + 17 : nullptr);
     LST_CUDA(c, cudaGetLastError());
+    LST_CUDA(c, cudaEventRecord(s0.seed_done, side));
     s0.ev_seed = c->cfg.timing != 0;
-    for (int b = 0; b < nb; ++b) c->slots[first + b0 + b].seeds_loaded = true;
+    for (int b = 0; b < nb; ++b) {
+      c->slots[first + b0 + b].seeds_loaded = true;
+      c->slots[first + b0 + b].seed_owner = first + b0;
+    }
   }
   return LST_OK;
 }
@@ -546,6 +588,7 @@ int lst_sync(lst_ctx* c, int slot, void* stream) {
   if (!sh.loaded) return LST_ERR_STATE;
   cudaStream_t s = (cudaStream_t)stream;
   LST_CUDA(c, cudaSetDevice(c->device));
+  LST_CUDA(c, join_seeds(c, slot, 1, s));
   const char* base = c->arena + (size_t)slot * c->P.slot_stride;
   LST_CUDA(c, cudaMemcpyAsync(sh.hdr, base + c->P.L.hdr, sizeof(SlotHeader), cudaMemcpyDeviceToHost, s));
   LST_CUDA(c, cudaStreamSynchronize(s));
@@ -726,6 +769,7 @@ int lst_sync_batch(lst_ctx* c, int first, int n, void* stream) {
     if (!c->slots[s].loaded) return LST_ERR_STATE;
   cudaStream_t st = (cudaStream_t)stream;
   LST_CUDA(c, cudaSetDevice(c->device));
+  LST_CUDA(c, join_seeds(c, first, n, st));
   // the n headers in ONE strided copy: they sit slot_stride apart on the device, contiguous in the pinned mirror
   LST_CUDA(c, cudaMemcpy2DAsync(c->pinned + first, sizeof(SlotHeader), c->arena + (size_t)first * c->P.slot_stride + c->P.L.hdr,
                                 c->P.slot_stride, sizeof(SlotHeader), (size_t)n, cudaMemcpyDeviceToHost, st));
