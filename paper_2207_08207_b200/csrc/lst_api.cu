@@ -56,6 +56,8 @@ struct lst_ctx {
   int* d_map_offsets = nullptr;
   int* d_map_targets = nullptr;
   float* d_map_dphi = nullptr;
+  int* d_map_targets_asc = nullptr;   // the rows as the caller gave them (ascending target), with their azimuth offsets
+  float* d_map_dphi_asc = nullptr;
   char* arena = nullptr;
   size_t arena_bytes = 0;
   std::vector<SlotHost> slots;
@@ -276,6 +278,7 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
   const int n_conn = m->row_offsets[n];
   std::vector<float> map_dphi((size_t)n_conn + 1, 0.0f);
   std::vector<int> map_tgt((size_t)n_conn + 1, 0);   // rows re-ordered by (azimuth offset, target) for the segment kernel
+  std::vector<float> map_dphi_asc((size_t)n_conn + 1, 0.0f);   // offsets in the caller's order (ascending target)
   std::vector<float2> mod_cs(n);
   for (int a = 0; a < n; ++a) {
     if (!std::isfinite(g->phi[a])) return LST_ERR_ARG;
@@ -290,6 +293,7 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
       if (d > kPi) d -= 2.0 * kPi;
       if (d <= -kPi) d += 2.0 * kPi;
       map_dphi[k] = (float)d;
+      map_dphi_asc[k] = (float)d;
       map_tgt[k] = t;
     }
     // insertion sort of the row (at most kMaxRow entries) by (azimuth offset, target)
@@ -324,12 +328,16 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
   if ((e = cudaMalloc(&c->d_map_offsets, sizeof(int) * (n + 1))) != cudaSuccess) return bail(LST_ERR_NOMEM, e);
   if ((e = cudaMalloc(&c->d_map_targets, sizeof(int) * ((size_t)n_conn + 1))) != cudaSuccess) return bail(LST_ERR_NOMEM, e);
   if ((e = cudaMalloc(&c->d_map_dphi, sizeof(float) * ((size_t)n_conn + 1))) != cudaSuccess) return bail(LST_ERR_NOMEM, e);
+  if ((e = cudaMalloc(&c->d_map_targets_asc, sizeof(int) * ((size_t)n_conn + 1))) != cudaSuccess) return bail(LST_ERR_NOMEM, e);
+  if ((e = cudaMalloc(&c->d_map_dphi_asc, sizeof(float) * ((size_t)n_conn + 1))) != cudaSuccess) return bail(LST_ERR_NOMEM, e);
   if ((e = cudaMalloc(&c->arena, c->arena_bytes)) != cudaSuccess) { cudaGetLastError(); return bail(LST_ERR_NOMEM, e); }
   if ((e = cudaMemcpy(c->d_layer, g->layer, n, cudaMemcpyHostToDevice)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   if ((e = cudaMemcpy(c->d_mod_cs, mod_cs.data(), sizeof(float2) * n, cudaMemcpyHostToDevice)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   if ((e = cudaMemcpy(c->d_map_offsets, m->row_offsets, sizeof(int) * (n + 1), cudaMemcpyHostToDevice)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   if (n_conn > 0 && (e = cudaMemcpy(c->d_map_targets, map_tgt.data(), sizeof(int) * (size_t)n_conn, cudaMemcpyHostToDevice)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   if (n_conn > 0 && (e = cudaMemcpy(c->d_map_dphi, map_dphi.data(), sizeof(float) * (size_t)n_conn, cudaMemcpyHostToDevice)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
+  if (n_conn > 0 && (e = cudaMemcpy(c->d_map_targets_asc, m->targets, sizeof(int) * (size_t)n_conn, cudaMemcpyHostToDevice)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
+  if (n_conn > 0 && (e = cudaMemcpy(c->d_map_dphi_asc, map_dphi_asc.data(), sizeof(float) * (size_t)n_conn, cudaMemcpyHostToDevice)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   if ((e = cudaMemset(c->arena, 0, c->arena_bytes)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   if ((e = cudaMallocHost(&c->pinned, sizeof(SlotHeader) * (size_t)cfg.n_slots)) != cudaSuccess) return bail(LST_ERR_CUDA, e);
   std::memset(c->pinned, 0, sizeof(SlotHeader) * (size_t)cfg.n_slots);
@@ -360,6 +368,8 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
   c->P.map_offsets = c->d_map_offsets;
   c->P.map_targets = c->d_map_targets;
   c->P.map_dphi = c->d_map_dphi;
+  c->P.map_targets_asc = c->d_map_targets_asc;
+  c->P.map_dphi_asc = c->d_map_dphi_asc;
   c->P.first_slot = 0;
   c->P.dup_min_shared = cfg.t5_dup_min_shared;
   c->P.store_half = cfg.store_half != 0;
@@ -393,6 +403,8 @@ int lst_destroy(lst_ctx* c) {
   if (c->pinned) cudaFreeHost(c->pinned);
   if (c->arena) cudaFree(c->arena);
   if (c->d_map_dphi) cudaFree(c->d_map_dphi);
+  if (c->d_map_dphi_asc) cudaFree(c->d_map_dphi_asc);
+  if (c->d_map_targets_asc) cudaFree(c->d_map_targets_asc);
   if (c->d_map_targets) cudaFree(c->d_map_targets);
   if (c->d_map_offsets) cudaFree(c->d_map_offsets);
   if (c->d_mod_cs) cudaFree(c->d_mod_cs);

@@ -118,6 +118,8 @@ struct Params {
   const int* map_offsets;        // [n_modules + 1] module map, CSR
   const int* map_targets;        // [map_offsets[n_modules]] rows ordered by (map_dphi, target): the entries an inner MD can reach are one run
   const float* map_dphi;         // [map_offsets[n_modules]] azimuth(source normal) - azimuth(target normal), in (-pi, pi], ascending per row
+  const int* map_targets_asc;    // the same rows ordered by target (k_seg's direct walk: segments arrive in CSR order)
+  const float* map_dphi_asc;     // azimuth offsets in that order
   int first_slot;
   int dup_min_shared;            // [D] D4: quintuplets sharing at least this many original hits are duplicates
   int store_half;                // [H] output floats that no selection reads are stored as binary16

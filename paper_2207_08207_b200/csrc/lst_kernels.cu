@@ -912,8 +912,9 @@ __device__ __forceinline__ int seg_walk(const Params& P, const Slot& S, SegWarp&
     e.dphi = 0.0f;
     e.info = make_int4(0, 0, 0, 0);
     if (t < nt) {
-      e.tgt = P.map_targets[row0 + t];
-      e.dphi = P.map_dphi[row0 + t];
+      // the direct walk reads the row in ascending target order: its segments arrive in CSR order
+      e.tgt = (DIRECT ? P.map_targets_asc : P.map_targets)[row0 + t];
+      e.dphi = (DIRECT ? P.map_dphi_asc : P.map_dphi)[row0 + t];
       e.info = mod_info[e.tgt];
     }
     return e;
@@ -1002,9 +1003,10 @@ __global__ void __launch_bounds__(kSegWarps * 32, 7) k_seg(const __grid_constant
         seg_emit(P, S, base + sh.tab[ol] + sh.stR[b][t], i0 + ol, v & (kMaxCap - 1), f.x, f.y);
       }
     // An owner's segments were found in the order of its row (by azimuth offset), not by outer MD: the owner lane puts its
-    // one to three segments in ascending outer MD (insertion sort of the stored records; the other lanes' stores first)
+    // one to three segments in ascending outer MD (insertion sort of the stored records; the other lanes' stores first).
+    // A chunk written by the direct walk is in order already (it reads the rows by ascending target).
     __syncwarp();
-    {
+    if (from_stash) {
       const int mine = sh.cnt[b][lane];
       const int lo = min(base + ex, cap), hi = min(base + ex + mine, cap);
       int2* smd = S.seg_md();
@@ -1095,7 +1097,15 @@ __global__ void __launch_bounds__(kSegWarps * 32, 7) k_seg(const __grid_constant
       sh.tab[lane] = warp_excl_scan(sh.cnt[buf][lane], tot);
       sh.cnt[buf ^ 1][lane] = 0;
       __syncwarp();
-      seg_walk<true>(P, S, sh, buf, nt, row0, i0, base, evals);
+      // over the WHOLE row in ascending target order (the reachable run is a run of the row ordered by azimuth offset only):
+      // an owner's segments then arrive by ascending outer MD and need no sort -- a chunk of a dense event holds thousands
+      int nt_all = 0, row_all = 0;
+      if (i < nMD && nt > 0) {
+        const int A = S.md_module()[i];
+        row_all = P.map_offsets[A];
+        nt_all = P.map_offsets[A + 1] - row_all;
+      }
+      seg_walk<true>(P, S, sh, buf, nt_all, row_all, i0, base, evals);
       finish(C, buf, total, base, false);
     }
   }
