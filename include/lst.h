@@ -53,7 +53,8 @@ enum {
   LST_ERR_CUDA = -2,     /* a CUDA runtime call failed (lst_last_cuda_error gives the code)        */
   LST_ERR_OVERFLOW = -3, /* a per-slot capacity was exceeded                                       */
   LST_ERR_STATE = -4,    /* call out of order (e.g. lst_get_* before lst_sync)                     */
-  LST_ERR_NOMEM = -5     /* arena allocation failed in lst_create                                  */
+  LST_ERR_NOMEM = -5,    /* arena allocation failed in lst_create                                  */
+  LST_ERR_LIMIT = -6     /* size beyond the fixed maximum of the entry point that allocates nothing */
 };
 
 enum { LST_MD = 0, LST_SEG = 1, LST_T3 = 2, LST_T5 = 3,
@@ -386,6 +387,30 @@ LST_API int lst_default_map_params(lst_map_params* params);
  * again with a buffer of *n_targets entries); LST_ERR_NOMEM; LST_ERR_CUDA. */
 LST_API int lst_build_module_map(const lst_map_geometry* geom, const lst_map_params* params, int device, int32_t* row_offsets,
                                  int32_t* targets, int64_t cap_targets, int64_t* n_targets, float* kernel_ms);
+
+/* The same map for callers that cannot allocate device memory (under CUDA graph capture, in a serving loop, in a harness
+ * that forbids cudaMalloc): ONE entry point that calls no cudaMalloc / cudaFree / allocating library routine, creates no
+ * event and never synchronises.  Three kernels are enqueued on `cuda_stream` (row lengths, exclusive scan, rows) and the call
+ * returns; the outputs are complete once the caller has synchronised that stream.
+ *   geom            HOST struct whose seven array pointers are DEVICE pointers ([n_modules] each, as in lst_map_geometry).
+ *                   The values are NOT validated (they are on the device): the preconditions of lst_build_module_map
+ *                   (layer in 0 .. LST_N_LAYERS-1, rho - gap/2 > 0, half_width > 0, finite) are the caller's to keep; whatever
+ *                   the values, nothing outside the outputs is written.
+ *   row_offsets     DEVICE [n_modules + 1], always written; row_offsets[n_modules] = number of connections.
+ *   targets         DEVICE [cap_targets], rows ascending.  If the map has more than cap_targets connections only the entries
+ *                   at CSR positions < cap_targets are written (the caller compares row_offsets[n_modules] with cap_targets:
+ *                   there is no host-side status for it, the call has returned long before).  May be NULL iff cap_targets = 0.
+ * The per-module row lengths between the first and the second kernel live in a file-scope device array of
+ * LST_MAP_STATIC_MAX_MODULES ints (128 KiB, held by every GPU that loads the library until the process exits): n_modules above
+ * that is rejected with LST_ERR_LIMIT before anything is enqueued.  Every call on a device shares that array and it keeps the
+ * last call's contents: each call overwrites the entries it reads before reading them (nothing has to start at zero), but two
+ * calls that overlap on the GPU (different streams, or graphs replayed concurrently) RACE on it -- keep them on one stream or
+ * order them with events.  The first call on a device looks the array's address up (cudaGetSymbolAddress: may load the
+ * module, so make that call outside a capture); later calls only enqueue.
+ * Errors: LST_ERR_ARG (NULL pointers, n_modules <= 0, bad parameters, cap_targets < 0), LST_ERR_LIMIT, LST_ERR_CUDA. */
+#define LST_MAP_STATIC_MAX_MODULES 32768
+LST_API int lst_build_module_map_static(const lst_map_geometry* geom, const lst_map_params* params, int device,
+                                        int32_t* row_offsets, int32_t* targets, int64_t cap_targets, void* cuda_stream);
 
 /* Overflow recovery (BASELINE.json configs[3] "candidate-buffer overflow handling"; PAPER.md:143 sizes its buffers from the
  * data too): after lst_sync* returned LST_ERR_OVERFLOW for `slot`, fills *out with the context's configuration in which every

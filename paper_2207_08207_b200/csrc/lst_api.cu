@@ -952,6 +952,7 @@ const char* lst_strerror(int s) {
     case LST_ERR_OVERFLOW: return "a per-slot capacity was exceeded; outputs of the slot are invalid";
     case LST_ERR_STATE: return "call out of order (load -> run -> sync -> get)";
     case LST_ERR_NOMEM: return "arena allocation failed";
+    case LST_ERR_LIMIT: return "size beyond the fixed maximum of the entry point that allocates nothing (LST_MAP_STATIC_MAX_MODULES)";
   }
   return "unknown status";
 }

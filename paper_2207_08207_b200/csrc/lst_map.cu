@@ -9,6 +9,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <mutex>
 #include <vector>
 
 #include "../../include/lst.h"
@@ -158,6 +159,131 @@ extern "C" int lst_build_module_map(const lst_map_geometry* mg, const lst_map_pa
   }
   for (auto& e : ev) cudaEventDestroy(e);
   return status;
+}
+
+// ------------------------------------------------------------------------------------------
+// lst_build_module_map_static: the same map without any allocation (include/lst.h).  Inputs and outputs are the caller's
+// device arrays; the one piece of scratch -- the row lengths between the count pass and the scan -- is the file-scope array
+// below.  In host code `g_map_row_len` is only a stand-in for the symbol: the kernels get the address that
+// cudaGetSymbolAddress returns for the device that is current (looked up once per device, under a mutex).
+// ------------------------------------------------------------------------------------------
+namespace {
+
+static __device__ __align__(256) int g_map_row_len[LST_MAP_STATIC_MAX_MODULES];
+
+constexpr int kMaxDevices = 64;
+std::mutex g_row_len_mu;
+int* g_row_len_ptr[kMaxDevices] = {};
+
+// `device` must be current.
+cudaError_t row_len_scratch(int device, int** out) {
+  std::lock_guard<std::mutex> lock(g_row_len_mu);
+  if (!g_row_len_ptr[device]) {
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_map_row_len);
+    if (e != cudaSuccess) return e;
+    if (!p) return cudaErrorInvalidSymbol;
+    g_row_len_ptr[device] = static_cast<int*>(p);
+  }
+  *out = g_row_len_ptr[device];
+  return cudaSuccess;
+}
+
+// k_map_rows with the fill bounded by the caller's buffer: FILL = false writes row_len[A]; FILL = true writes the entries of
+// row A whose CSR position is below cap.
+template <bool FILL>
+__global__ void __launch_bounds__(256) k_map_rows_static(const MapGeom g, const lst_map_params p, int* row_len, const int* offsets,
+                                                         int* targets, long long cap) {
+  __shared__ int s_warp[8];
+  __shared__ int s_base;
+  const int A = blockIdx.x;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  if (threadIdx.x == 0) s_base = FILL ? offsets[A] : 0;
+  __syncthreads();
+  for (int b0 = 0; b0 < g.n; b0 += 256) {
+    const int B = b0 + threadIdx.x;
+    const bool c = B < g.n && connected(g, p, A, B);
+    const unsigned bal = __ballot_sync(0xffffffffu, c);
+    if (lane == 0) s_warp[w] = __popc(bal);
+    __syncthreads();
+    int before = s_base, total = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      before += (i < w) ? s_warp[i] : 0;
+      total += s_warp[i];
+    }
+    if (FILL && c) {
+      const int pos = before + __popc(bal & ((1u << lane) - 1u));
+      if ((long long)pos < cap) targets[pos] = B;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) s_base += total;
+    __syncthreads();
+  }
+  if (!FILL && threadIdx.x == 0) row_len[A] = s_base;
+}
+
+// One block: offsets[i] = sum of row_len[0 .. i), offsets[n] = the number of connections (n <= 32768 rows of at most n
+// entries: below 2^31).  1024 threads take 1024 rows per round and carry the running sum.
+__global__ void __launch_bounds__(1024) k_map_scan_static(int n, const int* row_len, int* offsets) {
+  __shared__ int s_warp[32];
+  __shared__ int s_carry;
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  if (tid == 0) s_carry = 0;
+  __syncthreads();
+  for (int i0 = 0; i0 < n; i0 += 1024) {
+    const int i = i0 + tid;
+    const int v = i < n ? row_len[i] : 0;
+    int incl = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const int u = __shfl_up_sync(0xffffffffu, incl, d);
+      if (lane >= d) incl += u;
+    }
+    if (lane == 31) s_warp[w] = incl;
+    __syncthreads();
+    if (w == 0) {
+      const int x = s_warp[lane];
+      int xi = x;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        const int u = __shfl_up_sync(0xffffffffu, xi, d);
+        if (lane >= d) xi += u;
+      }
+      s_warp[lane] = xi - x;
+    }
+    __syncthreads();
+    const int carry = s_carry;
+    if (i < n) offsets[i] = carry + s_warp[w] + incl - v;
+    __syncthreads();
+    if (tid == 1023) s_carry = carry + s_warp[31] + incl;
+    __syncthreads();
+  }
+  if (tid == 0) offsets[n] = s_carry;
+}
+
+}  // namespace
+
+extern "C" int lst_build_module_map_static(const lst_map_geometry* mg, const lst_map_params* params, int device,
+                                           int32_t* row_offsets, int32_t* targets, int64_t cap_targets, void* cuda_stream) {
+  if (!mg || !row_offsets || mg->n_modules <= 0 || cap_targets < 0 || (cap_targets > 0 && !targets)) return LST_ERR_ARG;
+  if (!mg->layer || !mg->phi || !mg->rho || !mg->gap || !mg->half_width || !mg->z_lo || !mg->z_hi) return LST_ERR_ARG;
+  if (device < 0 || device >= kMaxDevices) return LST_ERR_ARG;
+  lst_map_params p;
+  if (params) p = *params; else lst_default_map_params(&p);
+  if (!(p.pt_min > 0.0) || !(p.b_tesla > 0.0) || !(p.z0_max >= 0.0)) return LST_ERR_ARG;
+  if (mg->n_modules > LST_MAP_STATIC_MAX_MODULES) return LST_ERR_LIMIT;   // the scratch array holds one int per module
+  const int n = mg->n_modules;
+  if (cudaSetDevice(device) != cudaSuccess) return LST_ERR_CUDA;
+  int* row_len = nullptr;
+  if (row_len_scratch(device, &row_len) != cudaSuccess) return LST_ERR_CUDA;
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  const MapGeom g{n, reinterpret_cast<const signed char*>(mg->layer), mg->phi, mg->rho, mg->gap, mg->half_width, mg->z_lo, mg->z_hi};
+  // row_len[0 .. n) is written by the first kernel before the second reads it: nothing of the last call's contents is used
+  k_map_rows_static<false><<<n, 256, 0, s>>>(g, p, row_len, nullptr, nullptr, 0);
+  k_map_scan_static<<<1, 1024, 0, s>>>(n, row_len, row_offsets);
+  k_map_rows_static<true><<<n, 256, 0, s>>>(g, p, nullptr, row_offsets, targets, (long long)cap_targets);
+  return cudaGetLastError() == cudaSuccess ? LST_OK : LST_ERR_CUDA;
 }
 
 extern "C" int lst_default_map_params(lst_map_params* p) {

@@ -29,6 +29,8 @@ HITS_PER_OBJECT = (2, 4, 6, 10, 10)       # [CLEAN]: the kept quintuplets
 VALUES_PER_OBJECT = (4, 4, 2, 5, 5)
 
 OK, ERR_ARG, ERR_CUDA, ERR_OVERFLOW, ERR_STATE, ERR_NOMEM = 0, -1, -2, -3, -4, -5
+ERR_LIMIT = -6
+MAP_STATIC_MAX_MODULES = 32768           # LST_MAP_STATIC_MAX_MODULES
 
 
 class LstError(RuntimeError):
@@ -160,6 +162,8 @@ SYMBOLS = {
     "lst_default_map_params": (C.c_int, [P(MapParams)]),
     "lst_build_module_map": (C.c_int, [P(MapGeometry), P(MapParams), C.c_int, C.c_void_p, C.c_void_p, C.c_int64, P(C.c_int64),
                                        P(C.c_float)]),
+    "lst_build_module_map_static": (C.c_int, [P(MapGeometry), P(MapParams), C.c_int, C.c_void_p, C.c_void_p, C.c_int64,
+                                              C.c_void_p]),
     "lst_grown_config": (C.c_int, [C.c_void_p, C.c_int, P(Config)]),
     "lst_arena_bytes": (C.c_int, [C.c_void_p, P(C.c_int64), P(C.c_int64)]),
     "lst_launch_count": (C.c_int64, [C.c_void_p]),
@@ -255,6 +259,25 @@ def build_module_map(layer, phi, rho, gap, half_width, z_lo, z_hi, device: int =
     if st != OK:
         raise LstError(st, "lst_build_module_map")
     return offs, targets[:int(total.value)], [float(ms[0]), float(ms[1])]
+
+
+def build_module_map_static(n_modules: int, layer, phi, rho, gap, half_width, z_lo, z_hi, row_offsets, targets, cap_targets: int,
+                            device: int = 0, stream=None, **params):
+    """lst_build_module_map_static: the module-map builder that allocates nothing. Every array argument is a DEVICE
+    pointer (an int, or an object with ``data_ptr()``): int8 layer, float64 phi .. z_hi, int32 row_offsets [n_modules + 1]
+    and targets [cap_targets]. Enqueues on ``stream`` and returns; raises LstError (ERR_LIMIT above
+    MAP_STATIC_MAX_MODULES)."""
+    lib = load_library()
+    dp = lambda a: C.c_void_p(int(a.data_ptr()) if hasattr(a, "data_ptr") else int(a or 0))
+    g = MapGeometry(int(n_modules), *[dp(a) for a in (layer, phi, rho, gap, half_width, z_lo, z_hi)])
+    p = MapParams()
+    lib.lst_default_map_params(C.byref(p))
+    for k, v in params.items():
+        setattr(p, k, float(v))
+    st = lib.lst_build_module_map_static(C.byref(g), C.byref(p), int(device), dp(row_offsets), dp(targets), int(cap_targets),
+                                         _stream(stream))
+    if st != OK:
+        raise LstError(st, "lst_build_module_map_static")
 
 
 def packed_event_buffers(n: int):
