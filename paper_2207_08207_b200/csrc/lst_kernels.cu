@@ -227,8 +227,10 @@ __device__ __forceinline__ void seg_window(const Cuts& c, int layer, float r_i, 
   }
   if (!(s_lo <= s_hi)) return;
   const float q_lo = fminf(1.0f, r_i / r_lo), q_hi = r_i / r_max_o;
-  const float hi = fmaxf(delta_of(s_hi, q_lo), delta_of(s_hi, q_hi));
-  const float lo = fminf(delta_of(s_lo, q_lo), delta_of(s_lo, q_hi));
+  // delta_of(s, q) falls with q for s > 0 and grows with q for s < 0 (d/dq = -s / sqrt(1 - q^2 s^2)): the extreme over
+  // q in [q_hi, q_lo] sits at the end the sign of s names, one evaluation per bound
+  const float hi = delta_of(s_hi, s_hi >= 0.0f ? q_hi : q_lo);
+  const float lo = delta_of(s_lo, s_lo >= 0.0f ? q_lo : q_hi);
   dlo = lo - (3e-5f + 1e-3f * fabsf(lo));
   dhi = hi + (3e-5f + 1e-3f * fabsf(hi));
 }
