@@ -34,6 +34,7 @@ import numpy as np  # noqa: E402
 METRIC = "events/sec at PU200-like density (1 B200)"
 UNIT = "events/s"
 N_EVENTS = 64
+NOMINAL_HBM_GBS = 8000.0           # the "about 8 TB/s" of BASELINE.json's north_star; fractions are reported against the measured peak AND this
 N_STREAMS = int(os.environ.get("LST_BENCH_STREAMS", "4"))   # BASELINE.json configs[2]: 4 streams (override: experiments only)
 # SURVEY.md 8(d) algorithmic bytes per unit (each input read once, each output written once)
 MAP_BYTES = 4 * (69630 + 6121)
@@ -419,7 +420,8 @@ def run_ours(args):
             "alu_tflops": spec_flops_step / (total_ms / args.steps * 1e-3) / 1e12, "alu_peak_tflops": alu_peak,
             "alu_frac": spec_flops_step / (total_ms / args.steps * 1e-3) / 1e12 / alu_peak,
             "hbm_gbs": sum(algorithmic_bytes(i, n_hits, needed) for i in range(5)) / (total_ms / args.steps * 1e-3) / 1e9,
-            "hbm_frac": sum(algorithmic_bytes(i, n_hits, needed) for i in range(5)) / (total_ms / args.steps * 1e-3) / 1e9 / peaks["hbm_gbs"]}
+            "hbm_frac": sum(algorithmic_bytes(i, n_hits, needed) for i in range(5)) / (total_ms / args.steps * 1e-3) / 1e9 / peaks["hbm_gbs"],
+            "hbm_frac_nominal": sum(algorithmic_bytes(i, n_hits, needed) for i in range(5)) / (total_ms / args.steps * 1e-3) / 1e9 / NOMINAL_HBM_GBS}
 
     # ---- the path followed by the optional duplicate-cleaning stage [D], same timing rules ----
     def step_device_clean():
@@ -736,6 +738,7 @@ def roofline(kernel_ms, alone_ms, n_hits, needed, cands, peaks, events_per_launc
         if not ms:
             return {"ms": ms}
         return {"ms": ms, "hbm_gbs": b / (ms * 1e-3) / 1e9, "hbm_frac": b / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                "hbm_frac_nominal": b / (ms * 1e-3) / 1e9 / NOMINAL_HBM_GBS,
                 "alu_tflops": fl / (ms * 1e-3) / 1e12, "alu_frac": fl / (ms * 1e-3) / 1e12 / alu_peak_tflops}
 
     per_stage = {}
@@ -759,6 +762,8 @@ def roofline(kernel_ms, alone_ms, n_hits, needed, cands, peaks, events_per_launc
                       "4-stream configuration (CUDA events on the launching stream), kernel_ms_alone = the same launch with the GPU "
                       "otherwise idle; achieved = algorithmic_bytes / kernel_ms",
             "alone": {"achieved": alo["hbm_gbs"], "frac": alo["hbm_frac"]},
+            "nominal": {"peak": NOMINAL_HBM_GBS, "frac": ins["hbm_frac_nominal"], "frac_alone": alo["hbm_frac_nominal"],
+                        "what": "the same against the nominal 8 TB/s BASELINE.json quotes (SURVEY 8(d) asks for both)"},
             "alu_view": {"what": "secondary bound: SPEC flops of the evaluated candidates / non-FMA fp32 peak", "spec_flops": int(fl),
                          "peak_tflops": alu_peak_tflops, "in_step": {"achieved_tflops": ins["alu_tflops"], "frac": ins["alu_frac"]},
                          "alone": {"achieved_tflops": alo["alu_tflops"], "frac": alo["alu_frac"]}},
@@ -821,7 +826,8 @@ def run_sweep(args):
             ms = sum(k_ms[k] for k in ks)
             b = algorithmic_bytes(stage, stt["n_hits"], need)
             per[name] = {"ms": ms, "algorithmic_bytes": int(b), "hbm_gbs": b / (ms * 1e-3) / 1e9,
-                         "hbm_frac": b / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"]}
+                         "hbm_frac": b / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                         "hbm_frac_nominal": b / (ms * 1e-3) / 1e9 / NOMINAL_HBM_GBS}
             if stage:
                 per[name].update(candidates=cand[stage - 1], evaluated=evl[stage - 1], passed=need[stage - 1],
                                  evaluated_per_s=evl[stage - 1] / (ms * 1e-3))
