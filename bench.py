@@ -192,7 +192,7 @@ def run_reference(args):
 def workload_config():
     return {"workload": "BASELINE.json configs[2]: 64 PU200-like events (configs[1] recipe, seeds 0..63), "
                         "4 CUDA streams x 16-event batched launches, arena reused",
-            "events_per_step": N_EVENTS, "streams": N_STREAMS, "geometry": "6-layer barrel, 6120 pT modules",
+            "events_per_step": N_EVENTS, "streams": N_STREAMS, "launches_in_flight_hint": N_STREAMS, "geometry": "6-layer barrel, 6120 pT modules",
             "l2": "explicit L2 flush (256 MiB memset) between timed steps, outside the timed intervals"}
 
 
@@ -220,6 +220,7 @@ def run_ours(args):
     per_stream = N_EVENTS // N_STREAMS
     cfg = lst.default_config()
     cfg.device, cfg.n_slots = local, 2 * N_EVENTS          # second half: the other buffer set of the end-to-end pipeline
+    cfg.launches_in_flight = N_STREAMS                    # the hint of include/lst.h: four batched launches side by side
     ctx = lst.Lst.from_synth(geom, mmap, cfg)
     streams = [torch.cuda.Stream(dev) for _ in range(N_STREAMS)]
     main = torch.cuda.current_stream(dev)
@@ -484,6 +485,7 @@ def run_ours(args):
     ctx.close()
     cfg_h = lst.default_config()
     cfg_h.device, cfg_h.n_slots, cfg_h.store_half = local, 2 * N_EVENTS, 1
+    cfg_h.launches_in_flight = N_STREAMS
     ctx_h = lst.Lst.from_synth(geom, mmap, cfg_h)
 
     def step_device_half():
@@ -643,6 +645,7 @@ def per_kernel_times(lst, geom, mmap, d_in, local, with_clean=False, reps=6, alo
     import torch
     cfg = lst.default_config()
     cfg.device, cfg.n_slots, cfg.timing, cfg.store_half = local, N_EVENTS, 1, int(store_half)
+    cfg.launches_in_flight = N_STREAMS
     ctx = lst.Lst.from_synth(geom, mmap, cfg)
     streams = [torch.cuda.Stream() for _ in range(N_STREAMS)]
     per = N_EVENTS // N_STREAMS

@@ -138,6 +138,12 @@ typedef struct {
   int32_t cap_seeds;  /* [P] per-slot capacities: pixel line segments (16 k), pixel triplets (64 k), pixel quintuplets (64 k) */
   int32_t cap_pt3;
   int32_t cap_pt5;
+  int32_t launches_in_flight; /* hint, >= 0: how many batched launches (lst_run_batch / lst_run_stage on different streams) the
+                         caller keeps running side by side.  0 .. 3 (default 0): every stage grid is sized for half of the
+                         machine, good for any use.  >= 4: the grids are sized so that FOUR launches of a stage together fill a
+                         whole number of residency waves (BASELINE.json configs[2], 4 streams x 16 events: +0.9 % events/s;
+                         a launch that runs alone, or two streams of 32 events, are then 15-50 % slower).  Results do not
+                         depend on it */
 } lst_config;
 
 /* Fills *cfg with the frozen SPEC constants, device 0, 4 slots and capacities that hold the

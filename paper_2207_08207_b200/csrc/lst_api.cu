@@ -247,6 +247,7 @@ int lst_default_config(lst_config* c) {
   c->timing = 0;
   c->t5_dup_min_shared = 7;
   c->store_half = 0;
+  c->launches_in_flight = 0;
   c->cap_seeds = 16 * 1024;
   c->cap_pt3 = 64 * 1024;
   c->cap_pt5 = 64 * 1024;
@@ -265,6 +266,7 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
   /* [D]: partners are found through a common mini-doublet, which two quintuplets sharing >= 6 of their 10 hits always
      have (five common layers with one common hit each give at most 5): smaller thresholds are refused, not approximated */
   if (cfg.t5_dup_min_shared < 6 || cfg.t5_dup_min_shared > 10) return LST_ERR_ARG;
+  if (cfg.launches_in_flight < 0) return LST_ERR_ARG;
   if (cfg.n_slots < 1 || cfg.cap_hits < 1 || cfg.cap_md < 1 || cfg.cap_seg < 1 || cfg.cap_t3 < 1 || cfg.cap_t5 < 1) return LST_ERR_ARG;
   if (cfg.cap_seeds < 1 || cfg.cap_pt3 < 1 || cfg.cap_pt5 < 1 || cfg.cap_seeds > kMaxCap || cfg.cap_pt3 > kMaxCap || cfg.cap_pt5 > kMaxCap) return LST_ERR_ARG;
   for (int i = 0; i < n; ++i)
@@ -373,6 +375,7 @@ int lst_create(const lst_geometry* g, const lst_module_map* m, const lst_config*
   c->P.first_slot = 0;
   c->P.dup_min_shared = cfg.t5_dup_min_shared;
   c->P.store_half = cfg.store_half != 0;
+  c->P.four_launches = cfg.launches_in_flight >= 4;
   for (int k = 0; k < 3; ++k) {  // are the modules of layers <= 1 / <= 3 / <= 4 a prefix of the module ids?
     const int max_layer = k == 0 ? 1 : k == 1 ? 3 : 4;
     int live = 0;

@@ -123,6 +123,7 @@ struct Params {
   int first_slot;
   int dup_min_shared;            // [D] D4: quintuplets sharing at least this many original hits are duplicates
   int store_half;                // [H] output floats that no selection reads are stored as binary16
+  int four_launches;             // lst_config.launches_in_flight >= 4: stage grids sized for four launches side by side (host side only)
   int live_modules[3];           // modules 0 .. live_modules[k]-1 are exactly those on layers <= 1 (k = 0) / <= 3 (k = 1) / <= 4 (k = 2) when the
                                  // module ids are ordered by layer, else n_modules: owners of the quintuplet and pixel / triplet / segment
                                  // kernel behind the corresponding CSR prefix have no candidates

@@ -2174,6 +2174,15 @@ constexpr int kGridShare = 2;
 // launch bounds (those set the register budget).  Segment kernel 4 / 5 / 6 / 7 / 8: 46.0 / 50.0 / 51.2 / 47.8 / 49.0 k events/s;
 // the others are flat within 1 % (MD 5, T3 5, T5 6 together: 51.2 -> 51.6 k).
 constexpr int kMdGrid = 5, kSegGrid = 6, kT3Grid = 5, kT5Grid = 6;
+// lst_config.launches_in_flight >= 4 (Params::four_launches): the caller runs FOUR launches side by side, and the four streams do
+// best in the same stage at the same time (profiles/r2_summary.md).  What counts is then whether the four launches of a stage
+// TOGETHER fill a whole number of residency waves: waves x (148 SMs x resident blocks per SM) / (4 launches x events per launch).
+//   k_seg  7 resident blocks per SM (1 036 slots), ONE wave: 16 blocks per event of a 16-event launch, 4 x 256 = 1 024 blocks
+//   k_md, k_t3  6 per SM (888 slots), two waves: 27 per event, 4 x 432 = 1 728 <= 1 776;  k_t5 4 per SM, three waves: 27 per event
+// Same-box sweep of the blocks per event (events/s, 4 x 16 events): k_seg 12 / 14 / 15 / 16 | 24 / 26 / 27 / 28 / 29 / 32 = 57.8 / 60.6 /
+// 61.6 / 62.2 | 60.6 / 61.4 / 61.9 / 61.9 / 60.0 / 57.9 k (17 and 29 spill into a partial wave); with k_seg at 16, k_md + k_t3
+// 13 / 23 / 27 / 41 = 61.7 / 62.1 / 62.5 / 61.4 k.  Alone such a k_seg launch takes 0.29 ms instead of 0.19: hence a hint, not the default.
+constexpr int kMdGrid4 = 6, kSegGrid4 = 7, kT3Grid4 = 6, kSegShare4 = 4;
 static int blocks_per_event(int wanted, int n_batch, int resident_per_sm, int share = 1) {
   const int per_event = max(8, 148 * resident_per_sm / (n_batch * share));
   return max(1, min(wanted, per_event));
@@ -2213,14 +2222,14 @@ int launch_stage(const Params& P, int n_batch, int stage, cudaStream_t s, cudaEv
   LST_EV(0);
   switch (stage) {
     case LST_MD_:
-      k_md<<<dim3(blocks_per_event((P.L.n_chunk[0] + kWarps - 1) / kWarps, n_batch, kMdGrid, kGridShare), nb), kWarps * 32, 0, s>>>(P);
+      k_md<<<dim3(blocks_per_event((P.L.n_chunk[0] + kWarps - 1) / kWarps, n_batch, P.four_launches ? kMdGrid4 : kMdGrid, kGridShare), nb), kWarps * 32, 0, s>>>(P);
       break;
     case LST_SEG_:
       // (a module-owner walk with a flat on-chip key-window compare was built and measured in round 2: it lost, profiles/r2_seg_ab.md)
-      k_seg<<<dim3(blocks_per_event((P.L.n_chunk[1] + kSegWarps - 1) / kSegWarps, n_batch, kSegGrid, kGridShare), nb), kSegWarps * 32, 0, s>>>(P);
+      k_seg<<<dim3(blocks_per_event((P.L.n_chunk[1] + kSegWarps - 1) / kSegWarps, n_batch, P.four_launches ? kSegGrid4 : kSegGrid, P.four_launches ? kSegShare4 : kGridShare), nb), kSegWarps * 32, 0, s>>>(P);
       break;
     case LST_T3_:
-      k_t3<<<dim3(blocks_per_event((P.L.n_chunk[2] + kWarps - 1) / kWarps, n_batch, kT3Grid, kGridShare), nb), kWarps * 32, 0, s>>>(P);
+      k_t3<<<dim3(blocks_per_event((P.L.n_chunk[2] + kWarps - 1) / kWarps, n_batch, P.four_launches ? kT3Grid4 : kT3Grid, kGridShare), nb), kWarps * 32, 0, s>>>(P);
       break;
     case LST_T5_:
       k_t5<<<dim3(blocks_per_event((P.L.n_chunk[3] + kWarps - 1) / kWarps, n_batch, kT5Grid, kGridShare), nb), kWarps * 32, 0, s>>>(P);

@@ -61,7 +61,8 @@ class Config(C.Structure):
                 ("device", C.c_int32), ("n_slots", C.c_int32), ("cap_hits", C.c_int32), ("cap_md", C.c_int32),
                 ("cap_seg", C.c_int32), ("cap_t3", C.c_int32), ("cap_t5", C.c_int32), ("timing", C.c_int32),
                 ("store_half", C.c_int32), ("t5_dup_min_shared", C.c_int32),
-                ("cap_seeds", C.c_int32), ("cap_pt3", C.c_int32), ("cap_pt5", C.c_int32)]
+                ("cap_seeds", C.c_int32), ("cap_pt3", C.c_int32), ("cap_pt5", C.c_int32),
+                ("launches_in_flight", C.c_int32)]
 
     CUT_FIELDS = ("half_kappa_max", "z_lum", "md_cos_eps", "md_sin_eps", "md_dz_res", "md_eps", "seg_cos_eps",
                   "seg_sin_eps", "seg_z0_max", "t3_kappa_max", "t3_chi2rz_max", "sigma_z2", "inv_sigma_z2",

@@ -313,6 +313,7 @@ def test_parity_in_the_bench_launch_configuration(lstmod, geom, mmap, o32, run_o
     evs = [synth.generate_event(geom, 1, s) for s in range(n_ev)]
     cfg = lstmod.default_config()
     cfg.n_slots = n_ev
+    cfg.launches_in_flight = n_streams                  # as bench.py sets it: grids sized for four launches side by side
     c = lstmod.Lst.from_synth(geom, mmap, cfg)
     d_in = [[torch.from_numpy(a).cuda() for a in (e.x, e.y, e.z, e.module, e.side)] for e in evs]
     streams = [torch.cuda.Stream() for _ in range(n_streams)]
@@ -788,4 +789,44 @@ def test_reduced_precision_store_parity(lstmod, geom, mmap, o32, run_oracle, con
             assert c.fetch_batch(1, lstmod.CLEAN, [idx], [val], stream=st, wait=True) == [len(kept)]
             assert np.array_equal(idx[:len(kept)], gpu[3][0][kept]) and np.array_equal(val[:len(kept)].view(np.uint16), gpu[3][1][kept].view(np.uint16))
     print(f"half store C{config}: {stt['needed']} objects, {n_off} atan2f outputs one binary16 ulp off")
+    c.close()
+
+
+def test_launches_in_flight_hint_changes_grids_only(lstmod, geom, mmap, o32, run_oracle):
+    """lst_config.launches_in_flight (include/lst.h): a sizing hint.  With it set to 4 -- single launches, batches of 3 and of
+    16, the optional stages, an event that needs the direct walks -- the results still equal the oracle's; negative values are
+    refused."""
+    import torch
+    cfg = lstmod.default_config()
+    cfg.launches_in_flight = -1
+    with pytest.raises(lstmod.LstError) as e:
+        lstmod.Lst.from_synth(geom, mmap, cfg)
+    assert e.value.status == lstmod.ERR_ARG
+    cfg.launches_in_flight, cfg.n_slots = 4, 20
+    c = lstmod.Lst.from_synth(geom, mmap, cfg)
+    evs = [synth.generate_event(geom, 1, 900 + i, n_particles=n) for i, n in enumerate((6000, 40, 0, 2500))] + [synth.generate_event(geom, 3, 4)]
+    evs += [synth.generate_event(geom, 1, 910 + i, n_particles=800 + 300 * i) for i in range(15)]
+    st = torch.cuda.Stream()
+    c.load_event(0, evs[0].x, evs[0].y, evs[0].z, evs[0].module, evs[0].side, st)     # one event on its own
+    c.run(0, st)
+    as_tuple = lambda ev: (ev.x, ev.y, ev.z, ev.module, ev.side)
+    c.load_events(1, [as_tuple(ev) for ev in evs[1:4]], stream=st)                      # a batch of 3
+    c.run_batch(1, 3, st)
+    c.load_events(4, [as_tuple(ev) for ev in evs[4:20]], stream=st)                     # a batch of 16
+    sd = synth.generate_seeds(evs[4], 4)
+    c.load_seeds(4, [sd.arrays()], st)
+    c.run_batch(4, 16, st)
+    c.run_stage(4, 16, lstmod.CLEAN, st)
+    c.run_stage(4, 1, lstmod.PIXEL, st)
+    assert c.sync_batch(0, 20, st) == 0
+    for k in (0, 1, 2, 3, 4, 9, 19):
+        ora = run_oracle(o32, evs[k], seeds=sd.arrays() if k == 4 else None)
+        parity.compare(parity.gpu_tables(c, k, st), parity.oracle_tables(ora), f"hint slot {k}")
+        stt = c.stats(k)
+        assert stt["needed"] == ora.counts and stt["candidates"] == ora.candidates
+        if k == 4:
+            keep = o32.t5_clean(ora.t5_hits(), ora.t5_chi2xy, ora.t5_chi2rz)
+            t5 = c.fetch_hit_indices(4, lstmod.T5, st)
+            assert set(map(tuple, t5[c.fetch_kept(4, st)].tolist())) == set(map(tuple, ora.t5_hits()[keep].tolist()))
+            assert stt["pix_needed"] == [ora.pix[0]["n"], ora.pix[1]["n"]]
     c.close()
