@@ -717,7 +717,7 @@ def csrc_digest() -> str:
     return h.hexdigest()[:16]
 
 
-NCU_SUMMARY = os.path.join("profiles", "r2_ncu_full_summary.csv")      # its .json sidecar holds the csrc digest of the capture
+NCU_SUMMARY = os.path.join("profiles", "r2_ncu_full_summary.csv")      # r2_ncu_full_summary.digest.txt beside it: "csrc_digest=..." and "commit=..." of the capture
 
 
 def ncu_traffic_bytes(kernel: str):
@@ -727,7 +727,7 @@ def ncu_traffic_bytes(kernel: str):
     import csv
     path = os.path.join(ROOT, NCU_SUMMARY)
     try:
-        meta = json.load(open(path[:-4] + ".json"))
+        meta = dict(l.strip().split("=", 1) for l in open(path[:-4] + ".digest.txt") if "=" in l)
         if meta.get("csrc_digest") != csrc_digest():
             return None, f"{NCU_SUMMARY} is stale: taken at csrc digest {meta.get('csrc_digest')}, this run is {csrc_digest()}"
         rows = list(csv.reader(open(path)))
